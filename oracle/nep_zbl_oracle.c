@@ -1,0 +1,766 @@
+/*
+ * nep_zbl_oracle.c -- plain fp64 CPU ORACLE for the NEP-ZBL hot path.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing in the product path (paper_2305_08140_b200/)
+ * may include, link, import or call this file; only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs do.  It shares no code,
+ * header, table or constant generator with the CUDA path.
+ *
+ * What it computes (citations: P:n = /root/reference/PAPER.md line n; S:x = SURVEY.md
+ * section 8(c) paragraph x, the reading of the NEP formulation the paper defers to
+ * ref. [25]; D:x = DESIGN.md reading x):
+ *
+ *   U_i = U_i^NEP({q^i_nu}) + 1/2 sum_{j != i} U_ZBL(r_ij)              Eq. 1
+ *   U_ZBL(r) = K Z_i Z_j / r * phi(r/a) * f_c(r)                        Eq. 2
+ *   phi(x) = sum_k c_k exp(-d_k x)                                      Eq. 3, parametrised
+ *   a = a_num / (Z_i^p + Z_j^p)                                         Eq. 4
+ *   f_c = Tersoff switch between r_inner and r_outer, S:D / D:C-7
+ *   descriptor: radial Chebyshev part and angular Legendre part, S:B, S:C
+ *   site energy: one hidden tanh layer, S:D
+ *   forces, virial: analytic derivatives of sum_i U_i, S:E
+ *   MD: velocity-Verlet, adaptive time step, S:F
+ *
+ * Every formula is written in its plain definitional form (Legendre double sums over
+ * neighbour pairs, Tr S^3 for the 4-body term, explicit periodic images) -- the forms
+ * the CUDA path does NOT use.  No blocking, fusion or reordering beyond that.
+ *
+ * Parity pins (tests/test_oracle_*.py): closed-form ZBL/Coulomb limits, T_k(cos t)=cos(kt),
+ * spherical-harmonic (scipy) and Wigner-3j (sympy) forms of the 3-/4-body terms,
+ * finite-difference forces and strain virial, invariances, brute-force neighbours,
+ * bcc shell counts, NVE drift ~ dt^2, time reversal.
+ * "parity unpinned": NEP numbers against the paper's trained W model (no weights, no
+ * printed values exist in the paper for this synthetic model).
+ *
+ * Layouts: positions pos[3n] = x[n] y[n] z[n]; force[3n] likewise; virial[9n] with
+ * component c = 3*alpha+beta at virial[c*n+i]; box[9] row vectors (orthogonal only).
+ * Units: eV, Angstrom, amu, fs.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_PI 3.14159265358979323846264338327950288
+#define ORC_AMU_A2_FS2_TO_EV 103.6426965  /* 1 amu*A^2/fs^2 in eV (SURVEY 8(b) units) */
+#define ORC_MAX_BASIS 32
+#define ORC_MAX_NMAX 32
+
+typedef struct {
+  int32_t n_types;
+  double rc_radial, rc_angular;
+  int32_t n_max_radial, n_max_angular; /* n = 0..n_max */
+  int32_t basis_radial, basis_angular; /* k = 0..basis  (D:C-2) */
+  int32_t l_max;                       /* 3-body l = 1..l_max */
+  int32_t has_4body;                   /* (2,2,2) term */
+  int32_t n_neurons;
+  const double *c_radial;  /* [n_types][n_types][n_max_R+1][basis_R+1] */
+  const double *c_angular; /* [n_types][n_types][n_max_A+1][basis_A+1] */
+  const double *q_scaler;  /* [D] */
+  const double *w0;        /* [n_neurons][D] */
+  const double *b0;        /* [n_neurons] */
+  const double *w1;        /* [n_neurons] */
+  double b1;
+  int32_t zbl_enabled;
+  double zbl_r_inner, zbl_r_outer;
+  int32_t zbl_n_terms;
+  double zbl_c[4], zbl_d[4];
+  double zbl_a_num, zbl_a_pow, coulomb_k;
+  const double *atomic_number; /* [n_types] */
+  const double *mass;          /* [n_types] */
+} orc_params;
+
+int orc_descriptor_dim(const orc_params *p) {
+  return (p->n_max_radial + 1) + (p->n_max_angular + 1) * p->l_max +
+         (p->has_4body ? (p->n_max_angular + 1) : 0);
+}
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* ------------------------------------------------------------------ ZBL, Eq. 2-4 */
+
+/* Tersoff switch (S:D): 1 for r<=r_in, 1/2+1/2 cos(pi (r-r_in)/(r_out-r_in)) between, 0 beyond */
+static void tersoff_switch(double r, double r_in, double r_out, double *f, double *df) {
+  if (r <= r_in) {
+    *f = 1.0;
+    *df = 0.0;
+  } else if (r < r_out) {
+    double w = ORC_PI / (r_out - r_in);
+    *f = 0.5 + 0.5 * cos(w * (r - r_in));
+    *df = -0.5 * w * sin(w * (r - r_in));
+  } else {
+    *f = 0.0;
+    *df = 0.0;
+  }
+}
+
+/* U_ZBL(r) and dU/dr for a pair of types (ti,tj).  Eq. 2, 3, 4. */
+void orc_zbl_pair(const orc_params *p, int ti, int tj, double r, double *u, double *dudr) {
+  double zi = p->atomic_number[ti], zj = p->atomic_number[tj];
+  double a = p->zbl_a_num / (pow(zi, p->zbl_a_pow) + pow(zj, p->zbl_a_pow)); /* Eq. 4 */
+  double x = r / a;
+  double phi = 0.0, dphi = 0.0; /* Eq. 3 and d(phi)/dr */
+  for (int k = 0; k < p->zbl_n_terms; ++k) {
+    double e = p->zbl_c[k] * exp(-p->zbl_d[k] * x);
+    phi += e;
+    dphi += -p->zbl_d[k] / a * e;
+  }
+  double fc, dfc;
+  tersoff_switch(r, p->zbl_r_inner, p->zbl_r_outer, &fc, &dfc);
+  double coul = p->coulomb_k * zi * zj / r; /* (1/4 pi eps0) Z_i Z_j e^2 / r */
+  double dcoul = -coul / r;
+  *u = coul * phi * fc; /* Eq. 2 */
+  *dudr = dcoul * phi * fc + coul * dphi * fc + coul * phi * dfc;
+}
+
+double orc_zbl_screening_length(const orc_params *p, int ti, int tj) {
+  return p->zbl_a_num /
+         (pow(p->atomic_number[ti], p->zbl_a_pow) + pow(p->atomic_number[tj], p->zbl_a_pow));
+}
+
+/* ------------------------------------------------------------------ radial functions, S:B */
+
+/* f_k(r) = 1/2 [T_k(x)+1] f_c(r),  x = 2 (r/rc - 1)^2 - 1,  f_c = 1/2 [1+cos(pi r/rc)],  k=0..basis.
+ * Also df_k/dr.  Zero for r >= rc. */
+void orc_radial_basis(double r, double rc, int basis, double *f, double *df) {
+  if (r >= rc) {
+    for (int k = 0; k <= basis; ++k) f[k] = df[k] = 0.0;
+    return;
+  }
+  double fc = 0.5 * (1.0 + cos(ORC_PI * r / rc));
+  double dfc = -0.5 * ORC_PI / rc * sin(ORC_PI * r / rc);
+  double u = r / rc - 1.0;
+  double x = 2.0 * u * u - 1.0;
+  double dx = 4.0 * u / rc;
+  double T[ORC_MAX_BASIS + 2], dT[ORC_MAX_BASIS + 2]; /* T_k(x), dT_k/dx */
+  T[0] = 1.0;
+  dT[0] = 0.0;
+  T[1] = x;
+  dT[1] = 1.0;
+  for (int k = 2; k <= basis; ++k) { /* T_k = 2 x T_{k-1} - T_{k-2} */
+    T[k] = 2.0 * x * T[k - 1] - T[k - 2];
+    dT[k] = 2.0 * T[k - 1] + 2.0 * x * dT[k - 1] - dT[k - 2];
+  }
+  for (int k = 0; k <= basis; ++k) {
+    f[k] = 0.5 * (T[k] + 1.0) * fc;
+    df[k] = 0.5 * dT[k] * dx * fc + 0.5 * (T[k] + 1.0) * dfc;
+  }
+}
+
+/* g_n(r) = sum_k c^{ti tj}_{nk} f_k(r), n = 0..n_max, and dg_n/dr.  which: 0 radial, 1 angular. */
+void orc_radial_functions(const orc_params *p, int which, int ti, int tj, double r, double *g,
+                          double *dg) {
+  double rc = which ? p->rc_angular : p->rc_radial;
+  int nmax = which ? p->n_max_angular : p->n_max_radial;
+  int basis = which ? p->basis_angular : p->basis_radial;
+  const double *c = which ? p->c_angular : p->c_radial;
+  double f[ORC_MAX_BASIS + 2], df[ORC_MAX_BASIS + 2];
+  orc_radial_basis(r, rc, basis, f, df);
+  const double *cp = c + ((size_t)(ti * p->n_types + tj)) * (nmax + 1) * (basis + 1);
+  for (int n = 0; n <= nmax; ++n) {
+    double s = 0.0, ds = 0.0;
+    for (int k = 0; k <= basis; ++k) {
+      s += cp[n * (basis + 1) + k] * f[k];
+      ds += cp[n * (basis + 1) + k] * df[k];
+    }
+    g[n] = s;
+    dg[n] = ds;
+  }
+}
+
+/* ------------------------------------------------------------------ Legendre polynomials */
+
+/* P_l(c) and dP_l/dc by the Bonnet recurrence (l+1) P_{l+1} = (2l+1) c P_l - l P_{l-1}. */
+static void legendre(int lmax, double c, double *P, double *dP) {
+  P[0] = 1.0;
+  dP[0] = 0.0;
+  if (lmax >= 1) {
+    P[1] = c;
+    dP[1] = 1.0;
+  }
+  for (int l = 1; l < lmax; ++l) {
+    P[l + 1] = ((2 * l + 1) * c * P[l] - l * P[l - 1]) / (l + 1);
+    dP[l + 1] = ((2 * l + 1) * (P[l] + c * dP[l]) - l * dP[l - 1]) / (l + 1);
+  }
+}
+
+/* ------------------------------------------------------------------ descriptor of one site, S:C */
+
+/* -45 / (8 sqrt(14) pi^{3/2}): the (2 2 2) Wigner-3j contraction of orthonormal Y_2m equals
+ * this constant times Tr(S^3) (S:C; pinned against sympy wigner_3j in tests/test_oracle_angular.py) */
+#define ORC_C4 (-45.0 / (8.0 * 3.7416573867739413856 * 5.5683279968317078453))
+
+/*
+ * q[D] and (optionally) dq[D][nn][3] = d q_nu / d r_ij for the site of type ti with nn neighbours
+ * (types tj[s], displacement vectors d[s][3] = r_j - r_i, all with |d| < rc_radial).
+ * Descriptor order (S:C): nu = n (radial); 3-body l-major nu = NR + (l-1)*NA + n; 4-body nu = NR + lmax*NA + n.
+ */
+void orc_descriptor_site(const orc_params *p, int ti, int nn, const int32_t *tj, const double *d,
+                         double *q, double *dq) {
+  int NR = p->n_max_radial + 1, NA = p->n_max_angular + 1, L = p->l_max;
+  int D = orc_descriptor_dim(p);
+  for (int v = 0; v < D; ++v) q[v] = 0.0;
+  if (dq) memset(dq, 0, sizeof(double) * (size_t)D * nn * 3);
+
+  double *r = (double *)malloc(sizeof(double) * nn);
+  double *rh = (double *)malloc(sizeof(double) * nn * 3);
+  double *gA = (double *)malloc(sizeof(double) * nn * NA);
+  double *dgA = (double *)malloc(sizeof(double) * nn * NA);
+  int *isA = (int *)malloc(sizeof(int) * nn);
+
+  for (int s = 0; s < nn; ++s) {
+    r[s] = sqrt(d[3 * s] * d[3 * s] + d[3 * s + 1] * d[3 * s + 1] + d[3 * s + 2] * d[3 * s + 2]);
+    for (int a = 0; a < 3; ++a) rh[3 * s + a] = d[3 * s + a] / r[s];
+  }
+
+  /* radial: q_n = sum_j g^R_n(r_ij)   (S:C first bullet) */
+  for (int s = 0; s < nn; ++s) {
+    if (!(r[s] < p->rc_radial)) continue;
+    double g[ORC_MAX_NMAX + 1], dg[ORC_MAX_NMAX + 1];
+    orc_radial_functions(p, 0, ti, tj[s], r[s], g, dg);
+    for (int n = 0; n < NR; ++n) {
+      q[n] += g[n];
+      if (dq)
+        for (int a = 0; a < 3; ++a) dq[((size_t)n * nn + s) * 3 + a] = dg[n] * rh[3 * s + a];
+    }
+  }
+
+  /* angular radial functions for neighbours inside rc_angular */
+  for (int s = 0; s < nn; ++s) {
+    isA[s] = (r[s] < p->rc_angular);
+    if (isA[s])
+      orc_radial_functions(p, 1, ti, tj[s], r[s], gA + (size_t)s * NA, dgA + (size_t)s * NA);
+  }
+
+  /* 3-body: q_nl = (2l+1)/(4 pi) sum_j sum_k g_n(r_ij) g_n(r_ik) P_l(rh_ij . rh_ik), j=k included (S:C) */
+  for (int j = 0; j < nn; ++j) {
+    if (!isA[j]) continue;
+    for (int k = 0; k < nn; ++k) {
+      if (!isA[k]) continue;
+      double c = rh[3 * j] * rh[3 * k] + rh[3 * j + 1] * rh[3 * k + 1] + rh[3 * j + 2] * rh[3 * k + 2];
+      if (j == k) c = 1.0;
+      double P[16], dP[16];
+      legendre(L, c, P, dP);
+      for (int l = 1; l <= L; ++l) {
+        double pref = (2 * l + 1) / (4.0 * ORC_PI);
+        for (int n = 0; n < NA; ++n) {
+          int v = NR + (l - 1) * NA + n;
+          double gj = gA[(size_t)j * NA + n], gk = gA[(size_t)k * NA + n];
+          q[v] += pref * gj * gk * P[l];
+          if (dq) {
+            /* d/dr_ij, S:E: 2 (2l+1)/(4pi) sum_k [ g'(r_ij) rh_ij g(r_ik) P_l(c)
+             *                       + g(r_ij) g(r_ik) P_l'(c) (rh_ik - c rh_ij)/r_ij ]          */
+            double dgj = dgA[(size_t)j * NA + n];
+            for (int a = 0; a < 3; ++a) {
+              double t = dgj * rh[3 * j + a] * gk * P[l] +
+                         gj * gk * dP[l] * (rh[3 * k + a] - c * rh[3 * j + a]) / r[j];
+              dq[((size_t)v * nn + j) * 3 + a] += 2.0 * pref * t;
+            }
+          }
+        }
+      }
+    }
+  }
+
+  /* 4-body: q_n = C4 Tr(S_n^3), S_n = sum_j g_n(r_ij) (rh rh^T - I/3)  (S:C third bullet) */
+  if (p->has_4body) {
+    for (int n = 0; n < NA; ++n) {
+      double S[3][3] = {{0}};
+      for (int j = 0; j < nn; ++j) {
+        if (!isA[j]) continue;
+        double g = gA[(size_t)j * NA + n];
+        for (int a = 0; a < 3; ++a)
+          for (int b = 0; b < 3; ++b)
+            S[a][b] += g * (rh[3 * j + a] * rh[3 * j + b] - (a == b ? 1.0 / 3.0 : 0.0));
+      }
+      double S2[3][3], tr3 = 0.0, tr2 = 0.0;
+      for (int a = 0; a < 3; ++a)
+        for (int b = 0; b < 3; ++b) {
+          S2[a][b] = 0.0;
+          for (int c = 0; c < 3; ++c) S2[a][b] += S[a][c] * S[c][b];
+        }
+      for (int a = 0; a < 3; ++a) {
+        tr2 += S2[a][a];
+        for (int b = 0; b < 3; ++b) tr3 += S2[a][b] * S[b][a];
+      }
+      int v = NR + L * NA + n;
+      q[v] = ORC_C4 * tr3;
+      if (dq) {
+        /* d Tr(S^3)/d r_ij^a = 3 Tr(S^2 dS/dr^a);
+         * dS/dr^a = g' rh^a (rh rh^T - I/3) + g (e_a rh^T + rh e_a^T - 2 rh^a rh rh^T)/r          */
+        for (int j = 0; j < nn; ++j) {
+          if (!isA[j]) continue;
+          double g = gA[(size_t)j * NA + n], dg = dgA[(size_t)j * NA + n];
+          const double *h = rh + 3 * j;
+          double S2h[3], hS2h = 0.0;
+          for (int a = 0; a < 3; ++a) {
+            S2h[a] = S2[a][0] * h[0] + S2[a][1] * h[1] + S2[a][2] * h[2];
+          }
+          for (int a = 0; a < 3; ++a) hS2h += h[a] * S2h[a];
+          for (int a = 0; a < 3; ++a) {
+            double t = dg * h[a] * (hS2h - tr2 / 3.0) + g * (2.0 / r[j]) * (S2h[a] - h[a] * hS2h);
+            dq[((size_t)v * nn + j) * 3 + a] = 3.0 * ORC_C4 * t;
+          }
+        }
+      }
+    }
+  }
+  free(r);
+  free(rh);
+  free(gA);
+  free(dgA);
+  free(isA);
+}
+
+/* ------------------------------------------------------------------ network, S:D */
+
+/* U^NEP = sum_mu w1_mu tanh( sum_nu w0_{mu nu} s_nu q_nu - b0_mu ) - b1 ;  Fp_nu = dU/dq_nu */
+void orc_site_energy(const orc_params *p, const double *q, double *U, double *Fp) {
+  int D = orc_descriptor_dim(p);
+  double u = -p->b1;
+  for (int v = 0; v < D; ++v) Fp[v] = 0.0;
+  for (int m = 0; m < p->n_neurons; ++m) {
+    double z = -p->b0[m];
+    for (int v = 0; v < D; ++v) z += p->w0[(size_t)m * D + v] * p->q_scaler[v] * q[v];
+    double h = tanh(z);
+    u += p->w1[m] * h;
+    for (int v = 0; v < D; ++v)
+      Fp[v] += p->w1[m] * (1.0 - h * h) * p->w0[(size_t)m * D + v] * p->q_scaler[v];
+  }
+  *U = u;
+}
+
+/* ------------------------------------------------------------------ neighbours, S:A */
+
+typedef struct {
+  int n;
+  double L[3];
+  int pbc[3];
+  double *xw; /* wrapped copy [3n] SoA */
+  /* cell list (own; only used when use_cell) */
+  int use_cell;
+  int nc[3];
+  double lo[3], cw[3];
+  int *cell_start, *cell_atoms;
+} orc_system;
+
+static int orc_system_init(orc_system *S, int n, const double *pos, const double *box,
+                           const int32_t *pbc, double rc, int use_cell) {
+  /* orthogonal boxes only */
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      if (a != b && box[3 * a + b] != 0.0) return -2;
+  S->n = n;
+  for (int a = 0; a < 3; ++a) {
+    S->L[a] = box[4 * a];
+    S->pbc[a] = pbc[a];
+  }
+  S->xw = (double *)malloc(sizeof(double) * 3 * (size_t)(n > 0 ? n : 1));
+  for (int a = 0; a < 3; ++a)
+    for (int i = 0; i < n; ++i) {
+      double x = pos[(size_t)a * n + i];
+      if (S->pbc[a]) x -= S->L[a] * floor(x / S->L[a]); /* wrap periodic axes */
+      S->xw[(size_t)a * n + i] = x;
+    }
+  S->use_cell = 0;
+  S->cell_start = S->cell_atoms = NULL;
+  if (use_cell && n > 0) {
+    int ok = 1;
+    for (int a = 0; a < 3; ++a) {
+      if (S->pbc[a]) {
+        S->lo[a] = 0.0;
+        S->nc[a] = (int)floor(S->L[a] / rc);
+        if (S->nc[a] < 3) ok = 0; /* too small for a cell walk without duplicate images */
+        S->cw[a] = S->L[a] / (S->nc[a] > 0 ? S->nc[a] : 1);
+      } else { /* open axis: cells span the atoms' bounding range (D:C-14) */
+        double mn = S->xw[(size_t)a * n], mx = mn;
+        for (int i = 1; i < n; ++i) {
+          double x = S->xw[(size_t)a * n + i];
+          if (x < mn) mn = x;
+          if (x > mx) mx = x;
+        }
+        S->lo[a] = mn;
+        S->nc[a] = (int)floor((mx - mn) / rc) + 1;
+        S->cw[a] = rc;
+      }
+    }
+    if (ok) {
+      S->use_cell = 1;
+      size_t ncell = (size_t)S->nc[0] * S->nc[1] * S->nc[2];
+      S->cell_start = (int *)calloc(ncell + 1, sizeof(int));
+      S->cell_atoms = (int *)malloc(sizeof(int) * n);
+      int *cid = (int *)malloc(sizeof(int) * n);
+      for (int i = 0; i < n; ++i) {
+        int c[3];
+        for (int a = 0; a < 3; ++a) {
+          c[a] = (int)floor((S->xw[(size_t)a * n + i] - S->lo[a]) / S->cw[a]);
+          if (c[a] < 0) c[a] = 0;
+          if (c[a] >= S->nc[a]) c[a] = S->nc[a] - 1;
+        }
+        cid[i] = (c[2] * S->nc[1] + c[1]) * S->nc[0] + c[0];
+        S->cell_start[cid[i] + 1]++;
+      }
+      for (size_t c = 0; c < ncell; ++c) S->cell_start[c + 1] += S->cell_start[c];
+      int *fill = (int *)calloc(ncell, sizeof(int));
+      for (int i = 0; i < n; ++i) { /* ascending i inside each cell */
+        S->cell_atoms[S->cell_start[cid[i]] + fill[cid[i]]++] = i;
+      }
+      free(fill);
+      free(cid);
+    }
+  }
+  return 0;
+}
+
+static void orc_system_free(orc_system *S) {
+  free(S->xw);
+  free(S->cell_start);
+  free(S->cell_atoms);
+}
+
+typedef struct {
+  int j;
+  int s[3];
+  double d[3];
+} orc_nbr;
+
+static int nbr_cmp(const void *a, const void *b) {
+  const orc_nbr *x = (const orc_nbr *)a, *y = (const orc_nbr *)b;
+  if (x->j != y->j) return x->j < y->j ? -1 : 1;
+  for (int k = 0; k < 3; ++k)
+    if (x->s[k] != y->s[k]) return x->s[k] < y->s[k] ? -1 : 1;
+  return 0;
+}
+
+/*
+ * All (j, image shift) with |x_j + s*L - x_i| < rc, strict (S:A, D:C-10); j = i only with s != 0.
+ * Returns the count (may exceed cap: then only cap are stored).  Canonical order: (j, shift).
+ */
+static int orc_site_neighbors(const orc_system *S, int i, double rc, orc_nbr *out, int cap) {
+  int n = S->n, cnt = 0;
+  double rc2 = rc * rc;
+  double xi[3] = {S->xw[i], S->xw[(size_t)n + i], S->xw[2 * (size_t)n + i]};
+  if (!S->use_cell) {
+    /* brute force: every atom, every image shift s in {-m..m}^3, m = ceil(rc/L) on periodic axes */
+    int m[3];
+    for (int a = 0; a < 3; ++a) m[a] = S->pbc[a] ? (int)ceil(rc / S->L[a]) : 0;
+    for (int j = 0; j < n; ++j) {
+      double dj[3] = {S->xw[j] - xi[0], S->xw[(size_t)n + j] - xi[1], S->xw[2 * (size_t)n + j] - xi[2]};
+      for (int sx = -m[0]; sx <= m[0]; ++sx)
+        for (int sy = -m[1]; sy <= m[1]; ++sy)
+          for (int sz = -m[2]; sz <= m[2]; ++sz) {
+            if (j == i && sx == 0 && sy == 0 && sz == 0) continue;
+            double dx = dj[0] + sx * S->L[0], dy = dj[1] + sy * S->L[1], dz = dj[2] + sz * S->L[2];
+            double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 < rc2) {
+              if (cnt < cap) {
+                out[cnt].j = j;
+                out[cnt].s[0] = sx; out[cnt].s[1] = sy; out[cnt].s[2] = sz;
+                out[cnt].d[0] = dx; out[cnt].d[1] = dy; out[cnt].d[2] = dz;
+              }
+              ++cnt;
+            }
+          }
+    }
+  } else {
+    int c[3];
+    for (int a = 0; a < 3; ++a) {
+      c[a] = (int)floor((xi[a] - S->lo[a]) / S->cw[a]);
+      if (c[a] < 0) c[a] = 0;
+      if (c[a] >= S->nc[a]) c[a] = S->nc[a] - 1;
+    }
+    for (int oz = -1; oz <= 1; ++oz)
+      for (int oy = -1; oy <= 1; ++oy)
+        for (int ox = -1; ox <= 1; ++ox) {
+          int o[3] = {ox, oy, oz}, cc[3], sh[3];
+          int skip = 0;
+          for (int a = 0; a < 3; ++a) {
+            cc[a] = c[a] + o[a];
+            sh[a] = 0;
+            if (cc[a] < 0) {
+              if (!S->pbc[a]) { skip = 1; break; }
+              cc[a] += S->nc[a];
+              sh[a] = -1;
+            } else if (cc[a] >= S->nc[a]) {
+              if (!S->pbc[a]) { skip = 1; break; }
+              cc[a] -= S->nc[a];
+              sh[a] = 1;
+            }
+          }
+          if (skip) continue;
+          int cid = (cc[2] * S->nc[1] + cc[1]) * S->nc[0] + cc[0];
+          for (int t = S->cell_start[cid]; t < S->cell_start[cid + 1]; ++t) {
+            int j = S->cell_atoms[t];
+            if (j == i && sh[0] == 0 && sh[1] == 0 && sh[2] == 0) continue;
+            double dx = (S->xw[j] - xi[0]) + sh[0] * S->L[0];
+            double dy = (S->xw[(size_t)n + j] - xi[1]) + sh[1] * S->L[1];
+            double dz = (S->xw[2 * (size_t)n + j] - xi[2]) + sh[2] * S->L[2];
+            double r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 < rc2) {
+              if (cnt < cap) {
+                out[cnt].j = j;
+                out[cnt].s[0] = sh[0]; out[cnt].s[1] = sh[1]; out[cnt].s[2] = sh[2];
+                out[cnt].d[0] = dx; out[cnt].d[1] = dy; out[cnt].d[2] = dz;
+              }
+              ++cnt;
+            }
+          }
+        }
+  }
+  qsort(out, cnt < cap ? cnt : cap, sizeof(orc_nbr), nbr_cmp);
+  return cnt;
+}
+
+/*
+ * Neighbour lists of every atom for cutoff rc.  nn[n]; nl[n*cap] (j), nd[n*cap*3] (optional,
+ * displacement vectors).  Returns max count; if it exceeds cap lists are truncated (caller checks).
+ * Returns -2 for a non-orthogonal box.
+ */
+int orc_neighbors(int n, const double *pos, const double *box, const int32_t *pbc, double rc,
+                  int use_cell, int cap, int32_t *nn, int32_t *nl, double *nd) {
+  orc_system S;
+  int rcode = orc_system_init(&S, n, pos, box, pbc, rc, use_cell);
+  if (rcode) return rcode;
+  int maxc = 0;
+#pragma omp parallel
+  {
+    orc_nbr *buf = (orc_nbr *)malloc(sizeof(orc_nbr) * cap);
+#pragma omp for schedule(dynamic, 64) reduction(max : maxc)
+    for (int i = 0; i < n; ++i) {
+      int c = orc_site_neighbors(&S, i, rc, buf, cap);
+      nn[i] = c;
+      if (c > maxc) maxc = c;
+      int m = c < cap ? c : cap;
+      for (int s = 0; s < m; ++s) {
+        nl[(size_t)i * cap + s] = buf[s].j;
+        if (nd)
+          for (int a = 0; a < 3; ++a) nd[((size_t)i * cap + s) * 3 + a] = buf[s].d[a];
+      }
+    }
+    free(buf);
+  }
+  orc_system_free(&S);
+  return maxc;
+}
+
+/* ------------------------------------------------------------------ energy / force / virial, S:D, S:E */
+
+#define ORC_NBR_CAP 512
+
+/*
+ * Full evaluation.  Outputs (any may be NULL): energy[n], force[3n], virial[9n], q_out[n*D].
+ * nsel < 0: all atoms.  nsel >= 0: outputs are complete only for the atoms in sel[]; the site
+ * derivatives of sel and of all their neighbours are evaluated (what F_i and W_i need, S:E).
+ * Returns 0, or <0 on error (-2 non-orthogonal box, -3 neighbour capacity).
+ */
+int orc_compute(const orc_params *p, int n, const double *pos, const int32_t *types,
+                const double *box, const int32_t *pbc, int use_cell, double *energy, double *force,
+                double *virial, double *q_out, int nsel, const int32_t *sel) {
+  orc_system S;
+  int rcode = orc_system_init(&S, n, pos, box, pbc, p->rc_radial, use_cell);
+  if (rcode) return rcode;
+  int D = orc_descriptor_dim(p);
+  if (energy) memset(energy, 0, sizeof(double) * n);
+  if (force) memset(force, 0, sizeof(double) * 3 * (size_t)n);
+  if (virial) memset(virial, 0, sizeof(double) * 9 * (size_t)n);
+  int need_deriv = (force || virial);
+
+  /* which sites must be evaluated */
+  char *center = (char *)malloc(n > 0 ? n : 1);
+  char *wanted = (char *)malloc(n > 0 ? n : 1);
+  if (nsel < 0) {
+    memset(center, 1, n);
+    memset(wanted, 1, n);
+  } else {
+    memset(center, 0, n);
+    memset(wanted, 0, n);
+    orc_nbr *buf = (orc_nbr *)malloc(sizeof(orc_nbr) * ORC_NBR_CAP);
+    for (int t = 0; t < nsel; ++t) {
+      int i = sel[t];
+      wanted[i] = 1;
+      center[i] = 1;
+      if (need_deriv) {
+        int c = orc_site_neighbors(&S, i, p->rc_radial, buf, ORC_NBR_CAP);
+        if (c > ORC_NBR_CAP) c = ORC_NBR_CAP;
+        for (int s = 0; s < c; ++s) center[buf[s].j] = 1;
+      }
+    }
+    free(buf);
+  }
+  int ncen = 0;
+  int *cen = (int *)malloc(sizeof(int) * (n > 0 ? n : 1));
+  for (int i = 0; i < n; ++i)
+    if (center[i]) cen[ncen++] = i;
+
+  int err = 0;
+  const int CH = 2048; /* sites per chunk: parallel evaluation, then serial ordered accumulation */
+  orc_nbr *nb = (orc_nbr *)malloc(sizeof(orc_nbr) * (size_t)CH * ORC_NBR_CAP);
+  int *cnt = (int *)malloc(sizeof(int) * CH);
+  double *part = (double *)malloc(sizeof(double) * (size_t)CH * ORC_NBR_CAP * 3); /* dU_i/dr_ij */
+  double *Usite = (double *)malloc(sizeof(double) * CH);
+
+  for (int c0 = 0; c0 < ncen && !err; c0 += CH) {
+    int c1 = c0 + CH < ncen ? c0 + CH : ncen;
+#pragma omp parallel
+    {
+      double *q = (double *)malloc(sizeof(double) * D);
+      double *Fp = (double *)malloc(sizeof(double) * D);
+      double *dq = (double *)malloc(sizeof(double) * (size_t)D * ORC_NBR_CAP * 3);
+      double *dv = (double *)malloc(sizeof(double) * ORC_NBR_CAP * 3);
+      int32_t *tj = (int32_t *)malloc(sizeof(int32_t) * ORC_NBR_CAP);
+#pragma omp for schedule(dynamic, 16)
+      for (int t = c0; t < c1; ++t) {
+        int i = cen[t], u = t - c0;
+        orc_nbr *mine = nb + (size_t)u * ORC_NBR_CAP;
+        int c = orc_site_neighbors(&S, i, p->rc_radial, mine, ORC_NBR_CAP);
+        if (c > ORC_NBR_CAP) {
+#pragma omp atomic write
+          err = -3;
+          c = ORC_NBR_CAP;
+        }
+        cnt[u] = c;
+        for (int s = 0; s < c; ++s) {
+          tj[s] = types[mine[s].j];
+          for (int a = 0; a < 3; ++a) dv[3 * s + a] = mine[s].d[a];
+        }
+        orc_descriptor_site(p, types[i], c, tj, dv, q, need_deriv ? dq : NULL);
+        double U;
+        orc_site_energy(p, q, &U, Fp);
+        if (q_out)
+          for (int v = 0; v < D; ++v) q_out[(size_t)i * D + v] = q[v];
+        double *pp = part + (size_t)u * ORC_NBR_CAP * 3;
+        for (int s = 0; s < c; ++s) {
+          double px = 0, py = 0, pz = 0;
+          if (need_deriv)
+            for (int v = 0; v < D; ++v) { /* chain rule dU_i/dr_ij = sum_nu Fp_nu dq_nu/dr_ij */
+              px += Fp[v] * dq[((size_t)v * c + s) * 3 + 0];
+              py += Fp[v] * dq[((size_t)v * c + s) * 3 + 1];
+              pz += Fp[v] * dq[((size_t)v * c + s) * 3 + 2];
+            }
+          /* ZBL: half of every pair term belongs to site i (Eq. 1) */
+          if (p->zbl_enabled) {
+            double r = sqrt(dv[3 * s] * dv[3 * s] + dv[3 * s + 1] * dv[3 * s + 1] +
+                            dv[3 * s + 2] * dv[3 * s + 2]);
+            if (r < p->zbl_r_outer) {
+              double uz, duz;
+              orc_zbl_pair(p, types[i], tj[s], r, &uz, &duz);
+              U += 0.5 * uz;
+              px += 0.5 * duz * dv[3 * s] / r;
+              py += 0.5 * duz * dv[3 * s + 1] / r;
+              pz += 0.5 * duz * dv[3 * s + 2] / r;
+            }
+          }
+          pp[3 * s] = px;
+          pp[3 * s + 1] = py;
+          pp[3 * s + 2] = pz;
+        }
+        Usite[u] = U;
+      }
+      free(q);
+      free(Fp);
+      free(dq);
+      free(dv);
+      free(tj);
+    }
+    /* ordered accumulation (S:E): F_i += dU_i/dr_ij ; F_j -= dU_i/dr_ij ; W_j -= r_ij (x) dU_i/dr_ij,
+     * i.e. F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji),  W_i = sum_j r_ij (x) dU_j/dr_ji  (r_ji = -r_ij). */
+    for (int t = c0; t < c1; ++t) {
+      int i = cen[t], u = t - c0;
+      if (energy) energy[i] = Usite[u];
+      if (!need_deriv) continue;
+      const orc_nbr *mine = nb + (size_t)u * ORC_NBR_CAP;
+      const double *pp = part + (size_t)u * ORC_NBR_CAP * 3;
+      for (int s = 0; s < cnt[u]; ++s) {
+        int j = mine[s].j;
+        for (int a = 0; a < 3; ++a) {
+          if (force) {
+            force[(size_t)a * n + i] += pp[3 * s + a];
+            force[(size_t)a * n + j] -= pp[3 * s + a];
+          }
+          if (virial)
+            for (int b = 0; b < 3; ++b)
+              virial[(size_t)(3 * a + b) * n + j] -= mine[s].d[a] * pp[3 * s + b];
+        }
+      }
+    }
+  }
+  /* atoms that were evaluated only as helpers carry incomplete sums: blank them */
+  if (nsel >= 0) {
+    for (int i = 0; i < n; ++i) {
+      if (wanted[i]) continue;
+      if (energy) energy[i] = NAN;
+      if (force)
+        for (int a = 0; a < 3; ++a) force[(size_t)a * n + i] = NAN;
+      if (virial)
+        for (int a = 0; a < 9; ++a) virial[(size_t)a * n + i] = NAN;
+    }
+  }
+  free(nb);
+  free(cnt);
+  free(part);
+  free(Usite);
+  free(cen);
+  free(center);
+  free(wanted);
+  orc_system_free(&S);
+  return err;
+}
+
+/* ------------------------------------------------------------------ MD, S:F */
+
+/*
+ * nsteps velocity-Verlet steps in place on pos[3n], vel[3n].  Per step (S:F, D:C-11, D:C-12):
+ *   v_max = max_i |v_i(t)|;  dt = min(dt_max, max_disp / v_max)  (dt_max if v_max = 0)
+ *   v += dt/2 F/m;  x += dt v;  wrap periodic axes;  F = F(x);  v += dt/2 F/m.
+ * Neighbours are found afresh every step (plain definition; no skin).
+ * Traces (length nsteps+1 for energies: index 0 is the initial state; dt_trace[nsteps]).
+ */
+int orc_md_run(const orc_params *p, int n, double *pos, double *vel, const int32_t *types,
+               const double *box, const int32_t *pbc, int nsteps, double dt_max, double max_disp,
+               int use_cell, double *dt_trace, double *epot_trace, double *ekin_trace) {
+  double *F = (double *)malloc(sizeof(double) * 3 * (size_t)n);
+  double *E = (double *)malloc(sizeof(double) * n);
+  int rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
+  for (int step = 0; step <= nsteps && !rc; ++step) {
+    double ep = 0.0, ek = 0.0, vmax2 = 0.0;
+    for (int i = 0; i < n; ++i) {
+      double v2 = vel[i] * vel[i] + vel[(size_t)n + i] * vel[(size_t)n + i] +
+                  vel[2 * (size_t)n + i] * vel[2 * (size_t)n + i];
+      ep += E[i];
+      ek += 0.5 * p->mass[types[i]] * v2 * ORC_AMU_A2_FS2_TO_EV;
+      if (v2 > vmax2) vmax2 = v2;
+    }
+    if (epot_trace) epot_trace[step] = ep;
+    if (ekin_trace) ekin_trace[step] = ek;
+    if (step == nsteps) break;
+    double vmax = sqrt(vmax2);
+    double dt = dt_max;
+    if (vmax > 0.0 && max_disp / vmax < dt) dt = max_disp / vmax;
+    if (dt_trace) dt_trace[step] = dt;
+    for (int a = 0; a < 3; ++a)
+      for (int i = 0; i < n; ++i) {
+        double acc = F[(size_t)a * n + i] / (p->mass[types[i]] * ORC_AMU_A2_FS2_TO_EV);
+        vel[(size_t)a * n + i] += 0.5 * dt * acc;
+        double x = pos[(size_t)a * n + i] + dt * vel[(size_t)a * n + i];
+        if (pbc[a]) x -= box[4 * a] * floor(x / box[4 * a]);
+        pos[(size_t)a * n + i] = x;
+      }
+    rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
+    for (int a = 0; a < 3; ++a)
+      for (int i = 0; i < n; ++i) {
+        double acc = F[(size_t)a * n + i] / (p->mass[types[i]] * ORC_AMU_A2_FS2_TO_EV);
+        vel[(size_t)a * n + i] += 0.5 * dt * acc;
+      }
+  }
+  free(F);
+  free(E);
+  return rc;
+}
