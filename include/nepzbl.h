@@ -1,0 +1,168 @@
+/*
+ * nepzbl.h -- C ABI of the B200-native NEP-ZBL hot path (arXiv 2305.08140).
+ *
+ * One library, libnepzbl.so, built from paper_2305_08140_b200/csrc for sm_100a.  Every step of the
+ * path -- state prep, cell-list neighbour build, radial/angular descriptors, network, force/virial
+ * back-pass, ZBL pair term, velocity-Verlet with adaptive time step -- runs in its CUDA kernels.
+ * There is no CPU fallback: without a CUDA device nep_zbl_create fails with NEPZBL_E_CUDA.
+ *
+ * Citations: P:n = PAPER.md line n; S:x = SURVEY.md section 8(c) paragraph x; D:x = DESIGN.md.
+ *
+ * Conventions
+ *   - Units: eV, Angstrom, amu, fs.  1 amu*A^2/fs^2 = 103.6426965 eV.
+ *   - "dev" pointers are device memory owned by the caller (e.g. torch tensors); "host" pointers
+ *     are host memory owned by the caller.  The library never frees caller memory and the caller
+ *     never frees library memory (the handle is released by nep_zbl_destroy only).
+ *   - Positions / velocities are fp64 SoA: x[n] y[n] z[n] (3n doubles).  Forces are fp32 SoA [3n],
+ *     virials fp32 SoA [9n] with component c = 3*alpha+beta at virial[c*n + i], energies fp64 [n].
+ *     All per-atom results are in the CALLER's atom order (the library sorts internally).
+ *   - box[9]: row vectors, host.  Only orthogonal boxes (off-diagonals == 0).  pbc[3]: 1 periodic,
+ *     0 open (bulk periodic xyz; foil open in z).  A periodic edge must be >= 2*(rc_radial+skin).
+ *   - All work is enqueued on the CUDA stream given at create.  Calls that return host scalars or
+ *     status from the device (neighbor_build, nep_zbl_compute, md_step, md_run, md_energies,
+ *     *_host) synchronise that stream before returning.
+ *   - Every int-returning call returns NEPZBL_OK (0) or a negative NEPZBL_E_* code;
+ *     nep_zbl_last_error gives a message.  Nothing is truncated silently: a neighbour list that
+ *     does not fit cap_radial / cap_angular is an error that names the count needed.
+ *   - Determinism: the same inputs give bit-identical outputs (no floating-point atomics; the only
+ *     atomics are integer counters/max whose result does not depend on order).
+ */
+#ifndef NEPZBL_H
+#define NEPZBL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nepzbl_handle nepzbl_handle; /* opaque, owned by the library */
+
+enum {
+  NEPZBL_OK = 0,
+  NEPZBL_E_INVALID_ARG = -1,
+  NEPZBL_E_BOX_NOT_ORTHOGONAL = -2,
+  NEPZBL_E_BOX_TOO_SMALL = -3,     /* periodic edge < 2*(rc_radial+skin): minimum image invalid */
+  NEPZBL_E_NEIGHBOR_OVERFLOW = -4, /* an atom has more neighbours than cap_radial / cap_angular */
+  NEPZBL_E_NONFINITE = -5,         /* NaN/Inf in positions */
+  NEPZBL_E_CUDA = -6,
+  NEPZBL_E_UNSUPPORTED = -7,       /* model shape outside what this build instantiates */
+  NEPZBL_E_WORKSPACE = -8,         /* workspace missing or too small */
+  NEPZBL_E_STATE = -9              /* call order (e.g. md_step before md_init) */
+};
+
+/*
+ * Model and list parameters.  Host memory; copied at create; the caller keeps ownership.
+ * NEP-ZBL site energy (Eq. 1): U_i = U_i^NEP({q}) + 1/2 sum_j U_ZBL(r_ij).
+ * Hyper-parameters as listed in P:106; functional forms per S:B-S:D (the paper defers them to its
+ * ref. [25]).  Descriptor order (S:C): radial n = 0..n_max_radial; 3-body l-major
+ * (l = 1..l_max, n = 0..n_max_angular); then the (2,2,2) 4-body term n = 0..n_max_angular.
+ */
+typedef struct {
+  int32_t n_types;                     /* >= 1 (this build: 1) */
+  double rc_radial, rc_angular;        /* cutoffs r_c^R, r_c^A (6.0, 4.0 A) */
+  int32_t n_max_radial, n_max_angular; /* n = 0..n_max */
+  int32_t basis_radial, basis_angular; /* Chebyshev basis k = 0..basis (D: C-2) */
+  int32_t l_max;                       /* Legendre order of the 3-body part (4) */
+  int32_t has_4body;                   /* 1: (l1,l2,l3) = (2,2,2) term */
+  int32_t n_neurons;                   /* hidden tanh neurons */
+  const double *c_radial;              /* [n_types][n_types][n_max_radial+1][basis_radial+1] */
+  const double *c_angular;             /* [n_types][n_types][n_max_angular+1][basis_angular+1] */
+  const double *q_scaler;              /* [D] (D: C-6) */
+  const double *w0;                    /* [n_neurons][D] */
+  const double *b0;                    /* [n_neurons] */
+  const double *w1;                    /* [n_neurons] */
+  double b1;
+  int32_t zbl_enabled;                 /* Eq. 2 */
+  double zbl_r_inner, zbl_r_outer;     /* Tersoff switch (1.0, 2.0 A) */
+  int32_t zbl_n_terms;                 /* <= 4 */
+  double zbl_c[4], zbl_d[4];           /* phi(x) = sum_k c_k exp(-d_k x)  (Eq. 3) */
+  double zbl_a_num, zbl_a_pow;         /* a = a_num / (Z_i^pow + Z_j^pow)  (Eq. 4) */
+  double coulomb_k;                    /* e^2/(4 pi eps0) in eV*A */
+  const double *atomic_number;         /* [n_types] */
+  const double *mass;                  /* [n_types], amu */
+  double skin;                         /* neighbour-list skin, A (D: C-15) */
+  int32_t cap_radial, cap_angular;     /* list capacities per atom (cap_angular <= 64) */
+} nepzbl_params;
+
+/* Create a handle on CUDA device `device`; all work goes to `cuda_stream` (a cudaStream_t, may be
+ * NULL for the default stream).  Uploads the parameters (S1 of the path needs none).  */
+int nep_zbl_create(const nepzbl_params *params, int device, void *cuda_stream, nepzbl_handle **out);
+void nep_zbl_destroy(nepzbl_handle *h);
+const char *nep_zbl_last_error(const nepzbl_handle *h); /* h may be NULL: create-time errors */
+int nep_zbl_descriptor_dim(const nepzbl_handle *h);
+
+/* Device workspace for up to n_atoms atoms.  The caller allocates it (e.g. a torch uint8 tensor),
+ * hands it over with set_workspace and keeps it alive until destroy or the next set_workspace. */
+size_t nep_zbl_workspace_bytes(const nepzbl_handle *h, int64_t n_atoms);
+int nep_zbl_set_workspace(nepzbl_handle *h, void *dev_ptr, size_t bytes, int64_t n_atoms);
+
+/*
+ * S2: cell-list neighbour build (BASELINE.json north_star; cutoffs P:106).  Sorts the atoms by
+ * cell (canonical order), then lists for every atom all j with r_ij < rc_radial+skin (radial list)
+ * and the subset r_ij < rc_angular+skin (angular list), minimum image on periodic axes, strict <.
+ * pos_soa, types: dev.  box, pbc: host.
+ */
+int neighbor_build(nepzbl_handle *h, int64_t n, const double *pos_soa, const int32_t *types,
+                   const double box[9], const int32_t pbc[3]);
+/* Copy the current lists out, in the caller's atom indices: nn dev [n]; nl dev [n][cap] row-major
+ * (entries beyond nn[i] are -1).  which: 0 radial, 1 angular.  Order inside a row is the
+ * library's deterministic cell-walk order. */
+int neighbor_get(nepzbl_handle *h, int which, int32_t *nn, int32_t *nl);
+
+/*
+ * S1,S3-S7: one NEP-ZBL evaluation (Eq. 1-4; S:B-S:E): per-atom energy, force, virial.
+ * Reuses the current neighbour list when it is still valid for these positions (same n, box, pbc
+ * and no atom moved more than skin/2 since the build), otherwise rebuilds it.
+ * F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji);  W_i = sum_j r_ij (x) dU_j/dr_ji  (r_ij = r_j - r_i), so
+ * sum_i W_i = -dE/d(strain), positive under compression.  Any output pointer may be NULL.
+ */
+int nep_zbl_compute(nepzbl_handle *h, int64_t n, const double *pos_soa, const int32_t *types,
+                    const double box[9], const int32_t pbc[3], double *energy, float *force,
+                    float *virial);
+/* Same call with HOST buffers: copies pos/types in and energy/force/virial out around the
+ * evaluation (staging buffers live in the workspace). */
+int nep_zbl_compute_host(nepzbl_handle *h, int64_t n, const double *pos_soa, const int32_t *types,
+                         const double box[9], const int32_t pbc[3], double *energy, float *force,
+                         float *virial);
+/* Descriptor vectors of the last evaluation, fp32 dev [n][D] row-major, caller's atom order
+ * (for parity tests of S3/S4). */
+int nep_zbl_get_descriptors(nepzbl_handle *h, float *q);
+
+/*
+ * S8: velocity-Verlet with the adaptive time step of P:77 (S:F, D: C-11, C-12).
+ * md_init registers caller-owned dev buffers pos_soa/vel_soa (integrated IN PLACE until destroy or
+ * the next md_init), builds the list and evaluates the initial forces.
+ * md_step: v_max = max_i |v_i|; dt = min(dt_max, max_displacement / v_max) (dt_max if v_max = 0);
+ *   v += dt/2 F/m; x += dt v; wrap periodic axes; rebuild the list if an atom moved > skin/2 since
+ *   the last build; F = F(x); v += dt/2 F/m.  Returns dt and whether the list was rebuilt (host).
+ * md_run: n_steps such steps with no host round trip in between; dt_trace (host, [n_steps]) and
+ *   n_rebuilds (host) may be NULL.
+ * max_displacement may be +inf (fixed dt = dt_max).
+ */
+int md_init(nepzbl_handle *h, int64_t n, double *pos_soa, double *vel_soa, const int32_t *types,
+            const double box[9], const int32_t pbc[3]);
+int md_step(nepzbl_handle *h, double dt_max, double max_displacement, double *dt_used,
+            int32_t *rebuilt);
+int md_run(nepzbl_handle *h, int64_t n_steps, double dt_max, double max_displacement,
+           double *dt_trace, int64_t *n_rebuilds);
+/* md_step with HOST state: copies pos/vel (host, 3n doubles each) to the registered device buffers,
+ * steps, copies them back. */
+int md_step_host(nepzbl_handle *h, double *pos_soa, double *vel_soa, double dt_max,
+                 double max_displacement, double *dt_used, int32_t *rebuilt);
+/* Total potential and kinetic energy of the current MD state (host scalars), fixed-order fp64
+ * reduction. */
+int md_energies(nepzbl_handle *h, double *e_pot, double *e_kin);
+/* Current MD forces (fp32 SoA [3n]) and per-atom potential energies (fp64 [n]) to dev buffers. */
+int md_get_forces(nepzbl_handle *h, float *force, double *energy);
+/* Counters since md_init: steps, list rebuilds, ZBL pair evaluations of the last step. */
+int md_get_counters(nepzbl_handle *h, int64_t *n_steps, int64_t *n_rebuilds, int64_t *n_zbl_atoms);
+
+/* Number of kernel launches issued by this handle so far (for bench.py's gpu_launches). */
+int64_t nep_zbl_launch_count(const nepzbl_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NEPZBL_H */

@@ -1,0 +1,90 @@
+// common.cuh -- device-side data layout of the NEP-ZBL hot path (sm_100a).
+//
+// Data layout in HBM:
+//   master state   pos/vel fp64 SoA in the CALLER's atom order (caller-owned)
+//   compute copy   xyzt[s] = {ux,uy,uz,type}: 32-bit FIXED-POINT coordinates (fraction of the box
+//                  span per axis, 2^-32 units) in CELL-SORTED order s.  Differences of two such
+//                  coordinates are exact integers and wrap modulo 2^32, i.e. the minimum image on
+//                  periodic axes comes for free; resolution L/2^32 (1.2e-7 A at L = 506 A).
+//   lists          column-major NL[slot][Npad] (coalesced over atoms), Npad = n rounded up to 128.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define NEPZBL_AMU_A2_FS2_TO_EV 103.6426965
+#define NEPZBL_PI_F 3.14159265358979323846f
+
+struct BoxMap {  // device-resident; recomputed by k_boxmap at every list rebuild
+  double lo[3];     // origin of the fixed-point grid per axis
+  double inv_h[3];  // 2^32 / span
+  double h[3];      // span / 2^32   (Angstrom per unit)
+  double L[3];      // box edge (periodic axes: span == L)
+  float hf[3];
+  int pbc[3];
+  int nc[3];        // cells per axis actually used
+  int ncv[3];       // cell index = (u * ncv) >> 32
+  int ncells;
+};
+
+struct Scalars {  // device-resident control block (one per handle)
+  int do_rebuild;
+  int force_rebuild;
+  unsigned int maxdisp2_bits;           // float bits: max_i |x_i - x_i(build)|^2
+  unsigned long long vmax2_bits[2];     // double bits: max_i |v_i|^2, double-buffered by step parity
+  double dt;
+  unsigned long long bmin[3], bmax[3];  // order-preserving encodings of min/max coordinate (open axes)
+  int overflow_radial, overflow_angular;  // largest neighbour counts seen at the last build
+  int nonfinite;
+  int box_too_small;
+  int zbl_count;
+  int n_rebuilds;
+  long long n_steps;
+};
+
+struct BoxHost {  // passed by value to k_boxmap
+  double L[3];
+  int pbc[3];
+  double rcs;      // rc_radial + skin: minimum cell edge
+  int ncell_cap;
+};
+
+// order-preserving map double -> uint64 (for atomicMin/Max on signed doubles)
+__host__ __device__ inline unsigned long long enc_double(double x) {
+#ifdef __CUDA_ARCH__
+  unsigned long long b = (unsigned long long)__double_as_longlong(x);
+#else
+  unsigned long long b;
+  memcpy(&b, &x, 8);
+#endif
+  return (b & 0x8000000000000000ull) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ inline double dec_double(unsigned long long k) {
+  unsigned long long b = (k & 0x8000000000000000ull) ? (k & 0x7fffffffffffffffull) : ~k;
+  return __longlong_as_double((long long)b);
+}
+
+// fixed-point coordinate of x on one axis (wraps modulo 2^32 on periodic axes)
+__device__ __forceinline__ unsigned int fix_coord(double x, double lo, double inv_h) {
+  return (unsigned int)(unsigned long long)__double2ll_rd((x - lo) * inv_h);
+}
+
+__device__ __forceinline__ int cell_of_u(unsigned int u, int ncv, int nc) {
+  int c = (int)(((unsigned long long)u * (unsigned long long)ncv) >> 32);
+  return c < nc ? c : nc - 1;
+}
+
+__device__ __forceinline__ float block_max_128(float v, float* sh) {
+  // max over a block of <= 1024 threads; result valid in thread 0
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) sh[w] = v;
+  __syncthreads();
+  if (w == 0) {
+    int nw = (blockDim.x + 31) >> 5;
+    v = l < nw ? sh[l] : 0.0f;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  }
+  return v;
+}

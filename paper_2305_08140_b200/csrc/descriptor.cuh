@@ -1,0 +1,407 @@
+// descriptor.cuh -- S3 (radial descriptor), S4 (angular descriptor), S6 (network) and the angular
+// half of S7 (per-pair partial forces), one thread per atom in cell-sorted order.
+//
+// Formulas (the paper defers them to its ref. [25]; SURVEY 8(c) B-E is the reading):
+//   f_c(r) = 1/2 [1 + cos(pi r / rc)],  x = 2 (r/rc - 1)^2 - 1,  f_k = 1/2 [T_k(x) + 1] f_c
+//   g_n(r) = sum_k c_nk f_k(r)
+//   q_n = sum_j g^R_n(r_ij);  q_nl = (2l+1)/(4 pi) sum_jk g^A_n g^A_n P_l(cos);  q^222_n (4-body)
+//   U = sum_mu w1_mu tanh(sum_nu w0_mu,nu s_nu q_nu - b0_mu) - b1
+// Factorisations used here (same numbers up to rounding):
+//   * g_n = f_c * sum_k ct_nk T_k with ct folded on the host (ct_n0 = c_n0 + 1/2 sum_{k>=1} c_nk,
+//     ct_nk = c_nk / 2), so q_n = sum_k ct_nk * (sum_j f_c T_k): the radial pass accumulates K
+//     basis sums per atom instead of n_max*K products per neighbour (one atom type).
+//   * 3-body by the addition theorem: q_nl = (2l+1)/(4 pi) sum_m C_lm A_nlm^2 with
+//     A_nlm = sum_j g_n(r_ij) b_lm(rhat_ij), b_lm = real harmonic polynomials (unnormalised,
+//     P_l^(m)(z) * Re/Im (x+iy)^m up to the scale folded into C_lm).
+//   * 4-body: q^222_n = 3 C4 det S_n, S_n the traceless tensor rebuilt from the five l=2 sums.
+//   * back-pass: dU_i/dr_ij = rhat S' + (v - rhat (rhat.v))/r with S' = sum_lm G'_lm b_lm,
+//     v = sum_lm G_lm grad b_lm, G_lm = sum_n g_n E_nlm, G'_lm = sum_n g'_n E_nlm, E = dU/dA.
+#pragma once
+#include "common.cuh"
+
+template <int NR_, int KR_, int NA_, int KA_, bool B4_>
+struct ModelShape {
+  static constexpr int NR = NR_;  // n_max_radial + 1
+  static constexpr int KR = KR_;  // basis_radial + 1
+  static constexpr int NA = NA_;
+  static constexpr int KA = KA_;
+  static constexpr bool B4 = B4_;
+  static constexpr int LMAX = 4;
+  static constexpr int NLM = 24;
+  static constexpr int D = NR + NA * LMAX + (B4 ? NA : 0);
+  static constexpr int DPAD = (D + 3) / 4 * 4;
+};
+
+// Small tables passed by value (constant bank): compile-time indexed, so they cost no loads.
+template <class MS>
+struct ModelTables {
+  float ctR[MS::NR][MS::KR];   // folded radial coefficients
+  float ctA[MS::NA][MS::KA];   // folded angular coefficients
+  float kctA[MS::NA][MS::KA];  // k * ctA (derivative through T_k' = k U_{k-1})
+  float inv_rcR, inv_rcA, rcR2, rcA2;
+  float zbl_flag_r2;           // (r_outer + margin)^2, 0 if ZBL disabled
+  float b1;
+  int n_neurons;
+};
+
+// (2l+1)/(4 pi) * addition-theorem weight of each b_lm (see DESIGN.md for the list of b_lm)
+__device__ __constant__ const float kClm[24] = {
+    0.238732414637843f, 0.238732414637843f, 0.238732414637843f,                       // l=1: 3/(4pi)*{1,1,1}
+    0.099471839432435f, 1.193662073189215f, 1.193662073189215f, 0.298415518297304f,
+    0.298415518297304f,                                                                // l=2: 5/(4pi)*{1/4,3,3,3/4,3/4}
+    0.139260575205408f, 0.208890862808112f, 0.208890862808112f, 2.088908628081126f,
+    2.088908628081126f, 0.348151438013521f, 0.348151438013521f,                        // l=3: 7/(4pi)*{1/4,3/8,3/8,15/4,15/4,5/8,5/8}
+    0.011190581936149f, 0.447623277445971f, 0.447623277445971f, 0.223811638722985f,
+    0.223811638722985f, 3.133362942121796f, 3.133362942121796f, 0.391670367765225f,
+    0.391670367765225f};                                                               // l=4: 9/(4pi)*{1/64,5/8,5/8,5/16,5/16,35/8,35/8,35/64,35/64}
+#define NEPZBL_C4 (-0.269981309759908f) /* -45/(8 sqrt(14) pi^1.5) */
+
+__device__ __forceinline__ int lm_to_l(int lm) { return lm < 3 ? 1 : (lm < 8 ? 2 : (lm < 15 ? 3 : 4)); }
+
+// real harmonic polynomials of the unit vector (x,y,z), l = 1..4
+__device__ __forceinline__ void eval_blm(float x, float y, float z, float b[24]) {
+  float z2 = z * z, x2 = x * x, y2 = y * y;
+  float c2 = x2 - y2, s2 = 2.0f * x * y;
+  float c3 = x * (x2 - 3.0f * y2), s3 = y * (3.0f * x2 - y2);
+  float c4 = c2 * c2 - s2 * s2, s4 = 2.0f * c2 * s2;
+  float p31 = 5.0f * z2 - 1.0f, p41 = (7.0f * z2 - 3.0f) * z, p42 = 7.0f * z2 - 1.0f;
+  b[0] = z; b[1] = x; b[2] = y;
+  b[3] = 3.0f * z2 - 1.0f; b[4] = x * z; b[5] = y * z; b[6] = c2; b[7] = s2;
+  b[8] = (5.0f * z2 - 3.0f) * z; b[9] = p31 * x; b[10] = p31 * y; b[11] = z * c2; b[12] = z * s2;
+  b[13] = c3; b[14] = s3;
+  b[15] = (35.0f * z2 - 30.0f) * z2 + 3.0f; b[16] = p41 * x; b[17] = p41 * y; b[18] = p42 * c2;
+  b[19] = p42 * s2; b[20] = z * c3; b[21] = z * s3; b[22] = c4; b[23] = s4;
+}
+
+// S' = sum_lm Gp_lm b_lm and v = sum_lm G_lm grad_u b_lm (gradient of the polynomials in free x,y,z)
+template <class F1, class F2>
+__device__ __forceinline__ void contract_blm_grad(float x, float y, float z, F1 G, F2 Gp, float& Sp,
+                                                  float& vx, float& vy, float& vz) {
+  float z2 = z * z, x2 = x * x, y2 = y * y;
+  float c2 = x2 - y2, s2 = 2.0f * x * y;
+  float c3 = x * (x2 - 3.0f * y2), s3 = y * (3.0f * x2 - y2);
+  float c4 = c2 * c2 - s2 * s2, s4 = 2.0f * c2 * s2;
+  float p31 = 5.0f * z2 - 1.0f, p41 = (7.0f * z2 - 3.0f) * z, p42 = 7.0f * z2 - 1.0f;
+  float xz = x * z, yz = y * z;
+  float q41 = 21.0f * z2 - 3.0f;
+  Sp = 0.0f; vx = 0.0f; vy = 0.0f; vz = 0.0f;
+  float g;
+  // l = 1
+  Sp = fmaf(Gp(0), z, Sp); vz += G(0);
+  Sp = fmaf(Gp(1), x, Sp); vx += G(1);
+  Sp = fmaf(Gp(2), y, Sp); vy += G(2);
+  // l = 2
+  g = G(3); Sp = fmaf(Gp(3), 3.0f * z2 - 1.0f, Sp); vz = fmaf(g, 6.0f * z, vz);
+  g = G(4); Sp = fmaf(Gp(4), xz, Sp); vx = fmaf(g, z, vx); vz = fmaf(g, x, vz);
+  g = G(5); Sp = fmaf(Gp(5), yz, Sp); vy = fmaf(g, z, vy); vz = fmaf(g, y, vz);
+  g = G(6); Sp = fmaf(Gp(6), c2, Sp); vx = fmaf(g, 2.0f * x, vx); vy = fmaf(g, -2.0f * y, vy);
+  g = G(7); Sp = fmaf(Gp(7), s2, Sp); vx = fmaf(g, 2.0f * y, vx); vy = fmaf(g, 2.0f * x, vy);
+  // l = 3
+  g = G(8); Sp = fmaf(Gp(8), (5.0f * z2 - 3.0f) * z, Sp); vz = fmaf(g, 15.0f * z2 - 3.0f, vz);
+  g = G(9); Sp = fmaf(Gp(9), p31 * x, Sp); vx = fmaf(g, p31, vx); vz = fmaf(g, 10.0f * xz, vz);
+  g = G(10); Sp = fmaf(Gp(10), p31 * y, Sp); vy = fmaf(g, p31, vy); vz = fmaf(g, 10.0f * yz, vz);
+  g = G(11); Sp = fmaf(Gp(11), z * c2, Sp); vx = fmaf(g, 2.0f * xz, vx); vy = fmaf(g, -2.0f * yz, vy); vz = fmaf(g, c2, vz);
+  g = G(12); Sp = fmaf(Gp(12), z * s2, Sp); vx = fmaf(g, 2.0f * yz, vx); vy = fmaf(g, 2.0f * xz, vy); vz = fmaf(g, s2, vz);
+  g = G(13); Sp = fmaf(Gp(13), c3, Sp); vx = fmaf(g, 3.0f * c2, vx); vy = fmaf(g, -3.0f * s2, vy);
+  g = G(14); Sp = fmaf(Gp(14), s3, Sp); vx = fmaf(g, 3.0f * s2, vx); vy = fmaf(g, 3.0f * c2, vy);
+  // l = 4
+  g = G(15); Sp = fmaf(Gp(15), (35.0f * z2 - 30.0f) * z2 + 3.0f, Sp); vz = fmaf(g, (140.0f * z2 - 60.0f) * z, vz);
+  g = G(16); Sp = fmaf(Gp(16), p41 * x, Sp); vx = fmaf(g, p41, vx); vz = fmaf(g, q41 * x, vz);
+  g = G(17); Sp = fmaf(Gp(17), p41 * y, Sp); vy = fmaf(g, p41, vy); vz = fmaf(g, q41 * y, vz);
+  g = G(18); Sp = fmaf(Gp(18), p42 * c2, Sp); vx = fmaf(g, 2.0f * p42 * x, vx); vy = fmaf(g, -2.0f * p42 * y, vy); vz = fmaf(g, 14.0f * z * c2, vz);
+  g = G(19); Sp = fmaf(Gp(19), p42 * s2, Sp); vx = fmaf(g, 2.0f * p42 * y, vx); vy = fmaf(g, 2.0f * p42 * x, vy); vz = fmaf(g, 14.0f * z * s2, vz);
+  g = G(20); Sp = fmaf(Gp(20), z * c3, Sp); vx = fmaf(g, 3.0f * z * c2, vx); vy = fmaf(g, -3.0f * z * s2, vy); vz = fmaf(g, c3, vz);
+  g = G(21); Sp = fmaf(Gp(21), z * s3, Sp); vx = fmaf(g, 3.0f * z * s2, vx); vy = fmaf(g, 3.0f * z * c2, vy); vz = fmaf(g, s3, vz);
+  g = G(22); Sp = fmaf(Gp(22), c4, Sp); vx = fmaf(g, 4.0f * c3, vx); vy = fmaf(g, -4.0f * s3, vy);
+  g = G(23); Sp = fmaf(Gp(23), s4, Sp); vx = fmaf(g, 4.0f * s3, vx); vy = fmaf(g, 4.0f * c3, vy);
+}
+
+// cutoff function and Chebyshev polynomials T_0..T_{K-1} at distance r
+template <int K>
+__device__ __forceinline__ void cheb_T(float r, float inv_rc, float& fc, float& dfc, float& x,
+                                       float& dx, float T[K]) {
+  float t = r * inv_rc;
+  float sn, cs;
+  sincospif(t, &sn, &cs);
+  fc = 0.5f + 0.5f * cs;
+  dfc = -0.5f * NEPZBL_PI_F * inv_rc * sn;
+  float u = t - 1.0f;
+  x = fmaf(2.0f * u, u, -1.0f);
+  dx = 4.0f * u * inv_rc;
+  T[0] = 1.0f;
+  if (K > 1) T[1] = x;
+  float x2 = 2.0f * x;
+#pragma unroll
+  for (int k = 2; k < K; ++k) T[k] = fmaf(x2, T[k - 1], -T[k - 2]);
+}
+// Chebyshev polynomials of the second kind U_0..U_{K-2}  (T_k' = k U_{k-1})
+template <int K>
+__device__ __forceinline__ void cheb_U(float x, float U[K]) {
+  U[0] = 1.0f;
+  float x2 = 2.0f * x;
+  if (K > 1) U[1] = x2;
+#pragma unroll
+  for (int k = 2; k < K; ++k) U[k] = fmaf(x2, U[k - 1], -U[k - 2]);
+}
+
+__device__ __forceinline__ float tanh_fast(float z) {
+  // 1 - 2/(e^{2z}+1): absolute error ~1e-7, enough for the 1e-5 eV energy tolerance
+  float e = __expf(2.0f * z);
+  return 1.0f - __fdividef(2.0f, e + 1.0f);
+}
+
+// ------------------------------------------------------------------------- S3: radial descriptor
+// q_n = sum_j g^R_n(r_ij) for r_ij < rc_radial; also flags atoms with a neighbour inside the ZBL range.
+template <class MS>
+__global__ void __launch_bounds__(128)
+k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
+         const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
+         const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,
+         int* __restrict__ zbl_list) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const int4 me = xyzt[s];
+  const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
+  float acc[MS::KR];
+#pragma unroll
+  for (int k = 0; k < MS::KR; ++k) acc[k] = 0.0f;
+  bool close = false;
+  const int cnt = nn_r[s];
+  int jn = cnt > 0 ? nl_r[s] : 0;
+  for (int t = 0; t < cnt; ++t) {
+    int j = jn;
+    if (t + 1 < cnt) jn = nl_r[(size_t)(t + 1) * npad + s];
+    int4 o = xyzt[j];
+    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
+    float r2 = dx * dx + dy * dy + dz * dz;
+    if (r2 < mt.rcR2) {
+      float r = sqrtf(r2), fc, dfc, x, dxdr, T[MS::KR];
+      cheb_T<MS::KR>(r, mt.inv_rcR, fc, dfc, x, dxdr, T);
+#pragma unroll
+      for (int k = 0; k < MS::KR; ++k) acc[k] = fmaf(fc, T[k], acc[k]);
+      close = close || (r2 < mt.zbl_flag_r2);
+    }
+  }
+#pragma unroll
+  for (int nq = 0; nq < MS::NR; ++nq) {
+    float q = 0.0f;
+#pragma unroll
+    for (int k = 0; k < MS::KR; ++k) q = fmaf(mt.ctR[nq][k], acc[k], q);
+    q_radial[(size_t)nq * npad + s] = q;
+  }
+  if (close) zbl_list[atomicAdd(&sc->zbl_count, 1)] = s;
+}
+
+// ------------------------------------------------------- S4 + S6 + angular partial forces of S7
+// Network weights staged in shared memory: w0 [neurons][DPAD], b0, w1 [neurons], q_scaler [DPAD].
+template <class MS>
+__global__ void __launch_bounds__(128)
+k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
+             const int* __restrict__ nn_a, const int* __restrict__ nl_a,
+             const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,
+             const float* __restrict__ q_radial, float* __restrict__ u_site,
+             float4* __restrict__ dk, float4* __restrict__ pforce, float* __restrict__ q_out) {
+  constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR, D = MS::D, DPAD = MS::DPAD;
+  extern __shared__ __align__(16) float smem[];
+  const int neu = mt.n_neurons;
+  float* s_w0 = smem;                  // [neu][DPAD]
+  float* s_b0 = s_w0 + neu * DPAD;     // [neu]
+  float* s_w1 = s_b0 + neu;            // [neu]
+  float* s_qs = s_w1 + neu;            // [DPAD]
+  for (int t = threadIdx.x; t < neu * DPAD + 2 * neu + DPAD; t += blockDim.x) smem[t] = nnw[t];
+  __syncthreads();
+
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const int4 me = xyzt[s];
+  const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
+  const int cnt = nn_a[s];
+
+  // which list entries are inside rc_angular right now (list carries the skin)
+  unsigned long long mask = 0ull;
+  for (int a = 0; a < cnt; ++a) {
+    int j = nl_a[(size_t)a * npad + s];
+    int4 o = xyzt[j];
+    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
+    float r2 = dx * dx + dy * dy + dz * dz;
+    if (r2 < mt.rcA2) mask |= 1ull << a;
+  }
+
+  // ---- S4 forward: A[n][lm] = sum_j g_n(r_ij) b_lm(rhat_ij)
+  float A[NA][24];
+#pragma unroll
+  for (int nq = 0; nq < NA; ++nq)
+#pragma unroll
+    for (int lm = 0; lm < 24; ++lm) A[nq][lm] = 0.0f;
+  for (unsigned long long m = mask; m; m &= m - 1) {
+    int a = __ffsll((long long)m) - 1;
+    int j = nl_a[(size_t)a * npad + s];
+    int4 o = xyzt[j];
+    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
+    float r2 = dx * dx + dy * dy + dz * dz;
+    float r = sqrtf(r2), rinv = 1.0f / r;
+    float fc, dfc, x, dxdr, T[KA];
+    cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
+    float b[24];
+    eval_blm(dx * rinv, dy * rinv, dz * rinv, b);
+#pragma unroll
+    for (int nq = 0; nq < NA; ++nq) {
+      float g = 0.0f;
+#pragma unroll
+      for (int k = 0; k < KA; ++k) g = fmaf(mt.ctA[nq][k], T[k], g);
+      g *= fc;
+#pragma unroll
+      for (int lm = 0; lm < 24; ++lm) A[nq][lm] = fmaf(g, b[lm], A[nq][lm]);
+    }
+  }
+
+  // ---- descriptor vector (SURVEY 8(c) C order), scaled
+  float q[D];
+#pragma unroll
+  for (int nq = 0; nq < NR; ++nq) q[nq] = q_radial[(size_t)nq * npad + s];
+#pragma unroll
+  for (int nq = 0; nq < NA; ++nq) {
+    float ql[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+    for (int lm = 0; lm < 24; ++lm) ql[lm_to_l(lm) - 1] = fmaf(kClm[lm] * A[nq][lm], A[nq][lm], ql[lm_to_l(lm) - 1]);
+#pragma unroll
+    for (int l = 0; l < 4; ++l) q[NR + l * NA + nq] = ql[l];
+  }
+  float dq4[MS::B4 ? NA : 1][5];  // d q4_n / d A[n][3..7]
+  if (MS::B4) {
+#pragma unroll
+    for (int nq = 0; nq < NA; ++nq) {
+      float a0 = A[nq][3], a1 = A[nq][4], a2 = A[nq][5], a3 = A[nq][6], a4 = A[nq][7];
+      float Szz = a0 * (1.0f / 3.0f), Sxz = a1, Syz = a2, Sxy = 0.5f * a4;
+      float Sxx = fmaf(-1.0f / 6.0f, a0, 0.5f * a3), Syy = fmaf(-1.0f / 6.0f, a0, -0.5f * a3);
+      float cxx = Syy * Szz - Syz * Syz, cyy = Sxx * Szz - Sxz * Sxz, czz = Sxx * Syy - Sxy * Sxy;
+      float cxy = Sxz * Syz - Sxy * Szz, cxz = Sxy * Syz - Syy * Sxz, cyz = Sxy * Sxz - Sxx * Syz;
+      float det = Sxx * cxx + Sxy * cxy + Sxz * cxz;
+      const float k3 = 3.0f * NEPZBL_C4;
+      q[NR + 4 * NA + nq] = k3 * det;
+      dq4[nq][0] = k3 * ((czz * (1.0f / 3.0f)) - (cxx + cyy) * (1.0f / 6.0f));
+      dq4[nq][1] = k3 * 2.0f * cxz;
+      dq4[nq][2] = k3 * 2.0f * cyz;
+      dq4[nq][3] = k3 * 0.5f * (cxx - cyy);
+      dq4[nq][4] = k3 * cxy;
+    }
+  }
+  if (q_out) {
+#pragma unroll
+    for (int v = 0; v < D; ++v) q_out[(size_t)v * npad + s] = q[v];
+  }
+
+  // ---- S6: network forward + gradient
+  float Fp[D];
+#pragma unroll
+  for (int v = 0; v < D; ++v) {
+    q[v] *= s_qs[v];
+    Fp[v] = 0.0f;
+  }
+  float U = -mt.b1;
+#pragma unroll 1
+  for (int m = 0; m < neu; ++m) {
+    const float4* w4 = reinterpret_cast<const float4*>(s_w0 + m * DPAD);  // broadcast LDS.128
+    float z0 = -s_b0[m], z1 = 0.0f;
+#pragma unroll
+    for (int v4 = 0; v4 < DPAD / 4; ++v4) {
+      float4 w = w4[v4];
+      if (4 * v4 + 0 < D) z0 = fmaf(w.x, q[4 * v4 + 0], z0);
+      if (4 * v4 + 1 < D) z1 = fmaf(w.y, q[4 * v4 + 1], z1);
+      if (4 * v4 + 2 < D) z0 = fmaf(w.z, q[4 * v4 + 2], z0);
+      if (4 * v4 + 3 < D) z1 = fmaf(w.w, q[4 * v4 + 3], z1);
+    }
+    float hh = tanh_fast(z0 + z1);
+    float w1 = s_w1[m];
+    U = fmaf(w1, hh, U);
+    float tt = w1 * fmaf(-hh, hh, 1.0f);
+#pragma unroll
+    for (int v4 = 0; v4 < DPAD / 4; ++v4) {
+      float4 w = w4[v4];
+      if (4 * v4 + 0 < D) Fp[4 * v4 + 0] = fmaf(tt, w.x, Fp[4 * v4 + 0]);
+      if (4 * v4 + 1 < D) Fp[4 * v4 + 1] = fmaf(tt, w.y, Fp[4 * v4 + 1]);
+      if (4 * v4 + 2 < D) Fp[4 * v4 + 2] = fmaf(tt, w.z, Fp[4 * v4 + 2]);
+      if (4 * v4 + 3 < D) Fp[4 * v4 + 3] = fmaf(tt, w.w, Fp[4 * v4 + 3]);
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < D; ++v) Fp[v] *= s_qs[v];
+  u_site[s] = U;
+
+  // radial back-pass coefficients d_k = sum_n Fp_n ct_nk  (used by k_force for both i and j)
+  {
+    float d[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) d[k] = 0.0f;
+#pragma unroll
+    for (int k = 0; k < KR; ++k)
+#pragma unroll
+      for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
+    dk[3 * (size_t)s + 0] = make_float4(d[0], d[1], d[2], d[3]);
+    dk[3 * (size_t)s + 1] = make_float4(d[4], d[5], d[6], d[7]);
+    dk[3 * (size_t)s + 2] = make_float4(d[8], d[9], d[10], d[11]);
+  }
+
+  // ---- E[n][lm] = dU/dA[n][lm] (in place)
+#pragma unroll
+  for (int nq = 0; nq < NA; ++nq) {
+#pragma unroll
+    for (int lm = 0; lm < 24; ++lm)
+      A[nq][lm] *= 2.0f * kClm[lm] * Fp[NR + (lm_to_l(lm) - 1) * NA + nq];
+    if (MS::B4) {
+#pragma unroll
+      for (int m5 = 0; m5 < 5; ++m5) A[nq][3 + m5] = fmaf(Fp[NR + 4 * NA + nq], dq4[nq][m5], A[nq][3 + m5]);
+    }
+  }
+
+  // ---- angular partial forces dU_i/dr_ij for every list entry (zero outside the cutoff)
+  {
+    unsigned long long all = cnt >= 64 ? ~0ull : ((1ull << cnt) - 1ull);
+    for (unsigned long long m = all & ~mask; m; m &= m - 1) {
+      int a = __ffsll((long long)m) - 1;
+      pforce[(size_t)a * npad + s] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    }
+  }
+  for (unsigned long long m = mask; m; m &= m - 1) {
+    int a = __ffsll((long long)m) - 1;
+    int j = nl_a[(size_t)a * npad + s];
+    int4 o = xyzt[j];
+    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
+    float r2 = dx * dx + dy * dy + dz * dz;
+    float r = sqrtf(r2), rinv = 1.0f / r;
+    float fc, dfc, x, dxdr, T[KA], Uc[KA];
+    cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
+    cheb_U<KA>(x, Uc);
+    float g[NA], dg[NA];
+#pragma unroll
+    for (int nq = 0; nq < NA; ++nq) {
+      float p = 0.0f, dp = 0.0f;
+#pragma unroll
+      for (int k = 0; k < KA; ++k) p = fmaf(mt.ctA[nq][k], T[k], p);
+#pragma unroll
+      for (int k = 1; k < KA; ++k) dp = fmaf(mt.kctA[nq][k], Uc[k - 1], dp);
+      g[nq] = fc * p;
+      dg[nq] = fmaf(dfc, p, fc * dxdr * dp);
+    }
+    float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+    auto G = [&](int lm) {
+      float t = 0.0f;
+#pragma unroll
+      for (int nq = 0; nq < NA; ++nq) t = fmaf(g[nq], A[nq][lm], t);
+      return t;
+    };
+    auto Gp = [&](int lm) {
+      float t = 0.0f;
+#pragma unroll
+      for (int nq = 0; nq < NA; ++nq) t = fmaf(dg[nq], A[nq][lm], t);
+      return t;
+    };
+    float Sp, vx, vy, vz;
+    contract_blm_grad(ux, uy, uz, G, Gp, Sp, vx, vy, vz);
+    float uv = ux * vx + uy * vy + uz * vz;
+    float px = fmaf(ux, Sp, (vx - ux * uv) * rinv);
+    float py = fmaf(uy, Sp, (vy - uy * uv) * rinv);
+    float pz = fmaf(uz, Sp, (vz - uz * uv) * rinv);
+    pforce[(size_t)a * npad + s] = make_float4(px, py, pz, 0.0f);
+  }
+}

@@ -1,0 +1,334 @@
+// neighbor.cuh -- S1 (state prep) and S2 (cell-list neighbour build) kernels.
+//
+// S2 (BASELINE.json north_star "cell-list neighbour build"; cutoffs P:106):
+//   bin atoms into cells of edge >= rc_radial+skin, canonical in-cell order (ascending caller
+//   index), then per atom walk the 27 surrounding cells and list every j with
+//   r_ij < rc_radial+skin (radial list) and the subset r_ij < rc_angular+skin (angular list).
+// Every rebuild kernel early-exits unless Scalars::do_rebuild is set, so the MD loop can enqueue
+// the whole chain each step with no host round trip.
+// Determinism: integer atomics only (counts / slot tickets); the ticket order is erased by the
+// per-cell sort, so the sorted order and the lists are reproducible bit for bit.
+#pragma once
+#include "common.cuh"
+
+// ---------------------------------------------------------------- open-axis bounds
+__global__ void k_bounds(Scalars* sc, int n, const double* __restrict__ pos, int open0, int open1,
+                         int open2) {
+  if (!sc->do_rebuild) return;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int open[3] = {open0, open1, open2};
+  for (int a = 0; a < 3; ++a) {
+    if (!open[a]) continue;
+    double x = i < n ? pos[(size_t)a * n + i] : 0.0;
+    bool ok = i < n && isfinite(x);
+    unsigned long long kmin = ok ? enc_double(x) : ~0ull, kmax = ok ? enc_double(x) : 0ull;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      unsigned long long a1 = __shfl_xor_sync(0xffffffffu, kmin, o);
+      unsigned long long a2 = __shfl_xor_sync(0xffffffffu, kmax, o);
+      kmin = a1 < kmin ? a1 : kmin;
+      kmax = a2 > kmax ? a2 : kmax;
+    }
+    if ((threadIdx.x & 31) == 0) {
+      atomicMin(&sc->bmin[a], kmin);
+      atomicMax(&sc->bmax[a], kmax);
+    }
+  }
+}
+
+__global__ void k_rebuild_begin(Scalars* sc) {
+  if (!sc->do_rebuild) return;
+  for (int a = 0; a < 3; ++a) {
+    sc->bmin[a] = ~0ull;
+    sc->bmax[a] = 0ull;
+  }
+  sc->overflow_radial = 0;
+  sc->overflow_angular = 0;
+  sc->maxdisp2_bits = 0u;
+}
+
+// Fixed-point grid and cell grid for this build (one thread).
+__global__ void k_boxmap(Scalars* sc, BoxMap* bm, BoxHost bh) {
+  if (!sc->do_rebuild) return;
+  const double two32 = 4294967296.0;
+  for (int f = 1;; f *= 2) {  // coarsen cells until the grid fits the cell arrays
+    double cw = bh.rcs * f;
+    long long total = 1;
+    for (int a = 0; a < 3; ++a) {
+      bm->pbc[a] = bh.pbc[a];
+      bm->L[a] = bh.L[a];
+      double span, lo;
+      int nc, ncv;
+      if (bh.pbc[a]) {
+        lo = 0.0;
+        span = bh.L[a];
+        nc = (int)floor(bh.L[a] / cw);
+        if (f == 1 && nc < 2) sc->box_too_small = 1;
+        if (nc < 1) nc = 1;
+        ncv = nc;
+      } else {
+        // open axis (SURVEY C-14): grid spans the atoms' bounding range plus margins; the 2^32
+        // span is twice that, so int32 differences never wrap for real pairs.
+        double mn = dec_double(sc->bmin[a]), mx = dec_double(sc->bmax[a]);
+        if (!(mx >= mn)) { mn = 0.0; mx = 0.0; }
+        double E = mx - mn, M = cw;
+        ncv = (int)ceil(2.0 * (E + 2.0 * M) / cw);
+        if (ncv < 2) ncv = 2;
+        span = ncv * cw;
+        lo = mn - M;
+        nc = (int)floor((M + E) / cw) + 1;
+        if (nc > ncv) nc = ncv;
+      }
+      bm->lo[a] = lo;
+      bm->inv_h[a] = two32 / span;
+      bm->h[a] = span / two32;
+      bm->hf[a] = (float)(span / two32);
+      bm->nc[a] = nc;
+      bm->ncv[a] = ncv;
+      total *= nc;
+    }
+    if (total <= bh.ncell_cap || f >= (1 << 20)) {
+      bm->ncells = (int)(total <= bh.ncell_cap ? total : bh.ncell_cap);
+      break;
+    }
+  }
+}
+
+__global__ void k_zero_cells(const Scalars* sc, const BoxMap* bm, int* cell_count, int* cell_fill,
+                             int ncell_cap) {
+  if (!sc->do_rebuild) return;
+  int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c <= ncell_cap) {
+    cell_count[c] = 0;
+    if (c < ncell_cap) cell_fill[c] = 0;
+  }
+}
+
+// S1 for a rebuild: fixed-point compute copy (caller order) + cell histogram.
+__global__ void k_bin(Scalars* sc, const BoxMap* __restrict__ bm, int n,
+                      const double* __restrict__ pos, const int32_t* __restrict__ types,
+                      int4* __restrict__ xyzt_tmp, int* __restrict__ cell_of, int* cell_count) {
+  if (!sc->do_rebuild) return;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double x = pos[i], y = pos[(size_t)n + i], z = pos[2 * (size_t)n + i];
+  if (!(isfinite(x) && isfinite(y) && isfinite(z))) {
+    sc->nonfinite = 1;
+    x = y = z = 0.0;
+  }
+  unsigned int ux = fix_coord(x, bm->lo[0], bm->inv_h[0]);
+  unsigned int uy = fix_coord(y, bm->lo[1], bm->inv_h[1]);
+  unsigned int uz = fix_coord(z, bm->lo[2], bm->inv_h[2]);
+  int cx = cell_of_u(ux, bm->ncv[0], bm->nc[0]);
+  int cy = cell_of_u(uy, bm->ncv[1], bm->nc[1]);
+  int cz = cell_of_u(uz, bm->ncv[2], bm->nc[2]);
+  int c = (cz * bm->nc[1] + cy) * bm->nc[0] + cx;
+  xyzt_tmp[i] = make_int4((int)ux, (int)uy, (int)uz, types ? types[i] : 0);
+  cell_of[i] = c;
+  atomicAdd(&cell_count[c], 1);
+}
+
+// exclusive scan of cell_count[0..ncells) -> cell_start[0..ncells]; one block of 1024 threads.
+__global__ void __launch_bounds__(1024) k_scan(const Scalars* sc, const BoxMap* bm,
+                                               const int* __restrict__ cell_count,
+                                               int* __restrict__ cell_start) {
+  if (!sc->do_rebuild) return;
+  __shared__ int part[1024];
+  int ncells = bm->ncells;
+  int chunk = (ncells + 1023) / 1024;
+  int b = threadIdx.x * chunk, e = min(b + chunk, ncells);
+  int s = 0;
+  for (int c = b; c < e; ++c) s += cell_count[c];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {  // Hillis-Steele inclusive scan of the partial sums
+    int v = threadIdx.x >= o ? part[threadIdx.x - o] : 0;
+    __syncthreads();
+    part[threadIdx.x] += v;
+    __syncthreads();
+  }
+  int run = threadIdx.x ? part[threadIdx.x - 1] : 0;
+  for (int c = b; c < e; ++c) {
+    cell_start[c] = run;
+    run += cell_count[c];
+  }
+  if (threadIdx.x == 1023) cell_start[ncells] = part[1023];
+}
+
+__global__ void k_place(const Scalars* sc, int n, const int* __restrict__ cell_of,
+                        const int* __restrict__ cell_start, int* cell_fill, int* __restrict__ order) {
+  if (!sc->do_rebuild) return;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int c = cell_of[i];
+  int t = atomicAdd(&cell_fill[c], 1);
+  order[cell_start[c] + t] = i;
+}
+
+// canonical in-cell order: ascending caller index (erases the ticket order of k_place)
+__global__ void k_sortcell(const Scalars* sc, const BoxMap* bm, const int* __restrict__ cell_start,
+                           int* __restrict__ order) {
+  if (!sc->do_rebuild) return;
+  int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= bm->ncells) return;
+  int b = cell_start[c], e = cell_start[c + 1];
+  for (int p = b + 1; p < e; ++p) {
+    int v = order[p], q = p - 1;
+    while (q >= b && order[q] > v) {
+      order[q + 1] = order[q];
+      --q;
+    }
+    order[q + 1] = v;
+  }
+}
+
+__global__ void k_permute(const Scalars* sc, int n, const int* __restrict__ order,
+                          const int4* __restrict__ xyzt_tmp, int* __restrict__ perm,
+                          int* __restrict__ inv_perm, int4* __restrict__ xyzt,
+                          int4* __restrict__ xyzt_build) {
+  if (!sc->do_rebuild) return;
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  int i = order[s];
+  perm[s] = i;
+  inv_perm[i] = s;
+  int4 v = xyzt_tmp[i];
+  xyzt[s] = v;
+  xyzt_build[s] = v;
+}
+
+// neighbour cells along one axis: up to 3 distinct indices, -1 = none
+__device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int out[3]) {
+  out[0] = c - 1;
+  out[1] = c;
+  out[2] = c + 1;
+  if (pbc) {
+    if (nc >= 3) {
+      if (out[0] < 0) out[0] += nc;
+      if (out[2] >= nc) out[2] -= nc;
+    } else if (nc == 2) {
+      out[0] = -1;             // c-1 and c+1 are the same cell
+      out[2] = 1 - c;
+    } else {
+      out[0] = out[2] = -1;
+    }
+  } else {
+    if (out[0] < 0) out[0] = -1;
+    if (out[2] >= nc) out[2] = -1;
+  }
+}
+
+// per atom (sorted order): walk the 27 cells, emit radial and angular lists (column-major).
+__global__ void __launch_bounds__(128)
+k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
+      const int* __restrict__ cell_start, float rcs2_radial, float rcs2_angular, int cap_r, int cap_a,
+      int* __restrict__ nn_r, int* __restrict__ nl_r, int* __restrict__ nn_a, int* __restrict__ nl_a) {
+  if (!sc->do_rebuild) return;
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const int4 me = xyzt[s];
+  const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
+  int sx[3], sy[3], sz[3];
+  axis_stencil(cell_of_u((unsigned)me.x, bm->ncv[0], bm->nc[0]), bm->nc[0], bm->pbc[0], sx);
+  axis_stencil(cell_of_u((unsigned)me.y, bm->ncv[1], bm->nc[1]), bm->nc[1], bm->pbc[1], sy);
+  axis_stencil(cell_of_u((unsigned)me.z, bm->ncv[2], bm->nc[2]), bm->nc[2], bm->pbc[2], sz);
+  int cr = 0, ca = 0;
+  for (int kz = 0; kz < 3; ++kz) {
+    if (sz[kz] < 0) continue;
+    for (int ky = 0; ky < 3; ++ky) {
+      if (sy[ky] < 0) continue;
+      for (int kx = 0; kx < 3; ++kx) {
+        if (sx[kx] < 0) continue;
+        int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
+        int b = cell_start[c], e = cell_start[c + 1];
+        for (int j = b; j < e; ++j) {
+          if (j == s) continue;
+          int4 o = xyzt[j];
+          float dx = (float)(o.x - me.x) * hx;  // int32 wrap-around = minimum image
+          float dy = (float)(o.y - me.y) * hy;
+          float dz = (float)(o.z - me.z) * hz;
+          float r2 = dx * dx + dy * dy + dz * dz;
+          if (r2 < rcs2_radial) {
+            if (cr < cap_r) nl_r[(size_t)cr * npad + s] = j;
+            ++cr;
+            if (r2 < rcs2_angular) {
+              if (ca < cap_a) nl_a[(size_t)ca * npad + s] = j;
+              ++ca;
+            }
+          }
+        }
+      }
+    }
+  }
+  nn_r[s] = min(cr, cap_r);
+  nn_a[s] = min(ca, cap_a);
+  if (cr > cap_r) atomicMax(&sc->overflow_radial, cr);
+  if (ca > cap_a) atomicMax(&sc->overflow_angular, ca);
+}
+
+// reverse index of the (symmetric) angular list: rev[a][s] = position of s in the list of j = nl_a[a][s]
+__global__ void k_rev(const Scalars* sc, int n, int npad, const int* __restrict__ nn_a,
+                      const int* __restrict__ nl_a, unsigned char* __restrict__ rev) {
+  if (!sc->do_rebuild) return;
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  int na = nn_a[s];
+  for (int a = 0; a < na; ++a) {
+    int j = nl_a[(size_t)a * npad + s];
+    int nj = nn_a[j], b = 0;
+    for (; b < nj; ++b)
+      if (nl_a[(size_t)b * npad + j] == s) break;
+    rev[(size_t)a * npad + s] = (unsigned char)(b < nj ? b : 255);
+  }
+}
+
+// S1 for a plain evaluation: refresh the compute copy from caller positions (keeps the sorted
+// order of the current list) and track the displacement since the build.
+__global__ void __launch_bounds__(256)
+k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restrict__ pos,
+       const int32_t* __restrict__ types, const int* __restrict__ inv_perm, int4* __restrict__ xyzt,
+       const int4* __restrict__ xyzt_build) {
+  __shared__ float sh[32];
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  float d2 = 0.0f;
+  if (i < n) {
+    double x = pos[i], y = pos[(size_t)n + i], z = pos[2 * (size_t)n + i];
+    if (!(isfinite(x) && isfinite(y) && isfinite(z))) {
+      sc->nonfinite = 1;
+      x = y = z = 0.0;
+    }
+    unsigned int ux = fix_coord(x, bm->lo[0], bm->inv_h[0]);
+    unsigned int uy = fix_coord(y, bm->lo[1], bm->inv_h[1]);
+    unsigned int uz = fix_coord(z, bm->lo[2], bm->inv_h[2]);
+    int s = inv_perm[i];
+    int4 b = xyzt_build[s];
+    xyzt[s] = make_int4((int)ux, (int)uy, (int)uz, types ? types[i] : 0);
+    float dx = (float)((int)ux - b.x) * bm->hf[0];
+    float dy = (float)((int)uy - b.y) * bm->hf[1];
+    float dz = (float)((int)uz - b.z) * bm->hf[2];
+    d2 = dx * dx + dy * dy + dz * dz;
+  }
+  float m = block_max_128(d2, sh);
+  if (threadIdx.x == 0 && m > 0.0f) atomicMax(&sc->maxdisp2_bits, __float_as_uint(m));
+}
+
+// decide whether the list must be rebuilt for this evaluation; reset per-evaluation counters.
+__global__ void k_flag(Scalars* sc, float half_skin2) {
+  int r = sc->force_rebuild || (__uint_as_float(sc->maxdisp2_bits) > half_skin2);
+  sc->do_rebuild = r;
+  sc->force_rebuild = 0;
+  sc->zbl_count = 0;
+  if (r) sc->n_rebuilds += 1;
+}
+
+// lists in the caller's indices, row-major [n][cap], -1 padded (neighbor_get)
+__global__ void k_export_list(int n, int npad, int cap, const int* __restrict__ perm,
+                              const int* __restrict__ nn, const int* __restrict__ nl,
+                              int32_t* __restrict__ out_nn, int32_t* __restrict__ out_nl) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  int i = perm[s], c = nn[s];
+  out_nn[i] = c;
+  for (int k = 0; k < cap; ++k)
+    out_nl[(size_t)i * cap + k] = k < c ? perm[nl[(size_t)k * npad + s]] : -1;
+}

@@ -1,0 +1,702 @@
+// nepzbl.cu -- host side of the C ABI declared in include/nepzbl.h: parameter upload, workspace
+// carving, kernel sequencing on one CUDA stream.  All arithmetic of the path runs in the kernels
+// of neighbor.cuh / descriptor.cuh / force.cuh / integrate.cuh.  No CPU fallback exists.
+#include "nepzbl.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "common.cuh"
+#include "neighbor.cuh"
+#include "descriptor.cuh"
+#include "force.cuh"
+#include "integrate.cuh"
+
+namespace {
+
+thread_local std::string g_create_error;
+
+constexpr int kTraceRing = 1024;
+
+struct Carve {  // byte offsets into the workspace
+  size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
+      nn_r, nn_a, nl_r, nl_a, rev, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
+      partial, st_pos, st_types, st_e, st_f, st_w, total;
+  int npad, ncell_cap;
+};
+
+struct ShapeId {
+  int nr, kr, na, ka, b4;
+};
+
+}  // namespace
+
+struct nepzbl_handle {
+  nepzbl_params p{};  // scalar fields only (pointers nulled)
+  int D = 0, shape = -1;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  std::string err;
+  long long launches = 0;
+
+  // library-owned small device block
+  Scalars* d_sc = nullptr;
+  BoxMap* d_bm = nullptr;
+  float* d_nnw = nullptr;
+  double* d_mass = nullptr;
+  double* d_inv_mass = nullptr;
+  double* d_trace = nullptr;  // [kTraceRing]
+  double* d_esum = nullptr;   // [2]
+  Scalars* h_sc = nullptr;    // pinned
+  double* h_trace = nullptr;  // pinned [kTraceRing]
+  double* h_esum = nullptr;   // pinned [2]
+  std::vector<char> tables;   // ModelTables<MS> for the dispatched shape
+  ZblParams zp{};
+  size_t smem_nn = 0;
+
+  // workspace
+  char* ws = nullptr;
+  size_t ws_bytes = 0;
+  long long n_cap = 0;
+  Carve cv{};
+
+  // list state
+  bool have_list = false;
+  long long n = 0;
+  double box[9] = {0};
+  int pbc[3] = {0, 0, 0};
+
+  // md state
+  bool md_ready = false;
+  double* md_pos = nullptr;
+  double* md_vel = nullptr;
+  const int32_t* md_types = nullptr;
+  int parity = 0;
+  long long md_steps = 0;
+
+  template <class T>
+  T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
+};
+
+namespace {
+
+int fail(nepzbl_handle* h, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (h) h->err = buf; else g_create_error = buf;
+  return code;
+}
+
+#define CU(call)                                                                             \
+  do {                                                                                       \
+    cudaError_t e_ = (call);                                                                 \
+    if (e_ != cudaSuccess)                                                                   \
+      return fail(h, NEPZBL_E_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                  __FILE__, __LINE__);                                                       \
+  } while (0)
+
+inline size_t al(size_t x) { return (x + 255) & ~size_t(255); }
+
+Carve carve(const nepzbl_params& p, int D, long long n_cap) {
+  Carve c{};
+  long long npad = (n_cap + 127) / 128 * 128;
+  if (npad < 128) npad = 128;
+  c.npad = (int)npad;
+  c.ncell_cap = (int)(n_cap / 4 + 8192);
+  size_t o = 0;
+  auto take = [&](size_t bytes) { size_t r = o; o = al(o + bytes); return r; };
+  c.xyzt = take(16 * npad);
+  c.xyzt_build = take(16 * npad);
+  c.xyzt_tmp = take(16 * npad);
+  c.perm = take(4 * npad);
+  c.inv_perm = take(4 * npad);
+  c.order = take(4 * npad);
+  c.cell_of = take(4 * npad);
+  c.cell_count = take(4 * ((size_t)c.ncell_cap + 1));
+  c.cell_fill = take(4 * ((size_t)c.ncell_cap + 1));
+  c.cell_start = take(4 * ((size_t)c.ncell_cap + 1));
+  c.nn_r = take(4 * npad);
+  c.nn_a = take(4 * npad);
+  c.nl_r = take(4 * (size_t)p.cap_radial * npad);
+  c.nl_a = take(4 * (size_t)p.cap_angular * npad);
+  c.rev = take((size_t)p.cap_angular * npad);
+  c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
+  c.dk = take(48 * npad);
+  c.pforce = take(16 * (size_t)p.cap_angular * npad);
+  c.u_site = take(4 * npad);
+  c.q_desc = take(4 * (size_t)D * npad);
+  c.zbl_list = take(4 * npad);
+  c.md_force = take(12 * npad);
+  c.md_energy = take(8 * npad);
+  c.partial = take(16 * 1024);
+  c.st_pos = take(24 * npad);
+  c.st_types = take(4 * npad);
+  c.st_e = take(8 * npad);
+  c.st_f = take(12 * npad);
+  c.st_w = take(36 * npad);
+  c.total = o;
+  return c;
+}
+
+const ShapeId kShapes[] = {{5, 9, 5, 9, 1}, {5, 9, 5, 9, 0}};
+using MS0 = ModelShape<5, 9, 5, 9, true>;
+using MS1 = ModelShape<5, 9, 5, 9, false>;
+
+template <class MS>
+void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
+  ModelTables<MS> t;
+  memset(&t, 0, sizeof t);
+  auto fold = [](const double* c, int N, int K, float* ct, float* kct) {
+    for (int n = 0; n < N; ++n) {
+      double s = 0.0;
+      for (int k = 1; k < K; ++k) s += c[n * K + k];
+      for (int k = 0; k < K; ++k) {
+        double v = k == 0 ? c[n * K] + 0.5 * s : 0.5 * c[n * K + k];
+        ct[n * K + k] = (float)v;
+        if (kct) kct[n * K + k] = (float)(k * v);
+      }
+    }
+  };
+  fold(p->c_radial, MS::NR, MS::KR, &t.ctR[0][0], nullptr);
+  fold(p->c_angular, MS::NA, MS::KA, &t.ctA[0][0], &t.kctA[0][0]);
+  t.inv_rcR = (float)(1.0 / p->rc_radial);
+  t.inv_rcA = (float)(1.0 / p->rc_angular);
+  t.rcR2 = (float)(p->rc_radial * p->rc_radial);
+  t.rcA2 = (float)(p->rc_angular * p->rc_angular);
+  double zf = p->zbl_r_outer + 0.01;
+  t.zbl_flag_r2 = p->zbl_enabled ? (float)(zf * zf) : 0.0f;
+  t.b1 = (float)p->b1;
+  t.n_neurons = p->n_neurons;
+  h->tables.resize(sizeof t);
+  memcpy(h->tables.data(), &t, sizeof t);
+  h->smem_nn = sizeof(float) * ((size_t)p->n_neurons * MS::DPAD + 2 * p->n_neurons + MS::DPAD);
+}
+
+template <class MS>
+std::vector<float> build_nnw(const nepzbl_params* p) {
+  std::vector<float> w((size_t)p->n_neurons * MS::DPAD + 2 * p->n_neurons + MS::DPAD, 0.0f);
+  for (int m = 0; m < p->n_neurons; ++m)
+    for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
+  float* b0 = w.data() + (size_t)p->n_neurons * MS::DPAD;
+  float* w1 = b0 + p->n_neurons;
+  float* qs = w1 + p->n_neurons;
+  for (int m = 0; m < p->n_neurons; ++m) {
+    b0[m] = (float)p->b0[m];
+    w1[m] = (float)p->w1[m];
+  }
+  for (int v = 0; v < MS::D; ++v) qs[v] = (float)p->q_scaler[v];
+  return w;
+}
+
+inline int blocks(long long n, int b) { return (int)((n + b - 1) / b); }
+
+// ------------------------------------------------------------------ kernel sequences
+
+// S2 chain; every kernel exits immediately unless Scalars::do_rebuild is set.
+void enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types) {
+  const Carve& c = h->cv;
+  const int n = (int)h->n, npad = c.npad;
+  cudaStream_t st = h->stream;
+  BoxHost bh;
+  for (int a = 0; a < 3; ++a) {
+    bh.L[a] = h->box[4 * a];
+    bh.pbc[a] = h->pbc[a];
+  }
+  bh.rcs = h->p.rc_radial + h->p.skin;
+  bh.ncell_cap = c.ncell_cap;
+  float rr = (float)(bh.rcs * bh.rcs);
+  double ra = h->p.rc_angular + h->p.skin;
+  float ra2 = (float)(ra * ra);
+  k_rebuild_begin<<<1, 1, 0, st>>>(h->d_sc);
+  h->launches++;
+  if (!(h->pbc[0] && h->pbc[1] && h->pbc[2])) {
+    k_bounds<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, pos, !h->pbc[0], !h->pbc[1], !h->pbc[2]);
+    h->launches++;
+  }
+  k_boxmap<<<1, 1, 0, st>>>(h->d_sc, h->d_bm, bh);
+  k_zero_cells<<<blocks(c.ncell_cap + 1, 256), 256, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count),
+                                                           h->at<int>(c.cell_fill), c.ncell_cap);
+  k_bin<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, pos, types, h->at<int4>(c.xyzt_tmp),
+                                       h->at<int>(c.cell_of), h->at<int>(c.cell_count));
+  k_scan<<<1, 1024, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count), h->at<int>(c.cell_start));
+  k_place<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->at<int>(c.cell_of), h->at<int>(c.cell_start),
+                                         h->at<int>(c.cell_fill), h->at<int>(c.order));
+  k_sortcell<<<blocks(c.ncell_cap, 128), 128, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_start),
+                                                      h->at<int>(c.order));
+  k_permute<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->at<int>(c.order), h->at<int4>(c.xyzt_tmp),
+                                           h->at<int>(c.perm), h->at<int>(c.inv_perm),
+                                           h->at<int4>(c.xyzt), h->at<int4>(c.xyzt_build));
+  k_nbr<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
+                                       h->at<int>(c.cell_start), rr, ra2, h->p.cap_radial,
+                                       h->p.cap_angular, h->at<int>(c.nn_r), h->at<int>(c.nl_r),
+                                       h->at<int>(c.nn_a), h->at<int>(c.nl_a));
+  k_rev<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, n, npad, h->at<int>(c.nn_a), h->at<int>(c.nl_a),
+                                       h->at<unsigned char>(c.rev));
+  h->launches += 9;
+}
+
+// S3-S7 (+S5): outputs in the caller's order; any of energy/force/virial may be null.
+template <class MS>
+void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
+                    bool want_q) {
+  const Carve& c = h->cv;
+  const int n = (int)h->n, npad = c.npad;
+  cudaStream_t st = h->stream;
+  const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
+  k_radial<MS><<<blocks(n, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
+                                              h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
+                                              h->at<float>(c.q_radial), h->at<int>(c.zbl_list));
+  k_angular_nn<MS><<<blocks(n, 128), 128, h->smem_nn, st>>>(
+      h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_a), h->at<int>(c.nl_a), mt, h->d_nnw,
+      h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<float4>(c.dk), h->at<float4>(c.pforce),
+      want_q ? h->at<float>(c.q_desc) : nullptr);
+  if (virial)
+    k_force<MS, true><<<blocks(n, 128), 128, 0, st>>>(
+        h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
+        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<float4>(c.dk),
+        h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial);
+  else
+    k_force<MS, false><<<blocks(n, 128), 128, 0, st>>>(
+        h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
+        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<float4>(c.dk),
+        h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
+  h->launches += 3;
+  if (h->p.zbl_enabled) {
+    k_zbl<<<32, 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), n, npad, h->at<int4>(c.xyzt),
+                            h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp,
+                            energy, force, virial);
+    h->launches++;
+  }
+}
+
+void enqueue_eval(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
+                  bool want_q) {
+  if (h->shape == 0) enqueue_eval_t<MS0>(h, pos, energy, force, virial, want_q);
+  else enqueue_eval_t<MS1>(h, pos, energy, force, virial, want_q);
+}
+
+int read_scalars(nepzbl_handle* h) {
+  CU(cudaMemcpyAsync(h->h_sc, h->d_sc, sizeof(Scalars), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  CU(cudaGetLastError());
+  return NEPZBL_OK;
+}
+
+int check_device_flags(nepzbl_handle* h) {
+  const Scalars& s = *h->h_sc;
+  if (s.nonfinite) {
+    h->have_list = false;
+    return fail(h, NEPZBL_E_NONFINITE, "NaN/Inf in positions");
+  }
+  if (s.box_too_small) {
+    h->have_list = false;
+    return fail(h, NEPZBL_E_BOX_TOO_SMALL, "periodic box edge < 2*(rc_radial+skin)");
+  }
+  if (s.overflow_radial > h->p.cap_radial || s.overflow_angular > h->p.cap_angular) {
+    h->have_list = false;
+    return fail(h, NEPZBL_E_NEIGHBOR_OVERFLOW,
+                "neighbour list overflow: an atom needs %d radial (cap %d) / %d angular (cap %d) slots",
+                s.overflow_radial, h->p.cap_radial, s.overflow_angular, h->p.cap_angular);
+  }
+  return NEPZBL_OK;
+}
+
+int set_system(nepzbl_handle* h, long long n, const double box[9], const int32_t pbc[3], bool* changed) {
+  if (!h->ws) return fail(h, NEPZBL_E_WORKSPACE, "no workspace set");
+  if (n < 0 || n > h->n_cap) return fail(h, NEPZBL_E_WORKSPACE, "n = %lld exceeds workspace capacity %lld", n, h->n_cap);
+  if (!box || !pbc) return fail(h, NEPZBL_E_INVALID_ARG, "box/pbc is NULL");
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      if (a != b && box[3 * a + b] != 0.0)
+        return fail(h, NEPZBL_E_BOX_NOT_ORTHOGONAL, "only orthogonal boxes are supported");
+  double rcs = h->p.rc_radial + h->p.skin;
+  for (int a = 0; a < 3; ++a) {
+    if (!(box[4 * a] > 0.0) || !std::isfinite(box[4 * a])) return fail(h, NEPZBL_E_INVALID_ARG, "box edge %d is not positive", a);
+    if (pbc[a] && box[4 * a] < 2.0 * rcs)
+      return fail(h, NEPZBL_E_BOX_TOO_SMALL, "periodic edge %d = %g A < 2*(rc_radial+skin) = %g A", a, box[4 * a], 2.0 * rcs);
+  }
+  bool ch = !h->have_list || n != h->n;
+  for (int a = 0; a < 9; ++a) ch = ch || box[a] != h->box[a];
+  for (int a = 0; a < 3; ++a) ch = ch || (pbc[a] != 0) != (h->pbc[a] != 0);
+  h->n = n;
+  memcpy(h->box, box, sizeof h->box);
+  for (int a = 0; a < 3; ++a) h->pbc[a] = pbc[a] != 0;
+  *changed = ch;
+  return NEPZBL_OK;
+}
+
+__global__ void k_set_force_rebuild(Scalars* sc) { sc->force_rebuild = 1; }
+
+int eval_common(nepzbl_handle* h, long long n, const double* pos, const int32_t* types,
+                const double box[9], const int32_t pbc[3], double* energy, float* force, float* virial,
+                bool force_rebuild, bool want_q, bool do_eval) {
+  bool changed = false;
+  int rc = set_system(h, n, box, pbc, &changed);
+  if (rc) return rc;
+  if (n == 0) return NEPZBL_OK;
+  if (!pos) return fail(h, NEPZBL_E_INVALID_ARG, "pos is NULL");
+  const Carve& c = h->cv;
+  float hs = (float)(0.5 * h->p.skin);
+  if (changed || force_rebuild) {
+    k_set_force_rebuild<<<1, 1, 0, h->stream>>>(h->d_sc);
+  } else {
+    k_prep<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, h->d_bm, (int)n, pos, types,
+                                                  h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
+                                                  h->at<int4>(c.xyzt_build));
+  }
+  k_flag<<<1, 1, 0, h->stream>>>(h->d_sc, hs * hs);
+  h->launches += 2;
+  enqueue_rebuild(h, pos, types);
+  if (do_eval) enqueue_eval(h, pos, energy, force, virial, want_q);
+  rc = read_scalars(h);
+  if (rc) return rc;
+  rc = check_device_flags(h);
+  if (rc) return rc;
+  h->have_list = true;
+  return NEPZBL_OK;
+}
+
+}  // namespace
+
+// =============================================================================== C ABI
+
+extern "C" {
+
+int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl_handle** out) {
+  nepzbl_handle* h = nullptr;
+  if (!p || !out) return fail(h, NEPZBL_E_INVALID_ARG, "params/out is NULL");
+  *out = nullptr;
+  if (p->n_types != 1) return fail(h, NEPZBL_E_UNSUPPORTED, "this build supports n_types == 1 (got %d)", p->n_types);
+  if (p->l_max != 4) return fail(h, NEPZBL_E_UNSUPPORTED, "this build supports l_max == 4 (got %d)", p->l_max);
+  int shape = -1;
+  for (int k = 0; k < (int)(sizeof kShapes / sizeof kShapes[0]); ++k)
+    if (kShapes[k].nr == p->n_max_radial + 1 && kShapes[k].kr == p->basis_radial + 1 &&
+        kShapes[k].na == p->n_max_angular + 1 && kShapes[k].ka == p->basis_angular + 1 &&
+        kShapes[k].b4 == (p->has_4body != 0))
+      shape = k;
+  if (shape < 0)
+    return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d is not instantiated in this build",
+                p->n_max_radial, p->n_max_angular, p->basis_radial, p->basis_angular, p->has_4body);
+  if (p->n_neurons < 1 || p->n_neurons > 256) return fail(h, NEPZBL_E_INVALID_ARG, "n_neurons out of range");
+  if (p->cap_angular < 1 || p->cap_angular > 64 || p->cap_radial < 1 || p->cap_radial > 1024)
+    return fail(h, NEPZBL_E_INVALID_ARG, "cap_angular must be in 1..64, cap_radial in 1..1024");
+  if (!(p->rc_radial > 0) || !(p->rc_angular > 0) || p->rc_angular > p->rc_radial || p->skin < 0)
+    return fail(h, NEPZBL_E_INVALID_ARG, "need 0 < rc_angular <= rc_radial and skin >= 0");
+  if (p->zbl_enabled && (p->zbl_n_terms < 1 || p->zbl_n_terms > 4 || !(p->zbl_r_inner < p->zbl_r_outer) ||
+                         p->zbl_r_outer + 0.01 > p->rc_radial))
+    return fail(h, NEPZBL_E_INVALID_ARG, "bad ZBL parameters");
+  if (!p->c_radial || !p->c_angular || !p->q_scaler || !p->w0 || !p->b0 || !p->w1 || !p->atomic_number || !p->mass)
+    return fail(h, NEPZBL_E_INVALID_ARG, "a parameter array is NULL");
+
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev <= device || device < 0)
+    return fail(h, NEPZBL_E_CUDA, "no CUDA device %d (%s): this library has no CPU fallback", device,
+                e == cudaSuccess ? "device count too small" : cudaGetErrorString(e));
+  h = new nepzbl_handle();
+  h->p = *p;
+  h->p.c_radial = h->p.c_angular = h->p.q_scaler = h->p.w0 = h->p.b0 = h->p.w1 = nullptr;
+  h->p.atomic_number = h->p.mass = nullptr;
+  h->shape = shape;
+  h->device = device;
+  h->stream = (cudaStream_t)cuda_stream;
+  std::vector<float> nnw;
+  if (shape == 0) { build_tables<MS0>(h, p); nnw = build_nnw<MS0>(p); h->D = MS0::D; }
+  else { build_tables<MS1>(h, p); nnw = build_nnw<MS1>(p); h->D = MS1::D; }
+  ZblParams& z = h->zp;
+  memset(&z, 0, sizeof z);
+  z.r_inner = p->zbl_r_inner; z.r_outer = p->zbl_r_outer; z.n_terms = p->zbl_n_terms;
+  for (int k = 0; k < 4; ++k) { z.c[k] = p->zbl_c[k]; z.d[k] = p->zbl_d[k]; }
+  z.a_num = p->zbl_a_num; z.a_pow = p->zbl_a_pow; z.coulomb_k = p->coulomb_k;
+  for (int t = 0; t < p->n_types && t < 8; ++t) z.Z[t] = p->atomic_number[t];
+  double zf = p->zbl_r_outer + 0.01;
+  z.filter_r2 = (float)(zf * zf);
+
+  auto die = [&](const char* what, cudaError_t ce) {
+    std::string msg = std::string(what) + ": " + cudaGetErrorString(ce);
+    nep_zbl_destroy(h);
+    g_create_error = msg;
+    return NEPZBL_E_CUDA;
+  };
+  cudaError_t ce;
+  if ((ce = cudaSetDevice(device)) != cudaSuccess) return die("cudaSetDevice", ce);
+  if ((ce = cudaMalloc(&h->d_sc, sizeof(Scalars))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_bm, sizeof(BoxMap))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_nnw, nnw.size() * sizeof(float))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_mass, 8 * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_inv_mass, 8 * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_trace, kTraceRing * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_esum, 2 * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMallocHost(&h->h_sc, sizeof(Scalars))) != cudaSuccess) return die("cudaMallocHost", ce);
+  if ((ce = cudaMallocHost(&h->h_trace, kTraceRing * sizeof(double))) != cudaSuccess) return die("cudaMallocHost", ce);
+  if ((ce = cudaMallocHost(&h->h_esum, 2 * sizeof(double))) != cudaSuccess) return die("cudaMallocHost", ce);
+  double mass[8] = {0}, inv_mass[8] = {0};
+  for (int t = 0; t < p->n_types && t < 8; ++t) {
+    mass[t] = p->mass[t];
+    inv_mass[t] = 1.0 / (p->mass[t] * NEPZBL_AMU_A2_FS2_TO_EV);
+  }
+  if ((ce = cudaMemsetAsync(h->d_sc, 0, sizeof(Scalars), h->stream)) != cudaSuccess) return die("cudaMemset", ce);
+  if ((ce = cudaMemsetAsync(h->d_bm, 0, sizeof(BoxMap), h->stream)) != cudaSuccess) return die("cudaMemset", ce);
+  if ((ce = cudaMemcpyAsync(h->d_nnw, nnw.data(), nnw.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
+  if ((ce = cudaMemcpyAsync(h->d_mass, mass, sizeof mass, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
+  if ((ce = cudaMemcpyAsync(h->d_inv_mass, inv_mass, sizeof inv_mass, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
+  if ((ce = cudaStreamSynchronize(h->stream)) != cudaSuccess) return die("cudaStreamSynchronize", ce);
+  *out = h;
+  return NEPZBL_OK;
+}
+
+void nep_zbl_destroy(nepzbl_handle* h) {
+  if (!h) return;
+  cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
+  cudaFree(h->d_trace); cudaFree(h->d_esum);
+  cudaFreeHost(h->h_sc); cudaFreeHost(h->h_trace); cudaFreeHost(h->h_esum);
+  delete h;
+}
+
+const char* nep_zbl_last_error(const nepzbl_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int nep_zbl_descriptor_dim(const nepzbl_handle* h) { return h ? h->D : 0; }
+
+size_t nep_zbl_workspace_bytes(const nepzbl_handle* h, int64_t n_atoms) {
+  if (!h || n_atoms < 0) return 0;
+  return carve(h->p, h->D, n_atoms).total;
+}
+
+int nep_zbl_set_workspace(nepzbl_handle* h, void* dev_ptr, size_t bytes, int64_t n_atoms) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!dev_ptr || n_atoms < 0 || n_atoms > 2000000000ll) return fail(h, NEPZBL_E_INVALID_ARG, "bad workspace arguments");
+  if (((uintptr_t)dev_ptr & 255) != 0) return fail(h, NEPZBL_E_WORKSPACE, "workspace must be 256-byte aligned");
+  Carve c = carve(h->p, h->D, n_atoms);
+  if (bytes < c.total) return fail(h, NEPZBL_E_WORKSPACE, "workspace too small: %zu < %zu bytes", bytes, c.total);
+  h->ws = (char*)dev_ptr;
+  h->ws_bytes = bytes;
+  h->n_cap = n_atoms;
+  h->cv = c;
+  h->have_list = false;
+  h->md_ready = false;
+  return NEPZBL_OK;
+}
+
+int neighbor_build(nepzbl_handle* h, int64_t n, const double* pos, const int32_t* types,
+                   const double box[9], const int32_t pbc[3]) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  return eval_common(h, n, pos, types, box, pbc, nullptr, nullptr, nullptr, true, false, false);
+}
+
+int neighbor_get(nepzbl_handle* h, int which, int32_t* nn, int32_t* nl) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->have_list) return fail(h, NEPZBL_E_STATE, "no neighbour list has been built");
+  if (!nn || !nl || (which != 0 && which != 1)) return fail(h, NEPZBL_E_INVALID_ARG, "bad neighbor_get arguments");
+  const Carve& c = h->cv;
+  if (h->n > 0) {
+    k_export_list<<<blocks(h->n, 128), 128, 0, h->stream>>>(
+        (int)h->n, c.npad, which ? h->p.cap_angular : h->p.cap_radial, h->at<int>(c.perm),
+        h->at<int>(which ? c.nn_a : c.nn_r), h->at<int>(which ? c.nl_a : c.nl_r), nn, nl);
+    h->launches++;
+  }
+  CU(cudaStreamSynchronize(h->stream));
+  CU(cudaGetLastError());
+  return NEPZBL_OK;
+}
+
+int nep_zbl_compute(nepzbl_handle* h, int64_t n, const double* pos, const int32_t* types,
+                    const double box[9], const int32_t pbc[3], double* energy, float* force,
+                    float* virial) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  return eval_common(h, n, pos, types, box, pbc, energy, force, virial, false, true, true);
+}
+
+int nep_zbl_compute_host(nepzbl_handle* h, int64_t n, const double* pos, const int32_t* types,
+                         const double box[9], const int32_t pbc[3], double* energy, float* force,
+                         float* virial) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->ws) return fail(h, NEPZBL_E_WORKSPACE, "no workspace set");
+  if (n < 0 || n > h->n_cap) return fail(h, NEPZBL_E_WORKSPACE, "n exceeds workspace capacity");
+  if (n == 0) return NEPZBL_OK;
+  if (!pos) return fail(h, NEPZBL_E_INVALID_ARG, "pos is NULL");
+  const Carve& c = h->cv;
+  double* dpos = h->at<double>(c.st_pos);
+  int32_t* dtyp = types ? h->at<int32_t>(c.st_types) : nullptr;
+  CU(cudaMemcpyAsync(dpos, pos, 24 * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+  if (types) CU(cudaMemcpyAsync(dtyp, types, 4 * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+  double* de = energy ? h->at<double>(c.st_e) : nullptr;
+  float* df = force ? h->at<float>(c.st_f) : nullptr;
+  float* dw = virial ? h->at<float>(c.st_w) : nullptr;
+  int rc = eval_common(h, n, dpos, dtyp, box, pbc, de, df, dw, false, true, true);
+  if (rc) return rc;
+  if (energy) CU(cudaMemcpyAsync(energy, de, 8 * (size_t)n, cudaMemcpyDeviceToHost, h->stream));
+  if (force) CU(cudaMemcpyAsync(force, df, 12 * (size_t)n, cudaMemcpyDeviceToHost, h->stream));
+  if (virial) CU(cudaMemcpyAsync(virial, dw, 36 * (size_t)n, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return NEPZBL_OK;
+}
+
+int nep_zbl_get_descriptors(nepzbl_handle* h, float* q) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->have_list) return fail(h, NEPZBL_E_STATE, "no evaluation has been made");
+  if (!q) return fail(h, NEPZBL_E_INVALID_ARG, "q is NULL");
+  const Carve& c = h->cv;
+  if (h->n > 0) {
+    k_export_q<<<blocks(h->n, 128), 128, 0, h->stream>>>((int)h->n, c.npad, h->D, h->at<int>(c.perm),
+                                                        h->at<float>(c.q_desc), q);
+    h->launches++;
+  }
+  CU(cudaStreamSynchronize(h->stream));
+  CU(cudaGetLastError());
+  return NEPZBL_OK;
+}
+
+// ---------------------------------------------------------------------------------- MD
+
+int md_init(nepzbl_handle* h, int64_t n, double* pos, double* vel, const int32_t* types,
+            const double box[9], const int32_t pbc[3]) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  h->md_ready = false;
+  if (!pos || !vel) return fail(h, NEPZBL_E_INVALID_ARG, "pos/vel is NULL");
+  bool changed;
+  int rc = set_system(h, n, box, pbc, &changed);
+  if (rc) return rc;
+  if (n == 0) return fail(h, NEPZBL_E_INVALID_ARG, "md_init needs n > 0");
+  const Carve& c = h->cv;
+  CU(cudaMemsetAsync(h->d_sc, 0, sizeof(Scalars), h->stream));
+  h->md_pos = pos;
+  h->md_vel = vel;
+  h->md_types = types;
+  h->parity = 0;
+  h->md_steps = 0;
+  rc = eval_common(h, n, pos, types, box, pbc, h->at<double>(c.md_energy), h->at<float>(c.md_force),
+                   nullptr, true, false, true);
+  if (rc) return rc;
+  k_kick<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, 0, (int)n, vel, h->at<float>(c.md_force), types,
+                                                h->d_inv_mass, 0);
+  h->launches++;
+  CU(cudaStreamSynchronize(h->stream));
+  CU(cudaGetLastError());
+  h->md_ready = true;
+  return NEPZBL_OK;
+}
+
+static void enqueue_md_step(nepzbl_handle* h, double dt_max, double max_disp, int trace_idx) {
+  const Carve& c = h->cv;
+  const int n = (int)h->n;
+  cudaStream_t st = h->stream;
+  float hs = (float)(0.5 * h->p.skin);
+  k_dt<<<1, 1, 0, st>>>(h->d_sc, h->parity, dt_max, max_disp, trace_idx >= 0 ? h->d_trace : nullptr,
+                        trace_idx >= 0 ? trace_idx : 0);
+  k_kick_drift<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, h->md_pos, h->md_vel,
+                                              h->at<float>(c.md_force), h->md_types, h->d_inv_mass,
+                                              h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
+                                              h->at<int4>(c.xyzt_build));
+  k_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs);
+  h->launches += 3;
+  enqueue_rebuild(h, h->md_pos, h->md_types);
+  enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false);
+  k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->parity ^ 1, n, h->md_vel, h->at<float>(c.md_force),
+                                        h->md_types, h->d_inv_mass, 1);
+  h->launches++;
+  h->parity ^= 1;
+  h->md_steps++;
+}
+
+int md_step(nepzbl_handle* h, double dt_max, double max_displacement, double* dt_used, int32_t* rebuilt) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_step before md_init");
+  if (!(dt_max > 0) || !(max_displacement > 0)) return fail(h, NEPZBL_E_INVALID_ARG, "dt_max and max_displacement must be > 0");
+  enqueue_md_step(h, dt_max, max_displacement, -1);
+  int rc = read_scalars(h);
+  if (rc) return rc;
+  if (dt_used) *dt_used = h->h_sc->dt;
+  if (rebuilt) *rebuilt = h->h_sc->do_rebuild;
+  rc = check_device_flags(h);
+  if (rc) h->md_ready = false;
+  return rc;
+}
+
+int md_run(nepzbl_handle* h, int64_t n_steps, double dt_max, double max_displacement, double* dt_trace,
+           int64_t* n_rebuilds) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_run before md_init");
+  if (!(dt_max > 0) || !(max_displacement > 0) || n_steps < 0) return fail(h, NEPZBL_E_INVALID_ARG, "bad md_run arguments");
+  int rc = read_scalars(h);
+  if (rc) return rc;
+  long long reb0 = h->h_sc->n_rebuilds;
+  for (int64_t done = 0; done < n_steps;) {
+    int chunk = (int)std::min<int64_t>(kTraceRing, n_steps - done);
+    for (int k = 0; k < chunk; ++k) enqueue_md_step(h, dt_max, max_displacement, k);
+    if (dt_trace) CU(cudaMemcpyAsync(h->h_trace, h->d_trace, chunk * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    rc = read_scalars(h);
+    if (rc) return rc;
+    if (dt_trace) memcpy(dt_trace + done, h->h_trace, chunk * sizeof(double));
+    rc = check_device_flags(h);
+    if (rc) { h->md_ready = false; return rc; }
+    done += chunk;
+  }
+  if (n_rebuilds) *n_rebuilds = h->h_sc->n_rebuilds - reb0;
+  return NEPZBL_OK;
+}
+
+int md_step_host(nepzbl_handle* h, double* pos, double* vel, double dt_max, double max_displacement,
+                 double* dt_used, int32_t* rebuilt) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_step_host before md_init");
+  if (!pos || !vel) return fail(h, NEPZBL_E_INVALID_ARG, "pos/vel is NULL");
+  size_t b = 24 * (size_t)h->n;
+  CU(cudaMemcpyAsync(h->md_pos, pos, b, cudaMemcpyHostToDevice, h->stream));
+  CU(cudaMemcpyAsync(h->md_vel, vel, b, cudaMemcpyHostToDevice, h->stream));
+  int rc = md_step(h, dt_max, max_displacement, dt_used, rebuilt);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(pos, h->md_pos, b, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaMemcpyAsync(vel, h->md_vel, b, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return NEPZBL_OK;
+}
+
+int md_energies(nepzbl_handle* h, double* e_pot, double* e_kin) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_energies before md_init");
+  const Carve& c = h->cv;
+  int nb = (int)std::min<long long>(1024, (h->n + 255) / 256);
+  k_energy_partial<<<nb, 256, 0, h->stream>>>((int)h->n, h->md_vel, h->at<double>(c.md_energy), h->md_types,
+                                              h->d_mass, h->at<double>(c.partial));
+  k_energy_final<<<1, 256, 0, h->stream>>>(nb, h->at<double>(c.partial), h->d_esum);
+  h->launches += 2;
+  CU(cudaMemcpyAsync(h->h_esum, h->d_esum, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  CU(cudaGetLastError());
+  if (e_pot) *e_pot = h->h_esum[0];
+  if (e_kin) *e_kin = h->h_esum[1];
+  return NEPZBL_OK;
+}
+
+int md_get_forces(nepzbl_handle* h, float* force, double* energy) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_get_forces before md_init");
+  const Carve& c = h->cv;
+  if (force) CU(cudaMemcpyAsync(force, h->at<float>(c.md_force), 12 * (size_t)h->n, cudaMemcpyDeviceToDevice, h->stream));
+  if (energy) CU(cudaMemcpyAsync(energy, h->at<double>(c.md_energy), 8 * (size_t)h->n, cudaMemcpyDeviceToDevice, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return NEPZBL_OK;
+}
+
+int md_get_counters(nepzbl_handle* h, int64_t* n_steps, int64_t* n_rebuilds, int64_t* n_zbl_atoms) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_get_counters before md_init");
+  int rc = read_scalars(h);
+  if (rc) return rc;
+  if (n_steps) *n_steps = h->h_sc->n_steps;
+  if (n_rebuilds) *n_rebuilds = h->h_sc->n_rebuilds;
+  if (n_zbl_atoms) *n_zbl_atoms = h->h_sc->zbl_count;
+  return NEPZBL_OK;
+}
+
+int64_t nep_zbl_launch_count(const nepzbl_handle* h) { return h ? h->launches : 0; }
+
+}  // extern "C"

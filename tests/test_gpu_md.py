@@ -1,0 +1,128 @@
+"""GPU MD tests: md_step / md_run against the oracle's velocity-Verlet."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2305_08140_b200 import workloads as wl
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nb():
+    from paper_2305_08140_b200 import binding
+    assert torch.cuda.is_available()
+    return binding
+
+
+def _md(nb, w, vel=None):
+    g = nb.NepZbl(w.model, w.n)
+    pos = torch.from_numpy(w.pos.copy()).cuda()
+    v = torch.from_numpy((w.vel if vel is None else vel).copy()).cuda()
+    types = torch.from_numpy(w.types).cuda()
+    g.md_init(pos, v, types, w.box, w.pbc)
+    return g, pos, v
+
+
+def _min_image(d, box):
+    L = box[[0, 4, 8]][:, None]
+    return d - L * np.round(d / L)
+
+
+def test_initial_forces_and_energies(nb):
+    w = wl.thermal_bulk(6, seed=2, sigma_pos=0.05)
+    g, pos, vel = _md(nb, w)
+    ref = oracle.compute(oracle.Params(w.model), w.pos, w.types, w.box, w.pbc)
+    f, e = g.md_get_forces()
+    parity_r = parity.compare(e.cpu().numpy(), f.cpu().numpy(), None, ref, label="md_init")
+    assert max(parity_r.values()) <= 1.0
+    ep, ek = g.md_energies()
+    assert ep == pytest.approx(ref.energy.sum(), abs=1e-5 * w.n)
+    assert ek == pytest.approx(0.5 * wl.W_MASS * wl.AMU_A2_FS2_TO_EV * (w.vel ** 2).sum(), rel=1e-12)
+
+
+def test_trajectory_follows_oracle_step_by_step(nb):
+    w = wl.thermal_bulk(6, seed=3, sigma_pos=0.03)
+    P = oracle.Params(w.model)
+    n = 60
+    opos, ovel, odt, oep, oek = oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, n, 1.0, np.inf)
+    g, pos, vel = _md(nb, w)
+    e0 = sum(g.md_energies())
+    for s in range(n):
+        dt, rebuilt = g.md_step(1.0, float("inf"))
+        assert dt == 1.0
+    d = _min_image(pos.cpu().numpy() - opos, w.box)
+    print("max |dx| after", n, "steps:", np.abs(d).max(), " max|dv|:", np.abs(vel.cpu().numpy() - ovel).max())
+    assert np.abs(d).max() < 5e-6                       # fp32 forces: ~1e-7 relative per step
+    assert np.abs(vel.cpu().numpy() - ovel).max() < 5e-7
+    ep, ek = g.md_energies()
+    assert ep == pytest.approx(oep[-1], abs=2e-5 * w.n)
+    assert ek == pytest.approx(oek[-1], rel=1e-4)
+    assert abs(ep + ek - e0) / w.n < 1e-5               # energy conservation over 60 fs
+
+
+def test_md_run_equals_repeated_md_step_bitwise(nb):
+    w = wl.thermal_bulk(6, seed=4, sigma_pos=0.03)
+    g1, p1, v1 = _md(nb, w)
+    g2, p2, v2 = _md(nb, w)
+    dts = [g1.md_step(1.0, 0.05)[0] for _ in range(25)]
+    tr, nreb = g2.md_run(25, 1.0, 0.05, want_trace=True)
+    assert np.array_equal(np.array(dts), tr)
+    assert torch.equal(p1, p2) and torch.equal(v1, v2)
+
+
+def test_adaptive_time_step_and_rebuilds_with_a_knock_on(nb):
+    # 1 keV knock-on in 8^3 cells: dt = 0.015/v_max, displacement per step <= 0.015 A, list rebuilt as it
+    # travels; compare with the oracle over the first steps and check invariants afterwards.
+    w = wl.bulk_cascade(8, 1000.0, seed=5, n_steps=0, name="pka")
+    P = oracle.Params(w.model)
+    n = 40
+    opos, ovel, odt, oep, oek = oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, n, 1.0, 0.015)
+    g, pos, vel = _md(nb, w)
+    prev = pos.cpu().numpy().copy()
+    nreb = 0
+    for s in range(n):
+        dt, rebuilt = g.md_step(1.0, 0.015)
+        nreb += rebuilt
+        assert dt == pytest.approx(odt[s], rel=1e-6)
+        assert dt <= 1.0
+        cur = pos.cpu().numpy()
+        step = np.sqrt((_min_image(cur - prev, w.box) ** 2).sum(axis=0)).max()
+        assert step <= 0.015 * (1 + 1e-3)
+        prev = cur.copy()
+    d = _min_image(pos.cpu().numpy() - opos, w.box)
+    assert np.abs(d).max() < 2e-5
+    # keep going: the knock-on crosses > skin/2, so the list must be rebuilt at least once
+    e0 = sum(g.md_energies())
+    tr, nr = g.md_run(400, 1.0, 0.015, want_trace=True)
+    assert nreb + nr >= 1
+    assert np.all(tr <= 1.0) and np.all(tr > 0)
+    e1 = sum(g.md_energies())
+    print("PKA run: dE/N =", (e1 - e0) / w.n, " rebuilds:", nreb + nr, " zbl atoms:", g.md_get_counters()[2])
+    assert abs(e1 - e0) < 0.05                           # total energy (1 keV scale) conserved to 5e-5 relative
+    # final-state parity against the oracle at the GPU's own positions
+    f, e = g.md_get_forces()
+    ref = oracle.compute(P, pos.cpu().numpy(), w.types, w.box, w.pbc)
+    r = parity.compare(e.cpu().numpy(), f.cpu().numpy(), None, ref, label="after cascade")
+    assert max(r.values()) <= 1.0
+
+
+def test_md_step_host_round_trip(nb):
+    w = wl.thermal_bulk(5, seed=6, sigma_pos=0.03)
+    g1, p1, v1 = _md(nb, w)
+    g2, p2, v2 = _md(nb, w)
+    hp = torch.from_numpy(w.pos.copy()).pin_memory(); hv = torch.from_numpy(w.vel.copy()).pin_memory()
+    for _ in range(5):
+        g1.md_step(1.0, float("inf"))
+        g2.md_step_host(hp, hv, 1.0, float("inf"))
+    assert np.array_equal(hp.numpy(), p1.cpu().numpy()) and np.array_equal(hv.numpy(), v1.cpu().numpy())
+
+
+def test_state_errors(nb):
+    w = wl.thermal_bulk(5, seed=6)
+    g = nb.NepZbl(w.model, w.n)
+    with pytest.raises(nb.NepZblError) as ei:
+        g.md_step(1.0, 0.015)
+    assert ei.value.code == -9
