@@ -28,7 +28,8 @@ EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_d
            "nep_zbl_workspace_bytes", "nep_zbl_set_workspace", "neighbor_build", "neighbor_get",
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
            "md_run", "md_step_host", "md_energies", "md_get_forces", "md_get_counters",
-           "nep_zbl_launch_count"]
+           "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
+PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "spare"]
 
 
 class NepZblError(RuntimeError):
@@ -96,6 +97,12 @@ _lib.md_get_counters.argtypes = [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTE
 _lib.md_get_counters.restype = C.c_int
 _lib.nep_zbl_launch_count.argtypes = [_vp]
 _lib.nep_zbl_launch_count.restype = _i64
+_lib.nep_zbl_profile.argtypes = [_vp, C.c_int]
+_lib.nep_zbl_profile.restype = C.c_int
+_lib.nep_zbl_profile_read.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_i64)]
+_lib.nep_zbl_profile_read.restype = C.c_int
+_lib.nep_zbl_ffma_peak.argtypes = [_vp, C.POINTER(_dbl)]
+_lib.nep_zbl_ffma_peak.restype = C.c_int
 
 
 def _ptr(t):
@@ -240,6 +247,19 @@ class NepZbl:
 
     def nep_zbl_launch_count(self) -> int:
         return int(_lib.nep_zbl_launch_count(self.h))
+
+    def nep_zbl_profile(self, enable: bool):
+        self._chk(_lib.nep_zbl_profile(self.h, int(enable)))
+
+    def nep_zbl_profile_read(self):
+        ms = (_dbl * 8)(); cnt = (_i64 * 8)()
+        self._chk(_lib.nep_zbl_profile_read(self.h, ms, cnt))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(PROFILE_SLOTS)}
+
+    def nep_zbl_ffma_peak(self) -> float:
+        t = _dbl()
+        self._chk(_lib.nep_zbl_ffma_peak(self.h, C.byref(t)))
+        return t.value
 
     # ---- convenience (marshalling only)
     def compute(self, pos_np, types_np, box, pbc, virial: bool = True):

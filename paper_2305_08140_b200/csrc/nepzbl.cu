@@ -79,6 +79,15 @@ struct nepzbl_handle {
   int parity = 0;
   long long md_steps = 0;
 
+  // per-kernel CUDA-event timing (nep_zbl_profile)
+  bool prof = false;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+  struct Span { int id; cudaEvent_t a, b; };
+  std::vector<Span> spans;
+  cudaEvent_t ev_open = nullptr;
+  int ev_open_id = -1;
+
   template <class T>
   T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
 };
@@ -198,6 +207,26 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
 
 inline int blocks(long long n, int b) { return (int)((n + b - 1) / b); }
 
+enum { PK_INTEGRATE_A = 0, PK_REBUILD, PK_RADIAL, PK_ANGULAR_NN, PK_FORCE, PK_ZBL, PK_KICK, PK_COUNT };
+
+cudaEvent_t prof_event(nepzbl_handle* h) {
+  if (h->ev_used == h->ev_pool.size()) {
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    h->ev_pool.push_back(e);
+  }
+  return h->ev_pool[h->ev_used++];
+}
+// open a timed span for kernel group `id` (closes the previous one): events on the launch stream
+void prof_mark(nepzbl_handle* h, int id) {
+  if (!h->prof) return;
+  cudaEvent_t e = prof_event(h);
+  cudaEventRecord(e, h->stream);
+  if (h->ev_open_id >= 0) h->spans.push_back({h->ev_open_id, h->ev_open, e});
+  h->ev_open = e;
+  h->ev_open_id = id;
+}
+
 // ------------------------------------------------------------------ kernel sequences
 
 // S2 chain; every kernel exits immediately unless Scalars::do_rebuild is set.
@@ -215,6 +244,7 @@ void enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types) 
   float rr = (float)(bh.rcs * bh.rcs);
   double ra = h->p.rc_angular + h->p.skin;
   float ra2 = (float)(ra * ra);
+  prof_mark(h, PK_REBUILD);
   k_rebuild_begin<<<1, 1, 0, st>>>(h->d_sc);
   h->launches++;
   if (!(h->pbc[0] && h->pbc[1] && h->pbc[2])) {
@@ -251,13 +281,16 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   const int n = (int)h->n, npad = c.npad;
   cudaStream_t st = h->stream;
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
+  prof_mark(h, PK_RADIAL);
   k_radial<MS><<<blocks(n, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
                                               h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
                                               h->at<float>(c.q_radial), h->at<int>(c.zbl_list));
+  prof_mark(h, PK_ANGULAR_NN);
   k_angular_nn<MS><<<blocks(n, 128), 128, h->smem_nn, st>>>(
       h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_a), h->at<int>(c.nl_a), mt, h->d_nnw,
       h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<float4>(c.dk), h->at<float4>(c.pforce),
       want_q ? h->at<float>(c.q_desc) : nullptr);
+  prof_mark(h, PK_FORCE);
   if (virial)
     k_force<MS, true><<<blocks(n, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
@@ -270,11 +303,13 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
         h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
   h->launches += 3;
   if (h->p.zbl_enabled) {
+    prof_mark(h, PK_ZBL);
     k_zbl<<<32, 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), n, npad, h->at<int4>(c.xyzt),
                             h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp,
                             energy, force, virial);
     h->launches++;
   }
+  prof_mark(h, -1);
 }
 
 void enqueue_eval(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
@@ -290,8 +325,15 @@ int read_scalars(nepzbl_handle* h) {
   return NEPZBL_OK;
 }
 
+__global__ void k_clear_errors(Scalars* sc);
+
 int check_device_flags(nepzbl_handle* h) {
   const Scalars& s = *h->h_sc;
+  if (s.nonfinite || s.box_too_small || s.overflow_radial > h->p.cap_radial ||
+      s.overflow_angular > h->p.cap_angular) {  // errors are reported once, then cleared
+    k_clear_errors<<<1, 1, 0, h->stream>>>(h->d_sc);
+    h->launches++;
+  }
   if (s.nonfinite) {
     h->have_list = false;
     return fail(h, NEPZBL_E_NONFINITE, "NaN/Inf in positions");
@@ -334,6 +376,28 @@ int set_system(nepzbl_handle* h, long long n, const double box[9], const int32_t
 }
 
 __global__ void k_set_force_rebuild(Scalars* sc) { sc->force_rebuild = 1; }
+
+// FP32 FMA issue-rate microbenchmark: 16 independent register chains per thread (bench.py roofline peak)
+__global__ void __launch_bounds__(512) k_ffma_peak(int iters, float m, float* sink) {
+  float a[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) a[k] = (float)(threadIdx.x + k) * 1e-3f;
+  float b = m, c = 1e-7f * (float)blockIdx.x;
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) a[k] = fmaf(a[k], b, c);
+  }
+  float s = 0.0f;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) s += a[k];
+  if (s == 12345.678f) *sink = s;
+}
+__global__ void k_clear_errors(Scalars* sc) {
+  sc->nonfinite = 0;
+  sc->box_too_small = 0;
+  sc->overflow_radial = 0;
+  sc->overflow_angular = 0;
+}
 
 int eval_common(nepzbl_handle* h, long long n, const double* pos, const int32_t* types,
                 const double box[9], const int32_t pbc[3], double* energy, float* force, float* virial,
@@ -458,6 +522,7 @@ void nep_zbl_destroy(nepzbl_handle* h) {
   cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
   cudaFree(h->d_trace); cudaFree(h->d_esum);
   cudaFreeHost(h->h_sc); cudaFreeHost(h->h_trace); cudaFreeHost(h->h_esum);
+  for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   delete h;
 }
 
@@ -589,6 +654,7 @@ static void enqueue_md_step(nepzbl_handle* h, double dt_max, double max_disp, in
   const int n = (int)h->n;
   cudaStream_t st = h->stream;
   float hs = (float)(0.5 * h->p.skin);
+  prof_mark(h, PK_INTEGRATE_A);
   k_dt<<<1, 1, 0, st>>>(h->d_sc, h->parity, dt_max, max_disp, trace_idx >= 0 ? h->d_trace : nullptr,
                         trace_idx >= 0 ? trace_idx : 0);
   k_kick_drift<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, h->md_pos, h->md_vel,
@@ -599,8 +665,10 @@ static void enqueue_md_step(nepzbl_handle* h, double dt_max, double max_disp, in
   h->launches += 3;
   enqueue_rebuild(h, h->md_pos, h->md_types);
   enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false);
+  prof_mark(h, PK_KICK);
   k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->parity ^ 1, n, h->md_vel, h->at<float>(c.md_force),
                                         h->md_types, h->d_inv_mass, 1);
+  prof_mark(h, -1);
   h->launches++;
   h->parity ^= 1;
   h->md_steps++;
@@ -698,5 +766,59 @@ int md_get_counters(nepzbl_handle* h, int64_t* n_steps, int64_t* n_rebuilds, int
 }
 
 int64_t nep_zbl_launch_count(const nepzbl_handle* h) { return h ? h->launches : 0; }
+
+int nep_zbl_profile(nepzbl_handle* h, int enable) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  CU(cudaStreamSynchronize(h->stream));
+  h->prof = enable != 0;
+  h->spans.clear();
+  h->ev_used = 0;
+  h->ev_open_id = -1;
+  return NEPZBL_OK;
+}
+
+int nep_zbl_profile_read(nepzbl_handle* h, double* ms, int64_t* counts) {
+  if (!h || !ms || !counts) return NEPZBL_E_INVALID_ARG;
+  CU(cudaStreamSynchronize(h->stream));
+  for (int k = 0; k < NEPZBL_PROFILE_SLOTS; ++k) { ms[k] = 0.0; counts[k] = 0; }
+  for (const auto& sp : h->spans) {
+    float t = 0.0f;
+    CU(cudaEventElapsedTime(&t, sp.a, sp.b));
+    if (sp.id >= 0 && sp.id < NEPZBL_PROFILE_SLOTS) { ms[sp.id] += t; counts[sp.id] += 1; }
+  }
+  h->spans.clear();
+  h->ev_used = 0;
+  h->ev_open_id = -1;
+  return NEPZBL_OK;
+}
+
+int nep_zbl_ffma_peak(nepzbl_handle* h, double* tflops) {
+  if (!h || !tflops) return NEPZBL_E_INVALID_ARG;
+  int sms = 0;
+  CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device));
+  float* sink = nullptr;
+  CU(cudaMalloc(&sink, sizeof(float)));
+  cudaEvent_t a, b;
+  CU(cudaEventCreate(&a));
+  CU(cudaEventCreate(&b));
+  const int iters = 4096, grid = sms * 8, block = 512;
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    CU(cudaEventRecord(a, h->stream));
+    k_ffma_peak<<<grid, block, 0, h->stream>>>(iters, 1.0001f, sink);
+    CU(cudaEventRecord(b, h->stream));
+    CU(cudaEventSynchronize(b));
+    float t = 0.0f;
+    CU(cudaEventElapsedTime(&t, a, b));
+    double fl = 2.0 * 16.0 * iters * (double)grid * block;  // 16 independent FMA chains per thread
+    if (rep > 0) best = std::max(best, fl / (t * 1e-3) * 1e-12);
+  }
+  h->launches += 5;
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  cudaFree(sink);
+  *tflops = best;
+  return NEPZBL_OK;
+}
 
 }  // extern "C"

@@ -60,7 +60,9 @@ def test_trajectory_follows_oracle_step_by_step(nb):
     ep, ek = g.md_energies()
     assert ep == pytest.approx(oep[-1], abs=2e-5 * w.n)
     assert ek == pytest.approx(oek[-1], rel=1e-4)
-    assert abs(ep + ek - e0) / w.n < 1e-5               # energy conservation over 60 fs
+    # Verlet's own error at dt = 1 fs with 0.03 A displacements is ~7e-5 eV/atom (oracle: the same)
+    assert abs(ep + ek - e0) / w.n < 2e-4
+    assert (ep + ek - e0) == pytest.approx(oep[-1] + oek[-1] - oep[0] - oek[0], abs=1e-5 * w.n)
 
 
 def test_md_run_equals_repeated_md_step_bitwise(nb):
@@ -78,8 +80,9 @@ def test_adaptive_time_step_and_rebuilds_with_a_knock_on(nb):
     # travels; compare with the oracle over the first steps and check invariants afterwards.
     w = wl.bulk_cascade(8, 1000.0, seed=5, n_steps=0, name="pka")
     P = oracle.Params(w.model)
-    n = 40
+    n, n2 = 40, 400
     opos, ovel, odt, oep, oek = oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, n, 1.0, 0.015)
+    _, _, odt2, oep2, oek2 = oracle.md_run(P, opos, ovel, w.types, w.box, w.pbc, n2, 1.0, 0.015)
     g, pos, vel = _md(nb, w)
     prev = pos.cpu().numpy().copy()
     nreb = 0
@@ -96,12 +99,16 @@ def test_adaptive_time_step_and_rebuilds_with_a_knock_on(nb):
     assert np.abs(d).max() < 2e-5
     # keep going: the knock-on crosses > skin/2, so the list must be rebuilt at least once
     e0 = sum(g.md_energies())
-    tr, nr = g.md_run(400, 1.0, 0.015, want_trace=True)
+    tr, nr = g.md_run(n2, 1.0, 0.015, want_trace=True)
     assert nreb + nr >= 1
     assert np.all(tr <= 1.0) and np.all(tr > 0)
     e1 = sum(g.md_energies())
-    print("PKA run: dE/N =", (e1 - e0) / w.n, " rebuilds:", nreb + nr, " zbl atoms:", g.md_get_counters()[2])
-    assert abs(e1 - e0) < 0.05                           # total energy (1 keV scale) conserved to 5e-5 relative
+    print("PKA run: dE =", e1 - e0, " oracle dE =", oep2[-1] + oek2[-1] - oep2[0] - oek2[0],
+          " rebuilds:", nreb + nr, " zbl atoms:", g.md_get_counters()[2])
+    # Verlet's own integration error at 0.015 A/step through a hard collision is ~1 eV of 1 keV for the
+    # oracle too; the GPU must reproduce the oracle's energy trace, not beat it
+    assert (e1 - e0) == pytest.approx(oep2[-1] + oek2[-1] - oep2[0] - oek2[0], abs=2e-2)
+    assert tr == pytest.approx(odt2, rel=1e-3)
     # final-state parity against the oracle at the GPU's own positions
     f, e = g.md_get_forces()
     ref = oracle.compute(P, pos.cpu().numpy(), w.types, w.box, w.pbc)
