@@ -1,0 +1,398 @@
+"""bench.py -- atom-steps/s of the NEP-ZBL MD hot path on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference] [--workload config2]
+
+One "step" = one velocity-Verlet step of the whole hot path (S1-S8 of DESIGN.md: integrator half
+kicks + drift, list rebuild when the skin is exhausted, radial/angular descriptors, network,
+force back-pass, ZBL) on BASELINE.json configs[1]: 128 000-atom bcc W, 300 K, dt = 1 fs, skin 1 A.
+Prints ONE JSON line (rank 0).  Keys: see DESIGN.md "Measurement".
+
+  value      K steps enqueued back to back by md_run (no host round trip), state resident in HBM,
+             timed with CUDA events on the launch stream, barrier + synchronize on both sides,
+             max over ranks.  `config.l2` says how the L2 rule is met.
+  e2e        the same steps through md_step_host: pos/vel copied host->device and device->host
+             every step from/to pinned host buffers, inside the timed region.
+  roofline   dominant kernel: algorithmic flops (DESIGN.md table) / CUDA-event duration per launch.
+  cpu_baseline  the fp64 oracle (oracle/, as it stands) timed on this box's host cores on a bounded
+             sample of the same workload (rank 0, N = 1 only).
+  --impl reference   times the oracle instead (this tier's reference arm); no GPU is touched.
+
+Multi-GPU: the path does not shard (north_star: one GPU, no collectives) -> "replicas only":
+every rank runs an independent replica (seed + rank) on its own GPU; value = sum of atom-steps
+over ranks / max time over ranks; scaling = "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import datetime
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "atom_steps_per_s"
+UNIT = "atom-steps/s"
+L2_BYTES = 126 * 1024 * 1024
+
+# Algorithmic FP32 work per atom-step of each force kernel for the configs' model (5+5 radial
+# functions, 9 basis functions, 24 (l,m), D = 30, 50 neurons) on bcc W at a = 3.165 A
+# (58 radial / 14 angular neighbours inside the cutoffs, 88 / 26 list entries with the 1 A skin).
+# Derivation: DESIGN.md "Algorithmic work per atom-step".  FMA = 2 flop.
+# Per step of the path (S3, S4, S6, S7a = angular back-pass, S7r = radial back-pass + angular gather):
+STEP_FLOP = {"S3": 3.2e3, "S4": 6.7e3, "S6": 6.6e3, "S7a": 14.0e3, "S7r": 8.6e3}
+KERNEL_STEPS = {"k_radial": ("S3",), "k_angular_nn": ("S4", "S6", "S7a"), "k_force": ("S7r",)}
+FLOP_PER_ATOM = {k: sum(STEP_FLOP[s] for s in v) for k, v in KERNEL_STEPS.items()}
+# Compulsory HBM bytes per atom-step of each kernel group (same table)
+BYTES_PER_ATOM = {"integrate_a": 152.0, "kick_b": 64.0, "k_radial": 392.0, "k_angular_nn": 612.0,
+                  "k_force": 1136.0}
+FP32_LANES_PER_SM = 128
+
+
+def _dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def make_workload(name: str, seed_offset: int = 0, cells=None):
+    from paper_2305_08140_b200 import workloads as wl
+    if name == "config2":
+        return wl.config2(seed=2 + seed_offset, cells=cells or 40)
+    if name == "config3":
+        return wl.config3(seed=3 + seed_offset, cells=cells or 80)
+    if name == "config4":
+        return wl.config4(seed=4 + seed_offset, cells=cells or 160)
+    if name == "config5":
+        return wl.config5(seed=5 + seed_offset, cells=cells or (160, 160, 100))
+    raise SystemExit(f"unknown workload {name}")
+
+
+# ------------------------------------------------------------------------------ clocks
+
+class ClockSampler:
+    """nvidia-smi sampled every 100 ms in the background; summarise the samples inside a window."""
+    FIELDS = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(gpu_index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            p = [x.strip() for x in line.split(",")]
+            if len(p) < 8:
+                continue
+            try:
+                ts = datetime.datetime.strptime(p[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                self.rows.append((ts, float(p[1]), float(p[2]), float(p[3]), p[4], p[5], p[6], p[7]))
+            except ValueError:
+                continue
+
+    def wait_first(self, timeout=5.0):
+        t0 = time.time()
+        while self.proc and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.05)
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+
+    def summary(self, t0: float, t1: float) -> dict:
+        rows = [r for r in self.rows if t0 - 0.05 <= r[0] <= t1 + 0.05] or self.rows[-3:]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        reasons = []
+        for k, name in ((4, "hw_slowdown"), (5, "hw_thermal_slowdown"), (6, "sw_thermal_slowdown"), (7, "sw_power_cap")):
+            if any(r[k] == "Active" for r in rows):
+                reasons.append(name)
+        return {"sm_mhz": float(np.median([r[1] for r in rows])), "sm_max_mhz": rows[0][2],
+                "power_w_max": max(r[3] for r in rows), "samples": len(rows), "reasons": reasons}
+
+
+# ------------------------------------------------------------------------------ oracle legs
+
+def oracle_md_rate(workload_name: str, n_steps: int | None, warmup: int, budget_s: float):
+    """Time the fp64 oracle's own MD loop (oracle.md_run, as it stands) on a bounded sample of the
+    workload: the same recipe (bcc W, 300 K, same model, dt = 1 fs).  With n_steps = None (the
+    cpu_baseline leg) the sample is the first steps of the FULL 40^3-cell system, as many as fit
+    `budget_s`; with n_steps given (the reference arm) it is the largest cell count from
+    (6, 8, 10, 12, 16, 24, 40)^3 for which (warmup + n_steps) steps fit `budget_s`.  Cost is linear in
+    N, so atom-steps/s carries over."""
+    import oracle
+    from paper_2305_08140_b200 import workloads as wl
+    w = wl.thermal_bulk(10, seed=2)
+    P = oracle.Params(w.model)
+    oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, 1, 1.0, np.inf)      # loads the library, spins up OpenMP
+    t = time.perf_counter()
+    oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, 2, 1.0, np.inf)
+    rate = 3 * w.n / (time.perf_counter() - t)                                 # atom-evaluations/s (3 evaluations)
+    if n_steps is None:
+        cells = 40
+        n_steps = int(max(3, min(200, budget_s * rate / (2 * cells ** 3) - 1)))
+    else:
+        cells = 6
+        for c in (8, 10, 12, 16, 24, 40):
+            if (warmup + n_steps + 2) * 2 * c ** 3 / rate <= budget_s:
+                cells = c
+    w = wl.thermal_bulk(cells, seed=2)
+    pos, vel = w.pos, w.vel
+    if warmup > 0:
+        pos, vel, *_ = oracle.md_run(P, pos, vel, w.types, w.box, w.pbc, warmup, 1.0, np.inf)
+    t = time.perf_counter()
+    oracle.md_run(P, pos, vel, w.types, w.box, w.pbc, n_steps, 1.0, np.inf)
+    dt = time.perf_counter() - t
+    # md_run evaluates forces once before the loop: n_steps + 1 evaluations for n_steps steps
+    return {"value": n_steps * w.n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{cells}^3 bcc cells ({w.n} atoms) of the {workload_name} recipe, {n_steps} oracle MD steps "
+                      f"(fp64, OpenMP, {n_steps + 1} force evaluations) in {dt:.1f} s"}, dt
+
+
+def run_reference(args):
+    rank, _, world = _dist_env()
+    if rank != 0:
+        return 0
+    cb, dt = oracle_md_rate(args.workload, args.steps, args.warmup, budget_s=150.0)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": args.workload + " (bounded sample, see cpu_baseline.sample)"},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------ B200 arm
+
+def aggregate_max(ms_local: float, world: int, device=None) -> float:
+    """max over ranks of a local duration (torch.distributed all-reduce; identity when world == 1)."""
+    if world == 1:
+        return ms_local
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_sum(x: float, world: int, device=None) -> float:
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+def run_b200(args):
+    import torch
+    rank, local_rank, world = _dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the B200 arm has no CPU fallback (use --impl reference for the oracle)")
+    from paper_2305_08140_b200 import build as cuda_build
+    cuda_build.build()
+    from paper_2305_08140_b200 import binding
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = make_workload(args.workload, seed_offset=rank, cells=args.cells)
+    n = w.n
+    stream = torch.cuda.Stream(device=dev)
+    g = binding.NepZbl(w.model, n, device=local_rank, stream=stream)
+    types = torch.from_numpy(w.types).to(dev)
+
+    def fresh_state():
+        pos = torch.from_numpy(w.pos.copy()).to(dev)
+        vel = torch.from_numpy(w.vel.copy()).to(dev)
+        g.md_init(pos, vel, types, w.box, w.pbc)
+        return pos, vel
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    K, W = args.steps, args.warmup
+    dt_max, max_disp = w.dt_max, w.max_displacement
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    if sampler:
+        sampler.wait_first()
+
+    # ---- device-resident run: K steps back to back (md_run), CUDA events on the launch stream
+    pos, vel = fresh_state()
+    e0 = sum(g.md_energies())
+    g.md_run(W, dt_max, max_disp)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    l0 = g.nep_zbl_launch_count()
+    reb0 = g.md_get_counters()[1]
+    t_wall0 = time.time()
+    ev0.record(stream)
+    g.md_run(K, dt_max, max_disp)
+    ev1.record(stream)
+    barrier()
+    t_wall1 = time.time()
+    launches = g.nep_zbl_launch_count() - l0
+    ms_local = ev0.elapsed_time(ev1)
+    ms = aggregate_max(ms_local, world, dev)
+    rebuilds = g.md_get_counters()[1] - reb0
+    e1 = sum(g.md_energies())
+    clocks = sampler.summary(t_wall0, t_wall1) if sampler else None
+    total_atoms = aggregate_sum(float(n), world, dev)
+    value = total_atoms * K / (ms * 1e-3)
+
+    # ---- same K steps, L2 flushed between steps (per-step event pairs; the flush is outside them)
+    flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
+    Kf = min(K, args.flush_steps)
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(Kf)]
+    with torch.cuda.stream(stream):
+        for a, b in evs:
+            flush.fill_(1)
+            a.record(stream)
+            g.md_step(dt_max, max_disp)
+            b.record(stream)
+    barrier()
+    ms_flushed = aggregate_max(sum(a.elapsed_time(b) for a, b in evs) / Kf, world, dev)
+    del flush
+
+    # ---- per-kernel CUDA-event spans over K more steps (profiling events between kernel groups)
+    g.nep_zbl_profile(True)
+    evp0, evp1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    Kp = min(K, 200)
+    evp0.record(stream)
+    g.md_run(Kp, dt_max, max_disp)
+    evp1.record(stream)
+    prof = g.nep_zbl_profile_read()
+    g.nep_zbl_profile(False)
+    ms_prof_step = evp0.elapsed_time(evp1) / Kp
+    kern_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in prof.items() if v[1]}
+    kern_share = {k: round(v[0] / Kp / ms_prof_step, 4) for k, v in prof.items() if v[1]}
+    ffma_measured = g.nep_zbl_ffma_peak()
+
+    # ---- end to end through the C ABI with HOST buffers (md_step_host): H2D + step + D2H per step
+    hp = torch.from_numpy(w.pos.copy()).pin_memory()
+    hv = torch.from_numpy(w.vel.copy()).pin_memory()
+    pos, vel = fresh_state()
+    Ke = min(K, args.e2e_steps)
+    for _ in range(min(W, 5)):
+        g.md_step_host(hp, hv, dt_max, max_disp)
+    eve0, eve1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0 = time.perf_counter()
+    eve0.record(stream)
+    for _ in range(Ke):
+        g.md_step_host(hp, hv, dt_max, max_disp)
+    eve1.record(stream)
+    barrier()
+    wall_e2e = (time.perf_counter() - t0) * 1e3
+    ms_e2e = aggregate_max(max(eve0.elapsed_time(eve1), wall_e2e), world, dev)
+    e2e_value = total_atoms * Ke / (ms_e2e * 1e-3)
+    if sampler:
+        sampler.stop()
+
+    if rank != 0:
+        return 0
+
+    # ---- roofline of the dominant kernel
+    force_kernels = {k: kern_ms[k] for k in ("k_radial", "k_angular_nn", "k_force") if k in kern_ms}
+    dom = max(force_kernels, key=force_kernels.get)
+    props = torch.cuda.get_device_properties(dev)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except OSError:
+        pass
+    sm_max_mhz = float(peaks.get("sm_max_mhz", (clocks or {}).get("sm_max_mhz") or 1965.0))
+    alu_peak = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12     # TFLOP/s
+    achieved = FLOP_PER_ATOM[dom] * n / (kern_ms[dom] * 1e-3) / 1e12
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": achieved / alu_peak, "traffic": args.traffic_bytes,
+                "peak_source": f"derived: {props.multi_processor_count} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max_mhz:.0f} MHz",
+                "ffma_measured_tflops": ffma_measured, "ms_per_launch": kern_ms[dom],
+                "flop_per_atom": FLOP_PER_ATOM[dom],
+                "hbm": {k: {"achieved_gbs": BYTES_PER_ATOM[k] * n / (kern_ms[k] * 1e-3) / 1e9,
+                            "frac": BYTES_PER_ATOM[k] * n / (kern_ms[k] * 1e-3) / 1e9 / hbm_peak}
+                        for k in BYTES_PER_ATOM if k in kern_ms},
+                "hbm_peak_gbs": hbm_peak, "hbm_peak_source": "measured" if peaks else "fallback"}
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu_baseline, _ = oracle_md_rate(args.workload, None, 0, budget_s=15.0)
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": args.workload, "atoms_per_gpu": n, "dt_max_fs": dt_max,
+                   "max_displacement_A": (None if not np.isfinite(max_disp) else max_disp), "skin_A": w.model["skin"],
+                   "model": "NEP-ZBL n_max 4/4, basis 8/8, l_max 4 + 4-body, 50 neurons, rc 6/4 A, universal ZBL 1-2 A",
+                   "precision": "fp32 descriptors/network/forces, fp64 positions/velocities/ZBL/energy sums",
+                   "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
+                   "l2": f"no flush for `value` (consecutive steps of one trajectory; workspace {g.workspace_bytes / 2**20:.0f} MiB "
+                         f"> {L2_BYTES / 2**20:.0f} MiB L2); `ms_per_step_l2_flushed` flushes L2 (2x L2 write) before every step",
+                   "list_rebuilds_in_timed_region": int(rebuilds)},
+        "ms_per_step_l2_flushed": ms_flushed, "value_l2_flushed": total_atoms / (ms_flushed * 1e-3),
+        "ms_per_step_profiled": ms_prof_step,
+        "kernel_ms": {k: round(v, 5) for k, v in kern_ms.items()}, "kernel_share": kern_share,
+        "energy_drift_ev_per_atom": (e1 - e0) / n,
+        "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
+                "steps": Ke, "api": "md_step_host"},
+        "gpu_launches": int(launches),
+        "context": {"paper": "1.3e7 atom-step/s, one 40-GB A100, trained W NEP-ZBL (n_max 15/10, 100 neurons), Table IV"},
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--cells", type=int, default=None, help="override the cell count (debug only)")
+    ap.add_argument("--e2e-steps", type=int, default=200)
+    ap.add_argument("--flush-steps", type=int, default=100)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic-bytes", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu capture")
+    args = ap.parse_args(argv)
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_b200(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,53 @@
+"""N > 1 path of bench.py on CPU: world_size-2 gloo run of the rank aggregation (max time, summed
+units) and of the reference arm's rank gating (rank 0 prints one JSON line, other ranks exit 0)."""
+import json
+import os
+import subprocess
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import torch.distributed as dist
+import bench
+dist.init_process_group("gloo")
+rank = dist.get_rank(); world = dist.get_world_size()
+ms = bench.aggregate_max(10.0 + 5.0 * rank, world)       # rank 1 is the slow one
+units = bench.aggregate_sum(1000.0 * (rank + 1), world)
+print(json.dumps({{"rank": rank, "ms": ms, "units": units}}), flush=True)
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+def _torchrun(args, timeout=300):
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", OMP_NUM_THREADS="1")
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+           "--master-addr", "127.0.0.1", "--master-port", "29731"] + args
+    return subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, env=env, cwd=ROOT)
+
+
+def test_aggregation_world_size_2_gloo(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER.format(root=ROOT))
+    r = _torchrun([str(script)])
+    assert r.returncode == 0, r.stderr[-2000:]
+    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(rows) == 2
+    for row in rows:
+        assert row["ms"] == 15.0           # max over ranks
+        assert row["units"] == 3000.0      # whole-job units
+
+
+def test_reference_arm_prints_one_line_under_torchrun():
+    r = _torchrun([os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "3",
+                   "--warmup", "3"])
+    assert r.returncode == 0, r.stderr[-2000:]
+    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(rows) == 1
+    line = rows[0]
+    assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["unit"] == "atom-steps/s"
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+    assert line["value"] > 0
