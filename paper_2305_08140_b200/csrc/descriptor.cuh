@@ -38,11 +38,28 @@ struct ModelTables {
   float ctR[MS::NR][MS::KR];   // folded radial coefficients
   float ctA[MS::NA][MS::KA];   // folded angular coefficients
   float kctA[MS::NA][MS::KA];  // k * ctA (derivative through T_k' = k U_{k-1})
+  float kctR[MS::NR][MS::KR];  // k * ctR
   float inv_rcR, inv_rcA, rcR2, rcA2;
   float zbl_flag_r2;           // (r_outer + margin)^2, 0 if ZBL disabled
   float b1;
   int n_neurons;
 };
+
+struct __align__(32) AtomRec {  // compute copy + radial back-pass input of one atom (sorted order)
+  int ux, uy, uz;                // fixed-point coordinates (same as xyzt)
+  float fp[5];                   // Fp[n] = dU/dq_n of the radial descriptor components
+};
+__device__ __forceinline__ AtomRec ld_rec(const AtomRec* p) {
+  AtomRec r;
+  unsigned v0, v1, v2, v3, v4, v5, v6, v7;
+  asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3), "=r"(v4), "=r"(v5), "=r"(v6), "=r"(v7)
+               : "l"(p));
+  r.ux = (int)v0; r.uy = (int)v1; r.uz = (int)v2;
+  r.fp[0] = __uint_as_float(v3); r.fp[1] = __uint_as_float(v4); r.fp[2] = __uint_as_float(v5);
+  r.fp[3] = __uint_as_float(v6); r.fp[4] = __uint_as_float(v7);
+  return r;
+}
 
 // (2l+1)/(4 pi) * addition-theorem weight of each b_lm (see DESIGN.md for the list of b_lm)
 __device__ __constant__ const float kClm[24] = {
@@ -116,15 +133,47 @@ __device__ __forceinline__ void contract_blm_grad(float x, float y, float z, F1 
   g = G(23); Sp = fmaf(Gp(23), s4, Sp); vx = fmaf(g, 4.0f * s3, vx); vy = fmaf(g, 4.0f * c3, vy);
 }
 
-// cutoff function and Chebyshev polynomials T_0..T_{K-1} at distance r
+// cos(pi t) and sin(pi t) for t in [0, 1] (t = r/rc inside the cutoff): with y = 1/2 - t in [-1/2, 1/2],
+// cos(pi t) = sin(pi y) = y P(y^2), sin(pi t) = cos(pi y) = Q(y^2).  P, Q: Chebyshev interpolants of
+// sin(pi sqrt(w))/sqrt(w) and cos(pi sqrt(w)) on w in [0, 1/4] (degree 4 / 5; truncation error 7e-9 / 2e-10,
+// below fp32 rounding).  Replaces sincospif (range reduction not needed here): ~12 instructions for both.
+__device__ __forceinline__ float cospi_unit(float t, float& y, float& w) {
+  y = 0.5f - t;
+  w = y * y;
+  float p = fmaf(w, 7.765591228e-02f, -5.982904113e-01f);
+  p = fmaf(w, p, 2.550077387e+00f);
+  p = fmaf(w, p, -5.167710077e+00f);
+  p = fmaf(w, p, 3.141592640e+00f);
+  return y * p;
+}
+__device__ __forceinline__ float sinpi_unit_from_w(float w) {
+  float q = fmaf(w, -2.439593201e-02f, 2.349370685e-01f);
+  q = fmaf(w, q, -1.335211949e+00f);
+  q = fmaf(w, q, 4.058709155e+00f);
+  q = fmaf(w, q, -4.934802137e+00f);
+  return fmaf(w, q, 9.999999998e-01f);
+}
+
+// cutoff function f_c and Chebyshev polynomials T_0..T_{K-1} at distance r (r < rc)
+template <int K>
+__device__ __forceinline__ void cheb_T_fwd(float r, float inv_rc, float& fc, float T[K]) {
+  float t = r * inv_rc, y, w;
+  fc = fmaf(0.5f, cospi_unit(t, y, w), 0.5f);
+  float u = t - 1.0f;
+  float x = fmaf(2.0f * u, u, -1.0f);
+  T[0] = 1.0f;
+  if (K > 1) T[1] = x;
+  float x2 = 2.0f * x;
+#pragma unroll
+  for (int k = 2; k < K; ++k) T[k] = fmaf(x2, T[k - 1], -T[k - 2]);
+}
+// the same plus derivatives: dfc = f_c'(r), x, dx = dx/dr
 template <int K>
 __device__ __forceinline__ void cheb_T(float r, float inv_rc, float& fc, float& dfc, float& x,
                                        float& dx, float T[K]) {
-  float t = r * inv_rc;
-  float sn, cs;
-  sincospif(t, &sn, &cs);
-  fc = 0.5f + 0.5f * cs;
-  dfc = -0.5f * NEPZBL_PI_F * inv_rc * sn;
+  float t = r * inv_rc, y, w;
+  fc = fmaf(0.5f, cospi_unit(t, y, w), 0.5f);
+  dfc = -0.5f * NEPZBL_PI_F * inv_rc * sinpi_unit_from_w(w);
   float u = t - 1.0f;
   x = fmaf(2.0f * u, u, -1.0f);
   dx = 4.0f * u * inv_rc;
@@ -152,44 +201,84 @@ __device__ __forceinline__ float tanh_fast(float z) {
 
 // ------------------------------------------------------------------------- S3: radial descriptor
 // q_n = sum_j g^R_n(r_ij) for r_ij < rc_radial; also flags atoms with a neighbour inside the ZBL range.
+// RADIAL_LANES lanes per atom: lane p owns list entries p, p+4, ...  The gathers are latency-bound
+// (ncu: long-scoreboard stalls on the dependent index -> position loads), so every lane issues 4
+// independent index loads and 4 independent position gathers per iteration before any arithmetic.
+// Which of a lane's entries are inside the cutoff is kept as a bit mask (bit b <-> entry p + 4 b) and
+// handed to k_force, which then gathers only those.  The K basis sums are combined over the 4 lanes
+// by a fixed-order shuffle tree (deterministic).
+#define RADIAL_LANES 4
+#define RADIAL_UNROLL 4
 template <class MS>
 __global__ void __launch_bounds__(128)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
          const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,
-         int* __restrict__ zbl_list) {
-  int s = blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= n) return;
-  const int4 me = xyzt[s];
+         unsigned* __restrict__ rmask, int mask_words, int* __restrict__ zbl_list) {
+  const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+  const int s = gt / RADIAL_LANES, sub = gt % RADIAL_LANES;
+  const bool valid = s < n;
+  const int sc_ = valid ? s : 0;
+  const int4 me = xyzt[sc_];
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
   float acc[MS::KR];
 #pragma unroll
   for (int k = 0; k < MS::KR; ++k) acc[k] = 0.0f;
   bool close = false;
-  const int cnt = nn_r[s];
-  int jn = cnt > 0 ? nl_r[s] : 0;
-  for (int t = 0; t < cnt; ++t) {
-    int j = jn;
-    if (t + 1 < cnt) jn = nl_r[(size_t)(t + 1) * npad + s];
-    int4 o = xyzt[j];
-    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
-    float r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 < mt.rcR2) {
-      float r = sqrtf(r2), fc, dfc, x, dxdr, T[MS::KR];
-      cheb_T<MS::KR>(r, mt.inv_rcR, fc, dfc, x, dxdr, T);
+  const int cnt = valid ? nn_r[sc_] : 0;
+  const int* lp = nl_r + (size_t)sub * npad + sc_;
+  const size_t lstride = (size_t)RADIAL_LANES * npad;
+  unsigned mword = 0u;
+  int bit = 0, word = 0;
+  for (int t = sub; t < cnt; t += RADIAL_LANES * RADIAL_UNROLL) {
+    int j[RADIAL_UNROLL];
+    int4 o[RADIAL_UNROLL];
 #pragma unroll
-      for (int k = 0; k < MS::KR; ++k) acc[k] = fmaf(fc, T[k], acc[k]);
-      close = close || (r2 < mt.zbl_flag_r2);
+    for (int u = 0; u < RADIAL_UNROLL; ++u)
+      j[u] = (t + RADIAL_LANES * u < cnt) ? lp[(size_t)u * lstride] : sc_;
+    lp += (size_t)RADIAL_UNROLL * lstride;
+#pragma unroll
+    for (int u = 0; u < RADIAL_UNROLL; ++u) o[u] = xyzt[j[u]];
+#pragma unroll
+    for (int u = 0; u < RADIAL_UNROLL; ++u) {
+      float dx = (float)(o[u].x - me.x) * hx, dy = (float)(o[u].y - me.y) * hy, dz = (float)(o[u].z - me.z) * hz;
+      float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+      if ((t + RADIAL_LANES * u < cnt) && r2 < mt.rcR2) {
+        float r = r2 * rsqrtf(r2), fc, T[MS::KR];
+        cheb_T_fwd<MS::KR>(r, mt.inv_rcR, fc, T);
+#pragma unroll
+        for (int k = 0; k < MS::KR; ++k) acc[k] = fmaf(fc, T[k], acc[k]);
+        close = close || (r2 < mt.zbl_flag_r2);
+        mword |= 1u << (bit + u);
+      }
+    }
+    bit += RADIAL_UNROLL;
+    if (bit == 32) {
+      rmask[((size_t)word * RADIAL_LANES + sub) * npad + sc_] = mword;
+      mword = 0u;
+      bit = 0;
+      ++word;
     }
   }
+  if (valid)
+    for (; word < mask_words; ++word) {
+      rmask[((size_t)word * RADIAL_LANES + sub) * npad + s] = mword;
+      mword = 0u;
+    }
 #pragma unroll
-  for (int nq = 0; nq < MS::NR; ++nq) {
+  for (int k = 0; k < MS::KR; ++k) {
+    acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], 1);
+    acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], 2);
+  }
+  unsigned cb = __ballot_sync(0xffffffffu, close);
+  if (!valid) return;
+  for (int nq = sub; nq < MS::NR; nq += RADIAL_LANES) {
     float q = 0.0f;
 #pragma unroll
     for (int k = 0; k < MS::KR; ++k) q = fmaf(mt.ctR[nq][k], acc[k], q);
     q_radial[(size_t)nq * npad + s] = q;
   }
-  if (close) zbl_list[atomicAdd(&sc->zbl_count, 1)] = s;
+  if (sub == 0 && ((cb >> (threadIdx.x & 28)) & 0xFu)) zbl_list[atomicAdd(&sc->zbl_count, 1)] = s;
 }
 
 // ------------------------------------------------------- S4 + S6 + angular partial forces of S7
@@ -200,7 +289,7 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restr
              const int* __restrict__ nn_a, const int* __restrict__ nl_a,
              const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,
              const float* __restrict__ q_radial, float* __restrict__ u_site,
-             float4* __restrict__ dk, float4* __restrict__ pforce, float* __restrict__ q_out) {
+             AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out) {
   constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR, D = MS::D, DPAD = MS::DPAD;
   extern __shared__ __align__(16) float smem[];
   const int neu = mt.n_neurons;
@@ -328,18 +417,15 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restr
   for (int v = 0; v < D; ++v) Fp[v] *= s_qs[v];
   u_site[s] = U;
 
-  // radial back-pass coefficients d_k = sum_n Fp_n ct_nk  (used by k_force for both i and j)
+  // record for the radial back-pass of k_force: position + Fp of the radial components
   {
-    float d[12];
+    static_assert(NR <= 5, "AtomRec holds 5 radial Fp components");
+    float f[5] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll
-    for (int k = 0; k < 12; ++k) d[k] = 0.0f;
-#pragma unroll
-    for (int k = 0; k < KR; ++k)
-#pragma unroll
-      for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
-    dk[3 * (size_t)s + 0] = make_float4(d[0], d[1], d[2], d[3]);
-    dk[3 * (size_t)s + 1] = make_float4(d[4], d[5], d[6], d[7]);
-    dk[3 * (size_t)s + 2] = make_float4(d[8], d[9], d[10], d[11]);
+    for (int nq = 0; nq < NR; ++nq) f[nq] = Fp[nq];
+    int4* rp = reinterpret_cast<int4*>(rec + s);
+    rp[0] = make_int4(me.x, me.y, me.z, __float_as_int(f[0]));
+    rp[1] = make_int4(__float_as_int(f[1]), __float_as_int(f[2]), __float_as_int(f[3]), __float_as_int(f[4]));
   }
 
   // ---- E[n][lm] = dU/dA[n][lm] (in place)

@@ -1,8 +1,12 @@
 // force.cuh -- S7 (force / virial accumulation, gather form) and S5 (ZBL pair term).
 //
 // S7:  F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji),  W_i = sum_j r_ij (x) dU_j/dr_ji.
-//   radial part:  dU_i/dr_ij = rhat_ij sum_k d_i[k] (f_c T_k)'(r_ij), d_i[k] = sum_n Fp_i[n] ct_nk,
-//                 so F_i += rhat_ij sum_k (d_i[k] + d_j[k]) (f_c T_k)'  -- one gather of d_j per pair;
+//   radial part:  dU_i/dr_ij = rhat_ij sum_n Fp_i[n] g_n'(r_ij), so F_i += rhat_ij sum_n (Fp_i[n] + Fp_j[n]) g_n'.
+//                 Per pair ONE 32-byte gather: the neighbour's record {ux,uy,uz,Fp[0..4]} written by
+//                 k_angular_nn, fetched with a single 256-bit load (LDG.E.256, new on sm_100).  The kernel
+//                 is bound by L1 tag lookups of these scattered gathers (ncu, profiles/), so the record
+//                 is kept to one sector and g_n' is re-evaluated on the ALUs instead of gathering 48 B of
+//                 pre-contracted coefficients;
 //   angular part: partial forces stored by k_angular_nn; F_i += p[i][a] - p[j][rev[i][a]].
 //   Gather form only: every atom sums its own pairs in list order -> no float atomics, bitwise
 //   reproducible.
@@ -11,68 +15,80 @@
 #pragma once
 #include "descriptor.cuh"
 
+// FORCE_LANES lanes per atom: lane p takes list entries p, p+4, ... of both lists (skipping ahead to the
+// next radial entry inside the cutoff before the convergent body); F and W are combined over the 4
+// lanes by a fixed-order shuffle tree, so the result is still bit-reproducible.
+#define FORCE_LANES 4
 template <class MS, bool VIRIAL>
 __global__ void __launch_bounds__(128)
 k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
         const int* __restrict__ nn_r, const int* __restrict__ nl_r, const int* __restrict__ nn_a,
         const int* __restrict__ nl_a, const unsigned char* __restrict__ rev,
-        const __grid_constant__ ModelTables<MS> mt, const float4* __restrict__ dk,
-        const float4* __restrict__ pforce, const float* __restrict__ u_site,
+        const __grid_constant__ ModelTables<MS> mt, const AtomRec* __restrict__ rec,
+        const unsigned* __restrict__ rmask, int mask_words, const float4* __restrict__ pforce, const float* __restrict__ u_site,
         const int* __restrict__ perm, double* __restrict__ energy, float* __restrict__ force,
         float* __restrict__ virial) {
-  constexpr int KR = MS::KR;
-  static_assert(KR <= 12, "d_k record holds 12 floats");
-  int s = blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= n) return;
-  const int4 me = xyzt[s];
+  constexpr int KR = MS::KR, NR = MS::NR;
+  static_assert(NR <= 5, "AtomRec holds 5 radial Fp components");
+  const int gt = blockIdx.x * blockDim.x + threadIdx.x;
+  const int s = gt / FORCE_LANES, sub = gt % FORCE_LANES;
+  const bool valid = s < n;
+  const int sc_ = valid ? s : 0;
+  const AtomRec me = ld_rec(rec + sc_);
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
-  float di[12];
-  {
-    float4 a = dk[3 * (size_t)s], b = dk[3 * (size_t)s + 1], c = dk[3 * (size_t)s + 2];
-    di[0] = a.x; di[1] = a.y; di[2] = a.z; di[3] = a.w; di[4] = b.x; di[5] = b.y; di[6] = b.z;
-    di[7] = b.w; di[8] = c.x; di[9] = c.y; di[10] = c.z; di[11] = c.w;
-  }
   float fx = 0.0f, fy = 0.0f, fz = 0.0f;
   float w[9];
 #pragma unroll
   for (int c = 0; c < 9; ++c) w[c] = 0.0f;
 
-  // ---- radial pairs
-  const int cnt = nn_r[s];
-  int jn = cnt > 0 ? nl_r[s] : 0;
-  for (int t = 0; t < cnt; ++t) {
-    int j = jn;
-    if (t + 1 < cnt) jn = nl_r[(size_t)(t + 1) * npad + s];
-    int4 o = xyzt[j];
-    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
-    float r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 < mt.rcR2) {
-      float dj[12];
-      {
-        float4 a = dk[3 * (size_t)j], b = dk[3 * (size_t)j + 1], c = dk[3 * (size_t)j + 2];
-        dj[0] = a.x; dj[1] = a.y; dj[2] = a.z; dj[3] = a.w; dj[4] = b.x; dj[5] = b.y; dj[6] = b.z;
-        dj[7] = b.w; dj[8] = c.x; dj[9] = c.y; dj[10] = c.z; dj[11] = c.w;
+  // ---- radial pairs: only the entries k_radial found inside the cutoff (bit mask per lane), with the
+  //      next entry's index and record gathers in flight while the current pair is evaluated
+  {
+    const int* lp = nl_r + (size_t)sub * npad + sc_;
+    const size_t lstride = (size_t)FORCE_LANES * npad;
+    int word = 0;
+    unsigned m = valid ? rmask[(size_t)sub * npad + sc_] : 0u;
+    // pop the next entry of this lane: returns its neighbour index or -1
+    auto next_j = [&]() -> int {
+      while (m == 0u) {
+        if (++word >= mask_words) return -1;
+        m = valid ? rmask[((size_t)word * FORCE_LANES + sub) * npad + sc_] : 0u;
       }
-      float r = sqrtf(r2), rinv = 1.0f / r;
+      int b = __ffs((int)m) - 1;
+      m &= m - 1u;
+      return lp[(size_t)(32 * word + b) * lstride];
+    };
+    int j_cur = next_j();
+    AtomRec o_cur = ld_rec(rec + (j_cur >= 0 ? j_cur : sc_));
+    int j_nxt = j_cur >= 0 ? next_j() : -1;
+    while (j_cur >= 0) {
+      AtomRec o_nxt = ld_rec(rec + (j_nxt >= 0 ? j_nxt : sc_));
+      int j_nn = j_nxt >= 0 ? next_j() : -1;
+      const AtomRec& o = o_cur;
+      float dx = (float)(o.ux - me.ux) * hx, dy = (float)(o.uy - me.uy) * hy, dz = (float)(o.uz - me.uz) * hz;
+      float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+      float rinv = rsqrtf(r2), r = r2 * rinv;
       float fc, dfc, x, dxdr, T[KR], Uc[KR];
       cheb_T<KR>(r, mt.inv_rcR, fc, dfc, x, dxdr, T);
       cheb_U<KR>(x, Uc);
-      // sum_k d[k] (f_c T_k)' = f_c' sum_k d[k] T_k + f_c x' sum_{k>=1} d[k] k U_{k-1}
-      float ai = 0.0f, bi = 0.0f, aj = 0.0f, bj = 0.0f;
+      // g_n'(r) = f_c' sum_k ct_nk T_k + f_c x' sum_{k>=1} k ct_nk U_{k-1}
+      const float e = fc * dxdr;
+      float gi = 0.0f, gj = 0.0f;
 #pragma unroll
-      for (int k = 0; k < KR; ++k) {
-        ai = fmaf(di[k], T[k], ai);
-        aj = fmaf(dj[k], T[k], aj);
-      }
+      for (int nq = 0; nq < NR; ++nq) {
+        float p = 0.0f, dp = 0.0f;
 #pragma unroll
-      for (int k = 1; k < KR; ++k) {
-        float ku = (float)k * Uc[k - 1];
-        bi = fmaf(di[k], ku, bi);
-        bj = fmaf(dj[k], ku, bj);
+        for (int k = 0; k < KR; ++k) p = fmaf(mt.ctR[nq][k], T[k], p);
+#pragma unroll
+        for (int k = 1; k < KR; ++k) dp = fmaf(mt.kctR[nq][k], Uc[k - 1], dp);
+        float dg = fmaf(dfc, p, e * dp);
+        if (VIRIAL) {
+          gi = fmaf(me.fp[nq], dg, gi);  // dU_i/dr along rhat_ij
+          gj = fmaf(o.fp[nq], dg, gj);   // dU_j/dr along rhat_ji (same scalar form)
+        } else {
+          gi = fmaf(me.fp[nq] + o.fp[nq], dg, gi);
+        }
       }
-      float e = fc * dxdr;
-      float gi = fmaf(dfc, ai, e * bi);  // dU_i/dr along rhat_ij
-      float gj = fmaf(dfc, aj, e * bj);  // dU_j/dr along rhat_ji (same scalar form)
       float fs = (gi + gj) * rinv;
       fx = fmaf(fs, dx, fx);
       fy = fmaf(fs, dy, fy);
@@ -84,39 +100,72 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
         w[3] = fmaf(dy, wx, w[3]); w[4] = fmaf(dy, wy, w[4]); w[5] = fmaf(dy, wz, w[5]);
         w[6] = fmaf(dz, wx, w[6]); w[7] = fmaf(dz, wy, w[7]); w[8] = fmaf(dz, wz, w[8]);
       }
+      j_cur = j_nxt;
+      o_cur = o_nxt;
+      j_nxt = j_nn;
     }
   }
 
-  // ---- angular pairs: own partial force minus the neighbour's partial force on the same pair
-  const int ca = nn_a[s];
-  for (int a = 0; a < ca; ++a) {
-    int j = nl_a[(size_t)a * npad + s];
-    int b = rev[(size_t)a * npad + s];
-    float4 pij = pforce[(size_t)a * npad + s];
-    float4 pji = pforce[(size_t)b * npad + j];
-    fx += pij.x - pji.x;
-    fy += pij.y - pji.y;
-    fz += pij.z - pji.z;
-    if (VIRIAL) {
-      int4 o = xyzt[j];
-      float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
-      w[0] = fmaf(dx, pji.x, w[0]); w[1] = fmaf(dx, pji.y, w[1]); w[2] = fmaf(dx, pji.z, w[2]);
-      w[3] = fmaf(dy, pji.x, w[3]); w[4] = fmaf(dy, pji.y, w[4]); w[5] = fmaf(dy, pji.z, w[5]);
-      w[6] = fmaf(dz, pji.x, w[6]); w[7] = fmaf(dz, pji.y, w[7]); w[8] = fmaf(dz, pji.z, w[8]);
+  // ---- angular pairs: own partial force minus the neighbour's partial force on the same pair;
+  //      2 entries per lane per iteration so that the dependent gathers overlap
+  {
+    const int ca = valid ? nn_a[sc_] : 0;
+    for (int a0 = sub; a0 < ca; a0 += 2 * FORCE_LANES) {
+      const int a1 = a0 + FORCE_LANES;
+      const bool ok1 = a1 < ca;
+      const size_t e0 = (size_t)a0 * npad + sc_, e1 = (size_t)(ok1 ? a1 : a0) * npad + sc_;
+      int j0 = nl_a[e0], j1 = nl_a[e1];
+      int b0 = rev[e0], b1 = rev[e1];
+      float4 pij0 = pforce[e0], pij1 = pforce[e1];
+      float4 pji0 = pforce[(size_t)b0 * npad + j0], pji1 = pforce[(size_t)b1 * npad + j1];
+      if (!ok1) pij1 = pji1 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+      fx += pij0.x - pji0.x;
+      fy += pij0.y - pji0.y;
+      fz += pij0.z - pji0.z;
+      fx += pij1.x - pji1.x;
+      fy += pij1.y - pji1.y;
+      fz += pij1.z - pji1.z;
+      if (VIRIAL) {
+        int4 o0 = xyzt[j0], o1 = xyzt[j1];
+        {
+          float dx = (float)(o0.x - me.ux) * hx, dy = (float)(o0.y - me.uy) * hy, dz = (float)(o0.z - me.uz) * hz;
+          w[0] = fmaf(dx, pji0.x, w[0]); w[1] = fmaf(dx, pji0.y, w[1]); w[2] = fmaf(dx, pji0.z, w[2]);
+          w[3] = fmaf(dy, pji0.x, w[3]); w[4] = fmaf(dy, pji0.y, w[4]); w[5] = fmaf(dy, pji0.z, w[5]);
+          w[6] = fmaf(dz, pji0.x, w[6]); w[7] = fmaf(dz, pji0.y, w[7]); w[8] = fmaf(dz, pji0.z, w[8]);
+        }
+        {
+          float dx = (float)(o1.x - me.ux) * hx, dy = (float)(o1.y - me.uy) * hy, dz = (float)(o1.z - me.uz) * hz;
+          w[0] = fmaf(dx, pji1.x, w[0]); w[1] = fmaf(dx, pji1.y, w[1]); w[2] = fmaf(dx, pji1.z, w[2]);
+          w[3] = fmaf(dy, pji1.x, w[3]); w[4] = fmaf(dy, pji1.y, w[4]); w[5] = fmaf(dy, pji1.z, w[5]);
+          w[6] = fmaf(dz, pji1.x, w[6]); w[7] = fmaf(dz, pji1.y, w[7]); w[8] = fmaf(dz, pji1.z, w[8]);
+        }
+      }
     }
   }
 
-  // ---- results in the caller's atom order
+  // ---- combine the 4 lanes (fixed order), results in the caller's atom order
+  fx += __shfl_xor_sync(0xffffffffu, fx, 1); fx += __shfl_xor_sync(0xffffffffu, fx, 2);
+  fy += __shfl_xor_sync(0xffffffffu, fy, 1); fy += __shfl_xor_sync(0xffffffffu, fy, 2);
+  fz += __shfl_xor_sync(0xffffffffu, fz, 1); fz += __shfl_xor_sync(0xffffffffu, fz, 2);
+  if (VIRIAL) {
+#pragma unroll
+    for (int c = 0; c < 9; ++c) {
+      w[c] += __shfl_xor_sync(0xffffffffu, w[c], 1);
+      w[c] += __shfl_xor_sync(0xffffffffu, w[c], 2);
+    }
+  }
+  if (!valid) return;
   int i = perm[s];
-  if (energy) energy[i] = (double)u_site[s];
+  if (sub == 0 && energy) energy[i] = (double)u_site[s];
   if (force) {
-    force[i] = fx;
-    force[(size_t)n + i] = fy;
-    force[2 * (size_t)n + i] = fz;
+    if (sub == 0) force[i] = fx;
+    if (sub == 1) force[(size_t)n + i] = fy;
+    if (sub == 2) force[2 * (size_t)n + i] = fz;
   }
   if (VIRIAL) {
 #pragma unroll
-    for (int c = 0; c < 9; ++c) virial[(size_t)c * n + i] = w[c];
+    for (int c = 0; c < 9; ++c)
+      if ((c & 3) == sub) virial[(size_t)c * n + i] = w[c];
   }
 }
 

@@ -25,7 +25,7 @@ constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
-      nn_r, nn_a, nl_r, nl_a, rev, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
+      nn_r, nn_a, nl_r, nl_a, rev, rmask, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
       partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
@@ -114,6 +114,9 @@ int fail(nepzbl_handle* h, int code, const char* fmt, ...) {
 
 inline size_t al(size_t x) { return (x + 255) & ~size_t(255); }
 
+// 32-bit words of the per-lane in-cutoff mask: lane p of RADIAL_LANES owns entries p, p+4, ...
+inline int mask_words(const nepzbl_params& p) { return (p.cap_radial + 32 * RADIAL_LANES - 1) / (32 * RADIAL_LANES); }
+
 Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   Carve c{};
   long long npad = (n_cap + 127) / 128 * 128;
@@ -137,8 +140,9 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.nl_r = take(4 * (size_t)p.cap_radial * npad);
   c.nl_a = take(4 * (size_t)p.cap_angular * npad);
   c.rev = take((size_t)p.cap_angular * npad);
+  c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
   c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
-  c.dk = take(48 * npad);
+  c.dk = take(32 * npad);  // AtomRec
   c.pforce = take(16 * (size_t)p.cap_angular * npad);
   c.u_site = take(4 * npad);
   c.q_desc = take(4 * (size_t)D * npad);
@@ -174,7 +178,7 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
       }
     }
   };
-  fold(p->c_radial, MS::NR, MS::KR, &t.ctR[0][0], nullptr);
+  fold(p->c_radial, MS::NR, MS::KR, &t.ctR[0][0], &t.kctR[0][0]);
   fold(p->c_angular, MS::NA, MS::KA, &t.ctA[0][0], &t.kctA[0][0]);
   t.inv_rcR = (float)(1.0 / p->rc_radial);
   t.inv_rcA = (float)(1.0 / p->rc_angular);
@@ -282,25 +286,26 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   cudaStream_t st = h->stream;
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
   prof_mark(h, PK_RADIAL);
-  k_radial<MS><<<blocks(n, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
+  k_radial<MS><<<blocks((long long)n * RADIAL_LANES, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
                                               h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
-                                              h->at<float>(c.q_radial), h->at<int>(c.zbl_list));
+                                              h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p),
+                                              h->at<int>(c.zbl_list));
   prof_mark(h, PK_ANGULAR_NN);
   k_angular_nn<MS><<<blocks(n, 128), 128, h->smem_nn, st>>>(
       h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_a), h->at<int>(c.nl_a), mt, h->d_nnw,
-      h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<float4>(c.dk), h->at<float4>(c.pforce),
+      h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
       want_q ? h->at<float>(c.q_desc) : nullptr);
   prof_mark(h, PK_FORCE);
   if (virial)
-    k_force<MS, true><<<blocks(n, 128), 128, 0, st>>>(
+    k_force<MS, true><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<float4>(c.dk),
-        h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial);
+        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
+        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial);
   else
-    k_force<MS, false><<<blocks(n, 128), 128, 0, st>>>(
+    k_force<MS, false><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<float4>(c.dk),
-        h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
+        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
+        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
   h->launches += 3;
   if (h->p.zbl_enabled) {
     prof_mark(h, PK_ZBL);

@@ -1,0 +1,86 @@
+"""GPU tests at BASELINE.json's full sizes (configs 3-5: 1 024 000, 8 192 000 and 5 120 000 atoms):
+sampled parity against the oracle (SURVEY 8(d) "spot parity at scale"), the adaptive-dt invariants of
+P:77 and the HBM footprint.  The oracle evaluates a seeded sample of atoms plus every atom close to
+the primary knock-on atom's track; it needs only their neighbourhoods, so it finishes in seconds."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2305_08140_b200 import workloads as wl
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def nb():
+    from paper_2305_08140_b200 import binding
+    assert torch.cuda.is_available()
+    return binding
+
+
+def _min_image(d, box, pbc):
+    L = box[[0, 4, 8]][:, None]
+    p = np.asarray(pbc, dtype=bool)[:, None]
+    return np.where(p, d - L * np.round(d / L), d)
+
+
+def _cascade(nb, w, n_steps, n_sample=2048, seed=11):
+    n = w.n
+    g = nb.NepZbl(w.model, n)
+    pos = torch.from_numpy(w.pos.copy()).cuda()
+    vel = torch.from_numpy(w.vel.copy()).cuda()
+    types = torch.from_numpy(w.types).cuda()
+    g.md_init(pos, vel, types, w.box, w.pbc)
+    P = oracle.Params(w.model)
+    pka = w.info["pka_atom"]
+    vmax0 = np.sqrt((w.vel ** 2).sum(axis=0)).max()
+
+    def check_parity(label):
+        p = pos.cpu().numpy()
+        f, e = g.md_get_forces()
+        d = _min_image(p - p[:, [pka]], w.box, w.pbc)
+        near = np.nonzero((d ** 2).sum(axis=0) < 8.0 ** 2)[0]
+        sel = np.union1d(wl.rng(seed, 30).choice(n, size=n_sample, replace=False), near).astype(np.int32)
+        ref = oracle.compute(P, p, w.types, w.box, w.pbc, sel=sel, want_virial=False)
+        r = parity.compare(e.cpu().numpy(), f.cpu().numpy(), None, ref, idx=sel, label=f"{w.name} {label}")
+        assert max(r.values()) <= 1.0, r
+        return p
+
+    p0 = check_parity("step 0")
+    e0 = sum(g.md_energies())
+    tr, nreb = g.md_run(n_steps, w.dt_max, w.max_displacement, want_trace=True)
+    # the fastest atom moves at most max_displacement per step, dt <= dt_max
+    assert tr[0] == pytest.approx(w.max_displacement / vmax0, rel=1e-9)
+    assert np.all(tr <= w.dt_max) and np.all(tr > 0)
+    p1 = check_parity(f"step {n_steps}")
+    disp = np.sqrt((_min_image(p1 - p0, w.box, w.pbc) ** 2).sum(axis=0)).max()
+    assert disp <= n_steps * w.max_displacement * (1 + 1e-3)
+    assert disp > 0.5 * n_steps * w.max_displacement            # the knock-on atom really moved
+    e1 = sum(g.md_energies())
+    steps, rebuilds, zbl_atoms = g.md_get_counters()
+    zmax = zbl_atoms
+    print(f"{w.name}: n={n} workspace={g.workspace_bytes / 2**30:.2f} GiB  dE={e1 - e0:.3e} eV of {w.info['pka_energy_ev']:.0f} eV  "
+          f"rebuilds={rebuilds} zbl_atoms={zbl_atoms} dt0={tr[0]:.5f} fs")
+    assert steps == n_steps
+    assert abs(e1 - e0) < 1e-3 * w.info["pka_energy_ev"]       # NVE: the PKA energy stays in the system
+    return g
+
+
+def test_config3_one_million_atoms_10keV(nb):
+    g = _cascade(nb, wl.config3(), n_steps=400)                 # 6 A of travel: a close collision (ZBL active)
+    assert g.md_get_counters()[1] >= 1 + 10                     # md_init's build + one per 0.5 A travelled
+
+
+def test_config4_eight_million_atoms_100keV(nb):
+    w = wl.config4()
+    assert w.n == 8_192_000
+    g = _cascade(nb, w, n_steps=40)
+    assert g.workspace_bytes < 40 * 2**30                       # fits one B200 many times over
+
+
+def test_config5_foil_open_z_100keV(nb):
+    w = wl.config5()
+    assert w.n == 5_120_000 and list(w.pbc) == [1, 1, 0]
+    _cascade(nb, w, n_steps=40)
