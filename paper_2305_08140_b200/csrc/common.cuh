@@ -32,6 +32,9 @@ struct Scalars {  // device-resident control block (one per handle)
   unsigned int maxdisp2_bits;           // float bits: max_i |x_i - x_i(build)|^2
   unsigned long long vmax2_bits[2];     // double bits: max_i |v_i|^2, double-buffered by step parity
   double dt;
+  double dt_max, max_disp;              // md_step arguments (set by k_md_params)
+  int parity;                           // which vmax2 slot holds max |v|^2 of the current state
+  int trace_pos;                        // next slot of the dt trace ring
   unsigned long long bmin[3], bmax[3];  // order-preserving encodings of min/max coordinate (open axes)
   int overflow_radial, overflow_angular;  // largest neighbour counts seen at the last build
   int nonfinite;

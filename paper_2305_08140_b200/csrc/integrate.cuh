@@ -8,18 +8,49 @@
 #pragma once
 #include "common.cuh"
 
-// one thread: time step of this step from the velocity maximum left by the previous half-kick
-__global__ void k_dt(Scalars* sc, int parity, double dt_max, double max_disp, double* dt_trace,
-                     int trace_idx) {
-  double v2 = __longlong_as_double((long long)sc->vmax2_bits[parity]);  // bits of a double >= 0
+// md_step arguments live on the device so that one captured CUDA graph serves every step
+__global__ void k_md_params(Scalars* sc, double dt_max, double max_disp) {
+  sc->dt_max = dt_max;
+  sc->max_disp = max_disp;
+  sc->trace_pos = 0;
+}
+
+// time step of this step from the velocity maximum left by the previous half-kick (C-11); every
+// thread of k_kick_drift evaluates the same expression on the same bits
+__device__ __forceinline__ double step_dt(const Scalars* sc) {
+  double v2 = __longlong_as_double((long long)sc->vmax2_bits[sc->parity]);  // bits of a double >= 0
   double vmax = sqrt(v2);
-  double dt = dt_max;
-  if (vmax > 0.0 && max_disp / vmax < dt) dt = max_disp / vmax;
+  double dt = sc->dt_max;
+  if (vmax > 0.0 && sc->max_disp / vmax < dt) dt = sc->max_disp / vmax;
+  return dt;
+}
+
+// one thread, after k_kick_drift: book-keeping of the step (dt for the second half-kick and the trace,
+// flip the vmax slot) and the rebuild decision; in a captured graph it also sets the IF nodes
+__global__ void k_step_flag(Scalars* sc, float half_skin2, double* dt_trace, int trace_ring,
+                            unsigned long long cond_rebuild, int use_cond) {
+  double dt = step_dt(sc);
   sc->dt = dt;
-  sc->vmax2_bits[parity ^ 1] = 0ull;
-  sc->maxdisp2_bits = 0u;
+  int p = sc->parity;
+  sc->vmax2_bits[p ^ 1] = 0ull;
+  sc->parity = p ^ 1;
   sc->n_steps += 1;
-  if (dt_trace) dt_trace[trace_idx] = dt;
+  if (dt_trace) dt_trace[sc->trace_pos % trace_ring] = dt;
+  sc->trace_pos += 1;
+  int r = sc->force_rebuild || (__uint_as_float(sc->maxdisp2_bits) > half_skin2);
+  sc->maxdisp2_bits = 0u;  // k_kick_drift of the next step accumulates the displacement since the build again
+  sc->do_rebuild = r;
+  sc->force_rebuild = 0;
+  sc->zbl_count = 0;
+  if (r) sc->n_rebuilds += 1;
+#if defined(__CUDA_ARCH__)
+  if (use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)cond_rebuild, (unsigned)r);
+#endif
+}
+
+// one thread, after k_force: run the ZBL node of the captured graph only if an atom was flagged
+__global__ void k_zbl_gate(const Scalars* sc, unsigned long long cond_zbl) {
+  cudaGraphSetConditional((cudaGraphConditionalHandle)cond_zbl, sc->zbl_count > 0 ? 1u : 0u);
 }
 
 // first half-kick + drift + wrap + S1 (fixed-point copy into the sorted slot) + displacement since build
@@ -33,7 +64,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   float d2 = 0.0f;
   if (i < n) {
-    const double dt = sc->dt;
+    const double dt = step_dt(sc);
     int t = types ? types[i] : 0;
     double im = inv_mass[t];  // 1 / (m * 103.6426965): acceleration in A/fs^2 per eV/A
     unsigned int u[3];
@@ -63,7 +94,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
 // second half-kick; leaves max |v|^2 for the next step's dt (integer atomicMax on the bits of a
 // non-negative double is order-independent)
 __global__ void __launch_bounds__(256)
-k_kick(Scalars* sc, int parity_next, int n, double* __restrict__ vel,
+k_kick(Scalars* sc, int n, double* __restrict__ vel,
        const float* __restrict__ force, const int32_t* __restrict__ types,
        const double* __restrict__ inv_mass, int do_kick) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -88,7 +119,7 @@ k_kick(Scalars* sc, int parity_next, int n, double* __restrict__ vel,
     unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o);
     b = t > b ? t : b;
   }
-  if ((threadIdx.x & 31) == 0 && b) atomicMax(&sc->vmax2_bits[parity_next], b);
+  if ((threadIdx.x & 31) == 0 && b) atomicMax(&sc->vmax2_bits[sc->parity], b);
 }
 
 // fixed-order fp64 reductions for md_energies: per-block tree -> partial[block]; then one block.

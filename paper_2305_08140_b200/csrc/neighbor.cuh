@@ -315,6 +315,7 @@ k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restri
 // decide whether the list must be rebuilt for this evaluation; reset per-evaluation counters.
 __global__ void k_flag(Scalars* sc, float half_skin2) {
   int r = sc->force_rebuild || (__uint_as_float(sc->maxdisp2_bits) > half_skin2);
+  sc->maxdisp2_bits = 0u;
   sc->do_rebuild = r;
   sc->force_rebuild = 0;
   sc->zbl_count = 0;

@@ -76,8 +76,15 @@ struct nepzbl_handle {
   double* md_pos = nullptr;
   double* md_vel = nullptr;
   const int32_t* md_types = nullptr;
-  int parity = 0;
   long long md_steps = 0;
+
+  // one MD step captured as a CUDA graph: the list-rebuild chain and the ZBL kernel sit in IF nodes
+  // whose conditions are set on the device (k_step_flag / k_zbl_gate), so a step is ONE launch
+  cudaGraph_t step_graph = nullptr;
+  cudaGraphExec_t step_exec = nullptr;
+  cudaStream_t cap_stream = nullptr;
+  int graph_kernels = 0, graph_rebuild_kernels = 0;  // launch accounting per graph replay
+  bool use_graph = true;
 
   // per-kernel CUDA-event timing (nep_zbl_profile)
   bool prof = false;
@@ -234,10 +241,10 @@ void prof_mark(nepzbl_handle* h, int id) {
 // ------------------------------------------------------------------ kernel sequences
 
 // S2 chain; every kernel exits immediately unless Scalars::do_rebuild is set.
-void enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types) {
+int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, cudaStream_t st) {
   const Carve& c = h->cv;
   const int n = (int)h->n, npad = c.npad;
-  cudaStream_t st = h->stream;
+  int nk = 0;
   BoxHost bh;
   for (int a = 0; a < 3; ++a) {
     bh.L[a] = h->box[4 * a];
@@ -248,12 +255,11 @@ void enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types) 
   float rr = (float)(bh.rcs * bh.rcs);
   double ra = h->p.rc_angular + h->p.skin;
   float ra2 = (float)(ra * ra);
-  prof_mark(h, PK_REBUILD);
   k_rebuild_begin<<<1, 1, 0, st>>>(h->d_sc);
-  h->launches++;
+  nk++;
   if (!(h->pbc[0] && h->pbc[1] && h->pbc[2])) {
     k_bounds<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, pos, !h->pbc[0], !h->pbc[1], !h->pbc[2]);
-    h->launches++;
+    nk++;
   }
   k_boxmap<<<1, 1, 0, st>>>(h->d_sc, h->d_bm, bh);
   k_zero_cells<<<blocks(c.ncell_cap + 1, 256), 256, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count),
@@ -274,13 +280,13 @@ void enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types) 
                                        h->at<int>(c.nn_a), h->at<int>(c.nl_a));
   k_rev<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, n, npad, h->at<int>(c.nn_a), h->at<int>(c.nl_a),
                                        h->at<unsigned char>(c.rev));
-  h->launches += 9;
+  return nk + 9;
 }
 
 // S3-S7 (+S5): outputs in the caller's order; any of energy/force/virial may be null.
 template <class MS>
 void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
-                    bool want_q) {
+                    bool want_q, bool with_zbl) {
   const Carve& c = h->cv;
   const int n = (int)h->n, npad = c.npad;
   cudaStream_t st = h->stream;
@@ -307,7 +313,7 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
         h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
         h->at<unsigned>(c.rmask), mask_words(h->p), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
   h->launches += 3;
-  if (h->p.zbl_enabled) {
+  if (h->p.zbl_enabled && with_zbl) {
     prof_mark(h, PK_ZBL);
     k_zbl<<<32, 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), n, npad, h->at<int4>(c.xyzt),
                             h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp,
@@ -318,9 +324,15 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
 }
 
 void enqueue_eval(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
-                  bool want_q) {
-  if (h->shape == 0) enqueue_eval_t<MS0>(h, pos, energy, force, virial, want_q);
-  else enqueue_eval_t<MS1>(h, pos, energy, force, virial, want_q);
+                  bool want_q, bool with_zbl = true) {
+  if (h->shape == 0) enqueue_eval_t<MS0>(h, pos, energy, force, virial, want_q, with_zbl);
+  else enqueue_eval_t<MS1>(h, pos, energy, force, virial, want_q, with_zbl);
+}
+
+void enqueue_zbl(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial, cudaStream_t st) {
+  const Carve& c = h->cv;
+  k_zbl<<<32, 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), (int)h->n, c.npad, h->at<int4>(c.xyzt),
+                          h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp, energy, force, virial);
 }
 
 int read_scalars(nepzbl_handle* h) {
@@ -423,7 +435,8 @@ int eval_common(nepzbl_handle* h, long long n, const double* pos, const int32_t*
   }
   k_flag<<<1, 1, 0, h->stream>>>(h->d_sc, hs * hs);
   h->launches += 2;
-  enqueue_rebuild(h, pos, types);
+  prof_mark(h, PK_REBUILD);
+  h->launches += enqueue_rebuild(h, pos, types, h->stream);
   if (do_eval) enqueue_eval(h, pos, energy, force, virial, want_q);
   rc = read_scalars(h);
   if (rc) return rc;
@@ -528,6 +541,9 @@ void nep_zbl_destroy(nepzbl_handle* h) {
   cudaFree(h->d_trace); cudaFree(h->d_esum);
   cudaFreeHost(h->h_sc); cudaFreeHost(h->h_trace); cudaFreeHost(h->h_esum);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
+  if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
+  if (h->step_graph) cudaGraphDestroy(h->step_graph);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   delete h;
 }
 
@@ -626,6 +642,8 @@ int nep_zbl_get_descriptors(nepzbl_handle* h, float* q) {
 
 // ---------------------------------------------------------------------------------- MD
 
+static bool build_step_graph(nepzbl_handle* h);
+
 int md_init(nepzbl_handle* h, int64_t n, double* pos, double* vel, const int32_t* types,
             const double box[9], const int32_t pbc[3]) {
   if (!h) return NEPZBL_E_INVALID_ARG;
@@ -640,54 +658,169 @@ int md_init(nepzbl_handle* h, int64_t n, double* pos, double* vel, const int32_t
   h->md_pos = pos;
   h->md_vel = vel;
   h->md_types = types;
-  h->parity = 0;
   h->md_steps = 0;
   rc = eval_common(h, n, pos, types, box, pbc, h->at<double>(c.md_energy), h->at<float>(c.md_force),
                    nullptr, true, false, true);
   if (rc) return rc;
-  k_kick<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, 0, (int)n, vel, h->at<float>(c.md_force), types,
+  k_kick<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, (int)n, vel, h->at<float>(c.md_force), types,
                                                 h->d_inv_mass, 0);
   h->launches++;
   CU(cudaStreamSynchronize(h->stream));
   CU(cudaGetLastError());
+  if (h->use_graph && !build_step_graph(h)) h->use_graph = false;  // falls back to plain stream launches
   h->md_ready = true;
   return NEPZBL_OK;
 }
 
-static void enqueue_md_step(nepzbl_handle* h, double dt_max, double max_disp, int trace_idx) {
+// One MD step as plain stream launches (profiling mode, or when graph capture is unavailable).
+static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
   const Carve& c = h->cv;
   const int n = (int)h->n;
   cudaStream_t st = h->stream;
   float hs = (float)(0.5 * h->p.skin);
   prof_mark(h, PK_INTEGRATE_A);
-  k_dt<<<1, 1, 0, st>>>(h->d_sc, h->parity, dt_max, max_disp, trace_idx >= 0 ? h->d_trace : nullptr,
-                        trace_idx >= 0 ? trace_idx : 0);
   k_kick_drift<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, h->md_pos, h->md_vel,
                                               h->at<float>(c.md_force), h->md_types, h->d_inv_mass,
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                               h->at<int4>(c.xyzt_build));
-  k_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs);
-  h->launches += 3;
-  enqueue_rebuild(h, h->md_pos, h->md_types);
+  k_step_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0);
+  h->launches += 2;
+  prof_mark(h, PK_REBUILD);
+  h->launches += enqueue_rebuild(h, h->md_pos, h->md_types, st);
   enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false);
   prof_mark(h, PK_KICK);
-  k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->parity ^ 1, n, h->md_vel, h->at<float>(c.md_force),
-                                        h->md_types, h->d_inv_mass, 1);
+  k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->md_vel, h->at<float>(c.md_force), h->md_types,
+                                        h->d_inv_mass, 1);
   prof_mark(h, -1);
   h->launches++;
-  h->parity ^= 1;
-  h->md_steps++;
+}
+
+static void destroy_step_graph(nepzbl_handle* h) {
+  if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
+  if (h->step_graph) cudaGraphDestroy(h->step_graph);
+  h->step_exec = nullptr;
+  h->step_graph = nullptr;
+}
+
+// Capture one MD step into a CUDA graph:
+//   k_kick_drift -> k_step_flag -> IF(rebuild){S2 chain} -> k_radial -> k_angular_nn -> k_force
+//   -> k_zbl_gate -> IF(zbl_count > 0){k_zbl} -> k_kick
+// Returns false (and leaves the stream path in use) if any capture call fails.
+static bool build_step_graph(nepzbl_handle* h) {
+  destroy_step_graph(h);
+  const Carve& c = h->cv;
+  const int n = (int)h->n;
+  cudaStream_t st = h->stream;
+  float hs = (float)(0.5 * h->p.skin);
+  if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
+  cudaGraph_t g = nullptr;
+  if (cudaGraphCreate(&g, 0) != cudaSuccess) return false;
+  cudaGraphConditionalHandle h_reb, h_zbl;
+  bool ok = cudaGraphConditionalHandleCreate(&h_reb, g, 0, cudaGraphCondAssignDefault) == cudaSuccess &&
+            cudaGraphConditionalHandleCreate(&h_zbl, g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+  ok = ok && cudaStreamBeginCaptureToGraph(st, g, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+  if (!ok) { cudaGraphDestroy(g); cudaGetLastError(); return false; }
+  bool saved_prof = h->prof;
+  h->prof = false;
+  long long saved_launches = h->launches;
+  auto add_if = [&](cudaGraphConditionalHandle handle, cudaGraph_t* body) -> bool {
+    cudaStreamCaptureStatus status;
+    const cudaGraphNode_t* deps = nullptr;
+    size_t ndeps = 0;
+    cudaGraph_t cg = nullptr;
+    if (cudaStreamGetCaptureInfo(st, &status, nullptr, &cg, &deps, &ndeps) != cudaSuccess) return false;
+    cudaGraphNodeParams np = {};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = handle;
+    np.conditional.type = cudaGraphCondTypeIf;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    if (cudaGraphAddNode(&node, g, deps, ndeps, &np) != cudaSuccess) return false;
+    *body = np.conditional.phGraph_out[0];
+    return cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies) == cudaSuccess;
+  };
+  int nk = 0, nk_reb = 0;
+  k_kick_drift<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, h->md_pos, h->md_vel,
+                                              h->at<float>(c.md_force), h->md_types, h->d_inv_mass,
+                                              h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
+                                              h->at<int4>(c.xyzt_build));
+  k_step_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1);
+  nk += 2;
+  cudaGraph_t body = nullptr;
+  ok = add_if(h_reb, &body);
+  if (ok) {
+    ok = cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+      nk_reb = enqueue_rebuild(h, h->md_pos, h->md_types, h->cap_stream);
+      ok = cudaStreamEndCapture(h->cap_stream, nullptr) == cudaSuccess;
+    }
+  }
+  if (ok) {
+    enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false, false);
+    nk += 3;
+    if (h->p.zbl_enabled) {
+      k_zbl_gate<<<1, 1, 0, st>>>(h->d_sc, (unsigned long long)h_zbl);
+      nk += 1;
+      ok = add_if(h_zbl, &body);
+      if (ok) {
+        ok = cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+        if (ok) {
+          enqueue_zbl(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, h->cap_stream);
+          ok = cudaStreamEndCapture(h->cap_stream, nullptr) == cudaSuccess;
+        }
+      }
+    }
+    k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->md_vel, h->at<float>(c.md_force), h->md_types,
+                                          h->d_inv_mass, 1);
+    nk += 1;
+  }
+  cudaGraph_t captured = nullptr;
+  cudaError_t ee = cudaStreamEndCapture(st, &captured);
+  h->prof = saved_prof;
+  h->launches = saved_launches;
+  ok = ok && ee == cudaSuccess;
+  if (ok) ok = cudaGraphInstantiate(&h->step_exec, g, 0) == cudaSuccess;
+  if (!ok) {
+    cudaGraphDestroy(g);
+    h->step_exec = nullptr;
+    cudaGetLastError();
+    return false;
+  }
+  h->step_graph = g;
+  h->graph_kernels = nk;
+  h->graph_rebuild_kernels = nk_reb;
+  return true;
+}
+
+// enqueue n_steps steps; dt_trace requests the device trace ring to be filled
+static int enqueue_md_steps(nepzbl_handle* h, int n_steps, bool trace) {
+  const bool graph = h->use_graph && !h->prof && h->step_exec;
+  for (int k = 0; k < n_steps; ++k) {
+    if (graph) {
+      CU(cudaGraphLaunch(h->step_exec, h->stream));
+      h->launches += h->graph_kernels;
+    } else {
+      enqueue_md_step_stream(h, trace);
+    }
+    h->md_steps++;
+  }
+  return NEPZBL_OK;
 }
 
 int md_step(nepzbl_handle* h, double dt_max, double max_displacement, double* dt_used, int32_t* rebuilt) {
   if (!h) return NEPZBL_E_INVALID_ARG;
   if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_step before md_init");
   if (!(dt_max > 0) || !(max_displacement > 0)) return fail(h, NEPZBL_E_INVALID_ARG, "dt_max and max_displacement must be > 0");
-  enqueue_md_step(h, dt_max, max_displacement, -1);
-  int rc = read_scalars(h);
+  k_md_params<<<1, 1, 0, h->stream>>>(h->d_sc, dt_max, max_displacement);
+  h->launches++;
+  int rc = enqueue_md_steps(h, 1, false);
+  if (rc) return rc;
+  rc = read_scalars(h);
   if (rc) return rc;
   if (dt_used) *dt_used = h->h_sc->dt;
   if (rebuilt) *rebuilt = h->h_sc->do_rebuild;
+  if (h->h_sc->do_rebuild && h->use_graph && !h->prof && h->step_exec) h->launches += h->graph_rebuild_kernels;
+  if (h->h_sc->zbl_count > 0 && h->use_graph && !h->prof && h->step_exec) h->launches += 1;
   rc = check_device_flags(h);
   if (rc) h->md_ready = false;
   return rc;
@@ -701,13 +834,19 @@ int md_run(nepzbl_handle* h, int64_t n_steps, double dt_max, double max_displace
   int rc = read_scalars(h);
   if (rc) return rc;
   long long reb0 = h->h_sc->n_rebuilds;
+  const bool graph = h->use_graph && !h->prof && h->step_exec;
   for (int64_t done = 0; done < n_steps;) {
     int chunk = (int)std::min<int64_t>(kTraceRing, n_steps - done);
-    for (int k = 0; k < chunk; ++k) enqueue_md_step(h, dt_max, max_displacement, k);
+    long long reb_before = h->h_sc->n_rebuilds;
+    k_md_params<<<1, 1, 0, h->stream>>>(h->d_sc, dt_max, max_displacement);  // also rewinds the trace ring
+    h->launches++;
+    rc = enqueue_md_steps(h, chunk, true);
+    if (rc) return rc;
     if (dt_trace) CU(cudaMemcpyAsync(h->h_trace, h->d_trace, chunk * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     rc = read_scalars(h);
     if (rc) return rc;
     if (dt_trace) memcpy(dt_trace + done, h->h_trace, chunk * sizeof(double));
+    if (graph) h->launches += (h->h_sc->n_rebuilds - reb_before) * h->graph_rebuild_kernels;
     rc = check_device_flags(h);
     if (rc) { h->md_ready = false; return rc; }
     done += chunk;
