@@ -24,6 +24,7 @@ struct BoxMap {  // device-resident; recomputed by k_boxmap at every list rebuil
   int nc[3];        // cells per axis actually used
   int ncv[3];       // cell index = (u * ncv) >> 32
   int ncells;
+  int S;            // stencil half-width in cells: cells have edge >= (rc_radial+skin)/S
 };
 
 struct Scalars {  // device-resident control block (one per handle)

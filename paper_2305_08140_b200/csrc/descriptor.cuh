@@ -45,20 +45,32 @@ struct ModelTables {
   int n_neurons;
 };
 
-struct __align__(32) AtomRec {  // compute copy + radial back-pass input of one atom (sorted order)
-  int ux, uy, uz;                // fixed-point coordinates (same as xyzt)
-  float fp[5];                   // Fp[n] = dU/dq_n of the radial descriptor components
+// Record of one atom for the radial back-pass of k_force (sorted order), 64-byte stride so that it
+// never straddles a 128-byte line: {ux,uy,uz,d0..d4 | d5..d11 pad}.  d[k] = sum_n Fp[n] ct_nk are the
+// atom's radial back-pass coefficients.  Fetched per pair with one 256-bit and one 128-bit load (two
+// sectors of one line) -- k_force is bound by L1 tag lookups of scattered gathers when it gathers
+// more, and by FP32 issue when it re-derives d from Fp per pair (both measured, profiles/).
+struct __align__(64) AtomRec {
+  int ux, uy, uz;  // fixed-point coordinates (same as xyzt)
+  float d[12];     // d[0..KR-1]; rest zero
+  float pad;
 };
-__device__ __forceinline__ AtomRec ld_rec(const AtomRec* p) {
-  AtomRec r;
+__device__ __forceinline__ void ld_rec(const AtomRec* p, int& ux, int& uy, int& uz, float d[12], int kr) {
   unsigned v0, v1, v2, v3, v4, v5, v6, v7;
   asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3), "=r"(v4), "=r"(v5), "=r"(v6), "=r"(v7)
                : "l"(p));
-  r.ux = (int)v0; r.uy = (int)v1; r.uz = (int)v2;
-  r.fp[0] = __uint_as_float(v3); r.fp[1] = __uint_as_float(v4); r.fp[2] = __uint_as_float(v5);
-  r.fp[3] = __uint_as_float(v6); r.fp[4] = __uint_as_float(v7);
-  return r;
+  ux = (int)v0; uy = (int)v1; uz = (int)v2;
+  d[0] = __uint_as_float(v3); d[1] = __uint_as_float(v4); d[2] = __uint_as_float(v5);
+  d[3] = __uint_as_float(v6); d[4] = __uint_as_float(v7);
+  float4 t = __ldg(reinterpret_cast<const float4*>(p) + 2);
+  d[5] = t.x; d[6] = t.y; d[7] = t.z; d[8] = t.w;
+  if (kr > 9) {
+    float4 u = __ldg(reinterpret_cast<const float4*>(p) + 3);
+    d[9] = u.x; d[10] = u.y; d[11] = u.z;
+  } else {
+    d[9] = d[10] = d[11] = 0.0f;
+  }
 }
 
 // (2l+1)/(4 pi) * addition-theorem weight of each b_lm (see DESIGN.md for the list of b_lm)
@@ -204,8 +216,8 @@ __device__ __forceinline__ float tanh_fast(float z) {
 // RADIAL_LANES lanes per atom: lane p owns list entries p, p+4, ...  The gathers are latency-bound
 // (ncu: long-scoreboard stalls on the dependent index -> position loads), so every lane issues 4
 // independent index loads and 4 independent position gathers per iteration before any arithmetic.
-// Which of a lane's entries are inside the cutoff is kept as a bit mask (bit b <-> entry p + 4 b) and
-// handed to k_force, which then gathers only those.  The K basis sums are combined over the 4 lanes
+// Which of a lane's entries are inside the cutoff is kept as a bit mask (word w, bit b <-> entry
+// p + 4 (32 w + b)) and handed to k_force, which then gathers only those.  The K basis sums are combined over the 4 lanes
 // by a fixed-order shuffle tree (deterministic).
 #define RADIAL_LANES 4
 #define RADIAL_UNROLL 4
@@ -417,15 +429,21 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restr
   for (int v = 0; v < D; ++v) Fp[v] *= s_qs[v];
   u_site[s] = U;
 
-  // record for the radial back-pass of k_force: position + Fp of the radial components
+  // record for the radial back-pass of k_force: position + d_k = sum_n Fp_n ct_nk
   {
-    static_assert(NR <= 5, "AtomRec holds 5 radial Fp components");
-    float f[5] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+    static_assert(KR <= 12, "AtomRec holds 12 coefficients");
+    float d[12];
 #pragma unroll
-    for (int nq = 0; nq < NR; ++nq) f[nq] = Fp[nq];
-    int4* rp = reinterpret_cast<int4*>(rec + s);
-    rp[0] = make_int4(me.x, me.y, me.z, __float_as_int(f[0]));
-    rp[1] = make_int4(__float_as_int(f[1]), __float_as_int(f[2]), __float_as_int(f[3]), __float_as_int(f[4]));
+    for (int k = 0; k < 12; ++k) d[k] = 0.0f;
+#pragma unroll
+    for (int k = 0; k < KR; ++k)
+#pragma unroll
+      for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
+    float4* rp = reinterpret_cast<float4*>(rec + s);
+    rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
+    rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+    rp[2] = make_float4(d[5], d[6], d[7], d[8]);
+    if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
   }
 
   // ---- E[n][lm] = dU/dA[n][lm] (in place)

@@ -1,12 +1,10 @@
 // force.cuh -- S7 (force / virial accumulation, gather form) and S5 (ZBL pair term).
 //
 // S7:  F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji),  W_i = sum_j r_ij (x) dU_j/dr_ji.
-//   radial part:  dU_i/dr_ij = rhat_ij sum_n Fp_i[n] g_n'(r_ij), so F_i += rhat_ij sum_n (Fp_i[n] + Fp_j[n]) g_n'.
-//                 Per pair ONE 32-byte gather: the neighbour's record {ux,uy,uz,Fp[0..4]} written by
-//                 k_angular_nn, fetched with a single 256-bit load (LDG.E.256, new on sm_100).  The kernel
-//                 is bound by L1 tag lookups of these scattered gathers (ncu, profiles/), so the record
-//                 is kept to one sector and g_n' is re-evaluated on the ALUs instead of gathering 48 B of
-//                 pre-contracted coefficients;
+//   radial part:  dU_i/dr_ij = rhat_ij sum_k d_i[k] (f_c T_k)'(r_ij), d_i[k] = sum_n Fp_i[n] ct_nk,
+//                 so F_i += rhat_ij sum_k (d_i[k] + d_j[k]) (f_c T_k)'.  Per pair the neighbour's
+//                 record {position, d_j} (AtomRec, one 128-byte line) is gathered with a 256-bit
+//                 (LDG.E.256, new on sm_100) and a 128-bit load;
 //   angular part: partial forces stored by k_angular_nn; F_i += p[i][a] - p[j][rev[i][a]].
 //   Gather form only: every atom sums its own pairs in list order -> no float atomics, bitwise
 //   reproducible.
@@ -28,13 +26,15 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
         const unsigned* __restrict__ rmask, int mask_words, const float4* __restrict__ pforce, const float* __restrict__ u_site,
         const int* __restrict__ perm, double* __restrict__ energy, float* __restrict__ force,
         float* __restrict__ virial) {
-  constexpr int KR = MS::KR, NR = MS::NR;
-  static_assert(NR <= 5, "AtomRec holds 5 radial Fp components");
+  constexpr int KR = MS::KR;
+  static_assert(KR <= 12, "AtomRec holds 12 coefficients");
   const int gt = blockIdx.x * blockDim.x + threadIdx.x;
   const int s = gt / FORCE_LANES, sub = gt % FORCE_LANES;
   const bool valid = s < n;
   const int sc_ = valid ? s : 0;
-  const AtomRec me = ld_rec(rec + sc_);
+  struct Rec { int ux, uy, uz; float d[12]; };
+  Rec me;
+  ld_rec(rec + sc_, me.ux, me.uy, me.uz, me.d, KR);
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
   float fx = 0.0f, fy = 0.0f, fz = 0.0f;
   float w[9];
@@ -59,35 +59,50 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       return lp[(size_t)(32 * word + b) * lstride];
     };
     int j_cur = next_j();
-    AtomRec o_cur = ld_rec(rec + (j_cur >= 0 ? j_cur : sc_));
+    Rec o_cur, o_nxt;
+    ld_rec(rec + (j_cur >= 0 ? j_cur : sc_), o_cur.ux, o_cur.uy, o_cur.uz, o_cur.d, KR);
     int j_nxt = j_cur >= 0 ? next_j() : -1;
     while (j_cur >= 0) {
-      AtomRec o_nxt = ld_rec(rec + (j_nxt >= 0 ? j_nxt : sc_));
+      ld_rec(rec + (j_nxt >= 0 ? j_nxt : sc_), o_nxt.ux, o_nxt.uy, o_nxt.uz, o_nxt.d, KR);
       int j_nn = j_nxt >= 0 ? next_j() : -1;
-      const AtomRec& o = o_cur;
+      const Rec& o = o_cur;
       float dx = (float)(o.ux - me.ux) * hx, dy = (float)(o.uy - me.uy) * hy, dz = (float)(o.uz - me.uz) * hz;
       float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
       float rinv = rsqrtf(r2), r = r2 * rinv;
       float fc, dfc, x, dxdr, T[KR], Uc[KR];
       cheb_T<KR>(r, mt.inv_rcR, fc, dfc, x, dxdr, T);
       cheb_U<KR>(x, Uc);
-      // g_n'(r) = f_c' sum_k ct_nk T_k + f_c x' sum_{k>=1} k ct_nk U_{k-1}
+      // sum_k d[k] (f_c T_k)' = f_c' sum_k d[k] T_k + f_c x' sum_{k>=1} d[k] k U_{k-1}
       const float e = fc * dxdr;
-      float gi = 0.0f, gj = 0.0f;
+      float gi, gj = 0.0f;
+      if (VIRIAL) {
+        float ai = 0.0f, bi = 0.0f, aj = 0.0f, bj = 0.0f;
 #pragma unroll
-      for (int nq = 0; nq < NR; ++nq) {
-        float p = 0.0f, dp = 0.0f;
-#pragma unroll
-        for (int k = 0; k < KR; ++k) p = fmaf(mt.ctR[nq][k], T[k], p);
-#pragma unroll
-        for (int k = 1; k < KR; ++k) dp = fmaf(mt.kctR[nq][k], Uc[k - 1], dp);
-        float dg = fmaf(dfc, p, e * dp);
-        if (VIRIAL) {
-          gi = fmaf(me.fp[nq], dg, gi);  // dU_i/dr along rhat_ij
-          gj = fmaf(o.fp[nq], dg, gj);   // dU_j/dr along rhat_ji (same scalar form)
-        } else {
-          gi = fmaf(me.fp[nq] + o.fp[nq], dg, gi);
+        for (int k = 0; k < KR; ++k) {
+          ai = fmaf(me.d[k], T[k], ai);
+          aj = fmaf(o.d[k], T[k], aj);
         }
+#pragma unroll
+        for (int k = 1; k < KR; ++k) {
+          float ku = (float)k * Uc[k - 1];
+          bi = fmaf(me.d[k], ku, bi);
+          bj = fmaf(o.d[k], ku, bj);
+        }
+        gi = fmaf(dfc, ai, e * bi);  // dU_i/dr along rhat_ij
+        gj = fmaf(dfc, aj, e * bj);  // dU_j/dr along rhat_ji (same scalar form)
+      } else {
+        // forces only need g_i + g_j: contract once with d_i + d_j (two partial sums each for ILP)
+        float a0 = 0.0f, a1 = 0.0f, b0 = 0.0f, b1 = 0.0f;
+#pragma unroll
+        for (int k = 0; k < KR; ++k) {
+          float ds = me.d[k] + o.d[k];
+          if (k & 1) a1 = fmaf(ds, T[k], a1); else a0 = fmaf(ds, T[k], a0);
+          if (k >= 1) {
+            float ku = (float)k * Uc[k - 1];
+            if (k & 1) b1 = fmaf(ds, ku, b1); else b0 = fmaf(ds, ku, b0);
+          }
+        }
+        gi = fmaf(dfc, a0 + a1, e * (b0 + b1));
       }
       float fs = (gi + gj) * rinv;
       fx = fmaf(fs, dx, fx);

@@ -1,11 +1,16 @@
 // neighbor.cuh -- S1 (state prep) and S2 (cell-list neighbour build) kernels.
 //
 // S2 (BASELINE.json north_star "cell-list neighbour build"; cutoffs P:106):
-//   bin atoms into cells of edge >= rc_radial+skin, canonical in-cell order (ascending caller
-//   index), then per atom walk the 27 surrounding cells and list every j with
+//   bin atoms into cells of edge >= (rc_radial+skin)/S (S = 2 when every periodic axis then holds >= 5
+//   cells, else 1), canonical in-cell order (ascending caller index), then per atom walk the (2S+1)^3
+//   surrounding cells (z, y, x ascending) and list every j with
 //   r_ij < rc_radial+skin (radial list) and the subset r_ij < rc_angular+skin (angular list).
-// Every rebuild kernel early-exits unless Scalars::do_rebuild is set, so the MD loop can enqueue
-// the whole chain each step with no host round trip.
+// Half-size cells are used for two reasons: fewer candidates per atom (342 instead of 590 in bcc W),
+// and -- because the atoms are STORED in cell order, x fastest -- consecutive list entries are then
+// mostly adjacent in memory, so the 4 lanes that share an atom in the force kernels gather from the
+// same 128-byte lines (the force kernels are bound by L1 wavefronts of scattered gathers, profiles/).
+// Every rebuild kernel early-exits unless Scalars::do_rebuild is set (the stream path enqueues the
+// chain every step; the graph path puts it in an IF node).
 // Determinism: integer atomics only (counts / slot tickets); the ticket order is erased by the
 // per-cell sort, so the sorted order and the lists are reproducible bit for bit.
 #pragma once
@@ -47,51 +52,66 @@ __global__ void k_rebuild_begin(Scalars* sc) {
   sc->maxdisp2_bits = 0u;
 }
 
-// Fixed-point grid and cell grid for this build (one thread).
+// Fixed-point grid and cell grid for cells of edge >= rcs * f / S.  Returns the number of cells, or
+// -1 if a periodic axis cannot hold the 2S+1 distinct stencil cells that S == 2 needs.
+__device__ long long make_grid(Scalars* sc, BoxMap* bm, const BoxHost& bh, int S, int f) {
+  const double two32 = 4294967296.0;
+  const double cw = bh.rcs * f / S;
+  long long total = 1;
+  for (int a = 0; a < 3; ++a) {
+    bm->pbc[a] = bh.pbc[a];
+    bm->L[a] = bh.L[a];
+    double span, lo;
+    int nc, ncv;
+    if (bh.pbc[a]) {
+      lo = 0.0;
+      span = bh.L[a];
+      nc = (int)floor(bh.L[a] / cw);
+      if (S == 2 && nc < 5) return -1;
+      if (f == 1 && nc < 2) sc->box_too_small = 1;
+      if (nc < 1) nc = 1;
+      ncv = nc;
+    } else {
+      // open axis (SURVEY C-14): grid spans the atoms' bounding range plus margins of rcs; the 2^32
+      // span is twice that, so int32 differences never wrap for real pairs.
+      double mn = dec_double(sc->bmin[a]), mx = dec_double(sc->bmax[a]);
+      if (!(mx >= mn)) { mn = 0.0; mx = 0.0; }
+      double E = mx - mn, M = bh.rcs * f;
+      ncv = (int)ceil(2.0 * (E + 2.0 * M) / cw);
+      if (ncv < 2) ncv = 2;
+      span = ncv * cw;
+      lo = mn - M;
+      nc = (int)floor((M + E) / cw) + 1;
+      if (nc > ncv) nc = ncv;
+    }
+    bm->lo[a] = lo;
+    bm->inv_h[a] = two32 / span;
+    bm->h[a] = span / two32;
+    bm->hf[a] = (float)(span / two32);
+    bm->nc[a] = nc;
+    bm->ncv[a] = ncv;
+    total *= nc;
+  }
+  return total;
+}
+
+// Choose the grid for this build (one thread): half-size cells (S = 2) if they fit, else full-size
+// cells (S = 1); coarsen (f = 2, 4, ...) only if the cell arrays are too small for the volume.
 __global__ void k_boxmap(Scalars* sc, BoxMap* bm, BoxHost bh) {
   if (!sc->do_rebuild) return;
-  const double two32 = 4294967296.0;
-  for (int f = 1;; f *= 2) {  // coarsen cells until the grid fits the cell arrays
-    double cw = bh.rcs * f;
-    long long total = 1;
-    for (int a = 0; a < 3; ++a) {
-      bm->pbc[a] = bh.pbc[a];
-      bm->L[a] = bh.L[a];
-      double span, lo;
-      int nc, ncv;
-      if (bh.pbc[a]) {
-        lo = 0.0;
-        span = bh.L[a];
-        nc = (int)floor(bh.L[a] / cw);
-        if (f == 1 && nc < 2) sc->box_too_small = 1;
-        if (nc < 1) nc = 1;
-        ncv = nc;
-      } else {
-        // open axis (SURVEY C-14): grid spans the atoms' bounding range plus margins; the 2^32
-        // span is twice that, so int32 differences never wrap for real pairs.
-        double mn = dec_double(sc->bmin[a]), mx = dec_double(sc->bmax[a]);
-        if (!(mx >= mn)) { mn = 0.0; mx = 0.0; }
-        double E = mx - mn, M = cw;
-        ncv = (int)ceil(2.0 * (E + 2.0 * M) / cw);
-        if (ncv < 2) ncv = 2;
-        span = ncv * cw;
-        lo = mn - M;
-        nc = (int)floor((M + E) / cw) + 1;
-        if (nc > ncv) nc = ncv;
+  for (int S = 2; S >= 1; --S) {
+    for (int f = 1; f <= (1 << 20); f *= 2) {
+      long long total = make_grid(sc, bm, bh, S, f);
+      if (total < 0) break;  // S = 2 does not fit this box: try S = 1
+      if (total <= bh.ncell_cap) {
+        bm->ncells = (int)total;
+        bm->S = S;
+        return;
       }
-      bm->lo[a] = lo;
-      bm->inv_h[a] = two32 / span;
-      bm->h[a] = span / two32;
-      bm->hf[a] = (float)(span / two32);
-      bm->nc[a] = nc;
-      bm->ncv[a] = ncv;
-      total *= nc;
-    }
-    if (total <= bh.ncell_cap || f >= (1 << 20)) {
-      bm->ncells = (int)(total <= bh.ncell_cap ? total : bh.ncell_cap);
-      break;
     }
   }
+  bm->ncells = 1;  // unreachable for finite boxes; keeps the chain well-defined
+  bm->S = 1;
 }
 
 __global__ void k_zero_cells(const Scalars* sc, const BoxMap* bm, int* cell_count, int* cell_fill,
@@ -197,8 +217,24 @@ __global__ void k_permute(const Scalars* sc, int n, const int* __restrict__ orde
   xyzt_build[s] = v;
 }
 
-// neighbour cells along one axis: up to 3 distinct indices, -1 = none
-__device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int out[3]) {
+// neighbour cells along one axis: up to 2S+1 distinct indices in out[0..2S], -1 = none
+__device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int S, int out[5]) {
+#pragma unroll
+  for (int k = 0; k < 5; ++k) out[k] = -1;
+  if (S == 2) {  // periodic axes hold >= 5 cells (k_boxmap), so the wrapped indices are distinct
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      int v = c + k - 2;
+      if (pbc) {
+        if (v < 0) v += nc;
+        if (v >= nc) v -= nc;
+      } else if (v < 0 || v >= nc) {
+        v = -1;
+      }
+      out[k] = v;
+    }
+    return;
+  }
   out[0] = c - 1;
   out[1] = c;
   out[2] = c + 1;
@@ -218,7 +254,7 @@ __device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int out[3])
   }
 }
 
-// per atom (sorted order): walk the 27 cells, emit radial and angular lists (column-major).
+// per atom (sorted order): walk the (2S+1)^3 cells, emit radial and angular lists (column-major).
 __global__ void __launch_bounds__(128)
 k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
       const int* __restrict__ cell_start, float rcs2_radial, float rcs2_angular, int cap_r, int cap_a,
@@ -228,16 +264,17 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
   if (s >= n) return;
   const int4 me = xyzt[s];
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
-  int sx[3], sy[3], sz[3];
-  axis_stencil(cell_of_u((unsigned)me.x, bm->ncv[0], bm->nc[0]), bm->nc[0], bm->pbc[0], sx);
-  axis_stencil(cell_of_u((unsigned)me.y, bm->ncv[1], bm->nc[1]), bm->nc[1], bm->pbc[1], sy);
-  axis_stencil(cell_of_u((unsigned)me.z, bm->ncv[2], bm->nc[2]), bm->nc[2], bm->pbc[2], sz);
+  const int S = bm->S, W = 2 * S + 1;
+  int sx[5], sy[5], sz[5];
+  axis_stencil(cell_of_u((unsigned)me.x, bm->ncv[0], bm->nc[0]), bm->nc[0], bm->pbc[0], S, sx);
+  axis_stencil(cell_of_u((unsigned)me.y, bm->ncv[1], bm->nc[1]), bm->nc[1], bm->pbc[1], S, sy);
+  axis_stencil(cell_of_u((unsigned)me.z, bm->ncv[2], bm->nc[2]), bm->nc[2], bm->pbc[2], S, sz);
   int cr = 0, ca = 0;
-  for (int kz = 0; kz < 3; ++kz) {
+  for (int kz = 0; kz < W; ++kz) {
     if (sz[kz] < 0) continue;
-    for (int ky = 0; ky < 3; ++ky) {
+    for (int ky = 0; ky < W; ++ky) {
       if (sy[ky] < 0) continue;
-      for (int kx = 0; kx < 3; ++kx) {
+      for (int kx = 0; kx < W; ++kx) {
         if (sx[kx] < 0) continue;
         int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
         int b = cell_start[c], e = cell_start[c + 1];

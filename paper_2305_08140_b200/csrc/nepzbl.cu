@@ -129,7 +129,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   long long npad = (n_cap + 127) / 128 * 128;
   if (npad < 128) npad = 128;
   c.npad = (int)npad;
-  c.ncell_cap = (int)(n_cap / 4 + 8192);
+  c.ncell_cap = (int)(n_cap + 8192);  // half-size cells hold ~2.7 atoms in bcc W
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = al(o + bytes); return r; };
   c.xyzt = take(16 * npad);
@@ -149,7 +149,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.rev = take((size_t)p.cap_angular * npad);
   c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
   c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
-  c.dk = take(32 * npad);  // AtomRec
+  c.dk = take(64 * npad);  // AtomRec
   c.pforce = take(16 * (size_t)p.cap_angular * npad);
   c.u_site = take(4 * npad);
   c.q_desc = take(4 * (size_t)D * npad);
