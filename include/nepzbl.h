@@ -140,6 +140,9 @@ int nep_zbl_get_descriptors(nepzbl_handle *h, float *q);
  * md_run: n_steps such steps with no host round trip in between; dt_trace (host, [n_steps]) and
  *   n_rebuilds (host) may be NULL.
  * max_displacement may be +inf (fixed dt = dt_max).
+ * A step is replayed as ONE CUDA graph (rebuild chain and ZBL kernel in device-set IF nodes).  ncu
+ * cannot see kernels inside conditional graphs: the environment variable NEPZBL_NO_GRAPH=1, read
+ * at nep_zbl_create, issues the same kernels as plain stream launches instead (same results).
  */
 int md_init(nepzbl_handle *h, int64_t n, double *pos_soa, double *vel_soa, const int32_t *types,
             const double box[9], const int32_t pbc[3]);

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -490,6 +491,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   h->shape = shape;
   h->device = device;
   h->stream = (cudaStream_t)cuda_stream;
+  if (const char* ng = getenv("NEPZBL_NO_GRAPH")) h->use_graph = !(ng[0] == '1');  // see nepzbl.h (md_step)
   std::vector<float> nnw;
   if (shape == 0) { build_tables<MS0>(h, p); nnw = build_nnw<MS0>(p); h->D = MS0::D; }
   else { build_tables<MS1>(h, p); nnw = build_nnw<MS1>(p); h->D = MS1::D; }
