@@ -294,218 +294,255 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
 }
 
 // ------------------------------------------------------- S4 + S6 + angular partial forces of S7
-// Network weights staged in shared memory: w0 [neurons][DPAD], b0, w1 [neurons], q_scaler [DPAD].
+// One thread per atom, persistent blocks (grid = resident blocks; a block walks tiles of ANG_THREADS
+// atoms), network weights staged in shared memory once per block: w0 [neurons][DPAD], b0, w1 [neurons],
+// q_scaler [DPAD].  The kernel holds A[n][lm] (120 values) in registers, which caps it at 2 warps per
+// scheduler, so latency has to be hidden inside the thread (ncu: 27 % of the stall samples of the first
+// version sat on the index -> position gathers of its three passes over the list):
+//   * ONE batched pre-pass gathers the neighbours (8 independent index loads, then 8 independent
+//     position gathers per round), keeps the in-cutoff ones as a bit mask (handed to k_force, which
+//     skips the other entries) and parks their displacement vectors in a per-thread column of shared
+//     memory (conflict-free: bank = lane); the forward and backward passes read them back with LDS;
+//   * the forward pass takes two neighbours per iteration (two independent Chebyshev / harmonic
+//     chains feeding 240 independent FMAs);
+//   * the network takes two neurons per iteration (four independent pre-activation chains, two
+//     interleaved tanh evaluations).
+#define ANG_THREADS 128
+#define ANG_GATHER 8
 template <class MS>
-__global__ void __launch_bounds__(128)
-k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
+__global__ void __launch_bounds__(ANG_THREADS)
+k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, int cap_a, const int4* __restrict__ xyzt,
              const int* __restrict__ nn_a, const int* __restrict__ nl_a,
              const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,
              const float* __restrict__ q_radial, float* __restrict__ u_site,
-             AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out) {
+             AtomRec* __restrict__ rec, float4* __restrict__ pforce,
+             unsigned long long* __restrict__ amask, float* __restrict__ q_out) {
   constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR, D = MS::D, DPAD = MS::DPAD;
+  constexpr int T_ = ANG_THREADS;
   extern __shared__ __align__(16) float smem[];
-  const int neu = mt.n_neurons;
-  float* s_w0 = smem;                  // [neu][DPAD]
-  float* s_b0 = s_w0 + neu * DPAD;     // [neu]
-  float* s_w1 = s_b0 + neu;            // [neu]
-  float* s_qs = s_w1 + neu;            // [DPAD]
-  for (int t = threadIdx.x; t < neu * DPAD + 2 * neu + DPAD; t += blockDim.x) smem[t] = nnw[t];
+  const int neu = mt.n_neurons;        // even-padded on the host: row neu (if odd) is all zero
+  const int neu2 = (neu + 1) & ~1;
+  float* s_w0 = smem;                  // [neu2][DPAD]
+  float* s_b0 = s_w0 + neu2 * DPAD;    // [neu2]
+  float* s_w1 = s_b0 + neu2;           // [neu2]
+  float* s_qs = s_w1 + neu2;           // [DPAD]
+  float* dcol = s_qs + DPAD + threadIdx.x;  // displacement cache [cap_a + 1][3][T_], this thread's column
+  for (int t = threadIdx.x; t < neu2 * DPAD + 2 * neu2 + DPAD; t += blockDim.x) smem[t] = nnw[t];
   __syncthreads();
-
-  int s = blockIdx.x * blockDim.x + threadIdx.x;
-  if (s >= n) return;
-  const int4 me = xyzt[s];
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
-  const int cnt = nn_a[s];
+  const int ntiles = (n + T_ - 1) / T_;
 
-  // which list entries are inside rc_angular right now (list carries the skin)
-  unsigned long long mask = 0ull;
-  for (int a = 0; a < cnt; ++a) {
-    int j = nl_a[(size_t)a * npad + s];
-    int4 o = xyzt[j];
-    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
-    float r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 < mt.rcA2) mask |= 1ull << a;
-  }
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const int s = tile * T_ + threadIdx.x;
+    if (s >= n) continue;  // nothing below synchronises the block
+    const int4 me = xyzt[s];
+    const int cnt = nn_a[s];
 
-  // ---- S4 forward: A[n][lm] = sum_j g_n(r_ij) b_lm(rhat_ij)
-  float A[NA][24];
+    // ---- pre-pass: which list entries are inside rc_angular right now (the list carries the skin)
+    unsigned long long mask = 0ull;
+    int nc = 0;
+    for (int a0 = 0; a0 < cnt; a0 += ANG_GATHER) {
+      int j[ANG_GATHER];
+      int4 o[ANG_GATHER];
 #pragma unroll
-  for (int nq = 0; nq < NA; ++nq)
+      for (int u = 0; u < ANG_GATHER; ++u) j[u] = (a0 + u < cnt) ? nl_a[(size_t)(a0 + u) * npad + s] : s;
 #pragma unroll
-    for (int lm = 0; lm < 24; ++lm) A[nq][lm] = 0.0f;
-  for (unsigned long long m = mask; m; m &= m - 1) {
-    int a = __ffsll((long long)m) - 1;
-    int j = nl_a[(size_t)a * npad + s];
-    int4 o = xyzt[j];
-    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
-    float r2 = dx * dx + dy * dy + dz * dz;
-    float r = sqrtf(r2), rinv = 1.0f / r;
-    float fc, dfc, x, dxdr, T[KA];
-    cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
-    float b[24];
-    eval_blm(dx * rinv, dy * rinv, dz * rinv, b);
+      for (int u = 0; u < ANG_GATHER; ++u) o[u] = xyzt[j[u]];
+#pragma unroll
+      for (int u = 0; u < ANG_GATHER; ++u) {
+        float dx = (float)(o[u].x - me.x) * hx, dy = (float)(o[u].y - me.y) * hy, dz = (float)(o[u].z - me.z) * hz;
+        float r2 = dx * dx + dy * dy + dz * dz;
+        if ((a0 + u < cnt) && r2 < mt.rcA2) {
+          mask |= 1ull << (a0 + u);
+          dcol[(3 * nc + 0) * T_] = dx;
+          dcol[(3 * nc + 1) * T_] = dy;
+          dcol[(3 * nc + 2) * T_] = dz;
+          ++nc;
+        }
+      }
+    }
+    amask[s] = mask;
+    // pad to an even count with a dummy neighbour (weight 0 below)
+    dcol[(3 * nc + 0) * T_] = 1.0f;
+    dcol[(3 * nc + 1) * T_] = 0.0f;
+    dcol[(3 * nc + 2) * T_] = 0.0f;
+
+    // ---- S4 forward: A[n][lm] = sum_j g_n(r_ij) b_lm(rhat_ij), two neighbours per iteration
+    float A[NA][24];
+#pragma unroll
+    for (int nq = 0; nq < NA; ++nq)
+#pragma unroll
+      for (int lm = 0; lm < 24; ++lm) A[nq][lm] = 0.0f;
+    for (int c = 0; c < nc; c += 2) {
+      float g2[2][NA], b2[2][24];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        float dx = dcol[(3 * (c + h) + 0) * T_], dy = dcol[(3 * (c + h) + 1) * T_], dz = dcol[(3 * (c + h) + 2) * T_];
+        float r2 = dx * dx + dy * dy + dz * dz;
+        float rinv = rsqrtf(r2), r = r2 * rinv;
+        float fc, T[KA];
+        cheb_T_fwd<KA>(r, mt.inv_rcA, fc, T);
+        if (h == 1 && c + 1 >= nc) fc = 0.0f;
+        eval_blm(dx * rinv, dy * rinv, dz * rinv, b2[h]);
+#pragma unroll
+        for (int nq = 0; nq < NA; ++nq) {
+          float g = 0.0f;
+#pragma unroll
+          for (int k = 0; k < KA; ++k) g = fmaf(mt.ctA[nq][k], T[k], g);
+          g2[h][nq] = g * fc;
+        }
+      }
+#pragma unroll
+      for (int nq = 0; nq < NA; ++nq)
+#pragma unroll
+        for (int lm = 0; lm < 24; ++lm) A[nq][lm] = fmaf(g2[1][nq], b2[1][lm], fmaf(g2[0][nq], b2[0][lm], A[nq][lm]));
+    }
+
+    // ---- descriptor vector (SURVEY 8(c) C order), scaled
+    float q[D];
+#pragma unroll
+    for (int nq = 0; nq < NR; ++nq) q[nq] = q_radial[(size_t)nq * npad + s];
 #pragma unroll
     for (int nq = 0; nq < NA; ++nq) {
-      float g = 0.0f;
+      float ql[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll
-      for (int k = 0; k < KA; ++k) g = fmaf(mt.ctA[nq][k], T[k], g);
-      g *= fc;
+      for (int lm = 0; lm < 24; ++lm) ql[lm_to_l(lm) - 1] = fmaf(kClm[lm] * A[nq][lm], A[nq][lm], ql[lm_to_l(lm) - 1]);
 #pragma unroll
-      for (int lm = 0; lm < 24; ++lm) A[nq][lm] = fmaf(g, b[lm], A[nq][lm]);
+      for (int l = 0; l < 4; ++l) q[NR + l * NA + nq] = ql[l];
     }
-  }
-
-  // ---- descriptor vector (SURVEY 8(c) C order), scaled
-  float q[D];
-#pragma unroll
-  for (int nq = 0; nq < NR; ++nq) q[nq] = q_radial[(size_t)nq * npad + s];
-#pragma unroll
-  for (int nq = 0; nq < NA; ++nq) {
-    float ql[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-#pragma unroll
-    for (int lm = 0; lm < 24; ++lm) ql[lm_to_l(lm) - 1] = fmaf(kClm[lm] * A[nq][lm], A[nq][lm], ql[lm_to_l(lm) - 1]);
-#pragma unroll
-    for (int l = 0; l < 4; ++l) q[NR + l * NA + nq] = ql[l];
-  }
-  float dq4[MS::B4 ? NA : 1][5];  // d q4_n / d A[n][3..7]
-  if (MS::B4) {
-#pragma unroll
-    for (int nq = 0; nq < NA; ++nq) {
-      float a0 = A[nq][3], a1 = A[nq][4], a2 = A[nq][5], a3 = A[nq][6], a4 = A[nq][7];
-      float Szz = a0 * (1.0f / 3.0f), Sxz = a1, Syz = a2, Sxy = 0.5f * a4;
-      float Sxx = fmaf(-1.0f / 6.0f, a0, 0.5f * a3), Syy = fmaf(-1.0f / 6.0f, a0, -0.5f * a3);
-      float cxx = Syy * Szz - Syz * Syz, cyy = Sxx * Szz - Sxz * Sxz, czz = Sxx * Syy - Sxy * Sxy;
-      float cxy = Sxz * Syz - Sxy * Szz, cxz = Sxy * Syz - Syy * Sxz, cyz = Sxy * Sxz - Sxx * Syz;
-      float det = Sxx * cxx + Sxy * cxy + Sxz * cxz;
-      const float k3 = 3.0f * NEPZBL_C4;
-      q[NR + 4 * NA + nq] = k3 * det;
-      dq4[nq][0] = k3 * ((czz * (1.0f / 3.0f)) - (cxx + cyy) * (1.0f / 6.0f));
-      dq4[nq][1] = k3 * 2.0f * cxz;
-      dq4[nq][2] = k3 * 2.0f * cyz;
-      dq4[nq][3] = k3 * 0.5f * (cxx - cyy);
-      dq4[nq][4] = k3 * cxy;
-    }
-  }
-  if (q_out) {
-#pragma unroll
-    for (int v = 0; v < D; ++v) q_out[(size_t)v * npad + s] = q[v];
-  }
-
-  // ---- S6: network forward + gradient
-  float Fp[D];
-#pragma unroll
-  for (int v = 0; v < D; ++v) {
-    q[v] *= s_qs[v];
-    Fp[v] = 0.0f;
-  }
-  float U = -mt.b1;
-#pragma unroll 1
-  for (int m = 0; m < neu; ++m) {
-    const float4* w4 = reinterpret_cast<const float4*>(s_w0 + m * DPAD);  // broadcast LDS.128
-    float z0 = -s_b0[m], z1 = 0.0f;
-#pragma unroll
-    for (int v4 = 0; v4 < DPAD / 4; ++v4) {
-      float4 w = w4[v4];
-      if (4 * v4 + 0 < D) z0 = fmaf(w.x, q[4 * v4 + 0], z0);
-      if (4 * v4 + 1 < D) z1 = fmaf(w.y, q[4 * v4 + 1], z1);
-      if (4 * v4 + 2 < D) z0 = fmaf(w.z, q[4 * v4 + 2], z0);
-      if (4 * v4 + 3 < D) z1 = fmaf(w.w, q[4 * v4 + 3], z1);
-    }
-    float hh = tanh_fast(z0 + z1);
-    float w1 = s_w1[m];
-    U = fmaf(w1, hh, U);
-    float tt = w1 * fmaf(-hh, hh, 1.0f);
-#pragma unroll
-    for (int v4 = 0; v4 < DPAD / 4; ++v4) {
-      float4 w = w4[v4];
-      if (4 * v4 + 0 < D) Fp[4 * v4 + 0] = fmaf(tt, w.x, Fp[4 * v4 + 0]);
-      if (4 * v4 + 1 < D) Fp[4 * v4 + 1] = fmaf(tt, w.y, Fp[4 * v4 + 1]);
-      if (4 * v4 + 2 < D) Fp[4 * v4 + 2] = fmaf(tt, w.z, Fp[4 * v4 + 2]);
-      if (4 * v4 + 3 < D) Fp[4 * v4 + 3] = fmaf(tt, w.w, Fp[4 * v4 + 3]);
-    }
-  }
-#pragma unroll
-  for (int v = 0; v < D; ++v) Fp[v] *= s_qs[v];
-  u_site[s] = U;
-
-  // record for the radial back-pass of k_force: position + d_k = sum_n Fp_n ct_nk
-  {
-    static_assert(KR <= 12, "AtomRec holds 12 coefficients");
-    float d[12];
-#pragma unroll
-    for (int k = 0; k < 12; ++k) d[k] = 0.0f;
-#pragma unroll
-    for (int k = 0; k < KR; ++k)
-#pragma unroll
-      for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
-    float4* rp = reinterpret_cast<float4*>(rec + s);
-    rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
-    rp[1] = make_float4(d[1], d[2], d[3], d[4]);
-    rp[2] = make_float4(d[5], d[6], d[7], d[8]);
-    if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
-  }
-
-  // ---- E[n][lm] = dU/dA[n][lm] (in place)
-#pragma unroll
-  for (int nq = 0; nq < NA; ++nq) {
-#pragma unroll
-    for (int lm = 0; lm < 24; ++lm)
-      A[nq][lm] *= 2.0f * kClm[lm] * Fp[NR + (lm_to_l(lm) - 1) * NA + nq];
+    float dq4[MS::B4 ? NA : 1][5];  // d q4_n / d A[n][3..7]
     if (MS::B4) {
 #pragma unroll
-      for (int m5 = 0; m5 < 5; ++m5) A[nq][3 + m5] = fmaf(Fp[NR + 4 * NA + nq], dq4[nq][m5], A[nq][3 + m5]);
+      for (int nq = 0; nq < NA; ++nq) {
+        float a0 = A[nq][3], a1 = A[nq][4], a2 = A[nq][5], a3 = A[nq][6], a4 = A[nq][7];
+        float Szz = a0 * (1.0f / 3.0f), Sxz = a1, Syz = a2, Sxy = 0.5f * a4;
+        float Sxx = fmaf(-1.0f / 6.0f, a0, 0.5f * a3), Syy = fmaf(-1.0f / 6.0f, a0, -0.5f * a3);
+        float cxx = Syy * Szz - Syz * Syz, cyy = Sxx * Szz - Sxz * Sxz, czz = Sxx * Syy - Sxy * Sxy;
+        float cxy = Sxz * Syz - Sxy * Szz, cxz = Sxy * Syz - Syy * Sxz, cyz = Sxy * Sxz - Sxx * Syz;
+        float det = Sxx * cxx + Sxy * cxy + Sxz * cxz;
+        const float k3 = 3.0f * NEPZBL_C4;
+        q[NR + 4 * NA + nq] = k3 * det;
+        dq4[nq][0] = k3 * ((czz * (1.0f / 3.0f)) - (cxx + cyy) * (1.0f / 6.0f));
+        dq4[nq][1] = k3 * 2.0f * cxz;
+        dq4[nq][2] = k3 * 2.0f * cyz;
+        dq4[nq][3] = k3 * 0.5f * (cxx - cyy);
+        dq4[nq][4] = k3 * cxy;
+      }
     }
-  }
+    if (q_out) {
+#pragma unroll
+      for (int v = 0; v < D; ++v) q_out[(size_t)v * npad + s] = q[v];
+    }
 
-  // ---- angular partial forces dU_i/dr_ij for every list entry (zero outside the cutoff)
-  {
-    unsigned long long all = cnt >= 64 ? ~0ull : ((1ull << cnt) - 1ull);
-    for (unsigned long long m = all & ~mask; m; m &= m - 1) {
-      int a = __ffsll((long long)m) - 1;
-      pforce[(size_t)a * npad + s] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+    // ---- S6: network forward + gradient, two neurons per iteration
+    float Fp[D];
+#pragma unroll
+    for (int v = 0; v < D; ++v) {
+      q[v] *= s_qs[v];
+      Fp[v] = 0.0f;
     }
-  }
-  for (unsigned long long m = mask; m; m &= m - 1) {
-    int a = __ffsll((long long)m) - 1;
-    int j = nl_a[(size_t)a * npad + s];
-    int4 o = xyzt[j];
-    float dx = (float)(o.x - me.x) * hx, dy = (float)(o.y - me.y) * hy, dz = (float)(o.z - me.z) * hz;
-    float r2 = dx * dx + dy * dy + dz * dz;
-    float r = sqrtf(r2), rinv = 1.0f / r;
-    float fc, dfc, x, dxdr, T[KA], Uc[KA];
-    cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
-    cheb_U<KA>(x, Uc);
-    float g[NA], dg[NA];
+    float U = -mt.b1;
+#pragma unroll 1
+    for (int m = 0; m < neu2; m += 2) {
+      const float4* wa = reinterpret_cast<const float4*>(s_w0 + m * DPAD);  // broadcast LDS.128
+      const float4* wb = wa + DPAD / 4;
+      float za0 = -s_b0[m], za1 = 0.0f, zb0 = -s_b0[m + 1], zb1 = 0.0f;
+#pragma unroll
+      for (int v4 = 0; v4 < DPAD / 4; ++v4) {
+        float4 w = wa[v4], x = wb[v4];
+        if (4 * v4 + 0 < D) { za0 = fmaf(w.x, q[4 * v4 + 0], za0); zb0 = fmaf(x.x, q[4 * v4 + 0], zb0); }
+        if (4 * v4 + 1 < D) { za1 = fmaf(w.y, q[4 * v4 + 1], za1); zb1 = fmaf(x.y, q[4 * v4 + 1], zb1); }
+        if (4 * v4 + 2 < D) { za0 = fmaf(w.z, q[4 * v4 + 2], za0); zb0 = fmaf(x.z, q[4 * v4 + 2], zb0); }
+        if (4 * v4 + 3 < D) { za1 = fmaf(w.w, q[4 * v4 + 3], za1); zb1 = fmaf(x.w, q[4 * v4 + 3], zb1); }
+      }
+      float ha = tanh_fast(za0 + za1), hb = tanh_fast(zb0 + zb1);
+      float w1a = s_w1[m], w1b = s_w1[m + 1];
+      U = fmaf(w1a, ha, U);
+      U = fmaf(w1b, hb, U);
+      float ta = w1a * fmaf(-ha, ha, 1.0f), tb = w1b * fmaf(-hb, hb, 1.0f);
+#pragma unroll
+      for (int v4 = 0; v4 < DPAD / 4; ++v4) {
+        float4 w = wa[v4], x = wb[v4];
+        if (4 * v4 + 0 < D) Fp[4 * v4 + 0] = fmaf(tb, x.x, fmaf(ta, w.x, Fp[4 * v4 + 0]));
+        if (4 * v4 + 1 < D) Fp[4 * v4 + 1] = fmaf(tb, x.y, fmaf(ta, w.y, Fp[4 * v4 + 1]));
+        if (4 * v4 + 2 < D) Fp[4 * v4 + 2] = fmaf(tb, x.z, fmaf(ta, w.z, Fp[4 * v4 + 2]));
+        if (4 * v4 + 3 < D) Fp[4 * v4 + 3] = fmaf(tb, x.w, fmaf(ta, w.w, Fp[4 * v4 + 3]));
+      }
+    }
+#pragma unroll
+    for (int v = 0; v < D; ++v) Fp[v] *= s_qs[v];
+    u_site[s] = U;
+
+    // record for the radial back-pass of k_force: position + d_k = sum_n Fp_n ct_nk
+    {
+      static_assert(KR <= 12, "AtomRec holds 12 coefficients");
+      float d[12];
+#pragma unroll
+      for (int k = 0; k < 12; ++k) d[k] = 0.0f;
+#pragma unroll
+      for (int k = 0; k < KR; ++k)
+#pragma unroll
+        for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
+      float4* rp = reinterpret_cast<float4*>(rec + s);
+      rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
+      rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+      rp[2] = make_float4(d[5], d[6], d[7], d[8]);
+      if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
+    }
+
+    // ---- E[n][lm] = dU/dA[n][lm] (in place)
 #pragma unroll
     for (int nq = 0; nq < NA; ++nq) {
-      float p = 0.0f, dp = 0.0f;
 #pragma unroll
-      for (int k = 0; k < KA; ++k) p = fmaf(mt.ctA[nq][k], T[k], p);
+      for (int lm = 0; lm < 24; ++lm)
+        A[nq][lm] *= 2.0f * kClm[lm] * Fp[NR + (lm_to_l(lm) - 1) * NA + nq];
+      if (MS::B4) {
 #pragma unroll
-      for (int k = 1; k < KA; ++k) dp = fmaf(mt.kctA[nq][k], Uc[k - 1], dp);
-      g[nq] = fc * p;
-      dg[nq] = fmaf(dfc, p, fc * dxdr * dp);
+        for (int m5 = 0; m5 < 5; ++m5) A[nq][3 + m5] = fmaf(Fp[NR + 4 * NA + nq], dq4[nq][m5], A[nq][3 + m5]);
+      }
     }
-    float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
-    auto G = [&](int lm) {
-      float t = 0.0f;
+
+    // ---- angular partial forces dU_i/dr_ij for the in-cutoff entries (k_force skips the others)
+    int c = 0;
+    for (unsigned long long m = mask; m; m &= m - 1, ++c) {
+      const int a = __ffsll((long long)m) - 1;
+      float dx = dcol[(3 * c + 0) * T_], dy = dcol[(3 * c + 1) * T_], dz = dcol[(3 * c + 2) * T_];
+      float r2 = dx * dx + dy * dy + dz * dz;
+      float rinv = rsqrtf(r2), r = r2 * rinv;
+      float fc, dfc, x, dxdr, T[KA], Uc[KA];
+      cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
+      cheb_U<KA>(x, Uc);
+      float g[NA], dg[NA];
 #pragma unroll
-      for (int nq = 0; nq < NA; ++nq) t = fmaf(g[nq], A[nq][lm], t);
-      return t;
-    };
-    auto Gp = [&](int lm) {
-      float t = 0.0f;
+      for (int nq = 0; nq < NA; ++nq) {
+        float p = 0.0f, dp = 0.0f;
 #pragma unroll
-      for (int nq = 0; nq < NA; ++nq) t = fmaf(dg[nq], A[nq][lm], t);
-      return t;
-    };
-    float Sp, vx, vy, vz;
-    contract_blm_grad(ux, uy, uz, G, Gp, Sp, vx, vy, vz);
-    float uv = ux * vx + uy * vy + uz * vz;
-    float px = fmaf(ux, Sp, (vx - ux * uv) * rinv);
-    float py = fmaf(uy, Sp, (vy - uy * uv) * rinv);
-    float pz = fmaf(uz, Sp, (vz - uz * uv) * rinv);
-    pforce[(size_t)a * npad + s] = make_float4(px, py, pz, 0.0f);
+        for (int k = 0; k < KA; ++k) p = fmaf(mt.ctA[nq][k], T[k], p);
+#pragma unroll
+        for (int k = 1; k < KA; ++k) dp = fmaf(mt.kctA[nq][k], Uc[k - 1], dp);
+        g[nq] = fc * p;
+        dg[nq] = fmaf(dfc, p, fc * dxdr * dp);
+      }
+      float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
+      auto G = [&](int lm) {
+        float t = 0.0f;
+#pragma unroll
+        for (int nq = 0; nq < NA; ++nq) t = fmaf(g[nq], A[nq][lm], t);
+        return t;
+      };
+      auto Gp = [&](int lm) {
+        float t = 0.0f;
+#pragma unroll
+        for (int nq = 0; nq < NA; ++nq) t = fmaf(dg[nq], A[nq][lm], t);
+        return t;
+      };
+      float Sp, vx, vy, vz;
+      contract_blm_grad(ux, uy, uz, G, Gp, Sp, vx, vy, vz);
+      float uv = ux * vx + uy * vy + uz * vz;
+      float px = fmaf(ux, Sp, (vx - ux * uv) * rinv);
+      float py = fmaf(uy, Sp, (vy - uy * uv) * rinv);
+      float pz = fmaf(uz, Sp, (vz - uz * uv) * rinv);
+      pforce[(size_t)a * npad + s] = make_float4(px, py, pz, 0.0f);
+    }
   }
 }

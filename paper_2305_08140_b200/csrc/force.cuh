@@ -23,7 +23,7 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
         const int* __restrict__ nn_r, const int* __restrict__ nl_r, const int* __restrict__ nn_a,
         const int* __restrict__ nl_a, const unsigned char* __restrict__ rev,
         const __grid_constant__ ModelTables<MS> mt, const AtomRec* __restrict__ rec,
-        const unsigned* __restrict__ rmask, int mask_words, const float4* __restrict__ pforce, const float* __restrict__ u_site,
+        const unsigned* __restrict__ rmask, int mask_words, const unsigned long long* __restrict__ amask, const float4* __restrict__ pforce, const float* __restrict__ u_site,
         const int* __restrict__ perm, double* __restrict__ energy, float* __restrict__ force,
         float* __restrict__ virial) {
   constexpr int KR = MS::KR;
@@ -121,14 +121,20 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
     }
   }
 
-  // ---- angular pairs: own partial force minus the neighbour's partial force on the same pair;
-  //      2 entries per lane per iteration so that the dependent gathers overlap
+  // ---- angular pairs inside the cutoff (bit mask from k_angular_nn; by symmetry of r_ij the reverse
+  //      entry is in j's mask too): own partial force minus the neighbour's partial force on the same
+  //      pair.  Lane p takes the in-cutoff entries number p, p+4, ...; 2 entries per lane per iteration
+  //      so that the dependent gathers overlap.
   {
-    const int ca = valid ? nn_a[sc_] : 0;
-    for (int a0 = sub; a0 < ca; a0 += 2 * FORCE_LANES) {
-      const int a1 = a0 + FORCE_LANES;
-      const bool ok1 = a1 < ca;
-      const size_t e0 = (size_t)a0 * npad + sc_, e1 = (size_t)(ok1 ? a1 : a0) * npad + sc_;
+    unsigned long long m = valid ? amask[sc_] : 0ull;
+    for (int k = 0; k < sub; ++k) m &= m - 1;  // drop the entries of the lanes below
+    while (m) {
+      const int a0 = __ffsll((long long)m) - 1;
+      m &= m - 1; m &= m - 1; m &= m - 1; m &= m - 1;
+      const bool ok1 = m != 0ull;
+      const int a1 = ok1 ? __ffsll((long long)m) - 1 : a0;
+      m &= m - 1; m &= m - 1; m &= m - 1; m &= m - 1;
+      const size_t e0 = (size_t)a0 * npad + sc_, e1 = (size_t)a1 * npad + sc_;
       int j0 = nl_a[e0], j1 = nl_a[e1];
       int b0 = rev[e0], b1 = rev[e1];
       float4 pij0 = pforce[e0], pij1 = pforce[e1];

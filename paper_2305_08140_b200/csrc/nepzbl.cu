@@ -26,7 +26,7 @@ constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
-      nn_r, nn_a, nl_r, nl_a, rev, rmask, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
+      nn_r, nn_a, nl_r, nl_a, rev, rmask, amask, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
       partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
@@ -59,6 +59,7 @@ struct nepzbl_handle {
   std::vector<char> tables;   // ModelTables<MS> for the dispatched shape
   ZblParams zp{};
   size_t smem_nn = 0;
+  int n_sm = 0, ang_grid = 0;  // k_angular_nn is persistent: grid = resident blocks
 
   // workspace
   char* ws = nullptr;
@@ -149,6 +150,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.nl_a = take(4 * (size_t)p.cap_angular * npad);
   c.rev = take((size_t)p.cap_angular * npad);
   c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
+  c.amask = take(8 * npad);
   c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
   c.dk = take(64 * npad);  // AtomRec
   c.pforce = take(16 * (size_t)p.cap_angular * npad);
@@ -198,17 +200,20 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   t.n_neurons = p->n_neurons;
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
-  h->smem_nn = sizeof(float) * ((size_t)p->n_neurons * MS::DPAD + 2 * p->n_neurons + MS::DPAD);
+  const size_t neu2 = (size_t)((p->n_neurons + 1) & ~1);
+  h->smem_nn = sizeof(float) * (neu2 * MS::DPAD + 2 * neu2 + MS::DPAD +
+                                3 * (size_t)(p->cap_angular + 1) * ANG_THREADS);
 }
 
 template <class MS>
 std::vector<float> build_nnw(const nepzbl_params* p) {
-  std::vector<float> w((size_t)p->n_neurons * MS::DPAD + 2 * p->n_neurons + MS::DPAD, 0.0f);
+  const int neu2 = (p->n_neurons + 1) & ~1;  // k_angular_nn takes two neurons per iteration: pad with a zero row
+  std::vector<float> w((size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD, 0.0f);
   for (int m = 0; m < p->n_neurons; ++m)
     for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
-  float* b0 = w.data() + (size_t)p->n_neurons * MS::DPAD;
-  float* w1 = b0 + p->n_neurons;
-  float* qs = w1 + p->n_neurons;
+  float* b0 = w.data() + (size_t)neu2 * MS::DPAD;
+  float* w1 = b0 + neu2;
+  float* qs = w1 + neu2;
   for (int m = 0; m < p->n_neurons; ++m) {
     b0[m] = (float)p->b0[m];
     w1[m] = (float)p->w1[m];
@@ -298,21 +303,21 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
                                               h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p),
                                               h->at<int>(c.zbl_list));
   prof_mark(h, PK_ANGULAR_NN);
-  k_angular_nn<MS><<<blocks(n, 128), 128, h->smem_nn, st>>>(
-      h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_a), h->at<int>(c.nl_a), mt, h->d_nnw,
+  k_angular_nn<MS><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
+      h->d_bm, n, npad, h->p.cap_angular, h->at<int4>(c.xyzt), h->at<int>(c.nn_a), h->at<int>(c.nl_a), mt, h->d_nnw,
       h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
-      want_q ? h->at<float>(c.q_desc) : nullptr);
+      h->at<unsigned long long>(c.amask), want_q ? h->at<float>(c.q_desc) : nullptr);
   prof_mark(h, PK_FORCE);
   if (virial)
     k_force<MS, true><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
         h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
-        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial);
+        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial);
   else
     k_force<MS, false><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
         h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
-        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
+        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
   h->launches += 3;
   if (h->p.zbl_enabled && with_zbl) {
     prof_mark(h, PK_ZBL);
@@ -512,6 +517,15 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   };
   cudaError_t ce;
   if ((ce = cudaSetDevice(device)) != cudaSuccess) return die("cudaSetDevice", ce);
+  if ((ce = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return die("cudaDeviceGetAttribute", ce);
+  {  // k_angular_nn: opt in to its dynamic shared memory and size the persistent grid to the resident blocks
+    const void* fn = shape == 0 ? (const void*)k_angular_nn<MS0> : (const void*)k_angular_nn<MS1>;
+    if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_nn)) != cudaSuccess) return die("cudaFuncSetAttribute(k_angular_nn)", ce);
+    int per_sm = 0;
+    if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ANG_THREADS, h->smem_nn)) != cudaSuccess) return die("cudaOccupancyMaxActiveBlocksPerMultiprocessor", ce);
+    if (per_sm < 1) return die("k_angular_nn does not fit one SM", cudaErrorInvalidConfiguration);
+    h->ang_grid = per_sm * h->n_sm;
+  }
   if ((ce = cudaMalloc(&h->d_sc, sizeof(Scalars))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_bm, sizeof(BoxMap))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_nnw, nnw.size() * sizeof(float))) != cudaSuccess) return die("cudaMalloc", ce);
