@@ -257,7 +257,7 @@ __device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int S, int 
 // per atom (sorted order): walk the (2S+1)^3 cells, emit radial and angular lists (column-major).
 __global__ void __launch_bounds__(128)
 k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
-      const int* __restrict__ cell_start, float rcs2_radial, float rcs2_angular, int cap_r, int cap_a,
+      const int* __restrict__ cell_start, float rc2_radial, float rcs2_radial, float rcs2_angular, int cap_r, int cap_a,
       int* __restrict__ nn_r, int* __restrict__ nl_r, int* __restrict__ nn_a, int* __restrict__ nl_a) {
   if (!sc->do_rebuild) return;
   int s = blockIdx.x * blockDim.x + threadIdx.x;
@@ -269,7 +269,13 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
   axis_stencil(cell_of_u((unsigned)me.x, bm->ncv[0], bm->nc[0]), bm->nc[0], bm->pbc[0], S, sx);
   axis_stencil(cell_of_u((unsigned)me.y, bm->ncv[1], bm->nc[1]), bm->nc[1], bm->pbc[1], S, sy);
   axis_stencil(cell_of_u((unsigned)me.z, bm->ncv[2], bm->nc[2]), bm->nc[2], bm->pbc[2], S, sz);
-  int cr = 0, ca = 0;
+  // The radial list is emitted in two segments, each in walk order: first the pairs inside rc_radial at
+  // build time, then the pairs in the skin shell.  k_radial tests every entry against the true cutoff
+  // each step; with this order the outcome is the same for almost all lanes of a warp (inside for the
+  // first segment, outside for the second), so the warp skips the Chebyshev body instead of idling
+  // through it.  The second segment is collected downwards from the top of the column and moved into
+  // place at the end.
+  int cr = 0, cb = 0, ca = 0;
   for (int kz = 0; kz < W; ++kz) {
     if (sz[kz] < 0) continue;
     for (int ky = 0; ky < W; ++ky) {
@@ -286,8 +292,13 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
           float dz = (float)(o.z - me.z) * hz;
           float r2 = dx * dx + dy * dy + dz * dz;
           if (r2 < rcs2_radial) {
-            if (cr < cap_r) nl_r[(size_t)cr * npad + s] = j;
-            ++cr;
+            if (r2 < rc2_radial) {
+              if (cr + cb < cap_r) nl_r[(size_t)cr * npad + s] = j;
+              ++cr;
+            } else {
+              if (cr + cb < cap_r) nl_r[(size_t)(cap_r - 1 - cb) * npad + s] = j;
+              ++cb;
+            }
             if (r2 < rcs2_angular) {
               if (ca < cap_a) nl_a[(size_t)ca * npad + s] = j;
               ++ca;
@@ -297,6 +308,17 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
       }
     }
   }
+  if (cr + cb <= cap_r) {
+    for (int k = 0; 2 * k + 1 < cb; ++k) {  // the shell segment was written top-down: restore walk order
+      size_t lo = (size_t)(cap_r - cb + k) * npad + s, hi = (size_t)(cap_r - 1 - k) * npad + s;
+      int t = nl_r[lo];
+      nl_r[lo] = nl_r[hi];
+      nl_r[hi] = t;
+    }
+    if (cr + cb < cap_r)
+      for (int k = 0; k < cb; ++k) nl_r[(size_t)(cr + k) * npad + s] = nl_r[(size_t)(cap_r - cb + k) * npad + s];
+  }
+  cr += cb;
   nn_r[s] = min(cr, cap_r);
   nn_a[s] = min(ca, cap_a);
   if (cr > cap_r) atomicMax(&sc->overflow_radial, cr);

@@ -259,6 +259,7 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
   bh.rcs = h->p.rc_radial + h->p.skin;
   bh.ncell_cap = c.ncell_cap;
   float rr = (float)(bh.rcs * bh.rcs);
+  float rc2 = (float)(h->p.rc_radial * h->p.rc_radial);
   double ra = h->p.rc_angular + h->p.skin;
   float ra2 = (float)(ra * ra);
   k_rebuild_begin<<<1, 1, 0, st>>>(h->d_sc);
@@ -281,7 +282,7 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
                                            h->at<int>(c.perm), h->at<int>(c.inv_perm),
                                            h->at<int4>(c.xyzt), h->at<int4>(c.xyzt_build));
   k_nbr<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
-                                       h->at<int>(c.cell_start), rr, ra2, h->p.cap_radial,
+                                       h->at<int>(c.cell_start), rc2, rr, ra2, h->p.cap_radial,
                                        h->p.cap_angular, h->at<int>(c.nn_r), h->at<int>(c.nl_r),
                                        h->at<int>(c.nn_a), h->at<int>(c.nl_a));
   k_rev<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, n, npad, h->at<int>(c.nn_a), h->at<int>(c.nl_a),
