@@ -219,6 +219,12 @@ __device__ __forceinline__ float tanh_fast(float z) {
 // Which of a lane's entries are inside the cutoff is kept as a bit mask (word w, bit b <-> entry
 // p + 4 (32 w + b)) and handed to k_force, which then gathers only those.  The K basis sums are combined over the 4 lanes
 // by a fixed-order shuffle tree (deterministic).
+// The same pass serves the angular descriptor: the first nn_a entries of the list are the angular list
+// (k_nbr).  For those, the displacement vectors of the entries inside rc_angular are compacted in list
+// order into adisp[c][s] (c = 0 .. popc(amask[s]) - 1) and their slots into the bit mask amask[s].
+// k_angular_nn holds 120 accumulators per thread and runs at 2 warps per scheduler, where it cannot
+// hide gather latency; this kernel can, so the gathers live here and k_angular_nn streams adisp with
+// coalesced loads.
 #define RADIAL_LANES 4
 #define RADIAL_UNROLL 4
 template <class MS>
@@ -226,7 +232,8 @@ __global__ void __launch_bounds__(128)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
          const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,
-         unsigned* __restrict__ rmask, int mask_words, int* __restrict__ zbl_list) {
+         unsigned* __restrict__ rmask, int mask_words, int* __restrict__ zbl_list,
+         const int* __restrict__ nn_a, unsigned long long* __restrict__ amask, float4* __restrict__ adisp) {
   const int gt = blockIdx.x * blockDim.x + threadIdx.x;
   const int s = gt / RADIAL_LANES, sub = gt % RADIAL_LANES;
   const bool valid = s < n;
@@ -238,11 +245,19 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   for (int k = 0; k < MS::KR; ++k) acc[k] = 0.0f;
   bool close = false;
   const int cnt = valid ? nn_r[sc_] : 0;
+  const int cnt_a = valid ? nn_a[sc_] : 0;
   const int* lp = nl_r + (size_t)sub * npad + sc_;
   const size_t lstride = (size_t)RADIAL_LANES * npad;
   unsigned mword = 0u;
   int bit = 0, word = 0;
-  for (int t = sub; t < cnt; t += RADIAL_LANES * RADIAL_UNROLL) {
+  unsigned alo = 0u, ahi = 0u;  // this lane's part of amask
+  int abase = 0;                // angular entries of this atom compacted so far
+  const unsigned below = (1u << sub) - 1u;
+  const int gshift = threadIdx.x & 28;
+  // warp-uniform trip count (entries past a lane's own count are guarded), so that the ballots below
+  // are taken by all 32 lanes
+  const int cnt_max = __reduce_max_sync(0xffffffffu, cnt);
+  for (int t = sub; t - sub < cnt_max; t += RADIAL_LANES * RADIAL_UNROLL) {
     int j[RADIAL_UNROLL];
     int4 o[RADIAL_UNROLL];
 #pragma unroll
@@ -251,11 +266,22 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
     lp += (size_t)RADIAL_UNROLL * lstride;
 #pragma unroll
     for (int u = 0; u < RADIAL_UNROLL; ++u) o[u] = xyzt[j[u]];
+    const bool ang_round = __any_sync(0xffffffffu, t - sub < cnt_a);  // any lane still in its angular prefix?
 #pragma unroll
     for (int u = 0; u < RADIAL_UNROLL; ++u) {
+      const int e = t + RADIAL_LANES * u;
       float dx = (float)(o[u].x - me.x) * hx, dy = (float)(o[u].y - me.y) * hy, dz = (float)(o[u].z - me.z) * hz;
       float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
-      if ((t + RADIAL_LANES * u < cnt) && r2 < mt.rcR2) {
+      if (ang_round) {
+        const bool pa = e < cnt_a && r2 < mt.rcA2;
+        const unsigned g = (__ballot_sync(0xffffffffu, pa) >> gshift) & 0xFu;
+        if (pa) {
+          adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, 0.0f);
+          if (e < 32) alo |= 1u << e; else ahi |= 1u << (e - 32);
+        }
+        abase += __popc(g);
+      }
+      if ((e < cnt) && r2 < mt.rcR2) {
         float r = r2 * rsqrtf(r2), fc, T[MS::KR];
         cheb_T_fwd<MS::KR>(r, mt.inv_rcR, fc, T);
 #pragma unroll
@@ -283,7 +309,10 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
     acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], 2);
   }
   unsigned cb = __ballot_sync(0xffffffffu, close);
+  alo |= __shfl_xor_sync(0xffffffffu, alo, 1); alo |= __shfl_xor_sync(0xffffffffu, alo, 2);
+  ahi |= __shfl_xor_sync(0xffffffffu, ahi, 1); ahi |= __shfl_xor_sync(0xffffffffu, ahi, 2);
   if (!valid) return;
+  if (sub == 0) amask[s] = ((unsigned long long)ahi << 32) | alo;
   for (int nq = sub; nq < MS::NR; nq += RADIAL_LANES) {
     float q = 0.0f;
 #pragma unroll
@@ -297,26 +326,23 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
 // One thread per atom, persistent blocks (grid = resident blocks; a block walks tiles of ANG_THREADS
 // atoms), network weights staged in shared memory once per block: w0 [neurons][DPAD], b0, w1 [neurons],
 // q_scaler [DPAD].  The kernel holds A[n][lm] (120 values) in registers, which caps it at 2 warps per
-// scheduler, so latency has to be hidden inside the thread (ncu: 27 % of the stall samples of the first
-// version sat on the index -> position gathers of its three passes over the list):
-//   * ONE batched pre-pass gathers the neighbours (8 independent index loads, then 8 independent
-//     position gathers per round), keeps the in-cutoff ones as a bit mask (handed to k_force, which
-//     skips the other entries) and parks their displacement vectors in a per-thread column of shared
-//     memory (conflict-free: bank = lane); the forward and backward passes read them back with LDS;
+// scheduler, so it must not wait on memory (ncu: 27 % of the stall samples of the first version sat on
+// the index -> position gathers of its three passes over the list):
+//   * no gathers here: k_radial leaves the displacement vectors of the in-cutoff angular neighbours,
+//     compacted, in adisp[c][s] and their list slots in amask[s]; the forward and backward passes stream
+//     them with coalesced loads issued one iteration ahead;
 //   * the forward pass takes two neighbours per iteration (two independent Chebyshev / harmonic
 //     chains feeding 240 independent FMAs);
 //   * the network takes two neurons per iteration (four independent pre-activation chains, two
 //     interleaved tanh evaluations).
 #define ANG_THREADS 128
-#define ANG_GATHER 8
 template <class MS>
 __global__ void __launch_bounds__(ANG_THREADS)
-k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, int cap_a, const int4* __restrict__ xyzt,
-             const int* __restrict__ nn_a, const int* __restrict__ nl_a,
+k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
+             const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
              const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,
              const float* __restrict__ q_radial, float* __restrict__ u_site,
-             AtomRec* __restrict__ rec, float4* __restrict__ pforce,
-             unsigned long long* __restrict__ amask, float* __restrict__ q_out) {
+             AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out) {
   constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR, D = MS::D, DPAD = MS::DPAD;
   constexpr int T_ = ANG_THREADS;
   extern __shared__ __align__(16) float smem[];
@@ -326,46 +352,30 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, int cap_a, const in
   float* s_b0 = s_w0 + neu2 * DPAD;    // [neu2]
   float* s_w1 = s_b0 + neu2;           // [neu2]
   float* s_qs = s_w1 + neu2;           // [DPAD]
-  float* dcol = s_qs + DPAD + threadIdx.x;  // displacement cache [cap_a + 1][3][T_], this thread's column
-  for (int t = threadIdx.x; t < neu2 * DPAD + 2 * neu2 + DPAD; t += blockDim.x) smem[t] = nnw[t];
+  {  // all loads of a thread in flight at once (the table is a multiple of 4 floats, 16-byte aligned)
+    const int n4 = (neu2 * DPAD + 2 * neu2 + DPAD) / 4;
+    const float4* src = reinterpret_cast<const float4*>(nnw);
+    float4* dst = reinterpret_cast<float4*>(smem);
+    for (int t = threadIdx.x; t < n4; t += 4 * T_) {
+      float4 v[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (t + u * T_ < n4) v[u] = src[t + u * T_];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) if (t + u * T_ < n4) dst[t + u * T_] = v[u];
+    }
+  }
   __syncthreads();
-  const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
   const int ntiles = (n + T_ - 1) / T_;
 
   for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const int s = tile * T_ + threadIdx.x;
     if (s >= n) continue;  // nothing below synchronises the block
-    const int4 me = xyzt[s];
-    const int cnt = nn_a[s];
-
-    // ---- pre-pass: which list entries are inside rc_angular right now (the list carries the skin)
-    unsigned long long mask = 0ull;
-    int nc = 0;
-    for (int a0 = 0; a0 < cnt; a0 += ANG_GATHER) {
-      int j[ANG_GATHER];
-      int4 o[ANG_GATHER];
+    const unsigned long long mask = amask[s];
+    const int nc = __popcll(mask);
+    const float4* dp = adisp + s;
+    float qr[NR];
 #pragma unroll
-      for (int u = 0; u < ANG_GATHER; ++u) j[u] = (a0 + u < cnt) ? nl_a[(size_t)(a0 + u) * npad + s] : s;
-#pragma unroll
-      for (int u = 0; u < ANG_GATHER; ++u) o[u] = xyzt[j[u]];
-#pragma unroll
-      for (int u = 0; u < ANG_GATHER; ++u) {
-        float dx = (float)(o[u].x - me.x) * hx, dy = (float)(o[u].y - me.y) * hy, dz = (float)(o[u].z - me.z) * hz;
-        float r2 = dx * dx + dy * dy + dz * dz;
-        if ((a0 + u < cnt) && r2 < mt.rcA2) {
-          mask |= 1ull << (a0 + u);
-          dcol[(3 * nc + 0) * T_] = dx;
-          dcol[(3 * nc + 1) * T_] = dy;
-          dcol[(3 * nc + 2) * T_] = dz;
-          ++nc;
-        }
-      }
-    }
-    amask[s] = mask;
-    // pad to an even count with a dummy neighbour (weight 0 below)
-    dcol[(3 * nc + 0) * T_] = 1.0f;
-    dcol[(3 * nc + 1) * T_] = 0.0f;
-    dcol[(3 * nc + 2) * T_] = 0.0f;
+    for (int nq = 0; nq < NR; ++nq) qr[nq] = q_radial[(size_t)nq * npad + s];
 
     // ---- S4 forward: A[n][lm] = sum_j g_n(r_ij) b_lm(rhat_ij), two neighbours per iteration
     float A[NA][24];
@@ -373,11 +383,16 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, int cap_a, const in
     for (int nq = 0; nq < NA; ++nq)
 #pragma unroll
       for (int lm = 0; lm < 24; ++lm) A[nq][lm] = 0.0f;
+    const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+    float4 nx0 = nc > 0 ? dp[0] : dummy, nx1 = nc > 1 ? dp[npad] : dummy;
     for (int c = 0; c < nc; c += 2) {
+      const float4 d2[2] = {nx0, nx1};
+      nx0 = c + 2 < nc ? dp[(size_t)(c + 2) * npad] : dummy;  // in flight during this iteration
+      nx1 = c + 3 < nc ? dp[(size_t)(c + 3) * npad] : dummy;
       float g2[2][NA], b2[2][24];
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        float dx = dcol[(3 * (c + h) + 0) * T_], dy = dcol[(3 * (c + h) + 1) * T_], dz = dcol[(3 * (c + h) + 2) * T_];
+        float dx = d2[h].x, dy = d2[h].y, dz = d2[h].z;
         float r2 = dx * dx + dy * dy + dz * dz;
         float rinv = rsqrtf(r2), r = r2 * rinv;
         float fc, T[KA];
@@ -401,7 +416,7 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, int cap_a, const in
     // ---- descriptor vector (SURVEY 8(c) C order), scaled
     float q[D];
 #pragma unroll
-    for (int nq = 0; nq < NR; ++nq) q[nq] = q_radial[(size_t)nq * npad + s];
+    for (int nq = 0; nq < NR; ++nq) q[nq] = qr[nq];
 #pragma unroll
     for (int nq = 0; nq < NA; ++nq) {
       float ql[4] = {0.0f, 0.0f, 0.0f, 0.0f};
@@ -483,6 +498,7 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, int cap_a, const in
       for (int k = 0; k < KR; ++k)
 #pragma unroll
         for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
+      const int4 me = xyzt[s];
       float4* rp = reinterpret_cast<float4*>(rec + s);
       rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
       rp[1] = make_float4(d[1], d[2], d[3], d[4]);
@@ -504,9 +520,11 @@ k_angular_nn(const BoxMap* __restrict__ bm, int n, int npad, int cap_a, const in
 
     // ---- angular partial forces dU_i/dr_ij for the in-cutoff entries (k_force skips the others)
     int c = 0;
+    float4 nx = nc > 0 ? dp[0] : dummy;
     for (unsigned long long m = mask; m; m &= m - 1, ++c) {
       const int a = __ffsll((long long)m) - 1;
-      float dx = dcol[(3 * c + 0) * T_], dy = dcol[(3 * c + 1) * T_], dz = dcol[(3 * c + 2) * T_];
+      const float dx = nx.x, dy = nx.y, dz = nx.z;
+      nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration
       float r2 = dx * dx + dy * dy + dz * dz;
       float rinv = rsqrtf(r2), r = r2 * rinv;
       float fc, dfc, x, dxdr, T[KA], Uc[KA];

@@ -254,11 +254,19 @@ __device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int S, int 
   }
 }
 
-// per atom (sorted order): walk the (2S+1)^3 cells, emit radial and angular lists (column-major).
+// per atom (sorted order): walk the (2S+1)^3 cells, emit ONE list (column-major) in three segments,
+// each in walk order:
+//   [0, nn_a)        pairs inside rc_angular + skin           -- this prefix IS the angular list
+//   [nn_a, n_in)     the other pairs inside rc_radial at build time
+//   [n_in, nn_r)     the pairs in the radial skin shell
+// k_radial tests every entry against the true cutoffs each step; with this order the outcome is the
+// same for almost all lanes of a warp, the in-cutoff entries k_force visits form a dense prefix, and
+// the angular neighbours need no second list or second gather.  Two walks: the first counts the
+// segments, the second places the entries (the cells are L1-hot by then).
 __global__ void __launch_bounds__(128)
 k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
       const int* __restrict__ cell_start, float rc2_radial, float rcs2_radial, float rcs2_angular, int cap_r, int cap_a,
-      int* __restrict__ nn_r, int* __restrict__ nl_r, int* __restrict__ nn_a, int* __restrict__ nl_a) {
+      int* __restrict__ nn_r, int* __restrict__ nl_r, int* __restrict__ nn_a) {
   if (!sc->do_rebuild) return;
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
@@ -269,63 +277,53 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
   axis_stencil(cell_of_u((unsigned)me.x, bm->ncv[0], bm->nc[0]), bm->nc[0], bm->pbc[0], S, sx);
   axis_stencil(cell_of_u((unsigned)me.y, bm->ncv[1], bm->nc[1]), bm->nc[1], bm->pbc[1], S, sy);
   axis_stencil(cell_of_u((unsigned)me.z, bm->ncv[2], bm->nc[2]), bm->nc[2], bm->pbc[2], S, sz);
-  // The radial list is emitted in two segments, each in walk order: first the pairs inside rc_radial at
-  // build time, then the pairs in the skin shell.  k_radial tests every entry against the true cutoff
-  // each step; with this order the outcome is the same for almost all lanes of a warp (inside for the
-  // first segment, outside for the second), so the warp skips the Chebyshev body instead of idling
-  // through it.  The second segment is collected downwards from the top of the column and moved into
-  // place at the end.
-  int cr = 0, cb = 0, ca = 0;
-  for (int kz = 0; kz < W; ++kz) {
-    if (sz[kz] < 0) continue;
-    for (int ky = 0; ky < W; ++ky) {
-      if (sy[ky] < 0) continue;
-      for (int kx = 0; kx < W; ++kx) {
-        if (sx[kx] < 0) continue;
-        int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
-        int b = cell_start[c], e = cell_start[c + 1];
-        for (int j = b; j < e; ++j) {
-          if (j == s) continue;
-          int4 o = xyzt[j];
-          float dx = (float)(o.x - me.x) * hx;  // int32 wrap-around = minimum image
-          float dy = (float)(o.y - me.y) * hy;
-          float dz = (float)(o.z - me.z) * hz;
-          float r2 = dx * dx + dy * dy + dz * dz;
-          if (r2 < rcs2_radial) {
-            if (r2 < rc2_radial) {
-              if (cr + cb < cap_r) nl_r[(size_t)cr * npad + s] = j;
-              ++cr;
-            } else {
-              if (cr + cb < cap_r) nl_r[(size_t)(cap_r - 1 - cb) * npad + s] = j;
-              ++cb;
-            }
-            if (r2 < rcs2_angular) {
-              if (ca < cap_a) nl_a[(size_t)ca * npad + s] = j;
-              ++ca;
+  int na = 0, nb = 0, nc = 0;   // segment sizes (first walk)
+  int oa = 0, ob = 0, oc = 0;   // next slot of each segment (second walk)
+  for (int pass = 0; pass < 2; ++pass) {
+    for (int kz = 0; kz < W; ++kz) {
+      if (sz[kz] < 0) continue;
+      for (int ky = 0; ky < W; ++ky) {
+        if (sy[ky] < 0) continue;
+        for (int kx = 0; kx < W; ++kx) {
+          if (sx[kx] < 0) continue;
+          int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
+          int b = cell_start[c], e = cell_start[c + 1];
+          for (int j = b; j < e; ++j) {
+            if (j == s) continue;
+            int4 o = xyzt[j];
+            float dx = (float)(o.x - me.x) * hx;  // int32 wrap-around = minimum image
+            float dy = (float)(o.y - me.y) * hy;
+            float dz = (float)(o.z - me.z) * hz;
+            float r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 < rcs2_radial) {
+              if (pass == 0) {
+                if (r2 < rcs2_angular) ++na; else if (r2 < rc2_radial) ++nb; else ++nc;
+              } else {
+                int slot = r2 < rcs2_angular ? oa++ : (r2 < rc2_radial ? ob++ : oc++);
+                nl_r[(size_t)slot * npad + s] = j;
+              }
             }
           }
         }
       }
     }
-  }
-  if (cr + cb <= cap_r) {
-    for (int k = 0; 2 * k + 1 < cb; ++k) {  // the shell segment was written top-down: restore walk order
-      size_t lo = (size_t)(cap_r - cb + k) * npad + s, hi = (size_t)(cap_r - 1 - k) * npad + s;
-      int t = nl_r[lo];
-      nl_r[lo] = nl_r[hi];
-      nl_r[hi] = t;
+    if (pass == 0) {
+      if (na + nb + nc > cap_r || na > cap_a) break;  // overflow: reported below, nothing is written
+      oa = 0;
+      ob = na;
+      oc = na + nb;
     }
-    if (cr + cb < cap_r)
-      for (int k = 0; k < cb; ++k) nl_r[(size_t)(cr + k) * npad + s] = nl_r[(size_t)(cap_r - cb + k) * npad + s];
   }
-  cr += cb;
+  const int cr = na + nb + nc;
   nn_r[s] = min(cr, cap_r);
-  nn_a[s] = min(ca, cap_a);
+  nn_a[s] = (cr > cap_r || na > cap_a) ? 0 : na;
   if (cr > cap_r) atomicMax(&sc->overflow_radial, cr);
-  if (ca > cap_a) atomicMax(&sc->overflow_angular, ca);
+  if (na > cap_a) atomicMax(&sc->overflow_angular, na);
+  if (cr > cap_r || na > cap_a) nn_r[s] = 0;
 }
 
-// reverse index of the (symmetric) angular list: rev[a][s] = position of s in the list of j = nl_a[a][s]
+// reverse index of the (symmetric) angular list (the prefix [0, nn_a) of the list):
+// rev[a][s] = position of s in the list of j = nl[a][s]
 __global__ void k_rev(const Scalars* sc, int n, int npad, const int* __restrict__ nn_a,
                       const int* __restrict__ nl_a, unsigned char* __restrict__ rev) {
   if (!sc->do_rebuild) return;

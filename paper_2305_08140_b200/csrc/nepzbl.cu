@@ -26,7 +26,7 @@ constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
-      nn_r, nn_a, nl_r, nl_a, rev, rmask, amask, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
+      nn_r, nn_a, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
       partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
@@ -147,10 +147,10 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.nn_r = take(4 * npad);
   c.nn_a = take(4 * npad);
   c.nl_r = take(4 * (size_t)p.cap_radial * npad);
-  c.nl_a = take(4 * (size_t)p.cap_angular * npad);
   c.rev = take((size_t)p.cap_angular * npad);
   c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
   c.amask = take(8 * npad);
+  c.adisp = take(16 * (size_t)p.cap_angular * npad);
   c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
   c.dk = take(64 * npad);  // AtomRec
   c.pforce = take(16 * (size_t)p.cap_angular * npad);
@@ -201,8 +201,7 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
   const size_t neu2 = (size_t)((p->n_neurons + 1) & ~1);
-  h->smem_nn = sizeof(float) * (neu2 * MS::DPAD + 2 * neu2 + MS::DPAD +
-                                3 * (size_t)(p->cap_angular + 1) * ANG_THREADS);
+  h->smem_nn = sizeof(float) * (neu2 * MS::DPAD + 2 * neu2 + MS::DPAD);
 }
 
 template <class MS>
@@ -284,8 +283,8 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
   k_nbr<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
                                        h->at<int>(c.cell_start), rc2, rr, ra2, h->p.cap_radial,
                                        h->p.cap_angular, h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-                                       h->at<int>(c.nn_a), h->at<int>(c.nl_a));
-  k_rev<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, n, npad, h->at<int>(c.nn_a), h->at<int>(c.nl_a),
+                                       h->at<int>(c.nn_a));
+  k_rev<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, n, npad, h->at<int>(c.nn_a), h->at<int>(c.nl_r),
                                        h->at<unsigned char>(c.rev));
   return nk + 9;
 }
@@ -302,22 +301,23 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   k_radial<MS><<<blocks((long long)n * RADIAL_LANES, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
                                               h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
                                               h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p),
-                                              h->at<int>(c.zbl_list));
+                                              h->at<int>(c.zbl_list), h->at<int>(c.nn_a),
+                                              h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp));
   prof_mark(h, PK_ANGULAR_NN);
   k_angular_nn<MS><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
-      h->d_bm, n, npad, h->p.cap_angular, h->at<int4>(c.xyzt), h->at<int>(c.nn_a), h->at<int>(c.nl_a), mt, h->d_nnw,
+      n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
       h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
-      h->at<unsigned long long>(c.amask), want_q ? h->at<float>(c.q_desc) : nullptr);
+      want_q ? h->at<float>(c.q_desc) : nullptr);
   prof_mark(h, PK_FORCE);
   if (virial)
     k_force<MS, true><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
+        h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
         h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial);
   else
     k_force<MS, false><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-        h->at<int>(c.nn_a), h->at<int>(c.nl_a), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
+        h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
         h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
   h->launches += 3;
   if (h->p.zbl_enabled && with_zbl) {
@@ -602,7 +602,7 @@ int neighbor_get(nepzbl_handle* h, int which, int32_t* nn, int32_t* nl) {
   if (h->n > 0) {
     k_export_list<<<blocks(h->n, 128), 128, 0, h->stream>>>(
         (int)h->n, c.npad, which ? h->p.cap_angular : h->p.cap_radial, h->at<int>(c.perm),
-        h->at<int>(which ? c.nn_a : c.nn_r), h->at<int>(which ? c.nl_a : c.nl_r), nn, nl);
+        h->at<int>(which ? c.nn_a : c.nn_r), h->at<int>(c.nl_r), nn, nl);  // angular list = prefix
     h->launches++;
   }
   CU(cudaStreamSynchronize(h->stream));
