@@ -54,6 +54,11 @@ FLOP_PER_ATOM = {k: sum(STEP_FLOP[s] for s in v) for k, v in KERNEL_STEPS.items(
 BYTES_PER_ATOM = {"integrate_a": 152.0, "kick_b": 64.0, "k_radial": 392.0, "k_angular_nn": 612.0,
                   "k_force": 1136.0}
 FP32_LANES_PER_SM = 128
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on config2 (128 000 atoms) from the committed
+# `ncu --set full` capture (NCU_TRAFFIC_SOURCE); reported as roofline.traffic for that workload only.
+NCU_TRAFFIC_BYTES = {"k_radial": 48.145152e6 + 3.609856e6, "k_angular_nn": 50.303232e6 + 17.240832e6,
+                     "k_force": 90.675456e6 + 3.625728e6}
+NCU_TRAFFIC_SOURCE = "profiles/r1c_ncu_full.md"
 
 
 def _dist_env():
@@ -334,7 +339,10 @@ def run_b200(args):
     achieved = FLOP_PER_ATOM[dom] * n / (kern_ms[dom] * 1e-3) / 1e12
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
-                "frac": achieved / alu_peak, "traffic": args.traffic_bytes,
+                "frac": achieved / alu_peak,
+                "traffic": args.traffic_bytes if args.traffic_bytes is not None else
+                (NCU_TRAFFIC_BYTES.get(dom) if (args.workload == "config2" and args.cells is None) else None),
+                "traffic_source": NCU_TRAFFIC_SOURCE,
                 "peak_source": f"derived: {props.multi_processor_count} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max_mhz:.0f} MHz",
                 "ffma_measured_tflops": ffma_measured, "ms_per_launch": kern_ms[dom],
                 "flop_per_atom": FLOP_PER_ATOM[dom],
