@@ -336,6 +336,9 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
 //   * the network takes two neurons per iteration (four independent pre-activation chains, two
 //     interleaved tanh evaluations).
 #define ANG_THREADS 128
+// rows of the staged weight table: n_neurons rounded up to even (two neurons per iteration) plus two
+// (the software pipeline reads one pair ahead); the padding rows are zero
+__host__ __device__ inline int nn_rows(int n_neurons) { return ((n_neurons + 1) & ~1) + 2; }
 template <class MS>
 __global__ void __launch_bounds__(ANG_THREADS)
 k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
@@ -346,14 +349,14 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
   constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR, D = MS::D, DPAD = MS::DPAD;
   constexpr int T_ = ANG_THREADS;
   extern __shared__ __align__(16) float smem[];
-  const int neu = mt.n_neurons;        // even-padded on the host: row neu (if odd) is all zero
-  const int neu2 = (neu + 1) & ~1;
-  float* s_w0 = smem;                  // [neu2][DPAD]
-  float* s_b0 = s_w0 + neu2 * DPAD;    // [neu2]
-  float* s_w1 = s_b0 + neu2;           // [neu2]
-  float* s_qs = s_w1 + neu2;           // [DPAD]
+  const int neu2 = (mt.n_neurons + 1) & ~1;
+  const int nrow = nn_rows(mt.n_neurons);  // zero rows beyond n_neurons (host: build_nnw)
+  float* s_w0 = smem;                  // [nrow][DPAD]
+  float* s_b0 = s_w0 + nrow * DPAD;    // [nrow]
+  float* s_w1 = s_b0 + nrow;           // [nrow]
+  float* s_qs = s_w1 + nrow;           // [DPAD]
   {  // all loads of a thread in flight at once (the table is a multiple of 4 floats, 16-byte aligned)
-    const int n4 = (neu2 * DPAD + 2 * neu2 + DPAD) / 4;
+    const int n4 = (nrow * DPAD + 2 * nrow + DPAD) / 4;
     const float4* src = reinterpret_cast<const float4*>(nnw);
     float4* dst = reinterpret_cast<float4*>(smem);
     for (int t = threadIdx.x; t < n4; t += 4 * T_) {
@@ -457,8 +460,9 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       Fp[v] = 0.0f;
     }
     float U = -mt.b1;
-#pragma unroll 1
-    for (int m = 0; m < neu2; m += 2) {
+    // software pipeline: the pre-activations of neurons m+2, m+3 are accumulated while the tanh of
+    // neurons m, m+1 (two dependent MUFU ops) is in flight; rows neu2, neu2+1 of w0/b0 are zero padding
+    auto preact = [&](int m, float& za, float& zb) {
       const float4* wa = reinterpret_cast<const float4*>(s_w0 + m * DPAD);  // broadcast LDS.128
       const float4* wb = wa + DPAD / 4;
       float za0 = -s_b0[m], za1 = 0.0f, zb0 = -s_b0[m + 1], zb1 = 0.0f;
@@ -470,7 +474,17 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
         if (4 * v4 + 2 < D) { za0 = fmaf(w.z, q[4 * v4 + 2], za0); zb0 = fmaf(x.z, q[4 * v4 + 2], zb0); }
         if (4 * v4 + 3 < D) { za1 = fmaf(w.w, q[4 * v4 + 3], za1); zb1 = fmaf(x.w, q[4 * v4 + 3], zb1); }
       }
-      float ha = tanh_fast(za0 + za1), hb = tanh_fast(zb0 + zb1);
+      za = za0 + za1;
+      zb = zb0 + zb1;
+    };
+    float za, zb;
+    preact(0, za, zb);
+#pragma unroll 1
+    for (int m = 0; m < neu2; m += 2) {
+      const float ha = tanh_fast(za), hb = tanh_fast(zb);
+      preact(m + 2, za, zb);
+      const float4* wa = reinterpret_cast<const float4*>(s_w0 + m * DPAD);
+      const float4* wb = wa + DPAD / 4;
       float w1a = s_w1[m], w1b = s_w1[m + 1];
       U = fmaf(w1a, ha, U);
       U = fmaf(w1b, hb, U);

@@ -200,13 +200,13 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   t.n_neurons = p->n_neurons;
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
-  const size_t neu2 = (size_t)((p->n_neurons + 1) & ~1);
-  h->smem_nn = sizeof(float) * (neu2 * MS::DPAD + 2 * neu2 + MS::DPAD);
+  const size_t nrow = (size_t)nn_rows(p->n_neurons);
+  h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
 }
 
 template <class MS>
 std::vector<float> build_nnw(const nepzbl_params* p) {
-  const int neu2 = (p->n_neurons + 1) & ~1;  // k_angular_nn takes two neurons per iteration: pad with a zero row
+  const int neu2 = nn_rows(p->n_neurons);  // zero padding rows, see nn_rows
   std::vector<float> w((size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD, 0.0f);
   for (int m = 0; m < p->n_neurons; ++m)
     for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
