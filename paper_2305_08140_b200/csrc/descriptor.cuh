@@ -30,6 +30,9 @@ struct ModelShape {
   static constexpr int NLM = 24;
   static constexpr int D = NR + NA * LMAX + (B4 ? NA : 0);
   static constexpr int DPAD = (D + 3) / 4 * 4;
+  // record gathered per radial pair by k_force: {position, Fp[0..NR-1]} in ONE 32-byte sector when the
+  // radial descriptor has at most 5 components, else {position, d[0..KR-1]} in 64 bytes (AtomRec)
+  static constexpr bool FPREC = NR_ <= 5;
 };
 
 // Small tables passed by value (constant bank): compile-time indexed, so they cost no loads.
@@ -71,6 +74,21 @@ __device__ __forceinline__ void ld_rec(const AtomRec* p, int& ux, int& uy, int& 
   } else {
     d[9] = d[10] = d[11] = 0.0f;
   }
+}
+
+// 32-byte record {ux,uy,uz,Fp0..Fp4} (ModelShape::FPREC): one sector, one 256-bit load per pair; the pair's
+// coefficients d_i[k] + d_j[k] = sum_n (Fp_i[n] + Fp_j[n]) ct_nk are contracted in k_force (NR*KR FMAs with
+// constant-bank operands) -- with the 64-byte record k_force was bound by the L1 data pipe (two scattered
+// sector requests per pair, profiles/r1c_ncu_full.md).
+__device__ __forceinline__ void ld_rec32(const void* base, int idx, int& ux, int& uy, int& uz, float f[5]) {
+  const char* p = reinterpret_cast<const char*>(base) + (size_t)idx * 32;
+  unsigned v0, v1, v2, v3, v4, v5, v6, v7;
+  asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3), "=r"(v4), "=r"(v5), "=r"(v6), "=r"(v7)
+               : "l"(p));
+  ux = (int)v0; uy = (int)v1; uz = (int)v2;
+  f[0] = __uint_as_float(v3); f[1] = __uint_as_float(v4); f[2] = __uint_as_float(v5);
+  f[3] = __uint_as_float(v6); f[4] = __uint_as_float(v7);
 }
 
 // (2l+1)/(4 pi) * addition-theorem weight of each b_lm (see DESIGN.md for the list of b_lm)
@@ -368,11 +386,16 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     }
   }
   __syncthreads();
-  const int ntiles = (n + T_ - 1) / T_;
+  // Work is handed out per WARP (tiles of 32 atoms; nothing below synchronises the block), with warp
+  // slot = warp_in_block * gridDim.x + blockIdx.x, so that the partly filled last round (4000 warp tiles
+  // over 1184 resident warps at 128 000 atoms) is spread over all SMs instead of landing on the first
+  // blocks only (measured: no difference at 128 000 atoms, 108.7 us either way).
+  const int ntiles = (n + 31) / 32;
+  const int nslots = gridDim.x * (T_ / 32);
 
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const int s = tile * T_ + threadIdx.x;
-    if (s >= n) continue;  // nothing below synchronises the block
+  for (int tile = (threadIdx.x >> 5) * gridDim.x + blockIdx.x; tile < ntiles; tile += nslots) {
+    const int s = tile * 32 + (threadIdx.x & 31);
+    if (s >= n) continue;
     const unsigned long long mask = amask[s];
     const int nc = __popcll(mask);
     const float4* dp = adisp + s;
@@ -502,8 +525,17 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     for (int v = 0; v < D; ++v) Fp[v] *= s_qs[v];
     u_site[s] = U;
 
-    // record for the radial back-pass of k_force: position + d_k = sum_n Fp_n ct_nk
-    {
+    // record for the radial back-pass of k_force: position + Fp[0..NR-1] (32 bytes) or position +
+    // d_k = sum_n Fp_n ct_nk (64 bytes), see ModelShape::FPREC
+    if (MS::FPREC) {
+      const int4 me = xyzt[s];
+      float f[5];
+#pragma unroll
+      for (int nq = 0; nq < 5; ++nq) f[nq] = nq < NR ? Fp[nq < NR ? nq : 0] : 0.0f;
+      float4* rp = reinterpret_cast<float4*>(reinterpret_cast<char*>(rec) + (size_t)s * 32);
+      rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), f[0]);
+      rp[1] = make_float4(f[1], f[2], f[3], f[4]);
+    } else {
       static_assert(KR <= 12, "AtomRec holds 12 coefficients");
       float d[12];
 #pragma unroll

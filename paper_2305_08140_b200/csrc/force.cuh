@@ -32,9 +32,24 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
   const int s = gt / FORCE_LANES, sub = gt % FORCE_LANES;
   const bool valid = s < n;
   const int sc_ = valid ? s : 0;
-  struct Rec { int ux, uy, uz; float d[12]; };
+  constexpr int NR = MS::NR;
+  struct Rec { int ux, uy, uz; float d[12]; };  // d[] holds Fp[0..4] when MS::FPREC
+  auto load = [&](Rec& r, int idx) {
+    if (MS::FPREC) ld_rec32(rec, idx, r.ux, r.uy, r.uz, r.d);
+    else ld_rec(rec + idx, r.ux, r.uy, r.uz, r.d, KR);
+  };
+  // d[k] = sum_n Fp[n] ct_nk from a 32-byte record's Fp
+  auto contract = [&](const float* fp, float* d) {
+#pragma unroll
+    for (int k = 0; k < KR; ++k) {
+      float t = 0.0f;
+#pragma unroll
+      for (int nq = 0; nq < NR; ++nq) t = fmaf(fp[nq < 12 ? nq : 0], mt.ctR[nq][k], t);
+      d[k] = t;
+    }
+  };
   Rec me;
-  ld_rec(rec + sc_, me.ux, me.uy, me.uz, me.d, KR);
+  load(me, sc_);
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
   float fx = 0.0f, fy = 0.0f, fz = 0.0f;
   float w[9];
@@ -60,10 +75,10 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
     };
     int j_cur = next_j();
     Rec o_cur, o_nxt;
-    ld_rec(rec + (j_cur >= 0 ? j_cur : sc_), o_cur.ux, o_cur.uy, o_cur.uz, o_cur.d, KR);
+    load(o_cur, j_cur >= 0 ? j_cur : sc_);
     int j_nxt = j_cur >= 0 ? next_j() : -1;
     while (j_cur >= 0) {
-      ld_rec(rec + (j_nxt >= 0 ? j_nxt : sc_), o_nxt.ux, o_nxt.uy, o_nxt.uz, o_nxt.d, KR);
+      load(o_nxt, j_nxt >= 0 ? j_nxt : sc_);
       int j_nn = j_nxt >= 0 ? next_j() : -1;
       const Rec& o = o_cur;
       float dx = (float)(o.ux - me.ux) * hx, dy = (float)(o.uy - me.uy) * hy, dz = (float)(o.uz - me.uz) * hz;
@@ -77,25 +92,43 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       float gi, gj = 0.0f;
       if (VIRIAL) {
         float ai = 0.0f, bi = 0.0f, aj = 0.0f, bj = 0.0f;
+        float di[KR], dj[KR];
+        if (MS::FPREC) {
+          contract(me.d, di);
+          contract(o.d, dj);
+        } else {
+#pragma unroll
+          for (int k = 0; k < KR; ++k) { di[k] = me.d[k]; dj[k] = o.d[k]; }
+        }
 #pragma unroll
         for (int k = 0; k < KR; ++k) {
-          ai = fmaf(me.d[k], T[k], ai);
-          aj = fmaf(o.d[k], T[k], aj);
+          ai = fmaf(di[k], T[k], ai);
+          aj = fmaf(dj[k], T[k], aj);
         }
 #pragma unroll
         for (int k = 1; k < KR; ++k) {
           float ku = (float)k * Uc[k - 1];
-          bi = fmaf(me.d[k], ku, bi);
-          bj = fmaf(o.d[k], ku, bj);
+          bi = fmaf(di[k], ku, bi);
+          bj = fmaf(dj[k], ku, bj);
         }
         gi = fmaf(dfc, ai, e * bi);  // dU_i/dr along rhat_ij
         gj = fmaf(dfc, aj, e * bj);  // dU_j/dr along rhat_ji (same scalar form)
       } else {
         // forces only need g_i + g_j: contract once with d_i + d_j (two partial sums each for ILP)
         float a0 = 0.0f, a1 = 0.0f, b0 = 0.0f, b1 = 0.0f;
+        float dsum[KR];
+        if (MS::FPREC) {
+          float fs5[5];
+#pragma unroll
+          for (int nq = 0; nq < 5; ++nq) fs5[nq] = me.d[nq] + o.d[nq];
+          contract(fs5, dsum);
+        } else {
+#pragma unroll
+          for (int k = 0; k < KR; ++k) dsum[k] = me.d[k] + o.d[k];
+        }
 #pragma unroll
         for (int k = 0; k < KR; ++k) {
-          float ds = me.d[k] + o.d[k];
+          float ds = dsum[k];
           if (k & 1) a1 = fmaf(ds, T[k], a1); else a0 = fmaf(ds, T[k], a0);
           if (k >= 1) {
             float ku = (float)k * Uc[k - 1];
