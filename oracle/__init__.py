@@ -251,3 +251,69 @@ def md_run(P: Params, pos, vel, types, box, pbc, nsteps: int, dt_max: float, max
     if r != 0:
         raise RuntimeError(f"oracle md failed: {r}")
     return pos, vel, dt[:nsteps], ep, ek
+
+
+KB_EV_PER_K = 8.617333262e-5
+
+
+def nhc_half_step(M: int, nf: float, kT: float, tau: float, delta: float, ke2: float, xi, vxi):
+    """One NHC(delta) operator (ref. [32]; DESIGN C-24) on copies of xi, vxi.  Returns s, xi, vxi."""
+    xi = np.ascontiguousarray(xi, dtype=np.float64).copy()
+    vxi = np.ascontiguousarray(vxi, dtype=np.float64).copy()
+    f = lib().orc_nhc_half_step
+    f.restype = C.c_double
+    s = f(C.c_int(M), C.c_double(nf), C.c_double(kT), C.c_double(tau), C.c_double(delta), C.c_double(ke2),
+          _dp(xi), _dp(vxi))
+    return float(s), xi, vxi
+
+
+def md_run_nhc(P: Params, pos, vel, types, box, pbc, nsteps: int, dt_max: float, max_disp: float,
+               group, T: float, tau: float, chain: int = 4, xi=None, vxi=None, use_cell: bool | None = None):
+    """md_run with a Nose-Hoover chain (ref. [32]) on the atoms with group != 0.
+    Returns a dict: pos, vel, dt, epot, ekin, conserved, t_group, xi, vxi."""
+    pos, n, types, box, pbc = _sys_args(pos, types, box, pbc)
+    pos = pos.copy()
+    vel = np.ascontiguousarray(vel, dtype=np.float64).copy()
+    group = np.ascontiguousarray(group, dtype=np.uint8)
+    assert group.size == n
+    if use_cell is None:
+        use_cell = n > 3000
+    xi = np.zeros(chain) if xi is None else np.ascontiguousarray(xi, dtype=np.float64).copy()
+    vxi = np.zeros(chain) if vxi is None else np.ascontiguousarray(vxi, dtype=np.float64).copy()
+    dt = np.zeros(max(nsteps, 1)); ep = np.zeros(nsteps + 1); ek = np.zeros(nsteps + 1)
+    cons = np.zeros(nsteps + 1); tg = np.zeros(nsteps + 1)
+    f = lib().orc_md_run_nhc
+    f.restype = C.c_int
+    r = f(P.ref, C.c_int(n), _dp(pos), _dp(vel), _ip(types), _dp(box), _ip(pbc), C.c_int(nsteps),
+          C.c_double(dt_max), C.c_double(max_disp), C.c_int(int(use_cell)),
+          group.ctypes.data_as(C.POINTER(C.c_uint8)), C.c_double(T), C.c_double(tau), C.c_int(chain),
+          _dp(xi), _dp(vxi), _dp(dt), _dp(ep), _dp(ek), _dp(cons), _dp(tg))
+    if r != 0:
+        raise RuntimeError(f"oracle md (nhc) failed: {r}")
+    return dict(pos=pos, vel=vel, dt=dt[:nsteps], epot=ep, ekin=ek, conserved=cons, t_group=tg, xi=xi, vxi=vxi)
+
+
+def wigner_seitz(site, pos, box, pbc, sel=None):
+    """Wigner-Seitz occupancy (ref. [34]): nearest[n], occ[n_sites], (n_vacancies, n_interstitials).
+    Brute force over all sites.  sel: only these atoms are assigned (others -1)."""
+    site = np.ascontiguousarray(site, dtype=np.float64)
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    assert site.ndim == 2 and site.shape[0] == 3 and pos.ndim == 2 and pos.shape[0] == 3
+    ns, n = site.shape[1], pos.shape[1]
+    box = np.ascontiguousarray(box, dtype=np.float64).reshape(9)
+    pbc = np.ascontiguousarray(pbc, dtype=np.int32).reshape(3)
+    nearest = np.full(n, -1, dtype=np.int32)
+    occ = np.zeros(ns, dtype=np.int32)
+    counts = np.zeros(2, dtype=np.int64)
+    if sel is None:
+        nsel, selp = -1, None
+    else:
+        sel = np.ascontiguousarray(sel, dtype=np.int32)
+        nsel, selp = sel.size, _ip(sel)
+    f = lib().orc_wigner_seitz
+    f.restype = C.c_int
+    r = f(C.c_int(ns), _dp(site), C.c_int(n), _dp(pos), _dp(box), _ip(pbc), C.c_int(nsel), selp,
+          _ip(nearest), _ip(occ), counts.ctypes.data_as(C.POINTER(C.c_int64)))
+    if r != 0:
+        raise RuntimeError(f"oracle wigner_seitz failed: {r}")
+    return nearest, occ, (int(counts[0]), int(counts[1]))

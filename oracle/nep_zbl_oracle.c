@@ -764,3 +764,197 @@ int orc_md_run(const orc_params *p, int n, double *pos, double *vel, const int32
   free(E);
   return rc;
 }
+
+/* ------------------------------------------------------------------ Nose-Hoover chain on a group (ref. [32]) */
+
+/*
+ * SURVEY 8(f) NEXT-1.  "Atoms within a thickness of 3 a0 of the boundaries of the simulation boxes ...
+ * are maintained at 300 K using the Nose-Hoover chain thermostat [32]".  Equations of motion of
+ * ref. [32] (Martyna, Klein, Tuckerman 1992) for the atoms of the group G, N_f = 3 |G| degrees of freedom,
+ * chain length M, thermostat "masses" Q_1 = N_f kT tau^2, Q_k = kT tau^2 (k >= 2):
+ *     dv_i/dt   = F_i/m_i - vxi_1 v_i                         (i in G)
+ *     dxi_k/dt  = vxi_k
+ *     dvxi_1/dt = (sum_{i in G} m_i v_i^2 - N_f kT)/Q_1 - vxi_1 vxi_2
+ *     dvxi_k/dt = (Q_{k-1} vxi_{k-1}^2 - kT)/Q_k - vxi_k vxi_{k+1}     (last link: no friction term)
+ * conserved:  H' = E_kin(all) + E_pot + sum_k Q_k vxi_k^2 / 2 + N_f kT xi_1 + kT sum_{k>=2} xi_k.
+ * The paper gives neither M, tau nor the integrator (D:C-24): the step is split as
+ *     NHC(dt/2) . velocity-Verlet(dt) . NHC(dt/2)
+ * and NHC(delta) is the explicit reversible chain update (one Suzuki-Yoshida weight, one sub-step):
+ *     for k = M..1:  vxi_k <- [vxi_k e^{-vxi_{k+1} delta/4} + G_k delta/2] e^{-vxi_{k+1} delta/4}
+ *     s = e^{-vxi_1 delta};  v_i <- s v_i (i in G);  xi_k += vxi_k delta
+ *     for k = 1..M:  the same velocity update with G_k recomputed from the scaled kinetic energy.
+ * This function is that operator for delta = `delta`: it updates xi[M], vxi[M] and returns the scale
+ * factor s; `ke2` = sum_{i in G} m_i v_i^2 (eV) BEFORE the call.
+ */
+double orc_nhc_half_step(int M, double nf, double kT, double tau, double delta, double ke2,
+                         double *xi, double *vxi) {
+  double Q[16];
+  if (M < 1) M = 1;
+  if (M > 16) M = 16;
+  Q[0] = nf * kT * tau * tau;
+  for (int k = 1; k < M; ++k) Q[k] = kT * tau * tau;
+  /* descending sweep: k = M-1 .. 0 (0-based) */
+  for (int k = M - 1; k >= 0; --k) {
+    double G = k == 0 ? (ke2 - nf * kT) / Q[0] : (Q[k - 1] * vxi[k - 1] * vxi[k - 1] - kT) / Q[k];
+    double e = k == M - 1 ? 1.0 : exp(-vxi[k + 1] * delta * 0.25);
+    vxi[k] = (vxi[k] * e + G * delta * 0.5) * e;
+  }
+  double s = exp(-vxi[0] * delta);
+  ke2 *= s * s;
+  for (int k = 0; k < M; ++k) xi[k] += vxi[k] * delta;
+  /* ascending sweep */
+  for (int k = 0; k < M; ++k) {
+    double G = k == 0 ? (ke2 - nf * kT) / Q[0] : (Q[k - 1] * vxi[k - 1] * vxi[k - 1] - kT) / Q[k];
+    double e = k == M - 1 ? 1.0 : exp(-vxi[k + 1] * delta * 0.25);
+    vxi[k] = (vxi[k] * e + G * delta * 0.5) * e;
+  }
+  return s;
+}
+
+#define ORC_KB 8.617333262e-5 /* eV/K (SURVEY 8(b) units) */
+
+static double group_ke2(const orc_params *p, int n, const double *vel, const int32_t *types,
+                        const uint8_t *group) {
+  double s = 0.0;
+  for (int i = 0; i < n; ++i)
+    if (group[i]) {
+      double v2 = vel[i] * vel[i] + vel[(size_t)n + i] * vel[(size_t)n + i] +
+                  vel[2 * (size_t)n + i] * vel[2 * (size_t)n + i];
+      s += p->mass[types[i]] * v2 * ORC_AMU_A2_FS2_TO_EV;
+    }
+  return s;
+}
+
+/*
+ * orc_md_run with the Nose-Hoover chain of the comment above acting on the atoms with group[i] != 0.
+ * Per step: dt from v(t) as in orc_md_run (D:C-11, before the thermostat half-step); NHC(dt/2); kick;
+ * drift; wrap; F; kick; NHC(dt/2).  xi[M], vxi[M] are the chain state (in/out).  Traces as in
+ * orc_md_run plus cons_trace[nsteps+1] = H' and tg_trace[nsteps+1] = group temperature
+ * sum_G m v^2 / (N_f k_B).  An empty group makes this identical to orc_md_run.
+ */
+int orc_md_run_nhc(const orc_params *p, int n, double *pos, double *vel, const int32_t *types,
+                   const double *box, const int32_t *pbc, int nsteps, double dt_max, double max_disp,
+                   int use_cell, const uint8_t *group, double T, double tau, int M, double *xi,
+                   double *vxi, double *dt_trace, double *epot_trace, double *ekin_trace,
+                   double *cons_trace, double *tg_trace) {
+  double *F = (double *)malloc(sizeof(double) * 3 * (size_t)n);
+  double *E = (double *)malloc(sizeof(double) * n);
+  int ng = 0;
+  for (int i = 0; i < n; ++i) ng += group[i] != 0;
+  const double nf = 3.0 * ng, kT = ORC_KB * T;
+  if (M < 1) M = 1;
+  if (M > 16) M = 16;
+  int rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
+  for (int step = 0; step <= nsteps && !rc; ++step) {
+    double ep = 0.0, ek = 0.0, vmax2 = 0.0;
+    for (int i = 0; i < n; ++i) {
+      double v2 = vel[i] * vel[i] + vel[(size_t)n + i] * vel[(size_t)n + i] +
+                  vel[2 * (size_t)n + i] * vel[2 * (size_t)n + i];
+      ep += E[i];
+      ek += 0.5 * p->mass[types[i]] * v2 * ORC_AMU_A2_FS2_TO_EV;
+      if (v2 > vmax2) vmax2 = v2;
+    }
+    if (epot_trace) epot_trace[step] = ep;
+    if (ekin_trace) ekin_trace[step] = ek;
+    if (tg_trace) tg_trace[step] = ng ? group_ke2(p, n, vel, types, group) / (nf * ORC_KB) : 0.0;
+    if (cons_trace) {
+      double h = ek + ep;
+      if (ng) {
+        for (int k = 0; k < M; ++k) {
+          double Qk = (k == 0 ? nf : 1.0) * kT * tau * tau;
+          h += 0.5 * Qk * vxi[k] * vxi[k] + (k == 0 ? nf : 1.0) * kT * xi[k];
+        }
+      }
+      cons_trace[step] = h;
+    }
+    if (step == nsteps) break;
+    double vmax = sqrt(vmax2);
+    double dt = dt_max;
+    if (vmax > 0.0 && max_disp / vmax < dt) dt = max_disp / vmax;
+    if (dt_trace) dt_trace[step] = dt;
+    if (ng) {
+      double s = orc_nhc_half_step(M, nf, kT, tau, 0.5 * dt, group_ke2(p, n, vel, types, group), xi, vxi);
+      for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < n; ++i)
+          if (group[i]) vel[(size_t)a * n + i] *= s;
+    }
+    for (int a = 0; a < 3; ++a)
+      for (int i = 0; i < n; ++i) {
+        double acc = F[(size_t)a * n + i] / (p->mass[types[i]] * ORC_AMU_A2_FS2_TO_EV);
+        vel[(size_t)a * n + i] += 0.5 * dt * acc;
+        double x = pos[(size_t)a * n + i] + dt * vel[(size_t)a * n + i];
+        if (pbc[a]) x -= box[4 * a] * floor(x / box[4 * a]);
+        pos[(size_t)a * n + i] = x;
+      }
+    rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
+    for (int a = 0; a < 3; ++a)
+      for (int i = 0; i < n; ++i) {
+        double acc = F[(size_t)a * n + i] / (p->mass[types[i]] * ORC_AMU_A2_FS2_TO_EV);
+        vel[(size_t)a * n + i] += 0.5 * dt * acc;
+      }
+    if (ng) {
+      double s = orc_nhc_half_step(M, nf, kT, tau, 0.5 * dt, group_ke2(p, n, vel, types, group), xi, vxi);
+      for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < n; ++i)
+          if (group[i]) vel[(size_t)a * n + i] *= s;
+    }
+  }
+  free(F);
+  free(E);
+  return rc;
+}
+
+/* ------------------------------------------------------------------ Wigner-Seitz defect count (ref. [34]) */
+
+/*
+ * SURVEY 8(f) NEXT-3.  "The interstitials and vacancies were identified by using the Wigner-Seitz cell
+ * methods [34]": every atom is assigned to the reference lattice site nearest to it (minimum
+ * image on periodic axes) -- i.e. to the Wigner-Seitz cell it sits in; a site with no atom is a vacancy,
+ * a site with m >= 2 atoms holds m - 1 interstitials.  Brute force over all sites (plain definition);
+ * ties go to the lowest site index (D:C-25; measure zero for the seeded inputs).
+ * Outputs: nearest[n] (site index per atom), occ[n_sites], counts[2] = {vacancies, interstitials}.
+ * sel/nsel: if nsel >= 0 only the atoms in sel[] are assigned (nearest[] filled for them, occ/counts
+ * then cover only those atoms).
+ */
+int orc_wigner_seitz(int n_sites, const double *site, int n, const double *pos, const double *box,
+                     const int32_t *pbc, int nsel, const int32_t *sel, int32_t *nearest, int32_t *occ,
+                     int64_t *counts) {
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      if (a != b && box[3 * a + b] != 0.0) return -2;
+  for (int s = 0; s < n_sites; ++s) occ[s] = 0;
+  const int m = nsel >= 0 ? nsel : n;
+#pragma omp parallel for schedule(static)
+  for (int t = 0; t < m; ++t) {
+    int i = nsel >= 0 ? sel[t] : t;
+    double best = INFINITY;
+    int bs = -1;
+    for (int s = 0; s < n_sites; ++s) {
+      double r2 = 0.0;
+      for (int a = 0; a < 3; ++a) {
+        double d = site[(size_t)a * n_sites + s] - pos[(size_t)a * n + i];
+        if (pbc[a]) d -= box[4 * a] * nearbyint(d / box[4 * a]);
+        r2 += d * d;
+      }
+      if (r2 < best) {
+        best = r2;
+        bs = s;
+      }
+    }
+    nearest[i] = bs;
+  }
+  for (int t = 0; t < m; ++t) {
+    int i = nsel >= 0 ? sel[t] : t;
+    if (nearest[i] >= 0) occ[nearest[i]] += 1;
+  }
+  int64_t nv = 0, ni = 0;
+  for (int s = 0; s < n_sites; ++s) {
+    if (occ[s] == 0) nv += 1;
+    if (occ[s] > 1) ni += occ[s] - 1;
+  }
+  if (counts) {
+    counts[0] = nv;
+    counts[1] = ni;
+  }
+  return 0;
+}

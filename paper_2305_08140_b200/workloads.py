@@ -266,3 +266,53 @@ def free_cluster(n: int = 40, seed: int = 7, radius: float = 7.0, min_sep: float
     pos = np.array(pts).T + 50.0
     return Workload("cluster", pos, None, np.zeros(n, dtype=np.int32), _box(100.0, 100.0, 100.0),
                     np.zeros(3, dtype=np.int32), model or synthetic_model())
+
+
+# ----------------------------------------------------------------------------- SURVEY 8(f) NEXT inputs
+
+def border_group(pos: np.ndarray, box: np.ndarray, pbc: np.ndarray, thickness: float = 3.0 * A0_CONFIG) -> np.ndarray:
+    """uint8 mask of the thermostatted border layer of P:77: atoms within `thickness` (3 a0) of the box
+    faces, "except for the surfaces along the z direction of the thin-foil systems", i.e. only the faces
+    of periodic axes count."""
+    L = np.asarray(box, dtype=np.float64).reshape(9)[[0, 4, 8]]
+    m = np.zeros(pos.shape[1], dtype=bool)
+    for a in range(3):
+        if pbc[a]:
+            x = np.mod(pos[a], L[a])
+            m |= (x < thickness) | (x >= L[a] - thickness)
+    return m.astype(np.uint8)
+
+
+def defective_lattice(cells, seed: int, n_vacancies: int, n_interstitials: int, n_frenkel: int = 0,
+                      sigma: float = 0.08, a: float = A0_CONFIG, pbc=(1, 1, 1), vacuum: float = 0.0):
+    """Reference bcc sites plus an atom configuration with known point defects, for the Wigner-Seitz count
+    (P:96): thermal-like Gaussian displacements (sigma), `n_vacancies` atoms removed, `n_interstitials`
+    atoms added 0.9 A from a site along a seed-drawn direction, `n_frenkel` atoms moved to 0.9 A from
+    another site.  Returns (site (3, ns), pos (3, n), box, pbc, info) with info['vacant'] / ['double'] the
+    site indices that must come out empty / doubly occupied.  All defect sites are distinct."""
+    nx, ny, nz = (cells, cells, cells) if np.isscalar(cells) else cells
+    site = bcc_lattice(nx, ny, nz, a, origin=(0.0, 0.0, vacuum))
+    ns = site.shape[1]
+    g = rng(seed, 8)
+    pos = site + g.standard_normal((3, ns)) * sigma
+    pick = g.permutation(ns)[: n_vacancies + n_interstitials + 2 * n_frenkel]
+    vac = list(pick[:n_vacancies])
+    dbl = list(pick[n_vacancies:n_vacancies + n_interstitials])
+    fr_from = list(pick[n_vacancies + n_interstitials:n_vacancies + n_interstitials + n_frenkel])
+    fr_to = list(pick[n_vacancies + n_interstitials + n_frenkel:])
+    extra = []
+    for s in dbl:
+        extra.append(site[:, s] + 0.9 * _random_unit_vector(g))
+    for s, t in zip(fr_from, fr_to):
+        pos[:, s] = site[:, t] + 0.9 * _random_unit_vector(g)
+    keep = np.ones(ns, dtype=bool)
+    keep[vac] = False
+    pos = np.concatenate([pos[:, keep], np.array(extra).T.reshape(3, -1)], axis=1)
+    pbc = np.asarray(pbc, dtype=np.int32)
+    box = _box(nx * a, ny * a, nz * a + 2 * vacuum)
+    L = box[[0, 4, 8]]
+    for ax in range(3):
+        if pbc[ax]:
+            pos[ax] = np.mod(pos[ax], L[ax])
+    info = dict(vacant=sorted(int(v) for v in vac + fr_from), double=sorted(int(v) for v in dbl + fr_to))
+    return site, np.ascontiguousarray(pos), box, pbc, info
