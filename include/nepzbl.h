@@ -162,6 +162,25 @@ int md_get_forces(nepzbl_handle *h, float *force, double *energy);
 /* Counters since md_init: steps, list rebuilds, ZBL pair evaluations of the last step. */
 int md_get_counters(nepzbl_handle *h, int64_t *n_steps, int64_t *n_rebuilds, int64_t *n_zbl_atoms);
 
+/*
+ * Nose-Hoover chain thermostat on a group of atoms: "Atoms within a thickness of
+ * 3 a0 of the boundaries of the simulation boxes ... are maintained at 300 K using the Nose-Hoover chain
+ * thermostat [32]".  Equations of motion of ref. [32] with N_f = 3|G|, Q_1 = N_f k_B T tau^2,
+ * Q_k = k_B T tau^2; every md_step / md_run step becomes NHC(dt/2) . velocity-Verlet(dt) . NHC(dt/2) with
+ * dt still chosen from v(t) at the start of the step (C-24; the paper gives neither the chain
+ * length, tau nor the splitting).
+ * group: dev uint8 [n] in the caller's atom order, non-zero = thermostatted; caller-owned, must stay
+ *   alive until destroy, the next md_init or md_set_thermostat(NULL, ...), which switches it off.
+ * temperature in K, tau in fs, 1 <= chain_length <= 8.  Call after md_init; the chain starts at rest.
+ * md_get_thermostat (host outputs, any may be NULL): chain positions xi[chain_length] and velocities
+ *   vxi[chain_length] (1/fs), the group's kinetic temperature sum_G m v^2 / (N_f k_B) in K, and the
+ *   thermostat's part of the conserved quantity of ref. [32],
+ *   sum_k Q_k vxi_k^2 / 2 + N_f k_B T xi_1 + k_B T sum_{k>=2} xi_k  (eV).
+ */
+int md_set_thermostat(nepzbl_handle *h, const uint8_t *group, double temperature, double tau,
+                      int32_t chain_length);
+int md_get_thermostat(nepzbl_handle *h, double *xi, double *vxi, double *t_group, double *conserved_extra);
+
 /* Number of kernel launches issued by this handle so far (for bench.py's gpu_launches). */
 int64_t nep_zbl_launch_count(const nepzbl_handle *h);
 

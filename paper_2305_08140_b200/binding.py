@@ -28,6 +28,7 @@ EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_d
            "nep_zbl_workspace_bytes", "nep_zbl_set_workspace", "neighbor_build", "neighbor_get",
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
            "md_run", "md_step_host", "md_energies", "md_get_forces", "md_get_counters",
+           "md_set_thermostat", "md_get_thermostat",
            "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
 PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "spare"]
 
@@ -95,6 +96,10 @@ _lib.md_get_forces.argtypes = [_vp, _vp, _vp]
 _lib.md_get_forces.restype = C.c_int
 _lib.md_get_counters.argtypes = [_vp, C.POINTER(_i64), C.POINTER(_i64), C.POINTER(_i64)]
 _lib.md_get_counters.restype = C.c_int
+_lib.md_set_thermostat.argtypes = [_vp, _vp, C.c_double, C.c_double, C.c_int32]
+_lib.md_set_thermostat.restype = C.c_int
+_lib.md_get_thermostat.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_dbl), C.POINTER(_dbl), C.POINTER(_dbl)]
+_lib.md_get_thermostat.restype = C.c_int
 _lib.nep_zbl_launch_count.argtypes = [_vp]
 _lib.nep_zbl_launch_count.restype = _i64
 _lib.nep_zbl_profile.argtypes = [_vp, C.c_int]
@@ -244,6 +249,18 @@ class NepZbl:
         a = _i64(); b = _i64(); c = _i64()
         self._chk(_lib.md_get_counters(self.h, C.byref(a), C.byref(b), C.byref(c)))
         return a.value, b.value, c.value
+
+    def md_set_thermostat(self, group, temperature: float, tau: float, chain_length: int = 4):
+        """group: uint8 device tensor [n] (non-zero = thermostatted) or None to switch off."""
+        self._group_keep = group
+        self._chain = chain_length
+        self._chk(_lib.md_set_thermostat(self.h, _ptr(group), temperature, tau, chain_length))
+
+    def md_get_thermostat(self):
+        xi = (_dbl * 8)(); vxi = (_dbl * 8)(); tg = _dbl(); ex = _dbl()
+        self._chk(_lib.md_get_thermostat(self.h, xi, vxi, C.byref(tg), C.byref(ex)))
+        m = self._chain
+        return np.array(xi[:m]), np.array(vxi[:m]), tg.value, ex.value
 
     def nep_zbl_launch_count(self) -> int:
         return int(_lib.nep_zbl_launch_count(self.h))

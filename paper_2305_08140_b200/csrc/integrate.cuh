@@ -53,25 +53,157 @@ __global__ void k_zbl_gate(const Scalars* sc, unsigned long long cond_zbl) {
   cudaGraphSetConditional((cudaGraphConditionalHandle)cond_zbl, sc->zbl_count > 0 ? 1u : 0u);
 }
 
+// ------------------------------------------------------------------ Nose-Hoover chain
+// "Atoms within a thickness of 3 a0 of the boundaries ... are maintained at 300 K using the Nose-Hoover
+// chain thermostat [32]".  Equations of motion of ref. [32] for the atoms of the group G
+// (N_f = 3|G|, chain length M, Q_1 = N_f kT tau^2, Q_k = kT tau^2):
+//   dv_i/dt = F_i/m_i - vxi_1 v_i;  dxi_k/dt = vxi_k;
+//   dvxi_1/dt = (sum_G m v^2 - N_f kT)/Q_1 - vxi_1 vxi_2;  dvxi_k/dt = (Q_{k-1} vxi_{k-1}^2 - kT)/Q_k - vxi_k vxi_{k+1}.
+// Splitting (C-24): NHC(dt/2) . velocity-Verlet(dt) . NHC(dt/2); NHC(delta) = descending chain
+// sweep, velocity scale s = exp(-vxi_1 delta), xi += vxi delta, ascending sweep.  The chain is a handful
+// of scalars: one thread advances it in fp64 after a fixed-order reduction of sum_G m v^2.
+#define NEPZBL_NHC_MAX 8
+struct NhcState {
+  int enabled, M;
+  double nf, kT, tau;
+  double xi[NEPZBL_NHC_MAX], vxi[NEPZBL_NHC_MAX];
+  double scale;   // s of the last NHC(delta), applied to the group's velocities by the next kernel
+  double ke2;     // sum_G m v^2 (eV) the last NHC(delta) started from
+  double n_group; // |G| (set by md_set_thermostat)
+};
+
+// partial[b] = sum over this block's grid-stride share of m v^2 (eV) of group atoms; cnt[b] = group atoms
+__global__ void __launch_bounds__(256)
+k_group_ke2_partial(int n, const double* __restrict__ vel, const int32_t* __restrict__ types,
+                    const double* __restrict__ mass, const unsigned char* __restrict__ group,
+                    double* __restrict__ partial, double* __restrict__ cnt) {
+  __shared__ double sp[256], sn[256];
+  double s = 0.0, c = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    if (group[i]) {
+      double vx = vel[i], vy = vel[(size_t)n + i], vz = vel[2 * (size_t)n + i];
+      s += mass[types ? types[i] : 0] * NEPZBL_AMU_A2_FS2_TO_EV * (vx * vx + vy * vy + vz * vz);
+      c += 1.0;
+    }
+  }
+  sp[threadIdx.x] = s;
+  sn[threadIdx.x] = c;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      sp[threadIdx.x] += sp[threadIdx.x + o];
+      sn[threadIdx.x] += sn[threadIdx.x + o];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    partial[blockIdx.x] = sp[0];
+    if (cnt) cnt[blockIdx.x] = sn[0];
+  }
+}
+
+// one block: fixed-order sum of the partials, then thread 0 advances the chain by delta = dt/2.
+// phase 0 (before the first half-kick): dt of THIS step = step_dt(sc) (k_step_flag has not run yet);
+// phase 1 (after the second half-kick): dt = sc->dt.  count != NULL: only set n_group / nf (setup).
+__global__ void __launch_bounds__(256)
+k_nhc(const Scalars* sc, NhcState* nh, int nblocks, const double* __restrict__ partial,
+      const double* __restrict__ cnt, int phase) {
+  __shared__ double sp[256];
+  double s = 0.0;
+  const double* src = cnt ? cnt : partial;
+  for (int b = threadIdx.x; b < nblocks; b += 256) s += src[b];
+  sp[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) sp[threadIdx.x] += sp[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x != 0) return;
+  if (cnt) {
+    nh->n_group = sp[0];
+    nh->nf = 3.0 * sp[0];
+    return;
+  }
+  double ke2 = sp[0];
+  nh->ke2 = ke2;
+  nh->scale = 1.0;
+  if (!(nh->nf > 0.0)) return;
+  const double dt = phase == 0 ? step_dt(sc) : sc->dt;
+  const double delta = 0.5 * dt;
+  const int M = nh->M;
+  const double nf = nh->nf, kT = nh->kT, tt = nh->tau * nh->tau;
+  double Q[NEPZBL_NHC_MAX];
+  Q[0] = nf * kT * tt;
+  for (int k = 1; k < M; ++k) Q[k] = kT * tt;
+  double* vxi = nh->vxi;
+  for (int k = M - 1; k >= 0; --k) {
+    double G = k == 0 ? (ke2 - nf * kT) / Q[0] : (Q[k - 1] * vxi[k - 1] * vxi[k - 1] - kT) / Q[k];
+    double e = k == M - 1 ? 1.0 : exp(-vxi[k + 1] * delta * 0.25);
+    vxi[k] = (vxi[k] * e + G * delta * 0.5) * e;
+  }
+  double sv = exp(-vxi[0] * delta);
+  ke2 *= sv * sv;
+  for (int k = 0; k < M; ++k) nh->xi[k] += vxi[k] * delta;
+  for (int k = 0; k < M; ++k) {
+    double G = k == 0 ? (ke2 - nf * kT) / Q[0] : (Q[k - 1] * vxi[k - 1] * vxi[k - 1] - kT) / Q[k];
+    double e = k == M - 1 ? 1.0 : exp(-vxi[k + 1] * delta * 0.25);
+    vxi[k] = (vxi[k] * e + G * delta * 0.5) * e;
+  }
+  nh->scale = sv;
+}
+
+// second NHC half-step: scale the group's velocities, then max |v|^2 over ALL atoms for the next dt
+__global__ void __launch_bounds__(256)
+k_scale_vmax(Scalars* sc, const NhcState* __restrict__ nh, int n, double* __restrict__ vel,
+             const unsigned char* __restrict__ group) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  double v2 = 0.0;
+  if (i < n) {
+    const bool g = group[i] != 0;
+    const double s = nh->scale;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      size_t k = (size_t)a * n + i;
+      double v = vel[k];
+      if (g) {
+        v *= s;
+        vel[k] = v;
+      }
+      v2 += v * v;
+    }
+  }
+  unsigned long long b = (unsigned long long)__double_as_longlong(v2);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o);
+    b = t > b ? t : b;
+  }
+  if ((threadIdx.x & 31) == 0 && b) atomicMax(&sc->vmax2_bits[sc->parity], b);
+}
+
 // first half-kick + drift + wrap + S1 (fixed-point copy into the sorted slot) + displacement since build
 __global__ void __launch_bounds__(256)
 k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restrict__ pos,
              double* __restrict__ vel, const float* __restrict__ force,
              const int32_t* __restrict__ types, const double* __restrict__ inv_mass,
              const int* __restrict__ inv_perm, int4* __restrict__ xyzt,
-             const int4* __restrict__ xyzt_build) {
+             const int4* __restrict__ xyzt_build, const unsigned char* __restrict__ group,
+             const NhcState* __restrict__ nh) {
   __shared__ float sh[32];
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   float d2 = 0.0f;
   if (i < n) {
     const double dt = step_dt(sc);
+    const double sg = (group && group[i]) ? nh->scale : 1.0;  // first NHC(dt/2) of the step (k_nhc)
     int t = types ? types[i] : 0;
     double im = inv_mass[t];  // 1 / (m * 103.6426965): acceleration in A/fs^2 per eV/A
     unsigned int u[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       size_t k = (size_t)a * n + i;
-      double v = vel[k] + 0.5 * dt * ((double)force[k] * im);
+      double v = vel[k];
+      if (group) v *= sg;
+      v += 0.5 * dt * ((double)force[k] * im);
       double xx = pos[k] + dt * v;
       if (bm->pbc[a]) xx -= bm->L[a] * floor(xx / bm->L[a]);
       vel[k] = v;
@@ -96,7 +228,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
 __global__ void __launch_bounds__(256)
 k_kick(Scalars* sc, int n, double* __restrict__ vel,
        const float* __restrict__ force, const int32_t* __restrict__ types,
-       const double* __restrict__ inv_mass, int do_kick) {
+       const double* __restrict__ inv_mass, int do_kick, int do_vmax) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   double v2 = 0.0;
   if (i < n) {
@@ -119,7 +251,7 @@ k_kick(Scalars* sc, int n, double* __restrict__ vel,
     unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o);
     b = t > b ? t : b;
   }
-  if ((threadIdx.x & 31) == 0 && b) atomicMax(&sc->vmax2_bits[sc->parity], b);
+  if (do_vmax && (threadIdx.x & 31) == 0 && b) atomicMax(&sc->vmax2_bits[sc->parity], b);
 }
 
 // fixed-order fp64 reductions for md_energies: per-block tree -> partial[block]; then one block.
@@ -153,9 +285,13 @@ __global__ void __launch_bounds__(256)
 k_energy_final(int nblocks, const double* __restrict__ partial, double* __restrict__ out) {
   __shared__ double sp[256], sk[256];
   double ep = 0.0, ek = 0.0;
-  for (int b = threadIdx.x; b < nblocks; b += 256) {
-    ep += partial[2 * b];
-    ek += partial[2 * b + 1];
+  if (nblocks < 0) {  // single array of -nblocks partial sums -> out[0]
+    for (int b = threadIdx.x; b < -nblocks; b += 256) ep += partial[b];
+  } else {
+    for (int b = threadIdx.x; b < nblocks; b += 256) {
+      ep += partial[2 * b];
+      ek += partial[2 * b + 1];
+    }
   }
   sp[threadIdx.x] = ep;
   sk[threadIdx.x] = ek;

@@ -27,7 +27,7 @@ constexpr int kTraceRing = 1024;
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
       nn_r, nn_a, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
-      partial, st_pos, st_types, st_e, st_f, st_w, total;
+      partial, nhc_partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
 
@@ -79,6 +79,12 @@ struct nepzbl_handle {
   double* md_vel = nullptr;
   const int32_t* md_types = nullptr;
   long long md_steps = 0;
+
+  // Nose-Hoover chain on a group of atoms (md_set_thermostat)
+  NhcState* d_nhc = nullptr;
+  NhcState* h_nhc = nullptr;              // pinned
+  const unsigned char* md_group = nullptr;  // dev, caller-owned
+  bool nhc_on = false;
 
   // one MD step captured as a CUDA graph: the list-rebuild chain and the ZBL kernel sit in IF nodes
   // whose conditions are set on the device (k_step_flag / k_zbl_gate), so a step is ONE launch
@@ -160,6 +166,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.md_force = take(12 * npad);
   c.md_energy = take(8 * npad);
   c.partial = take(16 * 1024);
+  c.nhc_partial = take(16 * 1024);  // [1024] sums + [1024] counts
   c.st_pos = take(24 * npad);
   c.st_types = take(4 * npad);
   c.st_e = take(8 * npad);
@@ -534,6 +541,9 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   if ((ce = cudaMalloc(&h->d_inv_mass, 8 * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_trace, kTraceRing * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_esum, 2 * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_nhc, sizeof(NhcState))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMallocHost(&h->h_nhc, sizeof(NhcState))) != cudaSuccess) return die("cudaMallocHost", ce);
+  if ((ce = cudaMemsetAsync(h->d_nhc, 0, sizeof(NhcState), h->stream)) != cudaSuccess) return die("cudaMemset", ce);
   if ((ce = cudaMallocHost(&h->h_sc, sizeof(Scalars))) != cudaSuccess) return die("cudaMallocHost", ce);
   if ((ce = cudaMallocHost(&h->h_trace, kTraceRing * sizeof(double))) != cudaSuccess) return die("cudaMallocHost", ce);
   if ((ce = cudaMallocHost(&h->h_esum, 2 * sizeof(double))) != cudaSuccess) return die("cudaMallocHost", ce);
@@ -555,7 +565,8 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
 void nep_zbl_destroy(nepzbl_handle* h) {
   if (!h) return;
   cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
-  cudaFree(h->d_trace); cudaFree(h->d_esum);
+  cudaFree(h->d_trace); cudaFree(h->d_esum); cudaFree(h->d_nhc);
+  cudaFreeHost(h->h_nhc);
   cudaFreeHost(h->h_sc); cudaFreeHost(h->h_trace); cudaFreeHost(h->h_esum);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
@@ -676,17 +687,35 @@ int md_init(nepzbl_handle* h, int64_t n, double* pos, double* vel, const int32_t
   h->md_vel = vel;
   h->md_types = types;
   h->md_steps = 0;
+  h->nhc_on = false;
+  h->md_group = nullptr;
   rc = eval_common(h, n, pos, types, box, pbc, h->at<double>(c.md_energy), h->at<float>(c.md_force),
                    nullptr, true, false, true);
   if (rc) return rc;
   k_kick<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, (int)n, vel, h->at<float>(c.md_force), types,
-                                                h->d_inv_mass, 0);
+                                                h->d_inv_mass, 0, 1);
   h->launches++;
   CU(cudaStreamSynchronize(h->stream));
   CU(cudaGetLastError());
   if (h->use_graph && !build_step_graph(h)) h->use_graph = false;  // falls back to plain stream launches
   h->md_ready = true;
   return NEPZBL_OK;
+}
+
+// one NHC(dt/2) operator on the thermostatted group (no-op unless md_set_thermostat
+// enabled it).  phase 0: before the first half-kick (the scale factor is applied inside k_kick_drift);
+// phase 1: after the second half-kick (k_scale_vmax applies it and leaves max |v|^2 for the next dt).
+static int enqueue_nhc(nepzbl_handle* h, int phase, cudaStream_t st) {
+  if (!h->nhc_on) return 0;
+  const Carve& c = h->cv;
+  const int n = (int)h->n;
+  const int nb = (int)std::min<long long>(1024, (h->n + 255) / 256);
+  k_group_ke2_partial<<<nb, 256, 0, st>>>(n, h->md_vel, h->md_types, h->d_mass, h->md_group,
+                                          h->at<double>(c.nhc_partial), nullptr);
+  k_nhc<<<1, 256, 0, st>>>(h->d_sc, h->d_nhc, nb, h->at<double>(c.nhc_partial), nullptr, phase);
+  if (phase == 0) return 2;
+  k_scale_vmax<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_nhc, n, h->md_vel, h->md_group);
+  return 3;
 }
 
 // One MD step as plain stream launches (profiling mode, or when graph capture is unavailable).
@@ -696,10 +725,12 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
   cudaStream_t st = h->stream;
   float hs = (float)(0.5 * h->p.skin);
   prof_mark(h, PK_INTEGRATE_A);
+  h->launches += enqueue_nhc(h, 0, st);
   k_kick_drift<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, h->md_pos, h->md_vel,
                                               h->at<float>(c.md_force), h->md_types, h->d_inv_mass,
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
-                                              h->at<int4>(c.xyzt_build));
+                                              h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
+                                              h->d_nhc);
   k_step_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0);
   h->launches += 2;
   prof_mark(h, PK_REBUILD);
@@ -707,9 +738,9 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
   enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false);
   prof_mark(h, PK_KICK);
   k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->md_vel, h->at<float>(c.md_force), h->md_types,
-                                        h->d_inv_mass, 1);
+                                        h->d_inv_mass, 1, h->nhc_on ? 0 : 1);
+  h->launches += 1 + enqueue_nhc(h, 1, st);
   prof_mark(h, -1);
-  h->launches++;
 }
 
 static void destroy_step_graph(nepzbl_handle* h) {
@@ -757,10 +788,12 @@ static bool build_step_graph(nepzbl_handle* h) {
     return cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies) == cudaSuccess;
   };
   int nk = 0, nk_reb = 0;
+  nk += enqueue_nhc(h, 0, st);
   k_kick_drift<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, h->md_pos, h->md_vel,
                                               h->at<float>(c.md_force), h->md_types, h->d_inv_mass,
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
-                                              h->at<int4>(c.xyzt_build));
+                                              h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
+                                              h->d_nhc);
   k_step_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1);
   nk += 2;
   cudaGraph_t body = nullptr;
@@ -788,8 +821,8 @@ static bool build_step_graph(nepzbl_handle* h) {
       }
     }
     k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->md_vel, h->at<float>(c.md_force), h->md_types,
-                                          h->d_inv_mass, 1);
-    nk += 1;
+                                          h->d_inv_mass, 1, h->nhc_on ? 0 : 1);
+    nk += 1 + enqueue_nhc(h, 1, st);
   }
   cudaGraph_t captured = nullptr;
   cudaError_t ee = cudaStreamEndCapture(st, &captured);
@@ -885,6 +918,71 @@ int md_step_host(nepzbl_handle* h, double* pos, double* vel, double dt_max, doub
   CU(cudaMemcpyAsync(pos, h->md_pos, b, cudaMemcpyDeviceToHost, h->stream));
   CU(cudaMemcpyAsync(vel, h->md_vel, b, cudaMemcpyDeviceToHost, h->stream));
   CU(cudaStreamSynchronize(h->stream));
+  return NEPZBL_OK;
+}
+
+int md_set_thermostat(nepzbl_handle* h, const uint8_t* group, double temperature, double tau,
+                      int32_t chain_length) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_set_thermostat before md_init");
+  if (!group) {
+    h->nhc_on = false;
+    h->md_group = nullptr;
+  } else {
+    if (!(temperature > 0) || !(tau > 0) || chain_length < 1 || chain_length > NEPZBL_NHC_MAX)
+      return fail(h, NEPZBL_E_INVALID_ARG, "need temperature > 0, tau > 0, 1 <= chain_length <= %d", NEPZBL_NHC_MAX);
+    const Carve& c = h->cv;
+    NhcState s;
+    memset(&s, 0, sizeof s);
+    s.enabled = 1;
+    s.M = chain_length;
+    s.kT = 8.617333262e-5 * temperature;
+    s.tau = tau;
+    s.scale = 1.0;
+    *h->h_nhc = s;
+    CU(cudaMemcpyAsync(h->d_nhc, h->h_nhc, sizeof s, cudaMemcpyHostToDevice, h->stream));
+    const int nb = (int)std::min<long long>(1024, (h->n + 255) / 256);
+    k_group_ke2_partial<<<nb, 256, 0, h->stream>>>((int)h->n, h->md_vel, h->md_types, h->d_mass, group,
+                                                   h->at<double>(c.nhc_partial), h->at<double>(c.nhc_partial) + 1024);
+    k_nhc<<<1, 256, 0, h->stream>>>(h->d_sc, h->d_nhc, nb, h->at<double>(c.nhc_partial),
+                                    h->at<double>(c.nhc_partial) + 1024, 0);
+    h->launches += 2;
+    CU(cudaStreamSynchronize(h->stream));
+    CU(cudaGetLastError());
+    h->md_group = group;
+    h->nhc_on = true;
+  }
+  if (h->use_graph && !build_step_graph(h)) h->use_graph = false;
+  return NEPZBL_OK;
+}
+
+int md_get_thermostat(nepzbl_handle* h, double* xi, double* vxi, double* t_group, double* conserved_extra) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready || !h->nhc_on) return fail(h, NEPZBL_E_STATE, "no thermostat is set");
+  const Carve& c = h->cv;
+  const int nb = (int)std::min<long long>(1024, (h->n + 255) / 256);
+  k_group_ke2_partial<<<nb, 256, 0, h->stream>>>((int)h->n, h->md_vel, h->md_types, h->d_mass, h->md_group,
+                                                 h->at<double>(c.nhc_partial), nullptr);
+  k_energy_final<<<1, 256, 0, h->stream>>>(-nb, h->at<double>(c.nhc_partial), h->d_esum);
+  h->launches += 2;
+  CU(cudaMemcpyAsync(h->h_esum, h->d_esum, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaMemcpyAsync(h->h_nhc, h->d_nhc, sizeof(NhcState), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  CU(cudaGetLastError());
+  const NhcState& s = *h->h_nhc;
+  for (int k = 0; k < s.M; ++k) {
+    if (xi) xi[k] = s.xi[k];
+    if (vxi) vxi[k] = s.vxi[k];
+  }
+  if (t_group) *t_group = s.nf > 0 ? h->h_esum[0] / (s.nf * 8.617333262e-5) : 0.0;
+  if (conserved_extra) {  // H' - E_kin - E_pot of ref. [32]
+    double e = 0.0;
+    for (int k = 0; k < s.M; ++k) {
+      double w = (k == 0 ? s.nf : 1.0) * s.kT;
+      e += 0.5 * w * s.tau * s.tau * s.vxi[k] * s.vxi[k] + w * s.xi[k];
+    }
+    *conserved_extra = e;
+  }
   return NEPZBL_OK;
 }
 
