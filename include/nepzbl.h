@@ -181,6 +181,23 @@ int md_set_thermostat(nepzbl_handle *h, const uint8_t *group, double temperature
                       int32_t chain_length);
 int md_get_thermostat(nepzbl_handle *h, double *xi, double *vxi, double *t_group, double *conserved_extra);
 
+/*
+ * Wigner-Seitz defect count: "The interstitials and vacancies were identified by
+ * using the Wigner-Seitz cell methods [34]".  Every atom is assigned to the reference site nearest
+ * to it (minimum image on periodic axes; exact for any atom position; ties go to the lowest site index,
+ * DESIGN.md C-25); a site with no atom is a vacancy, a site with m >= 2 atoms holds m - 1 interstitials.
+ * wigner_seitz_set_reference: site_soa dev fp64 [3][n_sites] (x[] y[] z[]), read during the call only
+ *   (the library keeps its own cell-sorted copy, freed at destroy or at the next set_reference); box, pbc
+ *   host.  Independent of the workspace and of md_init.
+ * wigner_seitz_count: pos_soa dev fp64 [3][n] (any n; the atoms need not be the reference's).  Outputs:
+ *   nearest dev int32 [n] (site index per atom, -1 for a non-finite position) or NULL; occupancy dev
+ *   int32 [n_sites] or NULL; n_vacancies, n_interstitials host or NULL.  Synchronises the stream.
+ */
+int wigner_seitz_set_reference(nepzbl_handle *h, int64_t n_sites, const double *site_soa,
+                               const double box[9], const int32_t pbc[3]);
+int wigner_seitz_count(nepzbl_handle *h, int64_t n, const double *pos_soa, int32_t *nearest,
+                       int32_t *occupancy, int64_t *n_vacancies, int64_t *n_interstitials);
+
 /* Number of kernel launches issued by this handle so far (for bench.py's gpu_launches). */
 int64_t nep_zbl_launch_count(const nepzbl_handle *h);
 

@@ -28,7 +28,7 @@ EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_d
            "nep_zbl_workspace_bytes", "nep_zbl_set_workspace", "neighbor_build", "neighbor_get",
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
            "md_run", "md_step_host", "md_energies", "md_get_forces", "md_get_counters",
-           "md_set_thermostat", "md_get_thermostat",
+           "md_set_thermostat", "md_get_thermostat", "wigner_seitz_set_reference", "wigner_seitz_count",
            "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
 PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "spare"]
 
@@ -100,6 +100,10 @@ _lib.md_set_thermostat.argtypes = [_vp, _vp, C.c_double, C.c_double, C.c_int32]
 _lib.md_set_thermostat.restype = C.c_int
 _lib.md_get_thermostat.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_dbl), C.POINTER(_dbl), C.POINTER(_dbl)]
 _lib.md_get_thermostat.restype = C.c_int
+_lib.wigner_seitz_set_reference.argtypes = [_vp, _i64, _vp, C.POINTER(_dbl), C.POINTER(_i32)]
+_lib.wigner_seitz_set_reference.restype = C.c_int
+_lib.wigner_seitz_count.argtypes = [_vp, _i64, _vp, _vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]
+_lib.wigner_seitz_count.restype = C.c_int
 _lib.nep_zbl_launch_count.argtypes = [_vp]
 _lib.nep_zbl_launch_count.restype = _i64
 _lib.nep_zbl_profile.argtypes = [_vp, C.c_int]
@@ -261,6 +265,20 @@ class NepZbl:
         self._chk(_lib.md_get_thermostat(self.h, xi, vxi, C.byref(tg), C.byref(ex)))
         m = self._chain
         return np.array(xi[:m]), np.array(vxi[:m]), tg.value, ex.value
+
+    def wigner_seitz_set_reference(self, site, box, pbc):
+        """site: fp64 device tensor (3, n_sites)."""
+        self._ws_ns = site.shape[-1]
+        self._chk(_lib.wigner_seitz_set_reference(self.h, self._ws_ns, _ptr(site), _box(box), _pbc(pbc)))
+
+    def wigner_seitz_count(self, pos, want_nearest: bool = True, want_occupancy: bool = True):
+        """pos: fp64 device tensor (3, n).  Returns nearest (n,), occupancy (n_sites,), (n_vac, n_sia)."""
+        n = pos.shape[-1]
+        nearest = torch.empty(n, dtype=torch.int32, device=self.device) if want_nearest else None
+        occ = torch.empty(self._ws_ns, dtype=torch.int32, device=self.device) if want_occupancy else None
+        nv = _i64(); ni = _i64()
+        self._chk(_lib.wigner_seitz_count(self.h, n, _ptr(pos), _ptr(nearest), _ptr(occ), C.byref(nv), C.byref(ni)))
+        return nearest, occ, (nv.value, ni.value)
 
     def nep_zbl_launch_count(self) -> int:
         return int(_lib.nep_zbl_launch_count(self.h))

@@ -17,6 +17,7 @@
 #include "descriptor.cuh"
 #include "force.cuh"
 #include "integrate.cuh"
+#include "wigner_seitz.cuh"
 
 namespace {
 
@@ -85,6 +86,17 @@ struct nepzbl_handle {
   NhcState* h_nhc = nullptr;              // pinned
   const unsigned char* md_group = nullptr;  // dev, caller-owned
   bool nhc_on = false;
+
+  // Wigner-Seitz reference (library-owned device arrays, freed at destroy)
+  struct {
+    long long ns = 0;
+    WsGrid g{};
+    int *cell_of = nullptr, *cell_count = nullptr, *cell_fill = nullptr, *cell_start = nullptr, *sidx = nullptr,
+        *occ = nullptr;
+    double *sx = nullptr, *sy = nullptr, *sz = nullptr;
+    unsigned long long* out = nullptr;    // dev [8]: bounds / counts
+    unsigned long long* h_out = nullptr;  // pinned [8]
+  } ws_ref;
 
   // one MD step captured as a CUDA graph: the list-rebuild chain and the ZBL kernel sit in IF nodes
   // whose conditions are set on the device (k_step_flag / k_zbl_gate), so a step is ONE launch
@@ -562,8 +574,20 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   return NEPZBL_OK;
 }
 
+static void ws_free(nepzbl_handle* h) {
+  auto& r = h->ws_ref;
+  cudaFree(r.cell_of); cudaFree(r.cell_count); cudaFree(r.cell_fill); cudaFree(r.cell_start); cudaFree(r.sidx);
+  cudaFree(r.occ); cudaFree(r.sx); cudaFree(r.sy); cudaFree(r.sz);
+  r.cell_of = r.cell_count = r.cell_fill = r.cell_start = r.sidx = r.occ = nullptr;
+  r.sx = r.sy = r.sz = nullptr;
+  r.ns = 0;
+}
+
 void nep_zbl_destroy(nepzbl_handle* h) {
   if (!h) return;
+  ws_free(h);
+  cudaFree(h->ws_ref.out);
+  cudaFreeHost(h->ws_ref.h_out);
   cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
   cudaFree(h->d_trace); cudaFree(h->d_esum); cudaFree(h->d_nhc);
   cudaFreeHost(h->h_nhc);
@@ -983,6 +1007,125 @@ int md_get_thermostat(nepzbl_handle* h, double* xi, double* vxi, double* t_group
     }
     *conserved_extra = e;
   }
+  return NEPZBL_OK;
+}
+
+// ------------------------------------------------------------------ Wigner-Seitz count
+
+int wigner_seitz_set_reference(nepzbl_handle* h, int64_t n_sites, const double* site_soa, const double box[9],
+                               const int32_t pbc[3]) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (n_sites < 1 || n_sites > 2000000000ll || !site_soa || !box || !pbc)
+    return fail(h, NEPZBL_E_INVALID_ARG, "bad wigner_seitz_set_reference arguments");
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      if (a != b && box[3 * a + b] != 0.0)
+        return fail(h, NEPZBL_E_BOX_NOT_ORTHOGONAL, "only orthogonal boxes are supported");
+  for (int a = 0; a < 3; ++a)
+    if (!(box[4 * a] > 0.0) || !std::isfinite(box[4 * a])) return fail(h, NEPZBL_E_INVALID_ARG, "box edge %d is not positive", a);
+  auto& r = h->ws_ref;
+  ws_free(h);
+  const int ns = (int)n_sites;
+  cudaStream_t st = h->stream;
+  if (!r.out) CU(cudaMalloc(&r.out, 8 * sizeof(unsigned long long)));
+  if (!r.h_out) CU(cudaMallocHost(&r.h_out, 8 * sizeof(unsigned long long)));
+  // bounds of the sites (grid extent on open axes)
+  for (int a = 0; a < 3; ++a) { r.h_out[a] = ~0ull; r.h_out[3 + a] = 0ull; }
+  CU(cudaMemcpyAsync(r.out, r.h_out, 6 * sizeof(unsigned long long), cudaMemcpyHostToDevice, st));
+  k_ws_bounds<<<blocks(ns, 256), 256, 0, st>>>(ns, site_soa, r.out);
+  CU(cudaMemcpyAsync(r.h_out, r.out, 6 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  h->launches += 1;
+  WsGrid g;
+  memset(&g, 0, sizeof g);
+  double ext[3], vol = 1.0;
+  for (int a = 0; a < 3; ++a) {
+    g.pbc[a] = pbc[a] != 0;
+    g.L[a] = box[4 * a];
+    if (g.pbc[a]) {
+      g.lo[a] = 0.0;
+      ext[a] = box[4 * a];
+    } else {
+      auto dec = [](unsigned long long k) {
+        unsigned long long b = (k & 0x8000000000000000ull) ? (k & 0x7fffffffffffffffull) : ~k;
+        double x;
+        memcpy(&x, &b, 8);
+        return x;
+      };
+      double mn = dec(r.h_out[a]), mx = dec(r.h_out[3 + a]);
+      if (!(mx >= mn)) return fail(h, NEPZBL_E_NONFINITE, "no finite reference site coordinates");
+      g.lo[a] = mn;
+      ext[a] = std::max(mx - mn, 1e-9);
+    }
+    vol *= ext[a];
+  }
+  // cells of about 4 sites: edge = cbrt(4 V / n_sites) (bcc W: 1.26 a0 = 4 A, well above the ~1.5 A an atom of
+  // a crystal sits from its nearest site, so the 27-cell block settles it)
+  const double edge = cbrt(4.0 * vol / (double)ns);
+  long long total = 1;
+  for (int a = 0; a < 3; ++a) {
+    long long nc = (long long)floor(ext[a] / edge);
+    if (nc < 1) nc = 1;
+    if (nc > 2048) nc = 2048;
+    g.nc[a] = (int)nc;
+    g.w[a] = ext[a] / (double)nc;
+    g.inv_w[a] = (double)nc / ext[a];
+    total *= nc;
+  }
+  while (total > 2000000000ll) {  // unreachable for n_sites < 2^31 with ~4 sites per cell; keeps ints safe
+    int a = g.nc[0] >= g.nc[1] && g.nc[0] >= g.nc[2] ? 0 : (g.nc[1] >= g.nc[2] ? 1 : 2);
+    total /= g.nc[a];
+    g.nc[a] = (g.nc[a] + 1) / 2;
+    g.w[a] = ext[a] / g.nc[a];
+    g.inv_w[a] = g.nc[a] / ext[a];
+    total *= g.nc[a];
+  }
+  g.ncells = (int)total;
+  CU(cudaMalloc(&r.cell_of, sizeof(int) * (size_t)ns));
+  CU(cudaMalloc(&r.cell_count, sizeof(int) * ((size_t)g.ncells + 1)));
+  CU(cudaMalloc(&r.cell_fill, sizeof(int) * ((size_t)g.ncells + 1)));
+  CU(cudaMalloc(&r.cell_start, sizeof(int) * ((size_t)g.ncells + 1)));
+  CU(cudaMalloc(&r.sidx, sizeof(int) * (size_t)ns));
+  CU(cudaMalloc(&r.occ, sizeof(int) * (size_t)ns));
+  CU(cudaMalloc(&r.sx, sizeof(double) * (size_t)ns));
+  CU(cudaMalloc(&r.sy, sizeof(double) * (size_t)ns));
+  CU(cudaMalloc(&r.sz, sizeof(double) * (size_t)ns));
+  CU(cudaMemsetAsync(r.cell_count, 0, sizeof(int) * ((size_t)g.ncells + 1), st));
+  CU(cudaMemsetAsync(r.cell_fill, 0, sizeof(int) * ((size_t)g.ncells + 1), st));
+  k_ws_bin<<<blocks(ns, 256), 256, 0, st>>>(g, ns, site_soa, r.cell_of, r.cell_count);
+  k_ws_scan<<<1, 1024, 0, st>>>(g.ncells, r.cell_count, r.cell_start);
+  k_ws_place<<<blocks(ns, 256), 256, 0, st>>>(ns, site_soa, r.cell_of, r.cell_start, r.cell_fill, r.sx, r.sy,
+                                             r.sz, r.sidx);
+  h->launches += 3;
+  CU(cudaStreamSynchronize(st));
+  CU(cudaGetLastError());
+  r.g = g;
+  r.ns = ns;
+  return NEPZBL_OK;
+}
+
+int wigner_seitz_count(nepzbl_handle* h, int64_t n, const double* pos_soa, int32_t* nearest, int32_t* occupancy,
+                       int64_t* n_vacancies, int64_t* n_interstitials) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  auto& r = h->ws_ref;
+  if (r.ns < 1) return fail(h, NEPZBL_E_STATE, "wigner_seitz_count before wigner_seitz_set_reference");
+  if (n < 0 || n > 2000000000ll || (n > 0 && !pos_soa)) return fail(h, NEPZBL_E_INVALID_ARG, "bad wigner_seitz_count arguments");
+  cudaStream_t st = h->stream;
+  int* occ = occupancy ? occupancy : r.occ;
+  CU(cudaMemsetAsync(occ, 0, sizeof(int) * (size_t)r.ns, st));
+  CU(cudaMemsetAsync(r.out, 0, 2 * sizeof(unsigned long long), st));
+  if (n > 0) {
+    k_ws_assign<<<blocks(n, 128), 128, 0, st>>>(r.g, (int)n, pos_soa, r.cell_start, r.sx, r.sy, r.sz, r.sidx,
+                                               nearest, occ);
+    h->launches += 1;
+  }
+  k_ws_count<<<std::min(blocks(r.ns, 256), 1184), 256, 0, st>>>((int)r.ns, occ, r.out);
+  h->launches += 1;
+  CU(cudaMemcpyAsync(r.h_out, r.out, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  CU(cudaStreamSynchronize(st));
+  CU(cudaGetLastError());
+  if (n_vacancies) *n_vacancies = (int64_t)r.h_out[0];
+  if (n_interstitials) *n_interstitials = (int64_t)r.h_out[1];
   return NEPZBL_OK;
 }
 

@@ -1,0 +1,193 @@
+// wigner_seitz.cuh -- SURVEY 8(f) NEXT-3: Wigner-Seitz defect count.
+//
+// "The interstitials and vacancies were identified by using the Wigner-Seitz cell methods [34]":
+// every atom is assigned to the reference lattice site nearest to it (minimum image on periodic axes), i.e.
+// to the Wigner-Seitz cell it sits in; a site with no atom is a vacancy, a site holding m >= 2 atoms carries
+// m - 1 interstitials.  Ties go to the lowest site index (C-25).
+//
+// Data-parallel over atoms, integer/HBM-bound: the reference sites are binned once into a grid of cells of
+// about 4 sites each (k_ws_bin / k_ws_scan / k_ws_place); k_ws_assign gives one thread per atom, scans the
+// 27 cells around the atom in fp64 and widens the block ring by ring until the best distance found is
+// provably smaller than the distance to every unscanned cell, so the result is the exact nearest site for
+// any atom position (sputtered atoms far from the lattice included).  Occupancies are integer atomics
+// (order-independent), so the counts are reproducible.
+#pragma once
+#include "common.cuh"
+
+struct WsGrid {  // host-filled, passed by value
+  double lo[3], L[3], w[3], inv_w[3];  // grid origin, box edge, cell width per axis
+  int nc[3], pbc[3];
+  int ncells;
+};
+
+__device__ __forceinline__ int ws_cell_1d(const WsGrid& g, int a, double x) {
+  if (g.pbc[a]) x -= g.L[a] * floor(x / g.L[a]);
+  int c = (int)floor((x - g.lo[a]) * g.inv_w[a]);
+  return c < 0 ? 0 : (c >= g.nc[a] ? g.nc[a] - 1 : c);
+}
+
+// min / max site coordinate per axis (order-preserving integer encoding), for the grid on open axes
+__global__ void __launch_bounds__(256)
+k_ws_bounds(int ns, const double* __restrict__ site, unsigned long long* __restrict__ mnmx) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  for (int a = 0; a < 3; ++a) {
+    double x = s < ns ? site[(size_t)a * ns + s] : 0.0;
+    bool ok = s < ns && isfinite(x);
+    unsigned long long kmin = ok ? enc_double(x) : ~0ull, kmax = ok ? enc_double(x) : 0ull;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      unsigned long long a1 = __shfl_xor_sync(0xffffffffu, kmin, o);
+      unsigned long long a2 = __shfl_xor_sync(0xffffffffu, kmax, o);
+      kmin = a1 < kmin ? a1 : kmin;
+      kmax = a2 > kmax ? a2 : kmax;
+    }
+    if ((threadIdx.x & 31) == 0) {
+      atomicMin(&mnmx[a], kmin);
+      atomicMax(&mnmx[3 + a], kmax);
+    }
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_ws_bin(const WsGrid g, int ns, const double* __restrict__ site, int* __restrict__ cell_of,
+         int* __restrict__ cell_count) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= ns) return;
+  int cx = ws_cell_1d(g, 0, site[s]), cy = ws_cell_1d(g, 1, site[(size_t)ns + s]),
+      cz = ws_cell_1d(g, 2, site[2 * (size_t)ns + s]);
+  int c = (cz * g.nc[1] + cy) * g.nc[0] + cx;
+  cell_of[s] = c;
+  atomicAdd(&cell_count[c], 1);
+}
+
+// exclusive scan of cell_count[0..ncells) -> cell_start[0..ncells]; one block of 1024 threads
+__global__ void __launch_bounds__(1024)
+k_ws_scan(int ncells, const int* __restrict__ cell_count, int* __restrict__ cell_start) {
+  __shared__ int part[1024];
+  int chunk = (ncells + 1023) / 1024;
+  int b = min(threadIdx.x * chunk, ncells), e = min(b + chunk, ncells);
+  int s = 0;
+  for (int c = b; c < e; ++c) s += cell_count[c];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {
+    int v = threadIdx.x >= o ? part[threadIdx.x - o] : 0;
+    __syncthreads();
+    part[threadIdx.x] += v;
+    __syncthreads();
+  }
+  int run = threadIdx.x ? part[threadIdx.x - 1] : 0;
+  for (int c = b; c < e; ++c) {
+    cell_start[c] = run;
+    run += cell_count[c];
+  }
+  if (threadIdx.x == 1023) cell_start[ncells] = part[1023];
+}
+
+// sites in cell order: {x, y, z} and the original index.  The order inside a cell is the ticket order of
+// the atomics; the assignment below does not depend on it (ties are broken by site index).
+__global__ void __launch_bounds__(256)
+k_ws_place(int ns, const double* __restrict__ site, const int* __restrict__ cell_of,
+           const int* __restrict__ cell_start, int* __restrict__ cell_fill, double* __restrict__ sx,
+           double* __restrict__ sy, double* __restrict__ sz, int* __restrict__ sidx) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= ns) return;
+  int c = cell_of[s];
+  int k = cell_start[c] + atomicAdd(&cell_fill[c], 1);
+  sx[k] = site[s];
+  sy[k] = site[(size_t)ns + s];
+  sz[k] = site[2 * (size_t)ns + s];
+  sidx[k] = s;
+}
+
+// One thread per atom: exact nearest reference site.  Distances are evaluated in fp64 with the same
+// operations in the same order as the plain definition (d = site - pos; d -= L rint(d / L) on periodic
+// axes; r2 = (dx^2 + dy^2) + dz^2, no FMA contraction), so the chosen index is the definition's.
+__global__ void __launch_bounds__(128)
+k_ws_assign(const WsGrid g, int n, const double* __restrict__ pos, const int* __restrict__ cell_start,
+            const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
+            const int* __restrict__ sidx, int* __restrict__ nearest, int* __restrict__ occ) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double p[3] = {pos[i], pos[(size_t)n + i], pos[2 * (size_t)n + i]};
+  if (!(isfinite(p[0]) && isfinite(p[1]) && isfinite(p[2]))) {
+    if (nearest) nearest[i] = -1;
+    return;
+  }
+  int c[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) c[a] = ws_cell_1d(g, a, p[a]);
+  double best = INFINITY;
+  int bs = 0x7fffffff;
+  // R = 1 (27 cells, ~100 sites) settles every atom of a crystal; a wider block is rescanned whole (rare)
+  for (int R = 1;; ++R) {
+    int lo[3], hi[3], covered[3];
+    double bound = INFINITY;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      lo[a] = c[a] - R;
+      hi[a] = c[a] + R;
+      if (g.pbc[a]) {
+        covered[a] = 2 * R + 1 >= g.nc[a];
+        if (covered[a]) { lo[a] = 0; hi[a] = g.nc[a] - 1; }
+      } else {
+        if (lo[a] < 0) lo[a] = 0;
+        if (hi[a] > g.nc[a] - 1) hi[a] = g.nc[a] - 1;
+        covered[a] = lo[a] == 0 && hi[a] == g.nc[a] - 1;
+      }
+      // a site in a cell outside the block along this axis is at least R cell widths away along it
+      if (!covered[a]) bound = fmin(bound, R * g.w[a]);
+    }
+    for (int vz = lo[2]; vz <= hi[2]; ++vz) {
+      int cz = vz;
+      if (g.pbc[2] && !covered[2]) cz = vz < 0 ? vz + g.nc[2] : (vz >= g.nc[2] ? vz - g.nc[2] : vz);
+      for (int vy = lo[1]; vy <= hi[1]; ++vy) {
+        int cy = vy;
+        if (g.pbc[1] && !covered[1]) cy = vy < 0 ? vy + g.nc[1] : (vy >= g.nc[1] ? vy - g.nc[1] : vy);
+        for (int vx = lo[0]; vx <= hi[0]; ++vx) {
+          int cx = vx;
+          if (g.pbc[0] && !covered[0]) cx = vx < 0 ? vx + g.nc[0] : (vx >= g.nc[0] ? vx - g.nc[0] : vx);
+          const int cell = (cz * g.nc[1] + cy) * g.nc[0] + cx;
+          const int b = cell_start[cell], e = cell_start[cell + 1];
+          for (int k = b; k < e; ++k) {
+            double d0 = sx[k] - p[0], d1 = sy[k] - p[1], d2 = sz[k] - p[2];
+            if (g.pbc[0]) d0 = __dsub_rn(d0, __dmul_rn(g.L[0], rint(d0 / g.L[0])));
+            if (g.pbc[1]) d1 = __dsub_rn(d1, __dmul_rn(g.L[1], rint(d1 / g.L[1])));
+            if (g.pbc[2]) d2 = __dsub_rn(d2, __dmul_rn(g.L[2], rint(d2 / g.L[2])));
+            double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d0, d0), __dmul_rn(d1, d1)), __dmul_rn(d2, d2));
+            int s = sidx[k];
+            if (r2 < best || (r2 == best && s < bs)) {
+              best = r2;
+              bs = s;
+            }
+          }
+        }
+      }
+    }
+    if (best < bound * bound || (covered[0] && covered[1] && covered[2])) break;
+  }
+  if (bs == 0x7fffffff) bs = -1;  // no reference sites at all
+  if (nearest) nearest[i] = bs;
+  if (bs >= 0) atomicAdd(&occ[bs], 1);
+}
+
+// out[0] = number of sites with no atom (vacancies), out[1] = sum over sites of max(occ - 1, 0)
+// (interstitials); integer atomics, order-independent
+__global__ void __launch_bounds__(256)
+k_ws_count(int ns, const int* __restrict__ occ, unsigned long long* __restrict__ out) {
+  unsigned long long v = 0, q = 0;
+  for (int s = blockIdx.x * blockDim.x + threadIdx.x; s < ns; s += gridDim.x * blockDim.x) {
+    int o = occ[s];
+    v += o == 0;
+    q += o > 1 ? (unsigned long long)(o - 1) : 0ull;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    v += __shfl_xor_sync(0xffffffffu, v, o);
+    q += __shfl_xor_sync(0xffffffffu, q, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    if (v) atomicAdd(&out[0], v);
+    if (q) atomicAdd(&out[1], q);
+  }
+}
