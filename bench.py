@@ -54,6 +54,9 @@ FLOP_PER_ATOM = {k: sum(STEP_FLOP[s] for s in v) for k, v in KERNEL_STEPS.items(
 BYTES_PER_ATOM = {"integrate_a": 152.0, "kick_b": 64.0, "k_radial": 392.0, "k_angular_nn": 612.0,
                   "k_force": 1136.0}
 FP32_LANES_PER_SM = 128
+# Wigner-Seitz count, compulsory HBM bytes per atom (one site per atom): position 24 + nearest 4 + occupancy
+# read-modify-write 8 + count read 4 + cell-sorted site record 28 (the 27-cell scan re-reads sites from L1/L2)
+WS_BYTES_PER_ATOM = 68.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on config2 (128 000 atoms) from the committed
 # `ncu --set full` capture (NCU_TRAFFIC_SOURCE); reported as roofline.traffic for that workload only.
 NCU_TRAFFIC_BYTES = {"k_radial": 48.145152e6 + 3.609856e6, "k_angular_nn": 50.303232e6 + 17.240832e6,
@@ -319,6 +322,53 @@ def run_b200(args):
     wall_e2e = (time.perf_counter() - t0) * 1e3
     ms_e2e = aggregate_max(max(eve0.elapsed_time(eve1), wall_e2e), world, dev)
     e2e_value = total_atoms * Ke / (ms_e2e * 1e-3)
+    # ---- SURVEY 8(f) NEXT rows, same workload: border-layer Nose-Hoover chain and Wigner-Seitz count
+    next_rows = None
+    if world == 1 and not args.no_next:
+        from paper_2305_08140_b200 import workloads as wl_
+        group = torch.from_numpy(wl_.border_group(w.pos, w.box, w.pbc)).to(dev)
+        pos, vel = fresh_state()
+        g.md_set_thermostat(group, 300.0, 100.0, 4)
+        Kn = min(K, 200)
+        g.md_run(W, dt_max, max_disp)
+        evn0, evn1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        evn0.record(stream)
+        g.md_run(Kn, dt_max, max_disp)
+        evn1.record(stream)
+        barrier()
+        ms_nhc = evn0.elapsed_time(evn1) / Kn
+        t_group = g.md_get_thermostat()[2]
+        g.md_set_thermostat(None, 300.0, 100.0, 4)
+        site = torch.from_numpy(w.pos.copy()).to(dev)       # reference = the initial lattice
+        g.wigner_seitz_set_reference(site, w.box, w.pbc)
+        for _ in range(3):
+            g.wigner_seitz_count(pos, want_nearest=True, want_occupancy=True)
+        evw0, evw1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 20
+        barrier()
+        evw0.record(stream)
+        for _ in range(reps):
+            _, _, ws_counts = g.wigner_seitz_count(pos, want_nearest=True, want_occupancy=True)
+        evw1.record(stream)
+        barrier()
+        ms_ws = evw0.elapsed_time(evw1) / reps
+        hbm_peak_ = 6650.0
+        try:
+            hbm_peak_ = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs", 6650.0))
+        except OSError:
+            pass
+        ws_gbs = WS_BYTES_PER_ATOM * n / (ms_ws * 1e-3) / 1e9
+        next_rows = {
+            "nhc_border_layer": {"ms_per_step": ms_nhc, "atom_steps_per_s": n / (ms_nhc * 1e-3), "steps": Kn,
+                                 "group_atoms": int(group.sum().item()), "t_group_K": t_group,
+                                 "chain": 4, "tau_fs": 100.0},
+            "wigner_seitz": {"ms_per_count": ms_ws, "atoms_per_s": n / (ms_ws * 1e-3), "sites": n,
+                             "vacancies": ws_counts[0], "interstitials": ws_counts[1],
+                             "roofline": {"bound": "hbm", "achieved": ws_gbs, "peak": hbm_peak_, "unit": "GB/s",
+                                          "frac": ws_gbs / hbm_peak_, "bytes_per_atom": WS_BYTES_PER_ATOM},
+                             "includes": "occupancy memset, assignment, count, 16-byte D2H of the totals, stream sync"},
+        }
     if sampler:
         sampler.stop()
 
@@ -375,6 +425,7 @@ def run_b200(args):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
                 "steps": Ke, "api": "md_step_host"},
         "gpu_launches": int(launches),
+        "next_rows": next_rows,
         "context": {"paper": "1.3e7 atom-step/s, one 40-GB A100, trained W NEP-ZBL (n_max 15/10, 100 neurons), Table IV"},
     }
     print(json.dumps(line))
@@ -392,6 +443,7 @@ def main(argv=None):
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--flush-steps", type=int, default=100)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the SURVEY 8(f) NEXT rows (thermostat, Wigner-Seitz)")
     ap.add_argument("--traffic-bytes", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture")
     args = ap.parse_args(argv)

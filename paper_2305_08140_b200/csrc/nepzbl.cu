@@ -91,9 +91,8 @@ struct nepzbl_handle {
   struct {
     long long ns = 0;
     WsGrid g{};
-    int *cell_of = nullptr, *cell_count = nullptr, *cell_fill = nullptr, *cell_start = nullptr, *sidx = nullptr,
-        *occ = nullptr;
-    double *sx = nullptr, *sy = nullptr, *sz = nullptr;
+    int *cell_of = nullptr, *cell_count = nullptr, *cell_fill = nullptr, *cell_start = nullptr, *occ = nullptr;
+    WsSite* rec = nullptr;                // cell-sorted {x, y, z, index}
     unsigned long long* out = nullptr;    // dev [8]: bounds / counts
     unsigned long long* h_out = nullptr;  // pinned [8]
   } ws_ref;
@@ -576,10 +575,10 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
 
 static void ws_free(nepzbl_handle* h) {
   auto& r = h->ws_ref;
-  cudaFree(r.cell_of); cudaFree(r.cell_count); cudaFree(r.cell_fill); cudaFree(r.cell_start); cudaFree(r.sidx);
-  cudaFree(r.occ); cudaFree(r.sx); cudaFree(r.sy); cudaFree(r.sz);
-  r.cell_of = r.cell_count = r.cell_fill = r.cell_start = r.sidx = r.occ = nullptr;
-  r.sx = r.sy = r.sz = nullptr;
+  cudaFree(r.cell_of); cudaFree(r.cell_count); cudaFree(r.cell_fill); cudaFree(r.cell_start);
+  cudaFree(r.occ); cudaFree(r.rec);
+  r.cell_of = r.cell_count = r.cell_fill = r.cell_start = r.occ = nullptr;
+  r.rec = nullptr;
   r.ns = 0;
 }
 
@@ -1085,17 +1084,13 @@ int wigner_seitz_set_reference(nepzbl_handle* h, int64_t n_sites, const double* 
   CU(cudaMalloc(&r.cell_count, sizeof(int) * ((size_t)g.ncells + 1)));
   CU(cudaMalloc(&r.cell_fill, sizeof(int) * ((size_t)g.ncells + 1)));
   CU(cudaMalloc(&r.cell_start, sizeof(int) * ((size_t)g.ncells + 1)));
-  CU(cudaMalloc(&r.sidx, sizeof(int) * (size_t)ns));
   CU(cudaMalloc(&r.occ, sizeof(int) * (size_t)ns));
-  CU(cudaMalloc(&r.sx, sizeof(double) * (size_t)ns));
-  CU(cudaMalloc(&r.sy, sizeof(double) * (size_t)ns));
-  CU(cudaMalloc(&r.sz, sizeof(double) * (size_t)ns));
+  CU(cudaMalloc(&r.rec, sizeof(WsSite) * (size_t)ns));
   CU(cudaMemsetAsync(r.cell_count, 0, sizeof(int) * ((size_t)g.ncells + 1), st));
   CU(cudaMemsetAsync(r.cell_fill, 0, sizeof(int) * ((size_t)g.ncells + 1), st));
   k_ws_bin<<<blocks(ns, 256), 256, 0, st>>>(g, ns, site_soa, r.cell_of, r.cell_count);
   k_ws_scan<<<1, 1024, 0, st>>>(g.ncells, r.cell_count, r.cell_start);
-  k_ws_place<<<blocks(ns, 256), 256, 0, st>>>(ns, site_soa, r.cell_of, r.cell_start, r.cell_fill, r.sx, r.sy,
-                                             r.sz, r.sidx);
+  k_ws_place<<<blocks(ns, 256), 256, 0, st>>>(ns, site_soa, r.cell_of, r.cell_start, r.cell_fill, r.rec);
   h->launches += 3;
   CU(cudaStreamSynchronize(st));
   CU(cudaGetLastError());
@@ -1115,8 +1110,7 @@ int wigner_seitz_count(nepzbl_handle* h, int64_t n, const double* pos_soa, int32
   CU(cudaMemsetAsync(occ, 0, sizeof(int) * (size_t)r.ns, st));
   CU(cudaMemsetAsync(r.out, 0, 2 * sizeof(unsigned long long), st));
   if (n > 0) {
-    k_ws_assign<<<blocks(n, 128), 128, 0, st>>>(r.g, (int)n, pos_soa, r.cell_start, r.sx, r.sy, r.sz, r.sidx,
-                                               nearest, occ);
+    k_ws_assign<<<blocks(n, 128), 128, 0, st>>>(r.g, (int)n, pos_soa, r.cell_start, r.rec, nearest, occ);
     h->launches += 1;
   }
   k_ws_count<<<std::min(blocks(r.ns, 256), 1184), 256, 0, st>>>((int)r.ns, occ, r.out);

@@ -84,29 +84,51 @@ k_ws_scan(int ncells, const int* __restrict__ cell_count, int* __restrict__ cell
   if (threadIdx.x == 1023) cell_start[ncells] = part[1023];
 }
 
-// sites in cell order: {x, y, z} and the original index.  The order inside a cell is the ticket order of
-// the atomics; the assignment below does not depend on it (ties are broken by site index).
+// sites in cell order as 32-byte records {x, y, z, index}: the assignment reads one record with ONE 256-bit
+// load (the first version kept x, y, z, index in four arrays and was bound by the L1 wavefronts of four
+// scattered loads per candidate: 102 us for 128 000 atoms).  The order inside a cell is the ticket order of
+// the atomics; the assignment does not depend on it (ties are broken by site index).
+struct __align__(32) WsSite {
+  double x, y, z;
+  int idx, pad;
+};
 __global__ void __launch_bounds__(256)
 k_ws_place(int ns, const double* __restrict__ site, const int* __restrict__ cell_of,
-           const int* __restrict__ cell_start, int* __restrict__ cell_fill, double* __restrict__ sx,
-           double* __restrict__ sy, double* __restrict__ sz, int* __restrict__ sidx) {
+           const int* __restrict__ cell_start, int* __restrict__ cell_fill, WsSite* __restrict__ rec) {
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= ns) return;
   int c = cell_of[s];
   int k = cell_start[c] + atomicAdd(&cell_fill[c], 1);
-  sx[k] = site[s];
-  sy[k] = site[(size_t)ns + s];
-  sz[k] = site[2 * (size_t)ns + s];
-  sidx[k] = s;
+  WsSite r;
+  r.x = site[s];
+  r.y = site[(size_t)ns + s];
+  r.z = site[2 * (size_t)ns + s];
+  r.idx = s;
+  r.pad = 0;
+  rec[k] = r;
+}
+__device__ __forceinline__ void ws_load(const WsSite* p, double& x, double& y, double& z, int& idx) {
+  unsigned v0, v1, v2, v3, v4, v5, v6, v7;
+  asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3), "=r"(v4), "=r"(v5), "=r"(v6), "=r"(v7)
+               : "l"(p));
+  (void)v7;
+  x = __hiloint2double((int)v1, (int)v0);
+  y = __hiloint2double((int)v3, (int)v2);
+  z = __hiloint2double((int)v5, (int)v4);
+  idx = (int)v6;
 }
 
 // One thread per atom: exact nearest reference site.  Distances are evaluated in fp64 with the same
 // operations in the same order as the plain definition (d = site - pos; d -= L rint(d / L) on periodic
 // axes; r2 = (dx^2 + dy^2) + dz^2, no FMA contraction), so the chosen index is the definition's.
+// The atom's own cell is scanned first; another cell of the block is scanned only if the box of that cell
+// comes closer to the atom than the best site found so far (with a 1e-9 safety margin for the rounding of
+// the cell geometry), which leaves ~10 candidates per atom of a crystal instead of the ~108 of all 27 cells
+// (the kernel is instruction-bound: ncu, profiles/).
 __global__ void __launch_bounds__(128)
 k_ws_assign(const WsGrid g, int n, const double* __restrict__ pos, const int* __restrict__ cell_start,
-            const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
-            const int* __restrict__ sidx, int* __restrict__ nearest, int* __restrict__ occ) {
+            const WsSite* __restrict__ rec, int* __restrict__ nearest, int* __restrict__ occ) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const double p[3] = {pos[i], pos[(size_t)n + i], pos[2 * (size_t)n + i]};
@@ -115,11 +137,44 @@ k_ws_assign(const WsGrid g, int n, const double* __restrict__ pos, const int* __
     return;
   }
   int c[3];
+  double fa[3];  // coordinate of the atom relative to the lower face of its cell (outside [0, w) only for
+                 // atoms beyond the grid on open axes, which are binned into the boundary cell)
 #pragma unroll
-  for (int a = 0; a < 3; ++a) c[a] = ws_cell_1d(g, a, p[a]);
+  for (int a = 0; a < 3; ++a) {
+    c[a] = ws_cell_1d(g, a, p[a]);
+    double x = p[a];
+    if (g.pbc[a]) x -= g.L[a] * floor(x / g.L[a]);
+    fa[a] = (x - g.lo[a]) - c[a] * g.w[a];
+  }
+  const double hL[3] = {0.5 * g.L[0], 0.5 * g.L[1], 0.5 * g.L[2]};
   double best = INFINITY;
   int bs = 0x7fffffff;
-  // R = 1 (27 cells, ~100 sites) settles every atom of a crystal; a wider block is rescanned whole (rare)
+  auto scan_cell = [&](int cell) {
+    const int b = cell_start[cell], e = cell_start[cell + 1];
+    for (int k = b; k < e; ++k) {
+      double qx, qy, qz;
+      int s;
+      ws_load(rec + k, qx, qy, qz, s);
+      double d0 = qx - p[0], d1 = qy - p[1], d2 = qz - p[2];
+      // |d| <= L/2  =>  rint(d / L) == 0 (correctly rounded division is monotone, halves round to
+      // even) and d - L * 0 == d: skipping the fp64 division there leaves every bit unchanged
+      if (g.pbc[0] && fabs(d0) > hL[0]) d0 = __dsub_rn(d0, __dmul_rn(g.L[0], rint(d0 / g.L[0])));
+      if (g.pbc[1] && fabs(d1) > hL[1]) d1 = __dsub_rn(d1, __dmul_rn(g.L[1], rint(d1 / g.L[1])));
+      if (g.pbc[2] && fabs(d2) > hL[2]) d2 = __dsub_rn(d2, __dmul_rn(g.L[2], rint(d2 / g.L[2])));
+      double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d0, d0), __dmul_rn(d1, d1)), __dmul_rn(d2, d2));
+      if (r2 < best || (r2 == best && s < bs)) {
+        best = r2;
+        bs = s;
+      }
+    }
+  };
+  // distance along axis a from the atom to the cell at offset o from its own cell (0 if it overlaps)
+  auto axis_gap = [&](int a, int o) -> double {
+    double lo = o * g.w[a] - fa[a], hi = lo + g.w[a];
+    return lo > 0.0 ? lo : (hi < 0.0 ? -hi : 0.0);
+  };
+  scan_cell((c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0]);
+  // R = 1 (27 cells) settles every atom of a crystal; a wider block is walked again whole (rare)
   for (int R = 1;; ++R) {
     int lo[3], hi[3], covered[3];
     double bound = INFINITY;
@@ -141,26 +196,20 @@ k_ws_assign(const WsGrid g, int n, const double* __restrict__ pos, const int* __
     for (int vz = lo[2]; vz <= hi[2]; ++vz) {
       int cz = vz;
       if (g.pbc[2] && !covered[2]) cz = vz < 0 ? vz + g.nc[2] : (vz >= g.nc[2] ? vz - g.nc[2] : vz);
+      const double gz = (g.pbc[2] && covered[2]) ? 0.0 : axis_gap(2, vz - c[2]);
       for (int vy = lo[1]; vy <= hi[1]; ++vy) {
         int cy = vy;
         if (g.pbc[1] && !covered[1]) cy = vy < 0 ? vy + g.nc[1] : (vy >= g.nc[1] ? vy - g.nc[1] : vy);
+        const double gy = (g.pbc[1] && covered[1]) ? 0.0 : axis_gap(1, vy - c[1]);
+        const double gyz = gy * gy + gz * gz;
         for (int vx = lo[0]; vx <= hi[0]; ++vx) {
           int cx = vx;
           if (g.pbc[0] && !covered[0]) cx = vx < 0 ? vx + g.nc[0] : (vx >= g.nc[0] ? vx - g.nc[0] : vx);
-          const int cell = (cz * g.nc[1] + cy) * g.nc[0] + cx;
-          const int b = cell_start[cell], e = cell_start[cell + 1];
-          for (int k = b; k < e; ++k) {
-            double d0 = sx[k] - p[0], d1 = sy[k] - p[1], d2 = sz[k] - p[2];
-            if (g.pbc[0]) d0 = __dsub_rn(d0, __dmul_rn(g.L[0], rint(d0 / g.L[0])));
-            if (g.pbc[1]) d1 = __dsub_rn(d1, __dmul_rn(g.L[1], rint(d1 / g.L[1])));
-            if (g.pbc[2]) d2 = __dsub_rn(d2, __dmul_rn(g.L[2], rint(d2 / g.L[2])));
-            double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d0, d0), __dmul_rn(d1, d1)), __dmul_rn(d2, d2));
-            int s = sidx[k];
-            if (r2 < best || (r2 == best && s < bs)) {
-              best = r2;
-              bs = s;
-            }
-          }
+          const double gx = (g.pbc[0] && covered[0]) ? 0.0 : axis_gap(0, vx - c[0]);
+          const double dmin2 = gx * gx + gyz;
+          if (dmin2 > best * (1.0 + 1e-9) + 1e-9) continue;  // no site of this cell can beat or tie the best
+          if (R == 1 && cx == c[0] && cy == c[1] && cz == c[2]) continue;  // own cell: scanned above
+          scan_cell((cz * g.nc[1] + cy) * g.nc[0] + cx);
         }
       }
     }
