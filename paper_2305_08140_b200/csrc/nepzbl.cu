@@ -15,6 +15,7 @@
 #include "common.cuh"
 #include "neighbor.cuh"
 #include "descriptor.cuh"
+#include "descriptor_split.cuh"
 #include "force.cuh"
 #include "integrate.cuh"
 #include "wigner_seitz.cuh"
@@ -187,9 +188,23 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   return c;
 }
 
-const ShapeId kShapes[] = {{5, 9, 5, 9, 1}, {5, 9, 5, 9, 0}};
+// instantiated model shapes: BASELINE.json configs (with / without the 4-body term) and the paper's own
+// sizes (n_max 15 / 10, l_max 4; basis 8 / 8 is DESIGN.md C-26) -- SURVEY 8(f) NEXT-2
+const ShapeId kShapes[] = {{5, 9, 5, 9, 1}, {5, 9, 5, 9, 0}, {16, 9, 11, 9, 0}};
 using MS0 = ModelShape<5, 9, 5, 9, true>;
 using MS1 = ModelShape<5, 9, 5, 9, false>;
+using MS2 = ModelShape<16, 9, 11, 9, false>;
+template <class F>
+void with_shape(int shape, F&& f) {
+  switch (shape) {
+    case 0: f(MS0{}); break;
+    case 1: f(MS1{}); break;
+    default: f(MS2{}); break;
+  }
+}
+// models with more than 5 angular channels use the four-lanes-per-atom kernel (descriptor_split.cuh)
+template <class MS>
+constexpr bool kSplit = MS::NA > 5;
 
 template <class MS>
 void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
@@ -218,14 +233,20 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   t.n_neurons = p->n_neurons;
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
-  const size_t nrow = (size_t)nn_rows(p->n_neurons);
-  h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
+  if (kSplit<MS>) {
+    h->smem_nn = sizeof(float) * (size_t)split_smem_floats<MS>(nn_rows_split(p->n_neurons));
+  } else {
+    const size_t nrow = (size_t)nn_rows(p->n_neurons);
+    h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
+  }
 }
 
 template <class MS>
 std::vector<float> build_nnw(const nepzbl_params* p) {
-  const int neu2 = nn_rows(p->n_neurons);  // zero padding rows, see nn_rows
-  std::vector<float> w((size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD, 0.0f);
+  // zero padding rows, see nn_rows / nn_rows_split; the split kernel's table also carries the folded
+  // angular coefficients ct[NAP][KA] (rows >= NA zero) behind q_scaler
+  const int neu2 = kSplit<MS> ? nn_rows_split(p->n_neurons) : nn_rows(p->n_neurons);
+  std::vector<float> w(kSplit<MS> ? (size_t)split_smem_floats<MS>(neu2) : (size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD, 0.0f);
   for (int m = 0; m < p->n_neurons; ++m)
     for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
   float* b0 = w.data() + (size_t)neu2 * MS::DPAD;
@@ -236,6 +257,15 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
     w1[m] = (float)p->w1[m];
   }
   for (int v = 0; v < MS::D; ++v) qs[v] = (float)p->q_scaler[v];
+  if (kSplit<MS>) {
+    float* ct = qs + MS::DPAD;
+    for (int nq = 0; nq < MS::NA; ++nq) {
+      double sum = 0.0;
+      for (int k = 1; k < MS::KA; ++k) sum += p->c_angular[nq * MS::KA + k];
+      for (int k = 0; k < MS::KA; ++k)
+        ct[nq * MS::KA + k] = (float)(k == 0 ? p->c_angular[nq * MS::KA] + 0.5 * sum : 0.5 * p->c_angular[nq * MS::KA + k]);
+    }
+  }
   return w;
 }
 
@@ -322,10 +352,16 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
                                               h->at<int>(c.zbl_list), h->at<int>(c.nn_a),
                                               h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp));
   prof_mark(h, PK_ANGULAR_NN);
-  k_angular_nn<MS><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
-      n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
-      h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
-      want_q ? h->at<float>(c.q_desc) : nullptr);
+  if constexpr (kSplit<MS>)
+    k_angular_nn_split<MS><<<std::min(blocks((long long)n * SPLIT_LANES, SPLIT_THREADS), h->ang_grid), SPLIT_THREADS, h->smem_nn, st>>>(
+        n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
+        h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
+        want_q ? h->at<float>(c.q_desc) : nullptr);
+  else
+    k_angular_nn<MS><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
+        n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
+        h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
+        want_q ? h->at<float>(c.q_desc) : nullptr);
   prof_mark(h, PK_FORCE);
   if (virial)
     k_force<MS, true><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
@@ -350,8 +386,7 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
 
 void enqueue_eval(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
                   bool want_q, bool with_zbl = true) {
-  if (h->shape == 0) enqueue_eval_t<MS0>(h, pos, energy, force, virial, want_q, with_zbl);
-  else enqueue_eval_t<MS1>(h, pos, energy, force, virial, want_q, with_zbl);
+  with_shape(h->shape, [&](auto ms) { enqueue_eval_t<decltype(ms)>(h, pos, energy, force, virial, want_q, with_zbl); });
 }
 
 void enqueue_zbl(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial, cudaStream_t st) {
@@ -517,8 +552,12 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   h->stream = (cudaStream_t)cuda_stream;
   if (const char* ng = getenv("NEPZBL_NO_GRAPH")) h->use_graph = !(ng[0] == '1');  // see nepzbl.h (md_step)
   std::vector<float> nnw;
-  if (shape == 0) { build_tables<MS0>(h, p); nnw = build_nnw<MS0>(p); h->D = MS0::D; }
-  else { build_tables<MS1>(h, p); nnw = build_nnw<MS1>(p); h->D = MS1::D; }
+  with_shape(shape, [&](auto ms) {
+    using MS = decltype(ms);
+    build_tables<MS>(h, p);
+    nnw = build_nnw<MS>(p);
+    h->D = MS::D;
+  });
   ZblParams& z = h->zp;
   memset(&z, 0, sizeof z);
   z.r_inner = p->zbl_r_inner; z.r_outer = p->zbl_r_outer; z.n_terms = p->zbl_n_terms;
@@ -538,10 +577,16 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   if ((ce = cudaSetDevice(device)) != cudaSuccess) return die("cudaSetDevice", ce);
   if ((ce = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return die("cudaDeviceGetAttribute", ce);
   {  // k_angular_nn: opt in to its dynamic shared memory and size the persistent grid to the resident blocks
-    const void* fn = shape == 0 ? (const void*)k_angular_nn<MS0> : (const void*)k_angular_nn<MS1>;
+    const void* fn = nullptr;
+    int threads = ANG_THREADS;
+    with_shape(shape, [&](auto ms) {
+      using MS = decltype(ms);
+      if constexpr (kSplit<MS>) { fn = (const void*)k_angular_nn_split<MS>; threads = SPLIT_THREADS; }
+      else fn = (const void*)k_angular_nn<MS>;
+    });
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_nn)) != cudaSuccess) return die("cudaFuncSetAttribute(k_angular_nn)", ce);
     int per_sm = 0;
-    if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, ANG_THREADS, h->smem_nn)) != cudaSuccess) return die("cudaOccupancyMaxActiveBlocksPerMultiprocessor", ce);
+    if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, h->smem_nn)) != cudaSuccess) return die("cudaOccupancyMaxActiveBlocksPerMultiprocessor", ce);
     if (per_sm < 1) return die("k_angular_nn does not fit one SM", cudaErrorInvalidConfiguration);
     h->ang_grid = per_sm * h->n_sm;
   }

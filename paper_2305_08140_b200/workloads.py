@@ -173,10 +173,9 @@ def config1(seed: int = 1, cells: int = 10, n_pairs: int = 5, sigma: float = 0.0
 
 
 def thermal_bulk(cells, seed: int, temperature: float = 300.0, model: dict | None = None,
-                 name: str = "bulk", sigma_pos: float = 0.0) -> Workload:
+                 name: str = "bulk", sigma_pos: float = 0.0, a: float = A0_CONFIG) -> Workload:
     """Perfect bcc W lattice (optionally displaced), periodic, Maxwell-Boltzmann velocities."""
     nx, ny, nz = (cells, cells, cells) if np.isscalar(cells) else cells
-    a = A0_CONFIG
     pos = bcc_lattice(nx, ny, nz, a)
     n = pos.shape[1]
     if sigma_pos > 0:
@@ -316,3 +315,25 @@ def defective_lattice(cells, seed: int, n_vacancies: int, n_interstitials: int, 
             pos[ax] = np.mod(pos[ax], L[ax])
     info = dict(vacant=sorted(int(v) for v in vac + fr_from), double=sorted(int(v) for v in dbl + fr_to))
     return site, np.ascontiguousarray(pos), box, pbc, info
+
+
+A0_PAPER = 3.185                      # lattice constant of the paper's NEP-ZBL model
+
+
+def paper_model(seed: int = 121, **kw) -> dict:
+    """a synthetic parameter set with the SIZES of the paper's trained W model (P:106:
+    n_max 15 / 10, l_max 4, 100 neurons, cutoffs 6 / 4 A; no 4-body term is mentioned) and the paper's own
+    W-W ZBL refit (Eq. 3) -- the weights themselves are seeded random numbers, the trained model
+    is not available.  Chebyshev basis size 8 / 8: DESIGN.md C-26 (the paper does not state it)."""
+    return synthetic_model(seed=seed, n_max_radial=15, n_max_angular=10, basis_radial=8, basis_angular=8,
+                           l_max=4, has_4body=0, n_neurons=100, zbl="paper", **kw)
+
+
+def paper_bulk(cells: int, seed: int, temperature: float = 300.0, sigma_pos: float = 0.0,
+               model: dict | None = None) -> Workload:
+    """Periodic bcc W at the paper's lattice constant with the paper-sized model; adaptive step
+    0.01 A per step, dt <= 1 fs."""
+    w = thermal_bulk(cells, seed, temperature=temperature, model=model or paper_model(), name="paper_bulk",
+                     sigma_pos=sigma_pos, a=A0_PAPER)
+    w.dt_max, w.max_displacement = 1.0, 0.01
+    return w
