@@ -50,6 +50,16 @@ L2_BYTES = 126 * 1024 * 1024
 STEP_FLOP = {"S3": 3.2e3, "S4": 6.7e3, "S6": 6.6e3, "S7a": 14.0e3, "S7r": 8.6e3}
 KERNEL_STEPS = {"k_radial": ("S3",), "k_angular_nn": ("S4", "S6", "S7a"), "k_force": ("S7r",)}
 FLOP_PER_ATOM = {k: sum(STEP_FLOP[s] for s in v) for k, v in KERNEL_STEPS.items()}
+# The same count for the paper-sized model (workload "paper": n_max 15/10, 100 neurons, no 4-body; DESIGN.md
+# section 10): S3 58 x 51 + 240 + 16*9*2; S4 14 x (91 + 11*9*2 + 11*24*2) + 0.8k; S6 100 x (60*4 + 11);
+# S7a 14 x (324 + 11*17*2 + 2*11*24*2) + 0.5k; S7r 58 x 142 + 16*9*2 + 0.2k
+PAPER_STEP_FLOP = {"S3": 3.5e3, "S4": 12.2e3, "S6": 25.1e3, "S7a": 25.1e3, "S7r": 8.7e3}
+PAPER_FLOP_PER_ATOM = {k: sum(PAPER_STEP_FLOP[s] for s in v) for k, v in KERNEL_STEPS.items()}
+MODEL_DESC = {
+    "paper": "NEP-ZBL at the paper's sizes: n_max 15/10, basis 8/8, l_max 4, 100 neurons, rc 6/4 A, ZBL Eq. 3 refit 1-2 A "
+             "(seeded random weights; a = 3.185 A)",
+}
+DEFAULT_MODEL_DESC = "NEP-ZBL n_max 4/4, basis 8/8, l_max 4 + 4-body, 50 neurons, rc 6/4 A, universal ZBL 1-2 A"
 # Compulsory HBM bytes per atom-step of each kernel group (same table)
 BYTES_PER_ATOM = {"integrate_a": 152.0, "kick_b": 64.0, "k_radial": 392.0, "k_angular_nn": 612.0,
                   "k_force": 1136.0}
@@ -78,6 +88,8 @@ def make_workload(name: str, seed_offset: int = 0, cells=None):
         return wl.config4(seed=4 + seed_offset, cells=cells or 160)
     if name == "config5":
         return wl.config5(seed=5 + seed_offset, cells=cells or (160, 160, 100))
+    if name == "paper":   # paper-sized model, a = 3.185 A, 0.01 A per step
+        return wl.paper_bulk(cells or 40, seed=12 + seed_offset)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -386,7 +398,8 @@ def run_b200(args):
         pass
     sm_max_mhz = float(peaks.get("sm_max_mhz", (clocks or {}).get("sm_max_mhz") or 1965.0))
     alu_peak = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12     # TFLOP/s
-    achieved = FLOP_PER_ATOM[dom] * n / (kern_ms[dom] * 1e-3) / 1e12
+    flop_table = PAPER_FLOP_PER_ATOM if args.workload == "paper" else FLOP_PER_ATOM
+    achieved = flop_table[dom] * n / (kern_ms[dom] * 1e-3) / 1e12
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": achieved / alu_peak,
@@ -395,7 +408,7 @@ def run_b200(args):
                 "traffic_source": NCU_TRAFFIC_SOURCE,
                 "peak_source": f"derived: {props.multi_processor_count} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max_mhz:.0f} MHz",
                 "ffma_measured_tflops": ffma_measured, "ms_per_launch": kern_ms[dom],
-                "flop_per_atom": FLOP_PER_ATOM[dom],
+                "flop_per_atom": flop_table[dom],
                 "hbm": {k: {"achieved_gbs": BYTES_PER_ATOM[k] * n / (kern_ms[k] * 1e-3) / 1e9,
                             "frac": BYTES_PER_ATOM[k] * n / (kern_ms[k] * 1e-3) / 1e9 / hbm_peak}
                         for k in BYTES_PER_ATOM if k in kern_ms},
@@ -411,7 +424,7 @@ def run_b200(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "atoms_per_gpu": n, "dt_max_fs": dt_max,
                    "max_displacement_A": (None if not np.isfinite(max_disp) else max_disp), "skin_A": w.model["skin"],
-                   "model": "NEP-ZBL n_max 4/4, basis 8/8, l_max 4 + 4-body, 50 neurons, rc 6/4 A, universal ZBL 1-2 A",
+                   "model": MODEL_DESC.get(args.workload, DEFAULT_MODEL_DESC),
                    "precision": "fp32 descriptors/network/forces, fp64 positions/velocities/ZBL/energy sums",
                    "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                    "l2": f"no flush for `value` (consecutive steps of one trajectory; workspace {g.workspace_bytes / 2**20:.0f} MiB "

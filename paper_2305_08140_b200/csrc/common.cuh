@@ -37,7 +37,7 @@ struct Scalars {  // device-resident control block (one per handle)
   int parity;                           // which vmax2 slot holds max |v|^2 of the current state
   int trace_pos;                        // next slot of the dt trace ring
   unsigned long long bmin[3], bmax[3];  // order-preserving encodings of min/max coordinate (open axes)
-  int overflow_radial, overflow_angular;  // largest neighbour counts seen at the last build
+  int overflow_radial, overflow_angular;  // largest neighbour counts seen since the host last cleared them
   int nonfinite;
   int box_too_small;
   int zbl_count;

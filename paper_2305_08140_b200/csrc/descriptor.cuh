@@ -310,7 +310,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
     }
     bit += RADIAL_UNROLL;
     if (bit == 32) {
-      rmask[((size_t)word * RADIAL_LANES + sub) * npad + sc_] = mword;
+      if (valid) rmask[((size_t)word * RADIAL_LANES + sub) * npad + sc_] = mword;
       mword = 0u;
       bit = 0;
       ++word;

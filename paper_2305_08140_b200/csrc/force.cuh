@@ -171,8 +171,12 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       int j0 = nl_a[e0], j1 = nl_a[e1];
       int b0 = rev[e0], b1 = rev[e1];
       float4 pij0 = pforce[e0], pij1 = pforce[e1];
-      float4 pji0 = pforce[(size_t)b0 * npad + j0], pji1 = pforce[(size_t)b1 * npad + j1];
-      if (!ok1) pij1 = pji1 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+      // rev == 255: j's list does not hold i -- only after a neighbour-capacity overflow (j's list was dropped and
+      // the call reports NEPZBL_E_NEIGHBOR_OVERFLOW); the value must never be used as a row index
+      const float4 zero4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+      float4 pji0 = b0 != 255 ? pforce[(size_t)b0 * npad + j0] : zero4;
+      float4 pji1 = b1 != 255 ? pforce[(size_t)b1 * npad + j1] : zero4;
+      if (!ok1) pij1 = pji1 = zero4;
       fx += pij0.x - pji0.x;
       fy += pij0.y - pji0.y;
       fz += pij0.z - pji0.z;

@@ -47,8 +47,9 @@ __global__ void k_rebuild_begin(Scalars* sc) {
     sc->bmin[a] = ~0ull;
     sc->bmax[a] = 0ull;
   }
-  sc->overflow_radial = 0;
-  sc->overflow_angular = 0;
+  // overflow_radial / overflow_angular are NOT reset here: they stay set until the host has reported them
+  // (check_device_flags -> k_clear_errors), so an overflow in the middle of an md_run chunk is not lost when
+  // a later rebuild of the same chunk happens to fit
   sc->maxdisp2_bits = 0u;
 }
 

@@ -133,3 +133,25 @@ def test_state_errors(nb):
     with pytest.raises(nb.NepZblError) as ei:
         g.md_step(1.0, 0.015)
     assert ei.value.code == -9
+
+
+def test_overflow_inside_a_long_md_run_is_reported_not_fatal(nb):
+    # a list-capacity overflow in the middle of an md_run chunk: the remaining steps of the chunk must stay
+    # memory-safe (the reverse index of a dropped list is a sentinel, not a row) and the call must report it
+    w = wl.bulk_cascade(8, 500.0, seed=11, n_steps=0, name="overflow")
+    w.model = dict(w.model, cap_angular=26)        # the ideal bcc count with the 1 A skin: md_init fits exactly,
+                                                   # a rebuild with the 500 eV recoil between lattice sites does not
+    g = nb.NepZbl(w.model, w.n)
+    pos = torch.from_numpy(w.pos.copy()).cuda(); vel = torch.from_numpy(w.vel.copy()).cuda()
+    g.md_init(pos, vel, torch.from_numpy(w.types).cuda(), w.box, w.pbc)   # fits: no error here
+    try:
+        g.md_run(3000, 1.0, 0.015)
+        raised = None
+    except nb.NepZblError as ex:
+        raised = ex
+    assert raised is not None and raised.code == -4
+    torch.cuda.synchronize()                       # no sticky CUDA error
+    w2 = wl.thermal_bulk(6, seed=11, sigma_pos=0.03)
+    g2 = nb.NepZbl(w2.model, w2.n)
+    e, f, v = g2.compute(w2.pos, w2.types, w2.box, w2.pbc)
+    assert np.isfinite(e).all()
