@@ -233,6 +233,7 @@ struct ZblParams {
   double c[4], d[4];
   double a_num, a_pow, coulomb_k;
   double Z[8];
+  double Zpow[8];   // Z^a_pow (Eq. 4), evaluated once on the host
   float filter_r2;  // fixed-point prefilter radius^2
 };
 
@@ -266,7 +267,7 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
       double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
       if (!(r < zp.r_outer)) continue;
       double Zi = zp.Z[me.w], Zj = zp.Z[o.w];
-      double a0 = zp.a_num / (pow(Zi, zp.a_pow) + pow(Zj, zp.a_pow));  // Eq. 4
+      double a0 = zp.a_num / (zp.Zpow[me.w] + zp.Zpow[o.w]);  // Eq. 4
       double x = r / a0, phi = 0.0, dphi = 0.0;
       for (int q = 0; q < zp.n_terms; ++q) {  // Eq. 3
         double ex = zp.c[q] * exp(-zp.d[q] * x);

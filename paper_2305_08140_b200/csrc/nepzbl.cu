@@ -270,6 +270,9 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
 }
 
 inline int blocks(long long n, int b) { return (int)((n + b - 1) / b); }
+// k_zbl walks the flagged atoms grid-stride: a handful in a thermal crystal (the graph skips the node when
+// there is none), thousands in a cascade core, so the grid covers the device
+inline int zbl_grid(const nepzbl_handle* h) { return std::max(1, std::min(blocks(h->n, 64), 8 * h->n_sm)); }
 
 enum { PK_INTEGRATE_A = 0, PK_REBUILD, PK_RADIAL, PK_ANGULAR_NN, PK_FORCE, PK_ZBL, PK_KICK, PK_COUNT };
 
@@ -376,7 +379,7 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   h->launches += 3;
   if (h->p.zbl_enabled && with_zbl) {
     prof_mark(h, PK_ZBL);
-    k_zbl<<<32, 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), n, npad, h->at<int4>(c.xyzt),
+    k_zbl<<<zbl_grid(h), 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), n, npad, h->at<int4>(c.xyzt),
                             h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp,
                             energy, force, virial);
     h->launches++;
@@ -391,7 +394,7 @@ void enqueue_eval(nepzbl_handle* h, const double* pos, double* energy, float* fo
 
 void enqueue_zbl(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial, cudaStream_t st) {
   const Carve& c = h->cv;
-  k_zbl<<<32, 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), (int)h->n, c.npad, h->at<int4>(c.xyzt),
+  k_zbl<<<zbl_grid(h), 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), (int)h->n, c.npad, h->at<int4>(c.xyzt),
                           h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp, energy, force, virial);
 }
 
@@ -563,7 +566,10 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   z.r_inner = p->zbl_r_inner; z.r_outer = p->zbl_r_outer; z.n_terms = p->zbl_n_terms;
   for (int k = 0; k < 4; ++k) { z.c[k] = p->zbl_c[k]; z.d[k] = p->zbl_d[k]; }
   z.a_num = p->zbl_a_num; z.a_pow = p->zbl_a_pow; z.coulomb_k = p->coulomb_k;
-  for (int t = 0; t < p->n_types && t < 8; ++t) z.Z[t] = p->atomic_number[t];
+  for (int t = 0; t < p->n_types && t < 8; ++t) {
+    z.Z[t] = p->atomic_number[t];
+    z.Zpow[t] = pow(p->atomic_number[t], p->zbl_a_pow);
+  }
   double zf = p->zbl_r_outer + 0.01;
   z.filter_r2 = (float)(zf * zf);
 

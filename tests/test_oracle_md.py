@@ -81,3 +81,20 @@ def test_pka_speed_values():
     # 10 keV -> 1.02453 A/fs, 100 keV -> 3.23986 A/fs for W
     assert wl.pka_speed(1.0e4, wl.W_MASS) == pytest.approx(1.02453, rel=1e-5)
     assert wl.pka_speed(1.0e5, wl.W_MASS) == pytest.approx(3.23986, rel=1e-5)
+
+
+def test_paper_sized_model_keeps_the_crystal():
+    # SURVEY 8(f) NEXT-2 input recipe: the seeded paper-sized potential (workloads.paper_model) must hold bcc W
+    # at 300 K, otherwise the "paper" workload would not have the paper's neighbour structure (58 / 14)
+    w = wl.paper_bulk(4, seed=12)
+    P = oracle.Params(w.model)
+    assert P.D == 60 and w.model["n_neurons"] == 100
+    pos, vel, dt, ep, ek = oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, 300, 1.0, 0.01)
+    L = w.box[[0, 4, 8]][:, None]
+    d = pos - w.pos
+    d -= L * np.round(d / L)
+    e = ep + ek
+    assert np.abs(d).max() < 0.5 and np.abs(e - e[0]).max() / w.n < 2e-4
+    nn, _ = oracle.neighbors(pos, w.box, w.pbc, 6.0)
+    na, _ = oracle.neighbors(pos, w.box, w.pbc, 4.0)
+    assert np.all(nn == 58) and np.all(na == 14)
