@@ -23,6 +23,13 @@ __host__ __device__ constexpr int split_smem_floats(int nrow) {
   return nrow * MS::DPAD + 2 * nrow + MS::DPAD + ((MS::NA + 3) / 4 * 4) * MS::KA;
 }
 
+// A[NSUB][24] is parked in shared memory while the network runs (q[D] + Fp[D] need its registers; without
+// this ptxas spilled ~100 registers to local memory): [NSUB * 24][SPLIT_THREADS] floats behind the table
+template <class MS>
+__host__ __device__ constexpr int split_stash_floats() {
+  return (MS::NA + SPLIT_LANES - 1) / SPLIT_LANES * 24 * SPLIT_THREADS;
+}
+
 template <class MS>
 __global__ void __launch_bounds__(SPLIT_THREADS)
 k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
@@ -40,6 +47,7 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
   float* s_w1 = s_b0 + nrow;         // [nrow]
   float* s_qs = s_w1 + nrow;         // [DPAD]
   float* s_ct = s_qs + DPAD;         // [NAP][KA], rows >= NA zero
+  float* s_stash = smem + split_smem_floats<MS>(nrow) + threadIdx.x;  // this thread's column of the A stash
   {  // the host lays the table out in exactly this order (build_nnw_split); its size is a multiple of 4 floats
     const int n4 = split_smem_floats<MS>(nrow) / 4;
     const float4* src = reinterpret_cast<const float4*>(nnw);
@@ -141,6 +149,13 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       for (int v = 0; v < D; ++v) q_out[(size_t)v * npad + s] = q[v];
     }
 
+    // park A in shared memory until the network is done
+#pragma unroll
+    for (int j = 0; j < NSUB; ++j)
+#pragma unroll
+      for (int lm = 0; lm < 24; ++lm) s_stash[(j * 24 + lm) * SPLIT_THREADS] = A[j][lm];
+    asm volatile("" ::: "memory");
+
     // ---- S6: lane p evaluates the neurons m = p, p+4, ... (two per iteration); partial U and dU/dq
     float Fp[D];
 #pragma unroll
@@ -215,6 +230,12 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
         if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
       }
     }
+
+    asm volatile("" ::: "memory");
+#pragma unroll
+    for (int j = 0; j < NSUB; ++j)
+#pragma unroll
+      for (int lm = 0; lm < 24; ++lm) A[j][lm] = s_stash[(j * 24 + lm) * SPLIT_THREADS];
 
     // ---- E[j][lm] = dU/dA[n_j][lm] (in place): pick this lane's channels out of Fp with compile-time indices
 #pragma unroll

@@ -234,7 +234,7 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
   if (kSplit<MS>) {
-    h->smem_nn = sizeof(float) * (size_t)split_smem_floats<MS>(nn_rows_split(p->n_neurons));
+    h->smem_nn = sizeof(float) * ((size_t)split_smem_floats<MS>(nn_rows_split(p->n_neurons)) + split_stash_floats<MS>());
   } else {
     const size_t nrow = (size_t)nn_rows(p->n_neurons);
     h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
