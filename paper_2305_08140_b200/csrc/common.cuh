@@ -43,6 +43,7 @@ struct Scalars {  // device-resident control block (one per handle)
   int zbl_count;
   int n_rebuilds;
   long long n_steps;
+  unsigned int blocks_done;             // ticket counter of k_kick_drift's last-block book-keeping
 };
 
 struct BoxHost {  // passed by value to k_boxmap

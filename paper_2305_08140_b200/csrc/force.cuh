@@ -17,6 +17,19 @@
 // next radial entry inside the cutoff before the convergent body); F and W are combined over the 4
 // lanes by a fixed-order shuffle tree, so the result is still bit-reproducible.
 #define FORCE_LANES 4
+// MD steps fuse the second half-kick of velocity-Verlet (S8b) into this kernel's epilogue (KickArgs::vel != NULL):
+// v += dt/2 F/m and max |v|^2 for the next step's dt, as k_kick does.  Atoms with a neighbour inside the ZBL
+// range are left to k_zbl, which adds the pair force first and then kicks them itself (their force is not final
+// here); the test is k_radial's, on the same bits.  In a captured graph thread 0 also opens / closes the IF
+// node of k_zbl (zbl_count is final once k_radial has run).
+struct KickArgs {
+  Scalars* sc;
+  double* vel;               // NULL: no kick (plain evaluation)
+  const double* inv_mass;
+  int do_vmax;               // 0 when a thermostat rescales the velocities afterwards (k_scale_vmax)
+  unsigned long long cond_zbl;
+  int use_cond;
+};
 template <class MS, bool VIRIAL>
 __global__ void __launch_bounds__(128)
 k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
@@ -25,8 +38,13 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
         const __grid_constant__ ModelTables<MS> mt, const AtomRec* __restrict__ rec,
         const unsigned* __restrict__ rmask, int mask_words, const unsigned long long* __restrict__ amask, const float4* __restrict__ pforce, const float* __restrict__ u_site,
         const int* __restrict__ perm, double* __restrict__ energy, float* __restrict__ force,
-        float* __restrict__ virial) {
+        float* __restrict__ virial, const KickArgs ka) {
   constexpr int KR = MS::KR;
+#if defined(__CUDA_ARCH__)
+  if (ka.use_cond && blockIdx.x == 0 && threadIdx.x == 0)
+    cudaGraphSetConditional((cudaGraphConditionalHandle)ka.cond_zbl, ka.sc->zbl_count > 0 ? 1u : 0u);
+#endif
+  bool close = false;
   static_assert(KR <= 12, "AtomRec holds 12 coefficients");
   const int gt = blockIdx.x * blockDim.x + threadIdx.x;
   const int s = gt / FORCE_LANES, sub = gt % FORCE_LANES;
@@ -83,6 +101,7 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       const Rec& o = o_cur;
       float dx = (float)(o.ux - me.ux) * hx, dy = (float)(o.uy - me.uy) * hy, dz = (float)(o.uz - me.uz) * hz;
       float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
+      close = close || (r2 < mt.zbl_flag_r2);
       float rinv = rsqrtf(r2), r = r2 * rinv;
       float fc, dfc, x, dxdr, T[KR], Uc[KR];
       cheb_T<KR>(r, mt.inv_rcR, fc, dfc, x, dxdr, T);
@@ -212,8 +231,34 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       w[c] += __shfl_xor_sync(0xffffffffu, w[c], 2);
     }
   }
+  const unsigned cb = __ballot_sync(0xffffffffu, close);
+  const int i = valid ? perm[s] : 0;
+  if (ka.vel) {  // S8b (uniform branch): lane a < 3 of the quad kicks component a; |v|^2 = (vx^2 + vy^2) + vz^2
+    const bool mine = valid && !((cb >> (threadIdx.x & 28)) & 0xFu);
+    double v = 0.0;
+    if (mine && sub < 3) {
+      const double dt = ka.sc->dt;
+      const double im = ka.inv_mass[xyzt[s].w];
+      const float fa = sub == 0 ? fx : (sub == 1 ? fy : fz);
+      const size_t k = (size_t)sub * n + i;
+      v = ka.vel[k] + 0.5 * dt * ((double)fa * im);
+      ka.vel[k] = v;
+    }
+    double v2 = v * v;
+    const double vy2 = __shfl_down_sync(0xffffffffu, v2, 1), vz2 = __shfl_down_sync(0xffffffffu, v2, 2);
+    v2 = (v2 + vy2) + vz2;  // meaningful on lane 0 of each quad
+    unsigned long long b = (ka.do_vmax && mine && sub == 0) ? (unsigned long long)__double_as_longlong(v2) : 0ull;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      unsigned long long t = __shfl_xor_sync(0xffffffffu, b, o);
+      b = t > b ? t : b;
+    }
+    if ((threadIdx.x & 31) == 0 && b) {
+      unsigned long long* slot = &ka.sc->vmax2_bits[ka.sc->parity];
+      if (b > *(volatile unsigned long long*)slot) atomicMax(slot, b);
+    }
+  }
   if (!valid) return;
-  int i = perm[s];
   if (sub == 0 && energy) energy[i] = (double)u_site[s];
   if (force) {
     if (sub == 0) force[i] = fx;
@@ -244,7 +289,7 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
       int npad, const int4* __restrict__ xyzt, const int* __restrict__ nn_r,
       const int* __restrict__ nl_r, const int* __restrict__ perm, const double* __restrict__ pos,
       const ZblParams zp, double* __restrict__ energy, float* __restrict__ force,
-      float* __restrict__ virial) {
+      float* __restrict__ virial, const KickArgs ka) {
   const int total = sc->zbl_count;
   for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += gridDim.x * blockDim.x) {
     int s = zbl_list[t];
@@ -296,8 +341,19 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
       }
     }
     if (energy) energy[i] += e;
+    double v2 = 0.0;
     if (force)
-      for (int a = 0; a < 3; ++a) force[(size_t)a * n + i] = (float)((double)force[(size_t)a * n + i] + f[a]);
+      for (int a = 0; a < 3; ++a) {
+        const float ft = (float)((double)force[(size_t)a * n + i] + f[a]);
+        force[(size_t)a * n + i] = ft;
+        if (ka.vel) {  // S8b for the atoms k_force left out (their force is final only now)
+          double v = ka.vel[(size_t)a * n + i] + 0.5 * ka.sc->dt * ((double)ft * ka.inv_mass[me.w]);
+          ka.vel[(size_t)a * n + i] = v;
+          v2 += v * v;
+        }
+      }
+    if (ka.vel && ka.do_vmax && v2 > 0.0)
+      atomicMax(&ka.sc->vmax2_bits[ka.sc->parity], (unsigned long long)__double_as_longlong(v2));
     if (virial)
       for (int c = 0; c < 9; ++c) virial[(size_t)c * n + i] = (float)((double)virial[(size_t)c * n + i] + w[c]);
   }

@@ -25,10 +25,10 @@ __device__ __forceinline__ double step_dt(const Scalars* sc) {
   return dt;
 }
 
-// one thread, after k_kick_drift: book-keeping of the step (dt for the second half-kick and the trace,
+// run by the last block of k_kick_drift: book-keeping of the step (dt for the second half-kick and the trace,
 // flip the vmax slot) and the rebuild decision; in a captured graph it also sets the IF nodes
-__global__ void k_step_flag(Scalars* sc, float half_skin2, double* dt_trace, int trace_ring,
-                            unsigned long long cond_rebuild, int use_cond) {
+__device__ __forceinline__ void step_flag(Scalars* sc, float half_skin2, double* dt_trace, int trace_ring,
+                                          unsigned long long cond_rebuild, int use_cond) {
   double dt = step_dt(sc);
   sc->dt = dt;
   int p = sc->parity;
@@ -47,11 +47,14 @@ __global__ void k_step_flag(Scalars* sc, float half_skin2, double* dt_trace, int
   if (use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)cond_rebuild, (unsigned)r);
 #endif
 }
+struct StepFlagArgs {  // passed by value to k_kick_drift, whose last block runs step_flag
+  float half_skin2;
+  double* dt_trace;
+  int trace_ring;
+  unsigned long long cond_rebuild;
+  int use_cond;
+};
 
-// one thread, after k_force: run the ZBL node of the captured graph only if an atom was flagged
-__global__ void k_zbl_gate(const Scalars* sc, unsigned long long cond_zbl) {
-  cudaGraphSetConditional((cudaGraphConditionalHandle)cond_zbl, sc->zbl_count > 0 ? 1u : 0u);
-}
 
 // ------------------------------------------------------------------ Nose-Hoover chain
 // "Atoms within a thickness of 3 a0 of the boundaries ... are maintained at 300 K using the Nose-Hoover
@@ -103,7 +106,7 @@ k_group_ke2_partial(int n, const double* __restrict__ vel, const int32_t* __rest
 }
 
 // one block: fixed-order sum of the partials, then thread 0 advances the chain by delta = dt/2.
-// phase 0 (before the first half-kick): dt of THIS step = step_dt(sc) (k_step_flag has not run yet);
+// phase 0 (before the first half-kick): dt of THIS step = step_dt(sc) (the step's book-keeping has not run yet);
 // phase 1 (after the second half-kick): dt = sc->dt.  count != NULL: only set n_group / nf (setup).
 __global__ void __launch_bounds__(256)
 k_nhc(const Scalars* sc, NhcState* nh, int nblocks, const double* __restrict__ partial,
@@ -188,7 +191,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
              const int32_t* __restrict__ types, const double* __restrict__ inv_mass,
              const int* __restrict__ inv_perm, int4* __restrict__ xyzt,
              const int4* __restrict__ xyzt_build, const unsigned char* __restrict__ group,
-             const NhcState* __restrict__ nh) {
+             const NhcState* __restrict__ nh, const StepFlagArgs fa) {
   __shared__ float sh[32];
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   float d2 = 0.0f;
@@ -220,7 +223,17 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
     d2 = dx * dx + dy * dy + dz * dz;
   }
   float m = block_max_128(d2, sh);
-  if (threadIdx.x == 0 && m > 0.0f) atomicMax(&sc->maxdisp2_bits, __float_as_uint(m));
+  if (threadIdx.x == 0) {
+    if (m > 0.0f) atomicMax(&sc->maxdisp2_bits, __float_as_uint(m));
+    // the block that finishes last does the step's book-keeping (formerly a one-thread kernel of its own):
+    // every other block has read dt / parity and published its displacement maximum before its ticket
+    __threadfence();
+    if (atomicAdd(&sc->blocks_done, 1u) == gridDim.x - 1) {
+      __threadfence();
+      sc->blocks_done = 0u;
+      step_flag(sc, fa.half_skin2, fa.dt_trace, fa.trace_ring, fa.cond_rebuild, fa.use_cond);
+    }
+  }
 }
 
 // second half-kick; leaves max |v|^2 for the next step's dt (integer atomicMax on the bits of a

@@ -99,7 +99,7 @@ struct nepzbl_handle {
   } ws_ref;
 
   // one MD step captured as a CUDA graph: the list-rebuild chain and the ZBL kernel sit in IF nodes
-  // whose conditions are set on the device (k_step_flag / k_zbl_gate), so a step is ONE launch
+  // whose conditions are set on the device (last block of k_kick_drift / k_force), so a step is ONE launch
   cudaGraph_t step_graph = nullptr;
   cudaGraphExec_t step_exec = nullptr;
   cudaStream_t cap_stream = nullptr;
@@ -343,7 +343,7 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
 // S3-S7 (+S5): outputs in the caller's order; any of energy/force/virial may be null.
 template <class MS>
 void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
-                    bool want_q, bool with_zbl) {
+                    bool want_q, bool with_zbl, const KickArgs& ka) {
   const Carve& c = h->cv;
   const int n = (int)h->n, npad = c.npad;
   cudaStream_t st = h->stream;
@@ -370,32 +370,33 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
     k_force<MS, true><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
         h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
-        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial);
+        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial, ka);
   else
     k_force<MS, false><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
         h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
-        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr);
+        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr, ka);
   h->launches += 3;
   if (h->p.zbl_enabled && with_zbl) {
     prof_mark(h, PK_ZBL);
     k_zbl<<<zbl_grid(h), 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), n, npad, h->at<int4>(c.xyzt),
                             h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp,
-                            energy, force, virial);
+                            energy, force, virial, ka);
     h->launches++;
   }
   prof_mark(h, -1);
 }
 
 void enqueue_eval(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
-                  bool want_q, bool with_zbl = true) {
-  with_shape(h->shape, [&](auto ms) { enqueue_eval_t<decltype(ms)>(h, pos, energy, force, virial, want_q, with_zbl); });
+                  bool want_q, bool with_zbl = true, const KickArgs& ka = KickArgs{}) {
+  with_shape(h->shape, [&](auto ms) { enqueue_eval_t<decltype(ms)>(h, pos, energy, force, virial, want_q, with_zbl, ka); });
 }
 
-void enqueue_zbl(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial, cudaStream_t st) {
+void enqueue_zbl(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial, cudaStream_t st,
+                 const KickArgs& ka) {
   const Carve& c = h->cv;
   k_zbl<<<zbl_grid(h), 64, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.zbl_list), (int)h->n, c.npad, h->at<int4>(c.xyzt),
-                          h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp, energy, force, virial);
+                          h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.perm), pos, h->zp, energy, force, virial, ka);
 }
 
 int read_scalars(nepzbl_handle* h) {
@@ -804,16 +805,16 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
                                               h->at<float>(c.md_force), h->md_types, h->d_inv_mass,
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
-                                              h->d_nhc);
-  k_step_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0);
-  h->launches += 2;
+                                              h->d_nhc,
+                                              StepFlagArgs{hs * hs, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0});
+  h->launches += 1;
   prof_mark(h, PK_REBUILD);
   h->launches += enqueue_rebuild(h, h->md_pos, h->md_types, st);
-  enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false);
+  // S8b (second half-kick, max |v|^2) runs in the epilogue of k_force / in k_zbl
+  enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false, true,
+               KickArgs{h->d_sc, h->md_vel, h->d_inv_mass, h->nhc_on ? 0 : 1, 0ull, 0});
   prof_mark(h, PK_KICK);
-  k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->md_vel, h->at<float>(c.md_force), h->md_types,
-                                        h->d_inv_mass, 1, h->nhc_on ? 0 : 1);
-  h->launches += 1 + enqueue_nhc(h, 1, st);
+  h->launches += enqueue_nhc(h, 1, st);
   prof_mark(h, -1);
 }
 
@@ -825,8 +826,9 @@ static void destroy_step_graph(nepzbl_handle* h) {
 }
 
 // Capture one MD step into a CUDA graph:
-//   k_kick_drift -> k_step_flag -> IF(rebuild){S2 chain} -> k_radial -> k_angular_nn -> k_force
-//   -> k_zbl_gate -> IF(zbl_count > 0){k_zbl} -> k_kick
+//   k_kick_drift (its last block: dt, rebuild decision) -> IF(rebuild){S2 chain} -> k_radial -> k_angular_nn
+//   -> k_force (+ second half-kick, opens the ZBL node) -> IF(zbl_count > 0){k_zbl (+ kick of its atoms)}
+//   5 kernels per step without rebuild / ZBL
 // Returns false (and leaves the stream path in use) if any capture call fails.
 static bool build_step_graph(nepzbl_handle* h) {
   destroy_step_graph(h);
@@ -867,9 +869,9 @@ static bool build_step_graph(nepzbl_handle* h) {
                                               h->at<float>(c.md_force), h->md_types, h->d_inv_mass,
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
-                                              h->d_nhc);
-  k_step_flag<<<1, 1, 0, st>>>(h->d_sc, hs * hs, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1);
-  nk += 2;
+                                              h->d_nhc,
+                                              StepFlagArgs{hs * hs, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1});
+  nk += 1;
   cudaGraph_t body = nullptr;
   ok = add_if(h_reb, &body);
   if (ok) {
@@ -880,23 +882,21 @@ static bool build_step_graph(nepzbl_handle* h) {
     }
   }
   if (ok) {
-    enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false, false);
+    const KickArgs ka{h->d_sc, h->md_vel, h->d_inv_mass, h->nhc_on ? 0 : 1, (unsigned long long)h_zbl,
+                      h->p.zbl_enabled ? 1 : 0};
+    enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false, false, ka);
     nk += 3;
     if (h->p.zbl_enabled) {
-      k_zbl_gate<<<1, 1, 0, st>>>(h->d_sc, (unsigned long long)h_zbl);
-      nk += 1;
       ok = add_if(h_zbl, &body);
       if (ok) {
         ok = cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
         if (ok) {
-          enqueue_zbl(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, h->cap_stream);
+          enqueue_zbl(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, h->cap_stream, ka);
           ok = cudaStreamEndCapture(h->cap_stream, nullptr) == cudaSuccess;
         }
       }
     }
-    k_kick<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->md_vel, h->at<float>(c.md_force), h->md_types,
-                                          h->d_inv_mass, 1, h->nhc_on ? 0 : 1);
-    nk += 1 + enqueue_nhc(h, 1, st);
+    nk += enqueue_nhc(h, 1, st);
   }
   cudaGraph_t captured = nullptr;
   cudaError_t ee = cudaStreamEndCapture(st, &captured);
