@@ -5,8 +5,9 @@
 //   * lane p of the quad owns the angular channels n = p, p+4, p+8 (< NA): A[3][24] = 72 accumulators; every
 //     lane walks all angular neighbours (the Chebyshev / harmonic evaluation is repeated per lane, the
 //     n-contractions -- the bulk of the work -- are split);
-//   * the network: lane p takes the neurons m = p, p+4, ...; the full descriptor is gathered with quad
-//     shuffles, the four partial dU/dq vectors are summed by a fixed-order xor butterfly (deterministic);
+//   * the network sees the descriptor in four SLICES, one per lane (SplitLayout): q and dU/dq never leave their
+//     lane; only the four pre-activations of a round (reduce-scatter butterfly, fixed order -> deterministic)
+//     and the four tanh derivatives cross the quad;
 //   * the back-pass is linear in G_lm = sum_n g_n E_nlm, so every lane contracts its own channels down to a
 //     partial force vector and only 3 numbers per neighbour cross the quad.
 // Weights and the folded angular coefficients sit in shared memory (lanes of a quad read different rows).
@@ -15,41 +16,69 @@
 
 #define SPLIT_LANES 4
 #define SPLIT_THREADS 128
-// rows of the staged weight table: n_neurons rounded up to a multiple of 8 (two neurons per lane per iteration)
-__host__ __device__ inline int nn_rows_split(int n_neurons) { return (n_neurons + 7) & ~7; }
-template <class MS>
-__host__ __device__ constexpr int split_smem_floats(int nrow) {
-  // w0 [nrow][DPAD], b0 [nrow], w1 [nrow], q_scaler [DPAD], ctA [NSUB*4][KA]
-  return nrow * MS::DPAD + 2 * nrow + MS::DPAD + ((MS::NA + 3) / 4 * 4) * MS::KA;
-}
 
-// A[NSUB][24] is parked in shared memory while the network runs (q[D] + Fp[D] need its registers; without
-// this ptxas spilled ~100 registers to local memory): [NSUB * 24][SPLIT_THREADS] floats behind the table
+// Who holds what.  Lane p of a quad owns the angular channels n = p + 4 j (j < NSUB) and the radial components
+// n = RSUB p + i (i < RSUB).  The network sees the descriptor as four SLICES, one per lane, so that neither q nor
+// dU/dq ever has to be gathered: slice entry idx of lane p is
+//   idx = 4 j + (l - 1)        -> q_{n_j, l}   (3-body, l = 1..4)
+//   idx = 4 NSUB + i           -> q_n radial, n = RSUB p + i
+//   idx = 4 NSUB + RSUB + j    -> q^222_{n_j}  (4-body, if the model has it)
+// and the host permutes the columns of w0 and q_scaler to match (entries beyond NA / NR are zero).
 template <class MS>
-__host__ __device__ constexpr int split_stash_floats() {
-  return (MS::NA + SPLIT_LANES - 1) / SPLIT_LANES * 24 * SPLIT_THREADS;
-}
+struct SplitLayout {
+  static constexpr int NSUB = (MS::NA + SPLIT_LANES - 1) / SPLIT_LANES;
+  static constexpr int RSUB = (MS::NR + SPLIT_LANES - 1) / SPLIT_LANES;
+  static constexpr int NAP = NSUB * SPLIT_LANES;
+  static constexpr int SL = 4 * NSUB + RSUB + (MS::B4 ? NSUB : 0);
+  static constexpr int SLP = (SL + 3) / 4 * 4;  // slice length, padded to float4
+  static constexpr int SLS = SLP + 4;           // slice stride: the four slices of a row fall into disjoint banks
+  // canonical descriptor index (SURVEY 8(c) C order) of slice entry idx of lane p, or -1
+  __host__ __device__ static constexpr int nu(int p, int idx) {
+    if (idx < 4 * NSUB) {
+      const int n = p + SPLIT_LANES * (idx / 4), l = idx % 4;
+      return n < MS::NA ? MS::NR + l * MS::NA + n : -1;
+    }
+    if (idx < 4 * NSUB + RSUB) {
+      const int n = RSUB * p + (idx - 4 * NSUB);
+      return n < MS::NR ? n : -1;
+    }
+    if (MS::B4 && idx < SL) {
+      const int n = p + SPLIT_LANES * (idx - 4 * NSUB - RSUB);
+      return n < MS::NA ? MS::NR + 4 * MS::NA + n : -1;
+    }
+    return -1;
+  }
+  // rows of the weight table: n_neurons rounded up to a multiple of 4 (one neuron per lane per round)
+  __host__ __device__ static constexpr int rows(int n_neurons) { return (n_neurons + 3) & ~3; }
+  // table (floats): w0 [nrow][4][SLS] | b0 [nrow] | w1 [nrow] | q_scaler [4][SLS] | ctA [NAP][KA] | ctR [4 RSUB][KR]
+  __host__ __device__ static constexpr int table_floats(int nrow) {
+    return nrow * 4 * SLS + 2 * nrow + 4 * SLS + NAP * MS::KA + 4 * RSUB * MS::KR;
+  }
+  // A[NSUB][24] is parked in shared memory while the network runs: [NSUB * 24][SPLIT_THREADS] floats
+  __host__ __device__ static constexpr int stash_floats() { return NSUB * 24 * SPLIT_THREADS; }
+};
 
 template <class MS>
-__global__ void __launch_bounds__(SPLIT_THREADS)
+__global__ void __launch_bounds__(SPLIT_THREADS, 3)
 k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
                    const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
                    const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,
                    const float* __restrict__ q_radial, float* __restrict__ u_site,
                    AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out) {
-  constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR, D = MS::D, DPAD = MS::DPAD;
-  constexpr int NSUB = (NA + SPLIT_LANES - 1) / SPLIT_LANES;  // channels per lane
-  constexpr int NAP = NSUB * SPLIT_LANES;
+  using LY = SplitLayout<MS>;
+  constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR;
+  constexpr int NSUB = LY::NSUB, RSUB = LY::RSUB, SLP = LY::SLP, SLS = LY::SLS, NAP = LY::NAP;
   extern __shared__ __align__(16) float smem[];
-  const int nrow = nn_rows_split(mt.n_neurons);
-  float* s_w0 = smem;                // [nrow][DPAD]
-  float* s_b0 = s_w0 + nrow * DPAD;  // [nrow]
-  float* s_w1 = s_b0 + nrow;         // [nrow]
-  float* s_qs = s_w1 + nrow;         // [DPAD]
-  float* s_ct = s_qs + DPAD;         // [NAP][KA], rows >= NA zero
-  float* s_stash = smem + split_smem_floats<MS>(nrow) + threadIdx.x;  // this thread's column of the A stash
-  {  // the host lays the table out in exactly this order (build_nnw_split); its size is a multiple of 4 floats
-    const int n4 = split_smem_floats<MS>(nrow) / 4;
+  const int nrow = LY::rows(mt.n_neurons);
+  float* s_w0 = smem;                     // [nrow][4][SLS]
+  float* s_b0 = s_w0 + nrow * 4 * SLS;    // [nrow]
+  float* s_w1 = s_b0 + nrow;              // [nrow]
+  float* s_qs = s_w1 + nrow;              // [4][SLS]
+  float* s_ct = s_qs + 4 * SLS;           // [NAP][KA], rows >= NA zero
+  float* s_ctr = s_ct + NAP * KA;         // [4 RSUB][KR], rows >= NR zero
+  float* s_stash = smem + LY::table_floats(nrow) + threadIdx.x;  // this thread's column of the A stash
+  {  // the host lays the table out in exactly this order (build_nnw); its size is a multiple of 4 floats
+    const int n4 = LY::table_floats(nrow) / 4;
     const float4* src = reinterpret_cast<const float4*>(nnw);
     float4* dst = reinterpret_cast<float4*>(smem);
     for (int t = threadIdx.x; t < n4; t += SPLIT_THREADS) dst[t] = src[t];
@@ -103,18 +132,19 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       }
     }
 
-    // ---- descriptor: this lane's angular components, then the full scaled vector via quad shuffles
-    float qmine[NSUB][4];
-    float dq4[MS::B4 ? NSUB : 1][5];
+    // ---- descriptor slice of this lane (SplitLayout): 3-body of its channels, its radial components, 4-body
+    float q[SLP];
+#pragma unroll
+    for (int i = 0; i < SLP; ++i) q[i] = 0.0f;
 #pragma unroll
     for (int j = 0; j < NSUB; ++j) {
       float ql[4] = {0.0f, 0.0f, 0.0f, 0.0f};
 #pragma unroll
       for (int lm = 0; lm < 24; ++lm) ql[lm_to_l(lm) - 1] = fmaf(kClm[lm] * A[j][lm], A[j][lm], ql[lm_to_l(lm) - 1]);
 #pragma unroll
-      for (int l = 0; l < 4; ++l) qmine[j][l] = ql[l];
+      for (int l = 0; l < 4; ++l) q[4 * j + l] = ql[l];
     }
-    float q4mine[MS::B4 ? NSUB : 1];
+    float dq4[MS::B4 ? NSUB : 1][5];
     if (MS::B4) {
 #pragma unroll
       for (int j = 0; j < NSUB; ++j) {
@@ -125,7 +155,7 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
         float cxy = Sxz * Syz - Sxy * Szz, cxz = Sxy * Syz - Syy * Sxz, cyz = Sxy * Sxz - Sxx * Syz;
         float det = Sxx * cxx + Sxy * cxy + Sxz * cxz;
         const float k3 = 3.0f * NEPZBL_C4;
-        q4mine[j] = k3 * det;
+        q[MS::B4 ? 4 * NSUB + RSUB + j : 0] = k3 * det;
         dq4[j][0] = k3 * ((czz * (1.0f / 3.0f)) - (cxx + cyy) * (1.0f / 6.0f));
         dq4[j][1] = k3 * 2.0f * cxz;
         dq4[j][2] = k3 * 2.0f * cyz;
@@ -133,20 +163,20 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
         dq4[j][4] = k3 * cxy;
       }
     }
-    float q[D];
 #pragma unroll
-    for (int nq = 0; nq < NR; ++nq) q[nq] = q_radial[(size_t)nq * npad + sc_];
-#pragma unroll
-    for (int nq = 0; nq < NA; ++nq) {  // channel nq lives in lane nq & 3, slot nq >> 2 (both compile-time)
-#pragma unroll
-      for (int l = 0; l < 4; ++l)
-        q[NR + l * NA + nq] = __shfl_sync(0xffffffffu, qmine[nq / SPLIT_LANES][l], qbase + (nq % SPLIT_LANES));
-      if (MS::B4)
-        q[NR + 4 * NA + nq] = __shfl_sync(0xffffffffu, q4mine[MS::B4 ? nq / SPLIT_LANES : 0], qbase + (nq % SPLIT_LANES));
+    for (int i = 0; i < RSUB; ++i) {
+      const int nq = RSUB * sub + i;
+      q[4 * NSUB + i] = nq < NR ? q_radial[(size_t)nq * npad + sc_] : 0.0f;
     }
-    if (q_out && valid && sub == 0) {
+    if (q_out && valid) {  // descriptor export (parity tests), canonical order
 #pragma unroll
-      for (int v = 0; v < D; ++v) q_out[(size_t)v * npad + s] = q[v];
+      for (int i = 0; i < LY::SL; ++i) {
+        int nu = -1;
+#pragma unroll
+        for (int p = 0; p < SPLIT_LANES; ++p)
+          if (sub == p) nu = LY::nu(p, i);
+        if (nu >= 0) q_out[(size_t)nu * npad + s] = q[i];
+      }
     }
 
     // park A in shared memory until the network is done
@@ -156,78 +186,99 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       for (int lm = 0; lm < 24; ++lm) s_stash[(j * 24 + lm) * SPLIT_THREADS] = A[j][lm];
     asm volatile("" ::: "memory");
 
-    // ---- S6: lane p evaluates the neurons m = p, p+4, ... (two per iteration); partial U and dU/dq
-    float Fp[D];
+    // ---- S6: four neurons per round.  Every lane forms the partial pre-activations of the four neurons over
+    //      ITS slice; a two-step butterfly (fixed order) leaves the complete sum of neuron m0 + p on lane p, which
+    //      takes the tanh; the four derivatives go round the quad and every lane accumulates dU/dq of its slice.
+    float Fp[SLP];
 #pragma unroll
-    for (int v = 0; v < D; ++v) {
-      q[v] *= s_qs[v];
-      Fp[v] = 0.0f;
+    for (int i = 0; i < SLP; ++i) {
+      q[i] *= s_qs[sub * SLS + i];
+      Fp[i] = 0.0f;
     }
     float U = 0.0f;
 #pragma unroll 1
-    for (int m = sub; m < nrow; m += 2 * SPLIT_LANES) {
-      const float4* wa = reinterpret_cast<const float4*>(s_w0 + m * DPAD);
-      const float4* wb = reinterpret_cast<const float4*>(s_w0 + (m + SPLIT_LANES) * DPAD);
-      float za0 = -s_b0[m], za1 = 0.0f, zb0 = -s_b0[m + SPLIT_LANES], zb1 = 0.0f;
+    for (int m0 = 0; m0 < nrow; m0 += SPLIT_LANES) {
+      float4 w[SPLIT_LANES][SLP / 4];
+      float z[SPLIT_LANES];
 #pragma unroll
-      for (int v4 = 0; v4 < DPAD / 4; ++v4) {
-        float4 w = wa[v4], x = wb[v4];
-        if (4 * v4 + 0 < D) { za0 = fmaf(w.x, q[4 * v4 + 0], za0); zb0 = fmaf(x.x, q[4 * v4 + 0], zb0); }
-        if (4 * v4 + 1 < D) { za1 = fmaf(w.y, q[4 * v4 + 1], za1); zb1 = fmaf(x.y, q[4 * v4 + 1], zb1); }
-        if (4 * v4 + 2 < D) { za0 = fmaf(w.z, q[4 * v4 + 2], za0); zb0 = fmaf(x.z, q[4 * v4 + 2], zb0); }
-        if (4 * v4 + 3 < D) { za1 = fmaf(w.w, q[4 * v4 + 3], za1); zb1 = fmaf(x.w, q[4 * v4 + 3], zb1); }
+      for (int p = 0; p < SPLIT_LANES; ++p) {
+        const float4* wp = reinterpret_cast<const float4*>(s_w0 + ((m0 + p) * SPLIT_LANES + sub) * SLS);
+        float z0 = 0.0f, z1 = 0.0f;
+#pragma unroll
+        for (int v4 = 0; v4 < SLP / 4; ++v4) {
+          w[p][v4] = wp[v4];
+          z0 = fmaf(w[p][v4].x, q[4 * v4 + 0], z0);
+          z1 = fmaf(w[p][v4].y, q[4 * v4 + 1], z1);
+          z0 = fmaf(w[p][v4].z, q[4 * v4 + 2], z0);
+          z1 = fmaf(w[p][v4].w, q[4 * v4 + 3], z1);
+        }
+        z[p] = z0 + z1;
       }
-      const float ha = tanh_fast(za0 + za1), hb = tanh_fast(zb0 + zb1);
-      const float w1a = s_w1[m], w1b = s_w1[m + SPLIT_LANES];  // zero in the padding rows
-      U = fmaf(w1a, ha, U);
-      U = fmaf(w1b, hb, U);
-      const float ta = w1a * fmaf(-ha, ha, 1.0f), tb = w1b * fmaf(-hb, hb, 1.0f);
+      const bool b0 = sub & 1, b1 = sub & 2;
+      float k01 = b0 ? z[1] : z[0], k23 = b0 ? z[3] : z[2];
+      k01 += __shfl_xor_sync(0xffffffffu, b0 ? z[0] : z[1], 1);
+      k23 += __shfl_xor_sync(0xffffffffu, b0 ? z[2] : z[3], 1);
+      float zm = b1 ? k23 : k01;
+      zm += __shfl_xor_sync(0xffffffffu, b1 ? k01 : k23, 2);
+      const float h = tanh_fast(zm - s_b0[m0 + sub]);
+      const float w1 = s_w1[m0 + sub];  // zero in the padding rows
+      U = fmaf(w1, h, U);
+      const float t = w1 * fmaf(-h, h, 1.0f);
 #pragma unroll
-      for (int v4 = 0; v4 < DPAD / 4; ++v4) {
-        float4 w = wa[v4], x = wb[v4];
-        if (4 * v4 + 0 < D) Fp[4 * v4 + 0] = fmaf(tb, x.x, fmaf(ta, w.x, Fp[4 * v4 + 0]));
-        if (4 * v4 + 1 < D) Fp[4 * v4 + 1] = fmaf(tb, x.y, fmaf(ta, w.y, Fp[4 * v4 + 1]));
-        if (4 * v4 + 2 < D) Fp[4 * v4 + 2] = fmaf(tb, x.z, fmaf(ta, w.z, Fp[4 * v4 + 2]));
-        if (4 * v4 + 3 < D) Fp[4 * v4 + 3] = fmaf(tb, x.w, fmaf(ta, w.w, Fp[4 * v4 + 3]));
+      for (int p = 0; p < SPLIT_LANES; ++p) {
+        const float tp = __shfl_sync(0xffffffffu, t, qbase + p);
+#pragma unroll
+        for (int v4 = 0; v4 < SLP / 4; ++v4) {
+          Fp[4 * v4 + 0] = fmaf(tp, w[p][v4].x, Fp[4 * v4 + 0]);
+          Fp[4 * v4 + 1] = fmaf(tp, w[p][v4].y, Fp[4 * v4 + 1]);
+          Fp[4 * v4 + 2] = fmaf(tp, w[p][v4].z, Fp[4 * v4 + 2]);
+          Fp[4 * v4 + 3] = fmaf(tp, w[p][v4].w, Fp[4 * v4 + 3]);
+        }
       }
     }
-    // quad all-reduce in a fixed order: (lane0 + lane1) + (lane2 + lane3) on every lane
+    // site energy: (lane0 + lane1) + (lane2 + lane3) on every lane
     U += __shfl_xor_sync(0xffffffffu, U, 1);
     U += __shfl_xor_sync(0xffffffffu, U, 2);
     U -= mt.b1;
 #pragma unroll
-    for (int v = 0; v < D; ++v) {
-      float f = Fp[v];
-      f += __shfl_xor_sync(0xffffffffu, f, 1);
-      f += __shfl_xor_sync(0xffffffffu, f, 2);
-      Fp[v] = f * s_qs[v];
-    }
+    for (int i = 0; i < SLP; ++i) Fp[i] *= s_qs[sub * SLS + i];
 
-    // ---- per-atom outputs (one lane of the quad): site energy and the record for k_force's radial pass
-    if (valid && sub == 0) {
-      u_site[s] = U;
-      const int4 me = xyzt[s];
-      if (MS::FPREC) {
-        float f[5];
+    // ---- per-atom outputs: site energy and the record for k_force's radial pass.  The radial dU/dq are spread
+    //      over the quad: every lane contracts its RSUB components, a fixed-order butterfly adds the four parts.
+    {
+      float d[12];
 #pragma unroll
-        for (int nq = 0; nq < 5; ++nq) f[nq] = nq < NR ? Fp[nq < NR ? nq : 0] : 0.0f;
-        float4* rp = reinterpret_cast<float4*>(reinterpret_cast<char*>(rec) + (size_t)s * 32);
-        rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), f[0]);
-        rp[1] = make_float4(f[1], f[2], f[3], f[4]);
+      for (int k = 0; k < 12; ++k) d[k] = 0.0f;
+      if (MS::FPREC) {  // record holds Fp[0..4] itself: component n sits on lane n / RSUB, entry n % RSUB
+#pragma unroll
+        for (int nq = 0; nq < 5; ++nq)
+          if (nq < NR) d[nq] = __shfl_sync(0xffffffffu, Fp[4 * NSUB + (nq < NR ? nq % RSUB : 0)], qbase + (nq < NR ? nq / RSUB : 0));
       } else {
         static_assert(KR <= 12, "AtomRec holds 12 coefficients");
-        float d[12];
 #pragma unroll
-        for (int k = 0; k < 12; ++k) d[k] = 0.0f;
+        for (int k = 0; k < KR; ++k) {
+          float t = 0.0f;
 #pragma unroll
-        for (int k = 0; k < KR; ++k)
-#pragma unroll
-          for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
-        float4* rp = reinterpret_cast<float4*>(rec + s);
-        rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
-        rp[1] = make_float4(d[1], d[2], d[3], d[4]);
-        rp[2] = make_float4(d[5], d[6], d[7], d[8]);
-        if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
+          for (int i = 0; i < RSUB; ++i) t = fmaf(Fp[4 * NSUB + i], s_ctr[(RSUB * sub + i) * KR + k], t);
+          t += __shfl_xor_sync(0xffffffffu, t, 1);
+          t += __shfl_xor_sync(0xffffffffu, t, 2);
+          d[k] = t;
+        }
+      }
+      if (valid && sub == 0) {
+        u_site[s] = U;
+        const int4 me = xyzt[s];
+        if (MS::FPREC) {
+          float4* rp = reinterpret_cast<float4*>(reinterpret_cast<char*>(rec) + (size_t)s * 32);
+          rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
+          rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+        } else {
+          float4* rp = reinterpret_cast<float4*>(rec + s);
+          rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
+          rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+          rp[2] = make_float4(d[5], d[6], d[7], d[8]);
+          if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
+        }
       }
     }
 
@@ -237,24 +288,15 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
 #pragma unroll
       for (int lm = 0; lm < 24; ++lm) A[j][lm] = s_stash[(j * 24 + lm) * SPLIT_THREADS];
 
-    // ---- E[j][lm] = dU/dA[n_j][lm] (in place): pick this lane's channels out of Fp with compile-time indices
+    // ---- E[j][lm] = dU/dA[n_j][lm] (in place): the slice holds exactly this lane's dU/dq
 #pragma unroll
     for (int j = 0; j < NSUB; ++j) {
-      float fl[4] = {0.0f, 0.0f, 0.0f, 0.0f}, f4 = 0.0f;
 #pragma unroll
-      for (int p = 0; p < SPLIT_LANES; ++p) {
-        const int nq = p + SPLIT_LANES * j;
-        if (nq < NA && sub == p) {
-#pragma unroll
-          for (int l = 0; l < 4; ++l) fl[l] = Fp[NR + l * NA + (nq < NA ? nq : 0)];
-          if (MS::B4) f4 = Fp[MS::B4 ? NR + 4 * NA + (nq < NA ? nq : 0) : 0];
-        }
-      }
-#pragma unroll
-      for (int lm = 0; lm < 24; ++lm) A[j][lm] *= 2.0f * kClm[lm] * fl[lm_to_l(lm) - 1];
+      for (int lm = 0; lm < 24; ++lm) A[j][lm] *= 2.0f * kClm[lm] * Fp[4 * j + lm_to_l(lm) - 1];
       if (MS::B4) {
 #pragma unroll
-        for (int m5 = 0; m5 < 5; ++m5) A[j][3 + m5] = fmaf(f4, dq4[MS::B4 ? j : 0][m5], A[j][3 + m5]);
+        for (int m5 = 0; m5 < 5; ++m5)
+          A[j][3 + m5] = fmaf(Fp[MS::B4 ? 4 * NSUB + RSUB + j : 0], dq4[MS::B4 ? j : 0][m5], A[j][3 + m5]);
       }
     }
 

@@ -234,39 +234,68 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
   if (kSplit<MS>) {
-    h->smem_nn = sizeof(float) * ((size_t)split_smem_floats<MS>(nn_rows_split(p->n_neurons)) + split_stash_floats<MS>());
+    using LY = SplitLayout<MS>;
+    h->smem_nn = sizeof(float) * ((size_t)LY::table_floats(LY::rows(p->n_neurons)) + LY::stash_floats());
   } else {
     const size_t nrow = (size_t)nn_rows(p->n_neurons);
     h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
   }
 }
 
+// folded Chebyshev coefficients (descriptor.cuh): ct_n0 = c_n0 + 1/2 sum_{k>=1} c_nk, ct_nk = c_nk / 2
+inline double folded(const double* c, int K, int n, int k) {
+  if (k > 0) return 0.5 * c[n * K + k];
+  double s = 0.0;
+  for (int j = 1; j < K; ++j) s += c[n * K + j];
+  return c[n * K] + 0.5 * s;
+}
+
 template <class MS>
 std::vector<float> build_nnw(const nepzbl_params* p) {
-  // zero padding rows, see nn_rows / nn_rows_split; the split kernel's table also carries the folded
-  // angular coefficients ct[NAP][KA] (rows >= NA zero) behind q_scaler
-  const int neu2 = kSplit<MS> ? nn_rows_split(p->n_neurons) : nn_rows(p->n_neurons);
-  std::vector<float> w(kSplit<MS> ? (size_t)split_smem_floats<MS>(neu2) : (size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD, 0.0f);
-  for (int m = 0; m < p->n_neurons; ++m)
-    for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
-  float* b0 = w.data() + (size_t)neu2 * MS::DPAD;
-  float* w1 = b0 + neu2;
-  float* qs = w1 + neu2;
-  for (int m = 0; m < p->n_neurons; ++m) {
-    b0[m] = (float)p->b0[m];
-    w1[m] = (float)p->w1[m];
-  }
-  for (int v = 0; v < MS::D; ++v) qs[v] = (float)p->q_scaler[v];
-  if (kSplit<MS>) {
-    float* ct = qs + MS::DPAD;
-    for (int nq = 0; nq < MS::NA; ++nq) {
-      double sum = 0.0;
-      for (int k = 1; k < MS::KA; ++k) sum += p->c_angular[nq * MS::KA + k];
-      for (int k = 0; k < MS::KA; ++k)
-        ct[nq * MS::KA + k] = (float)(k == 0 ? p->c_angular[nq * MS::KA] + 0.5 * sum : 0.5 * p->c_angular[nq * MS::KA + k]);
+  if constexpr (kSplit<MS>) {
+    // table of k_angular_nn_split, in the order SplitLayout::table_floats lists (weights and q_scaler permuted
+    // into the four lane slices; everything not written stays zero)
+    using LY = SplitLayout<MS>;
+    const int nrow = LY::rows(p->n_neurons);
+    std::vector<float> w((size_t)LY::table_floats(nrow), 0.0f);
+    float* w0 = w.data();
+    float* b0 = w0 + (size_t)nrow * 4 * LY::SLS;
+    float* w1 = b0 + nrow;
+    float* qs = w1 + nrow;
+    float* cta = qs + 4 * LY::SLS;
+    float* ctr = cta + LY::NAP * MS::KA;
+    for (int lane = 0; lane < 4; ++lane)
+      for (int idx = 0; idx < LY::SLP; ++idx) {
+        const int nu = LY::nu(lane, idx);
+        if (nu < 0) continue;
+        qs[lane * LY::SLS + idx] = (float)p->q_scaler[nu];
+        for (int m = 0; m < p->n_neurons; ++m)
+          w0[((size_t)m * 4 + lane) * LY::SLS + idx] = (float)p->w0[(size_t)m * MS::D + nu];
+      }
+    for (int m = 0; m < p->n_neurons; ++m) {
+      b0[m] = (float)p->b0[m];
+      w1[m] = (float)p->w1[m];
     }
+    for (int nq = 0; nq < MS::NA; ++nq)
+      for (int k = 0; k < MS::KA; ++k) cta[nq * MS::KA + k] = (float)folded(p->c_angular, MS::KA, nq, k);
+    for (int nq = 0; nq < MS::NR; ++nq)
+      for (int k = 0; k < MS::KR; ++k) ctr[nq * MS::KR + k] = (float)folded(p->c_radial, MS::KR, nq, k);
+    return w;
+  } else {
+    const int neu2 = nn_rows(p->n_neurons);  // zero padding rows, see nn_rows
+    std::vector<float> w((size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD, 0.0f);
+    for (int m = 0; m < p->n_neurons; ++m)
+      for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
+    float* b0 = w.data() + (size_t)neu2 * MS::DPAD;
+    float* w1 = b0 + neu2;
+    float* qs = w1 + neu2;
+    for (int m = 0; m < p->n_neurons; ++m) {
+      b0[m] = (float)p->b0[m];
+      w1[m] = (float)p->w1[m];
+    }
+    for (int v = 0; v < MS::D; ++v) qs[v] = (float)p->q_scaler[v];
+    return w;
   }
-  return w;
 }
 
 inline int blocks(long long n, int b) { return (int)((n + b - 1) / b); }
