@@ -61,17 +61,18 @@ MODEL_DESC = {
 }
 DEFAULT_MODEL_DESC = "NEP-ZBL n_max 4/4, basis 8/8, l_max 4 + 4-body, 50 neurons, rc 6/4 A, universal ZBL 1-2 A"
 # Compulsory HBM bytes per atom-step of each kernel group (same table)
-BYTES_PER_ATOM = {"integrate_a": 152.0, "kick_b": 64.0, "k_radial": 392.0, "k_angular_nn": 612.0,
-                  "k_force": 1136.0}
+# (k_force carries the second half-kick: + 48 B of fp64 velocities; the per-atom record is 32 B)
+BYTES_PER_ATOM = {"integrate_a": 152.0, "k_radial": 392.0, "k_angular_nn": 596.0, "k_force": 1168.0}
 FP32_LANES_PER_SM = 128
 # Wigner-Seitz count, compulsory HBM bytes per atom (one site per atom): position 24 + nearest 4 + occupancy
 # read-modify-write 8 + count read 4 + cell-sorted site record 28 (the 27-cell scan re-reads sites from L1/L2)
 WS_BYTES_PER_ATOM = 68.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on config2 (128 000 atoms) from the committed
 # `ncu --set full` capture (NCU_TRAFFIC_SOURCE); reported as roofline.traffic for that workload only.
-NCU_TRAFFIC_BYTES = {"k_radial": 48.145152e6 + 3.609856e6, "k_angular_nn": 50.303232e6 + 17.240832e6,
-                     "k_force": 90.675456e6 + 3.625728e6}
-NCU_TRAFFIC_SOURCE = "profiles/r1c_ncu_full.md"
+NCU_TRAFFIC_BYTES = {"config2": {"k_radial": 48.145408e6 + 3.536640e6, "k_angular_nn": 46.196992e6 + 13.029632e6,
+                                 "k_force": 91.716608e6 + 4.702976e6},
+                     "paper": {"k_angular_nn": 55.964928e6 + 18.282496e6}}
+NCU_TRAFFIC_SOURCE = "profiles/r1e_ncu_full.md"
 
 
 def _dist_env():
@@ -404,7 +405,7 @@ def run_b200(args):
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": achieved / alu_peak,
                 "traffic": args.traffic_bytes if args.traffic_bytes is not None else
-                (NCU_TRAFFIC_BYTES.get(dom) if (args.workload == "config2" and args.cells is None) else None),
+                (NCU_TRAFFIC_BYTES.get(args.workload, {}).get(dom) if args.cells is None else None),
                 "traffic_source": NCU_TRAFFIC_SOURCE,
                 "peak_source": f"derived: {props.multi_processor_count} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max_mhz:.0f} MHz",
                 "ffma_measured_tflops": ffma_measured, "ms_per_launch": kern_ms[dom],
