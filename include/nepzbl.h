@@ -150,8 +150,10 @@ int md_step(nepzbl_handle *h, double dt_max, double max_displacement, double *dt
             int32_t *rebuilt);
 int md_run(nepzbl_handle *h, int64_t n_steps, double dt_max, double max_displacement,
            double *dt_trace, int64_t *n_rebuilds);
-/* md_step with HOST state: copies pos/vel (host, 3n doubles each) to the registered device buffers,
- * steps, copies them back. */
+/* md_step with HOST state: copies pos/vel (host, 3n doubles each; pinned memory makes the copies
+ * asynchronous) to the registered device buffers, steps, copies them back.  The new positions are final
+ * after the drift, so their copy back runs on a second stream while the forces are evaluated; the call
+ * returns when both buffers are complete. */
 int md_step_host(nepzbl_handle *h, double *pos_soa, double *vel_soa, double dt_max,
                  double max_displacement, double *dt_used, int32_t *rebuilt);
 /* Total potential and kinetic energy of the current MD state (host scalars), fixed-order fp64

@@ -103,6 +103,10 @@ struct nepzbl_handle {
   cudaGraph_t step_graph = nullptr;
   cudaGraphExec_t step_exec = nullptr;
   cudaStream_t cap_stream = nullptr;
+  // md_step_host: the positions are final once k_kick_drift has run, so their device-to-host copy goes to a
+  // second stream behind this event and overlaps the force kernels
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_drift = nullptr;
   int graph_kernels = 0, graph_rebuild_kernels = 0;  // launch accounting per graph replay
   bool use_graph = true;
 
@@ -626,6 +630,8 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     if (per_sm < 1) return die("k_angular_nn does not fit one SM", cudaErrorInvalidConfiguration);
     h->ang_grid = per_sm * h->n_sm;
   }
+  if ((ce = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking)) != cudaSuccess) return die("cudaStreamCreate", ce);
+  if ((ce = cudaEventCreateWithFlags(&h->ev_drift, cudaEventDisableTiming)) != cudaSuccess) return die("cudaEventCreate", ce);
   if ((ce = cudaMalloc(&h->d_sc, sizeof(Scalars))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_bm, sizeof(BoxMap))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_nnw, nnw.size() * sizeof(float))) != cudaSuccess) return die("cudaMalloc", ce);
@@ -676,6 +682,8 @@ void nep_zbl_destroy(nepzbl_handle* h) {
   if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
   if (h->step_graph) cudaGraphDestroy(h->step_graph);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  if (h->ev_drift) cudaEventDestroy(h->ev_drift);
   delete h;
 }
 
@@ -836,6 +844,7 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
                                               h->d_nhc,
                                               StepFlagArgs{hs * hs, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0});
+  cudaEventRecord(h->ev_drift, st);
   h->launches += 1;
   prof_mark(h, PK_REBUILD);
   h->launches += enqueue_rebuild(h, h->md_pos, h->md_types, st);
@@ -900,9 +909,10 @@ static bool build_step_graph(nepzbl_handle* h) {
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
                                               h->d_nhc,
                                               StepFlagArgs{hs * hs, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1});
+  ok = ok && cudaEventRecordWithFlags(h->ev_drift, st, cudaEventRecordExternal) == cudaSuccess;
   nk += 1;
   cudaGraph_t body = nullptr;
-  ok = add_if(h_reb, &body);
+  ok = ok && add_if(h_reb, &body);
   if (ok) {
     ok = cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
     if (ok) {
@@ -960,15 +970,25 @@ static int enqueue_md_steps(nepzbl_handle* h, int n_steps, bool trace) {
   return NEPZBL_OK;
 }
 
-int md_step(nepzbl_handle* h, double dt_max, double max_displacement, double* dt_used, int32_t* rebuilt) {
-  if (!h) return NEPZBL_E_INVALID_ARG;
-  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_step before md_init");
+// one step; pos_host / vel_host (md_step_host): copy the new state out, the positions as soon as they are final
+static int md_step_impl(nepzbl_handle* h, double dt_max, double max_displacement, double* dt_used, int32_t* rebuilt,
+                        double* pos_host, double* vel_host) {
   if (!(dt_max > 0) || !(max_displacement > 0)) return fail(h, NEPZBL_E_INVALID_ARG, "dt_max and max_displacement must be > 0");
   k_md_params<<<1, 1, 0, h->stream>>>(h->d_sc, dt_max, max_displacement);
   h->launches++;
   int rc = enqueue_md_steps(h, 1, false);
   if (rc) return rc;
+  if (pos_host) {
+    const size_t b = 24 * (size_t)h->n;
+    CU(cudaStreamWaitEvent(h->copy_stream, h->ev_drift, 0));
+    CU(cudaMemcpyAsync(pos_host, h->md_pos, b, cudaMemcpyDeviceToHost, h->copy_stream));
+    CU(cudaMemcpyAsync(vel_host, h->md_vel, b, cudaMemcpyDeviceToHost, h->stream));
+  }
   rc = read_scalars(h);
+  if (pos_host) {
+    cudaError_t ce = cudaStreamSynchronize(h->copy_stream);
+    if (!rc && ce != cudaSuccess) rc = fail(h, NEPZBL_E_CUDA, "copy stream: %s", cudaGetErrorString(ce));
+  }
   if (rc) return rc;
   if (dt_used) *dt_used = h->h_sc->dt;
   if (rebuilt) *rebuilt = h->h_sc->do_rebuild;
@@ -977,6 +997,12 @@ int md_step(nepzbl_handle* h, double dt_max, double max_displacement, double* dt
   rc = check_device_flags(h);
   if (rc) h->md_ready = false;
   return rc;
+}
+
+int md_step(nepzbl_handle* h, double dt_max, double max_displacement, double* dt_used, int32_t* rebuilt) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_step before md_init");
+  return md_step_impl(h, dt_max, max_displacement, dt_used, rebuilt, nullptr, nullptr);
 }
 
 int md_run(nepzbl_handle* h, int64_t n_steps, double dt_max, double max_displacement, double* dt_trace,
@@ -1016,12 +1042,7 @@ int md_step_host(nepzbl_handle* h, double* pos, double* vel, double dt_max, doub
   size_t b = 24 * (size_t)h->n;
   CU(cudaMemcpyAsync(h->md_pos, pos, b, cudaMemcpyHostToDevice, h->stream));
   CU(cudaMemcpyAsync(h->md_vel, vel, b, cudaMemcpyHostToDevice, h->stream));
-  int rc = md_step(h, dt_max, max_displacement, dt_used, rebuilt);
-  if (rc) return rc;
-  CU(cudaMemcpyAsync(pos, h->md_pos, b, cudaMemcpyDeviceToHost, h->stream));
-  CU(cudaMemcpyAsync(vel, h->md_vel, b, cudaMemcpyDeviceToHost, h->stream));
-  CU(cudaStreamSynchronize(h->stream));
-  return NEPZBL_OK;
+  return md_step_impl(h, dt_max, max_displacement, dt_used, rebuilt, pos, vel);
 }
 
 int md_set_thermostat(nepzbl_handle* h, const uint8_t* group, double temperature, double tau,
