@@ -182,6 +182,9 @@ int md_get_counters(nepzbl_handle *h, int64_t *n_steps, int64_t *n_rebuilds, int
 int md_set_thermostat(nepzbl_handle *h, const uint8_t *group, double temperature, double tau,
                       int32_t chain_length);
 int md_get_thermostat(nepzbl_handle *h, double *xi, double *vxi, double *t_group, double *conserved_extra);
+/* Restore the chain (host xi[chain_length], vxi[chain_length]) -- with the caller-owned pos / vel buffers this is
+ * all a run needs to resume: md_init, md_set_thermostat, md_set_thermostat_state. */
+int md_set_thermostat_state(nepzbl_handle *h, const double *xi, const double *vxi);
 
 /*
  * Wigner-Seitz defect count: "The interstitials and vacancies were identified by

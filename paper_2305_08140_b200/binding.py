@@ -28,7 +28,7 @@ EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_d
            "nep_zbl_workspace_bytes", "nep_zbl_set_workspace", "neighbor_build", "neighbor_get",
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
            "md_run", "md_step_host", "md_energies", "md_get_forces", "md_get_counters",
-           "md_set_thermostat", "md_get_thermostat", "wigner_seitz_set_reference", "wigner_seitz_count",
+           "md_set_thermostat", "md_get_thermostat", "md_set_thermostat_state", "wigner_seitz_set_reference", "wigner_seitz_count",
            "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
 PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "spare"]
 
@@ -100,6 +100,8 @@ _lib.md_set_thermostat.argtypes = [_vp, _vp, C.c_double, C.c_double, C.c_int32]
 _lib.md_set_thermostat.restype = C.c_int
 _lib.md_get_thermostat.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_dbl), C.POINTER(_dbl), C.POINTER(_dbl)]
 _lib.md_get_thermostat.restype = C.c_int
+_lib.md_set_thermostat_state.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_dbl)]
+_lib.md_set_thermostat_state.restype = C.c_int
 _lib.wigner_seitz_set_reference.argtypes = [_vp, _i64, _vp, C.POINTER(_dbl), C.POINTER(_i32)]
 _lib.wigner_seitz_set_reference.restype = C.c_int
 _lib.wigner_seitz_count.argtypes = [_vp, _i64, _vp, _vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]
@@ -259,6 +261,11 @@ class NepZbl:
         self._group_keep = group
         self._chain = chain_length
         self._chk(_lib.md_set_thermostat(self.h, _ptr(group), temperature, tau, chain_length))
+
+    def md_set_thermostat_state(self, xi, vxi):
+        m = self._chain
+        a = (_dbl * 8)(*[float(x) for x in xi[:m]]); b = (_dbl * 8)(*[float(x) for x in vxi[:m]])
+        self._chk(_lib.md_set_thermostat_state(self.h, a, b))
 
     def md_get_thermostat(self):
         xi = (_dbl * 8)(); vxi = (_dbl * 8)(); tg = _dbl(); ex = _dbl()

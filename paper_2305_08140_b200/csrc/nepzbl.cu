@@ -1080,6 +1080,21 @@ int md_set_thermostat(nepzbl_handle* h, const uint8_t* group, double temperature
   return NEPZBL_OK;
 }
 
+int md_set_thermostat_state(nepzbl_handle* h, const double* xi, const double* vxi) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready || !h->nhc_on) return fail(h, NEPZBL_E_STATE, "no thermostat is set");
+  if (!xi || !vxi) return fail(h, NEPZBL_E_INVALID_ARG, "xi/vxi is NULL");
+  CU(cudaMemcpyAsync(h->h_nhc, h->d_nhc, sizeof(NhcState), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  for (int k = 0; k < h->h_nhc->M; ++k) {
+    h->h_nhc->xi[k] = xi[k];
+    h->h_nhc->vxi[k] = vxi[k];
+  }
+  CU(cudaMemcpyAsync(h->d_nhc, h->h_nhc, sizeof(NhcState), cudaMemcpyHostToDevice, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return NEPZBL_OK;
+}
+
 int md_get_thermostat(nepzbl_handle* h, double* xi, double* vxi, double* t_group, double* conserved_extra) {
   if (!h) return NEPZBL_E_INVALID_ARG;
   if (!h->md_ready || !h->nhc_on) return fail(h, NEPZBL_E_STATE, "no thermostat is set");

@@ -144,3 +144,21 @@ def test_border_layer_is_held_at_the_target_temperature(nb):
     vv = v2.cpu().numpy()
     t_nve = wl.W_MASS * wl.AMU_A2_FS2_TO_EV * (vv[:, group == 1] ** 2).sum() / (3 * group.sum() * KB)
     assert t_nve < 200.0
+
+
+def test_resume_from_saved_state(nb):
+    # checkpoint / resume: positions, velocities and the chain state are all a run needs
+    w = wl.thermal_bulk(6, seed=10, sigma_pos=0.03)
+    group = wl.border_group(w.pos, w.box, w.pbc, thickness=wl.A0_CONFIG)
+    g1, p1, v1 = _md(nb, w, group, 300.0, 40.0, 4)
+    g1.md_run(15, 1.0, 0.01)
+    xi, vxi, _, _ = g1.md_get_thermostat()
+    w2 = wl.thermal_bulk(6, seed=10, sigma_pos=0.03)
+    w2.pos, w2.vel = p1.cpu().numpy().copy(), v1.cpu().numpy().copy()
+    g2, p2, v2 = _md(nb, w2, group, 300.0, 40.0, 4)
+    g2.md_set_thermostat_state(xi, vxi)
+    g1.md_run(15, 1.0, 0.01)
+    g2.md_run(15, 1.0, 0.01)
+    # the resumed handle rebuilt its list (other fp32 summation order): equal to rounding
+    assert (p1 - p2).abs().max().item() < 1e-8 and (v1 - v2).abs().max().item() < 1e-9
+    assert np.allclose(g1.md_get_thermostat()[1], g2.md_get_thermostat()[1], rtol=1e-7, atol=1e-12)

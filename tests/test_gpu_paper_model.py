@@ -84,3 +84,17 @@ def test_md_follows_oracle(nb):
     assert np.abs(d).max() < 5e-6 and np.abs(vel.cpu().numpy() - ovel).max() < 5e-7
     ep, ek = g.md_energies()
     assert ep == pytest.approx(oep[-1], abs=2e-5 * w.n) and ek == pytest.approx(oek[-1], rel=1e-4)
+
+
+def test_bench_sized_system_sampled(nb):
+    # the system bench.py --workload paper times (40^3 cells, 128 000 atoms), positions displaced by 0.05 A:
+    # 512 sampled atoms against the oracle, which evaluates them one by one
+    w = wl.paper_bulk(40, seed=12)
+    w.pos = np.mod(w.pos + wl.rng(12, 23).standard_normal(w.pos.shape) * 0.05, w.box[[0, 4, 8]][:, None])
+    g = nb.NepZbl(w.model, w.n)
+    e, f, v = g.compute(w.pos, w.types, w.box, w.pbc)
+    sel = np.sort(wl.rng(12, 24).choice(w.n, size=512, replace=False)).astype(np.int32)
+    ref = oracle.compute(oracle.Params(w.model), w.pos, w.types, w.box, w.pbc, sel=sel)
+    r = parity.compare(e, f, v, ref, idx=sel, label="paper model, 128 000 atoms, sample")
+    assert max(r.values()) <= 1.0, r
+    assert np.abs(f.sum(axis=1)).max() < 0.1
