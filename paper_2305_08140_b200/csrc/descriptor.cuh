@@ -393,10 +393,29 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
   const int ntiles = (n + 31) / 32;
   const int nslots = gridDim.x * (T_ / 32);
 
-  for (int tile = (threadIdx.x >> 5) * gridDim.x + blockIdx.x; tile < ntiles; tile += nslots) {
+  // The start of a tile is a chain of dependent global loads (mask -> count -> first displacements) that two
+  // warps per scheduler cannot hide, so it is issued one tile ahead: the next tile's mask at the start of this
+  // tile, its first two displacement vectors before this tile's back-pass.
+  const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+  int tile = (threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+  unsigned long long mask_nx = 0ull;
+  float4 pre0 = dummy, pre1 = dummy;
+  {
+    const int s0 = tile * 32 + (threadIdx.x & 31);
+    if (tile < ntiles && s0 < n) {
+      mask_nx = amask[s0];
+      const int c0 = __popcll(mask_nx);
+      pre0 = c0 > 0 ? adisp[s0] : dummy;
+      pre1 = c0 > 1 ? adisp[(size_t)npad + s0] : dummy;
+    }
+  }
+  for (; tile < ntiles; tile += nslots) {
     const int s = tile * 32 + (threadIdx.x & 31);
+    const unsigned long long mask = mask_nx;
+    const int s2 = (tile + nslots) * 32 + (threadIdx.x & 31);
+    const bool v2 = tile + nslots < ntiles && s2 < n;
+    mask_nx = v2 ? amask[s2] : 0ull;
     if (s >= n) continue;
-    const unsigned long long mask = amask[s];
     const int nc = __popcll(mask);
     const float4* dp = adisp + s;
     float qr[NR];
@@ -409,8 +428,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     for (int nq = 0; nq < NA; ++nq)
 #pragma unroll
       for (int lm = 0; lm < 24; ++lm) A[nq][lm] = 0.0f;
-    const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
-    float4 nx0 = nc > 0 ? dp[0] : dummy, nx1 = nc > 1 ? dp[npad] : dummy;
+    float4 nx0 = pre0, nx1 = pre1;
     for (int c = 0; c < nc; c += 2) {
       const float4 d2[2] = {nx0, nx1};
       nx0 = c + 2 < nc ? dp[(size_t)(c + 2) * npad] : dummy;  // in flight during this iteration
@@ -566,7 +584,12 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
 
     // ---- angular partial forces dU_i/dr_ij for the in-cutoff entries (k_force skips the others)
     int c = 0;
-    float4 nx = nc > 0 ? dp[0] : dummy;
+    float4 nx = pre0;  // this tile's first displacement is still there; the next tile's are requested now
+    {
+      const int c2 = __popcll(mask_nx);
+      pre0 = c2 > 0 ? adisp[v2 ? s2 : 0] : dummy;
+      pre1 = c2 > 1 ? adisp[(size_t)npad + (v2 ? s2 : 0)] : dummy;
+    }
     for (unsigned long long m = mask; m; m &= m - 1, ++c) {
       const int a = __ffsll((long long)m) - 1;
       const float dx = nx.x, dy = nx.y, dz = nx.z;
