@@ -40,7 +40,7 @@ def synthetic_model(seed: int = 121, n_max_radial: int = 4, n_max_angular: int =
                     basis_radial: int = 8, basis_angular: int = 8, l_max: int = 4,
                     has_4body: int = 1, n_neurons: int = 50, zbl: str = "universal",
                     n_types: int = 1, skin: float = 1.0, cap_radial: int = 128,
-                    cap_angular: int = 48) -> dict:
+                    cap_angular: int = 64) -> dict:
     """Synthetic NEP-ZBL parameter set of BASELINE.json configs[0]: all c_nk and NN weights
     U(-0.5, 0.5) from the seed; q_scaler = block constants of SURVEY 8(c) C-6.
 
