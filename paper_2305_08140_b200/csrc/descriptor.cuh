@@ -245,8 +245,13 @@ __device__ __forceinline__ float tanh_fast(float z) {
 // coalesced loads.
 #define RADIAL_LANES 4
 #define RADIAL_UNROLL 4
+#ifndef RADIAL_BLOCK
+// one warp (8 atoms) per block: the grid is ~1.7 waves of resident threads, and the partly filled last wave
+// costs one block's duration -- 128-thread blocks: 49.4 us, 64: 48.6, 32: 47.7 (256 / 512: worse)
+#define RADIAL_BLOCK 32
+#endif
 template <class MS>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(RADIAL_BLOCK)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
          const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,

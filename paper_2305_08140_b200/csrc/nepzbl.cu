@@ -382,7 +382,7 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   cudaStream_t st = h->stream;
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
   prof_mark(h, PK_RADIAL);
-  k_radial<MS><<<blocks((long long)n * RADIAL_LANES, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
+  k_radial<MS><<<blocks((long long)n * RADIAL_LANES, RADIAL_BLOCK), RADIAL_BLOCK, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
                                               h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
                                               h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p),
                                               h->at<int>(c.zbl_list), h->at<int>(c.nn_a),
@@ -400,12 +400,12 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
         want_q ? h->at<float>(c.q_desc) : nullptr);
   prof_mark(h, PK_FORCE);
   if (virial)
-    k_force<MS, true><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
+    k_force<MS, true><<<blocks((long long)n * FORCE_LANES, FORCE_BLOCK), FORCE_BLOCK, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
         h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
         h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial, ka);
   else
-    k_force<MS, false><<<blocks((long long)n * FORCE_LANES, 128), 128, 0, st>>>(
+    k_force<MS, false><<<blocks((long long)n * FORCE_LANES, FORCE_BLOCK), FORCE_BLOCK, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
         h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
         h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr, ka);
