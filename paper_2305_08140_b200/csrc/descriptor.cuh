@@ -248,7 +248,7 @@ __device__ __forceinline__ float tanh_fast(float z) {
 #ifndef RADIAL_BLOCK
 // one warp (8 atoms) per block: the grid is ~1.7 waves of resident threads, and the partly filled last wave
 // costs one block's duration -- 128-thread blocks: 49.4 us, 64: 48.6, 32: 47.7 (256 / 512: worse)
-#define RADIAL_BLOCK 32
+#define RADIAL_BLOCK 64  // upper bound; the host launches 32 or 64 threads per block (nepzbl_handle::gather_block)
 #endif
 template <class MS>
 __global__ void __launch_bounds__(RADIAL_BLOCK)
@@ -358,12 +358,16 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
 //     chains feeding 240 independent FMAs);
 //   * the network takes two neurons per iteration (four independent pre-activation chains, two
 //     interleaved tanh evaluations).
-#define ANG_THREADS 128
+// One WARP per block (8 blocks per SM at 255 registers).  With 128-thread blocks the partly filled last round of
+// the persistent grid went to warps 0 and 1 of every block, i.e. to two of the four schedulers of each SM while the
+// other two idled; single-warp blocks spread it over all four: 98.7 us from 108.2 us at 128 000 atoms (64-thread
+// blocks: 106.2).  Capping the registers for a ninth / tenth warp spills and is slower (224: 135 us, 200: 146 us).
+#define ANG_THREADS 32
 // rows of the staged weight table: n_neurons rounded up to even (two neurons per iteration) plus two
 // (the software pipeline reads one pair ahead); the padding rows are zero
 __host__ __device__ inline int nn_rows(int n_neurons) { return ((n_neurons + 1) & ~1) + 2; }
 template <class MS>
-__global__ void __launch_bounds__(ANG_THREADS)
+__global__ void __launch_bounds__(ANG_THREADS, 8)
 k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
              const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
              const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,

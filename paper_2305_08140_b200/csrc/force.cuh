@@ -30,12 +30,10 @@ struct KickArgs {
   unsigned long long cond_zbl;
   int use_cond;
 };
-#ifndef FORCE_BLOCK
-// one warp (8 atoms) per block, as in k_radial: 128-thread blocks 83.1 us, 64: 80.5, 32: 78.7
-#define FORCE_BLOCK 32
-#endif
-template <class MS, bool VIRIAL>
-__global__ void __launch_bounds__(FORCE_BLOCK)
+// BLK = threads per block (32 or 64, chosen by the host from the grid size; a template parameter because the code
+// ptxas generates under __launch_bounds__(32) is 2 % faster than the same source under a bound of 64 or 128)
+template <class MS, bool VIRIAL, int BLK>
+__global__ void __launch_bounds__(BLK)
 k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
         const int* __restrict__ nn_r, const int* __restrict__ nl_r, const int* __restrict__ nn_a,
         const int* __restrict__ nl_a, const unsigned char* __restrict__ rev,

@@ -10,6 +10,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "common.cuh"
@@ -61,6 +62,10 @@ struct nepzbl_handle {
   std::vector<char> tables;   // ModelTables<MS> for the dispatched shape
   ZblParams zp{};
   size_t smem_nn = 0;
+  // threads per block of k_radial / k_force: one warp while the grid is only a few waves of resident threads (the
+  // partly filled last wave costs one block's duration: 128 000 atoms 32: 78.3 us, 64: 80.5, 128: 83.1 for
+  // k_force), two warps beyond (8.192 M atoms 32: 4.17 ms, 64: 4.02, 128: 4.11).  NEPZBL_GATHER_BLOCK overrides.
+  int gather_block = 0;
   int n_sm = 0, ang_grid = 0;  // k_angular_nn is persistent: grid = resident blocks
 
   // workspace
@@ -381,8 +386,9 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   const int n = (int)h->n, npad = c.npad;
   cudaStream_t st = h->stream;
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
+  const int gb = h->gather_block ? h->gather_block : ((long long)n * RADIAL_LANES < 8ll * 1024 * h->n_sm ? 32 : 64);
   prof_mark(h, PK_RADIAL);
-  k_radial<MS><<<blocks((long long)n * RADIAL_LANES, RADIAL_BLOCK), RADIAL_BLOCK, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
+  k_radial<MS><<<blocks((long long)n * RADIAL_LANES, gb), gb, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
                                               h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
                                               h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p),
                                               h->at<int>(c.zbl_list), h->at<int>(c.nn_a),
@@ -399,16 +405,23 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
         h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
         want_q ? h->at<float>(c.q_desc) : nullptr);
   prof_mark(h, PK_FORCE);
-  if (virial)
-    k_force<MS, true><<<blocks((long long)n * FORCE_LANES, FORCE_BLOCK), FORCE_BLOCK, 0, st>>>(
-        h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-        h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
-        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, virial, ka);
-  else
-    k_force<MS, false><<<blocks((long long)n * FORCE_LANES, FORCE_BLOCK), FORCE_BLOCK, 0, st>>>(
-        h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-        h->at<int>(c.nn_a), h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk),
-        h->at<unsigned>(c.rmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site), h->at<int>(c.perm), energy, force, nullptr, ka);
+  auto launch_force = [&](auto vir, auto blk) {
+    constexpr bool VIR = decltype(vir)::value;
+    constexpr int BLK = decltype(blk)::value;
+    k_force<MS, VIR, BLK><<<blocks((long long)n * FORCE_LANES, BLK), BLK, 0, st>>>(
+        h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.nn_a),
+        h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk), h->at<unsigned>(c.rmask),
+        mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site),
+        h->at<int>(c.perm), energy, force, VIR ? virial : nullptr, ka);
+  };
+  using std::integral_constant;
+  if (virial) {
+    if (gb == 32) launch_force(std::true_type{}, integral_constant<int, 32>{});
+    else launch_force(std::true_type{}, integral_constant<int, 64>{});
+  } else {
+    if (gb == 32) launch_force(std::false_type{}, integral_constant<int, 32>{});
+    else launch_force(std::false_type{}, integral_constant<int, 64>{});
+  }
   h->launches += 3;
   if (h->p.zbl_enabled && with_zbl) {
     prof_mark(h, PK_ZBL);
@@ -588,6 +601,10 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   h->device = device;
   h->stream = (cudaStream_t)cuda_stream;
   if (const char* ng = getenv("NEPZBL_NO_GRAPH")) h->use_graph = !(ng[0] == '1');  // see nepzbl.h (md_step)
+  if (const char* gb = getenv("NEPZBL_GATHER_BLOCK")) {
+    int v = atoi(gb);
+    if (v == 32 || v == 64) h->gather_block = v;
+  }
   std::vector<float> nnw;
   with_shape(shape, [&](auto ms) {
     using MS = decltype(ms);
