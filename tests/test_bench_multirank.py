@@ -16,7 +16,8 @@ dist.init_process_group("gloo")
 rank = dist.get_rank(); world = dist.get_world_size()
 ms = bench.aggregate_max(10.0 + 5.0 * rank, world)       # rank 1 is the slow one
 units = bench.aggregate_sum(1000.0 * (rank + 1), world)
-print(json.dumps({{"rank": rank, "ms": ms, "units": units}}), flush=True)
+sys.stdout.write(json.dumps({{"rank": rank, "ms": ms, "units": units}}) + "\n")   # one write: ranks share the pipe
+sys.stdout.flush()
 dist.barrier()
 dist.destroy_process_group()
 """
@@ -36,12 +37,27 @@ def _torchrun(args, timeout=300):
     return subprocess.run(cmd, capture_output=True, text=True, timeout=timeout, env=env, cwd=ROOT)
 
 
+def _json_objects(text):
+    """Every JSON object in the output, even if two ranks' lines ran together on the shared pipe."""
+    dec, out, i = json.JSONDecoder(), [], 0
+    while True:
+        i = text.find("{", i)
+        if i < 0:
+            return out
+        try:
+            obj, end = dec.raw_decode(text, i)
+            out.append(obj)
+            i = end
+        except json.JSONDecodeError:
+            i += 1
+
+
 def test_aggregation_world_size_2_gloo(tmp_path):
     script = tmp_path / "worker.py"
     script.write_text(_WORKER.format(root=ROOT))
     r = _torchrun([str(script)])
     assert r.returncode == 0, r.stderr[-2000:]
-    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    rows = _json_objects(r.stdout)
     assert len(rows) == 2
     for row in rows:
         assert row["ms"] == 15.0           # max over ranks
@@ -52,7 +68,7 @@ def test_reference_arm_prints_one_line_under_torchrun():
     r = _torchrun([os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "3",
                    "--warmup", "3"])
     assert r.returncode == 0, r.stderr[-2000:]
-    rows = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    rows = _json_objects(r.stdout)
     assert len(rows) == 1
     line = rows[0]
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["unit"] == "atom-steps/s"
