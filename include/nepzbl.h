@@ -143,6 +143,8 @@ int nep_zbl_get_descriptors(nepzbl_handle *h, float *q);
  * A step is replayed as ONE CUDA graph (rebuild chain and ZBL kernel in device-set IF nodes).  ncu
  * cannot see kernels inside conditional graphs: the environment variable NEPZBL_NO_GRAPH=1, read
  * at nep_zbl_create, issues the same kernels as plain stream launches instead (same results).
+ * NEPZBL_GATHER_BLOCK=32|64 (also read at create) fixes the threads per block of the two gather kernels, which
+ * the library otherwise picks from the grid size (a tuning aid; results do not depend on it).
  */
 int md_init(nepzbl_handle *h, int64_t n, double *pos_soa, double *vel_soa, const int32_t *types,
             const double box[9], const int32_t pbc[3]);
