@@ -340,3 +340,19 @@ def paper_bulk(cells: int, seed: int, temperature: float = 300.0, sigma_pos: flo
                      sigma_pos=sigma_pos, a=A0_PAPER)
     w.dt_max, w.max_displacement = 1.0, 0.01
     return w
+
+
+MO_Z, MO_MASS = 42.0, 95.95
+
+
+def alloy_model(seed: int = 121, **kw) -> dict:
+    """two atom types (W, Mo) with their own c_nk tables per ordered type pair (ti, tj), atomic
+    numbers and masses; one network (SURVEY 8(b) struct).  Synthetic, as every model here."""
+    m = synthetic_model(seed=seed, n_types=2, **kw)
+    m["atomic_number"] = np.array([W_Z, MO_Z])
+    m["mass"] = np.array([W_MASS, MO_MASS])
+    return m
+
+
+def random_types(n: int, seed: int, n_types: int = 2) -> np.ndarray:
+    return rng(seed, 10).integers(0, n_types, size=n).astype(np.int32)

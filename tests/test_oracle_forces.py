@@ -204,3 +204,51 @@ def test_block_isolated_forces_are_all_significant():
                            want_virial=False)
         rms = np.sqrt((r.force ** 2).mean())
         assert rms > 1e-2, (name, rms)
+
+
+# ------------------------------------------------------------------ two atom types
+
+def _alloy(seed=13, cells=3):
+    w = wl.config1(seed=seed, cells=cells, n_pairs=1, sigma=0.08, model=wl.alloy_model())
+    w.types = wl.random_types(w.n, seed)
+    return w
+
+
+def test_two_types_forces_equal_minus_gradient():
+    w = _alloy()
+    assert 0 < w.types.sum() < w.n
+    P = oracle.Params(w.model)
+    res = oracle.compute(P, w.pos, w.types, w.box, w.pbc, use_cell=False)
+    h = 1e-4
+    scale = np.abs(res.force).max()
+    i, j = w.info["pairs"][0]
+    for k in [i, j] + list(range(0, w.n, 7)):
+        for a in range(3):
+            pp = w.pos.copy(); pp[a, k] += h
+            pm = w.pos.copy(); pm[a, k] -= h
+            fd = -(_etot(P, w, pp) - _etot(P, w, pm)) / (2 * h)
+            assert fd == pytest.approx(res.force[a, k], abs=2e-6 * scale), (a, k)
+    assert np.abs(res.force.sum(axis=1)).max() < 1e-9 * scale * w.n
+
+
+def test_two_types_reduce_to_one_type_and_relabel():
+    w = _alloy(seed=14)
+    one = wl.synthetic_model()
+    # identical tables / Z / mass for every type pair: the labels cannot matter
+    same = dict(one, n_types=2)
+    same["c_radial"] = np.broadcast_to(one["c_radial"][0, 0], (2, 2) + one["c_radial"].shape[2:]).copy()
+    same["c_angular"] = np.broadcast_to(one["c_angular"][0, 0], (2, 2) + one["c_angular"].shape[2:]).copy()
+    same["atomic_number"] = np.array([wl.W_Z, wl.W_Z]); same["mass"] = np.array([wl.W_MASS, wl.W_MASS])
+    a = oracle.compute(oracle.Params(same), w.pos, w.types, w.box, w.pbc, use_cell=False)
+    b = oracle.compute(oracle.Params(one), w.pos, np.zeros_like(w.types), w.box, w.pbc, use_cell=False)
+    assert np.allclose(a.energy, b.energy, rtol=0, atol=1e-12) and np.allclose(a.force, b.force, rtol=0, atol=1e-11)
+    # swapping the labels 0 <-> 1 together with every per-type table is the same physical system
+    m = w.model
+    sw = dict(m, c_radial=m["c_radial"][::-1, ::-1].copy(), c_angular=m["c_angular"][::-1, ::-1].copy(),
+              atomic_number=m["atomic_number"][::-1].copy(), mass=m["mass"][::-1].copy())
+    c = oracle.compute(oracle.Params(m), w.pos, w.types, w.box, w.pbc, use_cell=False)
+    d = oracle.compute(oracle.Params(sw), w.pos, 1 - w.types, w.box, w.pbc, use_cell=False)
+    assert np.allclose(c.energy, d.energy, rtol=0, atol=1e-12) and np.allclose(c.virial, d.virial, rtol=0, atol=1e-10)
+    # and the two types really differ: the unswapped labels give other energies
+    e = oracle.compute(oracle.Params(m), w.pos, 1 - w.types, w.box, w.pbc, use_cell=False)
+    assert np.abs(e.energy - c.energy).max() > 1e-3
