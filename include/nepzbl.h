@@ -60,7 +60,7 @@ enum {
  * (l = 1..l_max, n = 0..n_max_angular); then the (2,2,2) 4-body term n = 0..n_max_angular.
  */
 typedef struct {
-  int32_t n_types;                     /* >= 1 (this build: 1) */
+  int32_t n_types;                     /* 1 or 2 in this build (2: config-sized model shape only) */
   double rc_radial, rc_angular;        /* cutoffs r_c^R, r_c^A (6.0, 4.0 A) */
   int32_t n_max_radial, n_max_angular; /* n = 0..n_max */
   int32_t basis_radial, basis_angular; /* Chebyshev basis k = 0..basis (D: C-2) */

@@ -19,8 +19,9 @@
 #pragma once
 #include "common.cuh"
 
-template <int NR_, int KR_, int NA_, int KA_, bool B4_>
+template <int NR_, int KR_, int NA_, int KA_, bool B4_, int NT_ = 1>
 struct ModelShape {
+  static constexpr int NT = NT_;  // atom types (2 = the type-pair tables c^{ti tj}_nk are exercised)
   static constexpr int NR = NR_;  // n_max_radial + 1
   static constexpr int KR = KR_;  // basis_radial + 1
   static constexpr int NA = NA_;
@@ -32,16 +33,16 @@ struct ModelShape {
   static constexpr int DPAD = (D + 3) / 4 * 4;
   // record gathered per radial pair by k_force: {position, Fp[0..NR-1]} in ONE 32-byte sector when the
   // radial descriptor has at most 5 components, else {position, d[0..KR-1]} in 64 bytes (AtomRec)
-  static constexpr bool FPREC = NR_ <= 5;
+  static constexpr bool FPREC = NR_ <= 5 && NT_ == 1;
 };
 
 // Small tables passed by value (constant bank): compile-time indexed, so they cost no loads.
 template <class MS>
 struct ModelTables {
-  float ctR[MS::NR][MS::KR];   // folded radial coefficients
-  float ctA[MS::NA][MS::KA];   // folded angular coefficients
-  float kctA[MS::NA][MS::KA];  // k * ctA (derivative through T_k' = k U_{k-1})
-  float kctR[MS::NR][MS::KR];  // k * ctR
+  // leading index: ordered type pair ti * NT + tj (central atom ti, neighbour tj)
+  float ctR[MS::NT * MS::NT][MS::NR][MS::KR];   // folded radial coefficients
+  float ctA[MS::NT * MS::NT][MS::NA][MS::KA];   // folded angular coefficients
+  float kctA[MS::NT * MS::NT][MS::NA][MS::KA];  // k * ctA (derivative through T_k' = k U_{k-1})
   float inv_rcR, inv_rcA, rcR2, rcA2;
   float zbl_flag_r2;           // (r_outer + margin)^2, 0 if ZBL disabled
   float b1;
@@ -74,6 +75,10 @@ __device__ __forceinline__ void ld_rec(const AtomRec* p, int& ux, int& uy, int& 
   } else {
     d[9] = d[10] = d[11] = 0.0f;
   }
+}
+// atom type stored in the record's last word (models with more than one type)
+__device__ __forceinline__ int ld_rec_type(const AtomRec* p) {
+  return __float_as_int(__ldg(reinterpret_cast<const float*>(p) + 15));
 }
 
 // 32-byte record {ux,uy,uz,Fp0..Fp4} (ModelShape::FPREC): one sector, one 256-bit load per pair; the pair's
@@ -263,9 +268,12 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   const int sc_ = valid ? s : 0;
   const int4 me = xyzt[sc_];
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
-  float acc[MS::KR];
+  // basis sums per NEIGHBOUR type: q_n = sum_tj sum_k ct^{ti tj}_nk acc[tj][k]
+  float acc[MS::NT][MS::KR];
 #pragma unroll
-  for (int k = 0; k < MS::KR; ++k) acc[k] = 0.0f;
+  for (int t = 0; t < MS::NT; ++t)
+#pragma unroll
+    for (int k = 0; k < MS::KR; ++k) acc[t][k] = 0.0f;
   bool close = false;
   const int cnt = valid ? nn_r[sc_] : 0;
   const int cnt_a = valid ? nn_a[sc_] : 0;
@@ -299,7 +307,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         const bool pa = e < cnt_a && r2 < mt.rcA2;
         const unsigned g = (__ballot_sync(0xffffffffu, pa) >> gshift) & 0xFu;
         if (pa) {
-          adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, 0.0f);
+          adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, __int_as_float(o[u].w));
           if (e < 32) alo |= 1u << e; else ahi |= 1u << (e - 32);
         }
         abase += __popc(g);
@@ -308,7 +316,11 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         float r = r2 * rsqrtf(r2), fc, T[MS::KR];
         cheb_T_fwd<MS::KR>(r, mt.inv_rcR, fc, T);
 #pragma unroll
-        for (int k = 0; k < MS::KR; ++k) acc[k] = fmaf(fc, T[k], acc[k]);
+        for (int t = 0; t < MS::NT; ++t) {
+          const float ft = (MS::NT == 1 || o[u].w == t) ? fc : 0.0f;
+#pragma unroll
+          for (int k = 0; k < MS::KR; ++k) acc[t][k] = fmaf(ft, T[k], acc[t][k]);
+        }
         close = close || (r2 < mt.zbl_flag_r2);
         mword |= 1u << (bit + u);
       }
@@ -327,10 +339,12 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
       mword = 0u;
     }
 #pragma unroll
-  for (int k = 0; k < MS::KR; ++k) {
-    acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], 1);
-    acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], 2);
-  }
+  for (int t = 0; t < MS::NT; ++t)
+#pragma unroll
+    for (int k = 0; k < MS::KR; ++k) {
+      acc[t][k] += __shfl_xor_sync(0xffffffffu, acc[t][k], 1);
+      acc[t][k] += __shfl_xor_sync(0xffffffffu, acc[t][k], 2);
+    }
   unsigned cb = __ballot_sync(0xffffffffu, close);
   alo |= __shfl_xor_sync(0xffffffffu, alo, 1); alo |= __shfl_xor_sync(0xffffffffu, alo, 2);
   ahi |= __shfl_xor_sync(0xffffffffu, ahi, 1); ahi |= __shfl_xor_sync(0xffffffffu, ahi, 2);
@@ -339,7 +353,11 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   for (int nq = sub; nq < MS::NR; nq += RADIAL_LANES) {
     float q = 0.0f;
 #pragma unroll
-    for (int k = 0; k < MS::KR; ++k) q = fmaf(mt.ctR[nq][k], acc[k], q);
+    for (int t = 0; t < MS::NT; ++t) {
+      const int pr = MS::NT == 1 ? 0 : me.w * MS::NT + t;
+#pragma unroll
+      for (int k = 0; k < MS::KR; ++k) q = fmaf(mt.ctR[pr][nq][k], acc[t][k], q);
+    }
     q_radial[(size_t)nq * npad + s] = q;
   }
   if (sub == 0 && ((cb >> (threadIdx.x & 28)) & 0xFu)) zbl_list[atomicAdd(&sc->zbl_count, 1)] = s;
@@ -427,6 +445,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     if (s >= n) continue;
     const int nc = __popcll(mask);
     const float4* dp = adisp + s;
+    const int ti = MS::NT > 1 ? xyzt[s].w : 0;  // type of the central atom (selects the c^{ti tj} tables)
     float qr[NR];
 #pragma unroll
     for (int nq = 0; nq < NR; ++nq) qr[nq] = q_radial[(size_t)nq * npad + s];
@@ -452,11 +471,12 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
         cheb_T_fwd<KA>(r, mt.inv_rcA, fc, T);
         if (h == 1 && c + 1 >= nc) fc = 0.0f;
         eval_blm(dx * rinv, dy * rinv, dz * rinv, b2[h]);
+        const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(d2[h].w) : 0;  // adisp.w = neighbour type
 #pragma unroll
         for (int nq = 0; nq < NA; ++nq) {
           float g = 0.0f;
 #pragma unroll
-          for (int k = 0; k < KA; ++k) g = fmaf(mt.ctA[nq][k], T[k], g);
+          for (int k = 0; k < KA; ++k) g = fmaf(mt.ctA[pr][nq][k], T[k], g);
           g2[h][nq] = g * fc;
         }
       }
@@ -563,20 +583,26 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), f[0]);
       rp[1] = make_float4(f[1], f[2], f[3], f[4]);
     } else {
+      // NT > 1: one 64-byte record per PARTNER type t, rec[NT * s + t] = {position, d^(t)_k = sum_n Fp_n ct^{ti t}_nk,
+      // own type}: k_force gathers the record of (neighbour j, my type), so the gather costs what it costs for one type
       static_assert(KR <= 12, "AtomRec holds 12 coefficients");
-      float d[12];
-#pragma unroll
-      for (int k = 0; k < 12; ++k) d[k] = 0.0f;
-#pragma unroll
-      for (int k = 0; k < KR; ++k)
-#pragma unroll
-        for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[nq][k], d[k]);
       const int4 me = xyzt[s];
-      float4* rp = reinterpret_cast<float4*>(rec + s);
-      rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
-      rp[1] = make_float4(d[1], d[2], d[3], d[4]);
-      rp[2] = make_float4(d[5], d[6], d[7], d[8]);
-      if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
+#pragma unroll
+      for (int t = 0; t < MS::NT; ++t) {
+        const int pr = MS::NT > 1 ? ti * MS::NT + t : 0;
+        float d[12];
+#pragma unroll
+        for (int k = 0; k < 12; ++k) d[k] = 0.0f;
+#pragma unroll
+        for (int k = 0; k < KR; ++k)
+#pragma unroll
+          for (int nq = 0; nq < NR; ++nq) d[k] = fmaf(Fp[nq], mt.ctR[pr][nq][k], d[k]);
+        float4* rp = reinterpret_cast<float4*>(rec + (size_t)MS::NT * s + t);
+        rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
+        rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+        rp[2] = make_float4(d[5], d[6], d[7], d[8]);
+        if (KR > 9 || MS::NT > 1) rp[3] = make_float4(d[9], d[10], d[11], __int_as_float(me.w));
+      }
     }
 
     // ---- E[n][lm] = dU/dA[n][lm] (in place)
@@ -601,7 +627,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     }
     for (unsigned long long m = mask; m; m &= m - 1, ++c) {
       const int a = __ffsll((long long)m) - 1;
-      const float dx = nx.x, dy = nx.y, dz = nx.z;
+      const float dx = nx.x, dy = nx.y, dz = nx.z, tjw = nx.w;
       nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration
       float r2 = dx * dx + dy * dy + dz * dz;
       float rinv = rsqrtf(r2), r = r2 * rinv;
@@ -609,13 +635,14 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
       cheb_U<KA>(x, Uc);
       float g[NA], dg[NA];
+      const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(tjw) : 0;
 #pragma unroll
       for (int nq = 0; nq < NA; ++nq) {
         float p = 0.0f, dp = 0.0f;
 #pragma unroll
-        for (int k = 0; k < KA; ++k) p = fmaf(mt.ctA[nq][k], T[k], p);
+        for (int k = 0; k < KA; ++k) p = fmaf(mt.ctA[pr][nq][k], T[k], p);
 #pragma unroll
-        for (int k = 1; k < KA; ++k) dp = fmaf(mt.kctA[nq][k], Uc[k - 1], dp);
+        for (int k = 1; k < KA; ++k) dp = fmaf(mt.kctA[pr][nq][k], Uc[k - 1], dp);
         g[nq] = fc * p;
         dg[nq] = fmaf(dfc, p, fc * dxdr * dp);
       }

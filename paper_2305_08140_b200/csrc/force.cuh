@@ -53,10 +53,18 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
   const bool valid = s < n;
   const int sc_ = valid ? s : 0;
   constexpr int NR = MS::NR;
-  struct Rec { int ux, uy, uz; float d[12]; };  // d[] holds Fp[0..4] when MS::FPREC
-  auto load = [&](Rec& r, int idx) {
+  constexpr int NT = MS::NT;
+  struct Rec { int ux, uy, uz, type; float d[12]; };  // d[] holds Fp[0..4] when MS::FPREC
+  // NT > 1: the records are rec[NT * atom + partner type] (k_angular_nn): the coefficients of `atom` as the central
+  // atom of a pair with a neighbour of that type; the record also carries the atom's own type
+  auto load = [&](Rec& r, int idx, int partner_type) {
+    r.type = 0;
     if (MS::FPREC) ld_rec32(rec, idx, r.ux, r.uy, r.uz, r.d);
-    else ld_rec(rec + idx, r.ux, r.uy, r.uz, r.d, KR);
+    else {
+      const AtomRec* p = rec + (size_t)NT * idx + (NT > 1 ? partner_type : 0);
+      ld_rec(p, r.ux, r.uy, r.uz, r.d, KR);
+      if (NT > 1) r.type = ld_rec_type(p);
+    }
   };
   // d[k] = sum_n Fp[n] ct_nk from a 32-byte record's Fp
   auto contract = [&](const float* fp, float* d) {
@@ -64,12 +72,21 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
     for (int k = 0; k < KR; ++k) {
       float t = 0.0f;
 #pragma unroll
-      for (int nq = 0; nq < NR; ++nq) t = fmaf(fp[nq < 12 ? nq : 0], mt.ctR[nq][k], t);
+      for (int nq = 0; nq < NR; ++nq) t = fmaf(fp[nq < 12 ? nq : 0], mt.ctR[0][nq][k], t);
       d[k] = t;
     }
   };
   Rec me;
-  load(me, sc_);
+  load(me, sc_, 0);
+  const int ti = me.type;
+  float me_d1[NT > 1 ? 12 : 1];  // my coefficients towards a neighbour of type 1 (me.d: towards type 0)
+  if (NT > 1) {
+    static_assert(NT <= 2, "k_force keeps one coefficient set per partner type in registers");
+    Rec t1;
+    load(t1, sc_, 1);
+#pragma unroll
+    for (int k = 0; k < 12; ++k) me_d1[NT > 1 ? k : 0] = t1.d[k];
+  }
   const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
   float fx = 0.0f, fy = 0.0f, fz = 0.0f;
   float w[9];
@@ -95,10 +112,10 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
     };
     int j_cur = next_j();
     Rec o_cur, o_nxt;
-    load(o_cur, j_cur >= 0 ? j_cur : sc_);
+    load(o_cur, j_cur >= 0 ? j_cur : sc_, ti);
     int j_nxt = j_cur >= 0 ? next_j() : -1;
     while (j_cur >= 0) {
-      load(o_nxt, j_nxt >= 0 ? j_nxt : sc_);
+      load(o_nxt, j_nxt >= 0 ? j_nxt : sc_, ti);
       int j_nn = j_nxt >= 0 ? next_j() : -1;
       const Rec& o = o_cur;
       float dx = (float)(o.ux - me.ux) * hx, dy = (float)(o.uy - me.uy) * hy, dz = (float)(o.uz - me.uz) * hz;
@@ -119,7 +136,10 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
           contract(o.d, dj);
         } else {
 #pragma unroll
-          for (int k = 0; k < KR; ++k) { di[k] = me.d[k]; dj[k] = o.d[k]; }
+          for (int k = 0; k < KR; ++k) {
+            di[k] = (NT > 1 && o.type == 1) ? me_d1[NT > 1 ? k : 0] : me.d[k];
+            dj[k] = o.d[k];
+          }
         }
 #pragma unroll
         for (int k = 0; k < KR; ++k) {
@@ -145,7 +165,7 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
           contract(fs5, dsum);
         } else {
 #pragma unroll
-          for (int k = 0; k < KR; ++k) dsum[k] = me.d[k] + o.d[k];
+          for (int k = 0; k < KR; ++k) dsum[k] = ((NT > 1 && o.type == 1) ? me_d1[NT > 1 ? k : 0] : me.d[k]) + o.d[k];
         }
 #pragma unroll
         for (int k = 0; k < KR; ++k) {

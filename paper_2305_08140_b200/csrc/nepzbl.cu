@@ -35,7 +35,7 @@ struct Carve {  // byte offsets into the workspace
 };
 
 struct ShapeId {
-  int nr, kr, na, ka, b4;
+  int nr, kr, na, ka, b4, nt;
 };
 
 }  // namespace
@@ -179,7 +179,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.amask = take(8 * npad);
   c.adisp = take(16 * (size_t)p.cap_angular * npad);
   c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
-  c.dk = take(64 * npad);  // AtomRec
+  c.dk = take(64 * (size_t)std::max(1, p.n_types) * npad);  // AtomRec, one per partner type
   c.pforce = take(16 * (size_t)p.cap_angular * npad);
   c.u_site = take(4 * npad);
   c.q_desc = take(4 * (size_t)D * npad);
@@ -199,16 +199,18 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
 
 // instantiated model shapes: BASELINE.json configs (with / without the 4-body term) and the paper's own
 // sizes (n_max 15 / 10, l_max 4; basis 8 / 8 is DESIGN.md C-26) -- SURVEY 8(f) NEXT-2
-const ShapeId kShapes[] = {{5, 9, 5, 9, 1}, {5, 9, 5, 9, 0}, {16, 9, 11, 9, 0}};
+const ShapeId kShapes[] = {{5, 9, 5, 9, 1, 1}, {5, 9, 5, 9, 0, 1}, {16, 9, 11, 9, 0, 1}, {5, 9, 5, 9, 1, 2}};
 using MS0 = ModelShape<5, 9, 5, 9, true>;
 using MS1 = ModelShape<5, 9, 5, 9, false>;
 using MS2 = ModelShape<16, 9, 11, 9, false>;
+using MS3 = ModelShape<5, 9, 5, 9, true, 2>;  // two atom types
 template <class F>
 void with_shape(int shape, F&& f) {
   switch (shape) {
     case 0: f(MS0{}); break;
     case 1: f(MS1{}); break;
-    default: f(MS2{}); break;
+    case 2: f(MS2{}); break;
+    default: f(MS3{}); break;
   }
 }
 // models with more than 5 angular channels use the four-lanes-per-atom kernel (descriptor_split.cuh)
@@ -230,8 +232,10 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
       }
     }
   };
-  fold(p->c_radial, MS::NR, MS::KR, &t.ctR[0][0], &t.kctR[0][0]);
-  fold(p->c_angular, MS::NA, MS::KA, &t.ctA[0][0], &t.kctA[0][0]);
+  for (int pr = 0; pr < MS::NT * MS::NT; ++pr) {  // params: [ti][tj][n][k]
+    fold(p->c_radial + (size_t)pr * MS::NR * MS::KR, MS::NR, MS::KR, &t.ctR[pr][0][0], nullptr);
+    fold(p->c_angular + (size_t)pr * MS::NA * MS::KA, MS::NA, MS::KA, &t.ctA[pr][0][0], &t.kctA[pr][0][0]);
+  }
   t.inv_rcR = (float)(1.0 / p->rc_radial);
   t.inv_rcA = (float)(1.0 / p->rc_angular);
   t.rcR2 = (float)(p->rc_radial * p->rc_radial);
@@ -566,17 +570,17 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   nepzbl_handle* h = nullptr;
   if (!p || !out) return fail(h, NEPZBL_E_INVALID_ARG, "params/out is NULL");
   *out = nullptr;
-  if (p->n_types != 1) return fail(h, NEPZBL_E_UNSUPPORTED, "this build supports n_types == 1 (got %d)", p->n_types);
+  if (p->n_types < 1 || p->n_types > 2) return fail(h, NEPZBL_E_UNSUPPORTED, "this build supports n_types 1 or 2 (got %d)", p->n_types);
   if (p->l_max != 4) return fail(h, NEPZBL_E_UNSUPPORTED, "this build supports l_max == 4 (got %d)", p->l_max);
   int shape = -1;
   for (int k = 0; k < (int)(sizeof kShapes / sizeof kShapes[0]); ++k)
     if (kShapes[k].nr == p->n_max_radial + 1 && kShapes[k].kr == p->basis_radial + 1 &&
         kShapes[k].na == p->n_max_angular + 1 && kShapes[k].ka == p->basis_angular + 1 &&
-        kShapes[k].b4 == (p->has_4body != 0))
+        kShapes[k].b4 == (p->has_4body != 0) && kShapes[k].nt == p->n_types)
       shape = k;
   if (shape < 0)
-    return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d is not instantiated in this build",
-                p->n_max_radial, p->n_max_angular, p->basis_radial, p->basis_angular, p->has_4body);
+    return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d with %d atom type(s) is not instantiated in this build",
+                p->n_max_radial, p->n_max_angular, p->basis_radial, p->basis_angular, p->has_4body, p->n_types);
   if (p->n_neurons < 1 || p->n_neurons > 256) return fail(h, NEPZBL_E_INVALID_ARG, "n_neurons out of range");
   if (p->cap_angular < 1 || p->cap_angular > 64 || p->cap_radial < 1 || p->cap_radial > 1024)
     return fail(h, NEPZBL_E_INVALID_ARG, "cap_angular must be in 1..64, cap_radial in 1..1024");

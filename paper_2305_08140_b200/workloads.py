@@ -348,7 +348,14 @@ MO_Z, MO_MASS = 42.0, 95.95
 def alloy_model(seed: int = 121, **kw) -> dict:
     """two atom types (W, Mo) with their own c_nk tables per ordered type pair (ti, tj), atomic
     numbers and masses; one network (SURVEY 8(b) struct).  Synthetic, as every model here."""
-    m = synthetic_model(seed=seed, n_types=2, **kw)
+    one = synthetic_model(seed=seed, **kw)
+    m = dict(one, n_types=2)
+    # W-like tables for every ordered pair, each coefficient changed by up to +-30 % (seeded): the descriptor keeps
+    # the magnitudes q_scaler was chosen for (SURVEY 8(c) C-6), yet all four (ti, tj) tables differ
+    g = rng(seed, 11)
+    for key in ("c_radial", "c_angular"):
+        c = np.broadcast_to(one[key][0, 0], (2, 2) + one[key].shape[2:])
+        m[key] = c * (1.0 + 0.3 * g.uniform(-1.0, 1.0, size=c.shape))
     m["atomic_number"] = np.array([W_Z, MO_Z])
     m["mass"] = np.array([W_MASS, MO_MASS])
     return m
