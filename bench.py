@@ -56,6 +56,7 @@ FLOP_PER_ATOM = {k: sum(STEP_FLOP[s] for s in v) for k, v in KERNEL_STEPS.items(
 PAPER_STEP_FLOP = {"S3": 3.5e3, "S4": 12.2e3, "S6": 25.1e3, "S7a": 25.1e3, "S7r": 8.7e3}
 PAPER_FLOP_PER_ATOM = {k: sum(PAPER_STEP_FLOP[s] for s in v) for k, v in KERNEL_STEPS.items()}
 MODEL_DESC = {
+    "alloy": "NEP-ZBL n_max 4/4, basis 8/8, l_max 4 + 4-body, 50 neurons, TWO atom types (W / Mo, type-pair tables), universal ZBL",
     "paper": "NEP-ZBL at the paper's sizes: n_max 15/10, basis 8/8, l_max 4, 100 neurons, rc 6/4 A, ZBL Eq. 3 refit 1-2 A "
              "(seeded random weights; a = 3.185 A)",
 }
@@ -89,6 +90,10 @@ def make_workload(name: str, seed_offset: int = 0, cells=None):
         return wl.config4(seed=4 + seed_offset, cells=cells or 160)
     if name == "config5":
         return wl.config5(seed=5 + seed_offset, cells=cells or (160, 160, 100))
+    if name == "alloy":   # config2's system with two atom types (W / Mo labels drawn 50/50)
+        w = wl.config2(seed=2 + seed_offset, cells=cells or 40, model=wl.alloy_model(spread=0.05, stream=13))
+        w.types = wl.random_types(w.n, 2 + seed_offset)
+        return w
     if name == "paper":   # paper-sized model, a = 3.185 A, 0.01 A per step
         return wl.paper_bulk(cells or 40, seed=12 + seed_offset)
     raise SystemExit(f"unknown workload {name}")

@@ -400,8 +400,13 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
   float* s_b0 = s_w0 + nrow * DPAD;    // [nrow]
   float* s_w1 = s_b0 + nrow;           // [nrow]
   float* s_qs = s_w1 + nrow;           // [DPAD]
+  // NT > 1: the folded angular coefficients of every ordered type pair, ct [NT*NT][NA][KA] then k * ct, behind the
+  // weights (the neighbour's type picks the table per thread: a shared-memory read, where an indexed read of
+  // the constant bank cost 2.4x the one-type kernel time)
+  const float* s_cta = s_qs + DPAD;
+  constexpr int CT_FLOATS = MS::NT > 1 ? (2 * MS::NT * MS::NT * NA * KA + 3) / 4 * 4 : 0;
   {  // all loads of a thread in flight at once (the table is a multiple of 4 floats, 16-byte aligned)
-    const int n4 = (nrow * DPAD + 2 * nrow + DPAD) / 4;
+    const int n4 = (nrow * DPAD + 2 * nrow + DPAD + CT_FLOATS) / 4;
     const float4* src = reinterpret_cast<const float4*>(nnw);
     float4* dst = reinterpret_cast<float4*>(smem);
     for (int t = threadIdx.x; t < n4; t += 4 * T_) {
@@ -476,7 +481,8 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
         for (int nq = 0; nq < NA; ++nq) {
           float g = 0.0f;
 #pragma unroll
-          for (int k = 0; k < KA; ++k) g = fmaf(mt.ctA[pr][nq][k], T[k], g);
+          for (int k = 0; k < KA; ++k)
+            g = fmaf(MS::NT > 1 ? s_cta[(pr * NA + nq) * KA + k] : mt.ctA[0][nq][k], T[k], g);
           g2[h][nq] = g * fc;
         }
       }
@@ -640,9 +646,11 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       for (int nq = 0; nq < NA; ++nq) {
         float p = 0.0f, dp = 0.0f;
 #pragma unroll
-        for (int k = 0; k < KA; ++k) p = fmaf(mt.ctA[pr][nq][k], T[k], p);
+        for (int k = 0; k < KA; ++k)
+          p = fmaf(MS::NT > 1 ? s_cta[(pr * NA + nq) * KA + k] : mt.ctA[0][nq][k], T[k], p);
 #pragma unroll
-        for (int k = 1; k < KA; ++k) dp = fmaf(mt.kctA[pr][nq][k], Uc[k - 1], dp);
+        for (int k = 1; k < KA; ++k)
+          dp = fmaf(MS::NT > 1 ? s_cta[((MS::NT * MS::NT + pr) * NA + nq) * KA + k] : mt.kctA[0][nq][k], Uc[k - 1], dp);
         g[nq] = fc * p;
         dg[nq] = fmaf(dfc, p, fc * dxdr * dp);
       }

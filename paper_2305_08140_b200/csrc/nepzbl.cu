@@ -252,6 +252,7 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   } else {
     const size_t nrow = (size_t)nn_rows(p->n_neurons);
     h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
+    if (MS::NT > 1) h->smem_nn += sizeof(float) * ((2 * MS::NT * MS::NT * MS::NA * MS::KA + 3) / 4 * 4);
   }
 }
 
@@ -296,7 +297,8 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
     return w;
   } else {
     const int neu2 = nn_rows(p->n_neurons);  // zero padding rows, see nn_rows
-    std::vector<float> w((size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD, 0.0f);
+    const size_t ct_floats = MS::NT > 1 ? (2 * MS::NT * MS::NT * MS::NA * MS::KA + 3) / 4 * 4 : 0;
+    std::vector<float> w((size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD + ct_floats, 0.0f);
     for (int m = 0; m < p->n_neurons; ++m)
       for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
     float* b0 = w.data() + (size_t)neu2 * MS::DPAD;
@@ -307,6 +309,16 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
       w1[m] = (float)p->w1[m];
     }
     for (int v = 0; v < MS::D; ++v) qs[v] = (float)p->q_scaler[v];
+    if (MS::NT > 1) {  // ct [NT*NT][NA][KA], then k * ct (k_angular_nn reads them from shared memory)
+      float* ct = qs + MS::DPAD;
+      for (int pr = 0; pr < MS::NT * MS::NT; ++pr)
+        for (int nq = 0; nq < MS::NA; ++nq)
+          for (int k = 0; k < MS::KA; ++k) {
+            const double v = folded(p->c_angular + (size_t)pr * MS::NA * MS::KA, MS::KA, nq, k);
+            ct[(pr * MS::NA + nq) * MS::KA + k] = (float)v;
+            ct[((MS::NT * MS::NT + pr) * MS::NA + nq) * MS::KA + k] = (float)(k * v);
+          }
+    }
     return w;
   }
 }
