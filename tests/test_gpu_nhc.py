@@ -162,3 +162,11 @@ def test_resume_from_saved_state(nb):
     # the resumed handle rebuilt its list (other fp32 summation order): equal to rounding
     assert (p1 - p2).abs().max().item() < 1e-8 and (v1 - v2).abs().max().item() < 1e-9
     assert np.allclose(g1.md_get_thermostat()[1], g2.md_get_thermostat()[1], rtol=1e-7, atol=1e-12)
+
+
+def test_cascade_example_runs(nb, capsys):
+    # the packaged protocol example (PKA + adaptive dt + border thermostat + Wigner-Seitz counts) on a small cell
+    from paper_2305_08140_b200 import cascade_example
+    assert cascade_example.main(["--cells", "12", "--energy-kev", "0.5", "--steps", "120", "--every", "60"]) == 0
+    out = capsys.readouterr().out
+    assert "step    120" in out and "atom-steps/s" in out
