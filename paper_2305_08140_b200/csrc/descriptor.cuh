@@ -307,7 +307,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         const bool pa = e < cnt_a && r2 < mt.rcA2;
         const unsigned g = (__ballot_sync(0xffffffffu, pa) >> gshift) & 0xFu;
         if (pa) {
-          adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, __int_as_float(o[u].w));
+          adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, MS::NT > 1 ? __int_as_float(o[u].w) : 0.0f);
           if (e < 32) alo |= 1u << e; else ahi |= 1u << (e - 32);
         }
         abase += __popc(g);
