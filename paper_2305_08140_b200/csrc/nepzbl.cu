@@ -731,7 +731,7 @@ size_t nep_zbl_workspace_bytes(const nepzbl_handle* h, int64_t n_atoms) {
 
 int nep_zbl_set_workspace(nepzbl_handle* h, void* dev_ptr, size_t bytes, int64_t n_atoms) {
   if (!h) return NEPZBL_E_INVALID_ARG;
-  if (!dev_ptr || n_atoms < 0 || n_atoms > 2000000000ll) return fail(h, NEPZBL_E_INVALID_ARG, "bad workspace arguments");
+  if (!dev_ptr || n_atoms < 0 || n_atoms > (1ll << 30)) return fail(h, NEPZBL_E_INVALID_ARG, "bad workspace arguments (n_atoms <= 2^30)");
   if (((uintptr_t)dev_ptr & 255) != 0) return fail(h, NEPZBL_E_WORKSPACE, "workspace must be 256-byte aligned");
   Carve c = carve(h->p, h->D, n_atoms);
   if (bytes < c.total) return fail(h, NEPZBL_E_WORKSPACE, "workspace too small: %zu < %zu bytes", bytes, c.total);
