@@ -114,7 +114,7 @@ int neighbor_get(nepzbl_handle *h, int which, int32_t *nn, int32_t *nl);
 /*
  * S1,S3-S7: one NEP-ZBL evaluation (Eq. 1-4; S:B-S:E): per-atom energy, force, virial.
  * Reuses the current neighbour list when it is still valid for these positions (same n, box, pbc
- * and no atom moved more than skin/2 since the build), otherwise rebuilds it.
+ * and the two largest atomic displacements since the build add up to at most the skin), otherwise rebuilds it.
  * F_i = sum_j (dU_i/dr_ij - dU_j/dr_ji);  W_i = sum_j r_ij (x) dU_j/dr_ji  (r_ij = r_j - r_i), so
  * sum_i W_i = -dE/d(strain), positive under compression.  Any output pointer may be NULL.
  */
@@ -135,8 +135,9 @@ int nep_zbl_get_descriptors(nepzbl_handle *h, float *q);
  * md_init registers caller-owned dev buffers pos_soa/vel_soa (integrated IN PLACE until destroy or
  * the next md_init), builds the list and evaluates the initial forces.
  * md_step: v_max = max_i |v_i|; dt = min(dt_max, max_displacement / v_max) (dt_max if v_max = 0);
- *   v += dt/2 F/m; x += dt v; wrap periodic axes; rebuild the list if an atom moved > skin/2 since
- *   the last build; F = F(x); v += dt/2 F/m.  Returns dt and whether the list was rebuilt (host).
+ *   v += dt/2 F/m; x += dt v; wrap periodic axes; rebuild the list if the two largest displacements since
+ *   the last build add up to more than the skin (C-15); F = F(x); v += dt/2 F/m.  Returns dt and
+ *   whether the list was rebuilt (host).
  * md_run: n_steps such steps with no host round trip in between; dt_trace (host, [n_steps]) and
  *   n_rebuilds (host) may be NULL.
  * max_displacement may be +inf (fixed dt = dt_max).

@@ -30,7 +30,7 @@ struct BoxMap {  // device-resident; recomputed by k_boxmap at every list rebuil
 struct Scalars {  // device-resident control block (one per handle)
   int do_rebuild;
   int force_rebuild;
-  unsigned int maxdisp2_bits;           // float bits: max_i |x_i - x_i(build)|^2
+  unsigned long long top2_bits;         // float bits of the TWO largest |x_i - x_i(build)|^2 (hi word: largest)
   unsigned long long vmax2_bits[2];     // double bits: max_i |v_i|^2, double-buffered by step parity
   double dt;
   double dt_max, max_disp;              // md_step arguments (set by k_md_params)
@@ -76,6 +76,60 @@ __device__ __forceinline__ unsigned int fix_coord(double x, double lo, double in
 __device__ __forceinline__ int cell_of_u(unsigned int u, int ncv, int nc) {
   int c = (int)(((unsigned long long)u * (unsigned long long)ncv) >> 32);
   return c < nc ? c : nc - 1;
+}
+
+// Rebuild criterion (C-15): a pair inside the cutoff now was inside cutoff + skin at the build as long as
+// d_i + d_j <= skin, and d_i + d_j <= d_(1) + d_(2), the two largest displacements since the build.  (The usual
+// test d_(1) > skin / 2 is the special case d_(2) = d_(1); with ONE fast atom -- a primary knock-on -- the list
+// lives twice as long.)  top-2 of squared displacements, kept as float bits (order-preserving for values >= 0).
+struct Top2 {
+  unsigned a, b;  // a >= b
+};
+__device__ __forceinline__ Top2 top2_merge(Top2 x, Top2 y) {
+  Top2 r;
+  r.a = max(x.a, y.a);
+  r.b = max(min(x.a, y.a), max(x.b, y.b));
+  return r;
+}
+// top-2 over a block of <= 1024 threads (one value per thread); result valid in thread 0
+__device__ __forceinline__ Top2 block_top2(float v, unsigned* sh /* [64] */) {
+  Top2 t{__float_as_uint(v), 0u};
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    Top2 u{__shfl_xor_sync(0xffffffffu, t.a, o), __shfl_xor_sync(0xffffffffu, t.b, o)};
+    t = top2_merge(t, u);
+  }
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { sh[2 * w] = t.a; sh[2 * w + 1] = t.b; }
+  __syncthreads();
+  if (w == 0) {
+    const int nw = (blockDim.x + 31) >> 5;
+    t.a = l < nw ? sh[2 * l] : 0u;
+    t.b = l < nw ? sh[2 * l + 1] : 0u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      Top2 u{__shfl_xor_sync(0xffffffffu, t.a, o), __shfl_xor_sync(0xffffffffu, t.b, o)};
+      t = top2_merge(t, u);
+    }
+  }
+  return t;
+}
+// Merge a block's top-2 into the global pair with two integer atomicMax (no CAS loop: ~500 blocks hit one address).
+// W1 (high word) = largest: the exchange old = atomicMax(W1, a) has a loser min(old, a); W2 (low word) takes the
+// maximum of all losers and of all blocks' second values.  Every loser is the smaller of two distinct atoms'
+// values, so W2 never exceeds the true second largest, and the true second largest s is always recorded: when its
+// block meets W1, either it loses at once (old >= s) or it wins and loses later to the one larger value.
+__device__ __forceinline__ void top2_publish(unsigned long long* addr, Top2 t) {
+  if (t.a == 0u) return;
+  unsigned* w = reinterpret_cast<unsigned*>(addr);  // little endian: w[1] = largest, w[0] = second largest
+  const unsigned old = atomicMax(&w[1], t.a);
+  const unsigned second = max(min(old, t.a), t.b);
+  if (second) atomicMax(&w[0], second);
+}
+// rebuild if the two largest displacements since the build add up to more than the skin (1e-5 safety margin for
+// the rounding of the fixed-point differences and of sqrtf)
+__device__ __forceinline__ int top2_exceeds(unsigned long long bits, float skin) {
+  return sqrtf(__uint_as_float((unsigned)(bits >> 32))) + sqrtf(__uint_as_float((unsigned)bits)) > skin * (1.0f - 1e-5f);
 }
 
 __device__ __forceinline__ float block_max_128(float v, float* sh) {

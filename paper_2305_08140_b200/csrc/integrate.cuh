@@ -27,7 +27,7 @@ __device__ __forceinline__ double step_dt(const Scalars* sc) {
 
 // run by the last block of k_kick_drift: book-keeping of the step (dt for the second half-kick and the trace,
 // flip the vmax slot) and the rebuild decision; in a captured graph it also sets the IF nodes
-__device__ __forceinline__ void step_flag(Scalars* sc, float half_skin2, double* dt_trace, int trace_ring,
+__device__ __forceinline__ void step_flag(Scalars* sc, float skin, double* dt_trace, int trace_ring,
                                           unsigned long long cond_rebuild, int use_cond) {
   double dt = step_dt(sc);
   sc->dt = dt;
@@ -37,8 +37,8 @@ __device__ __forceinline__ void step_flag(Scalars* sc, float half_skin2, double*
   sc->n_steps += 1;
   if (dt_trace) dt_trace[sc->trace_pos % trace_ring] = dt;
   sc->trace_pos += 1;
-  int r = sc->force_rebuild || (__uint_as_float(sc->maxdisp2_bits) > half_skin2);
-  sc->maxdisp2_bits = 0u;  // k_kick_drift of the next step accumulates the displacement since the build again
+  int r = sc->force_rebuild || top2_exceeds(sc->top2_bits, skin);
+  sc->top2_bits = 0ull;  // k_kick_drift of the next step accumulates the displacements since the build again
   sc->do_rebuild = r;
   sc->force_rebuild = 0;
   sc->zbl_count = 0;
@@ -48,7 +48,7 @@ __device__ __forceinline__ void step_flag(Scalars* sc, float half_skin2, double*
 #endif
 }
 struct StepFlagArgs {  // passed by value to k_kick_drift, whose last block runs step_flag
-  float half_skin2;
+  float skin;
   double* dt_trace;
   int trace_ring;
   unsigned long long cond_rebuild;
@@ -192,7 +192,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
              const int* __restrict__ inv_perm, int4* __restrict__ xyzt,
              const int4* __restrict__ xyzt_build, const unsigned char* __restrict__ group,
              const NhcState* __restrict__ nh, const StepFlagArgs fa) {
-  __shared__ float sh[32];
+  __shared__ unsigned sh[64];
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   float d2 = 0.0f;
   if (i < n) {
@@ -222,16 +222,16 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
     float dz = (float)((int)u[2] - b.z) * bm->hf[2];
     d2 = dx * dx + dy * dy + dz * dz;
   }
-  float m = block_max_128(d2, sh);
+  const Top2 m = block_top2(d2, sh);
   if (threadIdx.x == 0) {
-    if (m > 0.0f) atomicMax(&sc->maxdisp2_bits, __float_as_uint(m));
+    top2_publish(&sc->top2_bits, m);
     // the block that finishes last does the step's book-keeping (formerly a one-thread kernel of its own):
     // every other block has read dt / parity and published its displacement maximum before its ticket
     __threadfence();
     if (atomicAdd(&sc->blocks_done, 1u) == gridDim.x - 1) {
       __threadfence();
       sc->blocks_done = 0u;
-      step_flag(sc, fa.half_skin2, fa.dt_trace, fa.trace_ring, fa.cond_rebuild, fa.use_cond);
+      step_flag(sc, fa.skin, fa.dt_trace, fa.trace_ring, fa.cond_rebuild, fa.use_cond);
     }
   }
 }

@@ -50,7 +50,7 @@ __global__ void k_rebuild_begin(Scalars* sc) {
   // overflow_radial / overflow_angular are NOT reset here: they stay set until the host has reported them
   // (check_device_flags -> k_clear_errors), so an overflow in the middle of an md_run chunk is not lost when
   // a later rebuild of the same chunk happens to fit
-  sc->maxdisp2_bits = 0u;
+  sc->top2_bits = 0ull;
 }
 
 // Fixed-point grid and cell grid for cells of edge >= rcs * f / S.  Returns the number of cells, or
@@ -409,7 +409,7 @@ __global__ void __launch_bounds__(256)
 k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restrict__ pos,
        const int32_t* __restrict__ types, const int* __restrict__ inv_perm, int4* __restrict__ xyzt,
        const int4* __restrict__ xyzt_build) {
-  __shared__ float sh[32];
+  __shared__ unsigned sh[64];
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   float d2 = 0.0f;
   if (i < n) {
@@ -429,14 +429,14 @@ k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restri
     float dz = (float)((int)uz - b.z) * bm->hf[2];
     d2 = dx * dx + dy * dy + dz * dz;
   }
-  float m = block_max_128(d2, sh);
-  if (threadIdx.x == 0 && m > 0.0f) atomicMax(&sc->maxdisp2_bits, __float_as_uint(m));
+  const Top2 m = block_top2(d2, sh);
+  if (threadIdx.x == 0) top2_publish(&sc->top2_bits, m);
 }
 
 // decide whether the list must be rebuilt for this evaluation; reset per-evaluation counters.
-__global__ void k_flag(Scalars* sc, float half_skin2) {
-  int r = sc->force_rebuild || (__uint_as_float(sc->maxdisp2_bits) > half_skin2);
-  sc->maxdisp2_bits = 0u;
+__global__ void k_flag(Scalars* sc, float skin) {
+  int r = sc->force_rebuild || top2_exceeds(sc->top2_bits, skin);
+  sc->top2_bits = 0ull;
   sc->do_rebuild = r;
   sc->force_rebuild = 0;
   sc->zbl_count = 0;

@@ -551,7 +551,7 @@ int eval_common(nepzbl_handle* h, long long n, const double* pos, const int32_t*
   if (n == 0) return NEPZBL_OK;
   if (!pos) return fail(h, NEPZBL_E_INVALID_ARG, "pos is NULL");
   const Carve& c = h->cv;
-  float hs = (float)(0.5 * h->p.skin);
+  const float skin = (float)h->p.skin;
   if (changed || force_rebuild) {
     k_set_force_rebuild<<<1, 1, 0, h->stream>>>(h->d_sc);
   } else {
@@ -559,7 +559,7 @@ int eval_common(nepzbl_handle* h, long long n, const double* pos, const int32_t*
                                                   h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                                   h->at<int4>(c.xyzt_build));
   }
-  k_flag<<<1, 1, 0, h->stream>>>(h->d_sc, hs * hs);
+  k_flag<<<1, 1, 0, h->stream>>>(h->d_sc, skin);
   h->launches += 2;
   prof_mark(h, PK_REBUILD);
   h->launches += enqueue_rebuild(h, pos, types, h->stream);
@@ -868,7 +868,7 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
   const Carve& c = h->cv;
   const int n = (int)h->n;
   cudaStream_t st = h->stream;
-  float hs = (float)(0.5 * h->p.skin);
+  const float skin = (float)h->p.skin;
   prof_mark(h, PK_INTEGRATE_A);
   h->launches += enqueue_nhc(h, 0, st);
   k_kick_drift<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, h->md_pos, h->md_vel,
@@ -876,7 +876,7 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
                                               h->d_nhc,
-                                              StepFlagArgs{hs * hs, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0});
+                                              StepFlagArgs{skin, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0});
   cudaEventRecord(h->ev_drift, st);
   h->launches += 1;
   prof_mark(h, PK_REBUILD);
@@ -906,7 +906,7 @@ static bool build_step_graph(nepzbl_handle* h) {
   const Carve& c = h->cv;
   const int n = (int)h->n;
   cudaStream_t st = h->stream;
-  float hs = (float)(0.5 * h->p.skin);
+  const float skin = (float)h->p.skin;
   if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return false;
   cudaGraph_t g = nullptr;
   if (cudaGraphCreate(&g, 0) != cudaSuccess) return false;
@@ -941,7 +941,7 @@ static bool build_step_graph(nepzbl_handle* h) {
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
                                               h->d_nhc,
-                                              StepFlagArgs{hs * hs, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1});
+                                              StepFlagArgs{skin, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1});
   ok = ok && cudaEventRecordWithFlags(h->ev_drift, st, cudaEventRecordExternal) == cudaSuccess;
   nk += 1;
   cudaGraph_t body = nullptr;
