@@ -155,3 +155,32 @@ def test_overflow_inside_a_long_md_run_is_reported_not_fatal(nb):
     g2 = nb.NepZbl(w2.model, w2.n)
     e, f, v = g2.compute(w2.pos, w2.types, w2.box, w2.pbc)
     assert np.isfinite(e).all()
+
+
+def test_rebuild_criterion_two_largest_displacements(nb):
+    # DESIGN C-15: the list is rebuilt when the two largest displacements since the build add up to more than the
+    # skin (1 A).  One atom moved by 0.8 A: no rebuild, and the forces from the old list are still the oracle's;
+    # a second atom moved by 0.5 A: 1.3 A > skin, rebuild.
+    w = wl.thermal_bulk(6, seed=12, temperature=1.0)      # ~cold: thermal motion adds < 1e-3 A per step
+    g, pos, vel = _md(nb, w)
+    P = oracle.Params(w.model)
+    dt, rebuilt = g.md_step(1e-3, float("inf"))
+    assert rebuilt == 0
+    pos[0, 17] += 0.8                                      # the caller owns the state and may edit it between steps
+    dt, rebuilt = g.md_step(1e-3, float("inf"))
+    assert rebuilt == 0
+    f, e = g.md_get_forces()
+    ref = oracle.compute(P, pos.cpu().numpy(), w.types, w.box, w.pbc)
+    r = parity.compare(e.cpu().numpy(), f.cpu().numpy(), None, ref, label="0.8 A on the old list")
+    assert max(r.values()) <= 1.0, r
+    pos[1, 230] -= 0.5
+    dt, rebuilt = g.md_step(1e-3, float("inf"))
+    assert rebuilt == 1
+    f, e = g.md_get_forces()
+    ref = oracle.compute(P, pos.cpu().numpy(), w.types, w.box, w.pbc)
+    r = parity.compare(e.cpu().numpy(), f.cpu().numpy(), None, ref, label="after the rebuild")
+    assert max(r.values()) <= 1.0, r
+    # and the classic case: one atom beyond the whole skin
+    pos[2, 99] += 1.05
+    dt, rebuilt = g.md_step(1e-3, float("inf"))
+    assert rebuilt == 1
