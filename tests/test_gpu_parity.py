@@ -258,3 +258,19 @@ def test_config2_sampled_parity_at_full_size(nb):
     ref = oracle.compute(oracle.Params(w.model), w.pos, w.types, w.box, w.pbc, sel=sel)
     _assert_ok(parity.compare(e, f, v, ref, idx=sel, label="config2 sample"))
     assert np.abs(f.sum(axis=1)).max() < 0.05
+
+
+def test_neighbor_sets_with_a_large_capacity(nb):
+    # cap_radial above k_nbr's per-thread buffer (192) takes the two-walk path of the list build
+    w = wl.config1(seed=12, cells=6)
+    m = dict(w.model, cap_radial=256)
+    g = nb.NepZbl(m, w.n)
+    pos = torch.from_numpy(w.pos).cuda(); types = torch.from_numpy(w.types).cuda()
+    g.neighbor_build(pos, types, w.box, w.pbc)
+    for which, rc in ((0, 7.0), (1, 5.0)):
+        nn, nl = g.neighbor_get(which)
+        bad, dup, _ = parity.compare_neighbor_sets(nn.cpu().numpy(), nl.cpu().numpy(), w.pos, w.box, w.pbc, rc, oracle)
+        assert not bad and not dup
+    ref = oracle.compute(oracle.Params(m), w.pos, w.types, w.box, w.pbc)
+    e, f, v = g.compute(w.pos, w.types, w.box, w.pbc)
+    _assert_ok(parity.compare(e, f, v, ref, label="cap_radial 256"))
