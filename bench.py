@@ -70,8 +70,8 @@ FP32_LANES_PER_SM = 128
 WS_BYTES_PER_ATOM = 68.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on config2 (128 000 atoms) from the committed
 # `ncu --set full` capture (NCU_TRAFFIC_SOURCE); reported as roofline.traffic for that workload only.
-NCU_TRAFFIC_BYTES = {"config2": {"k_radial": 48.190720e6 + 6.329344e6, "k_angular_nn": 46.718464e6 + 13.804032e6,
-                                 "k_force": 91.835904e6 + 5.368064e6},
+NCU_TRAFFIC_BYTES = {"config2": {"k_radial": 54.474240e6, "k_angular_nn": 60.081920e6,
+                                 "k_force": 96.386304e6},
                      "paper": {"k_angular_nn": 55.964928e6 + 18.282496e6}}
 NCU_TRAFFIC_SOURCE = "profiles/r1e_ncu_full.md"
 
