@@ -43,6 +43,7 @@ struct Scalars {  // device-resident control block (one per handle)
   int zbl_count;
   int n_rebuilds;
   long long n_steps;
+  float disp_sum;                       // d_(1) + d_(2) of the current positions against the build (0 right after a build)
   unsigned int blocks_done;             // ticket counter of k_kick_drift's last-block book-keeping
 };
 
@@ -128,6 +129,10 @@ __device__ __forceinline__ void top2_publish(unsigned long long* addr, Top2 t) {
 }
 // rebuild if the two largest displacements since the build add up to more than the skin (1e-5 safety margin for
 // the rounding of the fixed-point differences and of sqrtf)
+// upper bound of d_(1) + d_(2) (rounded up a little: it decides which skin-shell entries may be skipped)
+__device__ __forceinline__ float top2_sum(unsigned long long bits) {
+  return (sqrtf(__uint_as_float((unsigned)(bits >> 32))) + sqrtf(__uint_as_float((unsigned)bits))) * (1.0f + 1e-5f) + 1e-6f;
+}
 __device__ __forceinline__ int top2_exceeds(unsigned long long bits, float skin) {
   return sqrtf(__uint_as_float((unsigned)(bits >> 32))) + sqrtf(__uint_as_float((unsigned)bits)) > skin * (1.0f - 1e-5f);
 }

@@ -45,6 +45,7 @@ struct ModelTables {
   float kctA[MS::NT * MS::NT][MS::NA][MS::KA];  // k * ctA (derivative through T_k' = k U_{k-1})
   float inv_rcR, inv_rcA, rcR2, rcA2;
   float zbl_flag_r2;           // (r_outer + margin)^2, 0 if ZBL disabled
+  float inv_shell_w;           // 8 / skin (0 without skin): sub-shells of the list's skin shell, see k_nbr
   float b1;
   int n_neurons;
 };
@@ -261,7 +262,8 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
          const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,
          unsigned* __restrict__ rmask, int mask_words, int* __restrict__ zbl_list,
-         const int* __restrict__ nn_a, unsigned long long* __restrict__ amask, float4* __restrict__ adisp) {
+         const int* __restrict__ nn_a, unsigned long long* __restrict__ amask, float4* __restrict__ adisp,
+         const unsigned long long* __restrict__ shellq) {
   const int gt = blockIdx.x * blockDim.x + threadIdx.x;
   const int s = gt / RADIAL_LANES, sub = gt % RADIAL_LANES;
   const bool valid = s < n;
@@ -275,8 +277,19 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
 #pragma unroll
     for (int k = 0; k < MS::KR; ++k) acc[t][k] = 0.0f;
   bool close = false;
-  const int cnt = valid ? nn_r[sc_] : 0;
+  int cnt = valid ? nn_r[sc_] : 0;
   const int cnt_a = valid ? nn_a[sc_] : 0;
+  {
+    // the skin shell is ordered by the distance at the build; with the two largest displacements adding up to D
+    // only its entries inside rc + D can have come inside the cutoff (k_nbr, Scalars::disp_sum)
+    const unsigned long long sq = valid ? shellq[sc_] : 0ull;
+    const int total = (int)(sq >> 56);
+    if (total < 255) {  // 255 = saturated count: walk everything
+      const int m = min(8, (int)ceilf(sc->disp_sum * mt.inv_shell_w));
+      const int reach = m > 0 ? (int)((sq >> (8 * (m - 1))) & 0xFFull) : 0;
+      cnt -= total - reach;
+    }
+  }
   const int* lp = nl_r + (size_t)sub * npad + sc_;
   const size_t lstride = (size_t)RADIAL_LANES * npad;
   unsigned mword = 0u;

@@ -38,6 +38,7 @@ __device__ __forceinline__ void step_flag(Scalars* sc, float skin, double* dt_tr
   if (dt_trace) dt_trace[sc->trace_pos % trace_ring] = dt;
   sc->trace_pos += 1;
   int r = sc->force_rebuild || top2_exceeds(sc->top2_bits, skin);
+  sc->disp_sum = r ? 0.0f : top2_sum(sc->top2_bits);
   sc->top2_bits = 0ull;  // k_kick_drift of the next step accumulates the displacements since the build again
   sc->do_rebuild = r;
   sc->force_rebuild = 0;

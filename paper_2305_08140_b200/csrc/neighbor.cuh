@@ -288,7 +288,8 @@ __device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int S, int 
 __global__ void __launch_bounds__(128)
 k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
       const int* __restrict__ cell_start, float rc2_radial, float rcs2_radial, float rcs2_angular, int cap_r, int cap_a,
-      int* __restrict__ nn_r, int* __restrict__ nl_r, int* __restrict__ nn_a) {
+      int* __restrict__ nn_r, int* __restrict__ nl_r, int* __restrict__ nn_a,
+      unsigned long long* __restrict__ shellq, float rc_radial, float shell_w) {
   if (!sc->do_rebuild) return;
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
@@ -300,12 +301,14 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
   axis_stencil(cell_of_u((unsigned)me.y, bm->ncv[1], bm->nc[1]), bm->nc[1], bm->pbc[1], S, sy);
   axis_stencil(cell_of_u((unsigned)me.z, bm->ncv[2], bm->nc[2]), bm->nc[2], bm->pbc[2], S, sz);
   int na = 0, nb = 0, nc = 0;   // segment sizes
+  unsigned long long shellq_val = ~0ull;  // "not ordered": set below when the shell could be sorted
   // ONE walk when the list fits the per-thread buffer (any cap_r <= NBR_BUF): the accepted candidates are parked,
   // tagged with their segment, in local memory (L1-resident) and then laid out segment by segment; the first
   // version walked the cells twice and evaluated the ~340 candidate distances twice (k_nbr 1.54 ms at 1.024 M atoms).
   constexpr int NBR_BUF = 192;
   if (cap_r <= NBR_BUF) {
     int buf[NBR_BUF];
+    float br[NBR_BUF];  // distance at the build (used to order the skin shell)
     int cnt = 0;
     for (int kz = 0; kz < W; ++kz) {
       if (sz[kz] < 0) continue;
@@ -325,7 +328,10 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
             if (r2 < rcs2_radial) {
               const int seg = r2 < rcs2_angular ? 0 : (r2 < rc2_radial ? 1 : 2);
               na += seg == 0; nb += seg == 1; nc += seg == 2;
-              if (cnt < NBR_BUF) buf[cnt] = j | (seg << 30);  // j < 2^30 (nep_zbl_set_workspace)
+              if (cnt < NBR_BUF) {
+                buf[cnt] = j | (seg << 30);  // j < 2^30 (nep_zbl_set_workspace)
+                br[cnt] = r2;
+              }
               ++cnt;
             }
           }
@@ -336,9 +342,42 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
       int oa = 0, ob = na, oc = na + nb;  // next slot of each segment (walk order kept inside a segment)
       for (int t = 0; t < cnt; ++t) {
         const int v = buf[t], seg = (unsigned)v >> 30;
-        const int slot = seg == 0 ? oa++ : (seg == 1 ? ob++ : oc++);
+        if (seg == 2) continue;
+        const int slot = seg == 0 ? oa++ : ob++;
         nl_r[(size_t)slot * npad + s] = v & 0x3fffffff;
       }
+      // The skin shell goes in ascending order of its distance at the build (stable: walk order between equals), and
+      // shellq[s] keeps, byte m - 1, how many of its entries lay inside rc + m * skin / 8.  An entry that lay at
+      // r_b cannot be inside rc while the two largest displacements since the build add up to less than r_b - rc
+      // (Scalars::disp_sum), so k_radial walks only the prefix of the shell that the current displacements can reach.
+      int ns = 0;
+      for (int t = 0; t < cnt; ++t)
+        if (((unsigned)buf[t] >> 30) == 2) {  // compact the shell entries to the front of the buffers, then sort them
+          buf[ns] = buf[t] & 0x3fffffff;
+          br[ns] = br[t];
+          ++ns;
+        }
+      for (int a = 1; a < ns; ++a) {
+        const int vj = buf[a];
+        const float vr = br[a];
+        int q = a - 1;
+        while (q >= 0 && br[q] > vr) {
+          buf[q + 1] = buf[q];
+          br[q + 1] = br[q];
+          --q;
+        }
+        buf[q + 1] = vj;
+        br[q + 1] = vr;
+      }
+      unsigned long long packed = 0ull;
+      int m = 1, upto = 0;
+      for (int t = 0; t < ns; ++t) nl_r[(size_t)(oc + t) * npad + s] = buf[t];
+      for (; m <= 8; ++m) {
+        const float lim = rc_radial + m * shell_w;
+        while (upto < ns && br[upto] < lim * lim) ++upto;
+        packed |= (unsigned long long)min(m == 8 ? ns : upto, 255) << (8 * (m - 1));
+      }
+      shellq_val = packed;
     }
   } else {
   int oa = 0, ob = 0, oc = 0;   // next slot of each segment (second walk)
@@ -379,6 +418,11 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
   }
   }
   const int cr = na + nb + nc;
+  if (shellq_val == ~0ull) {  // two-walk path or overflow: every sub-shell count = the whole shell (nothing is skipped)
+    const unsigned long long c8 = (unsigned long long)min(nc, 255);
+    shellq_val = c8 * 0x0101010101010101ull;
+  }
+  shellq[s] = shellq_val;
   nn_r[s] = min(cr, cap_r);
   nn_a[s] = (cr > cap_r || na > cap_a) ? 0 : na;
   if (cr > cap_r) atomicMax(&sc->overflow_radial, cr);
@@ -436,6 +480,7 @@ k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restri
 // decide whether the list must be rebuilt for this evaluation; reset per-evaluation counters.
 __global__ void k_flag(Scalars* sc, float skin) {
   int r = sc->force_rebuild || top2_exceeds(sc->top2_bits, skin);
+  sc->disp_sum = r ? 0.0f : top2_sum(sc->top2_bits);
   sc->top2_bits = 0ull;
   sc->do_rebuild = r;
   sc->force_rebuild = 0;

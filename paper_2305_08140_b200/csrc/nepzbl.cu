@@ -29,7 +29,7 @@ constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
-      nn_r, nn_a, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
+      nn_r, nn_a, shellq, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
       partial, nhc_partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
@@ -173,6 +173,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.cell_start = take(4 * ((size_t)c.ncell_cap + 1));
   c.nn_r = take(4 * npad);
   c.nn_a = take(4 * npad);
+  c.shellq = take(8 * npad);
   c.nl_r = take(4 * (size_t)p.cap_radial * npad);
   c.rev = take((size_t)p.cap_angular * npad);
   c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
@@ -242,6 +243,7 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   t.rcA2 = (float)(p->rc_angular * p->rc_angular);
   double zf = p->zbl_r_outer + 0.01;
   t.zbl_flag_r2 = p->zbl_enabled ? (float)(zf * zf) : 0.0f;
+  t.inv_shell_w = p->skin > 0 ? (float)(8.0 / p->skin) : 0.0f;
   t.b1 = (float)p->b1;
   t.n_neurons = p->n_neurons;
   h->tables.resize(sizeof t);
@@ -388,7 +390,8 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
   k_nbr<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
                                        h->at<int>(c.cell_start), rc2, rr, ra2, h->p.cap_radial,
                                        h->p.cap_angular, h->at<int>(c.nn_r), h->at<int>(c.nl_r),
-                                       h->at<int>(c.nn_a));
+                                       h->at<int>(c.nn_a), h->at<unsigned long long>(c.shellq),
+                                       (float)h->p.rc_radial, (float)(h->p.skin / 8.0));
   k_rev<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, n, npad, h->at<int>(c.nn_a), h->at<int>(c.nl_r),
                                        h->at<unsigned char>(c.rev));
   return nk + 9;
@@ -408,7 +411,8 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
                                               h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
                                               h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p),
                                               h->at<int>(c.zbl_list), h->at<int>(c.nn_a),
-                                              h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp));
+                                              h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp),
+                                              h->at<unsigned long long>(c.shellq));
   prof_mark(h, PK_ANGULAR_NN);
   if constexpr (kSplit<MS>)
     k_angular_nn_split<MS><<<std::min(blocks((long long)n * SPLIT_LANES, SPLIT_THREADS), h->ang_grid), SPLIT_THREADS, h->smem_nn, st>>>(
