@@ -63,15 +63,15 @@ MODEL_DESC = {
 DEFAULT_MODEL_DESC = "NEP-ZBL n_max 4/4, basis 8/8, l_max 4 + 4-body, 50 neurons, rc 6/4 A, universal ZBL 1-2 A"
 # Compulsory HBM bytes per atom-step of each kernel group (same table)
 # (k_force carries the second half-kick: + 48 B of fp64 velocities; the per-atom record is 32 B)
-BYTES_PER_ATOM = {"integrate_a": 152.0, "k_radial": 392.0, "k_angular_nn": 596.0, "k_force": 1168.0}
+BYTES_PER_ATOM = {"integrate_a": 152.0, "k_radial": 292.0, "k_angular_nn": 596.0, "k_force": 1168.0}
 FP32_LANES_PER_SM = 128
 # Wigner-Seitz count, compulsory HBM bytes per atom (one site per atom): position 24 + nearest 4 + occupancy
 # read-modify-write 8 + count read 4 + cell-sorted site record 28 (the 27-cell scan re-reads sites from L1/L2)
 WS_BYTES_PER_ATOM = 68.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on config2 (128 000 atoms) from the committed
 # `ncu --set full` capture (NCU_TRAFFIC_SOURCE); reported as roofline.traffic for that workload only.
-NCU_TRAFFIC_BYTES = {"config2": {"k_radial": 54.474240e6, "k_angular_nn": 60.081920e6,
-                                 "k_force": 96.386304e6},
+NCU_TRAFFIC_BYTES = {"config2": {"k_radial": 36.140544e6, "k_angular_nn": 58.577408e6,
+                                 "k_force": 96.876288e6},
                      "paper": {"k_angular_nn": 55.964928e6 + 18.282496e6}}
 NCU_TRAFFIC_SOURCE = "profiles/r1e_ncu_full.md"
 
