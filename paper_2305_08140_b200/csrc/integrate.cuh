@@ -216,7 +216,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
       u[a] = fix_coord(isfinite(xx) ? xx : 0.0, bm->lo[a], bm->inv_h[a]);
     }
     int s = inv_perm[i];
-    int4 b = xyzt_build[s];
+    int4 b = xyzt_build[i];
     xyzt[s] = make_int4((int)u[0], (int)u[1], (int)u[2], t);
     float dx = (float)((int)u[0] - b.x) * bm->hf[0];
     float dy = (float)((int)u[1] - b.y) * bm->hf[1];

@@ -236,7 +236,7 @@ __global__ void k_permute(const Scalars* sc, int n, const int* __restrict__ orde
   inv_perm[i] = s;
   int4 v = xyzt_tmp[i];
   xyzt[s] = v;
-  xyzt_build[s] = v;
+  xyzt_build[i] = v;  // CALLER order: k_kick_drift / k_prep read it coalesced, without waiting for inv_perm
 }
 
 // neighbour cells along one axis: up to 2S+1 distinct indices in out[0..2S], -1 = none
@@ -466,7 +466,7 @@ k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restri
     unsigned int uy = fix_coord(y, bm->lo[1], bm->inv_h[1]);
     unsigned int uz = fix_coord(z, bm->lo[2], bm->inv_h[2]);
     int s = inv_perm[i];
-    int4 b = xyzt_build[s];
+    int4 b = xyzt_build[i];
     xyzt[s] = make_int4((int)ux, (int)uy, (int)uz, types ? types[i] : 0);
     float dx = (float)((int)ux - b.x) * bm->hf[0];
     float dy = (float)((int)uy - b.y) * bm->hf[1];
