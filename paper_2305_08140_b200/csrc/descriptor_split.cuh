@@ -67,7 +67,7 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
                    AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out) {
   using LY = SplitLayout<MS>;
   static_assert(MS::NT == 1, "the four-lane kernel is instantiated for one atom type");
-  constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR;
+  constexpr int KA = MS::KA, NR = MS::NR, KR = MS::KR;
   constexpr int NSUB = LY::NSUB, RSUB = LY::RSUB, SLP = LY::SLP, SLS = LY::SLS, NAP = LY::NAP;
   extern __shared__ __align__(16) float smem[];
   const int nrow = LY::rows(mt.n_neurons);

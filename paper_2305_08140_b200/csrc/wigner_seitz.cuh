@@ -108,15 +108,14 @@ k_ws_place(int ns, const double* __restrict__ site, const int* __restrict__ cell
   rec[k] = r;
 }
 __device__ __forceinline__ void ws_load(const WsSite* p, double& x, double& y, double& z, int& idx) {
-  unsigned v0, v1, v2, v3, v4, v5, v6, v7;
+  unsigned v0, v1, v2, v3, v4, v5, v6, v7 = 0;
   asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-               : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3), "=r"(v4), "=r"(v5), "=r"(v6), "=r"(v7)
+               : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3), "=r"(v4), "=r"(v5), "=r"(v6), "+r"(v7)
                : "l"(p));
-  (void)v7;
+  idx = (int)(v6 | (v7 & 0u));  // (the padding word is part of the 256-bit load)
   x = __hiloint2double((int)v1, (int)v0);
   y = __hiloint2double((int)v3, (int)v2);
   z = __hiloint2double((int)v5, (int)v4);
-  idx = (int)v6;
 }
 
 // One thread per atom: exact nearest reference site.  Distances are evaluated in fp64 with the same
