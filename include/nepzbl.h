@@ -213,8 +213,9 @@ int64_t nep_zbl_launch_count(const nepzbl_handle *h);
  * Measurement aids (bench.py).  nep_zbl_profile(h, 1) makes every following evaluation / MD step
  * record CUDA events on the launch stream around each kernel group; nep_zbl_profile_read
  * synchronises, sums the elapsed milliseconds and span counts per group into ms[]/counts[]
- * (NEPZBL_PROFILE_SLOTS entries: 0 integrator first half (k_dt,k_kick_drift,k_flag), 1 list rebuild
- * chain, 2 k_radial, 3 k_angular_nn, 4 k_force, 5 k_zbl, 6 second half-kick) and resets them.
+ * (NEPZBL_PROFILE_SLOTS entries: 0 integrator first half (k_kick_drift incl. the step's book-keeping, and the
+ * thermostat's first half-step if set), 1 list rebuild chain, 2 k_radial, 3 k_angular_nn, 4 k_force (incl. the
+ * second half-kick in its epilogue), 5 k_zbl, 6 the thermostat's second half-step) and resets them.
  * nep_zbl_ffma_peak measures the FP32 FMA issue rate of the device (TFLOP/s, 2 flop per FMA) with a
  * register-only microbenchmark, the denominator of the "alu" roofline.
  */
