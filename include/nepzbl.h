@@ -86,8 +86,11 @@ typedef struct {
   int32_t cap_radial, cap_angular;     /* list capacities per atom (cap_radial <= 1024, cap_angular <= 64) */
 } nepzbl_params;
 
-/* Create a handle on CUDA device `device`; all work goes to `cuda_stream` (a cudaStream_t, may be
- * NULL for the default stream).  Uploads the parameters (S1 of the path needs none).  */
+/* Create a handle on CUDA device `device`; all work goes to `cuda_stream` (a cudaStream_t).  With NULL the library
+ * creates its own BLOCKING stream: it is ordered against work on the legacy default stream exactly as the default
+ * stream itself would be (so a caller that issues its own work there needs no extra synchronisation), but it can be
+ * captured, so MD steps are still replayed as a CUDA graph.  Uploads the parameters (S1 of the path needs none).
+ * Atom types must lie in [0, n_types); a type outside is reported as NEPZBL_E_INVALID_ARG by the call that reads it. */
 int nep_zbl_create(const nepzbl_params *params, int device, void *cuda_stream, nepzbl_handle **out);
 void nep_zbl_destroy(nepzbl_handle *h);
 const char *nep_zbl_last_error(const nepzbl_handle *h); /* h may be NULL: create-time errors */
@@ -147,6 +150,9 @@ int nep_zbl_get_descriptors(nepzbl_handle *h, float *q);
  * NEPZBL_GATHER_BLOCK=32|64 (also read at create) fixes the threads per block of the two gather kernels, which
  * the library otherwise picks from the grid size (a tuning aid; results do not depend on it).
  */
+/* An MD session ends with destroy, the next md_init, nep_zbl_set_workspace -- or ANY neighbor_build /
+ * nep_zbl_compute / nep_zbl_compute_host on the same handle (they overwrite the lists and the sorted order the session
+ * and its captured graph rely on); md_step then returns NEPZBL_E_STATE until md_init is called again. */
 int md_init(nepzbl_handle *h, int64_t n, double *pos_soa, double *vel_soa, const int32_t *types,
             const double box[9], const int32_t pbc[3]);
 int md_step(nepzbl_handle *h, double dt_max, double max_displacement, double *dt_used,
@@ -206,6 +212,17 @@ int wigner_seitz_set_reference(nepzbl_handle *h, int64_t n_sites, const double *
 int wigner_seitz_count(nepzbl_handle *h, int64_t n, const double *pos_soa, int32_t *nearest,
                        int32_t *occupancy, int64_t *n_vacancies, int64_t *n_interstitials);
 
+/* 1 when md_step / md_run replay the step as a captured CUDA graph, 0 when they issue plain stream launches
+ * (NEPZBL_NO_GRAPH=1, a failed capture -- nep_zbl_last_error then says why -- or no MD session). */
+int nep_zbl_uses_graph(const nepzbl_handle *h);
+
+/* Counts of the last evaluation / MD step (host outputs, any may be NULL): atoms with a neighbour inside the ZBL
+ * range (evaluated by the fp64 pair kernel, Eq. 2-4), and atoms whose angular network inputs |s_nu q_nu| exceeded the
+ * fp32 accuracy threshold and were re-evaluated in fp64 (none in a thermal crystal, the
+ * disordered core of a cascade; the environment variable NEPZBL_DENSE_THRESHOLD, read at create, overrides the
+ * threshold of 3, "off" disables the pass). */
+int nep_zbl_last_counts(nepzbl_handle *h, int64_t *n_zbl_atoms, int64_t *n_fp64_atoms);
+
 /* Number of kernel launches issued by this handle so far (for bench.py's gpu_launches). */
 int64_t nep_zbl_launch_count(const nepzbl_handle *h);
 
@@ -215,7 +232,7 @@ int64_t nep_zbl_launch_count(const nepzbl_handle *h);
  * synchronises, sums the elapsed milliseconds and span counts per group into ms[]/counts[]
  * (NEPZBL_PROFILE_SLOTS entries: 0 integrator first half (k_kick_drift incl. the step's book-keeping, and the
  * thermostat's first half-step if set), 1 list rebuild chain, 2 k_radial, 3 k_angular_nn, 4 k_force (incl. the
- * second half-kick in its epilogue), 5 k_zbl, 6 the thermostat's second half-step) and resets them.
+ * second half-kick in its epilogue), 5 k_zbl, 6 the thermostat's second half-step, 7 k_site_fp64) and resets them.
  * nep_zbl_ffma_peak measures the FP32 FMA issue rate of the device (TFLOP/s, 2 flop per FMA) with a
  * register-only microbenchmark, the denominator of the "alu" roofline.
  */

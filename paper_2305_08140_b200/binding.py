@@ -29,8 +29,8 @@ EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_d
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
            "md_run", "md_step_host", "md_energies", "md_get_forces", "md_get_counters",
            "md_set_thermostat", "md_get_thermostat", "md_set_thermostat_state", "wigner_seitz_set_reference", "wigner_seitz_count",
-           "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
-PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "spare"]
+           "nep_zbl_uses_graph", "nep_zbl_last_counts", "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
+PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "k_site_fp64"]
 
 
 class NepZblError(RuntimeError):
@@ -106,6 +106,10 @@ _lib.wigner_seitz_set_reference.argtypes = [_vp, _i64, _vp, C.POINTER(_dbl), C.P
 _lib.wigner_seitz_set_reference.restype = C.c_int
 _lib.wigner_seitz_count.argtypes = [_vp, _i64, _vp, _vp, _vp, C.POINTER(_i64), C.POINTER(_i64)]
 _lib.wigner_seitz_count.restype = C.c_int
+_lib.nep_zbl_uses_graph.argtypes = [_vp]
+_lib.nep_zbl_uses_graph.restype = C.c_int
+_lib.nep_zbl_last_counts.argtypes = [_vp, C.POINTER(_i64), C.POINTER(_i64)]
+_lib.nep_zbl_last_counts.restype = C.c_int
 _lib.nep_zbl_launch_count.argtypes = [_vp]
 _lib.nep_zbl_launch_count.restype = _i64
 _lib.nep_zbl_profile.argtypes = [_vp, C.c_int]
@@ -286,6 +290,14 @@ class NepZbl:
         nv = _i64(); ni = _i64()
         self._chk(_lib.wigner_seitz_count(self.h, n, _ptr(pos), _ptr(nearest), _ptr(occ), C.byref(nv), C.byref(ni)))
         return nearest, occ, (nv.value, ni.value)
+
+    def nep_zbl_uses_graph(self) -> bool:
+        return bool(_lib.nep_zbl_uses_graph(self.h))
+
+    def nep_zbl_last_counts(self):
+        a = _i64(); b = _i64()
+        self._chk(_lib.nep_zbl_last_counts(self.h, C.byref(a), C.byref(b)))
+        return a.value, b.value
 
     def nep_zbl_launch_count(self) -> int:
         return int(_lib.nep_zbl_launch_count(self.h))

@@ -41,6 +41,9 @@ struct Scalars {  // device-resident control block (one per handle)
   int nonfinite;
   int box_too_small;
   int zbl_count;
+  int dense_count;                      // atoms listed by k_angular_nn for the fp64 re-evaluation (site_fp64.cuh)
+  unsigned int ang_done;                // ticket counter of k_angular_nn's last-block book-keeping (graph IF node)
+  int bad_type;                         // an atom type outside [0, n_types) was seen (clamped; reported as INVALID_ARG)
   int n_rebuilds;
   long long n_steps;
   float disp_sum;                       // d_(1) + d_(2) of the current positions against the build (0 right after a build)
@@ -67,6 +70,16 @@ __host__ __device__ inline unsigned long long enc_double(double x) {
 __device__ inline double dec_double(unsigned long long k) {
   unsigned long long b = (k & 0x8000000000000000ull) ? (k & 0x7fffffffffffffffull) : ~k;
   return __longlong_as_double((long long)b);
+}
+
+// atom type of atom i, validated: a type outside [0, n_types) would index the per-type tables (masses, atomic
+// numbers, coefficient tables, records) out of bounds, so it is flagged (NEPZBL_E_INVALID_ARG) and replaced by 0
+__device__ __forceinline__ int checked_type(Scalars* sc, const int32_t* __restrict__ types, int i, int n_types) {
+  if (!types) return 0;
+  const int t = types[i];
+  if ((unsigned)t < (unsigned)n_types) return t;
+  sc->bad_type = 1;
+  return 0;
 }
 
 // fixed-point coordinate of x on one axis (wraps modulo 2^32 on periodic axes)

@@ -64,7 +64,8 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
                    const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
                    const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,
                    const float* __restrict__ q_radial, float* __restrict__ u_site,
-                   AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out) {
+                   AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out,
+                   const DenseArgs da) {
   using LY = SplitLayout<MS>;
   static_assert(MS::NT == 1, "the four-lane kernel is instantiated for one atom type");
   constexpr int KA = MS::KA, NR = MS::NR, KR = MS::KR;
@@ -195,6 +196,15 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
     for (int i = 0; i < SLP; ++i) {
       q[i] *= s_qs[sub * SLS + i];
       Fp[i] = 0.0f;
+    }
+    if (da.dense_list) {  // large angular inputs anywhere in the quad: list the atom for the fp64 pass (site_fp64.cuh)
+      float mx = 0.0f;
+#pragma unroll
+      for (int i = 0; i < SLP; ++i)
+        if (i < 4 * NSUB || i >= 4 * NSUB + RSUB) mx = fmaxf(mx, fabsf(q[i]));
+      const bool big = !(mx <= mt.dense_thr);
+      const unsigned bq = (__ballot_sync(0xffffffffu, big) >> qbase) & 0xFu;
+      if (bq && valid && sub == 0) da.dense_list[atomicAdd(&da.sc->dense_count, 1)] = s;
     }
     float U = 0.0f;
 #pragma unroll 1
@@ -363,4 +373,6 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       }
     }
   }
+  __syncthreads();
+  if (threadIdx.x == 0) dense_ticket(da);
 }

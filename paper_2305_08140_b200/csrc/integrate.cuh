@@ -43,6 +43,7 @@ __device__ __forceinline__ void step_flag(Scalars* sc, float skin, double* dt_tr
   sc->do_rebuild = r;
   sc->force_rebuild = 0;
   sc->zbl_count = 0;
+  sc->dense_count = 0;
   if (r) sc->n_rebuilds += 1;
 #if defined(__CUDA_ARCH__)
   if (use_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)cond_rebuild, (unsigned)r);
@@ -54,6 +55,7 @@ struct StepFlagArgs {  // passed by value to k_kick_drift, whose last block runs
   int trace_ring;
   unsigned long long cond_rebuild;
   int use_cond;
+  int n_types;
 };
 
 
@@ -199,7 +201,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
   if (i < n) {
     const double dt = step_dt(sc);
     const double sg = (group && group[i]) ? nh->scale : 1.0;  // first NHC(dt/2) of the step (k_nhc)
-    int t = types ? types[i] : 0;
+    int t = checked_type(sc, types, i, fa.n_types);
     double im = inv_mass[t];  // 1 / (m * 103.6426965): acceleration in A/fs^2 per eV/A
     unsigned int u[3];
 #pragma unroll

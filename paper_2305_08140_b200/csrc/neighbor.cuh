@@ -127,7 +127,7 @@ __global__ void k_zero_cells(const Scalars* sc, const BoxMap* bm, int* cell_coun
 
 // S1 for a rebuild: fixed-point compute copy (caller order) + cell histogram.
 __global__ void k_bin(Scalars* sc, const BoxMap* __restrict__ bm, int n,
-                      const double* __restrict__ pos, const int32_t* __restrict__ types,
+                      const double* __restrict__ pos, const int32_t* __restrict__ types, int n_types,
                       int4* __restrict__ xyzt_tmp, int* __restrict__ cell_of, int* cell_count) {
   if (!sc->do_rebuild) return;
   int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -144,7 +144,7 @@ __global__ void k_bin(Scalars* sc, const BoxMap* __restrict__ bm, int n,
   int cy = cell_of_u(uy, bm->ncv[1], bm->nc[1]);
   int cz = cell_of_u(uz, bm->ncv[2], bm->nc[2]);
   int c = (cz * bm->nc[1] + cy) * bm->nc[0] + cx;
-  xyzt_tmp[i] = make_int4((int)ux, (int)uy, (int)uz, types ? types[i] : 0);
+  xyzt_tmp[i] = make_int4((int)ux, (int)uy, (int)uz, checked_type(sc, types, i, n_types));
   cell_of[i] = c;
   atomicAdd(&cell_count[c], 1);
 }
@@ -451,7 +451,7 @@ __global__ void k_rev(const Scalars* sc, int n, int npad, const int* __restrict_
 // order of the current list) and track the displacement since the build.
 __global__ void __launch_bounds__(256)
 k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restrict__ pos,
-       const int32_t* __restrict__ types, const int* __restrict__ inv_perm, int4* __restrict__ xyzt,
+       const int32_t* __restrict__ types, int n_types, const int* __restrict__ inv_perm, int4* __restrict__ xyzt,
        const int4* __restrict__ xyzt_build) {
   __shared__ unsigned sh[64];
   int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -467,7 +467,7 @@ k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restri
     unsigned int uz = fix_coord(z, bm->lo[2], bm->inv_h[2]);
     int s = inv_perm[i];
     int4 b = xyzt_build[i];
-    xyzt[s] = make_int4((int)ux, (int)uy, (int)uz, types ? types[i] : 0);
+    xyzt[s] = make_int4((int)ux, (int)uy, (int)uz, checked_type(sc, types, i, n_types));
     float dx = (float)((int)ux - b.x) * bm->hf[0];
     float dy = (float)((int)uy - b.y) * bm->hf[1];
     float dz = (float)((int)uz - b.z) * bm->hf[2];
@@ -485,6 +485,7 @@ __global__ void k_flag(Scalars* sc, float skin) {
   sc->do_rebuild = r;
   sc->force_rebuild = 0;
   sc->zbl_count = 0;
+  sc->dense_count = 0;
   if (r) sc->n_rebuilds += 1;
 }
 

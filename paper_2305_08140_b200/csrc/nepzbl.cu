@@ -18,6 +18,7 @@
 #include "descriptor.cuh"
 #include "descriptor_split.cuh"
 #include "force.cuh"
+#include "site_fp64.cuh"
 #include "integrate.cuh"
 #include "wigner_seitz.cuh"
 
@@ -29,7 +30,7 @@ constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
-      nn_r, nn_a, shellq, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, md_force, md_energy,
+      nn_r, nn_a, shellq, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, dense_list, md_force, md_energy,
       partial, nhc_partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
@@ -45,7 +46,9 @@ struct nepzbl_handle {
   int D = 0, shape = -1;
   int device = 0;
   cudaStream_t stream = nullptr;
+  cudaStream_t own_stream = nullptr;  // created when the caller passes no stream (see nep_zbl_create)
   std::string err;
+  std::string graph_note;             // why MD steps are not replayed as a graph (empty: they are)
   long long launches = 0;
 
   // library-owned small device block
@@ -61,6 +64,10 @@ struct nepzbl_handle {
   double* h_esum = nullptr;   // pinned [2]
   std::vector<char> tables;   // ModelTables<MS> for the dispatched shape
   ZblParams zp{};
+  SiteModel site{};           // fp64 tables of k_site_fp64 (d_site holds them)
+  double* d_site = nullptr;
+  bool dense_on = true;       // NEPZBL_DENSE_THRESHOLD=off disables the fp64 re-evaluation (measurement aid)
+  cudaGraph_t building = nullptr;  // graph under construction (build_step_graph): enqueue_eval adds the fp64 IF node
   size_t smem_nn = 0;
   // threads per block of k_radial / k_force: one warp while the grid is only a few waves of resident threads (the
   // partly filled last wave costs one block's duration: 128 000 atoms 32: 78.3 us, 64: 80.5, 128: 83.1 for
@@ -185,6 +192,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.u_site = take(4 * npad);
   c.q_desc = take(4 * (size_t)D * npad);
   c.zbl_list = take(4 * npad);
+  c.dense_list = take(4 * npad);
   c.md_force = take(12 * npad);
   c.md_energy = take(8 * npad);
   c.partial = take(16 * 1024);
@@ -246,6 +254,14 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   t.inv_shell_w = p->skin > 0 ? (float)(8.0 / p->skin) : 0.0f;
   t.b1 = (float)p->b1;
   t.n_neurons = p->n_neurons;
+  // fp64 re-evaluation threshold on the angular network inputs |s q| (site_fp64.cuh):
+  // a 300 K crystal stays below 0.8, so the default lists no thermal atom; NEPZBL_DENSE_THRESHOLD overrides
+  // (a number, or "off")
+  t.dense_thr = 3.0f;
+  if (const char* dt = getenv("NEPZBL_DENSE_THRESHOLD")) {
+    if (!strcmp(dt, "off")) h->dense_on = false;
+    else if (atof(dt) > 0.0) t.dense_thr = (float)atof(dt);
+  }
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
   if (kSplit<MS>) {
@@ -325,12 +341,39 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
   }
 }
 
+// fp64 tables of k_site_fp64: folded Chebyshev coefficients, q_scaler, network weights (one device buffer)
+template <class MS>
+std::vector<double> build_site_tables(const nepzbl_params* p, SiteModel* sm, size_t off[6]) {
+  sm->NT = MS::NT; sm->NR = MS::NR; sm->KR = MS::KR; sm->NA = MS::NA; sm->KA = MS::KA; sm->B4 = MS::B4 ? 1 : 0;
+  sm->D = MS::D; sm->n_neurons = p->n_neurons; sm->fprec = MS::FPREC ? 1 : 0;
+  sm->b1 = p->b1; sm->rcA = p->rc_angular;
+  const int npr = MS::NT * MS::NT;
+  std::vector<double> v;
+  off[0] = v.size();
+  for (int pr = 0; pr < npr; ++pr)
+    for (int nq = 0; nq < MS::NA; ++nq)
+      for (int k = 0; k < MS::KA; ++k) v.push_back(folded(p->c_angular + (size_t)pr * MS::NA * MS::KA, MS::KA, nq, k));
+  off[1] = v.size();
+  for (int pr = 0; pr < npr; ++pr)
+    for (int nq = 0; nq < MS::NR; ++nq)
+      for (int k = 0; k < MS::KR; ++k) v.push_back(folded(p->c_radial + (size_t)pr * MS::NR * MS::KR, MS::KR, nq, k));
+  off[2] = v.size();
+  for (int d = 0; d < MS::D; ++d) v.push_back(p->q_scaler[d]);
+  off[3] = v.size();
+  for (size_t k = 0; k < (size_t)p->n_neurons * MS::D; ++k) v.push_back(p->w0[k]);
+  off[4] = v.size();
+  for (int m = 0; m < p->n_neurons; ++m) v.push_back(p->b0[m]);
+  off[5] = v.size();
+  for (int m = 0; m < p->n_neurons; ++m) v.push_back(p->w1[m]);
+  return v;
+}
+
 inline int blocks(long long n, int b) { return (int)((n + b - 1) / b); }
 // k_zbl walks the flagged atoms grid-stride: a handful in a thermal crystal (the graph skips the node when
 // there is none), thousands in a cascade core, so the grid covers the device
 inline int zbl_grid(const nepzbl_handle* h) { return std::max(1, std::min(blocks(h->n, 64), 8 * h->n_sm)); }
 
-enum { PK_INTEGRATE_A = 0, PK_REBUILD, PK_RADIAL, PK_ANGULAR_NN, PK_FORCE, PK_ZBL, PK_KICK, PK_COUNT };
+enum { PK_INTEGRATE_A = 0, PK_REBUILD, PK_RADIAL, PK_ANGULAR_NN, PK_FORCE, PK_ZBL, PK_KICK, PK_SITE64, PK_COUNT };
 
 cudaEvent_t prof_event(nepzbl_handle* h) {
   if (h->ev_used == h->ev_pool.size()) {
@@ -377,7 +420,7 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
   k_boxmap<<<1, 1, 0, st>>>(h->d_sc, h->d_bm, bh);
   k_zero_cells<<<blocks(c.ncell_cap + 1, 256), 256, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count),
                                                            h->at<int>(c.cell_fill), c.ncell_cap);
-  k_bin<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, pos, types, h->at<int4>(c.xyzt_tmp),
+  k_bin<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, pos, types, h->p.n_types, h->at<int4>(c.xyzt_tmp),
                                        h->at<int>(c.cell_of), h->at<int>(c.cell_count));
   k_scan<<<1, 1024, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count), h->at<int>(c.cell_start));
   k_place<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->at<int>(c.cell_of), h->at<int>(c.cell_start),
@@ -397,6 +440,37 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
   return nk + 9;
 }
 
+// Stream capture helper: add an IF node (condition `handle`, set on the device) behind whatever `st` has captured so
+// far into graph `g`, make the following captured work depend on it, and return the node's body graph.
+bool graph_add_if(cudaStream_t st, cudaGraph_t g, cudaGraphConditionalHandle handle, cudaGraph_t* body) {
+  cudaStreamCaptureStatus status;
+  const cudaGraphNode_t* deps = nullptr;
+  size_t ndeps = 0;
+  cudaGraph_t cg = nullptr;
+  if (cudaStreamGetCaptureInfo(st, &status, nullptr, &cg, &deps, &ndeps) != cudaSuccess) return false;
+  cudaGraphNodeParams np = {};
+  np.type = cudaGraphNodeTypeConditional;
+  np.conditional.handle = handle;
+  np.conditional.type = cudaGraphCondTypeIf;
+  np.conditional.size = 1;
+  cudaGraphNode_t node;
+  if (cudaGraphAddNode(&node, g, deps, ndeps, &np) != cudaSuccess) return false;
+  *body = np.conditional.phGraph_out[0];
+  return cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies) == cudaSuccess;
+}
+
+// fp64 re-evaluation of the atoms k_angular_nn listed (site_fp64.cuh); grid-stride over the list
+void launch_site_fp64(nepzbl_handle* h, const double* pos, bool want_q, cudaStream_t st) {
+  const Carve& c = h->cv;
+  const int n = (int)h->n;
+  const int grid = std::max(1, std::min(blocks(n, SITE64_WARPS), 8 * h->n_sm));
+  const size_t smem = sizeof(double) * SITE64_WARPS * (2 * (size_t)h->site.D + h->site.n_neurons);
+  k_site_fp64<<<grid, 32 * SITE64_WARPS, smem, st>>>(
+      h->d_sc, h->d_bm, h->site, h->at<int>(c.dense_list), n, c.npad, h->at<int4>(c.xyzt), h->at<int>(c.nl_r),
+      h->at<unsigned long long>(c.amask), h->at<int>(c.perm), pos, h->at<float>(c.q_radial), h->at<float>(c.u_site),
+      h->at<AtomRec>(c.dk), h->at<float4>(c.pforce), want_q ? h->at<float>(c.q_desc) : nullptr);
+}
+
 // S3-S7 (+S5): outputs in the caller's order; any of energy/force/virial may be null.
 template <class MS>
 void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* force, float* virial,
@@ -404,6 +478,11 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   const Carve& c = h->cv;
   const int n = (int)h->n, npad = c.npad;
   cudaStream_t st = h->stream;
+  // in a graph under construction the fp64 pass sits in an IF node that k_angular_nn's last block opens
+  cudaGraphConditionalHandle h_dense = 0;
+  const bool dense_if = h->dense_on && h->building &&
+                        cudaGraphConditionalHandleCreate(&h_dense, h->building, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+  const DenseArgs da{h->d_sc, h->dense_on ? h->at<int>(c.dense_list) : nullptr, (unsigned long long)h_dense, dense_if ? 1 : 0};
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
   const int gb = h->gather_block ? h->gather_block : ((long long)n * RADIAL_LANES < 8ll * 1024 * h->n_sm ? 32 : 64);
   prof_mark(h, PK_RADIAL);
@@ -418,12 +497,28 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
     k_angular_nn_split<MS><<<std::min(blocks((long long)n * SPLIT_LANES, SPLIT_THREADS), h->ang_grid), SPLIT_THREADS, h->smem_nn, st>>>(
         n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
         h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
-        want_q ? h->at<float>(c.q_desc) : nullptr);
+        want_q ? h->at<float>(c.q_desc) : nullptr, da);
   else
     k_angular_nn<MS><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
         n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
         h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
-        want_q ? h->at<float>(c.q_desc) : nullptr);
+        want_q ? h->at<float>(c.q_desc) : nullptr, da);
+  if (h->dense_on) {
+    prof_mark(h, PK_SITE64);
+    if (dense_if) {
+      cudaGraph_t body = nullptr;
+      if (graph_add_if(st, h->building, h_dense, &body) &&
+          cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+        launch_site_fp64(h, pos, want_q, h->cap_stream);
+        if (cudaStreamEndCapture(h->cap_stream, nullptr) != cudaSuccess) h->building = nullptr;  // reported by build_step_graph
+      } else {
+        h->building = nullptr;
+      }
+    } else {
+      launch_site_fp64(h, pos, want_q, st);
+      h->launches++;
+    }
+  }
   prof_mark(h, PK_FORCE);
   auto launch_force = [&](auto vir, auto blk) {
     constexpr bool VIR = decltype(vir)::value;
@@ -473,10 +568,11 @@ int read_scalars(nepzbl_handle* h) {
 }
 
 __global__ void k_clear_errors(Scalars* sc);
+void destroy_step_graph(nepzbl_handle* h);
 
 int check_device_flags(nepzbl_handle* h) {
   const Scalars& s = *h->h_sc;
-  if (s.nonfinite || s.box_too_small || s.overflow_radial > h->p.cap_radial ||
+  if (s.nonfinite || s.box_too_small || s.bad_type || s.overflow_radial > h->p.cap_radial ||
       s.overflow_angular > h->p.cap_angular) {  // errors are reported once, then cleared
     k_clear_errors<<<1, 1, 0, h->stream>>>(h->d_sc);
     h->launches++;
@@ -484,6 +580,10 @@ int check_device_flags(nepzbl_handle* h) {
   if (s.nonfinite) {
     h->have_list = false;
     return fail(h, NEPZBL_E_NONFINITE, "NaN/Inf in positions");
+  }
+  if (s.bad_type) {
+    h->have_list = false;
+    return fail(h, NEPZBL_E_INVALID_ARG, "an atom type is outside [0, n_types = %d)", h->p.n_types);
   }
   if (s.box_too_small) {
     h->have_list = false;
@@ -522,6 +622,13 @@ int set_system(nepzbl_handle* h, long long n, const double box[9], const int32_t
   return NEPZBL_OK;
 }
 
+void destroy_step_graph(nepzbl_handle* h) {
+  if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
+  if (h->step_graph) cudaGraphDestroy(h->step_graph);
+  h->step_exec = nullptr;
+  h->step_graph = nullptr;
+}
+
 __global__ void k_set_force_rebuild(Scalars* sc) { sc->force_rebuild = 1; }
 
 // FP32 FMA issue-rate microbenchmark: 16 independent register chains per thread (bench.py roofline peak)
@@ -541,6 +648,7 @@ __global__ void __launch_bounds__(512) k_ffma_peak(int iters, float m, float* si
 }
 __global__ void k_clear_errors(Scalars* sc) {
   sc->nonfinite = 0;
+  sc->bad_type = 0;
   sc->box_too_small = 0;
   sc->overflow_radial = 0;
   sc->overflow_angular = 0;
@@ -548,7 +656,13 @@ __global__ void k_clear_errors(Scalars* sc) {
 
 int eval_common(nepzbl_handle* h, long long n, const double* pos, const int32_t* types,
                 const double box[9], const int32_t pbc[3], double* energy, float* force, float* virial,
-                bool force_rebuild, bool want_q, bool do_eval) {
+                bool force_rebuild, bool want_q, bool do_eval, bool from_md = false) {
+  // A plain evaluation or list build on a handle with an MD session overwrites the lists, the sorted order and the
+  // system size the session (and its captured graph) rely on: the session ends here, md_init starts a new one.
+  if (!from_md && h->md_ready) {
+    h->md_ready = false;
+    destroy_step_graph(h);
+  }
   bool changed = false;
   int rc = set_system(h, n, box, pbc, &changed);
   if (rc) return rc;
@@ -559,7 +673,7 @@ int eval_common(nepzbl_handle* h, long long n, const double* pos, const int32_t*
   if (changed || force_rebuild) {
     k_set_force_rebuild<<<1, 1, 0, h->stream>>>(h->d_sc);
   } else {
-    k_prep<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, h->d_bm, (int)n, pos, types,
+    k_prep<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, h->d_bm, (int)n, pos, types, h->p.n_types,
                                                   h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                                   h->at<int4>(c.xyzt_build));
   }
@@ -621,6 +735,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   h->device = device;
   h->stream = (cudaStream_t)cuda_stream;
   if (const char* ng = getenv("NEPZBL_NO_GRAPH")) h->use_graph = !(ng[0] == '1');  // see nepzbl.h (md_step)
+  if (!h->use_graph) h->graph_note = "NEPZBL_NO_GRAPH=1";
   if (const char* gb = getenv("NEPZBL_GATHER_BLOCK")) {
     int v = atoi(gb);
     if (v == 32 || v == 64) h->gather_block = v;
@@ -632,6 +747,9 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     nnw = build_nnw<MS>(p);
     h->D = MS::D;
   });
+  std::vector<double> site_tab;
+  size_t site_off[6] = {0, 0, 0, 0, 0, 0};
+  with_shape(shape, [&](auto ms) { site_tab = build_site_tables<decltype(ms)>(p, &h->site, site_off); });
   ZblParams& z = h->zp;
   memset(&z, 0, sizeof z);
   z.r_inner = p->zbl_r_inner; z.r_outer = p->zbl_r_outer; z.n_terms = p->zbl_n_terms;
@@ -652,6 +770,13 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   };
   cudaError_t ce;
   if ((ce = cudaSetDevice(device)) != cudaSuccess) return die("cudaSetDevice", ce);
+  if (!h->stream) {
+    // No stream given: the library makes its own BLOCKING stream.  It orders itself with the legacy default stream
+    // (where a caller that passes NULL issues its own work) exactly as the default stream would, but -- unlike the
+    // default stream -- it can be captured, so MD steps are replayed as a CUDA graph for such callers too.
+    if ((ce = cudaStreamCreateWithFlags(&h->own_stream, cudaStreamDefault)) != cudaSuccess) return die("cudaStreamCreate", ce);
+    h->stream = h->own_stream;
+  }
   if ((ce = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) return die("cudaDeviceGetAttribute", ce);
   {  // k_angular_nn: opt in to its dynamic shared memory and size the persistent grid to the resident blocks
     const void* fn = nullptr;
@@ -672,6 +797,9 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   if ((ce = cudaMalloc(&h->d_sc, sizeof(Scalars))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_bm, sizeof(BoxMap))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_nnw, nnw.size() * sizeof(float))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_site, site_tab.size() * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
+  h->site.ctA = h->d_site + site_off[0]; h->site.ctR = h->d_site + site_off[1]; h->site.qs = h->d_site + site_off[2];
+  h->site.w0 = h->d_site + site_off[3]; h->site.b0 = h->d_site + site_off[4]; h->site.w1 = h->d_site + site_off[5];
   if ((ce = cudaMalloc(&h->d_mass, 8 * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_inv_mass, 8 * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_trace, kTraceRing * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
@@ -690,6 +818,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   if ((ce = cudaMemsetAsync(h->d_sc, 0, sizeof(Scalars), h->stream)) != cudaSuccess) return die("cudaMemset", ce);
   if ((ce = cudaMemsetAsync(h->d_bm, 0, sizeof(BoxMap), h->stream)) != cudaSuccess) return die("cudaMemset", ce);
   if ((ce = cudaMemcpyAsync(h->d_nnw, nnw.data(), nnw.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
+  if ((ce = cudaMemcpyAsync(h->d_site, site_tab.data(), site_tab.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
   if ((ce = cudaMemcpyAsync(h->d_mass, mass, sizeof mass, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
   if ((ce = cudaMemcpyAsync(h->d_inv_mass, inv_mass, sizeof inv_mass, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
   if ((ce = cudaStreamSynchronize(h->stream)) != cudaSuccess) return die("cudaStreamSynchronize", ce);
@@ -711,7 +840,7 @@ void nep_zbl_destroy(nepzbl_handle* h) {
   ws_free(h);
   cudaFree(h->ws_ref.out);
   cudaFreeHost(h->ws_ref.h_out);
-  cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
+  cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_site); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
   cudaFree(h->d_trace); cudaFree(h->d_esum); cudaFree(h->d_nhc);
   cudaFreeHost(h->h_nhc);
   cudaFreeHost(h->h_sc); cudaFreeHost(h->h_trace); cudaFreeHost(h->h_esum);
@@ -720,6 +849,7 @@ void nep_zbl_destroy(nepzbl_handle* h) {
   if (h->step_graph) cudaGraphDestroy(h->step_graph);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+  if (h->own_stream) cudaStreamDestroy(h->own_stream);
   if (h->ev_drift) cudaEventDestroy(h->ev_drift);
   delete h;
 }
@@ -839,14 +969,17 @@ int md_init(nepzbl_handle* h, int64_t n, double* pos, double* vel, const int32_t
   h->nhc_on = false;
   h->md_group = nullptr;
   rc = eval_common(h, n, pos, types, box, pbc, h->at<double>(c.md_energy), h->at<float>(c.md_force),
-                   nullptr, true, false, true);
+                   nullptr, true, false, true, true);
   if (rc) return rc;
   k_kick<<<blocks(n, 256), 256, 0, h->stream>>>(h->d_sc, (int)n, vel, h->at<float>(c.md_force), types,
                                                 h->d_inv_mass, 0, 1);
   h->launches++;
   CU(cudaStreamSynchronize(h->stream));
   CU(cudaGetLastError());
-  if (h->use_graph && !build_step_graph(h)) h->use_graph = false;  // falls back to plain stream launches
+  if (h->use_graph && !build_step_graph(h)) {  // falls back to plain stream launches; nep_zbl_uses_graph tells
+    h->use_graph = false;
+    h->graph_note = "CUDA graph capture of the MD step failed; steps are issued as plain stream launches";
+  }
   h->md_ready = true;
   return NEPZBL_OK;
 }
@@ -880,7 +1013,7 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
                                               h->d_nhc,
-                                              StepFlagArgs{skin, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0});
+                                              StepFlagArgs{skin, trace ? h->d_trace : nullptr, kTraceRing, 0ull, 0, h->p.n_types});
   cudaEventRecord(h->ev_drift, st);
   h->launches += 1;
   prof_mark(h, PK_REBUILD);
@@ -893,12 +1026,6 @@ static void enqueue_md_step_stream(nepzbl_handle* h, bool trace) {
   prof_mark(h, -1);
 }
 
-static void destroy_step_graph(nepzbl_handle* h) {
-  if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
-  if (h->step_graph) cudaGraphDestroy(h->step_graph);
-  h->step_exec = nullptr;
-  h->step_graph = nullptr;
-}
 
 // Capture one MD step into a CUDA graph:
 //   k_kick_drift (its last block: dt, rebuild decision) -> IF(rebuild){S2 chain} -> k_radial -> k_angular_nn
@@ -945,7 +1072,7 @@ static bool build_step_graph(nepzbl_handle* h) {
                                               h->at<int>(c.inv_perm), h->at<int4>(c.xyzt),
                                               h->at<int4>(c.xyzt_build), h->nhc_on ? h->md_group : nullptr,
                                               h->d_nhc,
-                                              StepFlagArgs{skin, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1});
+                                              StepFlagArgs{skin, h->d_trace, kTraceRing, (unsigned long long)h_reb, 1, h->p.n_types});
   ok = ok && cudaEventRecordWithFlags(h->ev_drift, st, cudaEventRecordExternal) == cudaSuccess;
   nk += 1;
   cudaGraph_t body = nullptr;
@@ -960,7 +1087,10 @@ static bool build_step_graph(nepzbl_handle* h) {
   if (ok) {
     const KickArgs ka{h->d_sc, h->md_vel, h->d_inv_mass, h->nhc_on ? 0 : 1, (unsigned long long)h_zbl,
                       h->p.zbl_enabled ? 1 : 0};
+    h->building = g;  // enqueue_eval puts k_site_fp64 into an IF node of this graph
     enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false, false, ka);
+    ok = h->building == g;
+    h->building = nullptr;
     nk += 3;
     if (h->p.zbl_enabled) {
       ok = add_if(h_zbl, &body);
@@ -1031,6 +1161,7 @@ static int md_step_impl(nepzbl_handle* h, double dt_max, double max_displacement
   if (rebuilt) *rebuilt = h->h_sc->do_rebuild;
   if (h->h_sc->do_rebuild && h->use_graph && !h->prof && h->step_exec) h->launches += h->graph_rebuild_kernels;
   if (h->h_sc->zbl_count > 0 && h->use_graph && !h->prof && h->step_exec) h->launches += 1;
+  if (h->h_sc->dense_count > 0 && h->use_graph && !h->prof && h->step_exec) h->launches += 1;
   rc = check_device_flags(h);
   if (rc) h->md_ready = false;
   return rc;
@@ -1113,7 +1244,10 @@ int md_set_thermostat(nepzbl_handle* h, const uint8_t* group, double temperature
     h->md_group = group;
     h->nhc_on = true;
   }
-  if (h->use_graph && !build_step_graph(h)) h->use_graph = false;
+  if (h->use_graph && !build_step_graph(h)) {
+    h->use_graph = false;
+    h->graph_note = "CUDA graph capture of the thermostatted MD step failed; steps are issued as plain stream launches";
+  }
   return NEPZBL_OK;
 }
 
@@ -1311,6 +1445,20 @@ int md_get_counters(nepzbl_handle* h, int64_t* n_steps, int64_t* n_rebuilds, int
   if (n_steps) *n_steps = h->h_sc->n_steps;
   if (n_rebuilds) *n_rebuilds = h->h_sc->n_rebuilds;
   if (n_zbl_atoms) *n_zbl_atoms = h->h_sc->zbl_count;
+  return NEPZBL_OK;
+}
+
+int nep_zbl_uses_graph(const nepzbl_handle* h) {
+  return h && h->md_ready && h->use_graph && h->step_exec ? 1 : 0;
+}
+
+int nep_zbl_last_counts(nepzbl_handle* h, int64_t* n_zbl_atoms, int64_t* n_fp64_atoms) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->have_list) return fail(h, NEPZBL_E_STATE, "no evaluation has been made");
+  int rc = read_scalars(h);
+  if (rc) return rc;
+  if (n_zbl_atoms) *n_zbl_atoms = h->h_sc->zbl_count;
+  if (n_fp64_atoms) *n_fp64_atoms = h->h_sc->dense_count;
   return NEPZBL_OK;
 }
 

@@ -135,6 +135,55 @@ def test_state_errors(nb):
     assert ei.value.code == -9
 
 
+def test_graph_is_active_without_a_caller_stream(nb):
+    # a handle created with no stream runs on the library's own (capturable) stream: the step is a CUDA graph
+    w = wl.thermal_bulk(5, seed=6, sigma_pos=0.03)
+    g, pos, vel = _md(nb, w)
+    assert g.nep_zbl_uses_graph()
+    s = torch.cuda.Stream()
+    g2 = nb.NepZbl(w.model, w.n, stream=s)
+    p2 = torch.from_numpy(w.pos.copy()).cuda(); v2 = torch.from_numpy(w.vel.copy()).cuda()
+    torch.cuda.synchronize()
+    g2.md_init(p2, v2, torch.from_numpy(w.types).cuda(), w.box, w.pbc)
+    assert g2.nep_zbl_uses_graph()
+    g.md_run(10, 1.0, 0.01); g2.md_run(10, 1.0, 0.01)
+    torch.cuda.synchronize()
+    assert torch.equal(pos, p2) and torch.equal(vel, v2)
+
+
+def test_an_evaluation_ends_the_md_session(nb):
+    # nep_zbl_compute / neighbor_build on a handle with an MD session overwrite the lists the session (and its
+    # captured graph) rely on: md_step must refuse until md_init is called again (nepzbl.h)
+    w = wl.thermal_bulk(5, seed=6, sigma_pos=0.03)
+    g, pos, vel = _md(nb, w)
+    g.md_step(1.0, 0.01)
+    w2 = wl.thermal_bulk(4, seed=7, sigma_pos=0.03)          # another size: stale launch geometry would be fatal
+    g.compute(w2.pos, w2.types, w2.box, w2.pbc)
+    assert not g.nep_zbl_uses_graph()
+    with pytest.raises(nb.NepZblError) as ei:
+        g.md_step(1.0, 0.01)
+    assert ei.value.code == -9
+    g.md_init(pos, vel, torch.from_numpy(w.types).cuda(), w.box, w.pbc)
+    g.md_step(1.0, 0.01)
+
+
+def test_atom_types_are_validated(nb):
+    w = wl.thermal_bulk(5, seed=6, sigma_pos=0.03)
+    bad = w.types.copy(); bad[7] = 3
+    g = nb.NepZbl(w.model, w.n)
+    with pytest.raises(nb.NepZblError) as ei:
+        g.compute(w.pos, bad, w.box, w.pbc)
+    assert ei.value.code == -1 and "type" in str(ei.value)
+    g.compute(w.pos, w.types, w.box, w.pbc)                   # the handle is still usable
+    pos = torch.from_numpy(w.pos.copy()).cuda(); vel = torch.from_numpy(w.vel.copy()).cuda()
+    types = torch.from_numpy(w.types).cuda()
+    g.md_init(pos, vel, types, w.box, w.pbc)
+    types[11] = -2                                            # the caller owns the array and breaks it mid-run
+    with pytest.raises(nb.NepZblError) as ei:
+        g.md_step(1.0, 0.01)
+    assert ei.value.code == -1
+
+
 def test_overflow_inside_a_long_md_run_is_reported_not_fatal(nb):
     # a list-capacity overflow in the middle of an md_run chunk: the remaining steps of the chunk must stay
     # memory-safe (the reverse index of a dropped list is a sentinel, not a row) and the call must report it

@@ -100,6 +100,25 @@ def test_md_run_graph_equals_md_step_and_switch_off(nb):
     assert (p1 - p3).abs().max().item() < 1e-8 and (v1 - v3).abs().max().item() < 1e-9
 
 
+def test_graph_path_is_active_and_equals_stream_launches_with_thermostat(nb, monkeypatch):
+    """The captured-graph step (what bench.py and every DESIGN.md number measure) against the same kernels as plain
+    stream launches (NEPZBL_NO_GRAPH=1), bit for bit, on a thermostatted cascade cell where both IF nodes (list
+    rebuild, ZBL) and the fp64 pass fire."""
+    w = wl.bulk_cascade(8, 800.0, seed=15, n_steps=0, name="nhc_graph")
+    group = wl.border_group(w.pos, w.box, w.pbc, thickness=wl.A0_CONFIG)
+    out = []
+    for no_graph in ("0", "1"):
+        monkeypatch.setenv("NEPZBL_NO_GRAPH", no_graph)
+        g, pos, vel = _md(nb, w, group, 300.0, 50.0, 4)
+        assert g.nep_zbl_uses_graph() == (no_graph == "0")
+        g.md_run(150, 1.0, 0.015)
+        steps, rebuilds, _ = g.md_get_counters()
+        out.append((pos.cpu().numpy().copy(), vel.cpu().numpy().copy(), g.md_get_thermostat()[1].copy(), rebuilds))
+    assert out[0][3] == out[1][3] and out[0][3] >= 2
+    for a, b in zip(out[0][:3], out[1][:3]):
+        assert a.tobytes() == b.tobytes()
+
+
 def test_border_layer_of_a_cascade_cell(nb):
     # 24^3 cells (27 648 atoms), 3 a0 border layer (P:77), 2 keV PKA at the centre, adaptive step: the
     # group temperature reported by the library is the group's, and the conserved quantity of ref. [32] holds
