@@ -4,7 +4,12 @@
 
 One "step" = one velocity-Verlet step of the whole hot path (S1-S8 of DESIGN.md: integrator half
 kicks + drift, list rebuild when the skin is exhausted, radial/angular descriptors, network,
-force back-pass, ZBL) on BASELINE.json configs[1]: 128 000-atom bcc W, 300 K, dt = 1 fs, skin 1 A.
+force back-pass, ZBL).  BASELINE.json's metric names no config, so the default workload is the largest
+single-GPU configuration, configs[3] ("config4"): the 8 192 000-atom bulk cascade (160^3 bcc cells, 300 K,
+100 keV PKA, adaptive time step); the other configs are timed in the same run and reported under `per_config`.
+The cascade configs rebuild their list once per ~60 steps; so that S2 is inside a timed region of any length, ONE
+rebuild is requested at the start of every cascade config's timed steps (config.forced_rebuilds) -- at --steps 20
+that over-represents the rebuild (conservative).
 Prints ONE JSON line (rank 0).  Keys: see DESIGN.md "Measurement".
 
   value      K steps enqueued back to back by md_run (no host round trip), state resident in HBM,
@@ -68,12 +73,31 @@ FP32_LANES_PER_SM = 128
 # Wigner-Seitz count, compulsory HBM bytes per atom (one site per atom): position 24 + nearest 4 + occupancy
 # read-modify-write 8 + count read 4 + cell-sorted site record 28 (the 27-cell scan re-reads sites from L1/L2)
 WS_BYTES_PER_ATOM = 68.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on config2 (128 000 atoms) from the committed
-# `ncu --set full` capture (NCU_TRAFFIC_SOURCE); reported as roofline.traffic for that workload only.
-NCU_TRAFFIC_BYTES = {"config2": {"k_radial": 36.140544e6, "k_angular_nn": 58.577408e6,
-                                 "k_force": 96.876288e6},
-                     "paper": {"k_angular_nn": 55.964928e6 + 18.282496e6}}
-NCU_TRAFFIC_SOURCE = "profiles/r1e_ncu_full.md"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture named in
+# "source", valid for the kernel sources whose hash is "csrc_sha16" (csrc_sha16() below): when the kernels have
+# changed since the capture, roofline.traffic is null and roofline.traffic_note says so.
+NCU_TRAFFIC = {"csrc_sha16": "unset", "source": "profiles/r2_ncu_full.md", "bytes": {}}
+
+
+def csrc_sha16() -> str:
+    """Hash of everything the kernels are built from (csrc/*.cu, *.cuh and the C header)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2305_08140_b200", "csrc")
+    files = sorted(os.path.join(d, f) for f in os.listdir(d) if f.endswith((".cu", ".cuh")))
+    for f in files + [os.path.join(ROOT, "include", "nepzbl.h")]:
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload: str, kernel: str, cells):
+    if cells is not None:
+        return None, "non-standard cell count"
+    if NCU_TRAFFIC["csrc_sha16"] != csrc_sha16():
+        return None, f"stale: kernels changed since the capture in {NCU_TRAFFIC['source']}"
+    v = NCU_TRAFFIC["bytes"].get(workload, {}).get(kernel)
+    return v, (NCU_TRAFFIC["source"] if v is not None else "no capture for this workload")
 
 
 def _dist_env():
@@ -157,40 +181,71 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------------ oracle legs
 
+CASCADE = {"config3": 1.0e4, "config4": 1.0e5, "config5": 1.0e5}     # PKA energies (eV) of the cascade configs
+
+
+def sample_workload(name: str, cells: int):
+    """The workload's own recipe at a smaller cell count (for the oracle legs: its cost is linear in N)."""
+    from paper_2305_08140_b200 import workloads as wl
+    if name in ("config3", "config4"):
+        return wl.bulk_cascade(cells, CASCADE[name], seed=3 if name == "config3" else 4, n_steps=0, name=name)
+    if name == "config5":
+        return wl.config5(seed=5, cells=(cells, cells, max(4, cells * 5 // 8)))
+    if name == "paper":
+        return wl.paper_bulk(cells, seed=12)
+    if name == "alloy":
+        w = wl.config2(seed=2, cells=cells, model=wl.alloy_model(spread=0.05, stream=13))
+        w.types = wl.random_types(w.n, 2)
+        return w
+    return wl.config2(seed=2, cells=cells)
+
+
 def oracle_md_rate(workload_name: str, n_steps: int | None, warmup: int, budget_s: float):
-    """Time the fp64 oracle's own MD loop (oracle.md_run, as it stands) on a bounded sample of the
-    workload: the same recipe (bcc W, 300 K, same model, dt = 1 fs).  With n_steps = None (the
-    cpu_baseline leg) the sample is the first steps of the FULL 40^3-cell system, as many as fit
-    `budget_s`; with n_steps given (the reference arm) it is the largest cell count from
-    (6, 8, 10, 12, 16, 24, 40)^3 for which (warmup + n_steps) steps fit `budget_s`.  Cost is linear in
-    N, so atom-steps/s carries over."""
+    """Time the fp64 oracle's own MD loop (oracle.md_run, as it stands) on a bounded sample of the workload: the
+    same recipe (lattice, temperature, PKA, model, dt rule) at the largest cell count from (6 ... 40)^3 whose run
+    fits `budget_s`.  n_steps = None (the cpu_baseline leg): as many steps as fit the budget at 40^3 cells (fewer
+    cells if not even 3 steps fit).  Cost is linear in N, so atom-steps/s carries over."""
     import oracle
     from paper_2305_08140_b200 import workloads as wl
-    w = wl.thermal_bulk(10, seed=2)
+    w = wl.thermal_bulk(10, seed=2, model=sample_workload(workload_name, 6).model)
     P = oracle.Params(w.model)
     oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, 1, 1.0, np.inf)      # loads the library, spins up OpenMP
     t = time.perf_counter()
     oracle.md_run(P, w.pos, w.vel, w.types, w.box, w.pbc, 2, 1.0, np.inf)
     rate = 3 * w.n / (time.perf_counter() - t)                                 # atom-evaluations/s (3 evaluations)
+    fits = lambda c, k: (warmup + k + 2) * 2 * c ** 3 / rate <= budget_s
+    cells = 6
+    for c in (8, 10, 12, 16, 24, 40):
+        if fits(c, 3 if n_steps is None else n_steps):
+            cells = c
     if n_steps is None:
-        cells = 40
         n_steps = int(max(3, min(200, budget_s * rate / (2 * cells ** 3) - 1)))
-    else:
-        cells = 6
-        for c in (8, 10, 12, 16, 24, 40):
-            if (warmup + n_steps + 2) * 2 * c ** 3 / rate <= budget_s:
-                cells = c
-    w = wl.thermal_bulk(cells, seed=2)
+    w = sample_workload(workload_name, cells)
     pos, vel = w.pos, w.vel
     if warmup > 0:
-        pos, vel, *_ = oracle.md_run(P, pos, vel, w.types, w.box, w.pbc, warmup, 1.0, np.inf)
+        pos, vel, *_ = oracle.md_run(P, pos, vel, w.types, w.box, w.pbc, warmup, w.dt_max, w.max_displacement)
     t = time.perf_counter()
-    oracle.md_run(P, pos, vel, w.types, w.box, w.pbc, n_steps, 1.0, np.inf)
+    oracle.md_run(P, pos, vel, w.types, w.box, w.pbc, n_steps, w.dt_max, w.max_displacement)
     dt = time.perf_counter() - t
     # md_run evaluates forces once before the loop: n_steps + 1 evaluations for n_steps steps
     return {"value": n_steps * w.n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"{cells}^3 bcc cells ({w.n} atoms) of the {workload_name} recipe, {n_steps} oracle MD steps "
-                      f"(fp64, OpenMP, {n_steps + 1} force evaluations) in {dt:.1f} s"}, dt
+            "sample": f"{w.n} atoms of the {workload_name} recipe ({cells}^3-cell box instead of the full one), "
+                      f"{n_steps} oracle MD steps (fp64, OpenMP, {n_steps + 1} force evaluations) in {dt:.1f} s"}, dt
+
+
+def oracle_single_evaluations():
+    """SURVEY 8(d) CPU-baseline item (i): ONE timed oracle evaluation (energy, force, virial) of config 1 and of
+    config 2's initial state."""
+    import oracle
+    from paper_2305_08140_b200 import workloads as wl
+    out = {}
+    for name, w in (("config1", wl.config1()), ("config2_initial_state", wl.config2())):
+        P = oracle.Params(w.model)
+        t = time.perf_counter()
+        oracle.compute(P, w.pos, w.types, w.box, w.pbc)
+        dt = time.perf_counter() - t
+        out[name] = {"atoms": w.n, "seconds": dt, "atoms_per_s": w.n / dt}
+    return out
 
 
 def run_reference(args):
@@ -201,7 +256,7 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": args.workload + " (bounded sample, see cpu_baseline.sample)"},
+            "data": "synthetic", "config": {"workload": args.workload},
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -245,18 +300,8 @@ def run_b200(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
-
-    w = make_workload(args.workload, seed_offset=rank, cells=args.cells)
-    n = w.n
     stream = torch.cuda.Stream(device=dev)
-    g = binding.NepZbl(w.model, n, device=local_rank, stream=stream)
-    types = torch.from_numpy(w.types).to(dev)
-
-    def fresh_state():
-        pos = torch.from_numpy(w.pos.copy()).to(dev)
-        vel = torch.from_numpy(w.vel.copy()).to(dev)
-        g.md_init(pos, vel, types, w.box, w.pbc)
-        return pos, vel
+    K, W = args.steps, args.warmup
 
     def barrier():
         torch.cuda.synchronize(dev)
@@ -265,36 +310,95 @@ def run_b200(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
-    K, W = args.steps, args.warmup
-    dt_max, max_disp = w.dt_max, w.max_displacement
     sampler = ClockSampler(local_rank) if rank == 0 else None
     if sampler:
         sampler.wait_first()
 
-    # ---- device-resident run: K steps back to back (md_run), CUDA events on the launch stream
-    pos, vel = fresh_state()
-    e0 = sum(g.md_energies())
-    g.md_run(W, dt_max, max_disp)
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    l0 = g.nep_zbl_launch_count()
-    reb0 = g.md_get_counters()[1]
-    t_wall0 = time.time()
-    ev0.record(stream)
-    g.md_run(K, dt_max, max_disp)
-    ev1.record(stream)
-    barrier()
-    t_wall1 = time.time()
-    launches = g.nep_zbl_launch_count() - l0
-    ms_local = ev0.elapsed_time(ev1)
-    ms = aggregate_max(ms_local, world, dev)
-    rebuilds = g.md_get_counters()[1] - reb0
-    e1 = sum(g.md_energies())
-    clocks = sampler.summary(t_wall0, t_wall1) if sampler else None
-    total_atoms = aggregate_sum(float(n), world, dev)
-    value = total_atoms * K / (ms * 1e-3)
+    class Run:
+        """One workload resident on the device: handle, state, and the timed legs."""
 
-    # ---- same K steps, L2 flushed between steps (per-step event pairs; the flush is outside them)
+        def __init__(self, name, cells=None):
+            self.name = name
+            self.w = w = make_workload(name, seed_offset=rank, cells=cells)
+            self.n = w.n
+            self.cascade = name in CASCADE
+            self.g = binding.NepZbl(w.model, w.n, device=local_rank, stream=stream)
+            self.types = torch.from_numpy(w.types).to(dev)
+            self.pos = self.vel = None
+
+        def fresh_state(self):
+            w = self.w
+            self.pos = torch.from_numpy(w.pos.copy()).to(dev)
+            self.vel = torch.from_numpy(w.vel.copy()).to(dev)
+            self.g.md_init(self.pos, self.vel, self.types, w.box, w.pbc)
+
+        def timed_steps(self):
+            """W warm-up steps, then K steps back to back (md_run: no host round trip), CUDA events on the launch
+            stream, barrier + synchronize on both sides; max over ranks."""
+            g, w = self.g, self.w
+            self.fresh_state()
+            e0 = sum(g.md_energies())
+            g.md_run(W, w.dt_max, w.max_displacement)
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            barrier()
+            l0 = g.nep_zbl_launch_count()
+            reb0 = g.md_get_counters()[1]
+            forced = 0
+            if self.cascade:            # S2 inside the timed region whatever K is (see the module docstring)
+                g.md_request_rebuild()
+                forced = 1
+            t0 = time.time()
+            ev0.record(stream)
+            g.md_run(K, w.dt_max, w.max_displacement)
+            ev1.record(stream)
+            barrier()
+            t1 = time.time()
+            ms = aggregate_max(ev0.elapsed_time(ev1), world, dev)
+            total_atoms = aggregate_sum(float(self.n), world, dev)
+            n_zbl, n_fp64 = g.nep_zbl_last_counts()
+            return {"ms": ms, "ms_per_step": ms / K, "value": total_atoms * K / (ms * 1e-3), "total_atoms": total_atoms,
+                    "launches": g.nep_zbl_launch_count() - l0, "rebuilds": g.md_get_counters()[1] - reb0,
+                    "forced_rebuilds": forced, "energy_drift_ev_per_atom": (sum(g.md_energies()) - e0) / self.n,
+                    "zbl_atoms": n_zbl, "fp64_atoms": n_fp64, "window": (t0, t1),
+                    "clocks": sampler.summary(t0, t1) if sampler else None, "graph": g.nep_zbl_uses_graph()}
+
+        def profiled_steps(self, Kp):
+            """Per-kernel CUDA-event spans (plain stream launches with events between the kernel groups)."""
+            g, w = self.g, self.w
+            g.nep_zbl_profile(True)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            g.md_run(Kp, w.dt_max, w.max_displacement)
+            b.record(stream)
+            prof = g.nep_zbl_profile_read()
+            ms_step = a.elapsed_time(b) / Kp
+            kern_ms = {k: v[0] / v[1] for k, v in prof.items() if v[1]}
+            share = {k: round(v[0] / Kp / ms_step, 4) for k, v in prof.items() if v[1]}
+            # one list rebuild: the rebuild slot of a step that rebuilds minus that of a step that does not (the
+            # chain is enqueued every step in this mode and exits early unless the flag is set)
+            reb = []
+            for _ in range(3):
+                g.md_request_rebuild()
+                g.md_run(1, w.dt_max, w.max_displacement)
+                p1 = g.nep_zbl_profile_read()
+                g.md_run(1, w.dt_max, w.max_displacement)
+                p0 = g.nep_zbl_profile_read()
+                reb.append(p1["rebuild"][0] - p0["rebuild"][0])
+            g.nep_zbl_profile(False)
+            return ms_step, kern_ms, share, float(np.median(reb))
+
+        def close(self):
+            self.g.close()
+            self.pos = self.vel = self.types = None
+            torch.cuda.empty_cache()
+
+    main_run = Run(args.workload, args.cells)
+    n, w, g = main_run.n, main_run.w, main_run.g
+    dt_max, max_disp = w.dt_max, w.max_displacement
+    r = main_run.timed_steps()
+    ms, value, total_atoms, clocks = r["ms"], r["value"], r["total_atoms"], r["clocks"]
+
+    # ---- same steps, L2 flushed between steps (per-step event pairs; the flush is outside them)
     flush = torch.empty(2 * L2_BYTES, dtype=torch.uint8, device=dev)
     Kf = min(K, args.flush_steps)
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(Kf)]
@@ -308,24 +412,13 @@ def run_b200(args):
     ms_flushed = aggregate_max(sum(a.elapsed_time(b) for a, b in evs) / Kf, world, dev)
     del flush
 
-    # ---- per-kernel CUDA-event spans over K more steps (profiling events between kernel groups)
-    g.nep_zbl_profile(True)
-    evp0, evp1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    Kp = min(K, 200)
-    evp0.record(stream)
-    g.md_run(Kp, dt_max, max_disp)
-    evp1.record(stream)
-    prof = g.nep_zbl_profile_read()
-    g.nep_zbl_profile(False)
-    ms_prof_step = evp0.elapsed_time(evp1) / Kp
-    kern_ms = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in prof.items() if v[1]}
-    kern_share = {k: round(v[0] / Kp / ms_prof_step, 4) for k, v in prof.items() if v[1]}
+    ms_prof_step, kern_ms, kern_share, rebuild_ms = main_run.profiled_steps(min(K, 200))
     ffma_measured = g.nep_zbl_ffma_peak()
 
     # ---- end to end through the C ABI with HOST buffers (md_step_host): H2D + step + D2H per step
     hp = torch.from_numpy(w.pos.copy()).pin_memory()
     hv = torch.from_numpy(w.vel.copy()).pin_memory()
-    pos, vel = fresh_state()
+    main_run.fresh_state()
     Ke = min(K, args.e2e_steps)
     for _ in range(min(W, 5)):
         g.md_step_host(hp, hv, dt_max, max_disp)
@@ -340,12 +433,22 @@ def run_b200(args):
     wall_e2e = (time.perf_counter() - t0) * 1e3
     ms_e2e = aggregate_max(max(eve0.elapsed_time(eve1), wall_e2e), world, dev)
     e2e_value = total_atoms * Ke / (ms_e2e * 1e-3)
+    del hp, hv
+
     # ---- SURVEY 8(f) NEXT rows, same workload: border-layer Nose-Hoover chain and Wigner-Seitz count
     next_rows = None
+    hbm_peak_ = 6650.0
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        hbm_peak_ = float(peaks.get("hbm_gbs", 6650.0))
+    except OSError:
+        pass
     if world == 1 and not args.no_next:
         from paper_2305_08140_b200 import workloads as wl_
         group = torch.from_numpy(wl_.border_group(w.pos, w.box, w.pbc)).to(dev)
-        pos, vel = fresh_state()
+        main_run.fresh_state()
+        pos = main_run.pos
         g.md_set_thermostat(group, 300.0, 100.0, 4)
         Kn = min(K, 200)
         g.md_run(W, dt_max, max_disp)
@@ -371,11 +474,6 @@ def run_b200(args):
         evw1.record(stream)
         barrier()
         ms_ws = evw0.elapsed_time(evw1) / reps
-        hbm_peak_ = 6650.0
-        try:
-            hbm_peak_ = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json"))).get("hbm_gbs", 6650.0))
-        except OSError:
-            pass
         ws_gbs = WS_BYTES_PER_ATOM * n / (ms_ws * 1e-3) / 1e9
         next_rows = {
             "nhc_border_layer": {"ms_per_step": ms_nhc, "atom_steps_per_s": n / (ms_nhc * 1e-3), "steps": Kn,
@@ -387,6 +485,27 @@ def run_b200(args):
                                           "frac": ws_gbs / hbm_peak_, "bytes_per_atom": WS_BYTES_PER_ATOM},
                              "includes": "occupancy memset, assignment, count, 16-byte D2H of the totals, stream sync"},
         }
+        del site, group
+    props = torch.cuda.get_device_properties(dev)
+    workspace_bytes = g.workspace_bytes
+    main_run.close()
+
+    # ---- the other configs of BASELINE.json in the same run (device-resident timing only)
+    per_config = None
+    if world == 1 and args.per_config and args.cells is None:
+        per_config = {}
+        for name in [c for c in ("config2", "config3", "config5") if c != args.workload]:
+            run = Run(name)
+            rr = run.timed_steps()
+            _, kms, _, reb_ms = run.profiled_steps(min(K, 50))
+            per_config[name] = {"atoms": run.n, "ms_per_step": rr["ms_per_step"], "value": rr["value"], "steps": K,
+                                "list_rebuilds_in_timed_region": int(rr["rebuilds"]),
+                                "forced_rebuilds": rr["forced_rebuilds"], "rebuild_ms": reb_ms,
+                                "kernel_ms": {k: round(v, 5) for k, v in kms.items()},
+                                "zbl_atoms": rr["zbl_atoms"], "fp64_atoms": rr["fp64_atoms"],
+                                "energy_drift_ev_per_atom": rr["energy_drift_ev_per_atom"],
+                                "workspace_gib": run.g.workspace_bytes / 2 ** 30, "clocks": rr["clocks"]}
+            run.close()
     if sampler:
         sampler.stop()
 
@@ -396,25 +515,18 @@ def run_b200(args):
     # ---- roofline of the dominant kernel
     force_kernels = {k: kern_ms[k] for k in ("k_radial", "k_angular_nn", "k_force") if k in kern_ms}
     dom = max(force_kernels, key=force_kernels.get)
-    props = torch.cuda.get_device_properties(dev)
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except OSError:
-        pass
     sm_max_mhz = float(peaks.get("sm_max_mhz", (clocks or {}).get("sm_max_mhz") or 1965.0))
     alu_peak = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12     # TFLOP/s
     flop_table = PAPER_FLOP_PER_ATOM if args.workload == "paper" else FLOP_PER_ATOM
     achieved = flop_table[dom] * n / (kern_ms[dom] * 1e-3) / 1e12
-    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_peak = hbm_peak_
+    traffic, traffic_note = (args.traffic_bytes, "--traffic-bytes") if args.traffic_bytes is not None else \
+        ncu_traffic(args.workload, dom, args.cells)
     roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
-                "frac": achieved / alu_peak,
-                "traffic": args.traffic_bytes if args.traffic_bytes is not None else
-                (NCU_TRAFFIC_BYTES.get(args.workload, {}).get(dom) if args.cells is None else None),
-                "traffic_source": NCU_TRAFFIC_SOURCE,
+                "frac": achieved / alu_peak, "traffic": traffic, "traffic_note": traffic_note,
                 "peak_source": f"derived: {props.multi_processor_count} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max_mhz:.0f} MHz",
                 "ffma_measured_tflops": ffma_measured, "ms_per_launch": kern_ms[dom],
-                "flop_per_atom": flop_table[dom],
+                "flop_per_atom": flop_table[dom], "units_per_launch": n,
                 # every force kernel and the whole step against the same ALU peak (algorithmic flops of DESIGN.md)
                 "alu": {k: {"achieved_tflops": flop_table[k] * n / (kern_ms[k] * 1e-3) / 1e12,
                             "frac": flop_table[k] * n / (kern_ms[k] * 1e-3) / 1e12 / alu_peak}
@@ -429,7 +541,8 @@ def run_b200(args):
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
-        cpu_baseline, _ = oracle_md_rate(args.workload, None, 0, budget_s=15.0)
+        cpu_baseline, _ = oracle_md_rate(args.workload, None, 0, budget_s=12.0)
+        cpu_baseline["single_evaluations"] = oracle_single_evaluations()
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -438,19 +551,23 @@ def run_b200(args):
         "config": {"workload": args.workload, "atoms_per_gpu": n, "dt_max_fs": dt_max,
                    "max_displacement_A": (None if not np.isfinite(max_disp) else max_disp), "skin_A": w.model["skin"],
                    "model": MODEL_DESC.get(args.workload, DEFAULT_MODEL_DESC),
-                   "precision": "fp32 descriptors/network/forces, fp64 positions/velocities/ZBL/energy sums",
+                   "precision": "fp32 descriptors/network/forces (fp64 re-evaluation of disordered sites), "
+                                "fp64 positions/velocities/ZBL/energy sums",
                    "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
-                   "l2": f"no flush for `value` (consecutive steps of one trajectory; workspace {g.workspace_bytes / 2**20:.0f} MiB "
+                   "l2": f"no flush for `value` (consecutive steps of one trajectory; workspace {workspace_bytes / 2**20:.0f} MiB "
                          f"> {L2_BYTES / 2**20:.0f} MiB L2); `ms_per_step_l2_flushed` flushes L2 (2x L2 write) before every step",
-                   "list_rebuilds_in_timed_region": int(rebuilds)},
+                   "list_rebuilds_in_timed_region": int(r["rebuilds"]), "forced_rebuilds": r["forced_rebuilds"],
+                   "cuda_graph": bool(r["graph"])},
         "ms_per_step_l2_flushed": ms_flushed, "value_l2_flushed": total_atoms / (ms_flushed * 1e-3),
-        "ms_per_step_profiled": ms_prof_step,
+        "ms_per_step_profiled": ms_prof_step, "rebuild_ms": rebuild_ms,
         "kernel_ms": {k: round(v, 5) for k, v in kern_ms.items()}, "kernel_share": kern_share,
-        "energy_drift_ev_per_atom": (e1 - e0) / n,
+        "energy_drift_ev_per_atom": r["energy_drift_ev_per_atom"],
+        "zbl_atoms": r["zbl_atoms"], "fp64_atoms": r["fp64_atoms"],
         "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 48 * n, "d2h_bytes_per_step": 48 * n,
                 "steps": Ke, "api": "md_step_host"},
-        "gpu_launches": int(launches),
+        "gpu_launches": int(r["launches"]),
+        "per_config": per_config,
         "next_rows": next_rows,
         "context": {"paper": "1.3e7 atom-step/s, one 40-GB A100, trained W NEP-ZBL (n_max 15/10, 100 neurons), Table IV"},
     }
@@ -461,10 +578,13 @@ def run_b200(args):
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=1000)
-    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--workload", default="config4",
+                    choices=["config2", "config3", "config4", "config5", "alloy", "paper"])
+    ap.add_argument("--no-per-config", dest="per_config", action="store_false",
+                    help="skip the other BASELINE.json configs (config2/3/5) timed in the same run")
     ap.add_argument("--cells", type=int, default=None, help="override the cell count (debug only)")
     ap.add_argument("--e2e-steps", type=int, default=200)
     ap.add_argument("--flush-steps", type=int, default=100)

@@ -165,6 +165,11 @@ int md_run(nepzbl_handle *h, int64_t n_steps, double dt_max, double max_displace
  * returns when both buffers are complete. */
 int md_step_host(nepzbl_handle *h, double *pos_soa, double *vel_soa, double dt_max,
                  double max_displacement, double *dt_used, int32_t *rebuilt);
+/* The next md_step / first step of the next md_run rebuilds the neighbour list (S2) whatever the displacement
+ * criterion says (asynchronous: one flag on the device).  bench.py uses it to put a list rebuild inside a short timed
+ * region; a caller that edits positions by more than the skin between steps does not need it (the criterion sees the
+ * edit). */
+int md_request_rebuild(nepzbl_handle *h);
 /* Total potential and kinetic energy of the current MD state (host scalars), fixed-order fp64
  * reduction. */
 int md_energies(nepzbl_handle *h, double *e_pot, double *e_kin);
@@ -220,7 +225,8 @@ int nep_zbl_uses_graph(const nepzbl_handle *h);
  * range (evaluated by the fp64 pair kernel, Eq. 2-4), and atoms whose angular network inputs |s_nu q_nu| exceeded the
  * fp32 accuracy threshold and were re-evaluated in fp64 (none in a thermal crystal, the
  * disordered core of a cascade; the environment variable NEPZBL_DENSE_THRESHOLD, read at create, overrides the
- * threshold of 3, "off" disables the pass). */
+ * thresholds -- 8 on the 3-body inputs, 3 on the 4-/5-body inputs -- with one number or "t3,t4"; "off" disables
+ * the pass). */
 int nep_zbl_last_counts(nepzbl_handle *h, int64_t *n_zbl_atoms, int64_t *n_fp64_atoms);
 
 /* Number of kernel launches issued by this handle so far (for bench.py's gpu_launches). */

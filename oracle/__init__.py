@@ -188,9 +188,24 @@ def _sys_args(pos, types, box, pbc):
     return pos, n, types, box, pbc
 
 
-def neighbors(pos, box, pbc, rc: float, use_cell: bool = False, cap: int = 256, want_d: bool = False):
-    """Neighbour lists (S:A): nn[n], nl[n][cap] (canonical order), optionally displacement vectors."""
+def neighbors(pos, box, pbc, rc: float, use_cell: bool = False, cap: int = 256, want_d: bool = False, sel=None):
+    """Neighbour lists (S:A): nn[n], nl[n][cap] (canonical order), optionally displacement vectors.
+    sel: only these atoms (row t of the result belongs to atom sel[t])."""
     pos, n, _, box, pbc = _sys_args(pos, None, box, pbc)
+    if sel is not None:
+        assert not want_d
+        sel = np.ascontiguousarray(sel, dtype=np.int32)
+        nn = np.zeros(sel.size, dtype=np.int32)
+        nl = np.full((sel.size, cap), -1, dtype=np.int32)
+        f = lib().orc_neighbors_sel
+        f.restype = C.c_int
+        r = f(C.c_int(n), _dp(pos), _dp(box), _ip(pbc), C.c_double(rc), C.c_int(int(use_cell)), C.c_int(cap),
+              C.c_int(sel.size), _ip(sel), _ip(nn), _ip(nl))
+        if r < 0:
+            raise RuntimeError(f"oracle neighbours failed: {r}")
+        if r > cap:
+            raise RuntimeError(f"oracle neighbour capacity {cap} < {r}")
+        return nn, nl
     nn = np.zeros(n, dtype=np.int32)
     nl = np.full((n, cap), -1, dtype=np.int32)
     nd = np.zeros((n, cap, 3)) if want_d else None

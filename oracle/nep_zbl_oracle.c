@@ -551,6 +551,31 @@ int orc_neighbors(int n, const double *pos, const double *box, const int32_t *pb
   return maxc;
 }
 
+/* The same lists for a SELECTION of atoms only (rows t = 0..nsel-1 belong to atom sel[t]): what the at-size
+ * parity tests need of a multi-million-atom system.  No arithmetic of its own: orc_site_neighbors per selected atom. */
+int orc_neighbors_sel(int n, const double *pos, const double *box, const int32_t *pbc, double rc,
+                      int use_cell, int cap, int nsel, const int32_t *sel, int32_t *nn, int32_t *nl) {
+  orc_system S;
+  int rcode = orc_system_init(&S, n, pos, box, pbc, rc, use_cell);
+  if (rcode) return rcode;
+  int maxc = 0;
+#pragma omp parallel
+  {
+    orc_nbr *buf = (orc_nbr *)malloc(sizeof(orc_nbr) * cap);
+#pragma omp for schedule(dynamic, 64) reduction(max : maxc)
+    for (int t = 0; t < nsel; ++t) {
+      int c = orc_site_neighbors(&S, sel[t], rc, buf, cap);
+      nn[t] = c;
+      if (c > maxc) maxc = c;
+      int m = c < cap ? c : cap;
+      for (int s = 0; s < m; ++s) nl[(size_t)t * cap + s] = buf[s].j;
+    }
+    free(buf);
+  }
+  orc_system_free(&S);
+  return maxc;
+}
+
 /* ------------------------------------------------------------------ energy / force / virial, S:D, S:E */
 
 #define ORC_NBR_CAP 512

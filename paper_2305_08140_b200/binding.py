@@ -27,7 +27,7 @@ ERRORS = {-1: "INVALID_ARG", -2: "BOX_NOT_ORTHOGONAL", -3: "BOX_TOO_SMALL", -4: 
 EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_descriptor_dim",
            "nep_zbl_workspace_bytes", "nep_zbl_set_workspace", "neighbor_build", "neighbor_get",
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
-           "md_run", "md_step_host", "md_energies", "md_get_forces", "md_get_counters",
+           "md_run", "md_step_host", "md_request_rebuild", "md_energies", "md_get_forces", "md_get_counters",
            "md_set_thermostat", "md_get_thermostat", "md_set_thermostat_state", "wigner_seitz_set_reference", "wigner_seitz_count",
            "nep_zbl_uses_graph", "nep_zbl_last_counts", "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
 PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "k_site_fp64"]
@@ -90,6 +90,8 @@ _lib.md_run.argtypes = [_vp, _i64, _dbl, _dbl, _vp, C.POINTER(_i64)]
 _lib.md_run.restype = C.c_int
 _lib.md_step_host.argtypes = [_vp, _vp, _vp, _dbl, _dbl, C.POINTER(_dbl), C.POINTER(_i32)]
 _lib.md_step_host.restype = C.c_int
+_lib.md_request_rebuild.argtypes = [_vp]
+_lib.md_request_rebuild.restype = C.c_int
 _lib.md_energies.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_dbl)]
 _lib.md_energies.restype = C.c_int
 _lib.md_get_forces.argtypes = [_vp, _vp, _vp]
@@ -243,6 +245,9 @@ class NepZbl:
         self._chk(_lib.md_step_host(self.h, _ptr(pos_host), _ptr(vel_host), dt_max, max_displacement,
                                     C.byref(dt), C.byref(rb)))
         return dt.value, rb.value
+
+    def md_request_rebuild(self):
+        self._chk(_lib.md_request_rebuild(self.h))
 
     def md_energies(self):
         ep = _dbl(); ek = _dbl()

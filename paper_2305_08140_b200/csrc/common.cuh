@@ -42,7 +42,6 @@ struct Scalars {  // device-resident control block (one per handle)
   int box_too_small;
   int zbl_count;
   int dense_count;                      // atoms listed by k_angular_nn for the fp64 re-evaluation (site_fp64.cuh)
-  unsigned int ang_done;                // ticket counter of k_angular_nn's last-block book-keeping (graph IF node)
   int bad_type;                         // an atom type outside [0, n_types) was seen (clamped; reported as INVALID_ARG)
   int n_rebuilds;
   long long n_steps;

@@ -48,30 +48,18 @@ struct ModelTables {
   float inv_shell_w;           // 8 / skin (0 without skin): sub-shells of the list's skin shell, see k_nbr
   float b1;
   int n_neurons;
-  float dense_thr;             // angular network inputs |s q| above this send the atom to the fp64 pass (site_fp64.cuh)
+  float dense_thr;             // 3-body network inputs |s q| above this send the atom to the fp64 pass (site_fp64.cuh)
+  float dense_thr4;            // the same for the 4-body (and 5-body) inputs, whose fp32 error grows faster
 };
 
 // hand-over to the fp64 re-evaluation (site_fp64.cuh): atoms are appended to dense_list (integer ticket: the order
-// of the list is free, every listed atom is evaluated on its own); in a captured graph the block that finishes last
-// opens / closes the IF node of k_site_fp64
+// of the list is free, every listed atom is evaluated on its own).  k_site_fp64 follows k_angular_nn as a plain
+// kernel node that walks the list (measured on config2, where the list is empty: an IF node opened by k_angular_nn's
+// last block cost 9.2 us per step, the plain node 5.5 us)
 struct DenseArgs {
   Scalars* sc;
   int* dense_list;              // NULL: no listing
-  unsigned long long cond;
-  int use_cond;
 };
-__device__ __forceinline__ void dense_ticket(const DenseArgs& da) {
-#if defined(__CUDA_ARCH__)
-  // called by ONE thread per block after the block's last listing (the caller synchronises the block first)
-  if (!da.use_cond) return;
-  __threadfence();
-  if (atomicAdd(&da.sc->ang_done, 1u) == gridDim.x - 1) {
-    __threadfence();
-    da.sc->ang_done = 0u;
-    cudaGraphSetConditional((cudaGraphConditionalHandle)da.cond, atomicAdd(&da.sc->dense_count, 0) > 0 ? 1u : 0u);
-  }
-#endif
-}
 
 // Record of one atom for the radial back-pass of k_force (sorted order), 64-byte stride so that it
 // never straddles a 128-byte line: {ux,uy,uz,d0..d4 | d5..d11 pad}.  d[k] = sum_n Fp[n] ct_nk are the
@@ -573,10 +561,12 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       Fp[v] = 0.0f;
     }
     if (da.dense_list) {  // large angular inputs: fp32 sums are not accurate enough, list the atom for the fp64 pass
-      float mx = 0.0f;
+      float mx = 0.0f, mx4 = 0.0f;
 #pragma unroll
-      for (int v = NR; v < D; ++v) mx = fmaxf(mx, fabsf(q[v]));
-      if (!(mx <= mt.dense_thr)) da.dense_list[atomicAdd(&da.sc->dense_count, 1)] = s;
+      for (int v = NR; v < NR + 4 * NA; ++v) mx = fmaxf(mx, fabsf(q[v]));
+#pragma unroll
+      for (int v = NR + 4 * NA; v < D; ++v) mx4 = fmaxf(mx4, fabsf(q[v]));
+      if (!(mx <= mt.dense_thr) || !(mx4 <= mt.dense_thr4)) da.dense_list[atomicAdd(&da.sc->dense_count, 1)] = s;
     }
     float U = -mt.b1;
     // software pipeline: the pre-activations of neurons m+2, m+3 are accumulated while the tanh of
@@ -719,6 +709,4 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       pforce[(size_t)a * npad + s] = make_float4(px, py, pz, 0.0f);
     }
   }
-  __syncthreads();
-  if (threadIdx.x == 0) dense_ticket(da);
 }

@@ -198,11 +198,13 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       Fp[i] = 0.0f;
     }
     if (da.dense_list) {  // large angular inputs anywhere in the quad: list the atom for the fp64 pass (site_fp64.cuh)
-      float mx = 0.0f;
+      float mx = 0.0f, mx4 = 0.0f;
 #pragma unroll
-      for (int i = 0; i < SLP; ++i)
-        if (i < 4 * NSUB || i >= 4 * NSUB + RSUB) mx = fmaxf(mx, fabsf(q[i]));
-      const bool big = !(mx <= mt.dense_thr);
+      for (int i = 0; i < SLP; ++i) {
+        if (i < 4 * NSUB) mx = fmaxf(mx, fabsf(q[i]));
+        else if (i >= 4 * NSUB + RSUB) mx4 = fmaxf(mx4, fabsf(q[i]));
+      }
+      const bool big = !(mx <= mt.dense_thr) || !(mx4 <= mt.dense_thr4);
       const unsigned bq = (__ballot_sync(0xffffffffu, big) >> qbase) & 0xFu;
       if (bq && valid && sub == 0) da.dense_list[atomicAdd(&da.sc->dense_count, 1)] = s;
     }
@@ -373,6 +375,4 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       }
     }
   }
-  __syncthreads();
-  if (threadIdx.x == 0) dense_ticket(da);
 }

@@ -67,7 +67,6 @@ struct nepzbl_handle {
   SiteModel site{};           // fp64 tables of k_site_fp64 (d_site holds them)
   double* d_site = nullptr;
   bool dense_on = true;       // NEPZBL_DENSE_THRESHOLD=off disables the fp64 re-evaluation (measurement aid)
-  cudaGraph_t building = nullptr;  // graph under construction (build_step_graph): enqueue_eval adds the fp64 IF node
   size_t smem_nn = 0;
   // threads per block of k_radial / k_force: one warp while the grid is only a few waves of resident threads (the
   // partly filled last wave costs one block's duration: 128 000 atoms 32: 78.3 us, 64: 80.5, 128: 83.1 for
@@ -254,13 +253,20 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   t.inv_shell_w = p->skin > 0 ? (float)(8.0 / p->skin) : 0.0f;
   t.b1 = (float)p->b1;
   t.n_neurons = p->n_neurons;
-  // fp64 re-evaluation threshold on the angular network inputs |s q| (site_fp64.cuh):
-  // a 300 K crystal stays below 0.8, so the default lists no thermal atom; NEPZBL_DENSE_THRESHOLD overrides
-  // (a number, or "off")
-  t.dense_thr = 3.0f;
+  // fp64 re-evaluation thresholds on the angular network inputs |s q| (site_fp64.cuh):
+  // 8 for the 3-body inputs, 3 for the 4-/5-body inputs.  A 300 K crystal stays below 0.8 / 0.4 and the atoms of a free
+  // (001) surface below 6.2 / 1.3 (coherent l = 1 sums, accurate in fp32), so neither is listed; the disordered
+  // sites that miss the tolerance in fp32 have 4-body inputs of 50-2500.  NEPZBL_DENSE_THRESHOLD overrides: "off",
+  // one number (both thresholds) or "t3,t4".
+  t.dense_thr = 8.0f;
+  t.dense_thr4 = 3.0f;
   if (const char* dt = getenv("NEPZBL_DENSE_THRESHOLD")) {
     if (!strcmp(dt, "off")) h->dense_on = false;
-    else if (atof(dt) > 0.0) t.dense_thr = (float)atof(dt);
+    else if (atof(dt) > 0.0) {
+      t.dense_thr = t.dense_thr4 = (float)atof(dt);
+      if (const char* comma = strchr(dt, ','))
+        if (atof(comma + 1) > 0.0) t.dense_thr4 = (float)atof(comma + 1);
+    }
   }
   h->tables.resize(sizeof t);
   memcpy(h->tables.data(), &t, sizeof t);
@@ -440,31 +446,12 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
   return nk + 9;
 }
 
-// Stream capture helper: add an IF node (condition `handle`, set on the device) behind whatever `st` has captured so
-// far into graph `g`, make the following captured work depend on it, and return the node's body graph.
-bool graph_add_if(cudaStream_t st, cudaGraph_t g, cudaGraphConditionalHandle handle, cudaGraph_t* body) {
-  cudaStreamCaptureStatus status;
-  const cudaGraphNode_t* deps = nullptr;
-  size_t ndeps = 0;
-  cudaGraph_t cg = nullptr;
-  if (cudaStreamGetCaptureInfo(st, &status, nullptr, &cg, &deps, &ndeps) != cudaSuccess) return false;
-  cudaGraphNodeParams np = {};
-  np.type = cudaGraphNodeTypeConditional;
-  np.conditional.handle = handle;
-  np.conditional.type = cudaGraphCondTypeIf;
-  np.conditional.size = 1;
-  cudaGraphNode_t node;
-  if (cudaGraphAddNode(&node, g, deps, ndeps, &np) != cudaSuccess) return false;
-  *body = np.conditional.phGraph_out[0];
-  return cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies) == cudaSuccess;
-}
-
 // fp64 re-evaluation of the atoms k_angular_nn listed (site_fp64.cuh); grid-stride over the list
 void launch_site_fp64(nepzbl_handle* h, const double* pos, bool want_q, cudaStream_t st) {
   const Carve& c = h->cv;
   const int n = (int)h->n;
   const int grid = std::max(1, std::min(blocks(n, SITE64_WARPS), 8 * h->n_sm));
-  const size_t smem = sizeof(double) * SITE64_WARPS * (2 * (size_t)h->site.D + h->site.n_neurons);
+  const size_t smem = sizeof(double) * SITE64_WARPS * (2 * (size_t)h->site.D + h->site.n_neurons + 8);
   k_site_fp64<<<grid, 32 * SITE64_WARPS, smem, st>>>(
       h->d_sc, h->d_bm, h->site, h->at<int>(c.dense_list), n, c.npad, h->at<int4>(c.xyzt), h->at<int>(c.nl_r),
       h->at<unsigned long long>(c.amask), h->at<int>(c.perm), pos, h->at<float>(c.q_radial), h->at<float>(c.u_site),
@@ -478,11 +465,7 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   const Carve& c = h->cv;
   const int n = (int)h->n, npad = c.npad;
   cudaStream_t st = h->stream;
-  // in a graph under construction the fp64 pass sits in an IF node that k_angular_nn's last block opens
-  cudaGraphConditionalHandle h_dense = 0;
-  const bool dense_if = h->dense_on && h->building &&
-                        cudaGraphConditionalHandleCreate(&h_dense, h->building, 0, cudaGraphCondAssignDefault) == cudaSuccess;
-  const DenseArgs da{h->d_sc, h->dense_on ? h->at<int>(c.dense_list) : nullptr, (unsigned long long)h_dense, dense_if ? 1 : 0};
+  const DenseArgs da{h->d_sc, h->dense_on ? h->at<int>(c.dense_list) : nullptr};
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
   const int gb = h->gather_block ? h->gather_block : ((long long)n * RADIAL_LANES < 8ll * 1024 * h->n_sm ? 32 : 64);
   prof_mark(h, PK_RADIAL);
@@ -505,19 +488,8 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
         want_q ? h->at<float>(c.q_desc) : nullptr, da);
   if (h->dense_on) {
     prof_mark(h, PK_SITE64);
-    if (dense_if) {
-      cudaGraph_t body = nullptr;
-      if (graph_add_if(st, h->building, h_dense, &body) &&
-          cudaStreamBeginCaptureToGraph(h->cap_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-        launch_site_fp64(h, pos, want_q, h->cap_stream);
-        if (cudaStreamEndCapture(h->cap_stream, nullptr) != cudaSuccess) h->building = nullptr;  // reported by build_step_graph
-      } else {
-        h->building = nullptr;
-      }
-    } else {
-      launch_site_fp64(h, pos, want_q, st);
-      h->launches++;
-    }
+    launch_site_fp64(h, pos, want_q, st);
+    h->launches++;
   }
   prof_mark(h, PK_FORCE);
   auto launch_force = [&](auto vir, auto blk) {
@@ -1087,11 +1059,8 @@ static bool build_step_graph(nepzbl_handle* h) {
   if (ok) {
     const KickArgs ka{h->d_sc, h->md_vel, h->d_inv_mass, h->nhc_on ? 0 : 1, (unsigned long long)h_zbl,
                       h->p.zbl_enabled ? 1 : 0};
-    h->building = g;  // enqueue_eval puts k_site_fp64 into an IF node of this graph
     enqueue_eval(h, h->md_pos, h->at<double>(c.md_energy), h->at<float>(c.md_force), nullptr, false, false, ka);
-    ok = h->building == g;
-    h->building = nullptr;
-    nk += 3;
+    nk += 3 + (h->dense_on ? 1 : 0);
     if (h->p.zbl_enabled) {
       ok = add_if(h_zbl, &body);
       if (ok) {
@@ -1161,7 +1130,6 @@ static int md_step_impl(nepzbl_handle* h, double dt_max, double max_displacement
   if (rebuilt) *rebuilt = h->h_sc->do_rebuild;
   if (h->h_sc->do_rebuild && h->use_graph && !h->prof && h->step_exec) h->launches += h->graph_rebuild_kernels;
   if (h->h_sc->zbl_count > 0 && h->use_graph && !h->prof && h->step_exec) h->launches += 1;
-  if (h->h_sc->dense_count > 0 && h->use_graph && !h->prof && h->step_exec) h->launches += 1;
   rc = check_device_flags(h);
   if (rc) h->md_ready = false;
   return rc;
@@ -1211,6 +1179,15 @@ int md_step_host(nepzbl_handle* h, double* pos, double* vel, double dt_max, doub
   CU(cudaMemcpyAsync(h->md_pos, pos, b, cudaMemcpyHostToDevice, h->stream));
   CU(cudaMemcpyAsync(h->md_vel, vel, b, cudaMemcpyHostToDevice, h->stream));
   return md_step_impl(h, dt_max, max_displacement, dt_used, rebuilt, pos, vel);
+}
+
+int md_request_rebuild(nepzbl_handle* h) {
+  if (!h) return NEPZBL_E_INVALID_ARG;
+  if (!h->md_ready) return fail(h, NEPZBL_E_STATE, "md_request_rebuild before md_init");
+  k_set_force_rebuild<<<1, 1, 0, h->stream>>>(h->d_sc);
+  h->launches++;
+  CU(cudaGetLastError());
+  return NEPZBL_OK;
 }
 
 int md_set_thermostat(nepzbl_handle* h, const uint8_t* group, double temperature, double tau,

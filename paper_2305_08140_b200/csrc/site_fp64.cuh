@@ -11,8 +11,8 @@
 // FP64 from the fp64 master positions (as k_zbl does for the pair term), overwriting u_site, the k_force record
 // and the atom's partial forces.  None in a thermal crystal; the core atoms of a cascade.
 //
-// One WARP per listed atom; lane n owns the angular channel n (A[n][24] in registers); the network runs with the
-// neurons / descriptor components spread over the lanes.  All sizes are run-time values (SiteModel), so the one
+// One WARP per listed atom; the lanes are (neighbour slice, angular channel) pairs (see the kernel); the network runs
+// with the neurons / descriptor components spread over the lanes.  All sizes are run-time values (SiteModel), so the one
 // kernel serves every model shape.  Reductions across lanes are fixed-order butterflies: deterministic.
 // Same mathematics as descriptor.cuh, same factorisations, FP64 throughout.
 #pragma once
@@ -92,6 +92,11 @@ __device__ __forceinline__ void disp_f64(const BoxMap* bm, const double* __restr
   }
 }
 
+// Lane map: lane = slice * NA + n for lane < NS * NA, NS = 32 / NA (config model: 6 slices x 5 channels; paper-sized
+// model: 2 x 11).  Slice s takes the in-cutoff angular neighbours number s, s + NS, ... of the atom, so a warp works
+// on NS neighbours at a time; A[n][lm] is then summed over the slices in slice order on every lane (the same bits
+// everywhere), and in the back-pass the per-channel parts of a neighbour's partial force are summed over n inside
+// its slice, again in a fixed order.
 __global__ void __launch_bounds__(32 * SITE64_WARPS)
 k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm, const int* __restrict__ dense_list,
             int n, int npad, const int4* __restrict__ xyzt, const int* __restrict__ nl_r,
@@ -101,11 +106,15 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
   extern __shared__ double sm64[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int NR = sm.NR, NA = sm.NA, KA = sm.KA, KR = sm.KR, D = sm.D, NT = sm.NT;
-  double* xs = sm64 + (size_t)wib * (2 * D + sm.n_neurons);  // network inputs x_nu
-  double* Fp = xs + D;                                       // dU/dq_nu
-  double* tt = Fp + D;                                       // w1 (1 - h^2) per neuron
+  const int per_warp = 2 * D + sm.n_neurons + 8;              // doubles per warp (+8: 64 one-byte slot numbers)
+  double* xs = sm64 + (size_t)wib * per_warp;                 // network inputs x_nu
+  double* Fp = xs + D;                                        // dU/dq_nu
+  double* tt = Fp + D;                                        // w1 (1 - h^2) per neuron
+  unsigned char* slot = reinterpret_cast<unsigned char*>(tt + sm.n_neurons);  // list slot of in-cutoff neighbour c
   const int total = sc->dense_count;
-  const bool own = lane < NA;  // this lane owns angular channel n = lane
+  const int NS = 32 / NA;                                     // >= 1 (NA <= 32, checked at create)
+  const bool own = lane < NS * NA;
+  const int ch = own ? lane % NA : 0, slice = own ? lane / NA : 0;
   const double rc = sm.rcA, inv_rc = 1.0 / sm.rcA;
   const double C4 = -45.0 / (8.0 * sqrt(14.0) * SITE64_PI * sqrt(SITE64_PI));
   for (int t = blockIdx.x * SITE64_WARPS + wib; t < total; t += gridDim.x * SITE64_WARPS) {
@@ -114,14 +123,22 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
     const int4 me = xyzt[s];
     const int ti = me.w;
     const unsigned long long mask = amask[s];
+    const int nc = __popcll(mask);
+    if (lane == 0) {
+      int c = 0;
+      for (unsigned long long m = mask; m; m &= m - 1) slot[c++] = (unsigned char)(__ffsll((long long)m) - 1);
+    }
+    __syncwarp();
+    const int rounds = (nc + NS - 1) / NS;
 
-    // ---- S4 forward in fp64: A[lm] of channel n = lane
+    // ---- S4 forward in fp64: this lane's part of A[ch][lm] (its slice of the neighbours)
     double A[24];
 #pragma unroll
     for (int lm = 0; lm < 24; ++lm) A[lm] = 0.0;
-    for (unsigned long long m = mask; m; m &= m - 1) {
-      const int a = __ffsll((long long)m) - 1;
-      const int j = nl_r[(size_t)a * npad + s];
+    for (int rd = 0; rd < rounds; ++rd) {
+      const int c = rd * NS + slice;
+      if (!own || c >= nc) continue;
+      const int j = nl_r[(size_t)slot[c] * npad + s];
       double d[3];
       disp_f64(bm, pos, n, i, perm[j], d);
       const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
@@ -129,7 +146,7 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
       const double tr = r * inv_rc, u = tr - 1.0;
       const double fc = 0.5 + 0.5 * cospi(tr);
       const double x = 2.0 * u * u - 1.0;
-      const double* ct = sm.ctA + ((size_t)(ti * NT + xyzt[j].w) * NA + (own ? lane : 0)) * KA;
+      const double* ct = sm.ctA + ((size_t)(ti * NT + xyzt[j].w) * NA + ch) * KA;
       double T0 = 1.0, T1 = x, g = ct[0];
       if (KA > 1) g += ct[1] * x;
       for (int k = 2; k < KA; ++k) {
@@ -138,10 +155,19 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
         T0 = T1;
         T1 = T2;
       }
-      g = own ? g * fc : 0.0;
+      g *= fc;
       const double ri = 1.0 / r;
       blm_and_grad_f64(d[0] * ri, d[1] * ri, d[2] * ri,
                        [&](int lm, double b, double, double, double) { A[lm] += g * b; });
+    }
+    __syncwarp();
+    // sum over the slices, slice 0 first, on every lane of the channel (fixed order: the same bits in all slices)
+#pragma unroll
+    for (int lm = 0; lm < 24; ++lm) {
+      const double mine = A[lm];
+      double tot = 0.0;
+      for (int sl = 0; sl < NS; ++sl) tot += __shfl_sync(0xffffffffu, mine, sl * NA + ch);
+      A[lm] = own ? tot : 0.0;
     }
 
     // ---- descriptor: 3-body q_nl, 4-body q_n^222, scaled into xs[]
@@ -163,10 +189,10 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
       dq4[3] = k3 * 0.5 * (cxx - cyy);
       dq4[4] = k3 * cxy;
     }
-    if (own) {
+    if (own && slice == 0) {
 #pragma unroll
-      for (int l = 0; l < 4; ++l) xs[NR + l * NA + lane] = ql[l];
-      if (sm.B4) xs[NR + 4 * NA + lane] = q4;
+      for (int l = 0; l < 4; ++l) xs[NR + l * NA + ch] = ql[l];
+      if (sm.B4) xs[NR + 4 * NA + ch] = q4;
     }
     for (int nq = lane; nq < NR; nq += 32) xs[nq] = (double)q_radial[(size_t)nq * npad + s];
     __syncwarp();
@@ -217,62 +243,74 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
       }
     }
 
-    // ---- E[lm] = dU/dA[n][lm] (in place)
+    // ---- E[lm] = dU/dA[ch][lm] (in place; the same on every slice of the channel)
 #pragma unroll
     for (int lm = 0; lm < 24; ++lm)
-      A[lm] *= own ? 2.0 * clm_f64(lm) * Fp[NR + (lm_to_l(lm) - 1) * NA + lane] : 0.0;
+      A[lm] *= own ? 2.0 * clm_f64(lm) * Fp[NR + (lm_to_l(lm) - 1) * NA + ch] : 0.0;
     if (sm.B4 && own) {
-      const double f4 = Fp[NR + 4 * NA + lane];
+      const double f4 = Fp[NR + 4 * NA + ch];
 #pragma unroll
       for (int m5 = 0; m5 < 5; ++m5) A[3 + m5] += f4 * dq4[m5];
     }
 
-    // ---- angular partial forces dU_i/dr_ij for every slot of the mask (k_force reads exactly those)
-    for (unsigned long long m = mask; m; m &= m - 1) {
-      const int a = __ffsll((long long)m) - 1;
-      const int j = nl_r[(size_t)a * npad + s];
-      double d[3];
-      disp_f64(bm, pos, n, i, perm[j], d);
-      const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-      double px = 0.0, py = 0.0, pz = 0.0;
-      if (r < rc) {
-        const double tr = r * inv_rc, u = tr - 1.0;
-        const double fc = 0.5 + 0.5 * cospi(tr);
-        const double dfc = -0.5 * SITE64_PI * inv_rc * sinpi(tr);
-        const double x = 2.0 * u * u - 1.0, dxdr = 4.0 * u * inv_rc;
-        const double* ct = sm.ctA + ((size_t)(ti * NT + xyzt[j].w) * NA + (own ? lane : 0)) * KA;
-        // p = sum_k ct_k T_k,  dp = sum_k ct_k k U_{k-1}   (T_k' = k U_{k-1})
-        double T0 = 1.0, T1 = x, U0 = 1.0, U1 = 2.0 * x;
-        double p = ct[0], dp = 0.0;
-        if (KA > 1) { p += ct[1] * x; dp += ct[1]; }
-        for (int k = 2; k < KA; ++k) {
-          const double T2 = 2.0 * x * T1 - T0;
-          p += ct[k] * T2;
-          dp += ct[k] * (double)k * U1;
-          const double U2 = 2.0 * x * U1 - U0;
-          T0 = T1; T1 = T2; U0 = U1; U1 = U2;
+    // ---- angular partial forces dU_i/dr_ij for every slot of the mask (k_force reads exactly those): slice s
+    //      evaluates neighbour rd * NS + s, every lane its channel's part, summed over the channels in channel order
+    for (int rd = 0; rd < rounds; ++rd) {
+      const int c = rd * NS + slice;
+      const bool act = own && c < nc;
+      double Sp = 0.0, vx = 0.0, vy = 0.0, vz = 0.0, ri = 0.0, ux = 0.0, uy = 0.0, uz = 0.0;
+      int a = 0;
+      if (act) {
+        a = slot[c];
+        const int j = nl_r[(size_t)a * npad + s];
+        double d[3];
+        disp_f64(bm, pos, n, i, perm[j], d);
+        const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (r < rc) {
+          const double tr = r * inv_rc, u = tr - 1.0;
+          const double fc = 0.5 + 0.5 * cospi(tr);
+          const double dfc = -0.5 * SITE64_PI * inv_rc * sinpi(tr);
+          const double x = 2.0 * u * u - 1.0, dxdr = 4.0 * u * inv_rc;
+          const double* ct = sm.ctA + ((size_t)(ti * NT + xyzt[j].w) * NA + ch) * KA;
+          // p = sum_k ct_k T_k,  dp = sum_k ct_k k U_{k-1}   (T_k' = k U_{k-1})
+          double T0 = 1.0, T1 = x, U0 = 1.0, U1 = 2.0 * x;
+          double p = ct[0], dp = 0.0;
+          if (KA > 1) { p += ct[1] * x; dp += ct[1]; }
+          for (int k = 2; k < KA; ++k) {
+            const double T2 = 2.0 * x * T1 - T0;
+            p += ct[k] * T2;
+            dp += ct[k] * (double)k * U1;
+            const double U2 = 2.0 * x * U1 - U0;
+            T0 = T1; T1 = T2; U0 = U1; U1 = U2;
+          }
+          const double g = fc * p;
+          const double dg = dfc * p + fc * dxdr * dp;
+          ri = 1.0 / r; ux = d[0] * ri; uy = d[1] * ri; uz = d[2] * ri;
+          blm_and_grad_f64(ux, uy, uz, [&](int lm, double b, double bx, double by, double bz) {
+            const double e = A[lm];
+            Sp += dg * e * b;
+            vx += g * e * bx;
+            vy += g * e * by;
+            vz += g * e * bz;
+          });
         }
-        const double g = own ? fc * p : 0.0;
-        const double dg = own ? dfc * p + fc * dxdr * dp : 0.0;
-        const double ri = 1.0 / r, ux = d[0] * ri, uy = d[1] * ri, uz = d[2] * ri;
-        double Sp = 0.0, vx = 0.0, vy = 0.0, vz = 0.0;
-        blm_and_grad_f64(ux, uy, uz, [&](int lm, double b, double bx, double by, double bz) {
-          const double e = A[lm];
-          Sp += dg * e * b;
-          vx += g * e * bx;
-          vy += g * e * by;
-          vz += g * e * bz;
-        });
-        Sp = warp_sum_f64(Sp);
-        vx = warp_sum_f64(vx);
-        vy = warp_sum_f64(vy);
-        vz = warp_sum_f64(vz);
-        const double uv = ux * vx + uy * vy + uz * vz;
-        px = ux * Sp + (vx - ux * uv) * ri;
-        py = uy * Sp + (vy - uy * uv) * ri;
-        pz = uz * Sp + (vz - uz * uv) * ri;
       }
-      if (lane == 0) pforce[(size_t)a * npad + s] = make_float4((float)px, (float)py, (float)pz, 0.0f);
+      __syncwarp();
+      double tS = 0.0, tx = 0.0, ty = 0.0, tz = 0.0;
+      for (int nq = 0; nq < NA; ++nq) {  // channels of this lane's slice, channel 0 first
+        const int src = slice * NA + nq;
+        tS += __shfl_sync(0xffffffffu, Sp, src);
+        tx += __shfl_sync(0xffffffffu, vx, src);
+        ty += __shfl_sync(0xffffffffu, vy, src);
+        tz += __shfl_sync(0xffffffffu, vz, src);
+      }
+      if (act && ch == 0) {
+        const double uv = ux * tx + uy * ty + uz * tz;
+        const double px = ux * tS + (tx - ux * uv) * ri;
+        const double py = uy * tS + (ty - uy * uv) * ri;
+        const double pz = uz * tS + (tz - uz * uv) * ri;
+        pforce[(size_t)a * npad + s] = make_float4((float)px, (float)py, (float)pz, 0.0f);
+      }
     }
     __syncwarp();
   }

@@ -38,3 +38,14 @@ def compare_neighbor_sets(nn_g, nl_g, pos, box, pbc, rc, oracle, margin=1e-6):
     bad = [i for i in range(len(g)) if not (lo[i] <= g[i] <= hi[i])]
     dup = [i for i in range(len(g)) if len(g[i]) != nn_g[i]]
     return bad, dup, sum(len(h) - len(l) for h, l in zip(hi, lo))
+
+
+def compare_neighbor_sets_sel(nn_g, nl_g, sel, pos, box, pbc, rc, oracle, margin=1e-6):
+    """The same for a selection of atoms of a large system: nn_g / nl_g are the GPU rows of the atoms sel[t]."""
+    cap = nl_g.shape[1] + 64
+    nn_lo, nl_lo = oracle.neighbors(pos, box, pbc, rc - margin, use_cell=True, cap=cap, sel=sel)
+    nn_hi, nl_hi = oracle.neighbors(pos, box, pbc, rc + margin, use_cell=True, cap=cap, sel=sel)
+    lo, hi, g = list_sets(nn_lo, nl_lo), list_sets(nn_hi, nl_hi), list_sets(nn_g, nl_g)
+    bad = [int(sel[t]) for t in range(len(g)) if not (lo[t] <= g[t] <= hi[t])]
+    dup = [int(sel[t]) for t in range(len(g)) if len(g[t]) != nn_g[t]]
+    return bad, dup, sum(len(h) - len(l) for h, l in zip(hi, lo))

@@ -157,7 +157,13 @@ def test_an_evaluation_ends_the_md_session(nb):
     w = wl.thermal_bulk(5, seed=6, sigma_pos=0.03)
     g, pos, vel = _md(nb, w)
     g.md_step(1.0, 0.01)
-    w2 = wl.thermal_bulk(4, seed=7, sigma_pos=0.03)          # another size: stale launch geometry would be fatal
+    w2 = wl.thermal_bulk((5, 5, 6), seed=7, sigma_pos=0.03)  # another size: stale launch geometry would be fatal
+    g2 = nb.NepZbl(w.model, w2.n)
+    p2 = torch.from_numpy(w2.pos.copy()).cuda(); v2 = torch.from_numpy(w2.vel.copy()).cuda()
+    g2.md_init(p2, v2, torch.from_numpy(w2.types).cuda(), w2.box, w2.pbc)
+    g2.md_step(1.0, 0.01)
+    g, pos, vel = g2, p2, v2                                 # the larger handle takes the smaller system
+    w, w2 = w2, w
     g.compute(w2.pos, w2.types, w2.box, w2.pbc)
     assert not g.nep_zbl_uses_graph()
     with pytest.raises(nb.NepZblError) as ei:

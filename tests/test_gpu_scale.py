@@ -26,6 +26,41 @@ def _min_image(d, box, pbc):
     return np.where(p, d - L * np.round(d / L), d)
 
 
+def _neighbor_sets_at_size(nb, w, seed):
+    """Neighbour sets at the config's full box size (fixed-point unit and fp32 distance test are coarsest in the
+    largest boxes): displaced positions (0.1 A Gaussian: pair distances straddle both list cutoffs), GPU rows of a
+    seeded sample of 4 096 atoms plus every atom within 8 A of the PKA against the oracle, bit for bit outside the
+    1e-6 A band (north_star)."""
+    n = w.n
+    L = w.box[[0, 4, 8]][:, None]
+    p = w.pos + wl.rng(seed, 41).standard_normal(w.pos.shape) * 0.1
+    p = np.where(np.asarray(w.pbc, dtype=bool)[:, None], np.mod(p, L), p)
+    g = nb.NepZbl(w.model, n)
+    pos = torch.from_numpy(p).cuda()
+    g.neighbor_build(pos, torch.from_numpy(w.types).cuda(), w.box, w.pbc)
+    pka = w.info["pka_atom"]
+    d = _min_image(p - p[:, [pka]], w.box, w.pbc)
+    near = np.nonzero((d ** 2).sum(axis=0) < 8.0 ** 2)[0]
+    sel = np.union1d(wl.rng(seed, 42).choice(n, size=4096, replace=False), near).astype(np.int32)
+    sel_t = torch.from_numpy(sel.astype(np.int64)).cuda()
+    skin = w.model["skin"]
+    for which, rc in ((0, w.model["rc_radial"] + skin), (1, w.model["rc_angular"] + skin)):
+        nn, nl = g.neighbor_get(which)
+        nn_s, nl_s = nn[sel_t].cpu().numpy(), nl[sel_t].cpu().numpy()
+        del nn, nl
+        bad, dup, amb = parity.compare_neighbor_sets_sel(nn_s, nl_s, sel, p, w.box, w.pbc, rc, oracle)
+        print(f"{w.name}: neighbour sets within {rc} A of {len(sel)} atoms: {int(nn_s.sum())} entries, "
+              f"{amb} pairs inside the 1e-6 A band")
+        assert not bad and not dup, (w.name, which, bad[:5], dup[:5])
+    g.close()
+
+
+@pytest.mark.parametrize("cfg", ["config3", "config4", "config5"])
+def test_neighbor_sets_at_full_box_size(nb, cfg):
+    w = getattr(wl, cfg)()
+    _neighbor_sets_at_size(nb, w, seed={"config3": 3, "config4": 4, "config5": 5}[cfg])
+
+
 def _cascade(nb, w, n_steps, n_sample=2048, seed=11):
     n = w.n
     g = nb.NepZbl(w.model, n)
@@ -65,25 +100,89 @@ def _cascade(nb, w, n_steps, n_sample=2048, seed=11):
           f"rebuilds={rebuilds} zbl_atoms={zbl_atoms} dt0={tr[0]:.5f} fs")
     assert steps == n_steps
     assert abs(e1 - e0) < 1e-3 * w.info["pka_energy_ev"]       # NVE: the PKA energy stays in the system
-    return g
+    return g, pos, p1
+
+
+def _virial_at_size(nb, g, w, p, n_sample=1024, seed=11):
+    """Energy / force / VIRIAL of a plain evaluation at the given positions (this ends the MD session of g) on a
+    seeded sample plus the atoms around the PKA, against the oracle."""
+    pka = w.info["pka_atom"]
+    d = _min_image(p - p[:, [pka]], w.box, w.pbc)
+    near = np.nonzero((d ** 2).sum(axis=0) < 8.0 ** 2)[0]
+    sel = np.union1d(wl.rng(seed, 32).choice(w.n, size=n_sample, replace=False), near).astype(np.int32)
+    e, f, v = g.compute(p, w.types, w.box, w.pbc, virial=True)
+    ref = oracle.compute(oracle.Params(w.model), p, w.types, w.box, w.pbc, sel=sel)
+    r = parity.compare(e, f, v, ref, idx=sel, label=f"{w.name} evaluation with virial")
+    assert max(r.values()) <= 1.0, r
+
+
+def _full_length(nb, w, n_steps):
+    """A cascade config at its full BASELINE.json length: invariants of P:77 during the run (in _cascade), oracle
+    parity of the final state incl. the virial, the list the run ended with still valid, atoms conserved in the
+    Wigner-Seitz count."""
+    g, pos, p1 = _cascade(nb, w, n_steps=n_steps)
+    n = w.n
+    g.wigner_seitz_set_reference(torch.from_numpy(w.pos.copy()).cuda(), w.box, w.pbc)
+    nearest, occ, (nv, ni) = g.wigner_seitz_count(pos)
+    assert nv == ni and int(occ.sum().item()) == n
+    del nearest, occ
+    # the list the run ended with gives the forces of a freshly built one (up to the fp32 summation order)
+    f, e = g.md_get_forces()
+    f, e = f.cpu().numpy(), e.cpu().numpy()
+    reb_before = g.md_get_counters()[1]
+    e2, f2, v2 = g.compute(p1, w.types, w.box, w.pbc, virial=False)       # same list (no displacement since)
+    assert np.array_equal(f, f2) and np.array_equal(e, e2)
+    g2 = nb.NepZbl(w.model, n)
+    e3, f3, _ = g2.compute(p1, w.types, w.box, w.pbc, virial=False)      # fresh list
+    fn = np.sqrt((f3 ** 2).sum(axis=0))
+    assert (np.sqrt(((f - f3) ** 2).sum(axis=0)) / np.maximum(1.0, fn)).max() < 2e-4 and np.abs(e - e3).max() < 2e-5
+    _virial_at_size(nb, g2, w, p1)
+    print(f"{w.name} full length: {n_steps} steps, Frenkel pairs {nv}, rebuilds {reb_before}")
 
 
 def test_config3_one_million_atoms_10keV(nb):
-    g = _cascade(nb, wl.config3(), n_steps=400)                 # 6 A of travel: a close collision (ZBL active)
+    w = wl.config3()
+    g, pos, p1 = _cascade(nb, w, n_steps=400)                   # 6 A of travel: a close collision (ZBL active)
     assert g.md_get_counters()[1] >= 1 + 5                      # md_init's build + one per ~1 A travelled (C-15)
+    _virial_at_size(nb, g, w, p1)
 
 
-def test_config4_eight_million_atoms_100keV(nb):
+def test_config4_eight_million_atoms_100keV_full_length(nb):
     w = wl.config4()
-    assert w.n == 8_192_000
-    g = _cascade(nb, w, n_steps=40)
-    assert g.workspace_bytes < 40 * 2**30                       # fits one B200 many times over
+    assert w.n == 8_192_000 and w.n_steps == 2000
+    _full_length(nb, w, w.n_steps)
 
 
-def test_config5_foil_open_z_100keV(nb):
+def test_config5_foil_open_z_100keV_full_length(nb):
     w = wl.config5()
-    assert w.n == 5_120_000 and list(w.pbc) == [1, 1, 0]
-    _cascade(nb, w, n_steps=40)
+    assert w.n == 5_120_000 and list(w.pbc) == [1, 1, 0] and w.n_steps == 2000
+    _full_length(nb, w, w.n_steps)
+
+
+def test_config2_thousand_nve_steps_energy_drift(nb):
+    """BASELINE.json configs[1]: 1 000 NVE steps at dt = 1 fs, "energy drift".  E_tot every 10 steps: the largest
+    excursion per atom and the linear drift, beside the fp64 oracle's own on a config-1-sized crystal of the same
+    recipe: the integrator sets both, the fp32 forces must not add to them."""
+    w = wl.config2()
+    g = nb.NepZbl(w.model, w.n)
+    pos = torch.from_numpy(w.pos.copy()).cuda(); vel = torch.from_numpy(w.vel.copy()).cuda()
+    g.md_init(pos, vel, torch.from_numpy(w.types).cuda(), w.box, w.pbc)
+    assert g.nep_zbl_uses_graph()
+    et = [sum(g.md_energies())]
+    for _ in range(100):
+        g.md_run(10, w.dt_max, w.max_displacement)
+        et.append(sum(g.md_energies()))
+    et = (np.array(et) - et[0]) / w.n
+    ws = wl.thermal_bulk(10, seed=2)                                       # 2 000 atoms, same recipe
+    _, _, _, oep, oek = oracle.md_run(oracle.Params(ws.model), ws.pos, ws.vel, ws.types, ws.box, ws.pbc, 1000, 1.0, np.inf)
+    ot = ((oep + oek)[::10] - (oep + oek)[0]) / ws.n
+    t_ps = np.arange(101) * 0.01
+    drift_g, drift_o = np.polyfit(t_ps, et, 1)[0], np.polyfit(t_ps, ot, 1)[0]
+    print(f"config2 1000 NVE steps: max|dE|/N = {np.abs(et).max():.3e} eV (oracle, 2 000 atoms: {np.abs(ot).max():.3e}); "
+          f"linear drift {drift_g:.3e} eV/atom/ps (oracle {drift_o:.3e}); rebuilds {g.md_get_counters()[1] - 1}")
+    assert np.abs(et).max() <= 1.5 * np.abs(ot).max() + 2e-6
+    assert abs(drift_g) <= abs(drift_o) + 2e-5
+    assert g.nep_zbl_last_counts() == (0, 0)
 
 
 def test_config3_full_length_cascade(nb):
@@ -97,6 +196,7 @@ def test_config3_full_length_cascade(nb):
     pos = torch.from_numpy(w.pos.copy()).cuda()
     vel = torch.from_numpy(w.vel.copy()).cuda()
     g.md_init(pos, vel, torch.from_numpy(w.types).cuda(), w.box, w.pbc)
+    assert g.nep_zbl_uses_graph()
     g.wigner_seitz_set_reference(torch.from_numpy(w.pos.copy()).cuda(), w.box, w.pbc)
     e0 = sum(g.md_energies())
     tr, nreb = g.md_run(5000, w.dt_max, w.max_displacement, want_trace=True)

@@ -76,3 +76,14 @@ def test_symmetry_of_neighbour_relation():
     for i in range(w.n):
         for j in S[i]:
             assert i in S[j]
+
+
+def test_selection_variant_returns_the_rows_of_the_full_search():
+    # orc_neighbors_sel (used by the at-size GPU tests) has no arithmetic of its own: same rows as the brute force
+    w = wl.config5(seed=5, cells=(6, 6, 4), vacuum=20.0)
+    w.pos = w.pos + wl.rng(5, 21).standard_normal(w.pos.shape) * 0.05
+    sel = wl.rng(5, 40).choice(w.n, size=50, replace=False).astype(np.int32)
+    for rc in (5.0, 7.0):
+        nn, nl = oracle.neighbors(w.pos, w.box, w.pbc, rc, use_cell=False)
+        ns, ls = oracle.neighbors(w.pos, w.box, w.pbc, rc, use_cell=True, sel=sel)
+        assert np.array_equal(ns, nn[sel]) and np.array_equal(ls, nl[sel])
