@@ -36,7 +36,7 @@ class _CParams(C.Structure):
         ("rc_radial", C.c_double), ("rc_angular", C.c_double),
         ("n_max_radial", C.c_int32), ("n_max_angular", C.c_int32),
         ("basis_radial", C.c_int32), ("basis_angular", C.c_int32),
-        ("l_max", C.c_int32), ("has_4body", C.c_int32), ("n_neurons", C.c_int32),
+        ("l_max", C.c_int32), ("has_4body", C.c_int32), ("has_5body", C.c_int32), ("n_neurons", C.c_int32),
         ("c_radial", C.POINTER(C.c_double)), ("c_angular", C.POINTER(C.c_double)),
         ("q_scaler", C.POINTER(C.c_double)),
         ("w0", C.POINTER(C.c_double)), ("b0", C.POINTER(C.c_double)), ("w1", C.POINTER(C.c_double)),
@@ -99,6 +99,7 @@ class Params:
         s.n_max_radial = int(m["n_max_radial"]); s.n_max_angular = int(m["n_max_angular"])
         s.basis_radial = int(m["basis_radial"]); s.basis_angular = int(m["basis_angular"])
         s.l_max = int(m["l_max"]); s.has_4body = int(m["has_4body"]); s.n_neurons = int(m["n_neurons"])
+        s.has_5body = int(m.get("has_5body", 0))
         s.c_radial = _dp(self.c_radial); s.c_angular = _dp(self.c_angular)
         s.q_scaler = _dp(self.q_scaler)
         s.w0 = _dp(self.w0); s.b0 = _dp(self.b0); s.w1 = _dp(self.w1)

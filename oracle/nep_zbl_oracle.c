@@ -55,6 +55,7 @@ typedef struct {
   int32_t basis_radial, basis_angular; /* k = 0..basis  (D:C-2) */
   int32_t l_max;                       /* 3-body l = 1..l_max */
   int32_t has_4body;                   /* (2,2,2) term */
+  int32_t has_5body;                   /* (1,1,1,1) term (D:C-27) */
   int32_t n_neurons;
   const double *c_radial;  /* [n_types][n_types][n_max_R+1][basis_R+1] */
   const double *c_angular; /* [n_types][n_types][n_max_A+1][basis_A+1] */
@@ -74,7 +75,7 @@ typedef struct {
 
 int orc_descriptor_dim(const orc_params *p) {
   return (p->n_max_radial + 1) + (p->n_max_angular + 1) * p->l_max +
-         (p->has_4body ? (p->n_max_angular + 1) : 0);
+         (p->has_4body ? (p->n_max_angular + 1) : 0) + (p->has_5body ? (p->n_max_angular + 1) : 0);
 }
 
 int orc_num_threads(void) {
@@ -201,7 +202,8 @@ static void legendre(int lmax, double c, double *P, double *dP) {
 /*
  * q[D] and (optionally) dq[D][nn][3] = d q_nu / d r_ij for the site of type ti with nn neighbours
  * (types tj[s], displacement vectors d[s][3] = r_j - r_i, all with |d| < rc_radial).
- * Descriptor order (S:C): nu = n (radial); 3-body l-major nu = NR + (l-1)*NA + n; 4-body nu = NR + lmax*NA + n.
+ * Descriptor order (S:C): nu = n (radial); 3-body l-major nu = NR + (l-1)*NA + n; 4-body nu = NR + lmax*NA + n;
+ * 5-body (D:C-27) behind the 4-body block (or in its place if there is none).
  */
 void orc_descriptor_site(const orc_params *p, int ti, int nn, const int32_t *tj, const double *d,
                          double *q, double *dq) {
@@ -312,6 +314,57 @@ void orc_descriptor_site(const orc_params *p, int ti, int nn, const int32_t *tj,
         }
       }
     }
+  }
+  /* 5-body (D:C-27), the (l1 l2 l3 l4) = (1 1 1 1) term of the NEP formulation the paper defers to: four
+   * l = 1 densities coupled pairwise to scalars,
+   *   q_n = sum_{m1 m2 m3 m4} (1 1 0; m1 m2 0)(1 1 0; m3 m4 0) A_1m1 A_1m2 A_1m3 A_1m4,
+   * which written out over the neighbours is the five-body correlation
+   *   q_n = 1/3 (3/4pi)^2 sum_j sum_k sum_l sum_m  (v_j . v_k)(v_l . v_m),   v_j = g_n(r_ij) rh_ij
+   * (pinned against the 3j form in tests/test_oracle_angular.py).  Plain quadruple sum; the derivative uses that the
+   * sum is symmetric in its four indices: d/dr_ij = 4 x (the terms with j in the first place). */
+  if (p->has_5body) {
+    const double c5 = (1.0 / 3.0) * (3.0 / (4.0 * ORC_PI)) * (3.0 / (4.0 * ORC_PI));
+    double *v = (double *)malloc(sizeof(double) * nn * 3);
+    for (int n = 0; n < NA; ++n) {
+      for (int j = 0; j < nn; ++j)
+        for (int a = 0; a < 3; ++a) v[3 * j + a] = isA[j] ? gA[(size_t)j * NA + n] * rh[3 * j + a] : 0.0;
+      double q5 = 0.0;
+      for (int j = 0; j < nn; ++j) {
+        if (!isA[j]) continue;
+        for (int k = 0; k < nn; ++k) {
+          if (!isA[k]) continue;
+          double vjk = v[3 * j] * v[3 * k] + v[3 * j + 1] * v[3 * k + 1] + v[3 * j + 2] * v[3 * k + 2];
+          for (int l = 0; l < nn; ++l) {
+            if (!isA[l]) continue;
+            for (int m = 0; m < nn; ++m) {
+              if (!isA[m]) continue;
+              q5 += vjk * (v[3 * l] * v[3 * m] + v[3 * l + 1] * v[3 * m + 1] + v[3 * l + 2] * v[3 * m + 2]);
+            }
+          }
+        }
+      }
+      int vi = NR + L * NA + (p->has_4body ? NA : 0) + n;
+      q[vi] = c5 * q5;
+      if (dq) {
+        /* sum_k v_k and sum_lm v_l . v_m do not depend on j */
+        double sv[3] = {0.0, 0.0, 0.0}, w2;
+        for (int k = 0; k < nn; ++k)
+          for (int a = 0; a < 3; ++a) sv[a] += v[3 * k + a];
+        w2 = sv[0] * sv[0] + sv[1] * sv[1] + sv[2] * sv[2];
+        for (int j = 0; j < nn; ++j) {
+          if (!isA[j]) continue;
+          double g = gA[(size_t)j * NA + n], dg = dgA[(size_t)j * NA + n];
+          const double *h = rh + 3 * j;
+          double hs = h[0] * sv[0] + h[1] * sv[1] + h[2] * sv[2];
+          for (int a = 0; a < 3; ++a) {
+            /* d v_j / d r_ij^a = g' rh^a rh + g (e_a - rh^a rh) / r, dotted with sum_k v_k */
+            double t = dg * h[a] * hs + g * (sv[a] - h[a] * hs) / r[j];
+            dq[((size_t)vi * nn + j) * 3 + a] = 4.0 * c5 * t * w2;
+          }
+        }
+      }
+    }
+    free(v);
   }
   free(r);
   free(rh);

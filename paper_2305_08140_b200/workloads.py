@@ -40,7 +40,7 @@ def synthetic_model(seed: int = 121, n_max_radial: int = 4, n_max_angular: int =
                     basis_radial: int = 8, basis_angular: int = 8, l_max: int = 4,
                     has_4body: int = 1, n_neurons: int = 50, zbl: str = "universal",
                     n_types: int = 1, skin: float = 1.0, cap_radial: int = 128,
-                    cap_angular: int = 64) -> dict:
+                    cap_angular: int = 64, has_5body: int = 0) -> dict:
     """Synthetic NEP-ZBL parameter set of BASELINE.json configs[0]: all c_nk and NN weights
     U(-0.5, 0.5) from the seed; q_scaler = block constants of SURVEY 8(c) C-6.
 
@@ -50,7 +50,7 @@ def synthetic_model(seed: int = 121, n_max_radial: int = 4, n_max_angular: int =
     keeps its structure and conserves energy for 1.5 ps, so configs 2-5 stay bcc-shaped."""
     g = rng(seed, 1)
     NR, NA = n_max_radial + 1, n_max_angular + 1
-    D = NR + NA * l_max + (NA if has_4body else 0)
+    D = NR + NA * l_max + (NA if has_4body else 0) + (NA if has_5body else 0)
     u = lambda *shape: g.uniform(-0.5, 0.5, size=shape)
     c_radial = u(n_types, n_types, NR, basis_radial + 1)
     c_angular = u(n_types, n_types, NA, basis_angular + 1)
@@ -63,13 +63,15 @@ def synthetic_model(seed: int = 121, n_max_radial: int = 4, n_max_angular: int =
     for l in range(1, l_max + 1):
         q_scaler[NR + (l - 1) * NA: NR + l * NA] = 100.0 if l <= 3 else 3.0
     if has_4body:
-        q_scaler[NR + l_max * NA:] = 1.0e4
+        q_scaler[NR + l_max * NA: NR + (l_max + 1) * NA] = 1.0e4
+    if has_5body:      # q5 = q_{l=1}^2 / 3 ~ 1e-7 on thermal bcc sites: 1e6 brings it to the 0.1-0.3 of the other blocks
+        q_scaler[D - NA:] = 1.0e6
     z = dict(ZBL_UNIVERSAL if zbl == "universal" else ZBL_PAPER_W)
     return dict(
         n_types=n_types, rc_radial=6.0, rc_angular=4.0,
         n_max_radial=n_max_radial, n_max_angular=n_max_angular,
         basis_radial=basis_radial, basis_angular=basis_angular,
-        l_max=l_max, has_4body=has_4body, n_neurons=n_neurons,
+        l_max=l_max, has_4body=has_4body, has_5body=has_5body, n_neurons=n_neurons,
         c_radial=c_radial, c_angular=c_angular, q_scaler=q_scaler,
         w0=w0, b0=b0, w1=w1, b1=b1,
         zbl_enabled=1, zbl_r_inner=1.0, zbl_r_outer=2.0,

@@ -158,3 +158,49 @@ def test_network_hand_computed_and_gradient():
         e = np.zeros(P.D); e[v] = 1e-6
         fd = (oracle.site_energy(P, q + e)[0] - oracle.site_energy(P, q - e)[0]) / 2e-6
         assert Fp[v] == pytest.approx(fd, rel=1e-7, abs=1e-9)
+
+
+# ------------------------------------------------------------------ 5-body term (C-27)
+
+def _five_body_model():
+    return wl.synthetic_model(has_5body=1)
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_five_body_equals_wigner_3j_contraction(seed):
+    # q^{1111}_n = sum_{m1..m4} (1 1 0; m1 m2 0)(1 1 0; m3 m4 0) A_1m1 A_1m2 A_1m3 A_1m4 with orthonormal complex Y_1m:
+    # the library 3j symbols and spherical harmonics against the oracle's quadruple sum over neighbours
+    from sympy.physics.wigner import wigner_3j
+    P = oracle.Params(_five_body_model())
+    assert P.D == 35
+    d = _random_neighbourhood(seed)
+    q = oracle.descriptor_site(P, d)
+    A = _A_nlm(P, d)
+    pair = 0
+    for m1 in (-1, 0, 1):
+        pair = pair + float(wigner_3j(1, 1, 0, m1, -m1, 0)) * A[(1, m1)] * A[(1, -m1)]
+    ref = pair * pair
+    assert np.abs(ref.imag).max() < 1e-14
+    assert q[NR + (LMAX + 1) * NA:] == pytest.approx(ref.real, rel=1e-11, abs=1e-18)
+    # and, by the addition theorem, one third of the squared l = 1 three-body component
+    assert q[NR + (LMAX + 1) * NA:] == pytest.approx(q[NR:NR + NA] ** 2 / 3.0, rel=1e-12, abs=1e-18)
+
+
+def test_five_body_single_neighbour_cubic_site_and_derivative():
+    P = oracle.Params(_five_body_model())
+    r = 2.7
+    g, _ = oracle.radial_functions(P, 1, r)
+    q = oracle.descriptor_site(P, np.array([[0.0, r, 0.0]]))
+    assert q[30:] == pytest.approx((3.0 / (4 * np.pi) * g ** 2) ** 2 / 3.0, rel=1e-13)      # one neighbour: v.v = g^2
+    a = wl.A0_CONFIG                                                                          # cubic site: sum_j v_j = 0
+    pts = np.array([[i, j, k] for i in (-1, 1) for j in (-1, 1) for k in (-1, 1)]) * a / 2
+    assert np.abs(oracle.descriptor_site(P, pts)[30:]).max() < 1e-18      # rounding of the cancelling quadruple sum
+    d = _random_neighbourhood(7, nn=9, rmax=5.0)
+    q, dq = oracle.descriptor_site(P, d, want_dq=True)
+    h = 1e-6
+    for j in range(len(d)):
+        for a_ in range(3):
+            dp = d.copy(); dp[j, a_] += h
+            dm = d.copy(); dm[j, a_] -= h
+            fd = (oracle.descriptor_site(P, dp) - oracle.descriptor_site(P, dm)) / (2 * h)
+            assert dq[30:, j, a_] == pytest.approx(fd[30:], rel=2e-6, abs=1e-12)

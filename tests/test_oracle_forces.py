@@ -252,3 +252,30 @@ def test_two_types_reduce_to_one_type_and_relabel():
     # and the two types really differ: the unswapped labels give other energies
     e = oracle.compute(oracle.Params(m), w.pos, 1 - w.types, w.box, w.pbc, use_cell=False)
     assert np.abs(e.energy - c.energy).max() > 1e-3
+
+
+def test_five_body_model_forces_and_virial_by_finite_differences():
+    # SURVEY 8(f) NEXT-4 / DESIGN C-27: the model with the (1,1,1,1) term, all 3N coordinates and the strain virial
+    w = wl.config1(seed=13, cells=3, n_pairs=1, sigma=0.08, model=wl.synthetic_model(has_5body=1))
+    P = oracle.Params(w.model)
+    res = oracle.compute(P, w.pos, w.types, w.box, w.pbc, use_cell=False)
+    h = 1e-4
+    fd = np.zeros_like(res.force)
+    for a in range(3):
+        for k in range(w.n):
+            pp = w.pos.copy(); pp[a, k] += h
+            pm = w.pos.copy(); pm[a, k] -= h
+            fd[a, k] = -(_etot(P, w, pp) - _etot(P, w, pm)) / (2 * h)
+    assert np.abs(fd - res.force).max() < 2e-6 * np.abs(res.force).max()
+    W = res.virial.sum(axis=1)
+    e = 1e-6
+    for a in range(3):
+        def E(eps):
+            pos = w.pos.copy(); pos[a] *= (1 + eps)
+            box = w.box.copy(); box[4 * a] *= (1 + eps)
+            return _etot(P, w, pos, box)
+        assert W[4 * a] == pytest.approx(-(E(e) - E(-e)) / (2 * e), rel=1e-6)
+    # the block matters: zeroing its W0 columns changes the energies
+    m0 = dict(w.model); w0 = m0["w0"].copy(); w0[:, 30:] = 0.0; m0["w0"] = w0
+    r0 = oracle.compute(oracle.Params(m0), w.pos, w.types, w.box, w.pbc, use_cell=False, want_force=False, want_virial=False)
+    assert np.abs(r0.energy - res.energy).max() > 1e-3
