@@ -57,15 +57,17 @@ enum {
  * NEP-ZBL site energy (Eq. 1): U_i = U_i^NEP({q}) + 1/2 sum_j U_ZBL(r_ij).
  * Hyper-parameters as listed in P:106; functional forms per S:B-S:D (the paper defers them to its
  * ref. [25]).  Descriptor order (S:C): radial n = 0..n_max_radial; 3-body l-major
- * (l = 1..l_max, n = 0..n_max_angular); then the (2,2,2) 4-body term n = 0..n_max_angular.
+ * (l = 1..l_max, n = 0..n_max_angular); then the (2,2,2) 4-body term n = 0..n_max_angular; then the (1,1,1,1)
+ * 5-body term n = 0..n_max_angular.
  */
 typedef struct {
-  int32_t n_types;                     /* 1 or 2 in this build (2: config-sized model shape only) */
+  int32_t n_types;                     /* 1 or 2 in this build */
   double rc_radial, rc_angular;        /* cutoffs r_c^R, r_c^A (6.0, 4.0 A) */
   int32_t n_max_radial, n_max_angular; /* n = 0..n_max */
   int32_t basis_radial, basis_angular; /* Chebyshev basis k = 0..basis (D: C-2) */
   int32_t l_max;                       /* Legendre order of the 3-body part (4) */
   int32_t has_4body;                   /* 1: (l1,l2,l3) = (2,2,2) term */
+  int32_t has_5body;                   /* 1: (l1,l2,l3,l4) = (1,1,1,1) term behind the 4-body block (D: C-27) */
   int32_t n_neurons;                   /* hidden tanh neurons */
   const double *c_radial;              /* [n_types][n_types][n_max_radial+1][basis_radial+1] */
   const double *c_angular;             /* [n_types][n_types][n_max_angular+1][basis_angular+1] */

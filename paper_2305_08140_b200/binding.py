@@ -45,7 +45,7 @@ class _CParams(C.Structure):
         ("rc_radial", C.c_double), ("rc_angular", C.c_double),
         ("n_max_radial", C.c_int32), ("n_max_angular", C.c_int32),
         ("basis_radial", C.c_int32), ("basis_angular", C.c_int32),
-        ("l_max", C.c_int32), ("has_4body", C.c_int32), ("n_neurons", C.c_int32),
+        ("l_max", C.c_int32), ("has_4body", C.c_int32), ("has_5body", C.c_int32), ("n_neurons", C.c_int32),
         ("c_radial", C.c_void_p), ("c_angular", C.c_void_p), ("q_scaler", C.c_void_p),
         ("w0", C.c_void_p), ("b0", C.c_void_p), ("w1", C.c_void_p),
         ("b1", C.c_double),
@@ -155,6 +155,7 @@ class NepZbl:
         p.n_max_radial = int(m["n_max_radial"]); p.n_max_angular = int(m["n_max_angular"])
         p.basis_radial = int(m["basis_radial"]); p.basis_angular = int(m["basis_angular"])
         p.l_max = int(m["l_max"]); p.has_4body = int(m["has_4body"]); p.n_neurons = int(m["n_neurons"])
+        p.has_5body = int(m.get("has_5body", 0))
         for k in ("c_radial", "c_angular", "q_scaler", "w0", "b0", "w1", "atomic_number", "mass"):
             setattr(p, k, f64(k).ctypes.data)
         p.b1 = float(m["b1"])

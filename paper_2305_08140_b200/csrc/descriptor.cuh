@@ -19,7 +19,7 @@
 #pragma once
 #include "common.cuh"
 
-template <int NR_, int KR_, int NA_, int KA_, bool B4_, int NT_ = 1>
+template <int NR_, int KR_, int NA_, int KA_, bool B4_, int NT_ = 1, bool B5_ = false>
 struct ModelShape {
   static constexpr int NT = NT_;  // atom types (2 = the type-pair tables c^{ti tj}_nk are exercised)
   static constexpr int NR = NR_;  // n_max_radial + 1
@@ -27,9 +27,11 @@ struct ModelShape {
   static constexpr int NA = NA_;
   static constexpr int KA = KA_;
   static constexpr bool B4 = B4_;
+  static constexpr bool B5 = B5_;  // (1,1,1,1) 5-body term q_n = q_{n,l=1}^2 / 3 (C-27), behind the 4-body block
   static constexpr int LMAX = 4;
   static constexpr int NLM = 24;
-  static constexpr int D = NR + NA * LMAX + (B4 ? NA : 0);
+  static constexpr int D = NR + NA * LMAX + (B4 ? NA : 0) + (B5 ? NA : 0);
+  static constexpr int V5 = NR + NA * LMAX + (B4 ? NA : 0);  // first 5-body component
   static constexpr int DPAD = (D + 3) / 4 * 4;
   // record gathered per radial pair by k_force: {position, Fp[0..NR-1]} in ONE 32-byte sector when the
   // radial descriptor has at most 5 components, else {position, d[0..KR-1]} in 64 bytes (AtomRec)
@@ -528,6 +530,12 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       for (int lm = 0; lm < 24; ++lm) ql[lm_to_l(lm) - 1] = fmaf(kClm[lm] * A[nq][lm], A[nq][lm], ql[lm_to_l(lm) - 1]);
 #pragma unroll
       for (int l = 0; l < 4; ++l) q[NR + l * NA + nq] = ql[l];
+      if (MS::B5) q[MS::B5 ? MS::V5 + nq : 0] = ql[0] * ql[0] * (1.0f / 3.0f);
+    }
+    float q1u[MS::B5 ? NA : 1];     // unscaled q_{n,l=1}: d q5_n / d q_{n1} = 2/3 q_{n1}
+    if (MS::B5) {
+#pragma unroll
+      for (int nq = 0; nq < NA; ++nq) q1u[nq] = q[NR + nq];
     }
     float dq4[MS::B4 ? NA : 1][5];  // d q4_n / d A[n][3..7]
     if (MS::B4) {
@@ -647,9 +655,10 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     // ---- E[n][lm] = dU/dA[n][lm] (in place)
 #pragma unroll
     for (int nq = 0; nq < NA; ++nq) {
+      const float f5 = MS::B5 ? Fp[MS::B5 ? MS::V5 + nq : 0] * (2.0f / 3.0f) * q1u[MS::B5 ? nq : 0] : 0.0f;
 #pragma unroll
       for (int lm = 0; lm < 24; ++lm)
-        A[nq][lm] *= 2.0f * kClm[lm] * Fp[NR + (lm_to_l(lm) - 1) * NA + nq];
+        A[nq][lm] *= 2.0f * kClm[lm] * (Fp[NR + (lm_to_l(lm) - 1) * NA + nq] + (lm < 3 ? f5 : 0.0f));
       if (MS::B4) {
 #pragma unroll
         for (int m5 = 0; m5 < 5; ++m5) A[nq][3 + m5] = fmaf(Fp[NR + 4 * NA + nq], dq4[nq][m5], A[nq][3 + m5]);

@@ -50,9 +50,11 @@ struct SplitLayout {
   }
   // rows of the weight table: n_neurons rounded up to a multiple of 4 (one neuron per lane per round)
   __host__ __device__ static constexpr int rows(int n_neurons) { return (n_neurons + 3) & ~3; }
-  // table (floats): w0 [nrow][4][SLS] | b0 [nrow] | w1 [nrow] | q_scaler [4][SLS] | ctA [NAP][KA] | ctR [4 RSUB][KR]
+  // table (floats): w0 [nrow][4][SLS] | b0 [nrow] | w1 [nrow] | q_scaler [4][SLS] | ctA [NT*NT][NAP][KA] |
+  // ctR [NT*NT][4 RSUB][KR]   (leading index of the coefficient tables: ordered type pair ti * NT + tj)
+  static constexpr int NPR = MS::NT * MS::NT;
   __host__ __device__ static constexpr int table_floats(int nrow) {
-    return nrow * 4 * SLS + 2 * nrow + 4 * SLS + NAP * MS::KA + 4 * RSUB * MS::KR;
+    return nrow * 4 * SLS + 2 * nrow + 4 * SLS + NPR * (NAP * MS::KA + 4 * RSUB * MS::KR);
   }
   // A[NSUB][24] is parked in shared memory while the network runs: [NSUB * 24][SPLIT_THREADS] floats
   __host__ __device__ static constexpr int stash_floats() { return NSUB * 24 * SPLIT_THREADS; }
@@ -67,7 +69,8 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
                    AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out,
                    const DenseArgs da) {
   using LY = SplitLayout<MS>;
-  static_assert(MS::NT == 1, "the four-lane kernel is instantiated for one atom type");
+  static_assert(!MS::B5, "the four-lane kernel has no 5-body slice entries yet");
+  constexpr int NT = MS::NT;
   constexpr int KA = MS::KA, NR = MS::NR, KR = MS::KR;
   constexpr int NSUB = LY::NSUB, RSUB = LY::RSUB, SLP = LY::SLP, SLS = LY::SLS, NAP = LY::NAP;
   extern __shared__ __align__(16) float smem[];
@@ -76,8 +79,8 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
   float* s_b0 = s_w0 + nrow * 4 * SLS;    // [nrow]
   float* s_w1 = s_b0 + nrow;              // [nrow]
   float* s_qs = s_w1 + nrow;              // [4][SLS]
-  float* s_ct = s_qs + 4 * SLS;           // [NAP][KA], rows >= NA zero
-  float* s_ctr = s_ct + NAP * KA;         // [4 RSUB][KR], rows >= NR zero
+  float* s_ct = s_qs + 4 * SLS;           // [NT*NT][NAP][KA], rows >= NA zero
+  float* s_ctr = s_ct + LY::NPR * NAP * KA;  // [NT*NT][4 RSUB][KR], rows >= NR zero
   float* s_stash = smem + LY::table_floats(nrow) + threadIdx.x;  // this thread's column of the A stash
   {  // the host lays the table out in exactly this order (build_nnw); its size is a multiple of 4 floats
     const int n4 = LY::table_floats(nrow) / 4;
@@ -99,6 +102,7 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
     const unsigned long long mask = valid ? amask[sc_] : 0ull;
     const int nc = __popcll(mask);
     const float4* dp = adisp + sc_;
+    const int ti = NT > 1 ? xyzt[sc_].w : 0;  // central atom's type: selects the c^{ti tj} tables per neighbour
     // ---- S4 forward: A[j][lm] = sum_neighbours g_{n_j}(r) b_lm(rhat)
     float A[NSUB][24];
 #pragma unroll
@@ -122,11 +126,12 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
         float fc, T[KA], b[24];
         cheb_T_fwd<KA>(r, mt.inv_rcA, fc, T);
         eval_blm(d.x * rinv, d.y * rinv, d.z * rinv, b);
+        const float* cts = s_ct + (NT > 1 ? (ti * NT + __float_as_int(d.w)) * NAP * KA : 0);  // adisp.w = neighbour type
 #pragma unroll
         for (int j = 0; j < NSUB; ++j) {
           float g = 0.0f;
 #pragma unroll
-          for (int k = 0; k < KA; ++k) g = fmaf(ct[j][k], T[k], g);
+          for (int k = 0; k < KA; ++k) g = fmaf(NT > 1 ? cts[(sub + SPLIT_LANES * j) * KA + k] : ct[j][k], T[k], g);
           g *= fc;
 #pragma unroll
           for (int lm = 0; lm < 24; ++lm) A[j][lm] = fmaf(g, b[lm], A[j][lm]);
@@ -259,38 +264,43 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
     // ---- per-atom outputs: site energy and the record for k_force's radial pass.  The radial dU/dq are spread
     //      over the quad: every lane contracts its RSUB components, a fixed-order butterfly adds the four parts.
     {
-      float d[12];
+      if (valid && sub == 0) u_site[s] = U;
+      // one record per PARTNER type tp (NT > 1: d^(tp)_k = sum_n Fp_n ct^{ti tp}_nk, as k_angular_nn writes them)
 #pragma unroll
-      for (int k = 0; k < 12; ++k) d[k] = 0.0f;
-      if (MS::FPREC) {  // record holds Fp[0..4] itself: component n sits on lane n / RSUB, entry n % RSUB
+      for (int tp = 0; tp < NT; ++tp) {
+        float d[12];
 #pragma unroll
-        for (int nq = 0; nq < 5; ++nq)
-          if (nq < NR) d[nq] = __shfl_sync(0xffffffffu, Fp[4 * NSUB + (nq < NR ? nq % RSUB : 0)], qbase + (nq < NR ? nq / RSUB : 0));
-      } else {
-        static_assert(KR <= 12, "AtomRec holds 12 coefficients");
+        for (int k = 0; k < 12; ++k) d[k] = 0.0f;
+        if (MS::FPREC) {  // record holds Fp[0..4] itself: component n sits on lane n / RSUB, entry n % RSUB
 #pragma unroll
-        for (int k = 0; k < KR; ++k) {
-          float t = 0.0f;
-#pragma unroll
-          for (int i = 0; i < RSUB; ++i) t = fmaf(Fp[4 * NSUB + i], s_ctr[(RSUB * sub + i) * KR + k], t);
-          t += __shfl_xor_sync(0xffffffffu, t, 1);
-          t += __shfl_xor_sync(0xffffffffu, t, 2);
-          d[k] = t;
-        }
-      }
-      if (valid && sub == 0) {
-        u_site[s] = U;
-        const int4 me = xyzt[s];
-        if (MS::FPREC) {
-          float4* rp = reinterpret_cast<float4*>(reinterpret_cast<char*>(rec) + (size_t)s * 32);
-          rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
-          rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+          for (int nq = 0; nq < 5; ++nq)
+            if (nq < NR) d[nq] = __shfl_sync(0xffffffffu, Fp[4 * NSUB + (nq < NR ? nq % RSUB : 0)], qbase + (nq < NR ? nq / RSUB : 0));
         } else {
-          float4* rp = reinterpret_cast<float4*>(rec + s);
-          rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
-          rp[1] = make_float4(d[1], d[2], d[3], d[4]);
-          rp[2] = make_float4(d[5], d[6], d[7], d[8]);
-          if (KR > 9) rp[3] = make_float4(d[9], d[10], d[11], 0.0f);
+          static_assert(KR <= 12, "AtomRec holds 12 coefficients");
+          const float* ctr = s_ctr + (NT > 1 ? (ti * NT + tp) * 4 * RSUB * KR : 0);
+#pragma unroll
+          for (int k = 0; k < KR; ++k) {
+            float t = 0.0f;
+#pragma unroll
+            for (int i = 0; i < RSUB; ++i) t = fmaf(Fp[4 * NSUB + i], ctr[(RSUB * sub + i) * KR + k], t);
+            t += __shfl_xor_sync(0xffffffffu, t, 1);
+            t += __shfl_xor_sync(0xffffffffu, t, 2);
+            d[k] = t;
+          }
+        }
+        if (valid && sub == 0) {
+          const int4 me = xyzt[s];
+          if (MS::FPREC) {
+            float4* rp = reinterpret_cast<float4*>(reinterpret_cast<char*>(rec) + (size_t)s * 32);
+            rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
+            rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+          } else {
+            float4* rp = reinterpret_cast<float4*>(rec + (size_t)NT * s + tp);
+            rp[0] = make_float4(__int_as_float(me.x), __int_as_float(me.y), __int_as_float(me.z), d[0]);
+            rp[1] = make_float4(d[1], d[2], d[3], d[4]);
+            rp[2] = make_float4(d[5], d[6], d[7], d[8]);
+            if (KR > 9 || NT > 1) rp[3] = make_float4(d[9], d[10], d[11], __int_as_float(me.w));
+          }
         }
       }
     }
@@ -327,6 +337,7 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       for (unsigned long long m = mask; m; m &= m - 1, ++c) {
         const int a = __ffsll((long long)m) - 1;
         const float dx = nx.x, dy = nx.y, dz = nx.z;
+        const float* cts = ctp + (NT > 1 ? (ti * NT + __float_as_int(nx.w)) * NAP * KA : 0);
         nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;
         float r2 = dx * dx + dy * dy + dz * dz;
         float rinv = rsqrtf(r2), r = r2 * rinv;
@@ -343,9 +354,9 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
         for (int j = 0; j < NSUB; ++j) {
           float p = 0.0f, dpk = 0.0f;
 #pragma unroll
-          for (int k = 0; k < KA; ++k) p = fmaf(ct[j][k], T[k], p);
+          for (int k = 0; k < KA; ++k) p = fmaf(NT > 1 ? cts[(sub + SPLIT_LANES * j) * KA + k] : ct[j][k], T[k], p);
 #pragma unroll
-          for (int k = 1; k < KA; ++k) dpk = fmaf(ct[j][k], kU[k], dpk);
+          for (int k = 1; k < KA; ++k) dpk = fmaf(NT > 1 ? cts[(sub + SPLIT_LANES * j) * KA + k] : ct[j][k], kU[k], dpk);
           g[j] = fc * p;
           dg[j] = fmaf(dfc, p, e * dpk);
         }

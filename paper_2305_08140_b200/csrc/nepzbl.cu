@@ -36,7 +36,7 @@ struct Carve {  // byte offsets into the workspace
 };
 
 struct ShapeId {
-  int nr, kr, na, ka, b4, nt;
+  int nr, kr, na, ka, b4, nt, b5;
 };
 
 }  // namespace
@@ -207,18 +207,23 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
 
 // instantiated model shapes: BASELINE.json configs (with / without the 4-body term) and the paper's own
 // sizes (n_max 15 / 10, l_max 4; basis 8 / 8 is DESIGN.md C-26) -- SURVEY 8(f) NEXT-2
-const ShapeId kShapes[] = {{5, 9, 5, 9, 1, 1}, {5, 9, 5, 9, 0, 1}, {16, 9, 11, 9, 0, 1}, {5, 9, 5, 9, 1, 2}};
+const ShapeId kShapes[] = {{5, 9, 5, 9, 1, 1, 0}, {5, 9, 5, 9, 0, 1, 0}, {16, 9, 11, 9, 0, 1, 0}, {5, 9, 5, 9, 1, 2, 0},
+                           {5, 9, 5, 9, 1, 1, 1}, {16, 9, 11, 9, 0, 2, 0}};
 using MS0 = ModelShape<5, 9, 5, 9, true>;
 using MS1 = ModelShape<5, 9, 5, 9, false>;
 using MS2 = ModelShape<16, 9, 11, 9, false>;
-using MS3 = ModelShape<5, 9, 5, 9, true, 2>;  // two atom types
+using MS3 = ModelShape<5, 9, 5, 9, true, 2>;         // two atom types
+using MS4 = ModelShape<5, 9, 5, 9, true, 1, true>;   // 4-body + 5-body terms (NEXT-4, C-27)
+using MS5 = ModelShape<16, 9, 11, 9, false, 2>;      // paper-sized model with two atom types (NEXT-4)
 template <class F>
 void with_shape(int shape, F&& f) {
   switch (shape) {
     case 0: f(MS0{}); break;
     case 1: f(MS1{}); break;
     case 2: f(MS2{}); break;
-    default: f(MS3{}); break;
+    case 3: f(MS3{}); break;
+    case 4: f(MS4{}); break;
+    default: f(MS5{}); break;
   }
 }
 // models with more than 5 angular channels use the four-lanes-per-atom kernel (descriptor_split.cuh)
@@ -301,7 +306,7 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
     float* w1 = b0 + nrow;
     float* qs = w1 + nrow;
     float* cta = qs + 4 * LY::SLS;
-    float* ctr = cta + LY::NAP * MS::KA;
+    float* ctr = cta + LY::NPR * LY::NAP * MS::KA;
     for (int lane = 0; lane < 4; ++lane)
       for (int idx = 0; idx < LY::SLP; ++idx) {
         const int nu = LY::nu(lane, idx);
@@ -314,10 +319,14 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
       b0[m] = (float)p->b0[m];
       w1[m] = (float)p->w1[m];
     }
-    for (int nq = 0; nq < MS::NA; ++nq)
-      for (int k = 0; k < MS::KA; ++k) cta[nq * MS::KA + k] = (float)folded(p->c_angular, MS::KA, nq, k);
-    for (int nq = 0; nq < MS::NR; ++nq)
-      for (int k = 0; k < MS::KR; ++k) ctr[nq * MS::KR + k] = (float)folded(p->c_radial, MS::KR, nq, k);
+    for (int pr = 0; pr < LY::NPR; ++pr) {  // params: [ti][tj][n][k]
+      for (int nq = 0; nq < MS::NA; ++nq)
+        for (int k = 0; k < MS::KA; ++k)
+          cta[((size_t)pr * LY::NAP + nq) * MS::KA + k] = (float)folded(p->c_angular + (size_t)pr * MS::NA * MS::KA, MS::KA, nq, k);
+      for (int nq = 0; nq < MS::NR; ++nq)
+        for (int k = 0; k < MS::KR; ++k)
+          ctr[((size_t)pr * 4 * LY::RSUB + nq) * MS::KR + k] = (float)folded(p->c_radial + (size_t)pr * MS::NR * MS::KR, MS::KR, nq, k);
+    }
     return w;
   } else {
     const int neu2 = nn_rows(p->n_neurons);  // zero padding rows, see nn_rows
@@ -351,6 +360,7 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
 template <class MS>
 std::vector<double> build_site_tables(const nepzbl_params* p, SiteModel* sm, size_t off[6]) {
   sm->NT = MS::NT; sm->NR = MS::NR; sm->KR = MS::KR; sm->NA = MS::NA; sm->KA = MS::KA; sm->B4 = MS::B4 ? 1 : 0;
+  sm->B5 = MS::B5 ? 1 : 0;
   sm->D = MS::D; sm->n_neurons = p->n_neurons; sm->fprec = MS::FPREC ? 1 : 0;
   sm->b1 = p->b1; sm->rcA = p->rc_angular;
   const int npr = MS::NT * MS::NT;
@@ -678,11 +688,11 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   for (int k = 0; k < (int)(sizeof kShapes / sizeof kShapes[0]); ++k)
     if (kShapes[k].nr == p->n_max_radial + 1 && kShapes[k].kr == p->basis_radial + 1 &&
         kShapes[k].na == p->n_max_angular + 1 && kShapes[k].ka == p->basis_angular + 1 &&
-        kShapes[k].b4 == (p->has_4body != 0) && kShapes[k].nt == p->n_types)
+        kShapes[k].b4 == (p->has_4body != 0) && kShapes[k].nt == p->n_types && kShapes[k].b5 == (p->has_5body != 0))
       shape = k;
   if (shape < 0)
-    return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d with %d atom type(s) is not instantiated in this build",
-                p->n_max_radial, p->n_max_angular, p->basis_radial, p->basis_angular, p->has_4body, p->n_types);
+    return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d 5body %d with %d atom type(s) is not instantiated in this build",
+                p->n_max_radial, p->n_max_angular, p->basis_radial, p->basis_angular, p->has_4body, p->has_5body, p->n_types);
   if (p->n_neurons < 1 || p->n_neurons > 256) return fail(h, NEPZBL_E_INVALID_ARG, "n_neurons out of range");
   if (p->cap_angular < 1 || p->cap_angular > 64 || p->cap_radial < 1 || p->cap_radial > 1024)
     return fail(h, NEPZBL_E_INVALID_ARG, "cap_angular must be in 1..64, cap_radial in 1..1024");

@@ -19,7 +19,7 @@
 #include "descriptor.cuh"
 
 struct SiteModel {  // tables are library-owned device arrays of doubles
-  int NT, NR, KR, NA, KA, B4, D, n_neurons;
+  int NT, NR, KR, NA, KA, B4, B5, D, n_neurons;
   int fprec;           // 1: 32-byte record {position, Fp[0..4]} (ModelShape::FPREC), 0: 64-byte AtomRec per partner type
   const double* ctA;   // folded angular coefficients [NT*NT][NA][KA]
   const double* ctR;   // folded radial coefficients  [NT*NT][NR][KR]
@@ -193,6 +193,7 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
 #pragma unroll
       for (int l = 0; l < 4; ++l) xs[NR + l * NA + ch] = ql[l];
       if (sm.B4) xs[NR + 4 * NA + ch] = q4;
+      if (sm.B5) xs[NR + (4 + sm.B4) * NA + ch] = ql[0] * ql[0] / 3.0;  // (1,1,1,1) term, C-27
     }
     for (int nq = lane; nq < NR; nq += 32) xs[nq] = (double)q_radial[(size_t)nq * npad + s];
     __syncwarp();
@@ -244,9 +245,10 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
     }
 
     // ---- E[lm] = dU/dA[ch][lm] (in place; the same on every slice of the channel)
+    const double f5 = (sm.B5 && own) ? Fp[NR + (4 + sm.B4) * NA + ch] * (2.0 / 3.0) * ql[0] : 0.0;
 #pragma unroll
     for (int lm = 0; lm < 24; ++lm)
-      A[lm] *= own ? 2.0 * clm_f64(lm) * Fp[NR + (lm_to_l(lm) - 1) * NA + ch] : 0.0;
+      A[lm] *= own ? 2.0 * clm_f64(lm) * (Fp[NR + (lm_to_l(lm) - 1) * NA + ch] + (lm < 3 ? f5 : 0.0)) : 0.0;
     if (sm.B4 && own) {
       const double f4 = Fp[NR + 4 * NA + ch];
 #pragma unroll
