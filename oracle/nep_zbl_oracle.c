@@ -397,6 +397,10 @@ typedef struct {
   int n;
   double L[3];
   int pbc[3];
+  /* triclinic box (D:C-28): rows of H are the lattice vectors a, b, c (box[9] row vectors),
+   * x = s H with fractional s; Hi = H^-1; hgt[a] = distance between the two faces that axis a connects */
+  int tri;
+  double H[9], Hi[9], hgt[3];
   double *xw; /* wrapped copy [3n] SoA */
   /* cell list (own; only used when use_cell) */
   int use_cell;
@@ -405,25 +409,64 @@ typedef struct {
   int *cell_start, *cell_atoms;
 } orc_system;
 
+/* inverse of the 3x3 matrix H (row-major); returns det H */
+static double mat3_inverse(const double *H, double *Hi) {
+  double c00 = H[4] * H[8] - H[5] * H[7], c01 = H[5] * H[6] - H[3] * H[8], c02 = H[3] * H[7] - H[4] * H[6];
+  double det = H[0] * c00 + H[1] * c01 + H[2] * c02;
+  Hi[0] = c00 / det; Hi[1] = (H[2] * H[7] - H[1] * H[8]) / det; Hi[2] = (H[1] * H[5] - H[2] * H[4]) / det;
+  Hi[3] = c01 / det; Hi[4] = (H[0] * H[8] - H[2] * H[6]) / det; Hi[5] = (H[2] * H[3] - H[0] * H[5]) / det;
+  Hi[6] = c02 / det; Hi[7] = (H[1] * H[6] - H[0] * H[7]) / det; Hi[8] = (H[0] * H[4] - H[1] * H[3]) / det;
+  return det;
+}
+
+/* wrap x[3] into the periodic cell: fractional s = x H^-1, s -= floor(s), x = s H (triclinic boxes: all axes periodic) */
+static void tri_wrap(const double *H, const double *Hi, double *x) {
+  double s[3];
+  for (int a = 0; a < 3; ++a) {
+    s[a] = x[0] * Hi[a] + x[1] * Hi[3 + a] + x[2] * Hi[6 + a];
+    s[a] -= floor(s[a]);
+  }
+  for (int b = 0; b < 3; ++b) x[b] = s[0] * H[b] + s[1] * H[3 + b] + s[2] * H[6 + b];
+}
+
 static int orc_system_init(orc_system *S, int n, const double *pos, const double *box,
                            const int32_t *pbc, double rc, int use_cell) {
-  /* orthogonal boxes only */
+  S->n = n;
+  S->tri = 0;
   for (int a = 0; a < 3; ++a)
     for (int b = 0; b < 3; ++b)
-      if (a != b && box[3 * a + b] != 0.0) return -2;
-  S->n = n;
+      if (a != b && box[3 * a + b] != 0.0) S->tri = 1;
   for (int a = 0; a < 3; ++a) {
     S->L[a] = box[4 * a];
     S->pbc[a] = pbc[a];
   }
   S->xw = (double *)malloc(sizeof(double) * 3 * (size_t)(n > 0 ? n : 1));
+  S->use_cell = 0;
+  S->cell_start = S->cell_atoms = NULL;
+  if (S->tri) {
+    /* triclinic (D:C-28): periodic along all three lattice vectors; brute-force neighbour search with explicit
+     * lattice-vector images only (no cell list) */
+    if (!(pbc[0] && pbc[1] && pbc[2])) { free(S->xw); return -2; }
+    memcpy(S->H, box, sizeof S->H);
+    double det = mat3_inverse(S->H, S->Hi);
+    if (!(fabs(det) > 0.0)) { free(S->xw); return -2; }
+    for (int a = 0; a < 3; ++a) { /* height_a = 1 / |column a of H^-1| (the reciprocal lattice vector) */
+      double g2 = S->Hi[a] * S->Hi[a] + S->Hi[3 + a] * S->Hi[3 + a] + S->Hi[6 + a] * S->Hi[6 + a];
+      S->hgt[a] = 1.0 / sqrt(g2);
+    }
+    for (int i = 0; i < n; ++i) {
+      double x[3] = {pos[i], pos[(size_t)n + i], pos[2 * (size_t)n + i]};
+      tri_wrap(S->H, S->Hi, x);
+      for (int a = 0; a < 3; ++a) S->xw[(size_t)a * n + i] = x[a];
+    }
+    return 0;
+  }
   for (int a = 0; a < 3; ++a)
     for (int i = 0; i < n; ++i) {
       double x = pos[(size_t)a * n + i];
       if (S->pbc[a]) x -= S->L[a] * floor(x / S->L[a]); /* wrap periodic axes */
       S->xw[(size_t)a * n + i] = x;
     }
-  S->use_cell = 0;
   S->cell_start = S->cell_atoms = NULL;
   if (use_cell && n > 0) {
     int ok = 1;
@@ -501,7 +544,30 @@ static int orc_site_neighbors(const orc_system *S, int i, double rc, orc_nbr *ou
   int n = S->n, cnt = 0;
   double rc2 = rc * rc;
   double xi[3] = {S->xw[i], S->xw[(size_t)n + i], S->xw[2 * (size_t)n + i]};
-  if (!S->use_cell) {
+  if (S->tri) {
+    /* triclinic: every atom, every lattice-vector image s0 a + s1 b + s2 c with |s_k| <= ceil(rc / height_k) */
+    int m[3];
+    for (int a = 0; a < 3; ++a) m[a] = (int)ceil(rc / S->hgt[a]);
+    for (int j = 0; j < n; ++j) {
+      double dj[3] = {S->xw[j] - xi[0], S->xw[(size_t)n + j] - xi[1], S->xw[2 * (size_t)n + j] - xi[2]};
+      for (int sx = -m[0]; sx <= m[0]; ++sx)
+        for (int sy = -m[1]; sy <= m[1]; ++sy)
+          for (int sz = -m[2]; sz <= m[2]; ++sz) {
+            if (j == i && sx == 0 && sy == 0 && sz == 0) continue;
+            double d[3];
+            for (int b = 0; b < 3; ++b) d[b] = dj[b] + sx * S->H[b] + sy * S->H[3 + b] + sz * S->H[6 + b];
+            double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+            if (r2 < rc2) {
+              if (cnt < cap) {
+                out[cnt].j = j;
+                out[cnt].s[0] = sx; out[cnt].s[1] = sy; out[cnt].s[2] = sz;
+                out[cnt].d[0] = d[0]; out[cnt].d[1] = d[1]; out[cnt].d[2] = d[2];
+              }
+              ++cnt;
+            }
+          }
+    }
+  } else if (!S->use_cell) {
     /* brute force: every atom, every image shift s in {-m..m}^3, m = ceil(rc/L) on periodic axes */
     int m[3];
     for (int a = 0; a < 3; ++a) m[a] = S->pbc[a] ? (int)ceil(rc / S->L[a]) : 0;
@@ -806,6 +872,12 @@ int orc_md_run(const orc_params *p, int n, double *pos, double *vel, const int32
                int use_cell, double *dt_trace, double *epot_trace, double *ekin_trace) {
   double *F = (double *)malloc(sizeof(double) * 3 * (size_t)n);
   double *E = (double *)malloc(sizeof(double) * n);
+  int tri = 0;
+  double Hi[9];
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      if (a != b && box[3 * a + b] != 0.0) tri = 1;
+  if (tri) mat3_inverse(box, Hi);
   int rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
   for (int step = 0; step <= nsteps && !rc; ++step) {
     double ep = 0.0, ek = 0.0, vmax2 = 0.0;
@@ -828,8 +900,14 @@ int orc_md_run(const orc_params *p, int n, double *pos, double *vel, const int32
         double acc = F[(size_t)a * n + i] / (p->mass[types[i]] * ORC_AMU_A2_FS2_TO_EV);
         vel[(size_t)a * n + i] += 0.5 * dt * acc;
         double x = pos[(size_t)a * n + i] + dt * vel[(size_t)a * n + i];
-        if (pbc[a]) x -= box[4 * a] * floor(x / box[4 * a]);
+        if (pbc[a] && !tri) x -= box[4 * a] * floor(x / box[4 * a]);
         pos[(size_t)a * n + i] = x;
+      }
+    if (tri) /* triclinic: wrap along the lattice vectors (D:C-28) */
+      for (int i = 0; i < n; ++i) {
+        double x[3] = {pos[i], pos[(size_t)n + i], pos[2 * (size_t)n + i]};
+        tri_wrap(box, Hi, x);
+        for (int a = 0; a < 3; ++a) pos[(size_t)a * n + i] = x[a];
       }
     rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
     for (int a = 0; a < 3; ++a)
@@ -922,6 +1000,12 @@ int orc_md_run_nhc(const orc_params *p, int n, double *pos, double *vel, const i
   const double nf = 3.0 * ng, kT = ORC_KB * T;
   if (M < 1) M = 1;
   if (M > 16) M = 16;
+  int tri = 0;
+  double Hi[9];
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b)
+      if (a != b && box[3 * a + b] != 0.0) tri = 1;
+  if (tri) mat3_inverse(box, Hi);
   int rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
   for (int step = 0; step <= nsteps && !rc; ++step) {
     double ep = 0.0, ek = 0.0, vmax2 = 0.0;
@@ -961,8 +1045,14 @@ int orc_md_run_nhc(const orc_params *p, int n, double *pos, double *vel, const i
         double acc = F[(size_t)a * n + i] / (p->mass[types[i]] * ORC_AMU_A2_FS2_TO_EV);
         vel[(size_t)a * n + i] += 0.5 * dt * acc;
         double x = pos[(size_t)a * n + i] + dt * vel[(size_t)a * n + i];
-        if (pbc[a]) x -= box[4 * a] * floor(x / box[4 * a]);
+        if (pbc[a] && !tri) x -= box[4 * a] * floor(x / box[4 * a]);
         pos[(size_t)a * n + i] = x;
+      }
+    if (tri) /* triclinic: wrap along the lattice vectors (D:C-28) */
+      for (int i = 0; i < n; ++i) {
+        double x[3] = {pos[i], pos[(size_t)n + i], pos[2 * (size_t)n + i]};
+        tri_wrap(box, Hi, x);
+        for (int a = 0; a < 3; ++a) pos[(size_t)a * n + i] = x[a];
       }
     rc = orc_compute(p, n, pos, types, box, pbc, use_cell, E, F, NULL, NULL, -1, NULL);
     for (int a = 0; a < 3; ++a)
