@@ -16,8 +16,12 @@
  *   - Positions / velocities are fp64 SoA: x[n] y[n] z[n] (3n doubles).  Forces are fp32 SoA [3n],
  *     virials fp32 SoA [9n] with component c = 3*alpha+beta at virial[c*n + i], energies fp64 [n].
  *     All per-atom results are in the CALLER's atom order (the library sorts internally).
- *   - box[9]: row vectors, host.  Only orthogonal boxes (off-diagonals == 0).  pbc[3]: 1 periodic,
- *     0 open (bulk periodic xyz; foil open in z).  A periodic edge must be >= 2*(rc_radial+skin).
+ *   - box[9]: the three lattice vectors as ROW vectors, host.  pbc[3]: 1 periodic, 0 open (bulk periodic xyz;
+ *     foil open in z).  Orthogonal boxes (off-diagonals == 0): any pbc; a periodic edge must be >= 2*(rc_radial+skin).
+ *     Triclinic boxes (any off-diagonal != 0, C-28): periodic along all three lattice
+ *     vectors (else NEPZBL_E_BOX_NOT_ORTHOGONAL); every distance between opposite cell faces must be
+ *     >= 2*(rc_radial+skin); positions are wrapped along the lattice vectors.  The Wigner-Seitz count takes
+ *     orthogonal boxes only.
  *   - All work is enqueued on the CUDA stream given at create.  Calls that return host scalars or
  *     status from the device (neighbor_build, nep_zbl_compute, md_step, md_run, md_energies,
  *     *_host) synchronise that stream before returning.
@@ -42,7 +46,7 @@ typedef struct nepzbl_handle nepzbl_handle; /* opaque, owned by the library */
 enum {
   NEPZBL_OK = 0,
   NEPZBL_E_INVALID_ARG = -1,
-  NEPZBL_E_BOX_NOT_ORTHOGONAL = -2,
+  NEPZBL_E_BOX_NOT_ORTHOGONAL = -2, /* a non-orthogonal box with an open axis, or given to the Wigner-Seitz count */
   NEPZBL_E_BOX_TOO_SMALL = -3,     /* periodic edge < 2*(rc_radial+skin): minimum image invalid */
   NEPZBL_E_NEIGHBOR_OVERFLOW = -4, /* an atom has more neighbours than cap_radial / cap_angular */
   NEPZBL_E_NONFINITE = -5,         /* NaN/Inf in positions */

@@ -25,7 +25,35 @@ struct BoxMap {  // device-resident; recomputed by k_boxmap at every list rebuil
   int ncv[3];       // cell index = (u * ncv) >> 32
   int ncells;
   int S;            // stencil half-width in cells: cells have edge >= (rc_radial+skin)/S
+  // Triclinic boxes (C-28; all three axes periodic): the fixed-point coordinates are
+  // the FRACTIONAL coordinates s = x H^-1 (H rows = lattice vectors), so integer differences still wrap to the
+  // minimum image along every lattice vector; a difference (du_x, du_y, du_z) is the Cartesian vector
+  // du_x hm[0..2] + du_y hm[3..5] + du_z hm[6..8], hm = H / 2^32.  Orthogonal boxes: tri = 0 and hm is diag(hf).
+  int tri;
+  double H[9], Hi[9];
+  float hm[9];
 };
+
+// Cartesian displacement of an integer fixed-point difference
+template <bool TRI>
+__device__ __forceinline__ void fixed_disp(const float* __restrict__ hm, int dux, int duy, int duz, float& dx,
+                                           float& dy, float& dz) {
+  const float fx = (float)dux, fy = (float)duy, fz = (float)duz;
+  if (TRI) {
+    dx = fmaf(fz, hm[6], fmaf(fy, hm[3], fx * hm[0]));
+    dy = fmaf(fz, hm[7], fmaf(fy, hm[4], fx * hm[1]));
+    dz = fmaf(fz, hm[8], fmaf(fy, hm[5], fx * hm[2]));
+  } else {
+    dx = fx * hm[0];
+    dy = fy * hm[4];
+    dz = fz * hm[8];
+  }
+}
+__device__ __forceinline__ void fixed_disp_rt(const BoxMap* __restrict__ bm, int dux, int duy, int duz, float& dx,
+                                              float& dy, float& dz) {
+  if (bm->tri) fixed_disp<true>(bm->hm, dux, duy, duz, dx, dy, dz);
+  else fixed_disp<false>(bm->hm, dux, duy, duz, dx, dy, dz);
+}
 
 struct Scalars {  // device-resident control block (one per handle)
   int do_rebuild;
@@ -54,6 +82,8 @@ struct BoxHost {  // passed by value to k_boxmap
   int pbc[3];
   double rcs;      // rc_radial + skin: minimum cell edge
   int ncell_cap;
+  int tri;         // triclinic: H, Hi, hgt are set
+  double H[9], Hi[9], hgt[3];  // lattice rows, inverse, distances between opposite faces
 };
 
 // order-preserving map double -> uint64 (for atomicMin/Max on signed doubles)
@@ -84,6 +114,20 @@ __device__ __forceinline__ int checked_type(Scalars* sc, const int32_t* __restri
 // fixed-point coordinate of x on one axis (wraps modulo 2^32 on periodic axes)
 __device__ __forceinline__ unsigned int fix_coord(double x, double lo, double inv_h) {
   return (unsigned int)(unsigned long long)__double2ll_rd((x - lo) * inv_h);
+}
+
+// fixed-point coordinates of a Cartesian position: per axis for orthogonal boxes, fractional for triclinic ones
+__device__ __forceinline__ void fix_position(const BoxMap* __restrict__ bm, double x, double y, double z,
+                                             unsigned int u[3]) {
+  if (bm->tri) {
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+      u[a] = fix_coord(x * bm->Hi[a] + y * bm->Hi[3 + a] + z * bm->Hi[6 + a], 0.0, 4294967296.0);
+  } else {
+    u[0] = fix_coord(x, bm->lo[0], bm->inv_h[0]);
+    u[1] = fix_coord(y, bm->lo[1], bm->inv_h[1]);
+    u[2] = fix_coord(z, bm->lo[2], bm->inv_h[2]);
+  }
 }
 
 __device__ __forceinline__ int cell_of_u(unsigned int u, int ncv, int nc) {

@@ -269,7 +269,7 @@ __device__ __forceinline__ float tanh_fast(float z) {
 // costs one block's duration -- 128-thread blocks: 49.4 us, 64: 48.6, 32: 47.7 (256 / 512: worse)
 #define RADIAL_BLOCK 64  // upper bound; the host launches 32 or 64 threads per block (nepzbl_handle::gather_block)
 #endif
-template <class MS>
+template <class MS, bool TRI>
 __global__ void __launch_bounds__(RADIAL_BLOCK)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
@@ -282,7 +282,9 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   const bool valid = s < n;
   const int sc_ = valid ? s : 0;
   const int4 me = xyzt[sc_];
-  const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
+  float hm[9];  // fixed-point difference -> Cartesian displacement (only the diagonal is live for orthogonal boxes)
+#pragma unroll
+  for (int k = 0; k < 9; ++k) hm[k] = (TRI || k % 4 == 0) ? bm->hm[k] : 0.0f;
   // basis sums per NEIGHBOUR type: q_n = sum_tj sum_k ct^{ti tj}_nk acc[tj][k]
   float acc[MS::NT][MS::KR];
 #pragma unroll
@@ -327,7 +329,8 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
 #pragma unroll
     for (int u = 0; u < RADIAL_UNROLL; ++u) {
       const int e = t + RADIAL_LANES * u;
-      float dx = (float)(o[u].x - me.x) * hx, dy = (float)(o[u].y - me.y) * hy, dz = (float)(o[u].z - me.z) * hz;
+      float dx, dy, dz;
+      fixed_disp<TRI>(hm, o[u].x - me.x, o[u].y - me.y, o[u].z - me.z, dx, dy, dz);
       float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
       if (ang_round) {
         const bool pa = e < cnt_a && r2 < mt.rcA2;

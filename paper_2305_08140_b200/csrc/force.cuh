@@ -32,7 +32,7 @@ struct KickArgs {
 };
 // BLK = threads per block (32 or 64, chosen by the host from the grid size; a template parameter because the code
 // ptxas generates under __launch_bounds__(32) is 2 % faster than the same source under a bound of 64 or 128)
-template <class MS, bool VIRIAL, int BLK>
+template <class MS, bool VIRIAL, int BLK, bool TRI>
 __global__ void __launch_bounds__(BLK)
 k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
         const int* __restrict__ nn_r, const int* __restrict__ nl_r, const int* __restrict__ nn_a,
@@ -87,7 +87,9 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
 #pragma unroll
     for (int k = 0; k < 12; ++k) me_d1[NT > 1 ? k : 0] = t1.d[k];
   }
-  const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
+  float hm[9];  // fixed-point difference -> Cartesian displacement (only the diagonal is live for orthogonal boxes)
+#pragma unroll
+  for (int k = 0; k < 9; ++k) hm[k] = (TRI || k % 4 == 0) ? bm->hm[k] : 0.0f;
   float fx = 0.0f, fy = 0.0f, fz = 0.0f;
   float w[9];
 #pragma unroll
@@ -118,7 +120,8 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       load(o_nxt, j_nxt >= 0 ? j_nxt : sc_, ti);
       int j_nn = j_nxt >= 0 ? next_j() : -1;
       const Rec& o = o_cur;
-      float dx = (float)(o.ux - me.ux) * hx, dy = (float)(o.uy - me.uy) * hy, dz = (float)(o.uz - me.uz) * hz;
+      float dx, dy, dz;
+      fixed_disp<TRI>(hm, o.ux - me.ux, o.uy - me.uy, o.uz - me.uz, dx, dy, dz);
       float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
       close = close || (r2 < mt.zbl_flag_r2);
       float rinv = rsqrtf(r2), r = r2 * rinv;
@@ -227,13 +230,15 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       if (VIRIAL) {
         int4 o0 = xyzt[j0], o1 = xyzt[j1];
         {
-          float dx = (float)(o0.x - me.ux) * hx, dy = (float)(o0.y - me.uy) * hy, dz = (float)(o0.z - me.uz) * hz;
+          float dx, dy, dz;
+          fixed_disp<TRI>(hm, o0.x - me.ux, o0.y - me.uy, o0.z - me.uz, dx, dy, dz);
           w[0] = fmaf(dx, pji0.x, w[0]); w[1] = fmaf(dx, pji0.y, w[1]); w[2] = fmaf(dx, pji0.z, w[2]);
           w[3] = fmaf(dy, pji0.x, w[3]); w[4] = fmaf(dy, pji0.y, w[4]); w[5] = fmaf(dy, pji0.z, w[5]);
           w[6] = fmaf(dz, pji0.x, w[6]); w[7] = fmaf(dz, pji0.y, w[7]); w[8] = fmaf(dz, pji0.z, w[8]);
         }
         {
-          float dx = (float)(o1.x - me.ux) * hx, dy = (float)(o1.y - me.uy) * hy, dz = (float)(o1.z - me.uz) * hz;
+          float dx, dy, dz;
+          fixed_disp<TRI>(hm, o1.x - me.ux, o1.y - me.uy, o1.z - me.uz, dx, dy, dz);
           w[0] = fmaf(dx, pji1.x, w[0]); w[1] = fmaf(dx, pji1.y, w[1]); w[2] = fmaf(dx, pji1.z, w[2]);
           w[3] = fmaf(dy, pji1.x, w[3]); w[4] = fmaf(dy, pji1.y, w[4]); w[5] = fmaf(dy, pji1.z, w[5]);
           w[6] = fmaf(dz, pji1.x, w[6]); w[7] = fmaf(dz, pji1.y, w[7]); w[8] = fmaf(dz, pji1.z, w[8]);
@@ -294,6 +299,25 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
   }
 }
 
+// minimum image of a Cartesian difference in fp64: per periodic axis for orthogonal boxes, along the lattice vectors
+// (s = d H^-1, s -= rint(s), d = s H) for triclinic ones; exact for pairs closer than half the smallest cell height
+__device__ __forceinline__ void min_image_f64(const BoxMap* __restrict__ bm, double d[3]) {
+  if (bm->tri) {
+    double sf[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      sf[a] = d[0] * bm->Hi[a] + d[1] * bm->Hi[3 + a] + d[2] * bm->Hi[6 + a];
+      sf[a] -= rint(sf[a]);
+    }
+#pragma unroll
+    for (int b = 0; b < 3; ++b) d[b] = sf[0] * bm->H[b] + sf[1] * bm->H[3 + b] + sf[2] * bm->H[6 + b];
+  } else {
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+      if (bm->pbc[a]) d[a] -= bm->L[a] * rint(d[a] / bm->L[a]);
+  }
+}
+
 struct ZblParams {
   double r_inner, r_outer;
   int n_terms;
@@ -328,14 +352,12 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
     for (int k = sub; k < cnt; k += ZBL_LANES) {
       int j = nl_r[(size_t)k * npad + s];
       int4 o = xyzt[j];
-      float fdx = (float)(o.x - me.x) * bm->hf[0], fdy = (float)(o.y - me.y) * bm->hf[1],
-            fdz = (float)(o.z - me.z) * bm->hf[2];
+      float fdx, fdy, fdz;
+      fixed_disp_rt(bm, o.x - me.x, o.y - me.y, o.z - me.z, fdx, fdy, fdz);
       if (fdx * fdx + fdy * fdy + fdz * fdz >= zp.filter_r2) continue;
       int jj = perm[j];
       double d[3] = {pos[jj] - xi, pos[(size_t)n + jj] - yi, pos[2 * (size_t)n + jj] - zi};
-#pragma unroll
-      for (int a = 0; a < 3; ++a)
-        if (bm->pbc[a]) d[a] -= bm->L[a] * rint(d[a] / bm->L[a]);  // minimum image in fp64
+      min_image_f64(bm, d);  // minimum image in fp64
       double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
       if (!(r < zp.r_outer)) continue;
       double Zi = zp.Z[me.w], Zj = zp.Z[o.w];

@@ -204,6 +204,8 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
     int t = checked_type(sc, types, i, fa.n_types);
     double im = inv_mass[t];  // 1 / (m * 103.6426965): acceleration in A/fs^2 per eV/A
     unsigned int u[3];
+    double xn[3];
+    bool finite = true;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       size_t k = (size_t)a * n + i;
@@ -211,18 +213,33 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
       if (group) v *= sg;
       v += 0.5 * dt * ((double)force[k] * im);
       double xx = pos[k] + dt * v;
-      if (bm->pbc[a]) xx -= bm->L[a] * floor(xx / bm->L[a]);
+      if (!bm->tri && bm->pbc[a]) xx -= bm->L[a] * floor(xx / bm->L[a]);
       vel[k] = v;
-      pos[k] = xx;
-      if (!isfinite(xx)) sc->nonfinite = 1;
-      u[a] = fix_coord(isfinite(xx) ? xx : 0.0, bm->lo[a], bm->inv_h[a]);
+      xn[a] = xx;
+      finite = finite && isfinite(xx);
     }
+    if (bm->tri && finite) {  // wrap along the lattice vectors: s = x H^-1, s -= floor(s), x = s H
+      double sf[3];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        sf[a] = xn[0] * bm->Hi[a] + xn[1] * bm->Hi[3 + a] + xn[2] * bm->Hi[6 + a];
+        sf[a] -= floor(sf[a]);
+      }
+#pragma unroll
+      for (int b = 0; b < 3; ++b) xn[b] = sf[0] * bm->H[b] + sf[1] * bm->H[3 + b] + sf[2] * bm->H[6 + b];
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) pos[(size_t)a * n + i] = xn[a];
+    if (!finite) {
+      sc->nonfinite = 1;
+      xn[0] = xn[1] = xn[2] = 0.0;
+    }
+    fix_position(bm, xn[0], xn[1], xn[2], u);
     int s = inv_perm[i];
     int4 b = xyzt_build[i];
     xyzt[s] = make_int4((int)u[0], (int)u[1], (int)u[2], t);
-    float dx = (float)((int)u[0] - b.x) * bm->hf[0];
-    float dy = (float)((int)u[1] - b.y) * bm->hf[1];
-    float dz = (float)((int)u[2] - b.z) * bm->hf[2];
+    float dx, dy, dz;
+    fixed_disp_rt(bm, (int)u[0] - b.x, (int)u[1] - b.y, (int)u[2] - b.z, dx, dy, dz);
     d2 = dx * dx + dy * dy + dz * dz;
   }
   const Top2 m = block_top2(d2, sh);

@@ -64,7 +64,15 @@ __device__ long long make_grid(Scalars* sc, BoxMap* bm, const BoxHost& bh, int S
     bm->L[a] = bh.L[a];
     double span, lo;
     int nc, ncv;
-    if (bh.pbc[a]) {
+    if (bh.tri) {  // fractional coordinates: span 1, cells counted along the distance between the faces of axis a
+      lo = 0.0;
+      span = 1.0;
+      nc = (int)floor(bh.hgt[a] / cw);
+      if (S == 2 && nc < 5) return -1;
+      if (f == 1 && nc < 2) sc->box_too_small = 1;
+      if (nc < 1) nc = 1;
+      ncv = nc;
+    } else if (bh.pbc[a]) {
       lo = 0.0;
       span = bh.L[a];
       nc = (int)floor(bh.L[a] / cw);
@@ -92,6 +100,17 @@ __device__ long long make_grid(Scalars* sc, BoxMap* bm, const BoxHost& bh, int S
     bm->nc[a] = nc;
     bm->ncv[a] = ncv;
     total *= nc;
+  }
+  bm->tri = bh.tri;
+  for (int k = 0; k < 9; ++k) {
+    bm->H[k] = bh.H[k];
+    bm->Hi[k] = bh.Hi[k];
+    bm->hm[k] = bh.tri ? (float)(bh.H[k] / two32) : 0.0f;
+  }
+  if (!bh.tri) {
+    bm->hm[0] = bm->hf[0];
+    bm->hm[4] = bm->hf[1];
+    bm->hm[8] = bm->hf[2];
   }
   return total;
 }
@@ -137,9 +156,9 @@ __global__ void k_bin(Scalars* sc, const BoxMap* __restrict__ bm, int n,
     sc->nonfinite = 1;
     x = y = z = 0.0;
   }
-  unsigned int ux = fix_coord(x, bm->lo[0], bm->inv_h[0]);
-  unsigned int uy = fix_coord(y, bm->lo[1], bm->inv_h[1]);
-  unsigned int uz = fix_coord(z, bm->lo[2], bm->inv_h[2]);
+  unsigned int uu[3];
+  fix_position(bm, x, y, z, uu);
+  const unsigned int ux = uu[0], uy = uu[1], uz = uu[2];
   int cx = cell_of_u(ux, bm->ncv[0], bm->nc[0]);
   int cy = cell_of_u(uy, bm->ncv[1], bm->nc[1]);
   int cz = cell_of_u(uz, bm->ncv[2], bm->nc[2]);
@@ -294,7 +313,6 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   const int4 me = xyzt[s];
-  const float hx = bm->hf[0], hy = bm->hf[1], hz = bm->hf[2];
   const int S = bm->S, W = 2 * S + 1;
   int sx[5], sy[5], sz[5];
   axis_stencil(cell_of_u((unsigned)me.x, bm->ncv[0], bm->nc[0]), bm->nc[0], bm->pbc[0], S, sx);
@@ -321,9 +339,8 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
           for (int j = b; j < e; ++j) {
             if (j == s) continue;
             int4 o = xyzt[j];
-            float dx = (float)(o.x - me.x) * hx;  // int32 wrap-around = minimum image
-            float dy = (float)(o.y - me.y) * hy;
-            float dz = (float)(o.z - me.z) * hz;
+            float dx, dy, dz;  // int32 wrap-around = minimum image
+            fixed_disp_rt(bm, o.x - me.x, o.y - me.y, o.z - me.z, dx, dy, dz);
             float r2 = dx * dx + dy * dy + dz * dz;
             if (r2 < rcs2_radial) {
               const int seg = r2 < rcs2_angular ? 0 : (r2 < rc2_radial ? 1 : 2);
@@ -393,9 +410,8 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
           for (int j = b; j < e; ++j) {
             if (j == s) continue;
             int4 o = xyzt[j];
-            float dx = (float)(o.x - me.x) * hx;  // int32 wrap-around = minimum image
-            float dy = (float)(o.y - me.y) * hy;
-            float dz = (float)(o.z - me.z) * hz;
+            float dx, dy, dz;  // int32 wrap-around = minimum image
+            fixed_disp_rt(bm, o.x - me.x, o.y - me.y, o.z - me.z, dx, dy, dz);
             float r2 = dx * dx + dy * dy + dz * dz;
             if (r2 < rcs2_radial) {
               if (pass == 0) {
@@ -462,15 +478,14 @@ k_prep(Scalars* sc, const BoxMap* __restrict__ bm, int n, const double* __restri
       sc->nonfinite = 1;
       x = y = z = 0.0;
     }
-    unsigned int ux = fix_coord(x, bm->lo[0], bm->inv_h[0]);
-    unsigned int uy = fix_coord(y, bm->lo[1], bm->inv_h[1]);
-    unsigned int uz = fix_coord(z, bm->lo[2], bm->inv_h[2]);
+    unsigned int uu[3];
+    fix_position(bm, x, y, z, uu);
+    const unsigned int ux = uu[0], uy = uu[1], uz = uu[2];
     int s = inv_perm[i];
     int4 b = xyzt_build[i];
     xyzt[s] = make_int4((int)ux, (int)uy, (int)uz, checked_type(sc, types, i, n_types));
-    float dx = (float)((int)ux - b.x) * bm->hf[0];
-    float dy = (float)((int)uy - b.y) * bm->hf[1];
-    float dz = (float)((int)uz - b.z) * bm->hf[2];
+    float dx, dy, dz;
+    fixed_disp_rt(bm, (int)ux - b.x, (int)uy - b.y, (int)uz - b.z, dx, dy, dz);
     d2 = dx * dx + dy * dy + dz * dz;
   }
   const Top2 m = block_top2(d2, sh);

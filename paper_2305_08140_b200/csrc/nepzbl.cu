@@ -85,6 +85,8 @@ struct nepzbl_handle {
   long long n = 0;
   double box[9] = {0};
   int pbc[3] = {0, 0, 0};
+  bool tri = false;            // triclinic box (all axes periodic): box_inv / box_hgt are set
+  double box_inv[9] = {0}, box_hgt[3] = {0};
 
   // md state
   bool md_ready = false;
@@ -423,6 +425,12 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
   }
   bh.rcs = h->p.rc_radial + h->p.skin;
   bh.ncell_cap = c.ncell_cap;
+  bh.tri = h->tri ? 1 : 0;
+  for (int k = 0; k < 9; ++k) {
+    bh.H[k] = h->box[k];
+    bh.Hi[k] = h->box_inv[k];
+  }
+  for (int a = 0; a < 3; ++a) bh.hgt[a] = h->box_hgt[a];
   float rr = (float)(bh.rcs * bh.rcs);
   float rc2 = (float)(h->p.rc_radial * h->p.rc_radial);
   double ra = h->p.rc_angular + h->p.skin;
@@ -479,12 +487,14 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
   const int gb = h->gather_block ? h->gather_block : ((long long)n * RADIAL_LANES < 8ll * 1024 * h->n_sm ? 32 : 64);
   prof_mark(h, PK_RADIAL);
-  k_radial<MS><<<blocks((long long)n * RADIAL_LANES, gb), gb, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt),
-                                              h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
-                                              h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p),
-                                              h->at<int>(c.zbl_list), h->at<int>(c.nn_a),
-                                              h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp),
-                                              h->at<unsigned long long>(c.shellq));
+  auto launch_radial = [&](auto tri) {
+    k_radial<MS, decltype(tri)::value><<<blocks((long long)n * RADIAL_LANES, gb), gb, 0, st>>>(
+        h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
+        h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p), h->at<int>(c.zbl_list),
+        h->at<int>(c.nn_a), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp),
+        h->at<unsigned long long>(c.shellq));
+  };
+  if (h->tri) launch_radial(std::true_type{}); else launch_radial(std::false_type{});
   prof_mark(h, PK_ANGULAR_NN);
   if constexpr (kSplit<MS>)
     k_angular_nn_split<MS><<<std::min(blocks((long long)n * SPLIT_LANES, SPLIT_THREADS), h->ang_grid), SPLIT_THREADS, h->smem_nn, st>>>(
@@ -502,14 +512,19 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
     h->launches++;
   }
   prof_mark(h, PK_FORCE);
-  auto launch_force = [&](auto vir, auto blk) {
+  auto launch_force_t = [&](auto vir, auto blk, auto tri) {
     constexpr bool VIR = decltype(vir)::value;
     constexpr int BLK = decltype(blk)::value;
-    k_force<MS, VIR, BLK><<<blocks((long long)n * FORCE_LANES, BLK), BLK, 0, st>>>(
+    k_force<MS, VIR, BLK, decltype(tri)::value><<<blocks((long long)n * FORCE_LANES, BLK), BLK, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.nn_a),
         h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk), h->at<unsigned>(c.rmask),
         mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site),
         h->at<int>(c.perm), energy, force, VIR ? virial : nullptr, ka);
+  };
+  // triclinic boxes take the 64-thread variant only (a NEXT row: fewer instantiations)
+  auto launch_force = [&](auto vir, auto blk) {
+    if (h->tri) launch_force_t(vir, std::integral_constant<int, 64>{}, std::true_type{});
+    else launch_force_t(vir, blk, std::false_type{});
   };
   using std::integral_constant;
   if (virial) {
@@ -584,15 +599,35 @@ int set_system(nepzbl_handle* h, long long n, const double box[9], const int32_t
   if (!h->ws) return fail(h, NEPZBL_E_WORKSPACE, "no workspace set");
   if (n < 0 || n > h->n_cap) return fail(h, NEPZBL_E_WORKSPACE, "n = %lld exceeds workspace capacity %lld", n, h->n_cap);
   if (!box || !pbc) return fail(h, NEPZBL_E_INVALID_ARG, "box/pbc is NULL");
+  bool tri = false;
   for (int a = 0; a < 3; ++a)
     for (int b = 0; b < 3; ++b)
-      if (a != b && box[3 * a + b] != 0.0)
-        return fail(h, NEPZBL_E_BOX_NOT_ORTHOGONAL, "only orthogonal boxes are supported");
+      if (a != b && box[3 * a + b] != 0.0) tri = true;
   double rcs = h->p.rc_radial + h->p.skin;
-  for (int a = 0; a < 3; ++a) {
-    if (!(box[4 * a] > 0.0) || !std::isfinite(box[4 * a])) return fail(h, NEPZBL_E_INVALID_ARG, "box edge %d is not positive", a);
-    if (pbc[a] && box[4 * a] < 2.0 * rcs)
-      return fail(h, NEPZBL_E_BOX_TOO_SMALL, "periodic edge %d = %g A < 2*(rc_radial+skin) = %g A", a, box[4 * a], 2.0 * rcs);
+  double inv[9] = {0}, hgt[3] = {0};
+  if (tri) {
+    // triclinic (C-28): periodic along all three lattice vectors; every distance between opposite
+    // faces must hold the minimum image
+    if (!(pbc[0] && pbc[1] && pbc[2]))
+      return fail(h, NEPZBL_E_BOX_NOT_ORTHOGONAL, "a non-orthogonal box must be periodic along all three lattice vectors");
+    const double* H = box;
+    const double c00 = H[4] * H[8] - H[5] * H[7], c01 = H[5] * H[6] - H[3] * H[8], c02 = H[3] * H[7] - H[4] * H[6];
+    const double det = H[0] * c00 + H[1] * c01 + H[2] * c02;
+    if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) return fail(h, NEPZBL_E_INVALID_ARG, "box is singular");
+    inv[0] = c00 / det; inv[1] = (H[2] * H[7] - H[1] * H[8]) / det; inv[2] = (H[1] * H[5] - H[2] * H[4]) / det;
+    inv[3] = c01 / det; inv[4] = (H[0] * H[8] - H[2] * H[6]) / det; inv[5] = (H[2] * H[3] - H[0] * H[5]) / det;
+    inv[6] = c02 / det; inv[7] = (H[1] * H[6] - H[0] * H[7]) / det; inv[8] = (H[0] * H[4] - H[1] * H[3]) / det;
+    for (int a = 0; a < 3; ++a) {
+      hgt[a] = 1.0 / std::sqrt(inv[a] * inv[a] + inv[3 + a] * inv[3 + a] + inv[6 + a] * inv[6 + a]);
+      if (hgt[a] < 2.0 * rcs)
+        return fail(h, NEPZBL_E_BOX_TOO_SMALL, "cell height %d = %g A < 2*(rc_radial+skin) = %g A", a, hgt[a], 2.0 * rcs);
+    }
+  } else {
+    for (int a = 0; a < 3; ++a) {
+      if (!(box[4 * a] > 0.0) || !std::isfinite(box[4 * a])) return fail(h, NEPZBL_E_INVALID_ARG, "box edge %d is not positive", a);
+      if (pbc[a] && box[4 * a] < 2.0 * rcs)
+        return fail(h, NEPZBL_E_BOX_TOO_SMALL, "periodic edge %d = %g A < 2*(rc_radial+skin) = %g A", a, box[4 * a], 2.0 * rcs);
+    }
   }
   bool ch = !h->have_list || n != h->n;
   for (int a = 0; a < 9; ++a) ch = ch || box[a] != h->box[a];
@@ -600,6 +635,9 @@ int set_system(nepzbl_handle* h, long long n, const double box[9], const int32_t
   h->n = n;
   memcpy(h->box, box, sizeof h->box);
   for (int a = 0; a < 3; ++a) h->pbc[a] = pbc[a] != 0;
+  h->tri = tri;
+  memcpy(h->box_inv, inv, sizeof inv);
+  memcpy(h->box_hgt, hgt, sizeof hgt);
   *changed = ch;
   return NEPZBL_OK;
 }

@@ -16,7 +16,7 @@
 // kernel serves every model shape.  Reductions across lanes are fixed-order butterflies: deterministic.
 // Same mathematics as descriptor.cuh, same factorisations, FP64 throughout.
 #pragma once
-#include "descriptor.cuh"
+#include "force.cuh"
 
 struct SiteModel {  // tables are library-owned device arrays of doubles
   int NT, NR, KR, NA, KA, B4, B5, D, n_neurons;
@@ -86,10 +86,8 @@ __device__ __forceinline__ double warp_sum_f64(double v) {
 __device__ __forceinline__ void disp_f64(const BoxMap* bm, const double* __restrict__ pos, int n, int i, int jj,
                                          double d[3]) {
 #pragma unroll
-  for (int a = 0; a < 3; ++a) {
-    d[a] = pos[(size_t)a * n + jj] - pos[(size_t)a * n + i];
-    if (bm->pbc[a]) d[a] -= bm->L[a] * rint(d[a] / bm->L[a]);
-  }
+  for (int a = 0; a < 3; ++a) d[a] = pos[(size_t)a * n + jj] - pos[(size_t)a * n + i];
+  min_image_f64(bm, d);
 }
 
 // Lane map: lane = slice * NA + n for lane < NS * NA, NS = 32 / NA (config model: 6 slices x 5 channels; paper-sized

@@ -204,9 +204,9 @@ def test_single_atom_and_empty(nb):
 def test_error_codes(nb):
     w = wl.config1(seed=9, cells=5, n_pairs=0)
     g = nb.NepZbl(w.model, w.n)
-    with pytest.raises(nb.NepZblError) as ei:                      # non-orthogonal
+    with pytest.raises(nb.NepZblError) as ei:                      # non-orthogonal box with an open axis
         box = w.box.copy(); box[1] = 0.5
-        g.compute(w.pos, w.types, box, w.pbc)
+        g.compute(w.pos, w.types, box, [1, 1, 0])
     assert ei.value.code == -2
     with pytest.raises(nb.NepZblError) as ei:                      # periodic edge < 2 (rc+skin)
         g.compute(w.pos, w.types, np.diag([13.0, 40, 40]).ravel(), w.pbc)
