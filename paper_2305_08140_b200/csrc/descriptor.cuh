@@ -18,6 +18,7 @@
 //     v = sum_lm G_lm grad b_lm, G_lm = sum_n g_n E_nlm, G'_lm = sum_n g'_n E_nlm, E = dU/dA.
 #pragma once
 #include "common.cuh"
+#include "stage.cuh"
 
 template <int NR_, int KR_, int NA_, int KA_, bool B4_, int NT_ = 1, bool B5_ = false>
 struct ModelShape {
@@ -269,14 +270,28 @@ __device__ __forceinline__ float tanh_fast(float z) {
 // costs one block's duration -- 128-thread blocks: 49.4 us, 64: 48.6, 32: 47.7 (256 / 512: worse)
 #define RADIAL_BLOCK 64  // upper bound; the host launches 32 or 64 threads per block (nepzbl_handle::gather_block)
 #endif
-template <class MS, bool TRI>
-__global__ void __launch_bounds__(RADIAL_BLOCK)
+// STAGE > 0 (stage.cuh, an experiment): the block is one tile of STAGE_TILE atoms whose neighbour ranges are copied
+// to shared memory first (1: plain copies, 2: bulk copies); list entries then come from nl_loc (16-bit offsets).
+template <class MS, bool TRI, int STAGE = 0>
+__global__ void __launch_bounds__(STAGE ? STAGE_TILE * 4 : RADIAL_BLOCK)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
          const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,
          unsigned* __restrict__ rmask, int mask_words, int* __restrict__ zbl_list,
          const int* __restrict__ nn_a, unsigned long long* __restrict__ amask, float4* __restrict__ adisp,
-         const unsigned long long* __restrict__ shellq) {
+         const unsigned long long* __restrict__ shellq, const TileDesc* __restrict__ tiles,
+         const unsigned short* __restrict__ nl_loc) {
+  extern __shared__ __align__(16) unsigned char s_stage[];  // STAGE: [TileDesc | mbarrier | int4 x STAGE_CAP]
+  bool staged = false;
+  const int4* s_xyzt = nullptr;
+  if (STAGE) {
+    TileDesc* sd = reinterpret_cast<TileDesc*>(s_stage);
+    unsigned long long* mbar = reinterpret_cast<unsigned long long*>(s_stage + sizeof(TileDesc));
+    int4* sx = reinterpret_cast<int4*>(s_stage + ((sizeof(TileDesc) + 8 + 15) / 16) * 16);
+    stage_tile<STAGE == 2 ? 2 : 1>(tiles + blockIdx.x, xyzt, sx, sd, mbar);
+    staged = sd->nranges >= 0;
+    s_xyzt = sx;
+  }
   const int gt = blockIdx.x * blockDim.x + threadIdx.x;
   const int s = gt / RADIAL_LANES, sub = gt % RADIAL_LANES;
   const bool valid = s < n;
@@ -306,6 +321,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
     }
   }
   const int* lp = nl_r + (size_t)sub * npad + sc_;
+  const unsigned short* lp16 = STAGE ? nl_loc + (size_t)sub * npad + sc_ : nullptr;
   const size_t lstride = (size_t)RADIAL_LANES * npad;
   unsigned mword = 0u;
   int bit = 0, word = 0;
@@ -319,12 +335,21 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   for (int t = sub; t - sub < cnt_max; t += RADIAL_LANES * RADIAL_UNROLL) {
     int j[RADIAL_UNROLL];
     int4 o[RADIAL_UNROLL];
+    if (STAGE && staged) {
 #pragma unroll
-    for (int u = 0; u < RADIAL_UNROLL; ++u)
-      j[u] = (t + RADIAL_LANES * u < cnt) ? lp[(size_t)u * lstride] : sc_;
-    lp += (size_t)RADIAL_UNROLL * lstride;
+      for (int u = 0; u < RADIAL_UNROLL; ++u)
+        j[u] = (t + RADIAL_LANES * u < cnt) ? (int)lp16[(size_t)u * lstride] : 0;
+      lp16 += (size_t)RADIAL_UNROLL * lstride;
 #pragma unroll
-    for (int u = 0; u < RADIAL_UNROLL; ++u) o[u] = xyzt[j[u]];
+      for (int u = 0; u < RADIAL_UNROLL; ++u) o[u] = s_xyzt[j[u]];
+    } else {
+#pragma unroll
+      for (int u = 0; u < RADIAL_UNROLL; ++u)
+        j[u] = (t + RADIAL_LANES * u < cnt) ? lp[(size_t)u * lstride] : sc_;
+      lp += (size_t)RADIAL_UNROLL * lstride;
+#pragma unroll
+      for (int u = 0; u < RADIAL_UNROLL; ++u) o[u] = xyzt[j[u]];
+    }
     const bool ang_round = __any_sync(0xffffffffu, t - sub < cnt_a);  // any lane still in its angular prefix?
 #pragma unroll
     for (int u = 0; u < RADIAL_UNROLL; ++u) {
@@ -412,8 +437,39 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
 #define ANG_THREADS 32
 // rows of the staged weight table: n_neurons rounded up to even (two neurons per iteration) plus two
 // (the software pipeline reads one pair ahead); the padding rows are zero
-__host__ __device__ inline int nn_rows(int n_neurons) { return ((n_neurons + 1) & ~1) + 2; }
-template <class MS>
+// (a multiple of 8: the tensor-core variant walks the neurons in tiles of 8)
+__host__ __device__ inline int nn_rows(int n_neurons) { return (((n_neurons + 1) & ~1) + 2 + 7) & ~7; }
+
+// ---- tensor-core variant of the network (north_star: "tensor cores only for the per-atom descriptor x W0 layer and
+//      only if ncu shows it beats CUDA-core FMA"; measured verdict in DESIGN.md section 5 / profiles/r2_*).
+// A warp tile is 32 atoms: Z[32 x NP] = X[32 x KP] W0^T, then Fp[32 x KP] = T[32 x NP] W0 with T = w1 (1 - tanh^2).
+// mma.sync m16n8k8 TF32 with the 3-term operand split x = x_hi + x_lo (x_hi w_hi + x_hi w_lo + x_lo w_hi: fp32-grade
+// products, fp32 accumulation).  The C fragments of Z are turned into the A fragments of T in place (the neuron index
+// of the second product is permuted consistently in A and B), so nothing moves between the two products.
+__device__ __forceinline__ unsigned tf32_hi(float x) {
+  unsigned r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+  return r;
+}
+__device__ __forceinline__ void tf32_split(float x, unsigned& hi, unsigned& lo) {
+  hi = tf32_hi(x);
+  lo = tf32_hi(x - __uint_as_float(hi));
+}
+__device__ __forceinline__ void mma_tf32(float c[4], const unsigned a[4], unsigned b0, unsigned b1) {
+  asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+// c += a * b with the 3-term split; a given as (hi, lo) fragments, b as two fp32 values split here
+__device__ __forceinline__ void mma_3xtf32(float c[4], const unsigned ah[4], const unsigned al[4], float b0, float b1) {
+  unsigned bh0, bl0, bh1, bl1;
+  tf32_split(b0, bh0, bl0);
+  tf32_split(b1, bh1, bl1);
+  mma_tf32(c, al, bh0, bh1);
+  mma_tf32(c, ah, bl0, bl1);
+  mma_tf32(c, ah, bh0, bh1);
+}
+template <class MS, bool MMA = false>
 __global__ void __launch_bounds__(ANG_THREADS, 8)
 k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
              const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
@@ -435,6 +491,11 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
   // the constant bank cost 2.4x the one-type kernel time)
   const float* s_cta = s_qs + DPAD;
   constexpr int CT_FLOATS = MS::NT > 1 ? (2 * MS::NT * MS::NT * NA * KA + 3) / 4 * 4 : 0;
+  // MMA: the warp's X / Fp tile [32][XS] and its 32 site energies behind the tables (XS = 4 mod 32: fragment loads
+  // hit 32 distinct banks)
+  constexpr int KP = (D + 7) / 8 * 8, XS = KP + 4;
+  float* s_x = smem + (nrow * DPAD + 2 * nrow + DPAD + CT_FLOATS);
+  float* s_u = s_x + 32 * XS;
   {  // all loads of a thread in flight at once (the table is a multiple of 4 floats, 16-byte aligned)
     const int n4 = (nrow * DPAD + 2 * nrow + DPAD + CT_FLOATS) / 4;
     const float4* src = reinterpret_cast<const float4*>(nnw);
@@ -477,13 +538,17 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     const int s2 = (tile + nslots) * 32 + (threadIdx.x & 31);
     const bool v2 = tile + nslots < ntiles && s2 < n;
     mask_nx = v2 ? amask[s2] : 0ull;
-    if (s >= n) continue;
-    const int nc = __popcll(mask);
-    const float4* dp = adisp + s;
-    const int ti = MS::NT > 1 ? xyzt[s].w : 0;  // type of the central atom (selects the c^{ti tj} tables)
+    // the tensor-core variant needs all 32 lanes in the network: a lane beyond the last atom carries an empty site
+    // (no neighbours, nothing written); the FFMA variant lets it skip the tile
+    const bool live = s < n;
+    if (!MMA && !live) continue;
+    const int sl = live ? s : 0;
+    const int nc = live ? __popcll(mask) : 0;
+    const float4* dp = adisp + sl;
+    const int ti = MS::NT > 1 ? xyzt[sl].w : 0;  // type of the central atom (selects the c^{ti tj} tables)
     float qr[NR];
 #pragma unroll
-    for (int nq = 0; nq < NR; ++nq) qr[nq] = q_radial[(size_t)nq * npad + s];
+    for (int nq = 0; nq < NR; ++nq) qr[nq] = q_radial[(size_t)nq * npad + sl];
 
     // ---- S4 forward: A[n][lm] = sum_j g_n(r_ij) b_lm(rhat_ij), two neighbours per iteration
     float A[NA][24];
@@ -559,7 +624,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
         dq4[nq][4] = k3 * cxy;
       }
     }
-    if (q_out) {
+    if (q_out && live) {
 #pragma unroll
       for (int v = 0; v < D; ++v) q_out[(size_t)v * npad + s] = q[v];
     }
@@ -571,7 +636,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       q[v] *= s_qs[v];
       Fp[v] = 0.0f;
     }
-    if (da.dense_list) {  // large angular inputs: fp32 sums are not accurate enough, list the atom for the fp64 pass
+    if (da.dense_list && live) {  // large angular inputs: fp32 sums are not accurate enough, list the atom for the fp64 pass
       float mx = 0.0f, mx4 = 0.0f;
 #pragma unroll
       for (int v = NR; v < NR + 4 * NA; ++v) mx = fmaxf(mx, fabsf(q[v]));
@@ -580,6 +645,103 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       if (!(mx <= mt.dense_thr) || !(mx4 <= mt.dense_thr4)) da.dense_list[atomicAdd(&da.sc->dense_count, 1)] = s;
     }
     float U = -mt.b1;
+    if (MMA) {
+      // ---- tensor-core path: this thread's row of X to shared memory, fragments from there
+      const int lane = threadIdx.x & 31, g = lane >> 2, tig = lane & 3;
+      __syncwarp();
+#pragma unroll
+      for (int v4 = 0; v4 < KP / 4; ++v4) {
+        float4 t4;
+        t4.x = 4 * v4 + 0 < D ? q[4 * v4 + 0 < D ? 4 * v4 + 0 : 0] : 0.0f;
+        t4.y = 4 * v4 + 1 < D ? q[4 * v4 + 1 < D ? 4 * v4 + 1 : 0] : 0.0f;
+        t4.z = 4 * v4 + 2 < D ? q[4 * v4 + 2 < D ? 4 * v4 + 2 : 0] : 0.0f;
+        t4.w = 4 * v4 + 3 < D ? q[4 * v4 + 3 < D ? 4 * v4 + 3 : 0] : 0.0f;
+        *reinterpret_cast<float4*>(s_x + lane * XS + 4 * v4) = t4;
+      }
+      __syncwarp();
+      // A fragments of X (hi / lo), both 16-row halves of the tile, all k-steps
+      unsigned xh[2][KP / 8][4], xl[2][KP / 8][4];
+#pragma unroll
+      for (int mtl = 0; mtl < 2; ++mtl)
+#pragma unroll
+        for (int ks = 0; ks < KP / 8; ++ks) {
+          const float* xp = s_x + (16 * mtl + g) * XS + 8 * ks + tig;
+          tf32_split(xp[0], xh[mtl][ks][0], xl[mtl][ks][0]);
+          tf32_split(xp[8 * XS], xh[mtl][ks][1], xl[mtl][ks][1]);
+          tf32_split(xp[4], xh[mtl][ks][2], xl[mtl][ks][2]);
+          tf32_split(xp[8 * XS + 4], xh[mtl][ks][3], xl[mtl][ks][3]);
+        }
+      float fpc[2][KP / 8][4];  // Fp tile in C fragments
+#pragma unroll
+      for (int mtl = 0; mtl < 2; ++mtl)
+#pragma unroll
+        for (int nt = 0; nt < KP / 8; ++nt)
+#pragma unroll
+          for (int e = 0; e < 4; ++e) fpc[mtl][nt][e] = 0.0f;
+      float ur[2][2] = {{0.0f, 0.0f}, {0.0f, 0.0f}};  // site-energy parts of rows g, g + 8 of both halves
+#pragma unroll 1
+      for (int nt = 0; nt < nrow / 8; ++nt) {  // 8 neurons at a time: Z tile -> tanh -> T -> Fp += T W0
+        float z[2][4];
+        const float bz0 = s_b0[8 * nt + 2 * tig], bz1 = s_b0[8 * nt + 2 * tig + 1];
+#pragma unroll
+        for (int mtl = 0; mtl < 2; ++mtl) { z[mtl][0] = -bz0; z[mtl][1] = -bz1; z[mtl][2] = -bz0; z[mtl][3] = -bz1; }
+#pragma unroll
+        for (int ks = 0; ks < KP / 8; ++ks) {  // B[k][n] = W0[neuron 8 nt + n][8 ks + k]
+          const float* wp = s_w0 + (8 * nt + g) * DPAD + 8 * ks + tig;
+          const float b0v = 8 * ks + tig < DPAD ? wp[0] : 0.0f, b1v = 8 * ks + tig + 4 < DPAD ? wp[4] : 0.0f;
+          mma_3xtf32(z[0], xh[0][ks], xl[0][ks], b0v, b1v);
+          mma_3xtf32(z[1], xh[1][ks], xl[1][ks], b0v, b1v);
+        }
+        const float w1a = s_w1[8 * nt + 2 * tig], w1b = s_w1[8 * nt + 2 * tig + 1];
+        unsigned th[2][4], tl[2][4];
+#pragma unroll
+        for (int mtl = 0; mtl < 2; ++mtl) {
+          const float h0 = tanh_fast(z[mtl][0]), h1 = tanh_fast(z[mtl][1]), h2 = tanh_fast(z[mtl][2]), h3 = tanh_fast(z[mtl][3]);
+          ur[mtl][0] = fmaf(w1b, h1, fmaf(w1a, h0, ur[mtl][0]));
+          ur[mtl][1] = fmaf(w1b, h3, fmaf(w1a, h2, ur[mtl][1]));
+          // A fragment of T for the second product, neuron order permuted: k' = tig <-> neuron 2 tig, k' = tig + 4 <-> 2 tig + 1
+          tf32_split(w1a * fmaf(-h0, h0, 1.0f), th[mtl][0], tl[mtl][0]);
+          tf32_split(w1a * fmaf(-h2, h2, 1.0f), th[mtl][1], tl[mtl][1]);
+          tf32_split(w1b * fmaf(-h1, h1, 1.0f), th[mtl][2], tl[mtl][2]);
+          tf32_split(w1b * fmaf(-h3, h3, 1.0f), th[mtl][3], tl[mtl][3]);
+        }
+#pragma unroll
+        for (int n2 = 0; n2 < KP / 8; ++n2) {  // B[k'][n] = W0[neuron 8 nt + 2 tig (+1)][8 n2 + n]
+          const float* wp = s_w0 + (8 * nt + 2 * tig) * DPAD + 8 * n2 + g;
+          const float b0v = 8 * n2 + g < DPAD ? wp[0] : 0.0f, b1v = 8 * n2 + g < DPAD ? wp[DPAD] : 0.0f;
+          mma_3xtf32(fpc[0][n2], th[0], tl[0], b0v, b1v);
+          mma_3xtf32(fpc[1][n2], th[1], tl[1], b0v, b1v);
+        }
+      }
+      // rows complete across the four lanes of a group; results back to the owning threads through shared memory
+#pragma unroll
+      for (int mtl = 0; mtl < 2; ++mtl)
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+          float u = ur[mtl][hf];
+          u += __shfl_xor_sync(0xffffffffu, u, 1);
+          u += __shfl_xor_sync(0xffffffffu, u, 2);
+          if (tig == 0) s_u[16 * mtl + 8 * hf + g] = u;
+        }
+      __syncwarp();
+#pragma unroll
+      for (int mtl = 0; mtl < 2; ++mtl)
+#pragma unroll
+        for (int n2 = 0; n2 < KP / 8; ++n2) {
+          *reinterpret_cast<float2*>(s_x + (16 * mtl + g) * XS + 8 * n2 + 2 * tig) = make_float2(fpc[mtl][n2][0], fpc[mtl][n2][1]);
+          *reinterpret_cast<float2*>(s_x + (16 * mtl + 8 + g) * XS + 8 * n2 + 2 * tig) = make_float2(fpc[mtl][n2][2], fpc[mtl][n2][3]);
+        }
+      __syncwarp();
+      U += s_u[lane];
+#pragma unroll
+      for (int v4 = 0; v4 < KP / 4; ++v4) {
+        const float4 t4 = *reinterpret_cast<const float4*>(s_x + lane * XS + 4 * v4);
+        if (4 * v4 + 0 < D) Fp[4 * v4 + 0 < D ? 4 * v4 + 0 : 0] = t4.x;
+        if (4 * v4 + 1 < D) Fp[4 * v4 + 1 < D ? 4 * v4 + 1 : 0] = t4.y;
+        if (4 * v4 + 2 < D) Fp[4 * v4 + 2 < D ? 4 * v4 + 2 : 0] = t4.z;
+        if (4 * v4 + 3 < D) Fp[4 * v4 + 3 < D ? 4 * v4 + 3 : 0] = t4.w;
+      }
+    } else {
     // software pipeline: the pre-activations of neurons m+2, m+3 are accumulated while the tanh of
     // neurons m, m+1 (two dependent MUFU ops) is in flight; rows neu2, neu2+1 of w0/b0 are zero padding
     auto preact = [&](int m, float& za, float& zb) {
@@ -618,13 +780,16 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
         if (4 * v4 + 3 < D) Fp[4 * v4 + 3] = fmaf(tb, x.w, fmaf(ta, w.w, Fp[4 * v4 + 3]));
       }
     }
+    }
 #pragma unroll
     for (int v = 0; v < D; ++v) Fp[v] *= s_qs[v];
-    u_site[s] = U;
+    if (live) u_site[s] = U;
 
     // record for the radial back-pass of k_force: position + Fp[0..NR-1] (32 bytes) or position +
     // d_k = sum_n Fp_n ct_nk (64 bytes), see ModelShape::FPREC
-    if (MS::FPREC) {
+    if (!live) {
+      // nothing to record for an empty lane
+    } else if (MS::FPREC) {
       const int4 me = xyzt[s];
       float f[5];
 #pragma unroll
@@ -676,7 +841,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       pre0 = c2 > 0 ? adisp[v2 ? s2 : 0] : dummy;
       pre1 = c2 > 1 ? adisp[(size_t)npad + (v2 ? s2 : 0)] : dummy;
     }
-    for (unsigned long long m = mask; m; m &= m - 1, ++c) {
+    for (unsigned long long m = live ? mask : 0ull; m; m &= m - 1, ++c) {
       const int a = __ffsll((long long)m) - 1;
       const float dx = nx.x, dy = nx.y, dz = nx.z, tjw = nx.w;
       nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration

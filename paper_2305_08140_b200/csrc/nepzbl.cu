@@ -30,7 +30,7 @@ constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
-      nn_r, nn_a, shellq, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, dense_list, md_force, md_energy,
+      nn_r, nn_a, shellq, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, dense_list, tiles, nl_loc, md_force, md_energy,
       partial, nhc_partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
@@ -66,6 +66,7 @@ struct nepzbl_handle {
   ZblParams zp{};
   SiteModel site{};           // fp64 tables of k_site_fp64 (d_site holds them)
   double* d_site = nullptr;
+  bool nn_mma = false;        // NEPZBL_NN_MMA=1: network of k_angular_nn on the tensor cores (mma.sync 3xTF32; experiment)
   bool dense_on = true;       // NEPZBL_DENSE_THRESHOLD=off disables the fp64 re-evaluation (measurement aid)
   size_t smem_nn = 0;
   // threads per block of k_radial / k_force: one warp while the grid is only a few waves of resident threads (the
@@ -161,6 +162,12 @@ inline size_t al(size_t x) { return (x + 255) & ~size_t(255); }
 // 32-bit words of the per-lane in-cutoff mask: lane p of RADIAL_LANES owns entries p, p+4, ...
 inline int mask_words(const nepzbl_params& p) { return (p.cap_radial + 32 * RADIAL_LANES - 1) / (32 * RADIAL_LANES); }
 
+// NEPZBL_STAGE=1|2: neighbour tiles staged in shared memory by k_radial (stage.cuh; measurement aid, default off)
+inline int stage_mode() {
+  static const int m = [] { const char* e = getenv("NEPZBL_STAGE"); const int v = e ? atoi(e) : 0; return v == 1 || v == 2 ? v : 0; }();
+  return m;
+}
+
 Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   Carve c{};
   long long npad = (n_cap + 127) / 128 * 128;
@@ -194,6 +201,10 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.q_desc = take(4 * (size_t)D * npad);
   c.zbl_list = take(4 * npad);
   c.dense_list = take(4 * npad);
+  if (stage_mode() > 0) {  // neighbour-tile staging experiment (stage.cuh)
+    c.tiles = take(sizeof(TileDesc) * (size_t)(npad / STAGE_TILE + 1));
+    c.nl_loc = take(2 * (size_t)p.cap_radial * npad);
+  }
   c.md_force = take(12 * npad);
   c.md_energy = take(8 * npad);
   c.partial = take(16 * 1024);
@@ -284,6 +295,7 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
     const size_t nrow = (size_t)nn_rows(p->n_neurons);
     h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
     if (MS::NT > 1) h->smem_nn += sizeof(float) * ((2 * MS::NT * MS::NT * MS::NA * MS::KA + 3) / 4 * 4);
+    if (h->nn_mma) h->smem_nn += sizeof(float) * (32 * ((MS::D + 7) / 8 * 8 + 4) + 32);  // X / Fp tile and site energies
   }
 }
 
@@ -461,6 +473,12 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
                                        (float)h->p.rc_radial, (float)(h->p.skin / 8.0));
   k_rev<<<blocks(n, 128), 128, 0, st>>>(h->d_sc, n, npad, h->at<int>(c.nn_a), h->at<int>(c.nl_r),
                                        h->at<unsigned char>(c.rev));
+  if (stage_mode() > 0) {
+    k_tiles<<<blocks(n, STAGE_TILE), STAGE_TILE, 0, st>>>(h->d_sc, h->d_bm, n, npad, h->at<int>(c.perm), h->at<int>(c.cell_of),
+                                                         h->at<int>(c.cell_start), h->at<int>(c.nn_r), h->at<int>(c.nl_r),
+                                                         h->at<TileDesc>(c.tiles), h->at<unsigned short>(c.nl_loc));
+    nk++;
+  }
   return nk + 9;
 }
 
@@ -487,22 +505,37 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
   const int gb = h->gather_block ? h->gather_block : ((long long)n * RADIAL_LANES < 8ll * 1024 * h->n_sm ? 32 : 64);
   prof_mark(h, PK_RADIAL);
-  auto launch_radial = [&](auto tri) {
-    k_radial<MS, decltype(tri)::value><<<blocks((long long)n * RADIAL_LANES, gb), gb, 0, st>>>(
+  auto launch_radial = [&](auto tri, auto stage) {
+    constexpr int STAGE = decltype(stage)::value;
+    const int blk = STAGE ? STAGE_TILE * RADIAL_LANES : gb;
+    const size_t smem = STAGE ? ((sizeof(TileDesc) + 8 + 15) / 16) * 16 + sizeof(int4) * STAGE_CAP : 0;
+    if (STAGE) cudaFuncSetAttribute((const void*)k_radial<MS, decltype(tri)::value, STAGE>,
+                                    cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    k_radial<MS, decltype(tri)::value, STAGE><<<blocks((long long)n * RADIAL_LANES, blk), blk, smem, st>>>(
         h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
         h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p), h->at<int>(c.zbl_list),
         h->at<int>(c.nn_a), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp),
-        h->at<unsigned long long>(c.shellq));
+        h->at<unsigned long long>(c.shellq), STAGE ? h->at<TileDesc>(c.tiles) : nullptr,
+        STAGE ? h->at<unsigned short>(c.nl_loc) : nullptr);
   };
-  if (h->tri) launch_radial(std::true_type{}); else launch_radial(std::false_type{});
+  using std::integral_constant;
+  if (h->tri) launch_radial(std::true_type{}, integral_constant<int, 0>{});
+  else if (std::is_same<MS, MS0>::value && stage_mode() == 1) launch_radial(std::false_type{}, integral_constant<int, std::is_same<MS, MS0>::value ? 1 : 0>{});
+  else if (std::is_same<MS, MS0>::value && stage_mode() == 2) launch_radial(std::false_type{}, integral_constant<int, std::is_same<MS, MS0>::value ? 2 : 0>{});
+  else launch_radial(std::false_type{}, integral_constant<int, 0>{});
   prof_mark(h, PK_ANGULAR_NN);
   if constexpr (kSplit<MS>)
     k_angular_nn_split<MS><<<std::min(blocks((long long)n * SPLIT_LANES, SPLIT_THREADS), h->ang_grid), SPLIT_THREADS, h->smem_nn, st>>>(
         n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
         h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
         want_q ? h->at<float>(c.q_desc) : nullptr, da);
+  else if (h->nn_mma)
+    k_angular_nn<MS, true><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
+        n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
+        h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
+        want_q ? h->at<float>(c.q_desc) : nullptr, da);
   else
-    k_angular_nn<MS><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
+    k_angular_nn<MS, false><<<std::min(blocks(n, ANG_THREADS), h->ang_grid), ANG_THREADS, h->smem_nn, st>>>(
         n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
         h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
         want_q ? h->at<float>(c.q_desc) : nullptr, da);
@@ -526,7 +559,6 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
     if (h->tri) launch_force_t(vir, std::integral_constant<int, 64>{}, std::true_type{});
     else launch_force_t(vir, blk, std::false_type{});
   };
-  using std::integral_constant;
   if (virial) {
     if (gb == 32) launch_force(std::true_type{}, integral_constant<int, 32>{});
     else launch_force(std::true_type{}, integral_constant<int, 64>{});
@@ -760,6 +792,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     int v = atoi(gb);
     if (v == 32 || v == 64) h->gather_block = v;
   }
+  if (const char* nm = getenv("NEPZBL_NN_MMA")) h->nn_mma = nm[0] == '1';
   std::vector<float> nnw;
   with_shape(shape, [&](auto ms) {
     using MS = decltype(ms);
@@ -804,7 +837,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     with_shape(shape, [&](auto ms) {
       using MS = decltype(ms);
       if constexpr (kSplit<MS>) { fn = (const void*)k_angular_nn_split<MS>; threads = SPLIT_THREADS; }
-      else fn = (const void*)k_angular_nn<MS>;
+      else fn = h->nn_mma ? (const void*)k_angular_nn<MS, true> : (const void*)k_angular_nn<MS, false>;
     });
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_nn)) != cudaSuccess) return die("cudaFuncSetAttribute(k_angular_nn)", ce);
     int per_sm = 0;
