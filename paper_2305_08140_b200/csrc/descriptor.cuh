@@ -19,6 +19,7 @@
 #pragma once
 #include "common.cuh"
 #include "stage.cuh"
+#include "tc05.cuh"
 
 template <int NR_, int KR_, int NA_, int KA_, bool B4_, int NT_ = 1, bool B5_ = false>
 struct ModelShape {
@@ -469,8 +470,34 @@ __device__ __forceinline__ void mma_3xtf32(float c[4], const unsigned ah[4], con
   mma_tf32(c, ah, bl0, bl1);
   mma_tf32(c, ah, bh0, bh1);
 }
-template <class MS, bool MMA = false>
-__global__ void __launch_bounds__(ANG_THREADS, 8)
+// ---- tcgen05 variant of the network (NN = 2): the Blackwell-native form of the same two products.  A block is FOUR
+//      warps = a tile of 128 atoms = the M = 128 rows of one tcgen05.mma; the accumulators live in tensor memory, where
+//      row r belongs to thread r (tcgen05.ld 32x32b), so pre-activations and dU/dq arrive in the thread that owns the
+//      atom and nothing is shuffled.  Per tile:  every thread stores its scaled descriptor row, split x = hi + lo (tf32
+//      + remainder), K-major into shared memory (column D carries the constant 1 against -b0) -> one thread issues
+//      Z = X W0^T as hi*hi + hi*lo + lo*hi (kind::tf32, fp32 accumulation in TMEM) and commits to an mbarrier -> every
+//      thread reads its 8-neuron chunks of Z, takes tanh, accumulates U and stores T = w1 (1 - h^2) split the same way
+//      -> Fp = T W0 in two K halves (neurons 0..31 while the threads are still working on neurons 32..).
+//      W0 / W0^T are split once per block.  Layouts and descriptors: tc05.cuh.
+struct TcShape {
+  int kp;   // K of the first product: D + 1 (bias column) rounded up to 8
+  int kn;   // N of the second product: D rounded up to 16 (tcgen05: N % 16 == 0 at M = 128)
+};
+template <class MS>
+__host__ __device__ constexpr TcShape tc_shape() { return TcShape{(MS::D + 1 + 7) / 8 * 8, (MS::D + 15) / 16 * 16}; }
+#define TC_NP 64        // neurons padded to the N of the first product (n_neurons <= 64 - 8 for this variant)
+#define TC_TMEM_COLS 128  // Z: columns 0..63, Fp: columns 64..64+kn-1
+template <class MS>
+__host__ __device__ constexpr size_t tc_smem_bytes() {
+  // B1 hi/lo [64][kp] + B2 hi/lo [kn][64] + X hi/lo [128][max(kp,32)] + T hi/lo [128][32] + barrier block, 128-byte aligned
+  constexpr TcShape t = tc_shape<MS>();
+  constexpr int kx = t.kp > 32 ? t.kp : 32;
+  return 128 + 4 * (size_t)(2 * TC_NP * t.kp + 2 * t.kn * TC_NP + 2 * 128 * kx + 2 * 128 * 32) + 64;
+}
+
+// NN: 0 = network on the CUDA cores (FFMA, weights broadcast from shared memory), 1 = mma.sync 3xTF32, 2 = tcgen05
+template <class MS, int NN = 0>
+__global__ void __launch_bounds__(NN == 2 ? 128 : ANG_THREADS, NN == 2 ? 2 : 8)
 k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
              const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
              const __grid_constant__ ModelTables<MS> mt, const float* __restrict__ nnw,
@@ -478,7 +505,9 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
              AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out,
              const DenseArgs da) {
   constexpr int NA = MS::NA, KA = MS::KA, NR = MS::NR, KR = MS::KR, D = MS::D, DPAD = MS::DPAD;
-  constexpr int T_ = ANG_THREADS;
+  constexpr bool MMA = NN == 1;
+  constexpr bool TC = NN == 2;
+  constexpr int T_ = TC ? 128 : ANG_THREADS;
   extern __shared__ __align__(16) float smem[];
   const int neu2 = (mt.n_neurons + 1) & ~1;
   const int nrow = nn_rows(mt.n_neurons);  // zero rows beyond n_neurons (host: build_nnw)
@@ -509,10 +538,54 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     }
   }
   __syncthreads();
+  // TC: operand tiles behind the tables (128-byte aligned), tensor memory, the mbarrier the MMAs commit to
+  constexpr TcShape tcs = tc_shape<MS>();
+  constexpr int TKP = tcs.kp, TKN = tcs.kn, TKX = TKP > 32 ? TKP : 32;
+  float *tB1h = nullptr, *tB1l = nullptr, *tB2h = nullptr, *tB2l = nullptr, *tXh = nullptr, *tXl = nullptr, *tTh = nullptr, *tTl = nullptr;
+  uint32_t tc_mbar = 0, tc_tmem = 0, tc_phase = 0;
+  if (TC) {
+    const uintptr_t base = (reinterpret_cast<uintptr_t>(smem + (nrow * DPAD + 2 * nrow + DPAD + CT_FLOATS)) + 127) & ~uintptr_t(127);
+    tB1h = reinterpret_cast<float*>(base);   // [64 neurons][TKP]   B of Z = X W0^T (column D: -b0)
+    tB1l = tB1h + TC_NP * TKP;
+    tB2h = tB1l + TC_NP * TKP;               // [TKN components][64 neurons]   B of Fp = T W0
+    tB2l = tB2h + TKN * TC_NP;
+    tXh = tB2l + TKN * TC_NP;                // [128 atoms][TKX]: X, later the second half of T
+    tXl = tXh + 128 * TKX;
+    tTh = tXl + 128 * TKX;                   // [128 atoms][32]: first half of T
+    tTl = tTh + 128 * 32;
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(tTl + 128 * 32);
+    uint32_t* tbase = reinterpret_cast<uint32_t*>(bar + 1);
+    for (int e = threadIdx.x; e < TC_NP * TKP; e += T_) {
+      const int m = e / TKP, k = e % TKP;
+      const float w = m < nrow ? (k < D ? s_w0[m * DPAD + k] : (k == D ? -s_b0[m] : 0.0f)) : 0.0f;
+      float hi, lo;
+      tc05::split_tf32(w, hi, lo);
+      *reinterpret_cast<float*>(reinterpret_cast<char*>(tB1h) + tc05::tile_off(TC_NP, m, k)) = hi;
+      *reinterpret_cast<float*>(reinterpret_cast<char*>(tB1l) + tc05::tile_off(TC_NP, m, k)) = lo;
+    }
+    for (int e = threadIdx.x; e < TKN * TC_NP; e += T_) {
+      const int v = e / TC_NP, m = e % TC_NP;
+      const float w = (m < nrow && v < D) ? s_w0[m * DPAD + v] : 0.0f;
+      float hi, lo;
+      tc05::split_tf32(w, hi, lo);
+      *reinterpret_cast<float*>(reinterpret_cast<char*>(tB2h) + tc05::tile_off(TKN, v, m)) = hi;
+      *reinterpret_cast<float*>(reinterpret_cast<char*>(tB2l) + tc05::tile_off(TKN, v, m)) = lo;
+    }
+    tc_mbar = tc05::smem_u32(bar);
+    if (threadIdx.x < 32) tc05::tmem_alloc<TC_TMEM_COLS>(tc05::smem_u32(tbase));
+    if (threadIdx.x == 0) tc05::mbar_init(tc_mbar, 1);
+    tc05::fence_smem_to_async();
+    tc05::fence_before_sync();
+    __syncthreads();
+    tc05::fence_after_sync();
+    tc_tmem = *tbase;
+  }
   // Work is handed out per WARP (tiles of 32 atoms; nothing below synchronises the block), with warp
   // slot = warp_in_block * gridDim.x + blockIdx.x, so that the partly filled last round (4000 warp tiles
   // over 1184 resident warps at 128 000 atoms) is spread over all SMs instead of landing on the first
   // blocks only (measured: no difference at 128 000 atoms, 108.7 us either way).
+  // TC: the four warps of a block take four consecutive warp tiles (the block synchronises around its MMAs, so
+  // all of them make the same number of rounds; a warp past the end carries empty sites).
   const int ntiles = (n + 31) / 32;
   const int nslots = gridDim.x * (T_ / 32);
 
@@ -520,7 +593,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
   // warps per scheduler cannot hide, so it is issued one tile ahead: the next tile's mask at the start of this
   // tile, its first two displacement vectors before this tile's back-pass.
   const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
-  int tile = (threadIdx.x >> 5) * gridDim.x + blockIdx.x;
+  int tile = TC ? blockIdx.x * (T_ / 32) + (threadIdx.x >> 5) : (threadIdx.x >> 5) * gridDim.x + blockIdx.x;
   unsigned long long mask_nx = 0ull;
   float4 pre0 = dummy, pre1 = dummy;
   {
@@ -532,7 +605,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       pre1 = c0 > 1 ? adisp[(size_t)npad + s0] : dummy;
     }
   }
-  for (; tile < ntiles; tile += nslots) {
+  for (; TC ? tile - (int)(threadIdx.x >> 5) < ntiles : tile < ntiles; tile += nslots) {
     const int s = tile * 32 + (threadIdx.x & 31);
     const unsigned long long mask = mask_nx;
     const int s2 = (tile + nslots) * 32 + (threadIdx.x & 31);
@@ -541,7 +614,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     // the tensor-core variant needs all 32 lanes in the network: a lane beyond the last atom carries an empty site
     // (no neighbours, nothing written); the FFMA variant lets it skip the tile
     const bool live = s < n;
-    if (!MMA && !live) continue;
+    if (!MMA && !TC && !live) continue;
     const int sl = live ? s : 0;
     const int nc = live ? __popcll(mask) : 0;
     const float4* dp = adisp + sl;
@@ -645,7 +718,108 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       if (!(mx <= mt.dense_thr) || !(mx4 <= mt.dense_thr4)) da.dense_list[atomicAdd(&da.sc->dense_count, 1)] = s;
     }
     float U = -mt.b1;
-    if (MMA) {
+    if (TC) {
+      // ---- tcgen05 path (see the comment above the kernel).  Row of X: q (scaled), 1 in column D, zeros beyond.
+      char* const xh = reinterpret_cast<char*>(tXh), * const xl = reinterpret_cast<char*>(tXl);
+#pragma unroll
+      for (int v4 = 0; v4 < TKP / 4; ++v4) {
+        float4 h4, l4;
+        float* hp = &h4.x;
+        float* lp = &l4.x;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int v = 4 * v4 + e;
+          const float x = v < D ? q[v < D ? v : 0] : (v == D ? 1.0f : 0.0f);
+          tc05::split_tf32(x, hp[e], lp[e]);
+        }
+        *reinterpret_cast<float4*>(xh + tc05::tile_off(128, threadIdx.x, 4 * v4)) = h4;
+        *reinterpret_cast<float4*>(xl + tc05::tile_off(128, threadIdx.x, 4 * v4)) = l4;
+      }
+      tc05::fence_smem_to_async();
+      tc05::fence_before_sync();
+      __syncthreads();
+      if (threadIdx.x == 0) {  // Z[128 x 64] = X[128 x TKP] B1^T, K = 8 per instruction
+        tc05::fence_after_sync();
+        constexpr uint32_t id1 = tc05::idesc_tf32(128, TC_NP);
+#pragma unroll
+        for (int ks = 0; ks < TKP / 8; ++ks) {
+          const uint32_t ao = ks * 2 * 16 * 128, bo = ks * 2 * 16 * TC_NP;
+          const uint64_t ah = tc05::smem_desc(tc05::smem_u32(tXh) + ao, 16 * 128, 128);
+          const uint64_t al = tc05::smem_desc(tc05::smem_u32(tXl) + ao, 16 * 128, 128);
+          const uint64_t bh = tc05::smem_desc(tc05::smem_u32(tB1h) + bo, 16 * TC_NP, 128);
+          const uint64_t bl = tc05::smem_desc(tc05::smem_u32(tB1l) + bo, 16 * TC_NP, 128);
+          tc05::mma_tf32(tc_tmem, al, bh, id1, ks > 0);
+          tc05::mma_tf32(tc_tmem, ah, bl, id1, true);
+          tc05::mma_tf32(tc_tmem, ah, bh, id1, true);
+        }
+        tc05::commit(tc_mbar);
+      }
+      __syncwarp();
+      tc05::mbar_wait(tc_mbar, tc_phase);
+      tc_phase ^= 1u;
+      tc05::fence_after_sync();
+      const uint32_t trow = tc_tmem + ((uint32_t)(threadIdx.x & 96) << 16);  // TMEM lane base of this warp: 32 (warp % 4)
+#pragma unroll 1
+      for (int half = 0; half < 2; ++half) {
+        // neurons 32 half .. : tanh, site energy, T = w1 (1 - h^2) split into the A tile of the second product
+        // (half 0 -> its own tile; half 1 -> X's tile, which the first product has finished reading)
+        char* const th = reinterpret_cast<char*>(half ? tXh : tTh), * const tl = reinterpret_cast<char*>(half ? tXl : tTl);
+        const int m_end = min(nrow, 32 * half + 32);
+#pragma unroll 1
+        for (int m0 = 32 * half; m0 < m_end; m0 += 8) {
+          float z[8];
+          tc05::tmem_ld8(trow + m0, z);
+          float4 h4[2], l4[2];
+          float* hp = &h4[0].x;
+          float* lp = &l4[0].x;
+#pragma unroll
+          for (int e = 0; e < 8; ++e) {
+            const float hh = tanh_fast(z[e]);
+            const float w1 = s_w1[m0 + e];  // zero in the padding rows
+            U = fmaf(w1, hh, U);
+            tc05::split_tf32(w1 * fmaf(-hh, hh, 1.0f), hp[e], lp[e]);
+          }
+          const int kk = m0 - 32 * half;
+          *reinterpret_cast<float4*>(th + tc05::tile_off(128, threadIdx.x, kk)) = h4[0];
+          *reinterpret_cast<float4*>(th + tc05::tile_off(128, threadIdx.x, kk + 4)) = h4[1];
+          *reinterpret_cast<float4*>(tl + tc05::tile_off(128, threadIdx.x, kk)) = l4[0];
+          *reinterpret_cast<float4*>(tl + tc05::tile_off(128, threadIdx.x, kk + 4)) = l4[1];
+        }
+        tc05::fence_smem_to_async();
+        tc05::fence_before_sync();
+        __syncthreads();
+        if (threadIdx.x == 0) {  // Fp[128 x TKN] += T[128 x (this half's neurons)] B2^T
+          tc05::fence_after_sync();
+          constexpr uint32_t id2 = tc05::idesc_tf32(128, TKN);
+          const int nks = (m_end - 32 * half) / 8;
+#pragma unroll 1
+          for (int ks = 0; ks < nks; ++ks) {
+            const uint32_t ao = ks * 2 * 16 * 128, bo = (8 * half + 2 * ks) * 16 * TKN;
+            const uint64_t ah = tc05::smem_desc(tc05::smem_u32(half ? tXh : tTh) + ao, 16 * 128, 128);
+            const uint64_t al = tc05::smem_desc(tc05::smem_u32(half ? tXl : tTl) + ao, 16 * 128, 128);
+            const uint64_t bh = tc05::smem_desc(tc05::smem_u32(tB2h) + bo, 16 * TKN, 128);
+            const uint64_t bl = tc05::smem_desc(tc05::smem_u32(tB2l) + bo, 16 * TKN, 128);
+            tc05::mma_tf32(tc_tmem + TC_NP, al, bh, id2, half > 0 || ks > 0);
+            tc05::mma_tf32(tc_tmem + TC_NP, ah, bl, id2, true);
+            tc05::mma_tf32(tc_tmem + TC_NP, ah, bh, id2, true);
+          }
+          if (half) tc05::commit(tc_mbar);
+        }
+        __syncwarp();
+      }
+      tc05::mbar_wait(tc_mbar, tc_phase);
+      tc_phase ^= 1u;
+      tc05::fence_after_sync();
+#pragma unroll
+      for (int c = 0; c < (D + 7) / 8 * 8; c += 8) {
+        float f[8];
+        tc05::tmem_ld8(trow + TC_NP + c, f);
+#pragma unroll
+        for (int e = 0; e < 8; ++e)
+          if (c + e < D) Fp[c + e < D ? c + e : 0] = f[e];
+      }
+      tc05::fence_before_sync();  // the next tile's products (behind its __syncthreads) overwrite Z and Fp
+    } else if (MMA) {
       // ---- tensor-core path: this thread's row of X to shared memory, fragments from there
       const int lane = threadIdx.x & 31, g = lane >> 2, tig = lane & 3;
       __syncwarp();
@@ -885,5 +1059,10 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       float pz = fmaf(uz, Sp, (vz - uz * uv) * rinv);
       pforce[(size_t)a * npad + s] = make_float4(px, py, pz, 0.0f);
     }
+  }
+  if (TC) {
+    tc05::fence_before_sync();
+    __syncthreads();
+    if (threadIdx.x < 32) tc05::tmem_dealloc<TC_TMEM_COLS>(tc_tmem);
   }
 }
