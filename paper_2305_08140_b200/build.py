@@ -10,7 +10,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libnepzbl.so")
 SOURCES = ["nepzbl.cu"]
-HEADERS = ["common.cuh", "neighbor.cuh", "descriptor.cuh", "force.cuh", "integrate.cuh", "wigner_seitz.cuh", "descriptor_split.cuh", "site_fp64.cuh", "stage.cuh"]
+HEADERS = ["common.cuh", "neighbor.cuh", "descriptor.cuh", "force.cuh", "integrate.cuh", "wigner_seitz.cuh", "descriptor_split.cuh", "site_fp64.cuh", "stage.cuh", "tc05.cuh", "descriptor_tc.cuh"]
 
 
 def nvcc_command(verbose: bool = False) -> list[str]:

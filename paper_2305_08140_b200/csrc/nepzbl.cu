@@ -17,6 +17,7 @@
 #include "neighbor.cuh"
 #include "descriptor.cuh"
 #include "descriptor_split.cuh"
+#include "descriptor_tc.cuh"
 #include "force.cuh"
 #include "site_fp64.cuh"
 #include "integrate.cuh"
@@ -66,8 +67,9 @@ struct nepzbl_handle {
   ZblParams zp{};
   SiteModel site{};           // fp64 tables of k_site_fp64 (d_site holds them)
   double* d_site = nullptr;
-  // network of k_angular_nn: 0 = CUDA cores (FFMA), 1 = mma.sync 3xTF32, 2 = tcgen05 3xTF32 with the accumulators in
-  // tensor memory (descriptor.cuh).  NEPZBL_NN=ffma|mma|tc overrides the default; measured verdict in DESIGN.md / profiles/r2_nn_tensor.md
+  // network layer: 0 = CUDA cores (FFMA, k_angular_nn), 1 = mma.sync 3xTF32, 2 = tcgen05 3xTF32 inside k_angular_nn
+  // (block-synchronous), 3 = k_angular_tc (descriptor_tc.cuh: tcgen05, software-pipelined over two tiles).
+  // NEPZBL_NN=ffma|mma|tcsync|tc overrides the default; measured verdict in DESIGN.md / profiles/r2_nn_tensor.md
   int nn_mode = 0;
   bool dense_on = true;       // NEPZBL_DENSE_THRESHOLD=off disables the fp64 re-evaluation (measurement aid)
   size_t smem_nn = 0;
@@ -297,9 +299,9 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
     const size_t nrow = (size_t)nn_rows(p->n_neurons);
     h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
     if (MS::NT > 1) h->smem_nn += sizeof(float) * ((2 * MS::NT * MS::NT * MS::NA * MS::KA + 3) / 4 * 4);
-    if (h->nn_mode == 2 && p->n_neurons > TC_NP - 8) h->nn_mode = 0;  // the tcgen05 variant holds at most 56 neurons
+    if (h->nn_mode >= 2 && p->n_neurons > TC_NP - 8) h->nn_mode = 0;  // the tcgen05 variants hold at most 56 neurons
     if (h->nn_mode == 1) h->smem_nn += sizeof(float) * (32 * ((MS::D + 7) / 8 * 8 + 4) + 32);  // X / Fp tile and site energies
-    if (h->nn_mode == 2) h->smem_nn += tc_smem_bytes<MS>();
+    if (h->nn_mode >= 2) h->smem_nn += tc_smem_bytes<MS>();
   }
 }
 
@@ -542,7 +544,12 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
           h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
           want_q ? h->at<float>(c.q_desc) : nullptr, da);
     };
-    if (h->nn_mode == 2) launch_nn(std::integral_constant<int, 2>{});
+    if (h->nn_mode == 3)
+      k_angular_tc<MS><<<std::min(blocks(n, TCP_THREADS), h->ang_grid), TCP_THREADS, h->smem_nn, st>>>(
+          n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
+          h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
+          want_q ? h->at<float>(c.q_desc) : nullptr, da);
+    else if (h->nn_mode == 2) launch_nn(std::integral_constant<int, 2>{});
     else if (h->nn_mode == 1) launch_nn(std::integral_constant<int, 1>{});
     else launch_nn(std::integral_constant<int, 0>{});
   }
@@ -799,7 +806,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     int v = atoi(gb);
     if (v == 32 || v == 64) h->gather_block = v;
   }
-  if (const char* nm = getenv("NEPZBL_NN")) h->nn_mode = !strcmp(nm, "tc") ? 2 : (!strcmp(nm, "mma") ? 1 : 0);
+  if (const char* nm = getenv("NEPZBL_NN")) h->nn_mode = !strcmp(nm, "tc") ? 3 : (!strcmp(nm, "tcsync") ? 2 : (!strcmp(nm, "mma") ? 1 : 0));
   std::vector<float> nnw;
   with_shape(shape, [&](auto ms) {
     using MS = decltype(ms);
@@ -844,19 +851,20 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     with_shape(shape, [&](auto ms) {
       using MS = decltype(ms);
       if constexpr (kSplit<MS>) { fn = (const void*)k_angular_nn_split<MS>; threads = SPLIT_THREADS; }
+      else if (h->nn_mode == 3) { fn = (const void*)k_angular_tc<MS>; threads = TCP_THREADS; }
       else if (h->nn_mode == 2) { fn = (const void*)k_angular_nn<MS, 2>; threads = 128; }
       else fn = h->nn_mode == 1 ? (const void*)k_angular_nn<MS, 1> : (const void*)k_angular_nn<MS, 0>;
     });
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_nn)) != cudaSuccess) return die("cudaFuncSetAttribute(k_angular_nn)", ce);
     // the tcgen05 variant needs two 105-KB blocks per SM: ask for the largest shared-memory carve-out
-    if (h->nn_mode == 2 && (ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
+    if (h->nn_mode >= 2 && (ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
       return die("cudaFuncSetAttribute(carveout)", ce);
     int per_sm = 0;
     if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, h->smem_nn)) != cudaSuccess) return die("cudaOccupancyMaxActiveBlocksPerMultiprocessor", ce);
     if (per_sm < 1) return die("k_angular_nn does not fit one SM", cudaErrorInvalidConfiguration);
     // two blocks of the tcgen05 variant do fit an SM (2 x 128 x 256 registers, 2 x 105 KB: ncu's occupancy limits say 2 and
     // the measured kernel time halves against a one-block grid), but the occupancy query answers 1
-    if (h->nn_mode == 2 && per_sm < 2 && 2 * (h->smem_nn + 1024) <= 227 * 1024) per_sm = 2;
+    if (h->nn_mode >= 2 && per_sm < 2 && 2 * (h->smem_nn + 1024) <= 227 * 1024) per_sm = 2;
     if (const char* e = getenv("NEPZBL_ANG_BLOCKS_PER_SM")) {  // measurement aid: size of the persistent grid
       fprintf(stderr, "nepzbl: k_angular_nn occupancy %d block(s) of %d threads per SM, %zu bytes of shared memory\n", per_sm, threads, h->smem_nn);
       if (atoi(e) > 0) per_sm = atoi(e);
