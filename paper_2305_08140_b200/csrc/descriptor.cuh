@@ -244,6 +244,27 @@ __device__ __forceinline__ void cheb_U(float x, float U[K]) {
   for (int k = 2; k < K; ++k) U[k] = fmaf(x2, U[k - 1], -U[k - 2]);
 }
 
+// One entry of adisp (written by k_radial, streamed by the angular kernels).  One atom type: {rhat, r} -- the
+// consumers need nothing else (the back-pass takes 1/r with one MUFU), and all four components of the loaded quad are
+// live: with {dx, dy, dz, unused} ptxas reused the dead .w register of a request still in flight as a temporary,
+// and that write waited for the load (ncu: long-scoreboard stall in the middle of the forward iteration).
+// Several types: {dx, dy, dz, neighbour type}.
+template <int NT, bool RINV>
+__device__ __forceinline__ void unpack_disp(const float4& d, float& ux, float& uy, float& uz, float& r, float& rinv) {
+  if (NT == 1) {
+    ux = d.x; uy = d.y; uz = d.z; r = d.w;
+    rinv = RINV ? __fdividef(1.0f, r) : 0.0f;
+  } else {
+    const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
+    rinv = rsqrtf(r2);
+    r = r2 * rinv;
+    ux = d.x * rinv; uy = d.y * rinv; uz = d.z * rinv;
+  }
+}
+// a harmless entry (r = 1) in either format: {rhat = x, r = 1} or {d = x, type 0}
+template <int NT>
+__device__ __forceinline__ float4 disp_dummy() { return make_float4(1.0f, 0.0f, 0.0f, NT == 1 ? 1.0f : 0.0f); }
+
 __device__ __forceinline__ float tanh_fast(float z) {
   // 1 - 2/(e^{2z}+1): absolute error ~1e-7, enough for the 1e-5 eV energy tolerance
   float e = __expf(2.0f * z);
@@ -362,7 +383,12 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         const bool pa = e < cnt_a && r2 < mt.rcA2;
         const unsigned g = (__ballot_sync(0xffffffffu, pa) >> gshift) & 0xFu;
         if (pa) {
-          adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, MS::NT > 1 ? __int_as_float(o[u].w) : 0.0f);
+          if (MS::NT > 1) {
+            adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, __int_as_float(o[u].w));
+          } else {  // {rhat, r}, see unpack_disp
+            const float ri = rsqrtf(r2);
+            adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx * ri, dy * ri, dz * ri, r2 * ri);
+          }
           if (e < 32) alo |= 1u << e; else ahi |= 1u << (e - 32);
         }
         abase += __popc(g);
@@ -592,7 +618,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
   // The start of a tile is a chain of dependent global loads (mask -> count -> first displacements) that two
   // warps per scheduler cannot hide, so it is issued one tile ahead: the next tile's mask at the start of this
   // tile, its first two displacement vectors before this tile's back-pass.
-  const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+  const float4 dummy = disp_dummy<MS::NT>();
   int tile = TC ? blockIdx.x * (T_ / 32) + (threadIdx.x >> 5) : (threadIdx.x >> 5) * gridDim.x + blockIdx.x;
   unsigned long long mask_nx = 0ull;
   float4 pre0 = dummy, pre1 = dummy;
@@ -637,13 +663,12 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       float g2[2][NA], b2[2][24];
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        float dx = d2[h].x, dy = d2[h].y, dz = d2[h].z;
-        float r2 = dx * dx + dy * dy + dz * dz;
-        float rinv = rsqrtf(r2), r = r2 * rinv;
+        float ux, uy, uz, r, rinv;
+        unpack_disp<MS::NT, false>(d2[h], ux, uy, uz, r, rinv);
         float fc, T[KA];
         cheb_T_fwd<KA>(r, mt.inv_rcA, fc, T);
         if (h == 1 && c + 1 >= nc) fc = 0.0f;
-        eval_blm(dx * rinv, dy * rinv, dz * rinv, b2[h]);
+        eval_blm(ux, uy, uz, b2[h]);
         const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(d2[h].w) : 0;  // adisp.w = neighbour type
 #pragma unroll
         for (int nq = 0; nq < NA; ++nq) {
@@ -1017,10 +1042,10 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     }
     for (unsigned long long m = live ? mask : 0ull; m; m &= m - 1, ++c) {
       const int a = __ffsll((long long)m) - 1;
-      const float dx = nx.x, dy = nx.y, dz = nx.z, tjw = nx.w;
+      float ux, uy, uz, r, rinv;
+      unpack_disp<MS::NT, true>(nx, ux, uy, uz, r, rinv);
+      const float tjw = nx.w;
       nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration
-      float r2 = dx * dx + dy * dy + dz * dz;
-      float rinv = rsqrtf(r2), r = r2 * rinv;
       float fc, dfc, x, dxdr, T[KA], Uc[KA];
       cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
       cheb_U<KA>(x, Uc);
@@ -1038,7 +1063,6 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
         g[nq] = fc * p;
         dg[nq] = fmaf(dfc, p, fc * dxdr * dp);
       }
-      float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
       auto G = [&](int lm) {
         float t = 0.0f;
 #pragma unroll

@@ -93,7 +93,7 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
   const unsigned qmask = 0xFu << qbase;  // shuffles inside loops whose trip count differs between quads
   const int ntiles = (n + 7) / 8;
   const int nslots = gridDim.x * (SPLIT_THREADS / 32);
-  const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+  const float4 dummy = disp_dummy<MS::NT>();
 
   for (int tile = (threadIdx.x >> 5) * gridDim.x + blockIdx.x; tile < ntiles; tile += nslots) {
     const int s = tile * 8 + (lane >> 2);
@@ -121,11 +121,11 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       for (int c = 0; c < nc; ++c) {
         const float4 d = nx;
         nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration
-        float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
-        float rinv = rsqrtf(r2), r = r2 * rinv;
+        float ux, uy, uz, r, rinv;
+        unpack_disp<NT, false>(d, ux, uy, uz, r, rinv);
         float fc, T[KA], b[24];
         cheb_T_fwd<KA>(r, mt.inv_rcA, fc, T);
-        eval_blm(d.x * rinv, d.y * rinv, d.z * rinv, b);
+        eval_blm(ux, uy, uz, b);
         const float* cts = s_ct + (NT > 1 ? (ti * NT + __float_as_int(d.w)) * NAP * KA : 0);  // adisp.w = neighbour type
 #pragma unroll
         for (int j = 0; j < NSUB; ++j) {
@@ -336,11 +336,10 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
       float4 nx = nc > 0 ? dp[0] : dummy;
       for (unsigned long long m = mask; m; m &= m - 1, ++c) {
         const int a = __ffsll((long long)m) - 1;
-        const float dx = nx.x, dy = nx.y, dz = nx.z;
+        float ux, uy, uz, r, rinv;
+        unpack_disp<NT, true>(nx, ux, uy, uz, r, rinv);
         const float* cts = ctp + (NT > 1 ? (ti * NT + __float_as_int(nx.w)) * NAP * KA : 0);
         nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;
-        float r2 = dx * dx + dy * dy + dz * dz;
-        float rinv = rsqrtf(r2), r = r2 * rinv;
         float fc, dfc, x, dxdr, T[KA], Uc[KA];
         cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
         cheb_U<KA>(x, Uc);
@@ -360,7 +359,6 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
           g[j] = fc * p;
           dg[j] = fmaf(dfc, p, e * dpk);
         }
-        float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
         auto G = [&](int lm) {
           float t = 0.0f;
 #pragma unroll

@@ -37,7 +37,7 @@ __device__ __forceinline__ void tcp_forward(float (&A)[MS::NA][24], int nc, cons
                                             float4 pre0, float4 pre1, const ModelTables<MS>& mt,
                                             const float* __restrict__ s_cta, int ti) {
   constexpr int NA = MS::NA, KA = MS::KA;
-  const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+  const float4 dummy = disp_dummy<MS::NT>();
 #pragma unroll
   for (int nq = 0; nq < NA; ++nq)
 #pragma unroll
@@ -50,13 +50,12 @@ __device__ __forceinline__ void tcp_forward(float (&A)[MS::NA][24], int nc, cons
     float g2[2][NA], b2[2][24];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      const float dx = d2[h].x, dy = d2[h].y, dz = d2[h].z;
-      const float r2 = dx * dx + dy * dy + dz * dz;
-      const float rinv = rsqrtf(r2), r = r2 * rinv;
+      float ux, uy, uz, r, rinv;
+      unpack_disp<MS::NT, false>(d2[h], ux, uy, uz, r, rinv);
       float fc, T[KA];
       cheb_T_fwd<KA>(r, mt.inv_rcA, fc, T);
       if (h == 1 && c + 1 >= nc) fc = 0.0f;
-      eval_blm(dx * rinv, dy * rinv, dz * rinv, b2[h]);
+      eval_blm(ux, uy, uz, b2[h]);
       const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(d2[h].w) : 0;  // adisp.w = neighbour type
 #pragma unroll
       for (int nq = 0; nq < NA; ++nq) {
@@ -106,15 +105,15 @@ __device__ __forceinline__ void tcp_backward(const float (&A)[MS::NA][24], unsig
                                              const ModelTables<MS>& mt, const float* __restrict__ s_cta, int ti,
                                              float4* __restrict__ pf /* pforce + s */) {
   constexpr int NA = MS::NA, KA = MS::KA;
-  const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+  const float4 dummy = disp_dummy<MS::NT>();
   int c = 0;
   float4 nx = first;
   for (unsigned long long m = mask; m; m &= m - 1, ++c) {
     const int a = __ffsll((long long)m) - 1;
-    const float dx = nx.x, dy = nx.y, dz = nx.z, tjw = nx.w;
+    float ux, uy, uz, r, rinv;
+    unpack_disp<MS::NT, true>(nx, ux, uy, uz, r, rinv);
+    const float tjw = nx.w;
     nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration
-    const float r2 = dx * dx + dy * dy + dz * dz;
-    const float rinv = rsqrtf(r2), r = r2 * rinv;
     float fc, dfc, x, dxdr, T[KA], Uc[KA];
     cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
     cheb_U<KA>(x, Uc);
@@ -132,7 +131,6 @@ __device__ __forceinline__ void tcp_backward(const float (&A)[MS::NA][24], unsig
       g[nq] = fc * p;
       dg[nq] = fmaf(dfc, p, fc * dxdr * dpk);
     }
-    const float ux = dx * rinv, uy = dy * rinv, uz = dz * rinv;
     auto G = [&](int lm) {
       float t = 0.0f;
 #pragma unroll
@@ -259,7 +257,7 @@ k_angular_tc(int n, int npad, const int4* __restrict__ xyzt,
 
   // a block's tiles: 128 consecutive atoms, tile index blockIdx.x + i gridDim.x (the same count for all its threads)
   const int ntiles = (n + T_ - 1) / T_;
-  const float4 dummy = make_float4(1.0f, 0.0f, 0.0f, 0.0f);
+  const float4 dummy = disp_dummy<MS::NT>();
   int t_cur = -1, t_nxt = blockIdx.x < ntiles ? (int)blockIdx.x : -1;
   float U_cur = 0.0f;  // site energy of the current tile's atom (set when its Z was consumed)
   // the head of a tile is a chain of dependent loads (mask -> count -> first displacements): requested one pass ahead
