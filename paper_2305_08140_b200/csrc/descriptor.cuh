@@ -265,6 +265,19 @@ __device__ __forceinline__ void unpack_disp(const float4& d, float& ux, float& u
 template <int NT>
 __device__ __forceinline__ float4 disp_dummy() { return make_float4(1.0f, 0.0f, 0.0f, NT == 1 ? 1.0f : 0.0f); }
 
+// 16-byte asynchronous copy global -> shared (no destination register: any number in flight)
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(tc05::smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+// request a line into L1 without a destination register: issued two iterations ahead of the load that uses it
+// (ptxas places that load, which needs eight registers across the most register-hungry part of the iteration,
+// half an iteration before its use: ncu showed the remaining latency as a long-scoreboard stall at the loop end)
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" :: "l"(p)); }
+
 __device__ __forceinline__ float tanh_fast(float z) {
   // 1 - 2/(e^{2z}+1): absolute error ~1e-7, enough for the 1e-5 eV energy tolerance
   float e = __expf(2.0f * z);
@@ -658,6 +671,8 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     float4 nx0 = pre0, nx1 = pre1;
     for (int c = 0; c < nc; c += 2) {
       const float4 d2[2] = {nx0, nx1};
+      if (c + 4 < nc) prefetch_l1(dp + (size_t)(c + 4) * npad);
+      if (c + 5 < nc) prefetch_l1(dp + (size_t)(c + 5) * npad);
       nx0 = c + 2 < nc ? dp[(size_t)(c + 2) * npad] : dummy;  // in flight during this iteration
       nx1 = c + 3 < nc ? dp[(size_t)(c + 3) * npad] : dummy;
       float g2[2][NA], b2[2][24];
@@ -1045,6 +1060,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       float ux, uy, uz, r, rinv;
       unpack_disp<MS::NT, true>(nx, ux, uy, uz, r, rinv);
       const float tjw = nx.w;
+      if (c + 3 < nc) prefetch_l1(dp + (size_t)(c + 3) * npad);
       nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration
       float fc, dfc, x, dxdr, T[KA], Uc[KA];
       cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);

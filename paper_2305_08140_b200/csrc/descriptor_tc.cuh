@@ -45,6 +45,8 @@ __device__ __forceinline__ void tcp_forward(float (&A)[MS::NA][24], int nc, cons
   float4 nx0 = pre0, nx1 = pre1;
   for (int c = 0; c < nc; c += 2) {
     const float4 d2[2] = {nx0, nx1};
+    if (c + 4 < nc) prefetch_l1(dp + (size_t)(c + 4) * npad);
+    if (c + 5 < nc) prefetch_l1(dp + (size_t)(c + 5) * npad);
     nx0 = c + 2 < nc ? dp[(size_t)(c + 2) * npad] : dummy;
     nx1 = c + 3 < nc ? dp[(size_t)(c + 3) * npad] : dummy;
     float g2[2][NA], b2[2][24];
@@ -113,6 +115,7 @@ __device__ __forceinline__ void tcp_backward(const float (&A)[MS::NA][24], unsig
     float ux, uy, uz, r, rinv;
     unpack_disp<MS::NT, true>(nx, ux, uy, uz, r, rinv);
     const float tjw = nx.w;
+    if (c + 3 < nc) prefetch_l1(dp + (size_t)(c + 3) * npad);
     nx = c + 1 < nc ? dp[(size_t)(c + 1) * npad] : dummy;  // in flight during this iteration
     float fc, dfc, x, dxdr, T[KA], Uc[KA];
     cheb_T<KA>(r, mt.inv_rcA, fc, dfc, x, dxdr, T);
@@ -211,8 +214,7 @@ k_angular_tc(int n, int npad, const int4* __restrict__ xyzt,
   constexpr int CT_FLOATS = MS::NT > 1 ? (2 * MS::NT * MS::NT * NA * KA + 3) / 4 * 4 : 0;
   const int tab_floats = nrow * DPAD + 2 * nrow + DPAD + CT_FLOATS;
   for (int t = threadIdx.x; t < tab_floats / 4; t += T_)
-    reinterpret_cast<float4*>(smem)[t] = reinterpret_cast<const float4*>(nnw)[t];
-  __syncthreads();
+    cp_async16(reinterpret_cast<float4*>(smem) + t, reinterpret_cast<const float4*>(nnw) + t);
   // operand tiles (layout: tc05.cuh), the two mbarriers, the TMEM base address
   const uintptr_t base = (reinterpret_cast<uintptr_t>(smem + tab_floats) + 127) & ~uintptr_t(127);
   float* const tB1h = reinterpret_cast<float*>(base);  // [64 neurons][KP]      B of Z = X W0^T (column D: -b0)
@@ -225,21 +227,11 @@ k_angular_tc(int n, int npad, const int4* __restrict__ xyzt,
   float* const tTl = tTh + 128 * 32;
   unsigned long long* const bars = reinterpret_cast<unsigned long long*>(tTl + 128 * 32);
   uint32_t* const tbase = reinterpret_cast<uint32_t*>(bars + 2);
-  for (int e = threadIdx.x; e < TC_NP * KP; e += T_) {
-    const int m = e / KP, k = e % KP;
-    const float w = m < nrow ? (k < D ? s_w0[m * DPAD + k] : (k == D ? -s_b0[m] : 0.0f)) : 0.0f;
-    float hi, lo;
-    tc05::split_tf32(w, hi, lo);
-    *reinterpret_cast<float*>(reinterpret_cast<char*>(tB1h) + tc05::tile_off(TC_NP, m, k)) = hi;
-    *reinterpret_cast<float*>(reinterpret_cast<char*>(tB1l) + tc05::tile_off(TC_NP, m, k)) = lo;
-  }
-  for (int e = threadIdx.x; e < KN * TC_NP; e += T_) {
-    const int v = e / TC_NP, m = e % TC_NP;
-    const float w = (m < nrow && v < D) ? s_w0[m * DPAD + v] : 0.0f;
-    float hi, lo;
-    tc05::split_tf32(w, hi, lo);
-    *reinterpret_cast<float*>(reinterpret_cast<char*>(tB2h) + tc05::tile_off(KN, v, m)) = hi;
-    *reinterpret_cast<float*>(reinterpret_cast<char*>(tB2l) + tc05::tile_off(KN, v, m)) = lo;
+  {  // the host has split and tiled both B operands (build_nnw): a straight copy
+    const float4* src = reinterpret_cast<const float4*>(nnw + (tab_floats + 31) / 32 * 32);
+    float4* dst = reinterpret_cast<float4*>(tB1h);
+    for (int t = threadIdx.x; t < (2 * TC_NP * KP + 2 * KN * TC_NP) / 4; t += T_) cp_async16(dst + t, src + t);
+    cp_async_wait_all();
   }
   const uint32_t bar_z = tc05::smem_u32(bars), bar_f = tc05::smem_u32(bars + 1);
   if (threadIdx.x < 32) tc05::tmem_alloc<TCP_TMEM_COLS>(tc05::smem_u32(tbase));

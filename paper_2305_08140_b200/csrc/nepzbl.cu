@@ -70,7 +70,7 @@ struct nepzbl_handle {
   // network layer: 0 = CUDA cores (FFMA, k_angular_nn), 1 = mma.sync 3xTF32, 2 = tcgen05 3xTF32 inside k_angular_nn
   // (block-synchronous), 3 = k_angular_tc (descriptor_tc.cuh: tcgen05, software-pipelined over two tiles).
   // NEPZBL_NN=ffma|mma|tcsync|tc overrides the default; measured verdict in DESIGN.md / profiles/r2_nn_tensor.md
-  int nn_mode = 0;
+  int nn_mode = 3;
   bool dense_on = true;       // NEPZBL_DENSE_THRESHOLD=off disables the fp64 re-evaluation (measurement aid)
   size_t smem_nn = 0;
   // threads per block of k_radial / k_force: one warp while the grid is only a few waves of resident threads (the
@@ -371,6 +371,36 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
             ct[(pr * MS::NA + nq) * MS::KA + k] = (float)v;
             ct[((MS::NT * MS::NT + pr) * MS::NA + nq) * MS::KA + k] = (float)(k * v);
           }
+    }
+    // k_angular_tc: behind the table (at the next multiple of 32 floats) the B operands of its two tensor-core products,
+    // split into tf32 hi + lo parts and laid out as the tiles tc05.cuh describes:
+    //   B1 hi/lo [64 neurons][kp]: w0 with -b0 in column D;  B2 hi/lo [kn components][64 neurons]: w0 transposed
+    if (p->n_neurons <= TC_NP - 8) {
+      constexpr TcShape ts = tc_shape<MS>();
+      const size_t off = (w.size() + 31) / 32 * 32;
+      w.resize(off + 2 * (size_t)TC_NP * ts.kp + 2 * (size_t)ts.kn * TC_NP, 0.0f);
+      float* b1h = w.data() + off;
+      float* b1l = b1h + TC_NP * ts.kp;
+      float* b2h = b1l + TC_NP * ts.kp;
+      float* b2l = b2h + ts.kn * TC_NP;
+      auto split = [](float x, float& hi, float& lo) {  // cvt.rna.tf32: nearest, ties away from zero, 13 low bits cleared
+        uint32_t u;
+        memcpy(&u, &x, 4);
+        u = (u + 0x1000u) & 0xFFFFE000u;
+        memcpy(&hi, &u, 4);
+        lo = x - hi;
+      };
+      for (int m = 0; m < p->n_neurons; ++m) {
+        for (int k = 0; k <= MS::D; ++k) {
+          const float x = k < MS::D ? (float)p->w0[(size_t)m * MS::D + k] : -(float)p->b0[m];
+          const size_t o = tc05::tile_off(TC_NP, m, k) / 4;
+          split(x, b1h[o], b1l[o]);
+        }
+        for (int v = 0; v < MS::D; ++v) {
+          const size_t o = tc05::tile_off(ts.kn, v, m) / 4;
+          split((float)p->w0[(size_t)m * MS::D + v], b2h[o], b2l[o]);
+        }
+      }
     }
     return w;
   }
