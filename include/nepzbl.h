@@ -89,7 +89,7 @@ typedef struct {
   const double *atomic_number;         /* [n_types] */
   const double *mass;                  /* [n_types], amu */
   double skin;                         /* neighbour-list skin, A (D: C-15) */
-  int32_t cap_radial, cap_angular;     /* list capacities per atom (cap_radial <= 1024, cap_angular <= 64) */
+  int32_t cap_radial, cap_angular;     /* list capacities per atom (cap_radial <= 1024, cap_angular <= 128) */
 } nepzbl_params;
 
 /* Create a handle on CUDA device `device`; all work goes to `cuda_stream` (a cudaStream_t).  With NULL the library

@@ -294,7 +294,9 @@ __device__ __forceinline__ float tanh_fast(float z) {
 // by a fixed-order shuffle tree (deterministic).
 // The same pass serves the angular descriptor: the first nn_a entries of the list are the angular list
 // (k_nbr).  For those, the displacement vectors of the entries inside rc_angular are compacted in list
-// order into adisp[c][s] (c = 0 .. popc(amask[s]) - 1) and their slots into the bit mask amask[s].
+// order into adisp[c][s] (c = 0 .. popc(amask[s]) - 1) and their slots into the bit mask amask[w][s] (AW = 1 or 2 64-bit
+// words per atom: list capacities up to 128; word 1 exists only when cap_angular > 64 -- a template parameter of every
+// kernel that walks the mask, because a run-time second word cost the common case 1-8 % in k_force / the angular kernels).
 // k_angular_nn holds 120 accumulators per thread and runs at 2 warps per scheduler, where it cannot
 // hide gather latency; this kernel can, so the gathers live here and k_angular_nn streams adisp with
 // coalesced loads.
@@ -307,7 +309,7 @@ __device__ __forceinline__ float tanh_fast(float z) {
 #endif
 // STAGE > 0 (stage.cuh, an experiment): the block is one tile of STAGE_TILE atoms whose neighbour ranges are copied
 // to shared memory first (1: plain copies, 2: bulk copies); list entries then come from nl_loc (16-bit offsets).
-template <class MS, bool TRI, int STAGE = 0>
+template <class MS, bool TRI, int STAGE = 0, int AW = 1>
 __global__ void __launch_bounds__(STAGE ? STAGE_TILE * 4 : RADIAL_BLOCK)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
@@ -360,7 +362,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   const size_t lstride = (size_t)RADIAL_LANES * npad;
   unsigned mword = 0u;
   int bit = 0, word = 0;
-  unsigned alo = 0u, ahi = 0u;  // this lane's part of amask
+  unsigned alo = 0u, ahi = 0u, blo = 0u, bhi = 0u;  // this lane's part of amask (entries 0..63 and, AW = 2, 64..127)
   int abase = 0;                // angular entries of this atom compacted so far
   const unsigned below = (1u << sub) - 1u;
   const int gshift = threadIdx.x & 28;
@@ -402,7 +404,12 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
             const float ri = rsqrtf(r2);
             adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx * ri, dy * ri, dz * ri, r2 * ri);
           }
-          if (e < 32) alo |= 1u << e; else ahi |= 1u << (e - 32);
+          if (AW == 1) {
+            if (e < 32) alo |= 1u << e; else ahi |= 1u << (e - 32);
+          } else {
+            const unsigned bitv = 1u << (e & 31);
+            if (e < 32) alo |= bitv; else if (e < 64) ahi |= bitv; else if (e < 96) blo |= bitv; else bhi |= bitv;
+          }
         }
         abase += __popc(g);
       }
@@ -442,8 +449,15 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   unsigned cb = __ballot_sync(0xffffffffu, close);
   alo |= __shfl_xor_sync(0xffffffffu, alo, 1); alo |= __shfl_xor_sync(0xffffffffu, alo, 2);
   ahi |= __shfl_xor_sync(0xffffffffu, ahi, 1); ahi |= __shfl_xor_sync(0xffffffffu, ahi, 2);
+  if (AW > 1) {
+    blo |= __shfl_xor_sync(0xffffffffu, blo, 1); blo |= __shfl_xor_sync(0xffffffffu, blo, 2);
+    bhi |= __shfl_xor_sync(0xffffffffu, bhi, 1); bhi |= __shfl_xor_sync(0xffffffffu, bhi, 2);
+  }
   if (!valid) return;
-  if (sub == 0) amask[s] = ((unsigned long long)ahi << 32) | alo;
+  if (sub == 0) {
+    amask[s] = ((unsigned long long)ahi << 32) | alo;
+    if (AW > 1) amask[(size_t)npad + s] = ((unsigned long long)bhi << 32) | blo;
+  }
   for (int nq = sub; nq < MS::NR; nq += RADIAL_LANES) {
     float q = 0.0f;
 #pragma unroll
@@ -535,7 +549,7 @@ __host__ __device__ constexpr size_t tc_smem_bytes() {
 }
 
 // NN: 0 = network on the CUDA cores (FFMA, weights broadcast from shared memory), 1 = mma.sync 3xTF32, 2 = tcgen05
-template <class MS, int NN = 0>
+template <class MS, int NN = 0, int AW = 1>
 __global__ void __launch_bounds__(NN == 2 ? 128 : ANG_THREADS, NN == 2 ? 2 : 8)
 k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
              const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
@@ -639,7 +653,7 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     const int s0 = tile * 32 + (threadIdx.x & 31);
     if (tile < ntiles && s0 < n) {
       mask_nx = amask[s0];
-      const int c0 = __popcll(mask_nx);
+      const int c0 = __popcll(mask_nx) + (AW > 1 ? __popcll(amask[(size_t)npad + s0]) : 0);
       pre0 = c0 > 0 ? adisp[s0] : dummy;
       pre1 = c0 > 1 ? adisp[(size_t)npad + s0] : dummy;
     }
@@ -655,7 +669,8 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     const bool live = s < n;
     if (!MMA && !TC && !live) continue;
     const int sl = live ? s : 0;
-    const int nc = live ? __popcll(mask) : 0;
+    const unsigned long long mask_hi = (AW > 1 && live) ? amask[(size_t)npad + s] : 0ull;  // entries 64..
+    const int nc = live ? __popcll(mask) + __popcll(mask_hi) : 0;
     const float4* dp = adisp + sl;
     const int ti = MS::NT > 1 ? xyzt[sl].w : 0;  // type of the central atom (selects the c^{ti tj} tables)
     float qr[NR];
@@ -1051,12 +1066,13 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
     int c = 0;
     float4 nx = pre0;  // this tile's first displacement is still there; the next tile's are requested now
     {
-      const int c2 = __popcll(mask_nx);
+      const int c2 = __popcll(mask_nx) + ((AW > 1 && v2) ? __popcll(amask[(size_t)npad + s2]) : 0);
       pre0 = c2 > 0 ? adisp[v2 ? s2 : 0] : dummy;
       pre1 = c2 > 1 ? adisp[(size_t)npad + (v2 ? s2 : 0)] : dummy;
     }
-    for (unsigned long long m = live ? mask : 0ull; m; m &= m - 1, ++c) {
-      const int a = __ffsll((long long)m) - 1;
+    auto back_word = [&](unsigned long long mbits, int abase) {
+    for (unsigned long long m = mbits; m; m &= m - 1, ++c) {
+      const int a = abase + __ffsll((long long)m) - 1;
       float ux, uy, uz, r, rinv;
       unpack_disp<MS::NT, true>(nx, ux, uy, uz, r, rinv);
       const float tjw = nx.w;
@@ -1099,6 +1115,9 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       float pz = fmaf(uz, Sp, (vz - uz * uv) * rinv);
       pforce[(size_t)a * npad + s] = make_float4(px, py, pz, 0.0f);
     }
+    };
+    back_word(live ? mask : 0ull, 0);
+    if (AW > 1) back_word(mask_hi, 64);
   }
   if (TC) {
     tc05::fence_before_sync();

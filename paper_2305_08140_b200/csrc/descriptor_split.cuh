@@ -60,7 +60,7 @@ struct SplitLayout {
   __host__ __device__ static constexpr int stash_floats() { return NSUB * 24 * SPLIT_THREADS; }
 };
 
-template <class MS>
+template <class MS, int AW = 1>
 __global__ void __launch_bounds__(SPLIT_THREADS, 3)
 k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
                    const unsigned long long* __restrict__ amask, const float4* __restrict__ adisp,
@@ -100,7 +100,8 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
     const bool valid = s < n;            // all 4 lanes of a quad agree; shuffles below stay inside the quad
     const int sc_ = valid ? s : 0;
     const unsigned long long mask = valid ? amask[sc_] : 0ull;
-    const int nc = __popcll(mask);
+    const unsigned long long mask_hi = (AW > 1 && valid) ? amask[(size_t)npad + sc_] : 0ull;  // entries 64..
+    const int nc = __popcll(mask) + __popcll(mask_hi);
     const float4* dp = adisp + sc_;
     const int ti = NT > 1 ? xyzt[sc_].w : 0;  // central atom's type: selects the c^{ti tj} tables per neighbour
     // ---- S4 forward: A[j][lm] = sum_neighbours g_{n_j}(r) b_lm(rhat)
@@ -334,8 +335,10 @@ k_angular_nn_split(int n, int npad, const int4* __restrict__ xyzt,
         for (int k = 0; k < KA; ++k) ct[j][k] = ctp[(sub + SPLIT_LANES * j) * KA + k];
       int c = 0;
       float4 nx = nc > 0 ? dp[0] : dummy;
-      for (unsigned long long m = mask; m; m &= m - 1, ++c) {
-        const int a = __ffsll((long long)m) - 1;
+#pragma unroll 1
+      for (int mw = 0; mw < AW; ++mw)  // AW = 1 unless cap_angular > 64
+      for (unsigned long long m = mw ? mask_hi : mask; m; m &= m - 1, ++c) {
+        const int a = 64 * mw + __ffsll((long long)m) - 1;
         float ux, uy, uz, r, rinv;
         unpack_disp<NT, true>(nx, ux, uy, uz, r, rinv);
         const float* cts = ctp + (NT > 1 ? (ti * NT + __float_as_int(nx.w)) * NAP * KA : 0);

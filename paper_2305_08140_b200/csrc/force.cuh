@@ -32,7 +32,7 @@ struct KickArgs {
 };
 // BLK = threads per block (32 or 64, chosen by the host from the grid size; a template parameter because the code
 // ptxas generates under __launch_bounds__(32) is 2 % faster than the same source under a bound of 64 or 128)
-template <class MS, bool VIRIAL, int BLK, bool TRI>
+template <class MS, bool VIRIAL, int BLK, bool TRI, int AW = 1>
 __global__ void __launch_bounds__(BLK)
 k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
         const int* __restrict__ nn_r, const int* __restrict__ nl_r, const int* __restrict__ nn_a,
@@ -203,14 +203,25 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
   //      pair.  Lane p takes the in-cutoff entries number p, p+4, ...; 2 entries per lane per iteration
   //      so that the dependent gathers overlap.
   {
+    // the in-cutoff entries in list order: word 0 of the mask, then (cap_angular > 64 only) word 1; TWO selects the
+    // two-word walk -- the common one-word case keeps its plain bit arithmetic
+    auto angular_part = [&](auto two) {
+    constexpr bool TWO = decltype(two)::value;
     unsigned long long m = valid ? amask[sc_] : 0ull;
-    for (int k = 0; k < sub; ++k) m &= m - 1;  // drop the entries of the lanes below
+    unsigned long long m_hi = (TWO && valid) ? amask[(size_t)npad + sc_] : 0ull;
+    int abase = 0;
+    auto drop = [&]() {  // remove the lowest set bit
+      m &= m - 1;
+      if (TWO && m == 0ull && m_hi != 0ull) { m = m_hi; m_hi = 0ull; abase = 64; }
+    };
+    if (TWO && m == 0ull && m_hi != 0ull) { m = m_hi; m_hi = 0ull; abase = 64; }
+    for (int k = 0; k < sub; ++k) drop();  // the entries of the lanes below
     while (m) {
-      const int a0 = __ffsll((long long)m) - 1;
-      m &= m - 1; m &= m - 1; m &= m - 1; m &= m - 1;
+      const int a0 = abase + __ffsll((long long)m) - 1;
+      drop(); drop(); drop(); drop();
       const bool ok1 = m != 0ull;
-      const int a1 = ok1 ? __ffsll((long long)m) - 1 : a0;
-      m &= m - 1; m &= m - 1; m &= m - 1; m &= m - 1;
+      const int a1 = ok1 ? abase + __ffsll((long long)m) - 1 : a0;
+      drop(); drop(); drop(); drop();
       const size_t e0 = (size_t)a0 * npad + sc_, e1 = (size_t)a1 * npad + sc_;
       int j0 = nl_a[e0], j1 = nl_a[e1];
       int b0 = rev[e0], b1 = rev[e1];
@@ -245,6 +256,8 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
         }
       }
     }
+    };
+    angular_part(std::integral_constant<bool, (AW > 1)>{});
   }
 
   // ---- combine the 4 lanes (fixed order), results in the caller's atom order

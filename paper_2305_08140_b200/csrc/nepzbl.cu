@@ -166,6 +166,9 @@ inline size_t al(size_t x) { return (x + 255) & ~size_t(255); }
 // 32-bit words of the per-lane in-cutoff mask: lane p of RADIAL_LANES owns entries p, p+4, ...
 inline int mask_words(const nepzbl_params& p) { return (p.cap_radial + 32 * RADIAL_LANES - 1) / (32 * RADIAL_LANES); }
 
+// 64-bit words of the angular in-cutoff mask per atom (cap_angular <= 128)
+inline int amask_words(const nepzbl_params& p) { return (p.cap_angular + 63) / 64; }
+
 // NEPZBL_STAGE=1|2: neighbour tiles staged in shared memory by k_radial (stage.cuh; measurement aid, default off)
 inline int stage_mode() {
   static const int m = [] { const char* e = getenv("NEPZBL_STAGE"); const int v = e ? atoi(e) : 0; return v == 1 || v == 2 ? v : 0; }();
@@ -196,7 +199,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.nl_r = take(4 * (size_t)p.cap_radial * npad);
   c.rev = take((size_t)p.cap_angular * npad);
   c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
-  c.amask = take(8 * npad);
+  c.amask = take(8 * (size_t)amask_words(p) * npad);
   c.adisp = take(16 * (size_t)p.cap_angular * npad);
   c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
   c.dk = take(64 * (size_t)std::max(1, p.n_types) * npad);  // AtomRec, one per partner type
@@ -523,10 +526,10 @@ void launch_site_fp64(nepzbl_handle* h, const double* pos, bool want_q, cudaStre
   const Carve& c = h->cv;
   const int n = (int)h->n;
   const int grid = std::max(1, std::min(blocks(n, SITE64_WARPS), 8 * h->n_sm));
-  const size_t smem = sizeof(double) * SITE64_WARPS * (2 * (size_t)h->site.D + h->site.n_neurons + 8);
+  const size_t smem = sizeof(double) * SITE64_WARPS * (2 * (size_t)h->site.D + h->site.n_neurons + 16);
   k_site_fp64<<<grid, 32 * SITE64_WARPS, smem, st>>>(
       h->d_sc, h->d_bm, h->site, h->at<int>(c.dense_list), n, c.npad, h->at<int4>(c.xyzt), h->at<int>(c.nl_r),
-      h->at<unsigned long long>(c.amask), h->at<int>(c.perm), pos, h->at<float>(c.q_radial), h->at<float>(c.u_site),
+      h->at<unsigned long long>(c.amask), amask_words(h->p), h->at<int>(c.perm), pos, h->at<float>(c.q_radial), h->at<float>(c.u_site),
       h->at<AtomRec>(c.dk), h->at<float4>(c.pforce), want_q ? h->at<float>(c.q_desc) : nullptr);
 }
 
@@ -541,13 +544,16 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   const ModelTables<MS>& mt = *reinterpret_cast<const ModelTables<MS>*>(h->tables.data());
   const int gb = h->gather_block ? h->gather_block : ((long long)n * RADIAL_LANES < 8ll * 1024 * h->n_sm ? 32 : 64);
   prof_mark(h, PK_RADIAL);
-  auto launch_radial = [&](auto tri, auto stage) {
+  // cap_angular > 64: two mask words per atom (AW = 2 instantiations; the FFMA angular kernel, 64-thread k_force)
+  const bool two_words = amask_words(h->p) > 1;
+  auto launch_radial = [&](auto tri, auto stage, auto aw) {
     constexpr int STAGE = decltype(stage)::value;
+    constexpr int AW = decltype(aw)::value;
     const int blk = STAGE ? STAGE_TILE * RADIAL_LANES : gb;
     const size_t smem = STAGE ? ((sizeof(TileDesc) + 8 + 15) / 16) * 16 + sizeof(int4) * STAGE_CAP : 0;
-    if (STAGE) cudaFuncSetAttribute((const void*)k_radial<MS, decltype(tri)::value, STAGE>,
+    if (STAGE) cudaFuncSetAttribute((const void*)k_radial<MS, decltype(tri)::value, STAGE, AW>,
                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    k_radial<MS, decltype(tri)::value, STAGE><<<blocks((long long)n * RADIAL_LANES, blk), blk, smem, st>>>(
+    k_radial<MS, decltype(tri)::value, STAGE, AW><<<blocks((long long)n * RADIAL_LANES, blk), blk, smem, st>>>(
         h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
         h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p), h->at<int>(c.zbl_list),
         h->at<int>(c.nn_a), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp),
@@ -555,33 +561,41 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
         STAGE ? h->at<unsigned short>(c.nl_loc) : nullptr);
   };
   using std::integral_constant;
-  if (h->tri) launch_radial(std::true_type{}, integral_constant<int, 0>{});
-  else if (std::is_same<MS, MS0>::value && stage_mode() == 1) launch_radial(std::false_type{}, integral_constant<int, std::is_same<MS, MS0>::value ? 1 : 0>{});
-  else if (std::is_same<MS, MS0>::value && stage_mode() == 2) launch_radial(std::false_type{}, integral_constant<int, std::is_same<MS, MS0>::value ? 2 : 0>{});
-  else launch_radial(std::false_type{}, integral_constant<int, 0>{});
+  using one = integral_constant<int, 1>;
+  using two = integral_constant<int, 2>;
+  if (two_words && h->tri) launch_radial(std::true_type{}, integral_constant<int, 0>{}, two{});
+  else if (two_words) launch_radial(std::false_type{}, integral_constant<int, 0>{}, two{});
+  else if (h->tri) launch_radial(std::true_type{}, integral_constant<int, 0>{}, one{});
+  else if (std::is_same<MS, MS0>::value && stage_mode() == 1) launch_radial(std::false_type{}, integral_constant<int, std::is_same<MS, MS0>::value ? 1 : 0>{}, one{});
+  else if (std::is_same<MS, MS0>::value && stage_mode() == 2) launch_radial(std::false_type{}, integral_constant<int, std::is_same<MS, MS0>::value ? 2 : 0>{}, one{});
+  else launch_radial(std::false_type{}, integral_constant<int, 0>{}, one{});
   prof_mark(h, PK_ANGULAR_NN);
-  if constexpr (kSplit<MS>)
-    k_angular_nn_split<MS><<<std::min(blocks((long long)n * SPLIT_LANES, SPLIT_THREADS), h->ang_grid), SPLIT_THREADS, h->smem_nn, st>>>(
-        n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
-        h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
-        want_q ? h->at<float>(c.q_desc) : nullptr, da);
-  else {
-    auto launch_nn = [&](auto mode) {
-      constexpr int NN = decltype(mode)::value;
-      constexpr int TH = NN == 2 ? 128 : ANG_THREADS;
-      k_angular_nn<MS, NN><<<std::min(blocks(n, TH), h->ang_grid), TH, h->smem_nn, st>>>(
+  if constexpr (kSplit<MS>) {
+    auto launch_split = [&](auto aw) {
+      k_angular_nn_split<MS, decltype(aw)::value><<<std::min(blocks((long long)n * SPLIT_LANES, SPLIT_THREADS), h->ang_grid), SPLIT_THREADS, h->smem_nn, st>>>(
           n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
           h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
           want_q ? h->at<float>(c.q_desc) : nullptr, da);
     };
-    if (h->nn_mode == 3)
+    if (two_words) launch_split(two{}); else launch_split(one{});
+  } else {
+    auto launch_nn = [&](auto mode, auto aw) {
+      constexpr int NN = decltype(mode)::value;
+      constexpr int TH = NN == 2 ? 128 : ANG_THREADS;
+      k_angular_nn<MS, NN, decltype(aw)::value><<<std::min(blocks(n, TH), h->ang_grid), TH, h->smem_nn, st>>>(
+          n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
+          h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
+          want_q ? h->at<float>(c.q_desc) : nullptr, da);
+    };
+    if (two_words) launch_nn(std::integral_constant<int, 0>{}, two{});  // nn_mode is 0 (nep_zbl_create)
+    else if (h->nn_mode == 3)
       k_angular_tc<MS><<<std::min(blocks(n, TCP_THREADS), h->ang_grid), TCP_THREADS, h->smem_nn, st>>>(
           n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
           h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
           want_q ? h->at<float>(c.q_desc) : nullptr, da);
-    else if (h->nn_mode == 2) launch_nn(std::integral_constant<int, 2>{});
-    else if (h->nn_mode == 1) launch_nn(std::integral_constant<int, 1>{});
-    else launch_nn(std::integral_constant<int, 0>{});
+    else if (h->nn_mode == 2) launch_nn(std::integral_constant<int, 2>{}, one{});
+    else if (h->nn_mode == 1) launch_nn(std::integral_constant<int, 1>{}, one{});
+    else launch_nn(std::integral_constant<int, 0>{}, one{});
   }
   if (h->dense_on) {
     prof_mark(h, PK_SITE64);
@@ -589,10 +603,10 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
     h->launches++;
   }
   prof_mark(h, PK_FORCE);
-  auto launch_force_t = [&](auto vir, auto blk, auto tri) {
+  auto launch_force_t = [&](auto vir, auto blk, auto tri, auto aw) {
     constexpr bool VIR = decltype(vir)::value;
     constexpr int BLK = decltype(blk)::value;
-    k_force<MS, VIR, BLK, decltype(tri)::value><<<blocks((long long)n * FORCE_LANES, BLK), BLK, 0, st>>>(
+    k_force<MS, VIR, BLK, decltype(tri)::value, decltype(aw)::value><<<blocks((long long)n * FORCE_LANES, BLK), BLK, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.nn_a),
         h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk), h->at<unsigned>(c.rmask),
         mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site),
@@ -600,8 +614,10 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
   };
   // triclinic boxes take the 64-thread variant only (a NEXT row: fewer instantiations)
   auto launch_force = [&](auto vir, auto blk) {
-    if (h->tri) launch_force_t(vir, std::integral_constant<int, 64>{}, std::true_type{});
-    else launch_force_t(vir, blk, std::false_type{});
+    if (two_words && h->tri) launch_force_t(vir, std::integral_constant<int, 64>{}, std::true_type{}, two{});
+    else if (two_words) launch_force_t(vir, std::integral_constant<int, 64>{}, std::false_type{}, two{});
+    else if (h->tri) launch_force_t(vir, std::integral_constant<int, 64>{}, std::true_type{}, one{});
+    else launch_force_t(vir, blk, std::false_type{}, one{});
   };
   if (virial) {
     if (gb == 32) launch_force(std::true_type{}, integral_constant<int, 32>{});
@@ -808,8 +824,8 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d 5body %d with %d atom type(s) is not instantiated in this build",
                 p->n_max_radial, p->n_max_angular, p->basis_radial, p->basis_angular, p->has_4body, p->has_5body, p->n_types);
   if (p->n_neurons < 1 || p->n_neurons > 256) return fail(h, NEPZBL_E_INVALID_ARG, "n_neurons out of range");
-  if (p->cap_angular < 1 || p->cap_angular > 64 || p->cap_radial < 1 || p->cap_radial > 1024)
-    return fail(h, NEPZBL_E_INVALID_ARG, "cap_angular must be in 1..64, cap_radial in 1..1024");
+  if (p->cap_angular < 1 || p->cap_angular > 128 || p->cap_radial < 1 || p->cap_radial > 1024)
+    return fail(h, NEPZBL_E_INVALID_ARG, "cap_angular must be in 1..128, cap_radial in 1..1024");
   if (!(p->rc_radial > 0) || !(p->rc_angular > 0) || p->rc_angular > p->rc_radial || p->skin < 0)
     return fail(h, NEPZBL_E_INVALID_ARG, "need 0 < rc_angular <= rc_radial and skin >= 0");
   if (p->zbl_enabled && (p->zbl_n_terms < 1 || p->zbl_n_terms > 4 || !(p->zbl_r_inner < p->zbl_r_outer) ||
@@ -836,7 +852,8 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     int v = atoi(gb);
     if (v == 32 || v == 64) h->gather_block = v;
   }
-  if (const char* nm = getenv("NEPZBL_NN")) h->nn_mode = !strcmp(nm, "tc") ? 3 : (!strcmp(nm, "tcsync") ? 2 : (!strcmp(nm, "mma") ? 1 : 0));
+  if (amask_words(*p) > 1) h->nn_mode = 0;  // two mask words per atom: only the FFMA angular kernel is instantiated for them
+  else if (const char* nm = getenv("NEPZBL_NN")) h->nn_mode = !strcmp(nm, "tc") ? 3 : (!strcmp(nm, "tcsync") ? 2 : (!strcmp(nm, "mma") ? 1 : 0));
   std::vector<float> nnw;
   with_shape(shape, [&](auto ms) {
     using MS = decltype(ms);
@@ -880,7 +897,11 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     int threads = ANG_THREADS;
     with_shape(shape, [&](auto ms) {
       using MS = decltype(ms);
-      if constexpr (kSplit<MS>) { fn = (const void*)k_angular_nn_split<MS>; threads = SPLIT_THREADS; }
+      if constexpr (kSplit<MS>) {
+        fn = amask_words(*p) > 1 ? (const void*)k_angular_nn_split<MS, 2> : (const void*)k_angular_nn_split<MS, 1>;
+        threads = SPLIT_THREADS;
+      }
+      else if (amask_words(*p) > 1) fn = (const void*)k_angular_nn<MS, 0, 2>;
       else if (h->nn_mode == 3) { fn = (const void*)k_angular_tc<MS>; threads = TCP_THREADS; }
       else if (h->nn_mode == 2) { fn = (const void*)k_angular_nn<MS, 2>; threads = 128; }
       else fn = h->nn_mode == 1 ? (const void*)k_angular_nn<MS, 1> : (const void*)k_angular_nn<MS, 0>;

@@ -98,13 +98,13 @@ __device__ __forceinline__ void disp_f64(const BoxMap* bm, const double* __restr
 __global__ void __launch_bounds__(32 * SITE64_WARPS)
 k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm, const int* __restrict__ dense_list,
             int n, int npad, const int4* __restrict__ xyzt, const int* __restrict__ nl_r,
-            const unsigned long long* __restrict__ amask, const int* __restrict__ perm,
+            const unsigned long long* __restrict__ amask, int aw, const int* __restrict__ perm,
             const double* __restrict__ pos, const float* __restrict__ q_radial, float* __restrict__ u_site,
             AtomRec* __restrict__ rec, float4* __restrict__ pforce, float* __restrict__ q_out) {
   extern __shared__ double sm64[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   const int NR = sm.NR, NA = sm.NA, KA = sm.KA, KR = sm.KR, D = sm.D, NT = sm.NT;
-  const int per_warp = 2 * D + sm.n_neurons + 8;              // doubles per warp (+8: 64 one-byte slot numbers)
+  const int per_warp = 2 * D + sm.n_neurons + 16;             // doubles per warp (+16: 128 one-byte slot numbers)
   double* xs = sm64 + (size_t)wib * per_warp;                 // network inputs x_nu
   double* Fp = xs + D;                                        // dU/dq_nu
   double* tt = Fp + D;                                        // w1 (1 - h^2) per neuron
@@ -121,10 +121,12 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
     const int4 me = xyzt[s];
     const int ti = me.w;
     const unsigned long long mask = amask[s];
-    const int nc = __popcll(mask);
+    const unsigned long long mask_hi = aw > 1 ? amask[(size_t)npad + s] : 0ull;  // entries 64.. (cap_angular > 64)
+    const int nc = __popcll(mask) + __popcll(mask_hi);
     if (lane == 0) {
       int c = 0;
       for (unsigned long long m = mask; m; m &= m - 1) slot[c++] = (unsigned char)(__ffsll((long long)m) - 1);
+      for (unsigned long long m = mask_hi; m; m &= m - 1) slot[c++] = (unsigned char)(64 + __ffsll((long long)m) - 1);
     }
     __syncwarp();
     const int rounds = (nc + NS - 1) / NS;

@@ -156,3 +156,23 @@ def test_md_through_a_collision_graph_and_stream_agree(nb, monkeypatch):
     # every atom is kicked exactly once per half step, also the ZBL atoms whose second half-kick is k_zbl's: a missed
     # or doubled half-kick of one of them (dt/2 F/m ~ 1e-5 A/fs here) would show up in the velocities
     assert np.abs(res[0][1] - ovel).max() < 2e-6
+
+
+def test_more_than_64_angular_neighbours(nb):
+    """cap_angular up to 128 (two mask words per atom): a cluster dense enough that some atoms have more than 64
+    neighbours inside rc_angular + skin = 5 A -- more than any of the paper-shaped cascades here produced (50), but
+    what a 100-200 keV core may reach ("cap_angular is capped at 64").  Same tolerances, sets bit-exact."""
+    m = wl.synthetic_model(cap_radial=256, cap_angular=128)
+    w = wl.free_cluster(n=180, seed=33, radius=5.6, min_sep=1.45, model=m)
+    g, _ = _check(nb, w, "dense cluster, cap_angular 128")
+    nn, nl = g.neighbor_get(1)
+    assert int(nn.max()) > 100, int(nn.max())          # the second mask word is really in use (113 list entries)
+    bad, dup, _ = parity.compare_neighbor_sets(nn.cpu().numpy(), nl.cpu().numpy(), w.pos, w.box, w.pbc,
+                                               m["rc_angular"] + m["skin"], oracle)
+    assert not bad and not dup, (bad[:5], dup[:5])
+    # the same capacity on a crystal: the two-word kernels (FFMA network) and the one-word ones (tensor-core network)
+    # agree far inside the oracle tolerance
+    wc = wl.config1(seed=2, cells=5, n_pairs=1)
+    e1, f1, v1 = nb.NepZbl(wc.model, wc.n).compute(wc.pos, wc.types, wc.box, wc.pbc)
+    e2, f2, v2 = nb.NepZbl(dict(wc.model, cap_angular=128), wc.n).compute(wc.pos, wc.types, wc.box, wc.pbc)
+    assert np.abs(e1 - e2).max() < 3e-6 and np.abs(f1 - f2).max() < 3e-5
