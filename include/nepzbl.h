@@ -67,8 +67,9 @@ enum {
 typedef struct {
   int32_t n_types;                     /* 1 or 2 in this build */
   double rc_radial, rc_angular;        /* cutoffs r_c^R, r_c^A (6.0, 4.0 A) */
-  int32_t n_max_radial, n_max_angular; /* n = 0..n_max */
-  int32_t basis_radial, basis_angular; /* Chebyshev basis k = 0..basis (D: C-2) */
+  int32_t n_max_radial, n_max_angular; /* n = 0..n_max; <= 15 / 10 (<= 4 / 4 with the 5-body term, or the 4-body term and two types) */
+  int32_t basis_radial, basis_angular; /* Chebyshev basis k = 0..basis (D: C-2); <= 8.  A model smaller than the kernel
+                                          shape it runs on is zero-padded to it at create; other sizes: NEPZBL_E_UNSUPPORTED */
   int32_t l_max;                       /* Legendre order of the 3-body part (4) */
   int32_t has_4body;                   /* 1: (l1,l2,l3) = (2,2,2) term */
   int32_t has_5body;                   /* 1: (l1,l2,l3,l4) = (1,1,1,1) term behind the 4-body block (D: C-27) */

@@ -433,10 +433,11 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
 }
 
 // descriptor export (parity tests): [D][npad] sorted -> [n][D] caller order
-__global__ void k_export_q(int n, int npad, int D, const int* __restrict__ perm,
+__global__ void k_export_q(int n, int npad, int D, const int* __restrict__ qmap, const int* __restrict__ perm,
                            const float* __restrict__ q_sorted, float* __restrict__ out) {
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   int i = perm[s];
-  for (int v = 0; v < D; ++v) out[(size_t)i * D + v] = q_sorted[(size_t)v * npad + s];
+  // qmap: component v of the caller's model is component qmap[v] of the kernel shape (identity unless padded)
+  for (int v = 0; v < D; ++v) out[(size_t)i * D + v] = q_sorted[(size_t)qmap[v] * npad + s];
 }

@@ -44,7 +44,11 @@ struct ShapeId {
 
 struct nepzbl_handle {
   nepzbl_params p{};  // scalar fields only (pointers nulled)
-  int D = 0, shape = -1;
+  int D = 0, shape = -1;      // D: descriptor components of the kernel shape
+  int D_model = 0;            // ... of the caller's model (smaller when the model runs zero-padded on a larger shape)
+  bool padded = false;
+  std::vector<int> qmap;      // model component -> shape component
+  int* d_qmap = nullptr;
   int device = 0;
   cudaStream_t stream = nullptr;
   cudaStream_t own_stream = nullptr;  // created when the caller passes no stream (see nep_zbl_create)
@@ -227,14 +231,20 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
 
 // instantiated model shapes: BASELINE.json configs (with / without the 4-body term) and the paper's own
 // sizes (n_max 15 / 10, l_max 4; basis 8 / 8 is DESIGN.md C-26) -- SURVEY 8(f) NEXT-2
+// Any model that FITS one of them runs on it (nep_zbl_create pads its tables with zeros: a channel whose coefficients are
+// zero has zero descriptor components, and their columns of w0 are zero too), so the sizes really are run-time
+// parameters within n_max <= 15 / 10 and basis <= 8; the table lists exact matches first, then by cost.
 const ShapeId kShapes[] = {{5, 9, 5, 9, 1, 1, 0}, {5, 9, 5, 9, 0, 1, 0}, {16, 9, 11, 9, 0, 1, 0}, {5, 9, 5, 9, 1, 2, 0},
-                           {5, 9, 5, 9, 1, 1, 1}, {16, 9, 11, 9, 0, 2, 0}};
+                           {5, 9, 5, 9, 1, 1, 1}, {16, 9, 11, 9, 0, 2, 0}, {16, 9, 11, 9, 1, 1, 0}};
+// order in which a model that matches none exactly looks for a shape that contains it (cheapest first)
+const int kShapeByCost[] = {1, 0, 4, 3, 2, 6, 5};
 using MS0 = ModelShape<5, 9, 5, 9, true>;
 using MS1 = ModelShape<5, 9, 5, 9, false>;
 using MS2 = ModelShape<16, 9, 11, 9, false>;
 using MS3 = ModelShape<5, 9, 5, 9, true, 2>;         // two atom types
 using MS4 = ModelShape<5, 9, 5, 9, true, 1, true>;   // 4-body + 5-body terms (NEXT-4, C-27)
 using MS5 = ModelShape<16, 9, 11, 9, false, 2>;      // paper-sized model with two atom types (NEXT-4)
+using MS6 = ModelShape<16, 9, 11, 9, true>;          // paper-sized channels with the 4-body term (hosts padded models)
 template <class F>
 void with_shape(int shape, F&& f) {
   switch (shape) {
@@ -243,12 +253,22 @@ void with_shape(int shape, F&& f) {
     case 2: f(MS2{}); break;
     case 3: f(MS3{}); break;
     case 4: f(MS4{}); break;
-    default: f(MS5{}); break;
+    case 5: f(MS5{}); break;
+    default: f(MS6{}); break;
   }
 }
 // models with more than 5 angular channels use the four-lanes-per-atom kernel (descriptor_split.cuh)
 template <class MS>
 constexpr bool kSplit = MS::NA > 5;
+
+// canonical descriptor index (SURVEY 8(c) C order) of a component in a model with nr radial / na angular channels:
+// block 0 radial n; blocks 1..4 the 3-body l; block 5 the 4-body term; block 6 the 5-body term (behind the 4-body one)
+inline int desc_index(int nr, int na, bool b4, int block, int n) {
+  if (block == 0) return n;
+  if (block <= 4) return nr + (block - 1) * na + n;
+  if (block == 5) return nr + 4 * na + n;
+  return nr + 4 * na + (b4 ? na : 0) + n;
+}
 
 template <class MS>
 void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
@@ -814,14 +834,29 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   *out = nullptr;
   if (p->n_types < 1 || p->n_types > 2) return fail(h, NEPZBL_E_UNSUPPORTED, "this build supports n_types 1 or 2 (got %d)", p->n_types);
   if (p->l_max != 4) return fail(h, NEPZBL_E_UNSUPPORTED, "this build supports l_max == 4 (got %d)", p->l_max);
+  if (p->n_max_radial < 0 || p->n_max_angular < 0 || p->basis_radial < 0 || p->basis_angular < 0)
+    return fail(h, NEPZBL_E_INVALID_ARG, "n_max / basis must be >= 0");
+  // the instantiated shape this model runs on: an exact match, else the cheapest one that contains it (see kShapes)
+  const ShapeId want{p->n_max_radial + 1, p->basis_radial + 1, p->n_max_angular + 1, p->basis_angular + 1,
+                     p->has_4body != 0, p->n_types, p->has_5body != 0};
+  auto fits = [&](const ShapeId& c) {
+    return c.nr >= want.nr && c.kr >= want.kr && c.na >= want.na && c.ka >= want.ka && c.b4 >= want.b4 &&
+           c.b5 >= want.b5 && c.nt == want.nt;
+  };
   int shape = -1;
-  for (int k = 0; k < (int)(sizeof kShapes / sizeof kShapes[0]); ++k)
-    if (kShapes[k].nr == p->n_max_radial + 1 && kShapes[k].kr == p->basis_radial + 1 &&
-        kShapes[k].na == p->n_max_angular + 1 && kShapes[k].ka == p->basis_angular + 1 &&
-        kShapes[k].b4 == (p->has_4body != 0) && kShapes[k].nt == p->n_types && kShapes[k].b5 == (p->has_5body != 0))
+  for (int k = 0; k < (int)(sizeof kShapes / sizeof kShapes[0]); ++k) {
+    const ShapeId& c = kShapes[k];
+    if (c.nr == want.nr && c.kr == want.kr && c.na == want.na && c.ka == want.ka && c.b4 == want.b4 && c.b5 == want.b5 &&
+        c.nt == want.nt)
       shape = k;
+  }
+  bool padded = false;
   if (shape < 0)
-    return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d 5body %d with %d atom type(s) is not instantiated in this build",
+    for (int k : kShapeByCost)
+      if (shape < 0 && fits(kShapes[k])) { shape = k; padded = true; }
+  if (shape < 0)
+    return fail(h, NEPZBL_E_UNSUPPORTED, "model shape n_max %d/%d basis %d/%d 4body %d 5body %d with %d atom type(s) fits no kernel of this build "
+                "(n_max <= 15 / 10, basis <= 8; 5-body or 4-body with two types: n_max <= 4 / 4)",
                 p->n_max_radial, p->n_max_angular, p->basis_radial, p->basis_angular, p->has_4body, p->has_5body, p->n_types);
   if (p->n_neurons < 1 || p->n_neurons > 256) return fail(h, NEPZBL_E_INVALID_ARG, "n_neurons out of range");
   if (p->cap_angular < 1 || p->cap_angular > 128 || p->cap_radial < 1 || p->cap_radial > 1024)
@@ -833,6 +868,45 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     return fail(h, NEPZBL_E_INVALID_ARG, "bad ZBL parameters");
   if (!p->c_radial || !p->c_angular || !p->q_scaler || !p->w0 || !p->b0 || !p->w1 || !p->atomic_number || !p->mass)
     return fail(h, NEPZBL_E_INVALID_ARG, "a parameter array is NULL");
+
+  // a model smaller than its kernel shape: zero-padded tables in the shape's sizes (its own descriptor components keep
+  // their values; the padding channels have zero coefficients, hence zero components, and zero columns in w0)
+  const int D_model = want.nr + 4 * want.na + (want.b4 ? want.na : 0) + (want.b5 ? want.na : 0);
+  std::vector<int> qmap(D_model);       // descriptor component of the model -> component of the shape
+  std::vector<double> pad_cr, pad_ca, pad_qs, pad_w0;
+  nepzbl_params pp = *p;
+  {
+    const ShapeId& c = kShapes[shape];
+    int v = 0;
+    for (int n = 0; n < want.nr; ++n) qmap[v++] = desc_index(c.nr, c.na, c.b4, 0, n);
+    for (int l = 1; l <= 4; ++l)
+      for (int n = 0; n < want.na; ++n) qmap[v++] = desc_index(c.nr, c.na, c.b4, l, n);
+    if (want.b4) for (int n = 0; n < want.na; ++n) qmap[v++] = desc_index(c.nr, c.na, c.b4, 5, n);
+    if (want.b5) for (int n = 0; n < want.na; ++n) qmap[v++] = desc_index(c.nr, c.na, c.b4, 6, n);
+    if (padded) {
+      const int npr = c.nt * c.nt, Ds = c.nr + 4 * c.na + (c.b4 ? c.na : 0) + (c.b5 ? c.na : 0);
+      pad_cr.assign((size_t)npr * c.nr * c.kr, 0.0);
+      pad_ca.assign((size_t)npr * c.na * c.ka, 0.0);
+      for (int pr = 0; pr < npr; ++pr) {
+        for (int n = 0; n < want.nr; ++n)
+          for (int k = 0; k < want.kr; ++k)
+            pad_cr[((size_t)pr * c.nr + n) * c.kr + k] = p->c_radial[((size_t)pr * want.nr + n) * want.kr + k];
+        for (int n = 0; n < want.na; ++n)
+          for (int k = 0; k < want.ka; ++k)
+            pad_ca[((size_t)pr * c.na + n) * c.ka + k] = p->c_angular[((size_t)pr * want.na + n) * want.ka + k];
+      }
+      pad_qs.assign(Ds, 0.0);
+      pad_w0.assign((size_t)p->n_neurons * Ds, 0.0);
+      for (int u = 0; u < D_model; ++u) {
+        pad_qs[qmap[u]] = p->q_scaler[u];
+        for (int m = 0; m < p->n_neurons; ++m) pad_w0[(size_t)m * Ds + qmap[u]] = p->w0[(size_t)m * D_model + u];
+      }
+      pp.n_max_radial = c.nr - 1; pp.basis_radial = c.kr - 1; pp.n_max_angular = c.na - 1; pp.basis_angular = c.ka - 1;
+      pp.has_4body = c.b4; pp.has_5body = c.b5;
+      pp.c_radial = pad_cr.data(); pp.c_angular = pad_ca.data(); pp.q_scaler = pad_qs.data(); pp.w0 = pad_w0.data();
+      p = &pp;
+    }
+  }
 
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
@@ -861,6 +935,9 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     nnw = build_nnw<MS>(p);
     h->D = MS::D;
   });
+  h->D_model = D_model;
+  h->padded = padded;
+  h->qmap = qmap;
   std::vector<double> site_tab;
   size_t site_off[6] = {0, 0, 0, 0, 0, 0};
   with_shape(shape, [&](auto ms) { site_tab = build_site_tables<decltype(ms)>(p, &h->site, site_off); });
@@ -927,6 +1004,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   if ((ce = cudaMalloc(&h->d_sc, sizeof(Scalars))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_bm, sizeof(BoxMap))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_nnw, nnw.size() * sizeof(float))) != cudaSuccess) return die("cudaMalloc", ce);
+  if ((ce = cudaMalloc(&h->d_qmap, h->qmap.size() * sizeof(int))) != cudaSuccess) return die("cudaMalloc", ce);
   if ((ce = cudaMalloc(&h->d_site, site_tab.size() * sizeof(double))) != cudaSuccess) return die("cudaMalloc", ce);
   h->site.ctA = h->d_site + site_off[0]; h->site.ctR = h->d_site + site_off[1]; h->site.qs = h->d_site + site_off[2];
   h->site.w0 = h->d_site + site_off[3]; h->site.b0 = h->d_site + site_off[4]; h->site.w1 = h->d_site + site_off[5];
@@ -948,6 +1026,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
   if ((ce = cudaMemsetAsync(h->d_sc, 0, sizeof(Scalars), h->stream)) != cudaSuccess) return die("cudaMemset", ce);
   if ((ce = cudaMemsetAsync(h->d_bm, 0, sizeof(BoxMap), h->stream)) != cudaSuccess) return die("cudaMemset", ce);
   if ((ce = cudaMemcpyAsync(h->d_nnw, nnw.data(), nnw.size() * sizeof(float), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
+  if ((ce = cudaMemcpyAsync(h->d_qmap, h->qmap.data(), h->qmap.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
   if ((ce = cudaMemcpyAsync(h->d_site, site_tab.data(), site_tab.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
   if ((ce = cudaMemcpyAsync(h->d_mass, mass, sizeof mass, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
   if ((ce = cudaMemcpyAsync(h->d_inv_mass, inv_mass, sizeof inv_mass, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess) return die("cudaMemcpy", ce);
@@ -970,7 +1049,7 @@ void nep_zbl_destroy(nepzbl_handle* h) {
   ws_free(h);
   cudaFree(h->ws_ref.out);
   cudaFreeHost(h->ws_ref.h_out);
-  cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_site); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
+  cudaFree(h->d_sc); cudaFree(h->d_bm); cudaFree(h->d_nnw); cudaFree(h->d_qmap); cudaFree(h->d_site); cudaFree(h->d_mass); cudaFree(h->d_inv_mass);
   cudaFree(h->d_trace); cudaFree(h->d_esum); cudaFree(h->d_nhc);
   cudaFreeHost(h->h_nhc);
   cudaFreeHost(h->h_sc); cudaFreeHost(h->h_trace); cudaFreeHost(h->h_esum);
@@ -986,7 +1065,7 @@ void nep_zbl_destroy(nepzbl_handle* h) {
 
 const char* nep_zbl_last_error(const nepzbl_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
 
-int nep_zbl_descriptor_dim(const nepzbl_handle* h) { return h ? h->D : 0; }
+int nep_zbl_descriptor_dim(const nepzbl_handle* h) { return h ? h->D_model : 0; }
 
 size_t nep_zbl_workspace_bytes(const nepzbl_handle* h, int64_t n_atoms) {
   if (!h || n_atoms < 0) return 0;
@@ -1068,7 +1147,7 @@ int nep_zbl_get_descriptors(nepzbl_handle* h, float* q) {
   if (!q) return fail(h, NEPZBL_E_INVALID_ARG, "q is NULL");
   const Carve& c = h->cv;
   if (h->n > 0) {
-    k_export_q<<<blocks(h->n, 128), 128, 0, h->stream>>>((int)h->n, c.npad, h->D, h->at<int>(c.perm),
+    k_export_q<<<blocks(h->n, 128), 128, 0, h->stream>>>((int)h->n, c.npad, h->D_model, h->d_qmap, h->at<int>(c.perm),
                                                         h->at<float>(c.q_desc), q);
     h->launches++;
   }
