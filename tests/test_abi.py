@@ -57,11 +57,11 @@ def test_create_fails_loudly_without_gpu_or_with_bad_params(lib):
         with pytest.raises(binding.NepZblError) as e:
             binding.NepZbl(m, 100)
         assert e.value.code == -6 and "no CPU fallback" in str(e.value)
-    bad = dict(m, n_max_radial=7)
+    bad = dict(m, n_max_radial=16)     # beyond the largest kernel shape (n_max <= 15 / 10, basis <= 8)
     with pytest.raises(binding.NepZblError) as e:
         binding.NepZbl(bad, 100)
     assert e.value.code == -7
-    bad = dict(m, cap_angular=100)
+    bad = dict(m, cap_angular=129)     # two 64-bit mask words per atom at most
     with pytest.raises(binding.NepZblError) as e:
         binding.NepZbl(bad, 100)
     assert e.value.code == -1
