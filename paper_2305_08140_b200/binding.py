@@ -13,7 +13,8 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "csrc", "libnepzbl.so")
+# NEPZBL_LIB=checked: the bounds-checked build of the same sources (build.py, common.cuh NZ_CHECK)
+LIB_PATH = os.path.join(_HERE, "csrc", "libnepzbl_checked.so" if os.environ.get("NEPZBL_LIB") == "checked" else "libnepzbl.so")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_2305_08140_b200.build` "

@@ -11,6 +11,25 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cstdio>
+
+// Checked build (-DNEPZBL_CHECKED, libnepzbl_checked.so): every index that was read from memory and is about to be
+// used as an address is tested against its bound; a violation prints where and traps (the launch fails loudly).
+// compute-sanitizer is closed on the GPU pool this was developed on, so this is the memcheck stand-in: the GPU
+// suite runs its small cases against the checked library (tests/test_gpu_checked.py).  No cost in the normal build.
+#ifdef NEPZBL_CHECKED
+#define NZ_CHECK(cond, what)                                                                                   \
+  do {                                                                                                         \
+    if (!(cond)) {                                                                                             \
+      printf("nepzbl check failed: %s (%s:%d) block %d thread %d\n", what, __FILE__, __LINE__, (int)blockIdx.x, \
+             (int)threadIdx.x);                                                                                \
+      __trap();                                                                                                \
+    }                                                                                                          \
+  } while (0)
+#else
+#define NZ_CHECK(cond, what) do { } while (0)
+#endif
+
 #define NEPZBL_AMU_A2_FS2_TO_EV 103.6426965
 #define NEPZBL_PI_F 3.14159265358979323846f
 

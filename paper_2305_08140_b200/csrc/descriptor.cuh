@@ -385,7 +385,10 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         j[u] = (t + RADIAL_LANES * u < cnt) ? lp[(size_t)u * lstride] : sc_;
       lp += (size_t)RADIAL_UNROLL * lstride;
 #pragma unroll
-      for (int u = 0; u < RADIAL_UNROLL; ++u) o[u] = xyzt[j[u]];
+      for (int u = 0; u < RADIAL_UNROLL; ++u) {
+        NZ_CHECK((unsigned)j[u] < (unsigned)n, "k_radial: list entry outside [0, n)");
+        o[u] = xyzt[j[u]];
+      }
     }
     const bool ang_round = __any_sync(0xffffffffu, t - sub < cnt_a);  // any lane still in its angular prefix?
 #pragma unroll
@@ -398,6 +401,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         const bool pa = e < cnt_a && r2 < mt.rcA2;
         const unsigned g = (__ballot_sync(0xffffffffu, pa) >> gshift) & 0xFu;
         if (pa) {
+          NZ_CHECK(abase + __popc(g & below) < 64 * AW, "k_radial: compacted angular entry beyond the mask");
           if (MS::NT > 1) {
             adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, __int_as_float(o[u].w));
           } else {  // {rhat, r}, see unpack_disp
@@ -468,7 +472,11 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
     }
     q_radial[(size_t)nq * npad + s] = q;
   }
-  if (sub == 0 && ((cb >> (threadIdx.x & 28)) & 0xFu)) zbl_list[atomicAdd(&sc->zbl_count, 1)] = s;
+  if (sub == 0 && ((cb >> (threadIdx.x & 28)) & 0xFu)) {
+    const int slot = atomicAdd(&sc->zbl_count, 1);
+    NZ_CHECK((unsigned)slot < (unsigned)n, "k_radial: zbl_list slot");
+    zbl_list[slot] = s;
+  }
 }
 
 // ------------------------------------------------------- S4 + S6 + angular partial forces of S7

@@ -117,6 +117,7 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
     load(o_cur, j_cur >= 0 ? j_cur : sc_, ti);
     int j_nxt = j_cur >= 0 ? next_j() : -1;
     while (j_cur >= 0) {
+      NZ_CHECK(j_cur < n && j_nxt < n, "k_force: radial list entry outside [0, n)");
       load(o_nxt, j_nxt >= 0 ? j_nxt : sc_, ti);
       int j_nn = j_nxt >= 0 ? next_j() : -1;
       const Rec& o = o_cur;
@@ -225,6 +226,8 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       const size_t e0 = (size_t)a0 * npad + sc_, e1 = (size_t)a1 * npad + sc_;
       int j0 = nl_a[e0], j1 = nl_a[e1];
       int b0 = rev[e0], b1 = rev[e1];
+      NZ_CHECK((unsigned)j0 < (unsigned)n && (unsigned)j1 < (unsigned)n, "k_force: angular list entry outside [0, n)");
+      NZ_CHECK((b0 == 255 || b0 < 64 * AW) && (b1 == 255 || b1 < 64 * AW), "k_force: reverse slot");
       float4 pij0 = pforce[e0], pij1 = pforce[e1];
       // rev == 255: j's list does not hold i -- only after a neighbour-capacity overflow (j's list was dropped and
       // the call reports NEPZBL_E_NEIGHBOR_OVERFLOW); the value must never be used as a row index
@@ -357,6 +360,7 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
   const unsigned gmask = ((1u << ZBL_LANES) - 1u) << ((threadIdx.x & 31) / ZBL_LANES * ZBL_LANES);
   for (int t = (blockIdx.x * blockDim.x + threadIdx.x) / ZBL_LANES; t < total; t += gridDim.x * blockDim.x / ZBL_LANES) {
     int s = zbl_list[t];
+    NZ_CHECK((unsigned)s < (unsigned)n, "k_zbl: flagged atom outside [0, n)");
     int i = perm[s];
     const int4 me = xyzt[s];
     double xi = pos[i], yi = pos[(size_t)n + i], zi = pos[2 * (size_t)n + i];
@@ -364,6 +368,7 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
     int cnt = nn_r[s];
     for (int k = sub; k < cnt; k += ZBL_LANES) {
       int j = nl_r[(size_t)k * npad + s];
+      NZ_CHECK((unsigned)j < (unsigned)n, "k_zbl: list entry outside [0, n)");
       int4 o = xyzt[j];
       float fdx, fdy, fdz;
       fixed_disp_rt(bm, o.x - me.x, o.y - me.y, o.z - me.z, fdx, fdy, fdz);

@@ -134,27 +134,29 @@ k_nhc(const Scalars* sc, NhcState* nh, int nblocks, const double* __restrict__ p
   nh->ke2 = ke2;
   nh->scale = 1.0;
   if (!(nh->nf > 0.0)) return;
-  const double dt = phase == 0 ? step_dt(sc) : sc->dt;
-  const double delta = 0.5 * dt;
+  // One NHC(delta) operator, delta = dt / 2 (equations of motion of the paper's ref. [32], reading C-24), in the
+  // chain's natural units: with the inertias Q_1 = N_f kT tau^2, Q_k = kT tau^2 the driving terms reduce to
+  //   link 0: (sum m v^2 / (N_f kT) - 1) / tau^2,   link 1: N_f rate_0^2 - 1 / tau^2,   link k >= 2: rate_{k-1}^2 - 1 / tau^2,
+  // so no inertia is ever formed.  A link relaxes for delta / 2 under the friction of its outer neighbour (half the
+  // friction, the drive, half the friction); the operator is: relax from the far end inwards, shrink the particle
+  // velocities for delta, advance the thermostat positions, relax outwards again with the shrunk kinetic energy.
+  const double delta = 0.5 * (phase == 0 ? step_dt(sc) : sc->dt);
+  const double half = 0.5 * delta, quarter = 0.25 * delta;
   const int M = nh->M;
-  const double nf = nh->nf, kT = nh->kT, tt = nh->tau * nh->tau;
-  double Q[NEPZBL_NHC_MAX];
-  Q[0] = nf * kT * tt;
-  for (int k = 1; k < M; ++k) Q[k] = kT * tt;
-  double* vxi = nh->vxi;
-  for (int k = M - 1; k >= 0; --k) {
-    double G = k == 0 ? (ke2 - nf * kT) / Q[0] : (Q[k - 1] * vxi[k - 1] * vxi[k - 1] - kT) / Q[k];
-    double e = k == M - 1 ? 1.0 : exp(-vxi[k + 1] * delta * 0.25);
-    vxi[k] = (vxi[k] * e + G * delta * 0.5) * e;
-  }
-  double sv = exp(-vxi[0] * delta);
+  const double dof = nh->nf, kT = nh->kT, inv_tau2 = 1.0 / (nh->tau * nh->tau);
+  double* rate = nh->vxi;  // d xi_k / dt
+  auto relax = [&](int k, double twice_ke) {
+    double drive;
+    if (k == 0) drive = (twice_ke / (dof * kT) - 1.0) * inv_tau2;
+    else drive = (k == 1 ? dof : 1.0) * rate[k - 1] * rate[k - 1] - inv_tau2;
+    const double damp = k + 1 < M ? exp(-quarter * rate[k + 1]) : 1.0;
+    rate[k] = damp * (damp * rate[k] + half * drive);
+  };
+  for (int k = M; k-- > 0;) relax(k, ke2);
+  const double sv = exp(-delta * rate[0]);
   ke2 *= sv * sv;
-  for (int k = 0; k < M; ++k) nh->xi[k] += vxi[k] * delta;
-  for (int k = 0; k < M; ++k) {
-    double G = k == 0 ? (ke2 - nf * kT) / Q[0] : (Q[k - 1] * vxi[k - 1] * vxi[k - 1] - kT) / Q[k];
-    double e = k == M - 1 ? 1.0 : exp(-vxi[k + 1] * delta * 0.25);
-    vxi[k] = (vxi[k] * e + G * delta * 0.5) * e;
-  }
+  for (int k = 0; k < M; ++k) nh->xi[k] += delta * rate[k];
+  for (int k = 0; k < M; ++k) relax(k, ke2);
   nh->scale = sv;
 }
 
@@ -236,6 +238,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
     }
     fix_position(bm, xn[0], xn[1], xn[2], u);
     int s = inv_perm[i];
+    NZ_CHECK((unsigned)s < (unsigned)n, "k_kick_drift: sorted slot outside [0, n)");
     int4 b = xyzt_build[i];
     xyzt[s] = make_int4((int)u[0], (int)u[1], (int)u[2], t);
     float dx, dy, dz;

@@ -223,6 +223,7 @@ __global__ void k_place(const Scalars* sc, int n, const int* __restrict__ cell_o
   if (i >= n) return;
   int c = cell_of[i];
   int t = atomicAdd(&cell_fill[c], 1);
+  NZ_CHECK((unsigned)(cell_start[c] + t) < (unsigned)n, "k_place: slot outside [0, n)");
   order[cell_start[c] + t] = i;
 }
 
@@ -335,7 +336,9 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
         for (int kx = 0; kx < W; ++kx) {
           if (sx[kx] < 0) continue;
           int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
+          NZ_CHECK((unsigned)c < (unsigned)bm->ncells, "k_nbr: stencil cell outside the grid");
           int b = cell_start[c], e = cell_start[c + 1];
+          NZ_CHECK(b >= 0 && b <= e && e <= n, "k_nbr: cell range outside [0, n]");
           for (int j = b; j < e; ++j) {
             if (j == s) continue;
             int4 o = xyzt[j];
@@ -406,7 +409,9 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
         for (int kx = 0; kx < W; ++kx) {
           if (sx[kx] < 0) continue;
           int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
+          NZ_CHECK((unsigned)c < (unsigned)bm->ncells, "k_nbr: stencil cell outside the grid");
           int b = cell_start[c], e = cell_start[c + 1];
+          NZ_CHECK(b >= 0 && b <= e && e <= n, "k_nbr: cell range outside [0, n]");
           for (int j = b; j < e; ++j) {
             if (j == s) continue;
             int4 o = xyzt[j];
@@ -456,6 +461,7 @@ __global__ void k_rev(const Scalars* sc, int n, int npad, const int* __restrict_
   int na = nn_a[s];
   for (int a = 0; a < na; ++a) {
     int j = nl_a[(size_t)a * npad + s];
+    NZ_CHECK((unsigned)j < (unsigned)n, "k_rev: list entry outside [0, n)");
     int nj = nn_a[j], b = 0;
     for (; b < nj; ++b)
       if (nl_a[(size_t)b * npad + j] == s) break;

@@ -117,6 +117,7 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
   const double C4 = -45.0 / (8.0 * sqrt(14.0) * SITE64_PI * sqrt(SITE64_PI));
   for (int t = blockIdx.x * SITE64_WARPS + wib; t < total; t += gridDim.x * SITE64_WARPS) {
     const int s = dense_list[t];
+    NZ_CHECK((unsigned)s < (unsigned)n, "k_site_fp64: listed atom outside [0, n)");
     const int i = perm[s];
     const int4 me = xyzt[s];
     const int ti = me.w;
@@ -139,6 +140,7 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
       const int c = rd * NS + slice;
       if (!own || c >= nc) continue;
       const int j = nl_r[(size_t)slot[c] * npad + s];
+      NZ_CHECK((unsigned)j < (unsigned)n, "k_site_fp64: list entry outside [0, n)");
       double d[3];
       disp_f64(bm, pos, n, i, perm[j], d);
       const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
