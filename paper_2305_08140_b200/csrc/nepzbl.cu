@@ -1572,7 +1572,10 @@ int wigner_seitz_set_reference(nepzbl_handle* h, int64_t n_sites, const double* 
     g.inv_w[a] = (double)nc / ext[a];
     total *= nc;
   }
-  while (total > 2000000000ll) {  // unreachable for n_sites < 2^31 with ~4 sites per cell; keeps ints safe
+  // never more cells than sites: a degenerate extent (all sites in one plane of an open axis, a single site) makes
+  // `edge` tiny, and a grid of millions of empty cells turns the ring-by-ring search of an atom far from every site
+  // into minutes (found by tests/test_gpu_ws.py::test_degenerate_inputs: 88 s for ONE site); also keeps ints safe
+  while (total > std::max<long long>(1, std::min<long long>(ns, 2000000000ll))) {
     int a = g.nc[0] >= g.nc[1] && g.nc[0] >= g.nc[2] ? 0 : (g.nc[1] >= g.nc[2] ? 1 : 2);
     total /= g.nc[a];
     g.nc[a] = (g.nc[a] + 1) / 2;
