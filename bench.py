@@ -488,6 +488,7 @@ def run_b200(args):
         del site, group
     props = torch.cuda.get_device_properties(dev)
     workspace_bytes = g.workspace_bytes
+    main_run_mode = g.nep_zbl_network_mode()
     main_run.close()
 
     # ---- the other configs of BASELINE.json in the same run (device-resident timing only)
@@ -522,8 +523,23 @@ def run_b200(args):
     hbm_peak = hbm_peak_
     traffic, traffic_note = (args.traffic_bytes, "--traffic-bytes") if args.traffic_bytes is not None else \
         ncu_traffic(args.workload, dom, args.cells)
-    roofline = {"kernel": dom, "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
-                "frac": achieved / alu_peak, "traffic": traffic, "traffic_note": traffic_note,
+    # which kernel the slot "k_angular_nn" timed: the network layer runs on the tensor cores in k_angular_tc
+    # (nep_zbl_network_mode 3); its S6 flops are then tensor-pipe work (3 tf32 products per fp32 product), the
+    # rest of the kernel CUDA-core work -- `achieved` counts the algorithmic flops of the whole kernel either way
+    nn_mode = main_run_mode
+    step_flop = PAPER_STEP_FLOP if args.workload == "paper" else STEP_FLOP
+    network = {"mode": nn_mode,
+               "kernel": {0: "k_angular_nn (FFMA)" if args.workload != "paper" else "k_angular_nn_split (FFMA)",
+                          1: "k_angular_nn (mma.sync 3xTF32)", 2: "k_angular_nn (tcgen05, block-synchronous)",
+                          3: "k_angular_tc (tcgen05 3xTF32, accumulators in tensor memory, two-tile pipeline)"}.get(nn_mode),
+               "tensor_core_flop_per_atom": step_flop["S6"] if nn_mode in (1, 2, 3) else 0.0,
+               "cuda_core_flop_per_atom": flop_table["k_angular_nn"] - (step_flop["S6"] if nn_mode in (1, 2, 3) else 0.0)}
+    if "k_angular_nn" in kern_ms:
+        network["cuda_core_tflops"] = network["cuda_core_flop_per_atom"] * n / (kern_ms["k_angular_nn"] * 1e-3) / 1e12
+        network["cuda_core_frac_of_alu_peak"] = network["cuda_core_tflops"] / alu_peak
+    roofline = {"kernel": dom if not (dom == "k_angular_nn" and nn_mode == 3) else "k_angular_tc",
+                "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
+                "frac": achieved / alu_peak, "network": network, "traffic": traffic, "traffic_note": traffic_note,
                 "peak_source": f"derived: {props.multi_processor_count} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max_mhz:.0f} MHz",
                 "ffma_measured_tflops": ffma_measured, "ms_per_launch": kern_ms[dom],
                 "flop_per_atom": flop_table[dom], "units_per_launch": n,

@@ -30,7 +30,7 @@ EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_d
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
            "md_run", "md_step_host", "md_request_rebuild", "md_energies", "md_get_forces", "md_get_counters",
            "md_set_thermostat", "md_get_thermostat", "md_set_thermostat_state", "wigner_seitz_set_reference", "wigner_seitz_count",
-           "nep_zbl_uses_graph", "nep_zbl_last_counts", "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
+           "nep_zbl_uses_graph", "nep_zbl_network_mode", "nep_zbl_last_counts", "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
 PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "k_site_fp64"]
 
 
@@ -111,6 +111,8 @@ _lib.wigner_seitz_count.argtypes = [_vp, _i64, _vp, _vp, _vp, C.POINTER(_i64), C
 _lib.wigner_seitz_count.restype = C.c_int
 _lib.nep_zbl_uses_graph.argtypes = [_vp]
 _lib.nep_zbl_uses_graph.restype = C.c_int
+_lib.nep_zbl_network_mode.argtypes = [_vp]
+_lib.nep_zbl_network_mode.restype = C.c_int
 _lib.nep_zbl_last_counts.argtypes = [_vp, C.POINTER(_i64), C.POINTER(_i64)]
 _lib.nep_zbl_last_counts.restype = C.c_int
 _lib.nep_zbl_launch_count.argtypes = [_vp]
@@ -300,6 +302,9 @@ class NepZbl:
 
     def nep_zbl_uses_graph(self) -> bool:
         return bool(_lib.nep_zbl_uses_graph(self.h))
+
+    def nep_zbl_network_mode(self) -> int:
+        return int(_lib.nep_zbl_network_mode(self.h))
 
     def nep_zbl_last_counts(self):
         a = _i64(); b = _i64()

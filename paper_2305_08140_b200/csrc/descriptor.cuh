@@ -279,9 +279,14 @@ __device__ __forceinline__ void cp_async_wait_all() {
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" :: "l"(p)); }
 
 __device__ __forceinline__ float tanh_fast(float z) {
-  // 1 - 2/(e^{2z}+1): absolute error ~1e-7, enough for the 1e-5 eV energy tolerance
-  float e = __expf(2.0f * z);
-  return 1.0f - __fdividef(2.0f, e + 1.0f);
+  // 1 - 2/(e^{2z}+1): absolute error ~1e-7, enough for the 1e-5 eV energy tolerance.  The two MUFU
+  // operations are issued as they are (ex2.approx.ftz, rcp.approx.ftz): __expf / __fdividef wrap them in range
+  // fix-ups (FSETP + predicated FMULs for denormal results / huge denominators) that this expression does not need --
+  // e underflows to 0 (tanh = -1) or overflows to inf (rcp(inf) = 0, tanh = 1) at the right limits.  5 instructions.
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * 2.8853900817779268f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.0f));
+  return fmaf(-2.0f, r, 1.0f);
 }
 
 // ------------------------------------------------------------------------- S3: radial descriptor

@@ -1665,6 +1665,13 @@ int md_get_counters(nepzbl_handle* h, int64_t* n_steps, int64_t* n_rebuilds, int
   return NEPZBL_OK;
 }
 
+int nep_zbl_network_mode(const nepzbl_handle* h) {
+  if (!h) return -1;
+  bool split = false;
+  with_shape(h->shape, [&](auto ms) { split = kSplit<decltype(ms)>; });
+  return split ? 0 : h->nn_mode;
+}
+
 int nep_zbl_uses_graph(const nepzbl_handle* h) {
   return h && h->md_ready && h->use_graph && h->step_exec ? 1 : 0;
 }

@@ -128,10 +128,10 @@ __host__ __device__ constexpr uint32_t tile_off(int rows, int r, int k) {
 }
 
 // x = hi + lo with hi representable in tf32 (round to nearest, low 13 mantissa bits zero) and lo = x - hi exact
+// (round to nearest, ties away from zero = cvt.rna.tf32.f32, done with integer arithmetic on the bits: ptxas expands
+// the cvt into FSETP + IADD3 + SEL + LOP3 to keep Inf / NaN intact, which finite network inputs do not need)
 __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo) {
-  uint32_t h;
-  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(h) : "f"(x));
-  hi = __uint_as_float(h);
+  hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u);
   lo = x - hi;
 }
 
