@@ -156,6 +156,10 @@ int nep_zbl_get_descriptors(nepzbl_handle *h, float *q);
  * at nep_zbl_create, issues the same kernels as plain stream launches instead (same results).
  * NEPZBL_GATHER_BLOCK=32|64 (also read at create) fixes the threads per block of the two gather kernels, which
  * the library otherwise picks from the grid size (a tuning aid; results do not depend on it).
+ * Other measurement switches read at create: NEPZBL_NN (network path, see nep_zbl_network_mode), NEPZBL_STAGE=1|2
+ * (neighbour tiles of k_radial staged in shared memory by plain / bulk copies: measured slower, profiles/r2_staging.md),
+ * NEPZBL_DENSE_THRESHOLD (fp64 re-evaluation thresholds, see nep_zbl_last_counts), NEPZBL_ANG_BLOCKS_PER_SM (size of the
+ * angular kernel's persistent grid).  None changes what is computed beyond rounding.
  */
 /* An MD session ends with destroy, the next md_init, nep_zbl_set_workspace -- or ANY neighbor_build /
  * nep_zbl_compute / nep_zbl_compute_host on the same handle (they overwrite the lists and the sorted order the session
@@ -254,7 +258,7 @@ int64_t nep_zbl_launch_count(const nepzbl_handle *h);
  * record CUDA events on the launch stream around each kernel group; nep_zbl_profile_read
  * synchronises, sums the elapsed milliseconds and span counts per group into ms[]/counts[]
  * (NEPZBL_PROFILE_SLOTS entries: 0 integrator first half (k_kick_drift incl. the step's book-keeping, and the
- * thermostat's first half-step if set), 1 list rebuild chain, 2 k_radial, 3 k_angular_nn, 4 k_force (incl. the
+ * thermostat's first half-step if set), 1 list rebuild chain, 2 k_radial, 3 the angular kernel (k_angular_tc / k_angular_nn / k_angular_nn_split, see nep_zbl_network_mode), 4 k_force (incl. the
  * second half-kick in its epilogue), 5 k_zbl, 6 the thermostat's second half-step, 7 k_site_fp64) and resets them.
  * nep_zbl_ffma_peak measures the FP32 FMA issue rate of the device (TFLOP/s, 2 flop per FMA) with a
  * register-only microbenchmark, the denominator of the "alu" roofline.
