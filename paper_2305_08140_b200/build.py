@@ -10,7 +10,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libnepzbl.so")
 SOURCES = ["nepzbl.cu"]
-HEADERS = ["common.cuh", "neighbor.cuh", "descriptor.cuh", "force.cuh", "integrate.cuh", "wigner_seitz.cuh", "descriptor_split.cuh", "site_fp64.cuh", "stage.cuh", "tc05.cuh", "descriptor_tc.cuh"]
+HEADERS = ["common.cuh", "neighbor.cuh", "descriptor.cuh", "force.cuh", "integrate.cuh", "wigner_seitz.cuh", "descriptor_split.cuh", "site_fp64.cuh", "stage.cuh", "tc05.cuh", "descriptor_tc.cuh", "descriptor_split_tc.cuh"]
 
 
 # the same sources with -DNEPZBL_CHECKED: bounds checks on every gathered index (common.cuh: NZ_CHECK); selected with

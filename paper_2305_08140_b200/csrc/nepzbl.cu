@@ -18,6 +18,7 @@
 #include "descriptor.cuh"
 #include "descriptor_split.cuh"
 #include "descriptor_tc.cuh"
+#include "descriptor_split_tc.cuh"
 #include "force.cuh"
 #include "site_fp64.cuh"
 #include "integrate.cuh"
@@ -75,6 +76,7 @@ struct nepzbl_handle {
   // (block-synchronous), 3 = k_angular_tc (descriptor_tc.cuh: tcgen05, software-pipelined over two tiles).
   // NEPZBL_NN=ffma|mma|tcsync|tc overrides the default; measured verdict in DESIGN.md / profiles/r2_nn_tensor.md
   int nn_mode = 3;
+  bool split_tc = false;      // four-lane models: k_angular_split_tc instead of k_angular_nn_split (nn_mode 3, <= 104 neurons)
   bool dense_on = true;       // NEPZBL_DENSE_THRESHOLD=off disables the fp64 re-evaluation (measurement aid)
   size_t smem_nn = 0;
   // threads per block of k_radial / k_force: one warp while the grid is only a few waves of resident threads (the
@@ -260,6 +262,9 @@ void with_shape(int shape, F&& f) {
 // models with more than 5 angular channels use the four-lanes-per-atom kernel (descriptor_split.cuh)
 template <class MS>
 constexpr bool kSplit = MS::NA > 5;
+// ... and its tensor-core form (descriptor_split_tc.cuh) when the slices are 16 entries (no 4-/5-body term)
+template <class MS>
+constexpr bool kSplitTc = kSplit<MS> && !MS::B4 && !MS::B5 && SplitLayout<MS>::SLP == 16;
 
 // canonical descriptor index (SURVEY 8(c) C order) of a component in a model with nr radial / na angular channels:
 // block 0 radial n; blocks 1..4 the 3-body l; block 5 the 4-body term; block 6 the 5-body term (behind the 4-body one)
@@ -318,6 +323,11 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   if (kSplit<MS>) {
     using LY = SplitLayout<MS>;
     h->smem_nn = sizeof(float) * ((size_t)LY::table_floats(LY::rows(p->n_neurons)) + LY::stash_floats());
+    h->split_tc = false;
+    if constexpr (kSplitTc<MS>) {
+      h->split_tc = h->nn_mode == 3 && p->n_neurons <= STC_KT;
+      if (h->split_tc) h->smem_nn = StcLayout<MS>::smem_bytes(LY::rows(p->n_neurons));
+    }
   } else {
     const size_t nrow = (size_t)nn_rows(p->n_neurons);
     h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
@@ -369,6 +379,37 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
       for (int nq = 0; nq < MS::NR; ++nq)
         for (int k = 0; k < MS::KR; ++k)
           ctr[((size_t)pr * 4 * LY::RSUB + nq) * MS::KR + k] = (float)folded(p->c_radial + (size_t)pr * MS::NR * MS::KR, MS::KR, nq, k);
+    }
+    // k_angular_split_tc: behind the table (next multiple of 32 floats) the B operands of its two products, tf32 hi + lo,
+    // tiled as tc05.cuh describes: B1 hi/lo [112 neurons][64 = 4 slices x 16], B2 hi/lo [64][104 neurons] (B1 transposed)
+    if constexpr (kSplitTc<MS>) {
+      if (p->n_neurons <= STC_KT) {
+        const size_t off = (w.size() + 31) / 32 * 32;
+        w.resize(off + 2 * (size_t)STC_NP * STC_KX + 2 * (size_t)STC_KX * STC_KT, 0.0f);
+        float* b1h = w.data() + off;
+        float* b1l = b1h + STC_NP * STC_KX;
+        float* b2h = b1l + STC_NP * STC_KX;
+        float* b2l = b2h + STC_KX * STC_KT;
+        auto split = [](float x, float& hi, float& lo) {  // round to nearest tf32 (13 low bits cleared), remainder
+          uint32_t u;
+          memcpy(&u, &x, 4);
+          u = (u + 0x1000u) & 0xFFFFE000u;
+          memcpy(&hi, &u, 4);
+          lo = x - hi;
+        };
+        for (int lane = 0; lane < 4; ++lane)
+          for (int idx = 0; idx < LY::SLP; ++idx) {
+            const int nu = LY::nu(lane, idx);
+            if (nu < 0) continue;
+            const int v = LY::SLP * lane + idx;
+            for (int m = 0; m < p->n_neurons; ++m) {
+              const float x = (float)p->w0[(size_t)m * MS::D + nu];
+              const size_t o1 = tc05::tile_off(STC_NP, m, v) / 4, o2 = tc05::tile_off(STC_KX, v, m) / 4;
+              split(x, b1h[o1], b1l[o1]);
+              split(x, b2h[o2], b2l[o2]);
+            }
+          }
+      }
     }
     return w;
   } else {
@@ -597,7 +638,18 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
           h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
           want_q ? h->at<float>(c.q_desc) : nullptr, da);
     };
-    if (two_words) launch_split(two{}); else launch_split(one{});
+    bool done = false;
+    if constexpr (kSplitTc<MS>) {
+      if (h->split_tc && !two_words) {
+        k_angular_split_tc<MS><<<std::min(blocks(n, 128), h->ang_grid), STC_THREADS, h->smem_nn, st>>>(
+            n, npad, h->at<int4>(c.xyzt), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp), mt, h->d_nnw,
+            h->at<float>(c.q_radial), h->at<float>(c.u_site), h->at<AtomRec>(c.dk), h->at<float4>(c.pforce),
+            want_q ? h->at<float>(c.q_desc) : nullptr, da);
+        done = true;
+      }
+    }
+    if (done) {}
+    else if (two_words) launch_split(two{}); else launch_split(one{});
   } else {
     auto launch_nn = [&](auto mode, auto aw) {
       constexpr int NN = decltype(mode)::value;
@@ -977,6 +1029,9 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
       if constexpr (kSplit<MS>) {
         fn = amask_words(*p) > 1 ? (const void*)k_angular_nn_split<MS, 2> : (const void*)k_angular_nn_split<MS, 1>;
         threads = SPLIT_THREADS;
+        if constexpr (kSplitTc<MS>) {
+          if (h->split_tc) { fn = (const void*)k_angular_split_tc<MS>; threads = STC_THREADS; }
+        }
       }
       else if (amask_words(*p) > 1) fn = (const void*)k_angular_nn<MS, 0, 2>;
       else if (h->nn_mode == 3) { fn = (const void*)k_angular_tc<MS>; threads = TCP_THREADS; }
@@ -985,7 +1040,7 @@ int nep_zbl_create(const nepzbl_params* p, int device, void* cuda_stream, nepzbl
     });
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->smem_nn)) != cudaSuccess) return die("cudaFuncSetAttribute(k_angular_nn)", ce);
     // the tcgen05 variant needs two 105-KB blocks per SM: ask for the largest shared-memory carve-out
-    if (h->nn_mode >= 2 && (ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
+    if ((h->nn_mode >= 2 || h->split_tc) && (ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
       return die("cudaFuncSetAttribute(carveout)", ce);
     int per_sm = 0;
     if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, threads, h->smem_nn)) != cudaSuccess) return die("cudaOccupancyMaxActiveBlocksPerMultiprocessor", ce);
@@ -1669,7 +1724,7 @@ int nep_zbl_network_mode(const nepzbl_handle* h) {
   if (!h) return -1;
   bool split = false;
   with_shape(h->shape, [&](auto ms) { split = kSplit<decltype(ms)>; });
-  return split ? 0 : h->nn_mode;
+  return split ? (h->split_tc ? 3 : 0) : h->nn_mode;
 }
 
 int nep_zbl_uses_graph(const nepzbl_handle* h) {
