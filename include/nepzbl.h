@@ -233,11 +233,12 @@ int wigner_seitz_count(nepzbl_handle *h, int64_t n, const double *pos_soa, int32
 int nep_zbl_uses_graph(const nepzbl_handle *h);
 
 /* Where the network layer (S6: descriptor x W0, tanh, dU/dq) of this handle runs:
- *   0  CUDA cores, FFMA with the weights broadcast from shared memory (k_angular_nn; every model; the only path for
- *      more than 56 neurons, for cap_angular > 64, and inside the four-lane kernel of models with n_max_angular > 4)
+ *   0  CUDA cores, FFMA with the weights broadcast from shared memory (k_angular_nn / k_angular_nn_split; every model;
+ *      the only path for cap_angular > 64 and for neuron counts beyond the limits below)
  *   1  mma.sync 3xTF32 (kept for the measurement: slower than 0 at 8 M atoms)
  *   2  tcgen05.mma 3xTF32, accumulators in tensor memory, block-synchronous (kept for the measurement)
- *   3  k_angular_tc: tcgen05.mma 3xTF32, software-pipelined over two 128-atom tiles -- the default where it applies
+ *   3  tcgen05.mma 3xTF32 -- the default where it applies: k_angular_tc (one thread per atom, <= 56 neurons; software-
+ *      pipelined over two 128-atom tiles) or k_angular_split_tc (four lanes per atom, 16-entry slices, <= 104 neurons)
  * (north_star: "tensor cores only for the per-atom descriptor x W0 layer and only if ncu shows it beats CUDA-core
  * FMA": DESIGN.md section 9, profiles/r2_nn_tensor.md).  NEPZBL_NN=ffma|mma|tcsync|tc overrides the default. */
 int nep_zbl_network_mode(const nepzbl_handle *h);

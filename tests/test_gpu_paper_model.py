@@ -98,3 +98,28 @@ def test_bench_sized_system_sampled(nb):
     r = parity.compare(e, f, v, ref, idx=sel, label="paper model, 128 000 atoms, sample")
     assert max(r.values()) <= 1.0, r
     assert np.abs(f.sum(axis=1)).max() < 0.1
+
+
+def test_both_network_paths(nb, monkeypatch):
+    """The four-lane kernel has two forms: k_angular_split_tc (network on the tensor cores, the default here) and
+    k_angular_nn_split (FFMA network; more than 104 neurons, cap_angular > 64, NEPZBL_NN=ffma).  Both against the oracle."""
+    w = _case(seed=3, cells=5, n_pairs=2)
+    ref = oracle.compute(oracle.Params(w.model), w.pos, w.types, w.box, w.pbc)
+    g = nb.NepZbl(w.model, w.n)
+    assert g.nep_zbl_network_mode() == 3
+    r = parity.compare(*g.compute(w.pos, w.types, w.box, w.pbc), ref, label="paper model, tensor-core network")
+    assert max(r.values()) <= 1.0, r
+    monkeypatch.setenv("NEPZBL_NN", "ffma")
+    g = nb.NepZbl(w.model, w.n)
+    assert g.nep_zbl_network_mode() == 0
+    r = parity.compare(*g.compute(w.pos, w.types, w.box, w.pbc), ref, label="paper model, FFMA network")
+    assert max(r.values()) <= 1.0, r
+    monkeypatch.delenv("NEPZBL_NN")
+    big = wl.paper_model()
+    big = dict(big, n_neurons=120, w0=np.vstack([big["w0"], big["w0"][:20] * 0.5]), b0=np.concatenate([big["b0"], big["b0"][:20]]),
+               w1=np.concatenate([big["w1"], big["w1"][:20] * 0.1]))
+    g = nb.NepZbl(big, w.n)
+    assert g.nep_zbl_network_mode() == 0       # 120 neurons: beyond the tensor-core form, same results path
+    ref = oracle.compute(oracle.Params(big), w.pos, w.types, w.box, w.pbc)
+    r = parity.compare(*g.compute(w.pos, w.types, w.box, w.pbc), ref, label="paper model, 120 neurons")
+    assert max(r.values()) <= 1.0, r
