@@ -190,7 +190,7 @@ k_scale_vmax(Scalars* sc, const NhcState* __restrict__ nh, int n, double* __rest
 }
 
 // first half-kick + drift + wrap + S1 (fixed-point copy into the sorted slot) + displacement since build
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 5)
 k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restrict__ pos,
              double* __restrict__ vel, const float* __restrict__ force,
              const int32_t* __restrict__ types, const double* __restrict__ inv_mass,
