@@ -33,6 +33,21 @@
 #define NEPZBL_AMU_A2_FS2_TO_EV 103.6426965
 #define NEPZBL_PI_F 3.14159265358979323846f
 
+// 1 / sqrt(x) as the bare MUFU operation: rsqrtf() wraps it in a denormal fix-up (FMUL x 2^24, FSETP, FSEL, FMUL
+// after) that squared pair distances of O(1 - 50 A^2) never need; x = 0 (coincident atoms) gives +inf either way
+__device__ __forceinline__ float rsqrt_fast(float x) {
+  float r;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
+// 1 / x likewise (__fdividef adds a range check for huge denominators)
+__device__ __forceinline__ float rcp_fast(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
+
 struct BoxMap {  // device-resident; recomputed by k_boxmap at every list rebuild
   double lo[3];     // origin of the fixed-point grid per axis
   double inv_h[3];  // 2^32 / span

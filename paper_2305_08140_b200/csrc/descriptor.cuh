@@ -253,10 +253,10 @@ template <int NT, bool RINV>
 __device__ __forceinline__ void unpack_disp(const float4& d, float& ux, float& uy, float& uz, float& r, float& rinv) {
   if (NT == 1) {
     ux = d.x; uy = d.y; uz = d.z; r = d.w;
-    rinv = RINV ? __fdividef(1.0f, r) : 0.0f;
+    rinv = RINV ? rcp_fast(r) : 0.0f;
   } else {
     const float r2 = d.x * d.x + d.y * d.y + d.z * d.z;
-    rinv = rsqrtf(r2);
+    rinv = rsqrt_fast(r2);
     r = r2 * rinv;
     ux = d.x * rinv; uy = d.y * rinv; uz = d.z * rinv;
   }
@@ -413,7 +413,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
           if (MS::NT > 1) {
             adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx, dy, dz, __int_as_float(o[u].w));
           } else {  // {rhat, r}, see unpack_disp
-            const float ri = rsqrtf(r2);
+            const float ri = rsqrt_fast(r2);
             adisp[(size_t)(abase + __popc(g & below)) * npad + sc_] = make_float4(dx * ri, dy * ri, dz * ri, r2 * ri);
           }
           if (AW == 1) {
@@ -426,7 +426,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         abase += __popc(g);
       }
       if ((e < cnt) && r2 < mt.rcR2) {
-        float r = r2 * rsqrtf(r2), fc, T[MS::KR];
+        float r = r2 * rsqrt_fast(r2), fc, T[MS::KR];
         cheb_T_fwd<MS::KR>(r, mt.inv_rcR, fc, T);
 #pragma unroll
         for (int t = 0; t < MS::NT; ++t) {

@@ -125,7 +125,7 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       fixed_disp<TRI>(hm, o.ux - me.ux, o.uy - me.uy, o.uz - me.uz, dx, dy, dz);
       float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
       close = close || (r2 < mt.zbl_flag_r2);
-      float rinv = rsqrtf(r2), r = r2 * rinv;
+      float rinv = rsqrt_fast(r2), r = r2 * rinv;
       float fc, dfc, x, dxdr, T[KR], Uc[KR];
       cheb_T<KR>(r, mt.inv_rcR, fc, dfc, x, dxdr, T);
       cheb_U<KR>(x, Uc);
