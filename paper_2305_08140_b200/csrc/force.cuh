@@ -33,12 +33,12 @@ struct KickArgs {
 // BLK = threads per block (32 or 64, chosen by the host from the grid size; a template parameter because the code
 // ptxas generates under __launch_bounds__(32) is 2 % faster than the same source under a bound of 64 or 128)
 template <class MS, bool VIRIAL, int BLK, bool TRI, int AW = 1>
-__global__ void __launch_bounds__(BLK)
+__global__ void __launch_bounds__(BLK, (MS::NT > 1 && MS::FPREC) ? 1024 / BLK : 0)
 k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__ xyzt,
         const int* __restrict__ nn_r, const int* __restrict__ nl_r, const int* __restrict__ nn_a,
         const int* __restrict__ nl_a, const unsigned char* __restrict__ rev,
         const __grid_constant__ ModelTables<MS> mt, const AtomRec* __restrict__ rec,
-        const unsigned* __restrict__ rmask, int mask_words, const unsigned long long* __restrict__ amask, const float4* __restrict__ pforce, const float* __restrict__ u_site,
+        const unsigned* __restrict__ rmask, const unsigned* __restrict__ tmask, int mask_words, const unsigned long long* __restrict__ amask, const float4* __restrict__ pforce, const float* __restrict__ u_site,
         const int* __restrict__ perm, double* __restrict__ energy, float* __restrict__ force,
         float* __restrict__ virial, const KickArgs ka) {
   constexpr int KR = MS::KR;
@@ -76,16 +76,46 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       d[k] = t;
     }
   };
+  // NT > 1 with 32-byte records {position, Fp}: the folded radial coefficients of all ordered type pairs in shared
+  // memory, rows padded to 12 floats (three aligned LDS.128 per row: the table of (neighbour type, my type) is picked per pair)
+  __shared__ __align__(16) float s_ctr[(NT > 1 && MS::FPREC) ? NT * NT * NR * 12 : 4];
+  if (NT > 1 && MS::FPREC) {
+    for (int e = threadIdx.x; e < NT * NT * NR * 12; e += BLK) {
+      const int pr = e / (NR * 12), nq = (e / 12) % NR, k = e % 12;
+      s_ctr[e] = k < KR ? mt.ctR[pr][nq][k] : 0.0f;
+    }
+    __syncthreads();
+  }
+  // d[k] = sum_n fp[n] ct^{pair}_nk from that table
+  auto contract_pair = [&](const float* fp, int pair, float* d) {
+#pragma unroll
+    for (int k = 0; k < KR; ++k) d[k] = 0.0f;
+#pragma unroll
+    for (int nq = 0; nq < NR; ++nq) {
+      float c[12];
+#pragma unroll
+      for (int v4 = 0; v4 < 3; ++v4)
+        *reinterpret_cast<float4*>(c + 4 * v4) = *reinterpret_cast<const float4*>(s_ctr + (pair * NR + nq) * 12 + 4 * v4);
+#pragma unroll
+      for (int k = 0; k < KR; ++k) d[k] = fmaf(fp[nq], c[k], d[k]);
+    }
+  };
   Rec me;
   load(me, sc_, 0);
-  const int ti = me.type;
-  float me_d1[NT > 1 ? 12 : 1];  // my coefficients towards a neighbour of type 1 (me.d: towards type 0)
+  const int ti = (NT > 1 && MS::FPREC) ? xyzt[sc_].w : me.type;
+  float me_d1[NT > 1 ? 12 : 1];  // my coefficients towards a neighbour of type 1 (me.d / me_d0: towards type 0)
+  float me_d0[(NT > 1 && MS::FPREC) ? 12 : 1];
   if (NT > 1) {
     static_assert(NT <= 2, "k_force keeps one coefficient set per partner type in registers");
-    Rec t1;
-    load(t1, sc_, 1);
+    if (MS::FPREC) {  // d_i^(t)[k] = sum_n Fp_i[n] ct^{ti t}_nk for both partner types, once per atom
+      contract_pair(me.d, ti * NT + 0, me_d0);
+      contract_pair(me.d, ti * NT + 1, me_d1);
+    } else {
+      Rec t1;
+      load(t1, sc_, 1);
 #pragma unroll
-    for (int k = 0; k < 12; ++k) me_d1[NT > 1 ? k : 0] = t1.d[k];
+      for (int k = 0; k < 12; ++k) me_d1[NT > 1 ? k : 0] = t1.d[k];
+    }
   }
   float hm[9];  // fixed-point difference -> Cartesian displacement (only the diagonal is live for orthogonal boxes)
 #pragma unroll
@@ -101,26 +131,35 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
     const int* lp = nl_r + (size_t)sub * npad + sc_;
     const size_t lstride = (size_t)FORCE_LANES * npad;
     int word = 0;
+    constexpr bool TM = NT > 1 && MS::FPREC;  // neighbour types from k_radial's type mask (the 32-byte record has none)
     unsigned m = valid ? rmask[(size_t)sub * npad + sc_] : 0u;
+    unsigned tm = (TM && valid) ? tmask[(size_t)sub * npad + sc_] : 0u;
+    int t_pop = 0;  // type of the entry next_j() returned last
     // pop the next entry of this lane: returns its neighbour index or -1
     auto next_j = [&]() -> int {
       while (m == 0u) {
         if (++word >= mask_words) return -1;
         m = valid ? rmask[((size_t)word * FORCE_LANES + sub) * npad + sc_] : 0u;
+        if (TM) tm = valid ? tmask[((size_t)word * FORCE_LANES + sub) * npad + sc_] : 0u;
       }
       int b = __ffs((int)m) - 1;
       m &= m - 1u;
+      if (TM) t_pop = (tm >> b) & 1u;
       return lp[(size_t)(32 * word + b) * lstride];
     };
     int j_cur = next_j();
+    int t_cur = t_pop;
     Rec o_cur, o_nxt;
     load(o_cur, j_cur >= 0 ? j_cur : sc_, ti);
     int j_nxt = j_cur >= 0 ? next_j() : -1;
+    int t_nxt = t_pop;
     while (j_cur >= 0) {
       NZ_CHECK(j_cur < n && j_nxt < n, "k_force: radial list entry outside [0, n)");
       load(o_nxt, j_nxt >= 0 ? j_nxt : sc_, ti);
       int j_nn = j_nxt >= 0 ? next_j() : -1;
+      const int t_nn = t_pop;
       const Rec& o = o_cur;
+      const int tj = TM ? t_cur : o.type;
       float dx, dy, dz;
       fixed_disp<TRI>(hm, o.ux - me.ux, o.uy - me.uy, o.uz - me.uz, dx, dy, dz);
       float r2 = fmaf(dx, dx, fmaf(dy, dy, dz * dz));
@@ -135,13 +174,17 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       if (VIRIAL) {
         float ai = 0.0f, bi = 0.0f, aj = 0.0f, bj = 0.0f;
         float di[KR], dj[KR];
-        if (MS::FPREC) {
+        if (TM) {
+          contract_pair(o.d, tj * NT + ti, dj);
+#pragma unroll
+          for (int k = 0; k < KR; ++k) di[k] = tj == 1 ? me_d1[NT > 1 ? k : 0] : me_d0[TM ? k : 0];
+        } else if (MS::FPREC) {
           contract(me.d, di);
           contract(o.d, dj);
         } else {
 #pragma unroll
           for (int k = 0; k < KR; ++k) {
-            di[k] = (NT > 1 && o.type == 1) ? me_d1[NT > 1 ? k : 0] : me.d[k];
+            di[k] = (NT > 1 && tj == 1) ? me_d1[NT > 1 ? k : 0] : me.d[k];
             dj[k] = o.d[k];
           }
         }
@@ -162,14 +205,18 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
         // forces only need g_i + g_j: contract once with d_i + d_j (two partial sums each for ILP)
         float a0 = 0.0f, a1 = 0.0f, b0 = 0.0f, b1 = 0.0f;
         float dsum[KR];
-        if (MS::FPREC) {
+        if (TM) {
+          contract_pair(o.d, tj * NT + ti, dsum);
+#pragma unroll
+          for (int k = 0; k < KR; ++k) dsum[k] += tj == 1 ? me_d1[NT > 1 ? k : 0] : me_d0[TM ? k : 0];
+        } else if (MS::FPREC) {
           float fs5[5];
 #pragma unroll
           for (int nq = 0; nq < 5; ++nq) fs5[nq] = me.d[nq] + o.d[nq];
           contract(fs5, dsum);
         } else {
 #pragma unroll
-          for (int k = 0; k < KR; ++k) dsum[k] = ((NT > 1 && o.type == 1) ? me_d1[NT > 1 ? k : 0] : me.d[k]) + o.d[k];
+          for (int k = 0; k < KR; ++k) dsum[k] = ((NT > 1 && tj == 1) ? me_d1[NT > 1 ? k : 0] : me.d[k]) + o.d[k];
         }
 #pragma unroll
         for (int k = 0; k < KR; ++k) {
@@ -196,6 +243,8 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       j_cur = j_nxt;
       o_cur = o_nxt;
       j_nxt = j_nn;
+      t_cur = t_nxt;
+      t_nxt = t_nn;
     }
   }
 

@@ -32,7 +32,7 @@ constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
   size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
-      nn_r, nn_a, shellq, nl_r, rev, rmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, dense_list, tiles, nl_loc, md_force, md_energy,
+      nn_r, nn_a, shellq, nl_r, rev, rmask, tmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, dense_list, tiles, nl_loc, md_force, md_energy,
       partial, nhc_partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
 };
@@ -205,6 +205,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.nl_r = take(4 * (size_t)p.cap_radial * npad);
   c.rev = take((size_t)p.cap_angular * npad);
   c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
+  c.tmask = p.n_types > 1 ? take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad) : c.rmask;  // types of the in-cutoff entries
   c.amask = take(8 * (size_t)amask_words(p) * npad);
   c.adisp = take(16 * (size_t)p.cap_angular * npad);
   c.q_radial = take(4 * (size_t)(p.n_max_radial + 1) * npad);
@@ -331,7 +332,7 @@ void build_tables(nepzbl_handle* h, const nepzbl_params* p) {
   } else {
     const size_t nrow = (size_t)nn_rows(p->n_neurons);
     h->smem_nn = sizeof(float) * (nrow * MS::DPAD + 2 * nrow + MS::DPAD);
-    if (MS::NT > 1) h->smem_nn += sizeof(float) * ((2 * MS::NT * MS::NT * MS::NA * MS::KA + 3) / 4 * 4);
+    if (MS::NT > 1) h->smem_nn += sizeof(float) * (2 * MS::NT * MS::NT * MS::NA * CT_ROW);
     if (h->nn_mode >= 2 && p->n_neurons > TC_NP - 8) h->nn_mode = 0;  // the tcgen05 variants hold at most 56 neurons
     if (h->nn_mode == 1) h->smem_nn += sizeof(float) * (32 * ((MS::D + 7) / 8 * 8 + 4) + 32);  // X / Fp tile and site energies
     if (h->nn_mode >= 2) h->smem_nn += tc_smem_bytes<MS>();
@@ -414,7 +415,7 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
     return w;
   } else {
     const int neu2 = nn_rows(p->n_neurons);  // zero padding rows, see nn_rows
-    const size_t ct_floats = MS::NT > 1 ? (2 * MS::NT * MS::NT * MS::NA * MS::KA + 3) / 4 * 4 : 0;
+    const size_t ct_floats = MS::NT > 1 ? 2 * MS::NT * MS::NT * MS::NA * CT_ROW : 0;  // rows padded to CT_ROW floats
     std::vector<float> w((size_t)neu2 * MS::DPAD + 2 * neu2 + MS::DPAD + ct_floats, 0.0f);
     for (int m = 0; m < p->n_neurons; ++m)
       for (int v = 0; v < MS::D; ++v) w[(size_t)m * MS::DPAD + v] = (float)p->w0[(size_t)m * MS::D + v];
@@ -432,8 +433,8 @@ std::vector<float> build_nnw(const nepzbl_params* p) {
         for (int nq = 0; nq < MS::NA; ++nq)
           for (int k = 0; k < MS::KA; ++k) {
             const double v = folded(p->c_angular + (size_t)pr * MS::NA * MS::KA, MS::KA, nq, k);
-            ct[(pr * MS::NA + nq) * MS::KA + k] = (float)v;
-            ct[((MS::NT * MS::NT + pr) * MS::NA + nq) * MS::KA + k] = (float)(k * v);
+            ct[(pr * MS::NA + nq) * CT_ROW + k] = (float)v;
+            ct[((MS::NT * MS::NT + pr) * MS::NA + nq) * CT_ROW + k] = (float)(k * v);
           }
     }
     // k_angular_tc: behind the table (at the next multiple of 32 floats) the B operands of its two tensor-core products,
@@ -616,7 +617,7 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     k_radial<MS, decltype(tri)::value, STAGE, AW><<<blocks((long long)n * RADIAL_LANES, blk), blk, smem, st>>>(
         h->d_sc, h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), mt,
-        h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), mask_words(h->p), h->at<int>(c.zbl_list),
+        h->at<float>(c.q_radial), h->at<unsigned>(c.rmask), h->at<unsigned>(c.tmask), mask_words(h->p), h->at<int>(c.zbl_list),
         h->at<int>(c.nn_a), h->at<unsigned long long>(c.amask), h->at<float4>(c.adisp),
         h->at<unsigned long long>(c.shellq), STAGE ? h->at<TileDesc>(c.tiles) : nullptr,
         STAGE ? h->at<unsigned short>(c.nl_loc) : nullptr);
@@ -681,7 +682,7 @@ void enqueue_eval_t(nepzbl_handle* h, const double* pos, double* energy, float* 
     k_force<MS, VIR, BLK, decltype(tri)::value, decltype(aw)::value><<<blocks((long long)n * FORCE_LANES, BLK), BLK, 0, st>>>(
         h->d_bm, n, npad, h->at<int4>(c.xyzt), h->at<int>(c.nn_r), h->at<int>(c.nl_r), h->at<int>(c.nn_a),
         h->at<int>(c.nl_r), h->at<unsigned char>(c.rev), mt, h->at<AtomRec>(c.dk), h->at<unsigned>(c.rmask),
-        mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site),
+        h->at<unsigned>(c.tmask), mask_words(h->p), h->at<unsigned long long>(c.amask), h->at<float4>(c.pforce), h->at<float>(c.u_site),
         h->at<int>(c.perm), energy, force, VIR ? virial : nullptr, ka);
   };
   // triclinic boxes take the 64-thread variant only (a NEXT row: fewer instantiations)
