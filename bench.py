@@ -77,9 +77,9 @@ WS_BYTES_PER_ATOM = 68.0
 # "source", valid for the kernel sources whose hash is "csrc_sha16" (csrc_sha16() below): when the kernels have
 # changed since the capture, roofline.traffic is null and roofline.traffic_note says so.
 NCU_TRAFFIC = {"csrc_sha16": "c7f2d21764e6fc2c", "source": "profiles/r2_ncu_full.md", "bytes": {
-    "config4": {"k_radial": 4327.3e6, "k_angular_nn": 6523.3e6, "k_force": 7103.2e6, "integrate_a": 1162.6e6},
-    "config2": {"k_radial": 35.4e6, "k_angular_nn": 58.7e6, "k_force": 96.5e6, "integrate_a": 10.8e6},
-    "paper": {"k_radial": 37.7e6, "k_angular_nn": 74.7e6, "k_force": 101.4e6}}}
+    "config4": {"k_radial": 4327.0e6, "k_angular_nn": 6517.3e6, "k_force": 7101.2e6, "integrate_a": 1162.4e6},
+    "config2": {"k_radial": 35.7e6, "k_angular_nn": 58.8e6, "k_force": 97.2e6, "integrate_a": 10.8e6},
+    "paper": {"k_radial": 37.3e6, "k_angular_nn": 75.0e6, "k_force": 101.8e6}}}
 
 
 def csrc_sha16() -> str:
@@ -534,13 +534,15 @@ def run_b200(args):
     network = {"mode": nn_mode,
                "kernel": {0: "k_angular_nn (FFMA)" if args.workload != "paper" else "k_angular_nn_split (FFMA)",
                           1: "k_angular_nn (mma.sync 3xTF32)", 2: "k_angular_nn (tcgen05, block-synchronous)",
-                          3: "k_angular_tc (tcgen05 3xTF32, accumulators in tensor memory, two-tile pipeline)"}.get(nn_mode),
+                          3: "k_angular_tc (tcgen05 3xTF32, accumulators in tensor memory, two-tile pipeline)" if args.workload != "paper"
+                          else "k_angular_split_tc (tcgen05 3xTF32, four lanes per atom in the passes, one row per thread in the network)"}.get(nn_mode),
                "tensor_core_flop_per_atom": step_flop["S6"] if nn_mode in (1, 2, 3) else 0.0,
                "cuda_core_flop_per_atom": flop_table["k_angular_nn"] - (step_flop["S6"] if nn_mode in (1, 2, 3) else 0.0)}
     if "k_angular_nn" in kern_ms:
         network["cuda_core_tflops"] = network["cuda_core_flop_per_atom"] * n / (kern_ms["k_angular_nn"] * 1e-3) / 1e12
         network["cuda_core_frac_of_alu_peak"] = network["cuda_core_tflops"] / alu_peak
-    roofline = {"kernel": dom if not (dom == "k_angular_nn" and nn_mode == 3) else "k_angular_tc",
+    roofline = {"kernel": dom if not (dom == "k_angular_nn" and nn_mode == 3) else
+                ("k_angular_split_tc" if args.workload == "paper" else "k_angular_tc"),
                 "bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s",
                 "frac": achieved / alu_peak, "network": network, "traffic": traffic, "traffic_note": traffic_note,
                 "peak_source": f"derived: {props.multi_processor_count} SM x {FP32_LANES_PER_SM} FP32 lanes x 2 x {sm_max_mhz:.0f} MHz",
