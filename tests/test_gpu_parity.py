@@ -272,3 +272,30 @@ def test_neighbor_sets_with_a_large_capacity(nb):
     ref = oracle.compute(oracle.Params(m), w.pos, w.types, w.box, w.pbc)
     e, f, v = g.compute(w.pos, w.types, w.box, w.pbc)
     _assert_ok(parity.compare(e, f, v, ref, label="cap_radial 256"))
+
+
+@pytest.mark.parametrize("mode,code", [("ffma", 0), ("mma", 1), ("tcsync", 2), ("tc", 3)])
+def test_every_network_path_meets_the_tolerances(nb, monkeypatch, mode, code):
+    """The network layer exists in four forms (include/nepzbl.h: nep_zbl_network_mode; profiles/r2_nn_tensor.md); the
+    default is the pipelined tcgen05 kernel, the others stay selectable for the measurement.  Each against the oracle,
+    energy / force / virial and a short MD run."""
+    monkeypatch.setenv("NEPZBL_NN", mode)
+    w = wl.config1(seed=4, cells=6, n_pairs=3)
+    ref = oracle.compute(oracle.Params(w.model), w.pos, w.types, w.box, w.pbc)
+    g = nb.NepZbl(w.model, w.n)
+    assert g.nep_zbl_network_mode() == code
+    r = parity.compare(*g.compute(w.pos, w.types, w.box, w.pbc), ref, label=f"network path {mode}")
+    assert max(r.values()) <= 1.0, (mode, r)
+    # ragged tile counts: 1 atom, 33 atoms, 129 atoms of a cluster (partly filled 32- / 128-atom tiles)
+    for n_at in (33, 129):
+        c = wl.free_cluster(n=n_at, seed=40 + n_at, radius=3.0 * n_at ** (1.0 / 3.0), min_sep=2.2)
+        refc = oracle.compute(oracle.Params(c.model), c.pos, c.types, c.box, c.pbc, use_cell=False)
+        rc = parity.compare(*nb.NepZbl(c.model, c.n).compute(c.pos, c.types, c.box, c.pbc), refc, label=f"{mode}, {n_at} atoms")
+        assert max(rc.values()) <= 1.0, (mode, n_at, rc)
+
+
+def test_default_network_path_is_the_tensor_core_pipeline(nb, monkeypatch):
+    monkeypatch.delenv("NEPZBL_NN", raising=False)
+    w = wl.config1(seed=4, cells=5, n_pairs=1)
+    assert nb.NepZbl(w.model, w.n).nep_zbl_network_mode() == 3
+    assert nb.NepZbl(dict(w.model, cap_angular=128), w.n).nep_zbl_network_mode() == 0     # two mask words: FFMA kernel
