@@ -168,52 +168,100 @@ __global__ void k_bin(Scalars* sc, const BoxMap* __restrict__ bm, int n,
   atomicAdd(&cell_count[c], 1);
 }
 
-// exclusive scan of cell_count[0..ncells) -> cell_start[0..ncells]; one block of 1024 threads walks the array in
-// tiles of 4096 cells (4 consecutive cells per thread: coalesced), warp-shuffle scan inside a tile and a running
-// carry between tiles.  (The first version gave every thread one contiguous chunk: strided, serial reads, 0.34 ms for
-// the 380 000 cells of 1.024 M atoms.)
-__global__ void __launch_bounds__(1024) k_scan(const Scalars* sc, const BoxMap* bm,
-                                               const int* __restrict__ cell_count,
-                                               int* __restrict__ cell_start) {
+// exclusive scan of cell_count[0..ncells) -> cell_start[0..ncells] in three launches over tiles of SCAN_TILE cells
+// (1024 threads x 4 consecutive cells: coalesced): k_scan_sums (tile totals) -> k_scan_tiles (ONE block scans the
+// totals: ncells / 4096 values) -> k_scan_apply (every tile scans itself from its offset).  The first version was one
+// block walking the whole array: 1.38 ms for the 3 M cells of 8.192 M atoms, one SM's worth of bandwidth.
+constexpr int SCAN_TILE = 4096;
+
+// exclusive scan of the block's tile v[4] per thread (1024 threads); returns the offset of the thread's first cell
+// inside the tile, *total = the tile total (the same value in every thread)
+__device__ __forceinline__ int scan_tile_1024(const int v[4], int* wsum, int* total) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int mine = v[0] + v[1] + v[2] + v[3];
+  int x = mine;  // inclusive scan over the warp
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += t;
+  }
+  if (lane == 31) wsum[w] = x;
+  __syncthreads();
+  if (w == 0) {
+    int y = wsum[lane];
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      int t = __shfl_up_sync(0xffffffffu, y, o);
+      if (lane >= o) y += t;
+    }
+    wsum[lane] = y;
+  }
+  __syncthreads();
+  *total = wsum[31];
+  return (w ? wsum[w - 1] : 0) + x - mine;
+}
+
+__global__ void __launch_bounds__(1024) k_scan_sums(const Scalars* sc, const BoxMap* bm,
+                                                    const int* __restrict__ cell_count, int* __restrict__ tile_sum) {
   if (!sc->do_rebuild) return;
   __shared__ int wsum[32];
   const int ncells = bm->ncells;
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  int run = 0;  // cells before this tile (the same value in every thread)
-  for (int base = 0; base < ncells; base += 4096) {
+  const int c0 = blockIdx.x * SCAN_TILE + 4 * threadIdx.x;
+  if (blockIdx.x * SCAN_TILE >= ncells) return;  // the grid is sized for the cell CAPACITY
+  int v = 0;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) v += c0 + k < ncells ? cell_count[c0 + k] : 0;
+  v = __reduce_add_sync(0xffffffffu, v);
+  if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    v = __reduce_add_sync(0xffffffffu, wsum[threadIdx.x]);
+    if (threadIdx.x == 0) tile_sum[blockIdx.x] = v;
+  }
+}
+
+// one block: exclusive scan of the tile totals (in tiles of 4096 with a running carry; 733 values at 8.192 M atoms)
+__global__ void __launch_bounds__(1024) k_scan_tiles(const Scalars* sc, const BoxMap* bm,
+                                                     const int* __restrict__ tile_sum, int* __restrict__ tile_off) {
+  if (!sc->do_rebuild) return;
+  __shared__ int wsum[32];
+  const int nt = (bm->ncells + SCAN_TILE - 1) / SCAN_TILE;
+  int run = 0;  // totals before this round (the same value in every thread)
+  for (int base = 0; base < nt; base += SCAN_TILE) {
     const int c0 = base + 4 * threadIdx.x;
-    int v[4];
+    int v[4], total;
 #pragma unroll
-    for (int k = 0; k < 4; ++k) v[k] = c0 + k < ncells ? cell_count[c0 + k] : 0;
-    const int mine = v[0] + v[1] + v[2] + v[3];
-    int x = mine;  // inclusive scan over the warp
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      int t = __shfl_up_sync(0xffffffffu, x, o);
-      if (lane >= o) x += t;
-    }
-    if (lane == 31) wsum[w] = x;
-    __syncthreads();
-    if (w == 0) {
-      int y = wsum[lane];
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, y, o);
-        if (lane >= o) y += t;
-      }
-      wsum[lane] = y;
-    }
-    __syncthreads();
-    int off = run + (w ? wsum[w - 1] : 0) + x - mine;
+    for (int k = 0; k < 4; ++k) v[k] = c0 + k < nt ? tile_sum[c0 + k] : 0;
+    int off = run + scan_tile_1024(v, wsum, &total);
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-      if (c0 + k < ncells) cell_start[c0 + k] = off;
+      if (c0 + k < nt) tile_off[c0 + k] = off;
       off += v[k];
     }
-    run += wsum[31];
+    run += total;
     __syncthreads();
   }
-  if (threadIdx.x == 0) cell_start[ncells] = run;
+}
+
+__global__ void __launch_bounds__(1024) k_scan_apply(const Scalars* sc, const BoxMap* bm,
+                                                     const int* __restrict__ cell_count,
+                                                     const int* __restrict__ tile_off, int* __restrict__ cell_start) {
+  if (!sc->do_rebuild) return;
+  __shared__ int wsum[32];
+  const int ncells = bm->ncells;
+  if (blockIdx.x * SCAN_TILE >= ncells) return;
+  const int c0 = blockIdx.x * SCAN_TILE + 4 * threadIdx.x;
+  int v[4], total;
+#pragma unroll
+  for (int k = 0; k < 4; ++k) v[k] = c0 + k < ncells ? cell_count[c0 + k] : 0;
+  const int base = tile_off[blockIdx.x];
+  int off = base + scan_tile_1024(v, wsum, &total);
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    if (c0 + k < ncells) cell_start[c0 + k] = off;
+    off += v[k];
+  }
+  if ((blockIdx.x + 1) * SCAN_TILE >= ncells && threadIdx.x == 0) cell_start[ncells] = base + total;
 }
 
 __global__ void k_place(const Scalars* sc, int n, const int* __restrict__ cell_of,
@@ -296,6 +344,79 @@ __device__ __forceinline__ void axis_stencil(int c, int nc, int pbc, int S, int 
   }
 }
 
+// Runs of consecutive cells along x in walk order: the cells of a run are adjacent in the sorted atom array, so a
+// run is ONE range of candidates (5 cells = ~13 atoms in bcc W instead of 5 ranges of ~2.7: a fifth of the
+// cell_start look-ups and loop set-ups of the walk).  One run in the bulk, two where the stencil wraps around a
+// periodic axis; the walk order (kz, ky, kx, then sorted index) is unchanged.
+struct XRuns {
+  int n, a[3], b[3];  // run r covers the x cells a[r] .. b[r]
+};
+__device__ __forceinline__ XRuns x_runs(const int sx[5], int W) {
+  XRuns R;
+  R.n = 0;
+#pragma unroll
+  for (int r = 0; r < 3; ++r) R.a[r] = R.b[r] = 0;
+  int last = -2;
+#pragma unroll
+  for (int k = 0; k < 5; ++k) {
+    if (k >= W || sx[k] < 0) continue;
+    if (R.n > 0 && sx[k] == last + 1) {
+#pragma unroll
+      for (int r = 0; r < 3; ++r)
+        if (r == R.n - 1) R.b[r] = sx[k];
+    } else if (R.n < 3) {
+#pragma unroll
+      for (int r = 0; r < 3; ++r)
+        if (r == R.n) R.a[r] = R.b[r] = sx[k];
+      ++R.n;
+    }
+    last = sx[k];
+  }
+  return R;
+}
+
+// every candidate of atom s (sorted index) in walk order: f(j, r2).  The box matrix is read ONCE into registers (the
+// first version went through fixed_disp_rt per candidate: four loads from the BoxMap and a branch in a 31-instruction
+// test, ncu source page).
+template <bool TRI, class F>
+__device__ __forceinline__ void walk_candidates_t(const BoxMap* __restrict__ bm, int n, const int4* __restrict__ xyzt,
+                                                  const int* __restrict__ cell_start, int s, const int4 me, int W,
+                                                  const int sy[5], const int sz[5], const XRuns& R, F&& f) {
+  float hm[9];
+#pragma unroll
+  for (int k = 0; k < 9; ++k) hm[k] = (TRI || k % 4 == 0) ? bm->hm[k] : 0.0f;
+  const int ncx = bm->nc[0], ncy = bm->nc[1];
+  for (int kz = 0; kz < W; ++kz) {
+    if (sz[kz] < 0) continue;
+    for (int ky = 0; ky < W; ++ky) {
+      if (sy[ky] < 0) continue;
+      const int row = (sz[kz] * ncy + sy[ky]) * ncx;
+      for (int r = 0; r < R.n; ++r) {
+        const int ca = row + (r == 0 ? R.a[0] : r == 1 ? R.a[1] : R.a[2]);
+        const int cb = row + (r == 0 ? R.b[0] : r == 1 ? R.b[1] : R.b[2]);
+        NZ_CHECK((unsigned)ca < (unsigned)bm->ncells && (unsigned)cb < (unsigned)bm->ncells,
+                 "k_nbr: stencil cell outside the grid");
+        const int b = cell_start[ca], e = cell_start[cb + 1];
+        NZ_CHECK(b >= 0 && b <= e && e <= n, "k_nbr: cell range outside [0, n]");
+        for (int j = b; j < e; ++j) {
+          if (j == s) continue;
+          const int4 o = xyzt[j];
+          float dx, dy, dz;  // int32 wrap-around = minimum image
+          fixed_disp<TRI>(hm, o.x - me.x, o.y - me.y, o.z - me.z, dx, dy, dz);
+          f(j, dx * dx + dy * dy + dz * dz);
+        }
+      }
+    }
+  }
+}
+template <class F>
+__device__ __forceinline__ void walk_candidates(const BoxMap* __restrict__ bm, int n, const int4* __restrict__ xyzt,
+                                                const int* __restrict__ cell_start, int s, const int4 me, int W,
+                                                const int sy[5], const int sz[5], const XRuns& R, F&& f) {
+  if (bm->tri) walk_candidates_t<true>(bm, n, xyzt, cell_start, s, me, W, sy, sz, R, f);
+  else walk_candidates_t<false>(bm, n, xyzt, cell_start, s, me, W, sy, sz, R, f);
+}
+
 // per atom (sorted order): walk the (2S+1)^3 cells, emit ONE list (column-major) in three segments,
 // each in walk order:
 //   [0, nn_a)        pairs inside rc_angular + skin           -- this prefix IS the angular list
@@ -319,117 +440,70 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
   axis_stencil(cell_of_u((unsigned)me.x, bm->ncv[0], bm->nc[0]), bm->nc[0], bm->pbc[0], S, sx);
   axis_stencil(cell_of_u((unsigned)me.y, bm->ncv[1], bm->nc[1]), bm->nc[1], bm->pbc[1], S, sy);
   axis_stencil(cell_of_u((unsigned)me.z, bm->ncv[2], bm->nc[2]), bm->nc[2], bm->pbc[2], S, sz);
+  const XRuns R = x_runs(sx, W);
   int na = 0, nb = 0, nc = 0;   // segment sizes
   unsigned long long shellq_val = ~0ull;  // "not ordered": set below when the shell could be sorted
   // ONE walk when the list fits the per-thread buffer (any cap_r <= NBR_BUF): the accepted candidates are parked,
-  // tagged with their segment, in local memory (L1-resident) and then laid out segment by segment; the first
-  // version walked the cells twice and evaluated the ~340 candidate distances twice (k_nbr 1.54 ms at 1.024 M atoms).
+  // tagged with their segment, in local memory and then laid out segment by segment; the first version walked the
+  // cells twice and evaluated the ~340 candidate distances twice (k_nbr 1.54 ms at 1.024 M atoms).
+  // The skin shell is laid out by SUB-SHELL (a counting sort over eight bins of width skin / 8, walk order inside a
+  // bin), and shellq[s] keeps, byte m - 1, how many of its entries were put below rc + m * skin / 8.  An entry that lay
+  // at r_b cannot be inside rc while the two largest displacements since the build add up to less than r_b - rc
+  // (Scalars::disp_sum), so k_radial walks only the prefix of the shell that the current displacements can reach.
+  // The bin of an entry is floor((r_b - rc) * 8 / skin - 1e-3): never ABOVE its true sub-shell (the 1e-3 covers the
+  // approximate square root many times over), so the prefix of m bins holds every entry inside rc + m * skin / 8.
+  // (The second version kept the distances beside the indices and insertion-sorted the shell: 1.5 KB of local memory
+  // per thread, 160 MB in flight on the whole GPU -- more than the L2 -- and 25 GB of DRAM traffic per build at
+  // 8.192 M atoms, ncu.)
   constexpr int NBR_BUF = 192;
   if (cap_r <= NBR_BUF) {
     int buf[NBR_BUF];
-    float br[NBR_BUF];  // distance at the build (used to order the skin shell)
     int cnt = 0;
-    for (int kz = 0; kz < W; ++kz) {
-      if (sz[kz] < 0) continue;
-      for (int ky = 0; ky < W; ++ky) {
-        if (sy[ky] < 0) continue;
-        for (int kx = 0; kx < W; ++kx) {
-          if (sx[kx] < 0) continue;
-          int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
-          NZ_CHECK((unsigned)c < (unsigned)bm->ncells, "k_nbr: stencil cell outside the grid");
-          int b = cell_start[c], e = cell_start[c + 1];
-          NZ_CHECK(b >= 0 && b <= e && e <= n, "k_nbr: cell range outside [0, n]");
-          for (int j = b; j < e; ++j) {
-            if (j == s) continue;
-            int4 o = xyzt[j];
-            float dx, dy, dz;  // int32 wrap-around = minimum image
-            fixed_disp_rt(bm, o.x - me.x, o.y - me.y, o.z - me.z, dx, dy, dz);
-            float r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 < rcs2_radial) {
-              const int seg = r2 < rcs2_angular ? 0 : (r2 < rc2_radial ? 1 : 2);
-              na += seg == 0; nb += seg == 1; nc += seg == 2;
-              if (cnt < NBR_BUF) {
-                buf[cnt] = j | (seg << 30);  // j < 2^30 (nep_zbl_set_workspace)
-                br[cnt] = r2;
-              }
-              ++cnt;
-            }
-          }
-        }
+    unsigned long long binc = 0ull;  // entries per sub-shell, one byte each (a full list holds < 256 entries)
+    const float inv_w = shell_w > 0.0f ? 1.0f / shell_w : 0.0f;
+    walk_candidates(bm, n, xyzt, cell_start, s, me, W, sy, sz, R, [&](int j, float r2) {
+      if (r2 < rcs2_radial) {
+        const bool in_a = r2 < rcs2_angular, in_r = r2 < rc2_radial;
+        const float fb = fmaf(r2, rsqrt_fast(r2), -rc_radial) * inv_w - 1e-3f;
+        const int bin = min(max(__float2int_rd(fb), 0), 7);
+        const int seg = in_a ? 0 : (in_r ? 1 : 2 + bin);
+        na += in_a;
+        nb += in_r && !in_a;
+        if (!in_r) binc += 1ull << (8 * bin);
+        if (cnt < NBR_BUF) buf[cnt] = j | (seg << 28);  // j < 2^28 (nep_zbl_set_workspace)
+        ++cnt;
       }
-    }
-    if (!(na + nb + nc > cap_r || na > cap_a)) {
-      int oa = 0, ob = na, oc = na + nb;  // next slot of each segment (walk order kept inside a segment)
+    });
+    nc = cnt - na - nb;
+    if (!(cnt > cap_r || na > cap_a)) {
+      // next slot of each segment: registers for the two inner ones, one byte per sub-shell of the skin shell
+      int oa = 0, ob = na;
+      const int oc = na + nb;
+      unsigned long long pre = binc * 0x0101010101010100ull;  // exclusive prefix sums of the eight bytes
+      shellq_val = binc * 0x0101010101010101ull;               // inclusive ones: byte m - 1 = entries below bin m
       for (int t = 0; t < cnt; ++t) {
-        const int v = buf[t], seg = (unsigned)v >> 30;
-        if (seg == 2) continue;
-        const int slot = seg == 0 ? oa++ : ob++;
-        nl_r[(size_t)slot * npad + s] = v & 0x3fffffff;
+        const int v = buf[t], seg = (unsigned)v >> 28;
+        const int sh = 8 * max(seg - 2, 0);
+        const int slot = seg == 0 ? oa : (seg == 1 ? ob : oc + (int)((pre >> sh) & 0xFFull));
+        oa += seg == 0;
+        ob += seg == 1;
+        if (seg >= 2) pre += 1ull << sh;
+        nl_r[(size_t)slot * npad + s] = v & 0x0fffffff;
       }
-      // The skin shell goes in ascending order of its distance at the build (stable: walk order between equals), and
-      // shellq[s] keeps, byte m - 1, how many of its entries lay inside rc + m * skin / 8.  An entry that lay at
-      // r_b cannot be inside rc while the two largest displacements since the build add up to less than r_b - rc
-      // (Scalars::disp_sum), so k_radial walks only the prefix of the shell that the current displacements can reach.
-      int ns = 0;
-      for (int t = 0; t < cnt; ++t)
-        if (((unsigned)buf[t] >> 30) == 2) {  // compact the shell entries to the front of the buffers, then sort them
-          buf[ns] = buf[t] & 0x3fffffff;
-          br[ns] = br[t];
-          ++ns;
-        }
-      for (int a = 1; a < ns; ++a) {
-        const int vj = buf[a];
-        const float vr = br[a];
-        int q = a - 1;
-        while (q >= 0 && br[q] > vr) {
-          buf[q + 1] = buf[q];
-          br[q + 1] = br[q];
-          --q;
-        }
-        buf[q + 1] = vj;
-        br[q + 1] = vr;
-      }
-      unsigned long long packed = 0ull;
-      int m = 1, upto = 0;
-      for (int t = 0; t < ns; ++t) nl_r[(size_t)(oc + t) * npad + s] = buf[t];
-      for (; m <= 8; ++m) {
-        const float lim = rc_radial + m * shell_w;
-        while (upto < ns && br[upto] < lim * lim) ++upto;
-        packed |= (unsigned long long)min(m == 8 ? ns : upto, 255) << (8 * (m - 1));
-      }
-      shellq_val = packed;
     }
   } else {
   int oa = 0, ob = 0, oc = 0;   // next slot of each segment (second walk)
   for (int pass = 0; pass < 2; ++pass) {
-    for (int kz = 0; kz < W; ++kz) {
-      if (sz[kz] < 0) continue;
-      for (int ky = 0; ky < W; ++ky) {
-        if (sy[ky] < 0) continue;
-        for (int kx = 0; kx < W; ++kx) {
-          if (sx[kx] < 0) continue;
-          int c = (sz[kz] * bm->nc[1] + sy[ky]) * bm->nc[0] + sx[kx];
-          NZ_CHECK((unsigned)c < (unsigned)bm->ncells, "k_nbr: stencil cell outside the grid");
-          int b = cell_start[c], e = cell_start[c + 1];
-          NZ_CHECK(b >= 0 && b <= e && e <= n, "k_nbr: cell range outside [0, n]");
-          for (int j = b; j < e; ++j) {
-            if (j == s) continue;
-            int4 o = xyzt[j];
-            float dx, dy, dz;  // int32 wrap-around = minimum image
-            fixed_disp_rt(bm, o.x - me.x, o.y - me.y, o.z - me.z, dx, dy, dz);
-            float r2 = dx * dx + dy * dy + dz * dz;
-            if (r2 < rcs2_radial) {
-              if (pass == 0) {
-                if (r2 < rcs2_angular) ++na; else if (r2 < rc2_radial) ++nb; else ++nc;
-              } else {
-                int slot = r2 < rcs2_angular ? oa++ : (r2 < rc2_radial ? ob++ : oc++);
-                nl_r[(size_t)slot * npad + s] = j;
-              }
-            }
-          }
+    walk_candidates(bm, n, xyzt, cell_start, s, me, W, sy, sz, R, [&](int j, float r2) {
+      if (r2 < rcs2_radial) {
+        if (pass == 0) {
+          if (r2 < rcs2_angular) ++na; else if (r2 < rc2_radial) ++nb; else ++nc;
+        } else {
+          int slot = r2 < rcs2_angular ? oa++ : (r2 < rc2_radial ? ob++ : oc++);
+          nl_r[(size_t)slot * npad + s] = j;
         }
       }
-    }
+    });
     if (pass == 0) {
       if (na + nb + nc > cap_r || na > cap_a) break;  // overflow: reported below, nothing is written
       oa = 0;
@@ -462,9 +536,18 @@ __global__ void k_rev(const Scalars* sc, int n, int npad, const int* __restrict_
   for (int a = 0; a < na; ++a) {
     int j = nl_a[(size_t)a * npad + s];
     NZ_CHECK((unsigned)j < (unsigned)n, "k_rev: list entry outside [0, n)");
-    int nj = nn_a[j], b = 0;
-    for (; b < nj; ++b)
-      if (nl_a[(size_t)b * npad + j] == s) break;
+    // A list is in walk order = ascending sorted index unless j's stencil wraps around a periodic axis: bisect
+    // (5 probes instead of ~13), and fall back to the plain search whenever the bisection does not land on s.
+    const int nj = nn_a[j];
+    int lo = 0, hi = nj;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (nl_a[(size_t)mid * npad + j] < s) lo = mid + 1; else hi = mid;
+    }
+    int b = lo;
+    if (!(b < nj && nl_a[(size_t)b * npad + j] == s))
+      for (b = 0; b < nj; ++b)
+        if (nl_a[(size_t)b * npad + j] == s) break;
     rev[(size_t)a * npad + s] = (unsigned char)(b < nj ? b : 255);
   }
 }

@@ -31,7 +31,7 @@ thread_local std::string g_create_error;
 constexpr int kTraceRing = 1024;
 
 struct Carve {  // byte offsets into the workspace
-  size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start,
+  size_t xyzt, xyzt_build, xyzt_tmp, perm, inv_perm, order, cell_of, cell_count, cell_fill, cell_start, scan_sum, scan_off,
       nn_r, nn_a, shellq, nl_r, rev, rmask, tmask, amask, adisp, q_radial, dk, pforce, u_site, q_desc, zbl_list, dense_list, tiles, nl_loc, md_force, md_energy,
       partial, nhc_partial, st_pos, st_types, st_e, st_f, st_w, total;
   int npad, ncell_cap;
@@ -199,6 +199,8 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.cell_count = take(4 * ((size_t)c.ncell_cap + 1));
   c.cell_fill = take(4 * ((size_t)c.ncell_cap + 1));
   c.cell_start = take(4 * ((size_t)c.ncell_cap + 1));
+  c.scan_sum = take(4 * ((size_t)c.ncell_cap / SCAN_TILE + 2));  // tile totals / offsets of the cell scan
+  c.scan_off = take(4 * ((size_t)c.ncell_cap / SCAN_TILE + 2));
   c.nn_r = take(4 * npad);
   c.nn_a = take(4 * npad);
   c.shellq = take(8 * npad);
@@ -559,7 +561,11 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
                                                            h->at<int>(c.cell_fill), c.ncell_cap);
   k_bin<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, h->d_bm, n, pos, types, h->p.n_types, h->at<int4>(c.xyzt_tmp),
                                        h->at<int>(c.cell_of), h->at<int>(c.cell_count));
-  k_scan<<<1, 1024, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count), h->at<int>(c.cell_start));
+  const int scan_tiles = c.ncell_cap / SCAN_TILE + 1;
+  k_scan_sums<<<scan_tiles, 1024, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count), h->at<int>(c.scan_sum));
+  k_scan_tiles<<<1, 1024, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.scan_sum), h->at<int>(c.scan_off));
+  k_scan_apply<<<scan_tiles, 1024, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_count), h->at<int>(c.scan_off),
+                                            h->at<int>(c.cell_start));
   k_place<<<blocks(n, 256), 256, 0, st>>>(h->d_sc, n, h->at<int>(c.cell_of), h->at<int>(c.cell_start),
                                          h->at<int>(c.cell_fill), h->at<int>(c.order));
   k_sortcell<<<blocks(c.ncell_cap, 128), 128, 0, st>>>(h->d_sc, h->d_bm, h->at<int>(c.cell_start),
@@ -580,7 +586,7 @@ int enqueue_rebuild(nepzbl_handle* h, const double* pos, const int32_t* types, c
                                                          h->at<TileDesc>(c.tiles), h->at<unsigned short>(c.nl_loc));
     nk++;
   }
-  return nk + 9;
+  return nk + 11;
 }
 
 // fp64 re-evaluation of the atoms k_angular_nn listed (site_fp64.cuh); grid-stride over the list
@@ -1130,7 +1136,7 @@ size_t nep_zbl_workspace_bytes(const nepzbl_handle* h, int64_t n_atoms) {
 
 int nep_zbl_set_workspace(nepzbl_handle* h, void* dev_ptr, size_t bytes, int64_t n_atoms) {
   if (!h) return NEPZBL_E_INVALID_ARG;
-  if (!dev_ptr || n_atoms < 0 || n_atoms > (1ll << 30)) return fail(h, NEPZBL_E_INVALID_ARG, "bad workspace arguments (n_atoms <= 2^30)");
+  if (!dev_ptr || n_atoms < 0 || n_atoms > (1ll << 28)) return fail(h, NEPZBL_E_INVALID_ARG, "bad workspace arguments (n_atoms <= 2^28)");
   if (((uintptr_t)dev_ptr & 255) != 0) return fail(h, NEPZBL_E_WORKSPACE, "workspace must be 256-byte aligned");
   Carve c = carve(h->p, h->D, n_atoms);
   if (bytes < c.total) return fail(h, NEPZBL_E_WORKSPACE, "workspace too small: %zu < %zu bytes", bytes, c.total);
