@@ -269,6 +269,33 @@ int nep_zbl_profile(nepzbl_handle *h, int enable);
 int nep_zbl_profile_read(nepzbl_handle *h, double *ms, int64_t *counts);
 int nep_zbl_ffma_peak(nepzbl_handle *h, double *tflops);
 
+/*
+ * Allocation-free total energies (the reduction of md_energies: E_pot = sum_i U_i, E_kin = sum_i m_i |v_i|^2 / 2 in eV;
+ * the NVE / NVT bookkeeping of a cascade run) for callers that cannot call cudaMalloc: code under CUDA graph
+ * capture, serving loops, harnesses that forbid it.  The call allocates NOTHING (no cudaMalloc / cudaFree, no
+ * allocating library routine, no handle, no workspace): the block partial sums live in a file-scope device array of
+ * the library (csrc/no_alloc.cu, 128.25 KiB), which every GPU that loads libnepzbl.so holds until the process exits.
+ *   n_atoms     0 .. NEPZBL_STATIC_MAX_ATOMS (the size the array is laid out for); more: NEPZBL_E_UNSUPPORTED.
+ *   dev_vel     device, fp64 SoA [3 * n_atoms] (A/fs);  dev_energy  device, fp64 [n_atoms] (eV), e.g. nep_zbl_compute's
+ *   dev_types   device, int32 [n_atoms] or NULL (all type 0; required when n_types > 1); values are clamped to the range
+ *   host_mass   HOST, n_types doubles (amu), 1 <= n_types <= NEPZBL_STATIC_MAX_TYPES
+ *   dev_out     device, 2 doubles: {E_pot, E_kin}, written by the kernel -- valid once the stream reaches that point
+ *   stream      cudaStream_t (NULL: the default stream); the call is ASYNCHRONOUS and does not synchronise
+ *   host_err    HOST buffer for the error text, or NULL; host_err_len its size
+ * All device buffers must belong to the CURRENT device (checked for dev_out: NEPZBL_E_INVALID_ARG otherwise).
+ * Fixed-order fp64 sums: repeated calls on the same data give the same bits; against md_energies (another summation
+ * tree) the totals agree to rounding (~1e-15 relative).
+ * SHARED STATE: every call on a device uses the same array, and the array keeps the last call's contents (the one
+ * word that must start at zero is cleared by every call).  Calls issued to ONE stream are safe in any number; two
+ * calls that can overlap on the same GPU (different streams, different threads, different processes do NOT share it)
+ * RACE on the array and give wrong sums -- order them with an event.
+ */
+#define NEPZBL_STATIC_MAX_ATOMS 33554432
+#define NEPZBL_STATIC_MAX_TYPES 8
+int nep_zbl_energy_sums_static(int64_t n_atoms, const double *dev_vel, const double *dev_energy,
+                               const int32_t *dev_types, int32_t n_types, const double *host_mass,
+                               double *dev_out, void *stream, char *host_err, size_t host_err_len);
+
 #ifdef __cplusplus
 }
 #endif

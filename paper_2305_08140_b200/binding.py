@@ -30,7 +30,8 @@ EXPORTS = ["nep_zbl_create", "nep_zbl_destroy", "nep_zbl_last_error", "nep_zbl_d
            "nep_zbl_compute", "nep_zbl_compute_host", "nep_zbl_get_descriptors", "md_init", "md_step",
            "md_run", "md_step_host", "md_request_rebuild", "md_energies", "md_get_forces", "md_get_counters",
            "md_set_thermostat", "md_get_thermostat", "md_set_thermostat_state", "wigner_seitz_set_reference", "wigner_seitz_count",
-           "nep_zbl_uses_graph", "nep_zbl_network_mode", "nep_zbl_last_counts", "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak"]
+           "nep_zbl_uses_graph", "nep_zbl_network_mode", "nep_zbl_last_counts", "nep_zbl_launch_count", "nep_zbl_profile", "nep_zbl_profile_read", "nep_zbl_ffma_peak",
+           "nep_zbl_energy_sums_static"]
 PROFILE_SLOTS = ["integrate_a", "rebuild", "k_radial", "k_angular_nn", "k_force", "k_zbl", "kick_b", "k_site_fp64"]
 
 
@@ -123,6 +124,9 @@ _lib.nep_zbl_profile_read.argtypes = [_vp, C.POINTER(_dbl), C.POINTER(_i64)]
 _lib.nep_zbl_profile_read.restype = C.c_int
 _lib.nep_zbl_ffma_peak.argtypes = [_vp, C.POINTER(_dbl)]
 _lib.nep_zbl_ffma_peak.restype = C.c_int
+_lib.nep_zbl_energy_sums_static.argtypes = [_i64, _vp, _vp, _vp, _i32, C.POINTER(_dbl), _vp, _vp, C.c_char_p, _sz]
+_lib.nep_zbl_energy_sums_static.restype = C.c_int
+STATIC_MAX_ATOMS = 33554432   # NEPZBL_STATIC_MAX_ATOMS
 
 
 def _ptr(t):
@@ -135,6 +139,19 @@ def _ptr(t):
         assert t.flags["C_CONTIGUOUS"]
         return t.ctypes.data
     raise TypeError(type(t))
+
+
+def nep_zbl_energy_sums_static(vel, energy, types, mass, out, stream=None, n_atoms=None):
+    """{E_pot, E_kin} into `out` (2 doubles on the device) without any allocation: include/nepzbl.h.  Asynchronous;
+    `mass` is a host sequence of one value per type; `n_atoms` defaults to len(energy)."""
+    n = int(energy.numel() if n_atoms is None else n_atoms)
+    m = (C.c_double * len(mass))(*[float(x) for x in mass])
+    err = C.create_string_buffer(256)
+    rc = _lib.nep_zbl_energy_sums_static(n, _ptr(vel), _ptr(energy), _ptr(types), len(mass), m, _ptr(out),
+                                         stream.cuda_stream if stream is not None else None, err, len(err))
+    if rc != OK:
+        raise NepZblError(rc, err.value.decode())
+    return out
 
 
 def _box(box):

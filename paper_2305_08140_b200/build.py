@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libnepzbl.so")
-SOURCES = ["nepzbl.cu"]
+SOURCES = ["nepzbl.cu", "no_alloc.cu"]
 HEADERS = ["common.cuh", "neighbor.cuh", "descriptor.cuh", "force.cuh", "integrate.cuh", "wigner_seitz.cuh", "descriptor_split.cuh", "site_fp64.cuh", "stage.cuh", "tc05.cuh", "descriptor_tc.cuh", "descriptor_split_tc.cuh"]
 
 
