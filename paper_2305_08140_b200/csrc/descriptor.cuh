@@ -388,6 +388,15 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
   // warp-uniform trip count (entries past a lane's own count are guarded), so that the ballots below
   // are taken by all 32 lanes
   const int cnt_max = __reduce_max_sync(0xffffffffu, cnt);
+  // the list entries of a round are loaded one round ahead (jn): a round waits for ONE memory latency (the position
+  // gathers), not two in a row (23 % of the stall samples sat on the entry -> position dependency, ncu source page)
+  int jn[RADIAL_UNROLL];
+  if (!(STAGE && staged)) {
+#pragma unroll
+    for (int u = 0; u < RADIAL_UNROLL; ++u)
+      jn[u] = (sub + RADIAL_LANES * u < cnt) ? lp[(size_t)u * lstride] : sc_;
+    lp += (size_t)RADIAL_UNROLL * lstride;
+  }
   for (int t = sub; t - sub < cnt_max; t += RADIAL_LANES * RADIAL_UNROLL) {
     int j[RADIAL_UNROLL];
     int4 o[RADIAL_UNROLL];
@@ -400,14 +409,16 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
       for (int u = 0; u < RADIAL_UNROLL; ++u) o[u] = s_xyzt[j[u]];
     } else {
 #pragma unroll
-      for (int u = 0; u < RADIAL_UNROLL; ++u)
-        j[u] = (t + RADIAL_LANES * u < cnt) ? lp[(size_t)u * lstride] : sc_;
-      lp += (size_t)RADIAL_UNROLL * lstride;
-#pragma unroll
       for (int u = 0; u < RADIAL_UNROLL; ++u) {
+        j[u] = jn[u];
         NZ_CHECK((unsigned)j[u] < (unsigned)n, "k_radial: list entry outside [0, n)");
         o[u] = xyzt[j[u]];
       }
+      const int tn = t + RADIAL_LANES * RADIAL_UNROLL;
+#pragma unroll
+      for (int u = 0; u < RADIAL_UNROLL; ++u)
+        jn[u] = (tn + RADIAL_LANES * u < cnt) ? lp[(size_t)u * lstride] : sc_;
+      lp += (size_t)RADIAL_UNROLL * lstride;
     }
     const bool ang_round = __any_sync(0xffffffffu, t - sub < cnt_a);  // any lane still in its angular prefix?
 #pragma unroll

@@ -145,7 +145,13 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       int b = __ffs((int)m) - 1;
       m &= m - 1u;
       if (TM) t_pop = (tm >> b) & 1u;
-      return lp[(size_t)(32 * word + b) * lstride];
+      const int* a = lp + (size_t)(32 * word + b) * lstride;
+      // Small systems (BLK == 32: the lists live in the L2): the lane's entry after next -- the in-cutoff entries are a
+      // dense prefix, so almost always two rows on -- is prefetched into the L1: k_force 78.6 -> 73.7 us at 128 000
+      // atoms.  At 8.192 M atoms, where the lists stream from DRAM, the same prefetch (L1 or L2) costs 3 %, and
+      // loading the entries two pairs ahead instead of one 2.5 %: not done there.
+      if (BLK == 32) prefetch_l1(a + 2 * lstride);
+      return *a;
     };
     int j_cur = next_j();
     int t_cur = t_pop;
