@@ -104,7 +104,9 @@ const char *nep_zbl_last_error(const nepzbl_handle *h); /* h may be NULL: create
 int nep_zbl_descriptor_dim(const nepzbl_handle *h);
 
 /* Device workspace for up to n_atoms atoms.  The caller allocates it (e.g. a torch uint8 tensor),
- * hands it over with set_workspace and keeps it alive until destroy or the next set_workspace. */
+ * hands it over with set_workspace and keeps it alive until destroy or the next set_workspace.
+ * dev_ptr must be 256-byte aligned; n_atoms <= 2^28 = 268 435 456 per handle (the list build tags 28-bit atom
+ * indices; about 3 KB of workspace per atom, so 180 GB hold ~55 million atoms anyway): NEPZBL_E_INVALID_ARG beyond. */
 size_t nep_zbl_workspace_bytes(const nepzbl_handle *h, int64_t n_atoms);
 int nep_zbl_set_workspace(nepzbl_handle *h, void *dev_ptr, size_t bytes, int64_t n_atoms);
 
