@@ -48,6 +48,14 @@ __device__ __forceinline__ float rcp_fast(float x) {
   return r;
 }
 
+// The neighbour list nl[cap][npad] is stored with four consecutive entries of an atom side by side (an int4 per atom
+// and group of four rows): the four lanes of an atom in k_radial / k_force read rows 4k .. 4k+3, so a warp's load of
+// one entry per lane is ONE contiguous 128-byte line instead of four 32-byte sectors in four lines (the L1 data pipe is
+// the second resource of those kernels, profiles/r2_ncu_full.md), and k_rev's bisection ends inside one sector.
+__device__ __forceinline__ size_t nl_at(int row, int s, int npad) {
+  return (((size_t)(row >> 2) * (size_t)npad + (size_t)s) << 2) + (size_t)(row & 3);
+}
+
 struct BoxMap {  // device-resident; recomputed by k_boxmap at every list rebuild
   double lo[3];     // origin of the fixed-point grid per axis
   double inv_h[3];  // 2^32 / span

@@ -375,7 +375,7 @@ k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
       cnt -= total - reach;
     }
   }
-  const int* lp = nl_r + (size_t)sub * npad + sc_;
+  const int* lp = nl_r + nl_at(sub, sc_, npad);  // rows sub, sub + 4, ...: lstride apart
   const unsigned short* lp16 = STAGE ? nl_loc + (size_t)sub * npad + sc_ : nullptr;
   const size_t lstride = (size_t)RADIAL_LANES * npad;
   unsigned mword = 0u;

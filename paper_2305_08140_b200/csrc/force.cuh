@@ -128,7 +128,7 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
   // ---- radial pairs: only the entries k_radial found inside the cutoff (bit mask per lane), with the
   //      next entry's index and record gathers in flight while the current pair is evaluated
   {
-    const int* lp = nl_r + (size_t)sub * npad + sc_;
+    const int* lp = nl_r + nl_at(sub, sc_, npad);  // rows sub, sub + 4, ...: lstride apart
     const size_t lstride = (size_t)FORCE_LANES * npad;
     int word = 0;
     constexpr bool TM = NT > 1 && MS::FPREC;  // neighbour types from k_radial's type mask (the 32-byte record has none)
@@ -279,7 +279,7 @@ k_force(const BoxMap* __restrict__ bm, int n, int npad, const int4* __restrict__
       const int a1 = ok1 ? abase + __ffsll((long long)m) - 1 : a0;
       drop(); drop(); drop(); drop();
       const size_t e0 = (size_t)a0 * npad + sc_, e1 = (size_t)a1 * npad + sc_;
-      int j0 = nl_a[e0], j1 = nl_a[e1];
+      int j0 = nl_a[nl_at(a0, sc_, npad)], j1 = nl_a[nl_at(a1, sc_, npad)];
       int b0 = rev[e0], b1 = rev[e1];
       NZ_CHECK((unsigned)j0 < (unsigned)n && (unsigned)j1 < (unsigned)n, "k_force: angular list entry outside [0, n)");
       NZ_CHECK((b0 == 255 || b0 < 64 * AW) && (b1 == 255 || b1 < 64 * AW), "k_force: reverse slot");
@@ -422,7 +422,7 @@ k_zbl(const Scalars* sc, const BoxMap* __restrict__ bm, const int* __restrict__ 
     double e = 0.0, f[3] = {0.0, 0.0, 0.0}, w[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     int cnt = nn_r[s];
     for (int k = sub; k < cnt; k += ZBL_LANES) {
-      int j = nl_r[(size_t)k * npad + s];
+      int j = nl_r[nl_at(k, s, npad)];
       NZ_CHECK((unsigned)j < (unsigned)n, "k_zbl: list entry outside [0, n)");
       int4 o = xyzt[j];
       float fdx, fdy, fdz;

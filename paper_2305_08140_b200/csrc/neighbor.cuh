@@ -487,7 +487,7 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
         oa += seg == 0;
         ob += seg == 1;
         if (seg >= 2) pre += 1ull << sh;
-        nl_r[(size_t)slot * npad + s] = v & 0x0fffffff;
+        nl_r[nl_at(slot, s, npad)] = v & 0x0fffffff;
       }
     }
   } else {
@@ -499,7 +499,7 @@ k_nbr(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const int4* _
           if (r2 < rcs2_angular) ++na; else if (r2 < rc2_radial) ++nb; else ++nc;
         } else {
           int slot = r2 < rcs2_angular ? oa++ : (r2 < rc2_radial ? ob++ : oc++);
-          nl_r[(size_t)slot * npad + s] = j;
+          nl_r[nl_at(slot, s, npad)] = j;
         }
       }
     });
@@ -533,7 +533,7 @@ __global__ void k_rev(const Scalars* sc, int n, int npad, const int* __restrict_
   if (s >= n) return;
   int na = nn_a[s];
   for (int a = 0; a < na; ++a) {
-    int j = nl_a[(size_t)a * npad + s];
+    int j = nl_a[nl_at(a, s, npad)];
     NZ_CHECK((unsigned)j < (unsigned)n, "k_rev: list entry outside [0, n)");
     // A list is in walk order = ascending sorted index unless j's stencil wraps around a periodic axis: bisect
     // (5 probes instead of ~13), and fall back to the plain search whenever the bisection does not land on s.
@@ -543,12 +543,12 @@ __global__ void k_rev(const Scalars* sc, int n, int npad, const int* __restrict_
     int lo = 0, hi = nj;
     while (lo < hi) {
       const int mid = (lo + hi) >> 1;
-      if (nl_a[(size_t)mid * npad + j] < s) lo = mid + 1; else hi = mid;
+      if (nl_a[nl_at(mid, j, npad)] < s) lo = mid + 1; else hi = mid;
     }
     int b = lo;
-    if (!(b < nj && nl_a[(size_t)b * npad + j] == s))
+    if (!(b < nj && nl_a[nl_at(b, j, npad)] == s))
       for (b = 0; b < nj; ++b)
-        if (nl_a[(size_t)b * npad + j] == s) break;
+        if (nl_a[nl_at(b, j, npad)] == s) break;
     rev[(size_t)a * npad + s] = (unsigned char)(b < nj ? b : 255);
   }
 }
@@ -603,5 +603,5 @@ __global__ void k_export_list(int n, int npad, int cap, const int* __restrict__ 
   int i = perm[s], c = nn[s];
   out_nn[i] = c;
   for (int k = 0; k < cap; ++k)
-    out_nl[(size_t)i * cap + k] = k < c ? perm[nl[(size_t)k * npad + s]] : -1;
+    out_nl[(size_t)i * cap + k] = k < c ? perm[nl[nl_at(k, s, npad)]] : -1;
 }

@@ -204,7 +204,7 @@ Carve carve(const nepzbl_params& p, int D, long long n_cap) {
   c.nn_r = take(4 * npad);
   c.nn_a = take(4 * npad);
   c.shellq = take(8 * npad);
-  c.nl_r = take(4 * (size_t)p.cap_radial * npad);
+  c.nl_r = take(4 * (size_t)((p.cap_radial + 3) / 4 * 4) * npad);  // whole groups of four rows (nl_at)
   c.rev = take((size_t)p.cap_angular * npad);
   c.rmask = take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad);
   c.tmask = p.n_types > 1 ? take(4 * (size_t)mask_words(p) * RADIAL_LANES * npad) : c.rmask;  // types of the in-cutoff entries

@@ -139,7 +139,7 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
     for (int rd = 0; rd < rounds; ++rd) {
       const int c = rd * NS + slice;
       if (!own || c >= nc) continue;
-      const int j = nl_r[(size_t)slot[c] * npad + s];
+      const int j = nl_r[nl_at(slot[c], s, npad)];
       NZ_CHECK((unsigned)j < (unsigned)n, "k_site_fp64: list entry outside [0, n)");
       double d[3];
       disp_f64(bm, pos, n, i, perm[j], d);
@@ -266,7 +266,7 @@ k_site_fp64(const Scalars* sc, const BoxMap* __restrict__ bm, const SiteModel sm
       int a = 0;
       if (act) {
         a = slot[c];
-        const int j = nl_r[(size_t)a * npad + s];
+        const int j = nl_r[nl_at(a, s, npad)];
         double d[3];
         disp_f64(bm, pos, n, i, perm[j], d);
         const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);

@@ -95,7 +95,7 @@ k_tiles(const Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad, const
   if (s >= n) return;
   const int cnt = nn_r[s], nr = d.nranges;
   for (int e = 0; e < cnt; ++e) {
-    const int j = nl_r[(size_t)e * npad + s];
+    const int j = nl_r[nl_at(e, s, npad)];
     int loc = 0;
     for (int r = 0; r < nr; ++r) {
       const unsigned rel = (unsigned)(j - d.start[r]);
