@@ -327,8 +327,10 @@ __device__ __forceinline__ float tanh_fast(float z) {
 #endif
 // STAGE > 0 (stage.cuh, an experiment): the block is one tile of STAGE_TILE atoms whose neighbour ranges are copied
 // to shared memory first (1: plain copies, 2: bulk copies); list entries then come from nl_loc (16-bit offsets).
+// Two types: capped at 80 registers (ptxas takes 92 otherwise: 57 against 53 us at 128 000 atoms).  One type: no cap --
+// 70 registers / 27 warps per SM beat 64 / 31 (2.04 against 2.13 ms at 8.192 M atoms).
 template <class MS, bool TRI, int STAGE = 0, int AW = 1>
-__global__ void __launch_bounds__(STAGE ? STAGE_TILE * 4 : RADIAL_BLOCK)
+__global__ void __launch_bounds__(STAGE ? STAGE_TILE * 4 : RADIAL_BLOCK, (MS::NT > 1 && !STAGE) ? 768 / RADIAL_BLOCK : 0)
 k_radial(Scalars* sc, const BoxMap* __restrict__ bm, int n, int npad,
          const int4* __restrict__ xyzt, const int* __restrict__ nn_r, const int* __restrict__ nl_r,
          const __grid_constant__ ModelTables<MS> mt, float* __restrict__ q_radial,
