@@ -173,8 +173,59 @@ k_ws_assign(const WsGrid g, int n, const double* __restrict__ pos, const int* __
     return lo > 0.0 ? lo : (hi < 0.0 ? -hi : 0.0);
   };
   scan_cell((c[2] * g.nc[1] + c[1]) * g.nc[0] + c[0]);
-  // R = 1 (27 cells) settles every atom of a crystal; a wider block is walked again whole (rare)
-  for (int R = 1;; ++R) {
+  // R = 1 (27 cells) settles every atom of a crystal; a wider block is walked again whole (rare).
+  // The 26 neighbour cells of R = 1 are almost all REJECTED by the gap test, so that test comes first and alone: the
+  // nine squared axis gaps are formed once, a rejected cell costs two additions and a compare, the periodic wrap and
+  // the cell index are computed for the accepted ones only (the general loop below spent ~40 instructions per
+  // rejected cell: 0.92 ms per count at 8.192 M atoms, ncu).  Same gaps, same sums, same comparisons as below.
+  int R0 = 1;
+  if ((!g.pbc[0] || g.nc[0] >= 4) && (!g.pbc[1] || g.nc[1] >= 4) && (!g.pbc[2] || g.nc[2] >= 4)) {
+    double g2[3][3];
+    bool in[3][3];  // the cell at offset o - 1 exists (open axes end at the grid)
+    bool all_covered = true;
+    double bound = INFINITY;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+#pragma unroll
+      for (int o = 0; o < 3; ++o) {
+        const double gp = axis_gap(a, o - 1);
+        g2[a][o] = gp * gp;
+        in[a][o] = g.pbc[a] || (c[a] + o - 1 >= 0 && c[a] + o - 1 <= g.nc[a] - 1);
+      }
+      const bool covered = !g.pbc[a] && c[a] - 1 <= 0 && c[a] + 1 >= g.nc[a] - 1;
+      if (!covered) bound = fmin(bound, g.w[a]);
+      all_covered = all_covered && covered;
+    }
+    // which of the 26 cells can hold a site that beats or ties the best of the own cell (a later scan can only lower
+    // the best: the set is a superset of what the general loop would scan, the result is the same)
+    const double thr = best * (1.0 + 1e-9) + 1e-9;
+    unsigned accept = 0u;
+#pragma unroll
+    for (int oz = 0; oz < 3; ++oz) {
+#pragma unroll
+      for (int oy = 0; oy < 3; ++oy) {
+        const double gyz = g2[1][oy] + g2[2][oz];
+#pragma unroll
+        for (int ox = 0; ox < 3; ++ox) {
+          if (ox == 1 && oy == 1 && oz == 1) continue;  // own cell: scanned above
+          const double dmin2 = g2[0][ox] + gyz;
+          if (!(dmin2 > thr) && in[0][ox] && in[1][oy] && in[2][oz]) accept |= 1u << ((oz * 3 + oy) * 3 + ox);
+        }
+      }
+    }
+    while (accept) {
+      const int bit = __ffs((int)accept) - 1;
+      accept &= accept - 1u;
+      const int oz = bit / 9, oy = (bit / 3) % 3, ox = bit % 3;
+      int cx = c[0] + ox - 1, cy = c[1] + oy - 1, cz = c[2] + oz - 1;
+      if (g.pbc[0]) cx = cx < 0 ? cx + g.nc[0] : (cx >= g.nc[0] ? cx - g.nc[0] : cx);
+      if (g.pbc[1]) cy = cy < 0 ? cy + g.nc[1] : (cy >= g.nc[1] ? cy - g.nc[1] : cy);
+      if (g.pbc[2]) cz = cz < 0 ? cz + g.nc[2] : (cz >= g.nc[2] ? cz - g.nc[2] : cz);
+      scan_cell((cz * g.nc[1] + cy) * g.nc[0] + cx);
+    }
+    R0 = (best < bound * bound || all_covered) ? 0 : 2;  // 0: settled
+  }
+  for (int R = R0; R > 0; ++R) {
     int lo[3], hi[3], covered[3];
     double bound = INFINITY;
 #pragma unroll
