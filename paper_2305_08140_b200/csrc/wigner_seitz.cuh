@@ -125,7 +125,9 @@ __device__ __forceinline__ void ws_load(const WsSite* p, double& x, double& y, d
 // comes closer to the atom than the best site found so far (with a 1e-9 safety margin for the rounding of
 // the cell geometry), which leaves ~10 candidates per atom of a crystal instead of the ~108 of all 27 cells
 // (the kernel is instruction-bound: ncu, profiles/).
-__global__ void __launch_bounds__(128)
+// latency-bound (three dependent loads, fp64 chains): 12 blocks per SM at 40 registers -- 0.71 ms (72 registers,
+// 7 blocks) -> 0.54 ms per count at 8.192 M atoms; 16 blocks at 32 registers 0.57 ms
+__global__ void __launch_bounds__(128, 12)
 k_ws_assign(const WsGrid g, int n, const double* __restrict__ pos, const int* __restrict__ cell_start,
             const WsSite* __restrict__ rec, int* __restrict__ nearest, int* __restrict__ occ) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
